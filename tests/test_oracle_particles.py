@@ -1,0 +1,409 @@
+"""Pins of the oracle's particle part: Boris push, charge-conserving deposits, sort, whole step.
+
+Everything is checked against closed forms, invariants, the definition-level brute force
+(oracle/brute_force.py) or a library routine -- never against the function's own formula."""
+import numpy as np
+import pytest
+
+from oracle.brute_force import BruteForce
+from oracle.psc_oracle import Oracle
+
+
+def _c(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+# ------------------------------------------------------------------------------------------------
+# Boris (Eq. 26-28)
+
+def _uniform_fields(orc, Evec, Bvec):
+    E, B = orc.zeros_field(), orc.zeros_field()
+    for c in range(3):
+        E[c] = Evec[c]
+        B[c] = Bvec[c]
+    return E, B
+
+
+def test_boris_gyration_radius_and_period():
+    """uniform B, E = 0: |u| conserved; positions x^{n+1/2} lie on a circle of radius
+    (v/w_c) sqrt(1+a^2), a = w_c dt/2, w_c = |q| B/(m gamma); the velocity turns by 2 atan(a) per
+    step (period 2 pi dt / (2 atan a)); both tend to v/w_c and 2 pi/w_c as dt -> 0."""
+    n, dx, dt = (16, 16, 1), (1.0, 1.0, 1.0), 0.35
+    q, m = -1.0, 1.0
+    orc = Oracle(n, dx, dt, 1, [q], [m])
+    Bz = 0.4
+    E, B = _uniform_fields(orc, (0, 0, 0), (0, 0, Bz))
+    J = orc.zeros_field()
+    u0 = np.array([0.3, -0.2, 0.05])
+    x, y, z = _c([8.0]), _c([8.0]), _c([0.5])
+    ux, uy, uz = _c([u0[0]]), _c([u0[1]]), _c([u0[2]])
+    qw, sp = _c([0.0]), np.zeros(1, dtype=np.int32)      # zero weight: fields stay uniform
+    gam = np.sqrt(1 + u0 @ u0)
+    wc = abs(q) * Bz / (m * gam)
+    a = wc * dt / 2
+    vperp = np.hypot(u0[0], u0[1]) / gam
+    pts, vel = [], []
+    px, py = x[0], y[0]
+    for _ in range(400):
+        xo, yo = x[0], y[0]
+        orc.push_particles(E, B, J, x, y, z, ux, uy, uz, qw, sp)
+        ddx = (x[0] - xo + 8) % 16 - 8
+        ddy = (y[0] - yo + 8) % 16 - 8
+        px, py = px + ddx, py + ddy
+        pts.append((px, py))
+        vel.append((ux[0], uy[0]))
+        assert abs(np.sqrt(1 + ux[0] ** 2 + uy[0] ** 2 + uz[0] ** 2) - gam) < 1e-13
+        assert abs(uz[0] - u0[2]) < 1e-15
+    pts, vel = np.array(pts), np.array(vel)
+    # circle through the points: algebraic least-squares fit
+    A = np.c_[2 * pts, np.ones(len(pts))]
+    sol = np.linalg.lstsq(A, (pts ** 2).sum(1), rcond=None)[0]
+    cx, cy = sol[0], sol[1]
+    R = np.sqrt(sol[2] + cx * cx + cy * cy)
+    R_want = vperp / wc * np.sqrt(1 + a * a)
+    assert abs(R - R_want) < 1e-11
+    assert np.abs(np.hypot(pts[:, 0] - cx, pts[:, 1] - cy) - R_want).max() < 1e-11
+    ang = np.unwrap(np.arctan2(vel[:, 1], vel[:, 0]))
+    dang = np.diff(ang)
+    # electron (q<0) in +B_z gyrates counter-clockwise: dphi = +2 atan(a)
+    assert np.abs(dang - 2 * np.arctan(a)).max() < 1e-12
+    # continuum limits within O(a^2)
+    assert abs(R / (vperp / wc) - 1) < a * a
+    assert abs((2 * np.pi * dt / (2 * np.arctan(a))) / (2 * np.pi / wc) - 1) < a * a
+
+
+def test_boris_sense_of_rotation_ion():
+    """dp/dt = q v x B: a positive charge moving along +x in +B_z is pushed towards -y."""
+    orc = Oracle((8, 8, 1), (1, 1, 1), 0.1, 1, [1.0], [1.0])
+    EB = np.zeros((1, 6))
+    EB[0, 5] = 1.0
+    ux, uy, uz = _c([0.1]), _c([0.0]), _c([0.0])
+    orc.boris(ux, uy, uz, np.zeros(1, dtype=np.int32), EB)
+    assert uy[0] < 0 and abs(np.hypot(ux[0], uy[0]) - 0.1) < 1e-15
+
+
+def test_boris_pure_electric_kick():
+    """B = 0: u^{n+1} = u^n + (q dt/m) E exactly."""
+    orc = Oracle((8, 8, 8), (1, 1, 1), 0.2, 1, [-1.0, 2.0], [1.0, 4.0])
+    EB = np.zeros((2, 6))
+    EB[:, :3] = [0.3, -0.5, 0.7]
+    ux, uy, uz = _c([0.1, 0.1]), _c([0.2, 0.2]), _c([-0.3, -0.3])
+    orc.boris(ux, uy, uz, np.array([0, 1], dtype=np.int32), EB)
+    for s, (q, m) in enumerate(((-1.0, 1.0), (2.0, 4.0))):
+        want = np.array([0.1, 0.2, -0.3]) + q * 0.2 / m * np.array([0.3, -0.5, 0.7])
+        assert np.abs(np.array([ux[s], uy[s], uz[s]]) - want).max() < 1e-15
+
+
+def test_exb_drift():
+    """E perp B: mean velocity over whole gyro-periods = E x B / B^2 (up to O(v^2/c^2))."""
+    n, dt = (32, 32, 1), 0.35
+    orc = Oracle(n, (1, 1, 1), dt, 1, [-1.0], [1.0])
+    Ey, Bz = 0.004, 0.4                      # drift 0.01 c along +x
+    E, B = _uniform_fields(orc, (0, Ey, 0), (0, 0, Bz))
+    J = orc.zeros_field()
+    x, y, z = _c([16.0]), _c([16.0]), _c([0.5])
+    ux, uy, uz = _c([0.0]), _c([0.0]), _c([0.0])
+    qw, sp = _c([0.0]), np.zeros(1, dtype=np.int32)
+    a = Bz * dt / 2
+    steps_per_period = 2 * np.pi / (2 * np.arctan(a))
+    nsteps = int(round(200 * steps_per_period))
+    px = py = 0.0
+    for _ in range(nsteps):
+        xo, yo = x[0], y[0]
+        orc.push_particles(E, B, J, x, y, z, ux, uy, uz, qw, sp)
+        px += (x[0] - xo + 16) % 32 - 16
+        py += (y[0] - yo + 16) % 32 - 16
+    vd = np.array([px, py]) / (nsteps * dt)
+    want = np.array([Ey * Bz, 0.0]) / Bz ** 2
+    assert abs(vd[0] / want[0] - 1) < 1e-3
+    assert abs(vd[1]) < 1e-3 * want[0]
+
+
+# ------------------------------------------------------------------------------------------------
+# deposits: continuity Eq. 25, total current, brute force, 1-d reduction
+
+def _random_moves(rng, n, dx, dt, npart, max_frac=0.999):
+    """random old/new positions with |move| < max_frac cell per direction (c dt < dx)"""
+    x0 = [rng.random(npart) * n[d] * dx[d] for d in range(3)]
+    x1 = []
+    for d in range(3):
+        if n[d] == 1:
+            x1.append(x0[d].copy())
+        else:
+            x1.append(x0[d] + (2 * rng.random(npart) - 1) * max_frac * dx[d])
+    v = [(x1[d] - x0[d]) / dt if n[d] > 1 else 0.6 * (2 * rng.random(npart) - 1) for d in range(3)]
+    return [_c(a) for a in x0], [_c(a) for a in x1], [_c(a) for a in v]
+
+
+def _wrapped(x1, n, dx):
+    return [_c(np.mod(x1[d], n[d] * dx[d])) for d in range(3)]
+
+
+CASES = [(1, (6, 5, 7), (1.0, 0.8, 1.3)), (1, (1, 8, 6), (1.0, 1.0, 0.7)), (1, (7, 1, 6), (1.1, 1.0, 0.9)),
+         (2, (6, 7, 8), (1.0, 0.8, 1.3)), (2, (1, 8, 6), (1.0, 1.0, 0.7)), (1, (9, 1, 1), (0.9, 1.0, 1.0))]
+
+
+@pytest.mark.parametrize("order,n,dx", CASES)
+def test_deposit_continuity_per_particle_and_summed(order, n, dx):
+    """Eq. 25: (rho^{n+3/2} - rho^{n+1/2})/dt + div- j^{n+1} = 0 at every node, for each particle
+    alone and for all together; rho assigned with b1 (order 1) / b2 (order 2)."""
+    dt = 0.45 * min(dx)
+    rng = np.random.default_rng(11 + order)
+    orc = Oracle(n, dx, dt, order, [-1.0], [1.0])
+    # order 2 with two ghost layers assumes moves <= 1/2 cell; the oracle itself has no such limit
+    x0, x1, v = _random_moves(rng, n, dx, dt, 40)
+    qw = _c(rng.standard_normal(40))
+    x1w = _wrapped(x1, n, dx)
+    scale = np.abs(qw).max() / (dx[0] * dx[1] * dx[2]) / dt
+    Jall = orc.zeros_field()
+    orc.deposit(Jall, *x0, *x1, *v, qw)
+    res = (orc.rho(*x1w, qw) - orc.rho(*x0, qw)) / dt + orc.div_minus(Jall)
+    assert np.abs(res).max() < 1e-12 * scale
+    for a in range(40):
+        sl = slice(a, a + 1)
+        J = orc.zeros_field()
+        orc.deposit(J, *[_c(c[sl]) for c in x0], *[_c(c[sl]) for c in x1], *[_c(c[sl]) for c in v], _c(qw[sl]))
+        res = (orc.rho(*[_c(c[sl]) for c in x1w], _c(qw[sl])) - orc.rho(*[_c(c[sl]) for c in x0], _c(qw[sl]))) / dt \
+            + orc.div_minus(J)
+        assert np.abs(res).max() < 1e-12 * scale
+        assert np.abs(J).max() > 0
+
+
+@pytest.mark.parametrize("order,n,dx", CASES)
+def test_deposit_total_current(order, n, dx):
+    """sum_grid j dV = sum_p qw (x1 - x0)/dt; along an invariant direction = sum_p qw v."""
+    dt = 0.45 * min(dx)
+    rng = np.random.default_rng(21 + order)
+    orc = Oracle(n, dx, dt, order, [-1.0], [1.0])
+    x0, x1, v = _random_moves(rng, n, dx, dt, 30)
+    qw = _c(rng.standard_normal(30))
+    J = orc.zeros_field()
+    orc.deposit(J, *x0, *x1, *v, qw)
+    dV = dx[0] * dx[1] * dx[2]
+    for c in range(3):
+        want = np.sum(qw * v[c])
+        assert abs(J[c].sum() * dV - want) < 1e-12 * max(1.0, abs(want))
+
+
+@pytest.mark.parametrize("n,dx", [((6, 5, 7), (1.0, 0.8, 1.3)), ((1, 6, 6), (1.0, 1.0, 0.7))])
+def test_vb_equals_flux_definition(n, dx):
+    """order 1: split-trajectory deposit == time integral of the instantaneous flux
+    qw/dV v_c 1[xi_c in cell] b1 b1 -- exact piecewise Gauss quadrature (1e-13) and a plain
+    midpoint rule on the same definition (2e5 samples, 1e-5)."""
+    dt = 0.45 * min(dx)
+    rng = np.random.default_rng(31)
+    orc = Oracle(n, dx, dt, 1, [-1.0], [1.0])
+    bf = BruteForce(n, dx, dt, 1, [-1.0], [1.0])
+    x0, x1, v = _random_moves(rng, n, dx, dt, 10)
+    # force specific crossing patterns: none, one face, all faces, landing exactly on a face
+    x1[2][0] = x0[2][0] = 2.3 * dx[2]
+    x1[1][0] = x0[1][0] + 1e-3
+    x0[1][1], x1[1][1] = 2.9 * dx[1], 3.2 * dx[1]
+    x0[2][2], x1[2][2] = 3.1 * dx[2], 2.6 * dx[2]
+    x0[1][2], x1[1][2] = 1.05 * dx[1], 0.8 * dx[1]
+    x0[2][3], x1[2][3] = 2.5 * dx[2], 3.0 * dx[2]
+    for d in range(3):
+        if n[d] > 1:
+            v[d][:] = (x1[d] - x0[d]) / dt
+    qw = _c(rng.standard_normal(10))
+    for a in range(10):
+        sl = slice(a, a + 1)
+        J = orc.zeros_field()
+        orc.deposit(J, *[_c(c[sl]) for c in x0], *[_c(c[sl]) for c in x1], *[_c(c[sl]) for c in v], _c(qw[sl]))
+        p0 = [x0[d][a] for d in range(3)]
+        p1 = [x1[d][a] for d in range(3)]
+        vv = [v[d][a] for d in range(3)]
+        Jex = bf.vb_exact(p0, p1, vv, qw[a])
+        assert np.abs(J - Jex).max() < 1e-13 * max(1.0, np.abs(Jex).max())
+        if a < 4:
+            Jmid = bf.vb_midpoint(p0, p1, vv, qw[a], 200000)
+            assert np.abs(J - Jmid).max() < 1e-5 * np.abs(J).max()
+
+
+@pytest.mark.parametrize("n,dx", [((6, 7, 8), (1.0, 0.8, 1.3)), ((1, 8, 6), (1.0, 1.0, 0.7))])
+def test_esirkepov_equals_whole_grid_decomposition(n, dx):
+    """order 2: 5-point-stencil deposit == density decomposition evaluated on every node of the
+    grid with Eq. 31, running sum started half a grid away from the particle."""
+    dt = 0.45 * min(dx)
+    rng = np.random.default_rng(41)
+    orc = Oracle(n, dx, dt, 2, [-1.0], [1.0])
+    bf = BruteForce(n, dx, dt, 2, [-1.0], [1.0])
+    x0, x1, v = _random_moves(rng, n, dx, dt, 8, max_frac=0.5)
+    qw = _c(rng.standard_normal(8))
+    for a in range(8):
+        sl = slice(a, a + 1)
+        J = orc.zeros_field()
+        orc.deposit(J, *[_c(c[sl]) for c in x0], *[_c(c[sl]) for c in x1], *[_c(c[sl]) for c in v], _c(qw[sl]))
+        Jbf = bf.esirkepov([x0[d][a] for d in range(3)], [x1[d][a] for d in range(3)],
+                           [v[d][a] for d in range(3)], qw[a])
+        assert np.abs(J - Jbf).max() < 1e-13 * max(1.0, np.abs(Jbf).max())
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_deposit_axis_aligned_is_cloud_flux_through_faces(order):
+    """a move along x only: j_x(i+1/2,j,k) = qw/(dV dt) dx * [charge fraction of the particle's
+    cloud (b0 for order 1, b1 for order 2) that passed the face i+1/2] * s(y-j) s(z-k); j_y = j_z = 0."""
+    n, dx, dt = (8, 6, 6), (1.0, 0.8, 1.25), 0.4
+
+    def cdf(u):   # fraction of the cloud centred at 0 lying below u
+        if order == 1:
+            return min(max(u + 0.5, 0.0), 1.0)
+        if u <= -1:
+            return 0.0
+        if u <= 0:
+            return 0.5 * (1 + u) ** 2
+        if u <= 1:
+            return 1 - 0.5 * (1 - u) ** 2
+        return 1.0
+
+    s = (lambda t: max(0.0, 1 - abs(t))) if order == 1 else \
+        (lambda t: 0.75 - t * t if abs(t) <= 0.5 else (0.5 * (1.5 - abs(t)) ** 2 if abs(t) <= 1.5 else 0.0))
+    orc = Oracle(n, dx, dt, order, [-1.0], [1.0])
+    dV = dx[0] * dx[1] * dx[2]
+    for (xa, xb) in ((2.2, 2.6), (2.7, 3.1), (3.3, 2.9), (4.0, 4.4), (5.6, 5.2)):
+        y, z, qw = 2.3 * dx[1], 3.6 * dx[2], 0.7
+        J = orc.zeros_field()
+        orc.deposit(J, _c([xa * dx[0]]), _c([y]), _c([z]), _c([xb * dx[0]]), _c([y]), _c([z]),
+                    _c([(xb - xa) * dx[0] / dt]), _c([0.0]), _c([0.0]), _c([qw]))
+        assert np.abs(J[1]).max() < 1e-15 and np.abs(J[2]).max() < 1e-15
+        for i in range(n[0]):
+            # cloud centre moves xa -> xb; fraction above the face before minus after = passed upward
+            passed = cdf(xb - (i + 0.5)) - cdf(xa - (i + 0.5))
+            for j in range(n[1]):
+                for k in range(n[2]):
+                    want = qw * dx[0] / (dV * dt) * passed * s(y / dx[1] - j) * s(z / dx[2] - k)
+                    assert abs(J[0, k, j, i] - want) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# sort
+
+@pytest.mark.parametrize("n,block", [((1, 16, 24), (1, 4, 8)), ((8, 12, 16), (4, 4, 4)), ((1, 8, 8), (1, 8, 8))])
+def test_sort_against_numpy_stable_argsort(n, block):
+    rng = np.random.default_rng(3)
+    npart = 5000
+    orc = Oracle(n, (1.0, 1.0, 1.0), 0.3, 1, [-1.0], [1.0], block=block)
+    pos = [(rng.random(npart) * n[d]).astype(np.float32) for d in range(3)]
+    for d in range(3):
+        pos[d][pos[d] >= n[d]] = np.nextafter(np.float32(n[d]), np.float32(0))
+    pos[1][:5] = [0.0, 1.0, 3.9999998, 4.0, n[1] - 1]            # exactly on faces
+    cell_idx, key, perm, offs = orc.sort(*pos)
+    c = [np.floor(pos[d]).astype(np.int64) if n[d] > 1 else np.zeros(npart, dtype=np.int64) for d in range(3)]
+    assert np.array_equal(cell_idx, (c[2] * n[1] + c[1]) * n[0] + c[0])
+    nb = [n[d] // block[d] for d in range(3)]
+    b = [c[d] // block[d] for d in range(3)]
+    l = [c[d] % block[d] for d in range(3)]
+    want_key = ((b[2] * nb[1] + b[1]) * nb[0] + b[0]) * (block[0] * block[1] * block[2]) \
+        + (l[2] * block[1] + l[1]) * block[0] + l[0]
+    assert np.array_equal(key, want_key)
+    assert np.array_equal(perm, np.argsort(want_key, kind="stable"))
+    assert np.array_equal(np.sort(perm), np.arange(npart))
+    assert np.all(np.diff(key[perm]) >= 0)
+    hist = np.bincount(want_key, minlength=n[0] * n[1] * n[2])
+    assert np.array_equal(offs, np.concatenate([[0], np.cumsum(hist)]))
+    # a block's particles are contiguous: keys of one block form one run
+    blk = key[perm] // (block[0] * block[1] * block[2])
+    assert np.all(np.diff(blk) >= 0)
+
+
+def test_sort_rejects_out_of_domain():
+    orc = Oracle((1, 8, 8), (1.0, 1.0, 1.0), 0.3, 1, [-1.0], [1.0], block=(1, 4, 4))
+    z = np.array([8.0], dtype=np.float32)
+    with pytest.raises(ValueError):
+        orc.sort(np.zeros(1, dtype=np.float32), np.zeros(1, dtype=np.float32), z)
+
+
+# ------------------------------------------------------------------------------------------------
+# whole step (Fig. 8)
+
+def _small_plasma(rng, n, dx, npart, vth):
+    pos = [_c(rng.random(npart) * n[d] * dx[d]) for d in range(3)]
+    u = [_c(rng.standard_normal(npart) * vth) for _ in range(3)]
+    species = (np.arange(npart) % 2).astype(np.int32)
+    qw = _c(np.where(species == 0, -1.0, 1.0) * (0.05 + 0.1 * rng.random(npart)))
+    return pos, u, qw, species
+
+
+@pytest.mark.parametrize("order,n", [(1, (5, 4, 6)), (1, (1, 6, 5)), (2, (6, 6, 7)), (2, (1, 7, 6)), (1, (6, 1, 1))])
+@pytest.mark.parametrize("npart", [1, 8])
+def test_step_t1_equals_t0(order, n, npart):
+    """three full steps of the stencil oracle == the definition-level brute force (gather over the
+    whole grid, flux-integral / whole-grid deposits, np.roll FDTD) on 1-8 particles."""
+    dx = (1.0, 0.9, 1.2)
+    dt = 0.45 / np.sqrt(sum(1 / dx[d] ** 2 for d in range(3) if n[d] > 1))
+    q, m = [-1.0, 1.0], [1.0, 4.0]
+    rng = np.random.default_rng(100 * order + npart + n[0])
+    orc = Oracle(n, dx, dt, order, q, m)
+    bf = BruteForce(n, dx, dt, order, q, m)
+    pos, u, qw, species = _small_plasma(rng, n, dx, npart, 0.6)
+    E = 0.3 * rng.standard_normal(orc.fshape)
+    B = 0.3 * rng.standard_normal(orc.fshape)
+    J = orc.zeros_field()
+    E0, B0 = E.copy(), B.copy()
+    xs = np.stack(pos, axis=1).copy()
+    us = np.stack(u, axis=1).copy()
+    for _ in range(3):
+        orc.step(E, B, J, *pos, *u, qw, species, 1)
+        J0 = bf.step(E0, B0, xs, us, qw, species)
+        assert np.abs(J - J0).max() < 1e-12
+    assert np.abs(E - E0).max() < 1e-12 and np.abs(B - B0).max() < 1e-12
+    for d in range(3):
+        L = n[d] * dx[d]
+        dd = np.abs((pos[d] - xs[:, d] + 0.5 * L) % L - 0.5 * L)
+        assert dd.max() < 1e-12
+        assert np.abs(u[d] - us[:, d]).max() < 1e-12
+
+
+@pytest.mark.parametrize("order,n", [(1, (1, 16, 16)), (1, (8, 8, 8)), (2, (8, 8, 8)), (2, (1, 12, 12))])
+def test_step_gauss_law_and_divb_invariants(order, n):
+    """with a charge-conserving j, div- E - rho keeps its initial value and
+    div+ B stays 0 to round-off; no particle moves more than one cell per step."""
+    dx = (1.0, 1.0, 1.0)
+    dt = 0.5 / np.sqrt(sum(1 / dx[d] ** 2 for d in range(3) if n[d] > 1))
+    q, m = [-1.0, 1.0], [1.0, 25.0]
+    rng = np.random.default_rng(5 + order)
+    orc = Oracle(n, dx, dt, order, q, m)
+    npart = 4000
+    pos, u, qw, species = _small_plasma(rng, n, dx, npart, 0.3)
+    E = 0.05 * rng.standard_normal(orc.fshape)
+    F = rng.standard_normal(orc.fshape)
+    B = 0.2 * orc.curl_plus(F)                     # divergence-free by Eq. 23
+    J = orc.zeros_field()
+    g0 = orc.div_minus(E) - orc.rho(*pos, qw)
+    scale = np.abs(orc.rho(*[p[species == 0] for p in map(np.ascontiguousarray, pos)],
+                           _c(qw[species == 0]))).max()
+    for _ in range(20):
+        old = [p.copy() for p in pos]
+        orc.step(E, B, J, *pos, *u, qw, species, 1)
+        for d in range(3):
+            if n[d] > 1:
+                dc = np.floor(pos[d] / dx[d]) - np.floor(old[d] / dx[d])
+                dc = (dc + n[d] // 2) % n[d] - n[d] // 2
+                assert np.abs(dc).max() <= 1
+    g1 = orc.div_minus(E) - orc.rho(*pos, qw)
+    assert np.abs(g1 - g0).max() < 1e-12 * max(scale, 1.0)
+    assert np.abs(orc.div_plus(B)).max() < 1e-13
+
+
+def test_energy_drift_bounded_config1_1000_steps():
+    """energy is not conserved exactly; on BASELINE.json config 1 (2-d thermal
+    plasma, 131072 particles) total energy drifts by less than 5 % over 1000 steps."""
+    import psc_inputs
+
+    pl = psc_inputs.make_config(1)
+    orc = Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m)
+    cols = [_c(t.numpy()) for t in (pl.x, pl.y, pl.z, pl.ux, pl.uy, pl.uz, pl.qw)]
+    sp = np.ascontiguousarray(pl.species.numpy())
+    E, B, J = _c(pl.E.numpy()), _c(pl.B.numpy()), orc.zeros_field()
+    e0 = orc.energy(E, B, cols[3], cols[4], cols[5], cols[6], sp).sum()
+    g0 = orc.div_minus(E) - orc.rho(cols[0], cols[1], cols[2], cols[6])
+    assert np.abs(g0).max() < 1e-12          # co-located species: rho = 0, E = 0 (A21)
+    hist = []
+    for _ in range(10):
+        orc.step(E, B, J, *cols, sp, 100)
+        hist.append(orc.energy(E, B, cols[3], cols[4], cols[5], cols[6], sp).sum())
+    hist = np.array(hist)
+    assert np.abs(hist / e0 - 1).max() < 0.05
+    g1 = orc.div_minus(E) - orc.rho(cols[0], cols[1], cols[2], cols[6])
+    assert np.abs(g1 - g0).max() < 1e-12
+    assert np.abs(orc.div_plus(B)).max() < 1e-13
