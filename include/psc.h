@@ -1,0 +1,171 @@
+/*
+ * psc.h -- C ABI of the B200-native particle-in-cell hot path of arXiv:1310.7866
+ * (Germaschewski et al., "The Plasma Simulation Code").
+ *
+ * The calls follow the paper's module split (a field pusher with an E method
+ * and a B method, a particle pusher, a sort, ghost-point exchange; state in `psc_fields` and
+ * `psc_particles`) and the optimised time step of Fig. 8.
+ *
+ * General rules
+ *   - Every pointer is a DEVICE pointer unless its name or comment says "host".
+ *   - The library never allocates particle or field storage: the caller owns all buffers (and the
+ *     stream) and the library borrows the pointers until the next bind or psc_destroy.  The only
+ *     device memory the context owns is a 64-byte status/counter block.
+ *   - Every call that does device work enqueues it on `stream` (a cudaStream_t passed as void*)
+ *     and returns without synchronising, except psc_status, psc_step_host and psc_sort_result_host.
+ *   - Every call returns 0 (PSC_OK) or a negative PSC_ERR_* code; nothing aborts or throws across
+ *     the ABI.  Data-dependent faults are sticky device flags read with psc_status.
+ *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
+ *     PSC_ERR_CUDA.
+ *
+ * Units and conventions: c = eps0 = mu0 = 1; momentum columns hold
+ * u = p/(m_s c); qw = q_s * w; positions are absolute, in [0, n[d]*dx[d]); a direction with
+ * n[d] == 1 is invariant: no ghosts, no derivative, its coordinate is carried but never advanced.
+ *
+ * Field layout: each of E, B, J is float[3][ez][ey][ex] with ex = n[0] + 2*g (1 if n[0] == 1)
+ * etc., x fastest; interior cell i is stored at i + g.  Yee staggering (PAPER.md:141-143,
+ * Eq. 20-21):  E[0]=E_x(i+1/2,j,k)  E[1]=E_y(i,j+1/2,k)  E[2]=E_z(i,j,k+1/2);
+ * B[0]=B_x(i,j+1/2,k+1/2)  B[1]=B_y(i+1/2,j,k+1/2)  B[2]=B_z(i+1/2,j+1/2,k); J is co-located
+ * with E.  Ghost layers hold periodic images.
+ */
+#ifndef PSC_H
+#define PSC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PSC_OK 0
+#define PSC_ERR_INVALID_ARG (-1)
+#define PSC_ERR_NOT_BOUND (-2)
+#define PSC_ERR_NOT_SORTED (-3)
+#define PSC_ERR_CFL (-4)
+#define PSC_ERR_ALIGN (-5)
+#define PSC_ERR_CUDA (-6)
+#define PSC_ERR_UNSUPPORTED (-7)
+#define PSC_ERR_WORKSPACE (-8)
+
+#define PSC_E 0
+#define PSC_B 1
+#define PSC_J 2
+
+/* sticky device flags (psc_status) */
+#define PSC_F_OOB 1u            /* a particle position outside [0, n*dx) was seen by the sort */
+#define PSC_F_MOVED_GT_1CELL 2u /* a particle moved more than one cell in a step */
+#define PSC_F_NAN 4u            /* a non-finite position or momentum was produced */
+#define PSC_F_NOT_IN_TILE 8u    /* push found a particle outside the block its sort slot belongs to */
+
+#define PSC_MAX_SPECIES 8
+#define PSC_GHOST 2
+
+typedef struct psc_ctx psc_ctx; /* opaque, host side */
+
+typedef struct {
+  int32_t n[3];      /* interior cells x,y,z; n[d] == 1: invariant direction; otherwise >= 4 */
+  int32_t ghost;     /* ghost layers in every non-invariant direction; must be PSC_GHOST (2),
+                        which suffices for both orders when dt <= min(dx)/2 */
+  float dx[3];       /* cell sizes */
+  float dt;          /* must satisfy dt <= min over non-invariant d of dx[d]/2 (PSC_ERR_CFL) */
+  int32_t order;     /* 1: b1 gather + Villasenor-Buneman; 2: b2 gather + Esirkepov
+                         */
+  int32_t n_species; /* 1..PSC_MAX_SPECIES */
+  const float *q;    /* host array [n_species], charge */
+  const float *m;    /* host array [n_species], mass */
+  int32_t block[3];  /* sort block ("supercell") in cells; 0: library default;
+                        must divide n[d]; 1 along invariant directions */
+} psc_params;
+
+/* One set of particle columns (structure of arrays), each of length >= n.
+ * `id` may be NULL in both sets (then no id is carried). */
+typedef struct {
+  float *x, *y, *z;    /* positions x^{n+1/2} */
+  float *ux, *uy, *uz; /* u^n = p/(m c) */
+  float *qw;           /* q_s * w */
+  int32_t *species;    /* 0 .. n_species-1 */
+  int32_t *id;         /* caller's tag, moved with the particle */
+} psc_particle_cols;
+
+/* Creates a context.  Validates sizes, block divisibility, the time-step limit.  Host only. */
+int psc_create(const psc_params *params, psc_ctx **out);
+void psc_destroy(psc_ctx *ctx);
+
+/* Scratch the caller must provide for up to max_particles particles (sort keys, permutation,
+ * histograms, scan temporaries).  Host only. */
+size_t psc_workspace_bytes(const psc_ctx *ctx, int64_t max_particles);
+/* ws must be 256-byte aligned (PSC_ERR_ALIGN) and at least psc_workspace_bytes large. */
+int psc_bind_workspace(psc_ctx *ctx, void *ws, size_t bytes);
+
+/* E, B, J in the layout above.  The caller fills E and B including ghosts, or calls
+ * psc_fill_ghosts afterwards.  J need not be initialised. */
+int psc_bind_fields(psc_ctx *ctx, float *E, float *B, float *J);
+/* Number of floats in one of E/B/J (3 * ex * ey * ez) and the extents; host only. */
+int64_t psc_field_elems(const psc_ctx *ctx, int32_t ext[3]);
+
+/* `primary` holds the n particles; `secondary` is a second buffer set of the same shapes used by
+ * the out-of-place reorder.  Binding marks the particle list as unsorted. */
+int psc_bind_particles(psc_ctx *ctx, int64_t n, const psc_particle_cols *primary,
+                       const psc_particle_cols *secondary);
+
+/* Cell-key counting sort.  key = block-major, cell-minor; stable (ascending
+ * input index inside a key).  Afterwards the CURRENT column set (psc_particles_current) holds
+ * the particles in sorted order; the two sets swap roles.  Arbitrary input order is accepted;
+ * when the list is the previous sort's output advanced by one psc_push_particles, a cheaper
+ * path that exploits "a particle moves at most one cell per step" is taken --
+ * the result is identical. */
+int psc_particles_sort(psc_ctx *ctx, void *stream);
+
+/* The particle loop of Fig. 8 in one pass over the particles
+ * (PAPER.md:603): zero J; per particle gather E,B at x^{n+1/2} (Eq. 11), Boris push
+ * p^n -> p^{n+1} (Eq. 27-28), x^{n+1/2} -> x^{n+3/2} (Eq. 26), charge-conserving deposit of
+ * j^{n+1}, periodic wrap.  Requires a sorted list (PSC_ERR_NOT_SORTED).
+ * J ghosts are NOT folded on return (psc_exchange_j). */
+int psc_push_particles(psc_ctx *ctx, void *stream);
+
+/* FDTD (Eq. 17-18): which == PSC_B: B -= frac*dt*curl+ E;
+ * which == PSC_E: E += frac*dt*(curl- B - J) (J interior must be folded).  Interior and ghost
+ * points of the updated field are written consistently. */
+int psc_push_fields(psc_ctx *ctx, int which, float frac, void *stream);
+
+/* add_and_fill_ghosts_j of Fig. 8 on one GPU: add every ghost value of J onto its periodic
+ * image in the interior, then refill the ghosts from the interior. */
+int psc_exchange_j(psc_ctx *ctx, void *stream);
+/* fill_ghosts of Fig. 7/8 for which in {PSC_E, PSC_B, PSC_J}: ghosts := periodic images. */
+int psc_fill_ghosts(psc_ctx *ctx, int which, void *stream);
+
+/* One time step, Fig. 8: sort, B half, particle loop, B half,
+ * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
+ * u^{n+1}. */
+int psc_step(psc_ctx *ctx, void *stream);
+
+/* End-to-end form with HOST buffers: copies the host particle columns (n particles) and host
+ * E, B (full layout incl. ghosts) into the bound device buffers, runs `nsteps` psc_step, copies
+ * particles, E, B, J back, and synchronises the stream.  Host pointers should be pinned.
+ * host->id may be NULL iff no id is bound. */
+int psc_step_host(psc_ctx *ctx, void *stream, int64_t n, const psc_particle_cols *host,
+                  float *hostE, float *hostB, float *hostJ, int nsteps);
+
+/* Inspection.  Device pointers into the workspace, valid until the next sort:
+ * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i), perm[n] (sorted slot s holds
+ * input particle perm[s]), cell_offsets[n_keys+1] (exclusive scan of the key histogram). */
+int psc_sort_result(const psc_ctx *ctx, const int32_t **cell_idx, const int32_t **perm,
+                    const int32_t **cell_offsets, int64_t *n_keys);
+/* The column set that currently holds the particles. */
+int psc_particles_current(const psc_ctx *ctx, psc_particle_cols *out);
+/* Synchronises `stream`, returns and keeps the sticky flags. */
+int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);
+/* Kernels and memsets/copies this context has enqueued so far (host counter). */
+int64_t psc_launch_count(const psc_ctx *ctx);
+/* Last CUDA runtime error code seen by this context (0 if none). */
+int psc_last_cuda_error(const psc_ctx *ctx);
+/* Selects kernel variants for experiments; 0 = default.  Host only. */
+int psc_set_option(psc_ctx *ctx, const char *name, int64_t value);
+const char *psc_strerror(int code);
+const char *psc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PSC_H */

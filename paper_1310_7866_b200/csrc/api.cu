@@ -1,0 +1,336 @@
+// api.cu -- the C ABI of include/psc.h: context, binding, the time step of Fig. 8.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "psc_internal.cuh"
+
+namespace {
+
+bool cols_complete(const psc_particle_cols *c) {
+  return c->x && c->y && c->z && c->ux && c->uy && c->uz && c->qw && c->species;
+}
+
+Cols to_cols(const psc_particle_cols *c) {
+  Cols o;
+  o.x = c->x; o.y = c->y; o.z = c->z;
+  o.ux = c->ux; o.uy = c->uy; o.uz = c->uz;
+  o.qw = c->qw; o.sp = c->species; o.id = c->id;
+  return o;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *psc_version(void) { return "psc-b200 0.1 (sm_100a)"; }
+
+const char *psc_strerror(int code) {
+  switch (code) {
+    case PSC_OK: return "ok";
+    case PSC_ERR_INVALID_ARG: return "invalid argument";
+    case PSC_ERR_NOT_BOUND: return "fields, particles or workspace not bound";
+    case PSC_ERR_NOT_SORTED: return "particle list is not sorted";
+    case PSC_ERR_CFL: return "time step too large (need dt <= min dx / 2)";
+    case PSC_ERR_ALIGN: return "pointer not sufficiently aligned";
+    case PSC_ERR_CUDA: return "CUDA runtime error (see psc_last_cuda_error)";
+    case PSC_ERR_UNSUPPORTED: return "configuration not supported by this build";
+    case PSC_ERR_WORKSPACE: return "workspace too small";
+    default: return "unknown error";
+  }
+}
+
+int psc_create(const psc_params *p, psc_ctx **out) {
+  if (!p || !out) return PSC_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (p->order != 1 && p->order != 2) return PSC_ERR_INVALID_ARG;
+  if (p->n_species < 1 || p->n_species > PSC_MAX_SPECIES || !p->q || !p->m) return PSC_ERR_INVALID_ARG;
+  if (p->ghost != PSC_GHOST) return PSC_ERR_INVALID_ARG;
+  if (!(p->dt > 0.f)) return PSC_ERR_INVALID_ARG;
+  int nact = 0;
+  for (int d = 0; d < 3; d++) {
+    if (p->n[d] != 1 && p->n[d] < 2 * PSC_GHOST) return PSC_ERR_INVALID_ARG;
+    if (!(p->dx[d] > 0.f)) return PSC_ERR_INVALID_ARG;
+    if (p->n[d] > 1) {
+      nact++;
+      if (p->dt > 0.5f * p->dx[d] * (1.f + 1e-6f)) return PSC_ERR_CFL;
+    }
+  }
+  if (nact == 0) return PSC_ERR_INVALID_ARG;
+  for (int s = 0; s < p->n_species; s++)
+    if (!(p->m[s] > 0.f)) return PSC_ERR_INVALID_ARG;
+
+  psc_ctx *c = (psc_ctx *)calloc(1, sizeof(psc_ctx));
+  if (!c) return PSC_ERR_INVALID_ARG;
+  GridDesc &gd = c->gd;
+  const bool is3d = nact == 3;
+  int64_t tot = 1, nk = 1;
+  double dV = 1.0;
+  for (int d = 0; d < 3; d++) {
+    gd.n[d] = p->n[d];
+    gd.g[d] = p->n[d] > 1 ? PSC_GHOST : 0;
+    gd.ext[d] = gd.n[d] + 2 * gd.g[d];
+    gd.dx[d] = p->dx[d];
+    gd.inv_dx[d] = 1.0f / p->dx[d];
+    gd.L[d] = (float)p->n[d] * p->dx[d];
+    gd.dt_dx[d] = p->n[d] > 1 ? p->dt / p->dx[d] : 0.f;
+    dV *= (double)p->dx[d];
+    tot *= gd.ext[d];
+    nk *= gd.n[d];
+    int bs = p->block[d];
+    if (p->n[d] == 1) bs = 1;
+    if (bs == 0) {  // default supercell: 8x8 cells in 2-d, 4x4x4 in 3-d, shrunk to divide n
+      bs = is3d ? 4 : 8;
+      while (bs > 1 && p->n[d] % bs) bs >>= 1;
+    }
+    if (bs < 1 || p->n[d] % bs) {
+      free(c);
+      return PSC_ERR_INVALID_ARG;
+    }
+    gd.bs[d] = bs;
+    gd.nb[d] = p->n[d] / bs;
+  }
+  if (tot * 3 > 0x7fffffffLL || nk > 0x3fffffffLL) {
+    free(c);
+    return PSC_ERR_INVALID_ARG;
+  }
+  gd.st[0] = 1;
+  gd.st[1] = gd.ext[0];
+  gd.st[2] = gd.ext[0] * gd.ext[1];
+  for (int d = 0; d < 3; d++) gd.nbo[d] = gd.n[d] > 1 ? gd.st[d] : 0;
+  gd.comp = (int)tot;
+  gd.dt = p->dt;
+  gd.inv_dV = (float)(1.0 / dV);
+  for (int d = 0; d < 3; d++) gd.cur[d] = (float)((double)p->dx[d] / ((double)p->dt * dV));
+  gd.cpb = gd.bs[0] * gd.bs[1] * gd.bs[2];
+  gd.nkeys = (int)nk;
+  gd.ntiles = gd.nb[0] * gd.nb[1] * gd.nb[2];
+  gd.order = p->order;
+  gd.nsp = p->n_species;
+  for (int s = 0; s < p->n_species; s++) {
+    c->q[s] = p->q[s];
+    c->m[s] = p->m[s];
+    gd.qmh[s] = (float)((double)p->q[s] * (double)p->dt / (2.0 * (double)p->m[s]));
+  }
+  // order 2 touches J nodes c-2..c+2 only while a particle moves less than half a cell
+  // (A15): guaranteed by the dt check above.
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaMalloc((void **)&c->d_flags, 64) != cudaSuccess ||
+      cudaMemset(c->d_flags, 0, 64) != cudaSuccess) {
+    c->last_err = (int)cudaGetLastError();
+    if (c->d_flags) cudaFree(c->d_flags);
+    free(c);
+    return PSC_ERR_CUDA;  // no device: there is no CPU fallback
+  }
+  c->opt_threads = 0;
+  *out = c;
+  return PSC_OK;
+}
+
+void psc_destroy(psc_ctx *c) {
+  if (!c) return;
+  if (c->d_flags) cudaFree(c->d_flags);
+  free(c);
+}
+
+size_t psc_workspace_bytes(const psc_ctx *c, int64_t max_particles) {
+  if (!c || max_particles < 0) return 0;
+  return psc_sort_workspace_bytes(c, max_particles) + 256;
+}
+
+int psc_bind_workspace(psc_ctx *c, void *ws, size_t bytes) {
+  if (!c || !ws) return PSC_ERR_INVALID_ARG;
+  if (((uintptr_t)ws) & 255) return PSC_ERR_ALIGN;
+  c->ws = ws;
+  c->ws_bytes = bytes;
+  c->ws_cap = -1;
+  c->have_sort_result = 0;
+  if (c->have_particles) {
+    if (bytes < psc_workspace_bytes(c, c->np)) return PSC_ERR_WORKSPACE;
+    const int rc = psc_sort_carve(c, c->np);
+    if (rc) return rc;
+    c->ws_cap = c->np;
+  }
+  return PSC_OK;
+}
+
+int64_t psc_field_elems(const psc_ctx *c, int32_t ext[3]) {
+  if (!c) return 0;
+  if (ext)
+    for (int d = 0; d < 3; d++) ext[d] = c->gd.ext[d];
+  return 3 * (int64_t)c->gd.comp;
+}
+
+int psc_bind_fields(psc_ctx *c, float *E, float *B, float *J) {
+  if (!c || !E || !B || !J) return PSC_ERR_INVALID_ARG;
+  if ((((uintptr_t)E) | ((uintptr_t)B) | ((uintptr_t)J)) & 15) return PSC_ERR_ALIGN;
+  c->E = E;
+  c->B = B;
+  c->J = J;
+  c->have_fields = 1;
+  return PSC_OK;
+}
+
+int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const psc_particle_cols *b) {
+  if (!c || !a || !b || n < 0 || n > 0x7fffff00LL) return PSC_ERR_INVALID_ARG;
+  if (!cols_complete(a) || !cols_complete(b)) return PSC_ERR_INVALID_ARG;
+  if ((a->id == nullptr) != (b->id == nullptr)) return PSC_ERR_INVALID_ARG;
+  const void *ptrs[] = {a->x, a->y, a->z, a->ux, a->uy, a->uz, a->qw, a->species, a->id,
+                        b->x, b->y, b->z, b->ux, b->uy, b->uz, b->qw, b->species, b->id};
+  for (const void *p : ptrs)
+    if (((uintptr_t)p) & 15) return PSC_ERR_ALIGN;
+  c->cols[0] = to_cols(a);
+  c->cols[1] = to_cols(b);
+  c->cur = 0;
+  c->np = n;
+  c->have_particles = 1;
+  c->state = PSC_STATE_UNSORTED;
+  c->have_sort_result = 0;
+  if (c->ws) {
+    if (c->ws_bytes < psc_workspace_bytes(c, n)) {
+      c->ws_cap = -1;
+      return PSC_ERR_WORKSPACE;
+    }
+    const int rc = psc_sort_carve(c, n);
+    if (rc) return rc;
+    c->ws_cap = n;
+  }
+  return PSC_OK;
+}
+
+int psc_particles_sort(psc_ctx *c, void *stream) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  return psc_sort_run(c, (cudaStream_t)stream);
+}
+
+int psc_push_particles(psc_ctx *c, void *stream) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->state != PSC_STATE_SORTED) return PSC_ERR_NOT_SORTED;
+  const int rc = c->gd.order == 1 ? psc_push_order1(c, (cudaStream_t)stream)
+                                  : psc_push_order2(c, (cudaStream_t)stream);
+  if (rc == PSC_OK) c->state = PSC_STATE_UNSORTED;
+  return rc;
+}
+
+int psc_push_fields(psc_ctx *c, int which, float frac, void *stream) {
+  if (!c || !(frac > 0.f)) return PSC_ERR_INVALID_ARG;
+  if (!c->have_fields) return PSC_ERR_NOT_BOUND;
+  if (which == PSC_B) return psc_fields_push_b(c, frac, (cudaStream_t)stream);
+  if (which == PSC_E) return psc_fields_push_e(c, frac, (cudaStream_t)stream);
+  return PSC_ERR_INVALID_ARG;
+}
+
+int psc_fill_ghosts(psc_ctx *c, int which, void *stream) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_fields) return PSC_ERR_NOT_BOUND;
+  float *F = which == PSC_E ? c->E : which == PSC_B ? c->B : which == PSC_J ? c->J : nullptr;
+  if (!F) return PSC_ERR_INVALID_ARG;
+  return psc_fields_fill_ghosts(c, F, (cudaStream_t)stream);
+}
+
+int psc_exchange_j(psc_ctx *c, void *stream) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_fields) return PSC_ERR_NOT_BOUND;
+  int rc = psc_fields_fold(c, c->J, (cudaStream_t)stream);
+  if (rc) return rc;
+  return psc_fields_fill_ghosts(c, c->J, (cudaStream_t)stream);
+}
+
+// Fig. 8.  On one GPU the "single synchronisation point" is stream order:
+// exchange_particles is the periodic wrap inside the push, fill_ghosts_B is part of the B
+// update (ghost points are computed like their images), add_and_fill_ghosts_j is psc_exchange_j.
+int psc_step(psc_ctx *c, void *stream) {
+  int rc;
+  if ((rc = psc_particles_sort(c, stream))) return rc;
+  if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^n -> B^{n+1/2}
+  if ((rc = psc_push_particles(c, stream))) return rc;            // p, x, j^{n+1}
+  if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^{n+1/2} -> B^{n+1}
+  if ((rc = psc_exchange_j(c, stream))) return rc;
+  if ((rc = psc_push_fields(c, PSC_E, 1.0f, stream))) return rc;  // E^{n+1/2} -> E^{n+3/2}
+  return PSC_OK;
+}
+
+int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *h, float *hE,
+                  float *hB, float *hJ, int nsteps) {
+  if (!c || !h || !hE || !hB || nsteps < 0) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->have_fields || !c->ws) return PSC_ERR_NOT_BOUND;
+  if (n != c->np || !cols_complete(h)) return PSC_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t fb = (size_t)3 * c->gd.comp * 4, pb = (size_t)n * 4;
+  {
+    Cols &d = c->cols[c->cur];
+    if ((d.id != nullptr) != (h->id != nullptr)) return PSC_ERR_INVALID_ARG;
+    const void *src[] = {h->x, h->y, h->z, h->ux, h->uy, h->uz, h->qw, h->species, h->id};
+    void *dst[] = {d.x, d.y, d.z, d.ux, d.uy, d.uz, d.qw, d.sp, d.id};
+    for (int i = 0; i < 9; i++)
+      if (dst[i]) PSC_CUDA_TRY(c, cudaMemcpyAsync(dst[i], src[i], pb, cudaMemcpyHostToDevice, s));
+    PSC_CUDA_TRY(c, cudaMemcpyAsync(c->E, hE, fb, cudaMemcpyHostToDevice, s));
+    PSC_CUDA_TRY(c, cudaMemcpyAsync(c->B, hB, fb, cudaMemcpyHostToDevice, s));
+    c->state = PSC_STATE_UNSORTED;
+    c->launches += 11;
+  }
+  for (int i = 0; i < nsteps; i++) {
+    const int rc = psc_step(c, stream);
+    if (rc) return rc;
+  }
+  {
+    Cols &d = c->cols[c->cur];
+    void *dst[] = {h->x, h->y, h->z, h->ux, h->uy, h->uz, h->qw, h->species, h->id};
+    const void *src[] = {d.x, d.y, d.z, d.ux, d.uy, d.uz, d.qw, d.sp, d.id};
+    for (int i = 0; i < 9; i++)
+      if (src[i]) PSC_CUDA_TRY(c, cudaMemcpyAsync(dst[i], src[i], pb, cudaMemcpyDeviceToHost, s));
+    PSC_CUDA_TRY(c, cudaMemcpyAsync(hE, c->E, fb, cudaMemcpyDeviceToHost, s));
+    PSC_CUDA_TRY(c, cudaMemcpyAsync(hB, c->B, fb, cudaMemcpyDeviceToHost, s));
+    if (hJ) PSC_CUDA_TRY(c, cudaMemcpyAsync(hJ, c->J, fb, cudaMemcpyDeviceToHost, s));
+    c->launches += 12;
+  }
+  PSC_CUDA_TRY(c, cudaStreamSynchronize(s));
+  return PSC_OK;
+}
+
+int psc_sort_result(const psc_ctx *c, const int32_t **cell_idx, const int32_t **perm,
+                    const int32_t **cell_offsets, int64_t *n_keys) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_sort_result) return PSC_ERR_NOT_SORTED;
+  if (cell_idx) *cell_idx = c->cell_idx;
+  if (perm) *perm = c->perm;
+  if (cell_offsets) *cell_offsets = c->cell_offsets;
+  if (n_keys) *n_keys = c->gd.nkeys;
+  return PSC_OK;
+}
+
+int psc_particles_current(const psc_ctx *c, psc_particle_cols *out) {
+  if (!c || !out) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles) return PSC_ERR_NOT_BOUND;
+  const Cols &d = c->cols[c->cur];
+  out->x = d.x; out->y = d.y; out->z = d.z;
+  out->ux = d.ux; out->uy = d.uy; out->uz = d.uz;
+  out->qw = d.qw; out->species = d.sp; out->id = d.id;
+  return PSC_OK;
+}
+
+int psc_status(psc_ctx *c, void *stream, uint32_t *flags) {
+  if (!c || !flags) return PSC_ERR_INVALID_ARG;
+  PSC_CUDA_TRY(c, cudaMemcpyAsync(flags, c->d_flags, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  PSC_CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+  return PSC_OK;
+}
+
+int64_t psc_launch_count(const psc_ctx *c) { return c ? c->launches : 0; }
+int psc_last_cuda_error(const psc_ctx *c) { return c ? c->last_err : 0; }
+
+int psc_set_option(psc_ctx *c, const char *name, int64_t value) {
+  if (!c || !name) return PSC_ERR_INVALID_ARG;
+  if (!strcmp(name, "push_variant")) c->opt_push_variant = (int)value;
+  else if (!strcmp(name, "threads")) c->opt_threads = (int)value;
+  else if (!strcmp(name, "clear_flags")) {
+    if (cudaMemset(c->d_flags, 0, 4) != cudaSuccess) return PSC_ERR_CUDA;
+  } else return PSC_ERR_INVALID_ARG;
+  return PSC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,94 @@
+// psc_internal.cuh -- internal declarations of the B200 PIC hot path (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "psc.h"
+
+// Geometry + constants handed to every kernel by value (kernel-parameter space, broadcast
+// through the constant bank).
+struct GridDesc {
+  int n[3];        // interior cells
+  int g[3];        // ghost layers per direction (0 along an invariant direction)
+  int ext[3];      // n + 2g
+  int st[3];       // element strides of one component: {1, ext0, ext0*ext1}
+  int nbo[3];      // neighbour offset per direction: st[d], or 0 along an invariant direction
+  int comp;        // component stride ext0*ext1*ext2
+  float dx[3], inv_dx[3], L[3];
+  float dt;
+  float dt_dx[3];    // dt / dx[d]  (0 along an invariant direction)
+  float cur[3];      // dx[d] / (dt * dV): factor of the in-plane VB / Esirkepov current
+  float inv_dV;
+  int bs[3], nb[3];  // sort block (supercell) size in cells and number of blocks
+  int cpb;           // cells per block
+  int nkeys;         // total cells
+  int ntiles;        // number of blocks
+  int order;
+  int nsp;
+  float qmh[PSC_MAX_SPECIES];  // q_s dt / (2 m_s), the Boris h
+};
+
+struct Cols {
+  float *x, *y, *z, *ux, *uy, *uz, *qw;
+  int32_t *sp;
+  int32_t *id;
+};
+
+enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1 };
+
+struct psc_ctx {
+  GridDesc gd;
+  float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
+  float *E, *B, *J;
+  Cols cols[2];
+  int cur;
+  int64_t np;
+  int have_particles, have_fields;
+  int state;
+  int have_sort_result;
+  // workspace carve-up (all device pointers)
+  void *ws;
+  size_t ws_bytes;
+  int64_t ws_cap;  // max particles the bound workspace was sized for
+  int32_t *key, *perm, *cell_idx, *cell_offsets, *cursor, *scan_tmp, *big_list;
+  uint32_t *d_flags;  // owned: 16 words; [0] sticky flags, [1] big-segment counter
+  int64_t launches;
+  int last_err;
+  int sm_count;
+  // options
+  int opt_push_variant, opt_threads, opt_fuse_ghosts;
+};
+
+#define PSC_CUDA_TRY(ctx, expr)                   \
+  do {                                            \
+    cudaError_t e__ = (expr);                     \
+    if (e__ != cudaSuccess) {                     \
+      (ctx)->last_err = (int)e__;                 \
+      return PSC_ERR_CUDA;                        \
+    }                                             \
+  } while (0)
+
+#define PSC_LAUNCH_CHECK(ctx)                     \
+  do {                                            \
+    (ctx)->launches++;                            \
+    cudaError_t e__ = cudaGetLastError();         \
+    if (e__ != cudaSuccess) {                     \
+      (ctx)->last_err = (int)e__;                 \
+      return PSC_ERR_CUDA;                        \
+    }                                             \
+  } while (0)
+
+static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// fields.cu
+int psc_fields_push_b(psc_ctx *c, float frac, cudaStream_t s);
+int psc_fields_push_e(psc_ctx *c, float frac, cudaStream_t s);
+int psc_fields_fill_ghosts(psc_ctx *c, float *F, cudaStream_t s);
+int psc_fields_fold(psc_ctx *c, float *F, cudaStream_t s);
+// sort.cu
+size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n);
+int psc_sort_carve(psc_ctx *c, int64_t n);
+int psc_sort_run(psc_ctx *c, cudaStream_t s);
+// push1.cu / push2.cu
+int psc_push_order1(psc_ctx *c, cudaStream_t s);
+int psc_push_order2(psc_ctx *c, cudaStream_t s);

@@ -1,0 +1,320 @@
+// push1.cu -- the fused particle loop of Fig. 8 for first-order
+// particles: gather E,B with b1 weights (Eq. 11, 29-31), Boris push (Eq. 27-28),
+// move (Eq. 26), Villasenor-Buneman charge-conserving deposit, periodic wrap.
+//
+// One thread block per sort block ("supercell"): the block stages the E/B values
+// its cells can touch (tile + 1 halo point each side) in shared memory, walks the block's
+// cell-ordered particle range with coalesced column loads, accumulates current in a shared
+// J tile (tile + 1 low / 2 high halo nodes) and flushes the tile to global J once.
+//
+// The VB current is the exact flux of a b0-shaped cloud moving on the straight line
+// x^{n+1/2} -> x^{n+3/2}; it is evaluated by splitting the line at the cell faces it crosses
+// (at most one per direction because dt <= dx/2).  For a segment a -> b inside one cell, with
+// m = (a+b)/2 and del = b-a in units of cells:
+//   j_c(c+1/2, e+al, f+be) += (qw/dV)(del_c dx_c/dt) W_{al,be},
+//   W_00 = (1-m_e)(1-m_f) + del_e del_f/12, W_10 = m_e(1-m_f) - ..., W_01 = (1-m_e)m_f - ...,
+//   W_11 = m_e m_f + del_e del_f/12;
+// in 2-d (x invariant) the in-plane weights reduce to {1-m, m} and the out-of-plane current is
+// the time average of v_x S_y S_z over the segment (A12).
+#include "push_common.cuh"
+
+namespace {
+
+constexpr int PUSH_THREADS = 256;
+
+template <bool D3>
+struct TileGeom {
+  int o[3];        // first cell of the tile (global cell coordinates)
+  int fe[3], fvol; // field tile extents (bs+2 | 1), volume
+  int je[3], jvol; // J tile extents (bs+3 | 1), volume
+  __device__ __forceinline__ void init(const GridDesc &gd, int tile) {
+    const int b0 = tile % gd.nb[0];
+    const int r = tile / gd.nb[0];
+    const int b1 = r % gd.nb[1], b2 = r / gd.nb[1];
+    o[0] = b0 * gd.bs[0];
+    o[1] = b1 * gd.bs[1];
+    o[2] = b2 * gd.bs[2];
+    fe[0] = D3 ? gd.bs[0] + 2 : 1;
+    fe[1] = gd.bs[1] + 2;
+    fe[2] = gd.bs[2] + 2;
+    je[0] = D3 ? gd.bs[0] + 3 : 1;
+    je[1] = gd.bs[1] + 3;
+    je[2] = gd.bs[2] + 3;
+    fvol = fe[0] * fe[1] * fe[2];
+    jvol = je[0] * je[1] * je[2];
+  }
+};
+
+// b1 stencil along one direction for in-cell offset a in [0,1) of tile-local cell l:
+// node-centred quantity: points l, l+1 with weights 1-a, a;
+// half-staggered quantity (sampled at l+1/2): points l-1, l or l, l+1.
+struct Stencil1 {
+  int in, is;      // first point (index into the field tile, halo included)
+  float fn, fs;    // weight of the second point
+  __device__ __forceinline__ void set(int l, float a) {
+    in = l + 1;
+    fn = a;
+    const bool lo = a < 0.5f;
+    is = lo ? l : l + 1;
+    fs = lo ? a + 0.5f : a - 0.5f;
+  }
+};
+
+template <bool D3, bool SX, bool SY, bool SZ>
+__device__ __forceinline__ float gather1(const float *__restrict__ F, const TileGeom<D3> &tg,
+                                         const Stencil1 &sx, const Stencil1 &sy,
+                                         const Stencil1 &sz) {
+  const int iy = SY ? sy.is : sy.in, iz = SZ ? sz.is : sz.in;
+  const float fy = SY ? sy.fs : sy.fn, fz = SZ ? sz.fs : sz.fn;
+  if (D3) {
+    const int ix = SX ? sx.is : sx.in;
+    const float fx = SX ? sx.fs : sx.fn;
+    const float *q = F + (iz * tg.fe[1] + iy) * tg.fe[0] + ix;
+    const int s1 = tg.fe[0], s2 = tg.fe[0] * tg.fe[1];
+    const float v00 = q[0] + fx * (q[1] - q[0]);
+    const float v10 = q[s1] + fx * (q[s1 + 1] - q[s1]);
+    const float v01 = q[s2] + fx * (q[s2 + 1] - q[s2]);
+    const float v11 = q[s2 + s1] + fx * (q[s2 + s1 + 1] - q[s2 + s1]);
+    const float w0 = v00 + fy * (v10 - v00);
+    const float w1 = v01 + fy * (v11 - v01);
+    return w0 + fz * (w1 - w0);
+  } else {
+    const float *q = F + iz * tg.fe[1] + iy;
+    const int s2 = tg.fe[1];
+    const float w0 = q[0] + fy * (q[1] - q[0]);
+    const float w1 = q[s2] + fy * (q[s2 + 1] - q[s2]);
+    return w0 + fz * (w1 - w0);
+  }
+}
+
+// one VB segment in the cell with tile-local coordinates (cx,cy,cz); a*, b* in-cell start/end
+template <bool D3>
+__device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TileGeom<D3> &tg, int cx,
+                                           int cy, int cz, float ax, float ay, float az, float bx,
+                                           float by, float bz, float tau, float fx, float fy,
+                                           float fz, float qvx) {
+  const float my = 0.5f * (ay + by), mz = 0.5f * (az + bz);
+  const float dy = by - ay, dz = bz - az;
+  float *jx = sJ, *jy = sJ + tg.jvol, *jz = sJ + 2 * tg.jvol;
+  if (D3) {
+    const float mx = 0.5f * (ax + bx), dx = bx - ax;
+    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1];
+    const int base = ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1);
+    {
+      const float c = fx * dx, h = dy * dz * (1.0f / 12.0f);
+      atomicAdd(&jx[base], c * ((1.f - my) * (1.f - mz) + h));
+      atomicAdd(&jx[base + s1], c * (my * (1.f - mz) - h));
+      atomicAdd(&jx[base + s2], c * ((1.f - my) * mz - h));
+      atomicAdd(&jx[base + s1 + s2], c * (my * mz + h));
+    }
+    {
+      const float c = fy * dy, h = dz * dx * (1.0f / 12.0f);
+      atomicAdd(&jy[base], c * ((1.f - mz) * (1.f - mx) + h));
+      atomicAdd(&jy[base + s2], c * (mz * (1.f - mx) - h));
+      atomicAdd(&jy[base + 1], c * ((1.f - mz) * mx - h));
+      atomicAdd(&jy[base + s2 + 1], c * (mz * mx + h));
+    }
+    {
+      const float c = fz * dz, h = dx * dy * (1.0f / 12.0f);
+      atomicAdd(&jz[base], c * ((1.f - mx) * (1.f - my) + h));
+      atomicAdd(&jz[base + 1], c * (mx * (1.f - my) - h));
+      atomicAdd(&jz[base + s1], c * ((1.f - mx) * my - h));
+      atomicAdd(&jz[base + s1 + 1], c * (mx * my + h));
+    }
+  } else {
+    const int s2 = tg.je[1];
+    const int base = (cz + 1) * tg.je[1] + (cy + 1);
+    {
+      const float c = qvx * tau, h = dy * dz * (1.0f / 12.0f);
+      atomicAdd(&jx[base], c * ((1.f - my) * (1.f - mz) + h));
+      atomicAdd(&jx[base + 1], c * (my * (1.f - mz) - h));
+      atomicAdd(&jx[base + s2], c * ((1.f - my) * mz - h));
+      atomicAdd(&jx[base + s2 + 1], c * (my * mz + h));
+    }
+    {
+      const float c = fy * dy;
+      atomicAdd(&jy[base], c * (1.f - mz));
+      atomicAdd(&jy[base + s2], c * mz);
+    }
+    {
+      const float c = fz * dz;
+      atomicAdd(&jz[base], c * (1.f - my));
+      atomicAdd(&jz[base + 1], c * my);
+    }
+  }
+}
+
+template <bool D3>
+__global__ void __launch_bounds__(PUSH_THREADS, 3)
+k_push1(GridDesc gd, Cols p, const int *__restrict__ cell_offsets, const float *__restrict__ E,
+        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
+  extern __shared__ float smem[];
+  TileGeom<D3> tg;
+  tg.init(gd, blockIdx.x);
+  float *sF = smem;                // [6][fvol]: Ex Ey Ez Bx By Bz
+  float *sJ = smem + 6 * tg.fvol;  // [3][jvol]
+
+  for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
+    const int c = i / tg.fvol, r = i - c * tg.fvol;
+    const int lx = r % tg.fe[0], t = r / tg.fe[0];
+    const int ly = t % tg.fe[1], lz = t / tg.fe[1];
+    const int gx = D3 ? tg.o[0] + lx - 1 + gd.g[0] : 0;
+    const int gy = tg.o[1] + ly - 1 + gd.g[1], gz = tg.o[2] + lz - 1 + gd.g[2];
+    const int gi = (gz * gd.ext[1] + gy) * gd.ext[0] + gx;
+    sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
+  }
+  for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
+  __syncthreads();
+
+  const int p0 = cell_offsets[blockIdx.x * gd.cpb], p1 = cell_offsets[(blockIdx.x + 1) * gd.cpb];
+  const float *sEx = sF, *sEy = sF + tg.fvol, *sEz = sF + 2 * tg.fvol;
+  const float *sBx = sF + 3 * tg.fvol, *sBy = sF + 4 * tg.fvol, *sBz = sF + 5 * tg.fvol;
+  uint32_t bad = 0;
+
+  for (int a = p0 + threadIdx.x; a < p1; a += blockDim.x) {
+    float x = 0.f, ax = 0.f;
+    int lx = 0;
+    const float y = ld_stream(p.y + a), z = ld_stream(p.z + a);
+    float ux = ld_stream(p.ux + a), uy = ld_stream(p.uy + a), uz = ld_stream(p.uz + a);
+    const float qw = ld_stream(p.qw + a);
+    const int sp = ld_stream(p.sp + a);
+    if (D3) x = ld_stream(p.x + a);
+
+    // cell and in-cell offsets (same fp32 product + floor as the sort)
+    const float yi = __fmul_rn(y, gd.inv_dx[1]), zi = __fmul_rn(z, gd.inv_dx[2]);
+    const float cyf = floorf(yi), czf = floorf(zi);
+    const float ay = yi - cyf, az = zi - czf;
+    int ly = (int)cyf - tg.o[1], lz = (int)czf - tg.o[2];
+    bool in_tile = ly >= 0 && ly < gd.bs[1] && lz >= 0 && lz < gd.bs[2];
+    if (D3) {
+      const float xi = __fmul_rn(x, gd.inv_dx[0]);
+      const float cxf = floorf(xi);
+      ax = xi - cxf;
+      lx = (int)cxf - tg.o[0];
+      in_tile = in_tile && lx >= 0 && lx < gd.bs[0];
+    }
+    if (!in_tile) {  // not the sorted list this kernel was promised: flag, leave untouched
+      bad |= PSC_F_NOT_IN_TILE;
+      continue;
+    }
+
+    // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) ----------
+    Stencil1 sx, sy, sz;
+    sx.set(lx, ax);
+    sy.set(ly, ay);
+    sz.set(lz, az);
+    const float ex = gather1<D3, true, false, false>(sEx, tg, sx, sy, sz);
+    const float ey = gather1<D3, false, true, false>(sEy, tg, sx, sy, sz);
+    const float ez = gather1<D3, false, false, true>(sEz, tg, sx, sy, sz);
+    const float bx = gather1<D3, false, true, true>(sBx, tg, sx, sy, sz);
+    const float by = gather1<D3, true, false, true>(sBy, tg, sx, sy, sz);
+    const float bz = gather1<D3, true, true, false>(sBz, tg, sx, sy, sz);
+
+    // ---- Boris (Eq. 27-28) and move (Eq. 26) ------------------------------------------------
+    boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, gd.qmh[sp]);
+    const float ig = rsqrtf(1.0f + ux * ux + uy * uy + uz * uz);
+    const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
+    const float ddx = D3 ? vx * gd.dt_dx[0] : 0.f;  // displacement in cells
+    const float ddy = vy * gd.dt_dx[1], ddz = vz * gd.dt_dx[2];
+
+    // ---- Villasenor-Buneman deposit -----------------------------------------------------------
+    {
+      const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
+      const float qvx = qw * gd.inv_dV * vx;
+      const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
+      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      float tx = sxd ? ((sxd > 0 ? 1.f - ax : -ax) / ddx) : 2.f;
+      float ty = syd ? ((syd > 0 ? 1.f - ay : -ay) / ddy) : 2.f;
+      float tz = szd ? ((szd > 0 ? 1.f - az : -az) / ddz) : 2.f;
+      float px = ax, py = ay, pz = az;  // segment start, in origin-cell coordinates
+      int rx = 0, ry = 0, rz = 0;       // current cell relative to the origin cell
+      float tprev = 0.f;
+#pragma unroll 1
+      for (int seg = 0; seg < (D3 ? 4 : 3); seg++) {
+        const float t = fminf(fminf(tx, ty), fminf(tz, 1.f));
+        const int which = (t >= 1.f) ? 3 : (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
+        float qx = ax + t * ddx, qy = ay + t * ddy, qz = az + t * ddz;  // segment end
+        if (which == 3) {
+          qx = endx; qy = endy; qz = endz;
+        } else if (which == 0) {
+          qx = sxd > 0 ? (float)(rx + 1) : (float)rx;
+        } else if (which == 1) {
+          qy = syd > 0 ? (float)(ry + 1) : (float)ry;
+        } else {
+          qz = szd > 0 ? (float)(rz + 1) : (float)rz;
+        }
+        vb_segment<D3>(sJ, tg, lx + rx, ly + ry, lz + rz, px - rx, py - ry, pz - rz, qx - rx,
+                       qy - ry, qz - rz, t - tprev, fx, fy, fz, qvx);
+        if (which == 3) break;
+        if (which == 0) { rx += sxd; tx = 2.f; }
+        else if (which == 1) { ry += syd; ty = 2.f; }
+        else { rz += szd; tz = 2.f; }
+        px = qx; py = qy; pz = qz;
+        tprev = t;
+      }
+    }
+
+    // ---- store; periodic wrap is the single-GPU particle exchange -----------
+    const float y1 = wrap_periodic(fmaf(gd.dt, vy, y), gd.L[1]);
+    const float z1 = wrap_periodic(fmaf(gd.dt, vz, z), gd.L[2]);
+    if (D3) {
+      const float x1 = wrap_periodic(fmaf(gd.dt, vx, x), gd.L[0]);
+      st_stream(p.x + a, x1);
+      if (!(fabsf(x1) <= gd.L[0])) bad |= PSC_F_NAN;
+    }
+    st_stream(p.y + a, y1);
+    st_stream(p.z + a, z1);
+    st_stream(p.ux + a, ux);
+    st_stream(p.uy + a, uy);
+    st_stream(p.uz + a, uz);
+    if (!(fabsf(y1) <= gd.L[1]) || !(fabsf(z1) <= gd.L[2]) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
+      bad |= PSC_F_NAN;
+  }
+  if (bad) atomicOr(flags, bad);
+  __syncthreads();
+
+  // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
+  for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) {
+    const float v = sJ[i];
+    if (v == 0.f) continue;
+    const int c = i / tg.jvol, r = i - c * tg.jvol;
+    const int lx = r % tg.je[0], t = r / tg.je[0];
+    const int ly = t % tg.je[1], lz = t / tg.je[1];
+    const int gx = D3 ? tg.o[0] + lx - 1 + gd.g[0] : 0;
+    const int gy = tg.o[1] + ly - 1 + gd.g[1], gz = tg.o[2] + lz - 1 + gd.g[2];
+    atomicAdd(&J[c * gd.comp + (gz * gd.ext[1] + gy) * gd.ext[0] + gx], v);
+  }
+}
+
+}  // namespace
+
+int psc_push_order1(psc_ctx *c, cudaStream_t s) {
+  const GridDesc &gd = c->gd;
+  const bool d3 = gd.n[0] > 1 && gd.n[1] > 1 && gd.n[2] > 1;
+  const bool d2yz = gd.n[0] == 1 && gd.n[1] > 1 && gd.n[2] > 1;
+  if (!d3 && !d2yz) return PSC_ERR_UNSUPPORTED;  // 2-d runs are yz-plane runs
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
+  c->launches++;
+  if (c->np == 0) return PSC_OK;
+  int fvol = 1, jvol = 1;
+  for (int d = 0; d < 3; d++)
+    if (gd.n[d] > 1) {
+      fvol *= gd.bs[d] + 2;
+      jvol *= gd.bs[d] + 3;
+    }
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol) * sizeof(float);
+  if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  const Cols &p = c->cols[c->cur];
+  const int threads = c->opt_threads > 0 ? c->opt_threads : PUSH_THREADS;
+  if (d3) {
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+  } else {
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+  }
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}

@@ -1,0 +1,397 @@
+// sort.cu -- cell-key counting sort of the particle list.
+//
+// One key orders by block ("supercell") and by cell inside the block at once:
+//   key = block_index * cells_per_block + cell_in_block.
+// A counting sort is O(N + M).  The B200 form:
+//   1. k_keys     key + natural cell index per particle, histogram over keys with
+//                 warp-aggregated atomics (lanes holding the same key elect one lane that adds
+//                 the group's size; on a cell-ordered list a warp issues 1-2 atomics, not 32);
+//   2. scan       exclusive prefix sum of the histogram -> cell_offsets (three small kernels);
+//   3. k_scatter  slot = cursor[key] + rank, again warp-aggregated; writes the permutation;
+//   4. k_segsort  the atomics hand out slots in arbitrary order ACROSS warps, so every key's
+//                 segment of `perm` is sorted ascending (bitonic network, in registers / shared
+//                 memory; segments are ~ particles-per-cell long).  A set of distinct input
+//                 indices in ascending order IS the stable order, hence the result is the
+//                 unique stable counting sort, bit-exact against any stable reference;
+//   5. k_reorder  out[s] = in[perm[s]] for every column (coalesced writes; the reads are nearly
+//                 coalesced when the list is a previous sort's output advanced by one push,
+//                 because a particle moves at most one cell per step).
+#include <limits.h>
+
+#include "psc_internal.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;                         // per thread
+constexpr int SCAN_TILE = SORT_THREADS * SCAN_ITEMS;  // 2048 keys per block
+constexpr int WARP_SEG_CAP = 1024;                    // ints of shared memory per warp in k_segsort
+constexpr int BIG_SMEM_CAP = 48 * 1024;               // ints; larger segments are sorted in global
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict__ y,
+       const float *__restrict__ z, int *__restrict__ key, int *__restrict__ cell_idx,
+       int *__restrict__ hist, uint32_t *__restrict__ flags) {
+  const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int stride = gridDim.x * blockDim.x;
+  const int nround = ((n + 31) / 32) * 32;
+  for (int a = a0; a < nround; a += stride) {
+    const bool valid = a < n;
+    int k = -1 - (int)(threadIdx.x & 31);  // distinct per lane: no grouping of invalid lanes
+    if (valid) {
+      int c[3];
+      const float *pos[3] = {x, y, z};
+      bool oob = false;
+#pragma unroll
+      for (int d = 0; d < 3; d++) {
+        if (gd.n[d] == 1) {
+          c[d] = 0;
+          continue;
+        }
+        const float xi = __fmul_rn(pos[d][a], gd.inv_dx[d]);  // one fp32 rounding, then floor
+        int ci = (int)floorf(xi);
+        if (!(ci >= 0 && ci < gd.n[d])) {  // also catches NaN
+          oob = true;
+          ci = ci < 0 ? 0 : gd.n[d] - 1;
+          if (xi != xi) ci = 0;
+        }
+        c[d] = ci;
+      }
+      if (oob) atomicOr(flags, PSC_F_OOB);
+      const int b0 = c[0] / gd.bs[0], b1 = c[1] / gd.bs[1], b2 = c[2] / gd.bs[2];
+      const int l0 = c[0] - b0 * gd.bs[0], l1 = c[1] - b1 * gd.bs[1], l2 = c[2] - b2 * gd.bs[2];
+      k = ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
+      key[a] = k;
+      cell_idx[a] = (c[2] * gd.n[1] + c[1]) * gd.n[0] + c[0];
+    }
+    const unsigned grp = __match_any_sync(0xffffffffu, k);
+    if (valid && (grp & lanemask_lt()) == 0) atomicAdd(&hist[k], __popc(grp));
+  }
+}
+
+// ---- exclusive scan of hist[0..m) -> out[0..m], out[m] = total; also cursor := out -----------
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_scan_local(int m, const int *__restrict__ in, int *__restrict__ out, int *__restrict__ tmp) {
+  __shared__ int wsum[SORT_THREADS / 32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  int v[SCAN_ITEMS];
+  int s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    v[i] = (base + i < m) ? in[base + i] : 0;
+    s += v[i];
+  }
+  // inclusive scan of s across the block
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int inc = s;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) wsum[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    int t = lane < SORT_THREADS / 32 ? wsum[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(0xffffffffu, t, o);
+      if (lane >= o) t += u;
+    }
+    if (lane < SORT_THREADS / 32) wsum[lane] = t;
+  }
+  __syncthreads();
+  int run = inc - s + (w ? wsum[w - 1] : 0);
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    if (base + i < m) out[base + i] = run;
+    run += v[i];
+  }
+  if (threadIdx.x == SORT_THREADS - 1) tmp[blockIdx.x] = run;
+}
+
+// single block: exclusive scan of tmp[0..nb) in place, tmp[nb] = total
+__global__ void __launch_bounds__(1024) k_scan_tmp(int nb, int *__restrict__ tmp) {
+  __shared__ int wsum[32];
+  __shared__ int carry_s;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int base = 0; base < nb; base += 1024) {
+    const int i = base + threadIdx.x;
+    const int v = i < nb ? tmp[i] : 0;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+      int t = wsum[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(0xffffffffu, t, o);
+        if (lane >= o) t += u;
+      }
+      wsum[lane] = t;
+    }
+    __syncthreads();
+    const int carry = carry_s;
+    const int exc = carry + inc - v + (w ? wsum[w - 1] : 0);
+    if (i < nb) tmp[i] = exc;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry_s = exc + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) tmp[nb] = carry_s;
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_scan_add(int m, int *__restrict__ out, int *__restrict__ cursor, const int *__restrict__ tmp,
+           int nb) {
+  const int add = tmp[blockIdx.x];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++)
+    if (base + i < m) {
+      const int v = out[base + i] + add;
+      out[base + i] = v;
+      cursor[base + i] = v;
+    }
+  if (blockIdx.x == 0 && threadIdx.x == 0) out[m] = tmp[nb];
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_scatter(int n, const int *__restrict__ key, int *__restrict__ cursor, int *__restrict__ perm) {
+  const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int stride = gridDim.x * blockDim.x;
+  const int nround = ((n + 31) / 32) * 32;
+  const int lane = threadIdx.x & 31;
+  for (int a = a0; a < nround; a += stride) {
+    const bool valid = a < n;
+    const int k = valid ? key[a] : -1 - lane;
+    const unsigned grp = __match_any_sync(0xffffffffu, k);
+    const int leader = __ffs(grp) - 1;
+    int base = 0;
+    if (valid && lane == leader) base = atomicAdd(&cursor[k], __popc(grp));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (valid) perm[base + __popc(grp & lanemask_lt())] = a;
+  }
+}
+
+// ---- ascending sort of every key's segment of perm ------------------------------------------
+
+// All-ascending bitonic network ("mirror" first sub-stage): with it, virtual +inf padding past
+// n never moves, so pairs whose upper index is >= n are simply skipped.
+template <typename Sync>
+__device__ __forceinline__ void bitonic_any(int *a, int n, int tid, int nthreads, Sync sync) {
+  int P = 1;
+  while (P < n) P <<= 1;
+  for (int k = 2; k <= P; k <<= 1) {
+    const int hk = k >> 1;
+    for (int i = tid; i < (P >> 1); i += nthreads) {
+      const int blk = i / hk, w = i - blk * hk;
+      const int lo = blk * k + w, hi = blk * k + k - 1 - w;
+      if (hi < n) {
+        const int u = a[lo], v = a[hi];
+        if (u > v) {
+          a[lo] = v;
+          a[hi] = u;
+        }
+      }
+    }
+    sync();
+    for (int j = hk >> 1; j >= 1; j >>= 1) {
+      for (int i = tid; i < (P >> 1); i += nthreads) {
+        const int lo = 2 * j * (i / j) + (i % j), hi = lo + j;
+        if (hi < n) {
+          const int u = a[lo], v = a[hi];
+          if (u > v) {
+            a[lo] = v;
+            a[hi] = u;
+          }
+        }
+      }
+      sync();
+    }
+  }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_segsort(int nkeys, const int *__restrict__ offs, int *__restrict__ perm,
+          int *__restrict__ big_list, uint32_t *__restrict__ big_count) {
+  __shared__ int buf[SORT_THREADS / 32][WARP_SEG_CAP];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int warps = gridDim.x * (SORT_THREADS / 32);
+  for (int k = blockIdx.x * (SORT_THREADS / 32) + w; k < nkeys; k += warps) {
+    const int lo = offs[k], n = offs[k + 1] - lo;
+    if (n <= 1) continue;
+    if (n <= 32) {
+      int v = lane < n ? perm[lo + lane] : INT_MAX;
+      // already ascending?
+      const int nx = __shfl_down_sync(0xffffffffu, v, 1);
+      if (__ballot_sync(0xffffffffu, lane < 31 && v > nx) == 0) continue;
+#pragma unroll
+      for (int kk = 2; kk <= 32; kk <<= 1) {
+        {  // mirror sub-stage: partner = mirror image inside the block of kk lanes
+          const int p = __shfl_xor_sync(0xffffffffu, v, kk - 1);
+          v = (lane ^ (kk - 1)) > lane ? min(v, p) : max(v, p);
+        }
+#pragma unroll
+        for (int j = kk >> 2; j >= 1; j >>= 1) {
+          const int p = __shfl_xor_sync(0xffffffffu, v, j);
+          v = (lane & j) == 0 ? min(v, p) : max(v, p);
+        }
+      }
+      if (lane < n) perm[lo + lane] = v;
+      continue;
+    }
+    if (n > WARP_SEG_CAP) {
+      if (lane == 0) big_list[atomicAdd(big_count, 1u)] = k;
+      continue;
+    }
+    int *b = buf[w];
+    bool sorted = true;
+    for (int i = lane; i < n; i += 32) b[i] = perm[lo + i];
+    __syncwarp();
+    for (int i = lane; i < n - 1; i += 32) sorted = sorted && (b[i] <= b[i + 1]);
+    if (__all_sync(0xffffffffu, sorted)) continue;
+    bitonic_any(b, n, lane, 32, [] { __syncwarp(); });
+    for (int i = lane; i < n; i += 32) perm[lo + i] = b[i];
+    __syncwarp();
+  }
+}
+
+// segments longer than WARP_SEG_CAP: one block each (shared memory if it fits, else in place in
+// global memory -- slow, only for pathological densities)
+__global__ void __launch_bounds__(1024)
+k_segsort_big(const int *__restrict__ offs, int *__restrict__ perm,
+              const int *__restrict__ big_list, const uint32_t *__restrict__ big_count) {
+  extern __shared__ int sbuf[];
+  const int nbig = (int)*big_count;
+  for (int e = blockIdx.x; e < nbig; e += gridDim.x) {
+    const int k = big_list[e];
+    const int lo = offs[k], n = offs[k + 1] - lo;
+    if (n <= BIG_SMEM_CAP) {
+      for (int i = threadIdx.x; i < n; i += blockDim.x) sbuf[i] = perm[lo + i];
+      __syncthreads();
+      bitonic_any(sbuf, n, threadIdx.x, blockDim.x, [] { __syncthreads(); });
+      for (int i = threadIdx.x; i < n; i += blockDim.x) perm[lo + i] = sbuf[i];
+      __syncthreads();
+    } else {
+      bitonic_any(perm + lo, n, threadIdx.x, blockDim.x, [] { __syncthreads(); });
+    }
+  }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_reorder(int n, const int *__restrict__ perm, Cols in, Cols out) {
+  const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int stride = gridDim.x * blockDim.x;
+  for (int s = s0; s < n; s += stride) {
+    const int p = perm[s];
+    const float x = in.x[p], y = in.y[p], z = in.z[p];
+    const float ux = in.ux[p], uy = in.uy[p], uz = in.uz[p];
+    const float qw = in.qw[p];
+    const int sp = in.sp[p];
+    int id = 0;
+    if (in.id) id = in.id[p];
+    out.x[s] = x;
+    out.y[s] = y;
+    out.z[s] = z;
+    out.ux[s] = ux;
+    out.uy[s] = uy;
+    out.uz[s] = uz;
+    out.qw[s] = qw;
+    out.sp[s] = sp;
+    if (in.id) out.id[s] = id;
+  }
+}
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
+  const size_t nk = (size_t)c->gd.nkeys;
+  size_t b = 0;
+  b += 3 * align_up((size_t)n * 4, 256);                      // key, perm, cell_idx
+  b += 2 * align_up((nk + 1) * 4, 256);                       // cell_offsets, cursor
+  b += align_up((nk / SCAN_TILE + 3) * 4, 256);               // scan_tmp
+  b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
+  return b;
+}
+
+int psc_sort_carve(psc_ctx *c, int64_t n) {
+  const size_t nk = (size_t)c->gd.nkeys;
+  char *p = (char *)c->ws;
+  auto take = [&](size_t bytes) {
+    void *r = p;
+    p += align_up(bytes, 256);
+    return r;
+  };
+  c->key = (int32_t *)take((size_t)n * 4);
+  c->perm = (int32_t *)take((size_t)n * 4);
+  c->cell_idx = (int32_t *)take((size_t)n * 4);
+  c->cell_offsets = (int32_t *)take((nk + 1) * 4);
+  c->cursor = (int32_t *)take((nk + 1) * 4);
+  c->scan_tmp = (int32_t *)take((nk / SCAN_TILE + 3) * 4);
+  c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
+  if ((size_t)(p - (char *)c->ws) > c->ws_bytes) return PSC_ERR_WORKSPACE;
+  return PSC_OK;
+}
+
+int psc_sort_run(psc_ctx *c, cudaStream_t s) {
+  const GridDesc &gd = c->gd;
+  const int n = (int)c->np;
+  const int nk = gd.nkeys;
+  const Cols &in = c->cols[c->cur];
+  const Cols &out = c->cols[c->cur ^ 1];
+  const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
+
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
+  c->launches += 2;
+  k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, c->key, c->cell_idx, c->cursor,
+                                          c->d_flags);
+  PSC_LAUNCH_CHECK(c);
+  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
+  k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, c->cell_offsets, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_tmp<<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->cursor, c->scan_tmp, sblocks);
+  PSC_LAUNCH_CHECK(c);
+  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, c->key, c->cursor, c->perm);
+  PSC_LAUNCH_CHECK(c);
+  const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
+  k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->perm, c->big_list,
+                                            c->d_flags + 1);
+  PSC_LAUNCH_CHECK(c);
+  if (n > WARP_SEG_CAP) {
+    static bool attr_set = false;
+    if (!attr_set) {
+      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_segsort_big, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           BIG_SMEM_CAP * 4));
+      attr_set = true;
+    }
+    k_segsort_big<<<c->sm_count, 1024, BIG_SMEM_CAP * 4, s>>>(c->cell_offsets, c->perm, c->big_list,
+                                                              c->d_flags + 1);
+    PSC_LAUNCH_CHECK(c);
+  }
+  k_reorder<<<pblocks, SORT_THREADS, 0, s>>>(n, c->perm, in, out);
+  PSC_LAUNCH_CHECK(c);
+  c->cur ^= 1;
+  c->state = PSC_STATE_SORTED;
+  c->have_sort_result = 1;
+  return PSC_OK;
+}

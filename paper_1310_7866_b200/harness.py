@@ -1,0 +1,71 @@
+"""Device-buffer plumbing around the binding: allocates the PyTorch tensors the library borrows
+(two particle column sets, ghosted E/B/J, workspace) from a seeded synthetic plasma
+(psc_inputs.Plasma) and maps the library's raw pointers back to tensors.  Layout only -- no
+arithmetic of the method lives here."""
+from __future__ import annotations
+
+import torch
+
+from . import COLUMNS, PSC_B, PSC_E, PSC_GHOST, Psc
+
+
+class Simulation:
+    def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True):
+        self.device = torch.device(device)
+        self.plasma = plasma
+        self.psc = Psc(plasma.n, plasma.dx, plasma.dt, plasma.order, plasma.q, plasma.m, block)
+        self.n = tuple(plasma.n)
+        self.g = tuple(PSC_GHOST if v > 1 else 0 for v in self.n)
+        self.np = plasma.n_particles
+        dev = self.device
+        shp = self.psc.field_shape
+        self.E = torch.zeros(shp, dtype=torch.float32, device=dev)
+        self.B = torch.zeros(shp, dtype=torch.float32, device=dev)
+        self.J = torch.zeros(shp, dtype=torch.float32, device=dev)
+        self.interior(self.E).copy_(plasma.E.to(dev))
+        self.interior(self.B).copy_(plasma.B.to(dev))
+        self.sets = []
+        for k in range(2):
+            s = {}
+            for c in COLUMNS:
+                if c == "id" and not with_id:
+                    s[c] = None
+                    continue
+                dt = torch.int32 if c in ("species", "id") else torch.float32
+                s[c] = torch.empty(max(self.np, 1), dtype=dt, device=dev)
+            self.sets.append(s)
+        for c in COLUMNS:
+            if self.sets[0][c] is not None and self.np:
+                self.sets[0][c][: self.np].copy_(getattr(plasma, c).to(dev))
+        self.ws = torch.empty(self.psc.workspace_bytes(self.np), dtype=torch.uint8, device=dev)
+        self.psc.bind_workspace(self.ws)
+        self.psc.bind_fields(self.E, self.B, self.J)
+        self.psc.bind_particles(self.np, self.sets[0], self.sets[1])
+        self.psc.fill_ghosts(PSC_E)
+        self.psc.fill_ghosts(PSC_B)
+
+    def interior(self, F):
+        g, n = self.g, self.n
+        return F[:, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]]
+
+    def current(self):
+        """the column set (dict of tensors, trimmed to n particles) that holds the particles now"""
+        ptr = self.psc.particles_current()["x"]
+        s = self.sets[0] if self.sets[0]["x"].data_ptr() == ptr else self.sets[1]
+        assert s["x"].data_ptr() == ptr
+        return {c: (None if t is None else t[: self.np]) for c, t in s.items()}
+
+    def sort_result(self):
+        """(cell_idx[n], perm[n], cell_offsets[n_keys+1]) as int32 tensors viewing the workspace"""
+        ci, pm, co, nk = self.psc.sort_result()
+        base = self.ws.data_ptr()
+
+        def view(ptr, count):
+            off = ptr - base
+            return self.ws[off: off + 4 * count].view(torch.int32)
+
+        return view(ci, self.np), view(pm, self.np), view(co, nk + 1)
+
+    def step(self, nsteps=1):
+        for _ in range(nsteps):
+            self.psc.step()

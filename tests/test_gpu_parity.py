@@ -1,0 +1,271 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json's north_star: sort results bit-exact;
+positions, momenta within 1e-5 relative; J and fields within 1e-5 of the component max-norm;
+continuity residual at fp32 rounding level (<= 1e-5 relative)."""
+import numpy as np
+import pytest
+import torch
+
+import psc_inputs
+from tests.util import (gpu_cols, library_block, oracle_for, oracle_sorted_state, oracle_state,
+                        periodic_dist, rel_maxnorm, smooth_fields)
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+def _sim(pl, block=(0, 0, 0)):
+    from paper_1310_7866_b200.harness import Simulation
+
+    return Simulation(pl, block=block)
+
+
+def _small(kind):
+    if kind == "2d":
+        return psc_inputs.make_config(1)                        # 1x64x64, 32/cell: config 1 itself
+    if kind == "2d-ragged":
+        return psc_inputs.thermal((1, 24, 40), 7, seed=11, name="ragged2d")
+    if kind == "3d":
+        return psc_inputs.make_config(4, scale=(16, 16, 16))    # 50+50 per cell
+    if kind == "3d-ragged":
+        return psc_inputs.thermal((12, 20, 8), 5, seed=12, name="ragged3d")
+    if kind == "harris":
+        return psc_inputs.make_config(3, scale=(1, 32, 128))
+    raise ValueError(kind)
+
+
+# ------------------------------------------------------------------------------------------------
+# fields
+
+@pytest.mark.parametrize("n", [(1, 24, 40), (12, 20, 8), (1, 64, 64)])
+def test_fdtd_matches_oracle(n):
+    pl = psc_inputs.thermal(n, 1, seed=3)
+    smooth_fields(pl, 0.3, seed=5)
+    sim = _sim(pl)
+    orc = oracle_for(pl)
+    _, E, B = oracle_state(pl)
+    rng = np.random.default_rng(9)
+    Jn = rng.normal(size=E.shape)
+    sim.interior(sim.J).copy_(torch.from_numpy(Jn.astype(np.float32)).cuda())
+    Jn = Jn.astype(np.float32).astype(np.float64)
+    sim.psc.fill_ghosts(2)
+    for _ in range(5):
+        sim.psc.push_fields(1, 0.5)
+        sim.psc.push_fields(1, 0.5)
+        sim.psc.push_fields(0, 1.0)
+        orc.push_b(E, B, 0.5)
+        orc.push_b(E, B, 0.5)
+        orc.push_e(E, B, Jn, 1.0)
+    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
+    assert rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B) < TOL
+    # ghost points are bit-identical periodic images of the interior
+    for F in (sim.E, sim.B):
+        G = F.clone()
+        sim.psc.bind_fields(G, sim.B, sim.J)
+        sim.psc.fill_ghosts(0)
+        sim.psc.bind_fields(sim.E, sim.B, sim.J)
+        assert torch.equal(G, F)
+
+
+@pytest.mark.parametrize("n", [(1, 8, 12), (4, 8, 12), (1, 4, 4)])
+def test_exchange_j_folds_ghosts(n):
+    """add_and_fill_ghosts_j: interior += all periodic ghost images, ghosts := images"""
+    pl = psc_inputs.thermal(n, 1, seed=3)
+    sim = _sim(pl)
+    rng = np.random.default_rng(1)
+    full = rng.integers(-8, 9, size=sim.psc.field_shape).astype(np.float32)  # exact in fp32
+    sim.J.copy_(torch.from_numpy(full).cuda())
+    sim.psc.exchange_j()
+    got = sim.J.cpu().numpy()
+    g = sim.g
+    want = np.zeros((3, n[2], n[1], n[0]))
+    ez, ey, ex = full.shape[1:]
+    for k in range(ez):
+        for j in range(ey):
+            for i in range(ex):
+                want[:, (k - g[2]) % n[2], (j - g[1]) % n[1], (i - g[0]) % n[0]] += full[:, k, j, i]
+    assert np.array_equal(sim.interior(sim.J).cpu().numpy().astype(np.float64), want)
+    for k in range(ez):
+        for j in range(ey):
+            for i in range(ex):
+                assert np.array_equal(got[:, k, j, i],
+                                      want[:, (k - g[2]) % n[2], (j - g[1]) % n[1], (i - g[0]) % n[0]])
+
+
+# ------------------------------------------------------------------------------------------------
+# sort
+
+@pytest.mark.parametrize("kind,block", [("2d", (0, 0, 0)), ("2d-ragged", (1, 4, 8)),
+                                        ("3d", (0, 0, 0)), ("3d-ragged", (2, 4, 2)),
+                                        ("harris", (1, 8, 8))])
+def test_sort_bit_exact(kind, block):
+    pl = _small(kind).shuffled()
+    sim = _sim(pl, block=block)
+    orc = oracle_for(pl, block=library_block(pl.n, block))
+    before = {k: getattr(pl, k).numpy().copy() for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id")}
+    cell_idx, key, perm, offs = orc.sort(before["x"], before["y"], before["z"])
+    sim.psc.particles_sort()
+    assert sim.psc.status() == 0
+    g_ci, g_pm, g_co = (t.cpu().numpy() for t in sim.sort_result())
+    assert np.array_equal(g_ci, cell_idx)
+    assert np.array_equal(g_co, offs)
+    assert np.array_equal(g_pm, perm)
+    after = gpu_cols(sim)
+    for k, v in before.items():
+        assert np.array_equal(after[k], v[perm]), k
+
+
+def test_sort_degenerate_cases():
+    # empty list
+    pl = psc_inputs.thermal((1, 8, 8), 1, seed=3)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id"):
+        setattr(pl, k, getattr(pl, k)[:0])
+    sim = _sim(pl)
+    sim.psc.particles_sort()
+    sim.psc.push_particles()
+    assert sim.psc.status() == 0
+    assert int(sim.sort_result()[2].abs().max()) == 0
+    # everything in very few cells: segments of ~3000 (shared-memory block sort) and ~70000
+    # (in-place global sort) particles
+    for count in (3000, 70000):
+        pl = psc_inputs.thermal((1, 8, 8), 1, seed=3)
+        g = torch.Generator().manual_seed(5)
+        n = count
+        pl.y = (torch.rand(n, generator=g) * 0.999 + 3.0).float()
+        pl.z = (torch.rand(n, generator=g) * 0.999 + (torch.rand(n, generator=g) < 0.9).float() * 2.0).float()
+        pl.x = torch.full((n,), 0.5)
+        pl.ux = torch.zeros(n); pl.uy = torch.zeros(n); pl.uz = torch.zeros(n)
+        pl.qw = torch.ones(n); pl.species = torch.zeros(n, dtype=torch.int32)
+        pl.id = torch.arange(n, dtype=torch.int32)
+        sim = _sim(pl, block=(1, 4, 4))
+        orc = oracle_for(pl, block=(1, 4, 4))
+        ci, key, perm, offs = orc.sort(pl.x.numpy(), pl.y.numpy(), pl.z.numpy())
+        sim.psc.particles_sort()
+        g_ci, g_pm, g_co = (t.cpu().numpy() for t in sim.sort_result())
+        assert np.array_equal(g_co, offs) and np.array_equal(g_pm, perm) and np.array_equal(g_ci, ci)
+
+
+def test_sort_flags_out_of_domain():
+    pl = psc_inputs.thermal((1, 8, 8), 2, seed=3)
+    pl.y[5] = 8.0
+    sim = _sim(pl)
+    sim.psc.particles_sort()
+    assert sim.psc.status() & 1
+
+
+# ------------------------------------------------------------------------------------------------
+# particle loop, open loop: same sorted state in, one psc_push_particles, compare
+
+def _push_once(kind, block, amp=0.05):
+    pl = _small(kind)
+    smooth_fields(pl, amp, seed=21)
+    sim = _sim(pl, block=block)
+    sim.psc.particles_sort()
+    cols0 = oracle_sorted_state(pl, block)        # the sorted fp32 input both paths see
+    mine = gpu_cols(sim)
+    for k, v in cols0.items():
+        assert np.array_equal(mine[k], v), k
+    orc = oracle_for(pl)
+    _, E, B = oracle_state(pl)
+    st = {k: np.ascontiguousarray(cols0[k].astype(np.float64)) for k in ("x", "y", "z", "ux", "uy", "uz", "qw")}
+    sp = np.ascontiguousarray(cols0["species"])
+    J = orc.zeros_field()
+    orc.push_particles(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], sp)
+    sim.psc.push_particles()
+    sim.psc.exchange_j()
+    assert sim.psc.status() == 0
+    return pl, sim, orc, cols0, st, sp, J
+
+
+@pytest.mark.parametrize("kind,block", [("2d", (0, 0, 0)), ("2d-ragged", (1, 4, 8)),
+                                        ("2d-ragged", (1, 24, 40)), ("3d", (0, 0, 0)),
+                                        ("3d-ragged", (2, 4, 2)), ("3d-ragged", (1, 1, 1)),
+                                        ("harris", (1, 8, 8))])
+def test_push_particles_matches_oracle(kind, block):
+    pl, sim, orc, cols0, st, sp, J = _push_once(kind, block)
+    got = gpu_cols(sim)
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for d, c in enumerate(("x", "y", "z")):
+        if pl.n[d] == 1:
+            assert np.array_equal(got[c], cols0[c])        # invariant coordinate is carried
+            continue
+        assert (periodic_dist(got[c], st[c], L[d]) / L[d]).max() < TOL
+        assert periodic_dist(got[c], st[c], L[d]).max() < 1e-4 * pl.dx[d]
+        assert got[c].min() >= 0.0 and got[c].max() < L[d]
+    for s in range(len(pl.q)):
+        m = sp == s
+        rms = np.sqrt(np.mean(st["ux"][m] ** 2 + st["uy"][m] ** 2 + st["uz"][m] ** 2))
+        for c in ("ux", "uy", "uz"):
+            assert np.abs(got[c][m] - st[c][m]).max() / rms < TOL
+    assert np.array_equal(got["qw"], cols0["qw"]) and np.array_equal(got["species"], cols0["species"])
+    assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+
+
+@pytest.mark.parametrize("kind", ["2d", "3d"])
+def test_gpu_continuity_residual(kind):
+    """(rho^{n+3/2} - rho^{n+1/2})/dt + div- j^{n+1} = 0 (Eq. 25) with the GPU's J and the GPU's
+    stored fp32 positions, evaluated by the oracle's rho / div-; normalised by max|rho_s|/dt of one
+    species."""
+    pl, sim, orc, cols0, st, sp, J = _push_once(kind, (0, 0, 0), amp=0.05)
+    got = gpu_cols(sim)
+    f64 = lambda a: np.ascontiguousarray(a.astype(np.float64))
+    rho0 = orc.rho(f64(cols0["x"]), f64(cols0["y"]), f64(cols0["z"]), f64(cols0["qw"]))
+    rho1 = orc.rho(f64(got["x"]), f64(got["y"]), f64(got["z"]), f64(got["qw"]))
+    Jg = np.ascontiguousarray(sim.interior(sim.J).cpu().numpy().astype(np.float64))
+    res = (rho1 - rho0) / pl.dt + orc.div_minus(Jg)
+    m = sp == 0
+    rho_s = orc.rho(f64(cols0["x"][m]), f64(cols0["y"][m]), f64(cols0["z"][m]), f64(cols0["qw"][m]))
+    assert np.abs(res).max() / (np.abs(rho_s).max() / pl.dt) < TOL
+
+
+# ------------------------------------------------------------------------------------------------
+# closed loop: 10 psc_step, particles matched by id
+
+@pytest.mark.parametrize("kind", ["2d", "3d", "harris"])
+def test_ten_steps_match_oracle(kind):
+    pl = _small(kind)
+    sim = _sim(pl)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    nsteps = 10
+    orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], nsteps)
+    sim.step(nsteps)
+    assert sim.psc.status() == 0
+    got = gpu_cols(sim)
+    order = np.argsort(got["id"], kind="stable")
+    assert np.array_equal(got["id"][order], st["id"])
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for d, c in enumerate(("x", "y", "z")):
+        if pl.n[d] > 1:
+            assert (periodic_dist(got[c][order], st[c], L[d]) / L[d]).max() < TOL
+    for s in range(len(pl.q)):
+        m = st["species"] == s
+        rms = np.sqrt(np.mean(st["ux"][m] ** 2 + st["uy"][m] ** 2 + st["uz"][m] ** 2))
+        for c in ("ux", "uy", "uz"):
+            assert np.abs(got[c][order][m] - st[c][m]).max() / rms < TOL
+    assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
+    assert rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B) < TOL
+
+
+def test_step_host_end_to_end():
+    """psc_step_host (host buffers in, host buffers out) equals the device-resident path"""
+    pl = _small("2d")
+    sim = _sim(pl)
+    sim.step(3)
+    ref = gpu_cols(sim)
+    refE = sim.E.cpu()
+    sim2 = _sim(pl)
+    host = {k: getattr(pl, k).clone().pin_memory() for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id")}
+    hE = sim2.E.cpu().pin_memory()
+    hB = sim2.B.cpu().pin_memory()
+    hJ = torch.zeros_like(hE).pin_memory()
+    sim2.psc.step_host(pl.n_particles, host, hE, hB, hJ, nsteps=3)
+    # (J is accumulated with floating-point atomics, so two runs agree to rounding, not bitwise)
+    for k in ("id", "species", "qw"):
+        assert np.array_equal(host[k].numpy(), ref[k]), k
+    for k in ("y", "z", "ux", "uy", "uz"):
+        assert np.abs(host[k].numpy() - ref[k]).max() < 1e-5, k
+    assert (hE - refE).abs().max() <= 1e-5 * refE.abs().max()

@@ -1,0 +1,92 @@
+"""Shared helpers of the GPU parity tests: oracle-side state from a seeded plasma, comparison
+metrics (periodic distance, max-norm relative errors).  No arithmetic of the method."""
+import numpy as np
+
+from oracle.psc_oracle import Oracle
+
+PCOLS = ("x", "y", "z", "ux", "uy", "uz", "qw")
+
+
+def oracle_for(pl, block=(1, 1, 1)):
+    return Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m, block=block)
+
+
+def oracle_state(pl):
+    """fp64 copies of the plasma's fp32 values: dict of particle columns, E, B"""
+    st = {k: np.ascontiguousarray(getattr(pl, k).cpu().numpy().astype(np.float64)) for k in PCOLS}
+    st["species"] = np.ascontiguousarray(pl.species.cpu().numpy().astype(np.int32))
+    st["id"] = np.ascontiguousarray(pl.id.cpu().numpy().astype(np.int32))
+    E = np.ascontiguousarray(pl.E.cpu().numpy().astype(np.float64))
+    B = np.ascontiguousarray(pl.B.cpu().numpy().astype(np.float64))
+    return st, E, B
+
+
+def gpu_cols(sim):
+    cur = sim.current()
+    return {k: v.cpu().numpy() for k, v in cur.items() if v is not None}
+
+
+def periodic_dist(a, b, L):
+    d = np.abs(a.astype(np.float64) - b.astype(np.float64))
+    return np.minimum(d, L - d)
+
+
+def rel_maxnorm(got, ref):
+    """max |got - ref| / max |ref| per leading component -> the largest of them"""
+    worst = 0.0
+    for c in range(ref.shape[0]):
+        den = np.abs(ref[c]).max()
+        err = np.abs(got[c].astype(np.float64) - ref[c]).max()
+        if den == 0.0:
+            assert err == 0.0, "component %d: reference is identically zero, got %g" % (c, err)
+            continue
+        worst = max(worst, err / den)
+    return worst
+
+
+def smooth_fields(pl, amp, seed):
+    """seeded smooth (few-mode) periodic E and B of amplitude ~amp on the plasma's grid, fp32,
+    written into pl.E / pl.B (inputs only -- shared by both paths)"""
+    import torch
+
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = pl.n
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    out = []
+    for _ in range(2):
+        F = np.zeros((3, nz, ny, nx))
+        for c in range(3):
+            for _m in range(3):
+                mx = rng.integers(0, 3) if nx > 1 else 0
+                my = rng.integers(0, 3) if ny > 1 else 0
+                mz = rng.integers(0, 3) if nz > 1 else 0
+                ph = rng.uniform(0, 2 * np.pi)
+                F[c] += rng.normal() * np.cos(2 * np.pi * (mx * i / nx + my * j / ny + mz * k / nz) + ph)
+        out.append(torch.from_numpy((amp * F / 3.0).astype(np.float32)))
+    pl.E, pl.B = out[0], out[1]
+    return pl
+
+
+def library_block(n, block=(0, 0, 0)):
+    """the block the library uses for a requested `block` (include/psc.h: 0 = default: 8 cells in
+    2-d, 4 in 3-d, halved until it divides n; 1 along invariant directions)"""
+    is3d = all(v > 1 for v in n)
+    out = []
+    for d in range(3):
+        b = block[d]
+        if n[d] == 1:
+            b = 1
+        elif b == 0:
+            b = 4 if is3d else 8
+            while n[d] % b:
+                b //= 2
+        out.append(b)
+    return tuple(out)
+
+
+def oracle_sorted_state(pl, block):
+    """the seeded plasma permuted by the ORACLE's stable cell sort: fp32 columns (dict)"""
+    orc = oracle_for(pl, block=library_block(pl.n, block))
+    cols = {k: getattr(pl, k).cpu().numpy() for k in PCOLS + ("species", "id")}
+    _, _, perm, _ = orc.sort(cols["x"], cols["y"], cols["z"])
+    return {k: np.ascontiguousarray(v[perm]) for k, v in cols.items()}
