@@ -12,15 +12,24 @@
  *     stream) and the library borrows the pointers until the next bind or psc_destroy.  The only
  *     device memory the context owns is a 64-byte status/counter block.
  *   - Every call that does device work enqueues it on `stream` (a cudaStream_t passed as void*)
- *     and returns without synchronising, except psc_status, psc_step_host and psc_sort_result_host.
+ *     and returns without synchronising, except psc_status and psc_step_host.
  *   - Every call returns 0 (PSC_OK) or a negative PSC_ERR_* code; nothing aborts or throws across
  *     the ABI.  Data-dependent faults are sticky device flags read with psc_status.
  *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with
  *     PSC_ERR_CUDA.
  *
  * Units and conventions: c = eps0 = mu0 = 1; momentum columns hold
- * u = p/(m_s c); qw = q_s * w; positions are absolute, in [0, n[d]*dx[d]); a direction with
- * n[d] == 1 is invariant: no ghosts, no derivative, its coordinate is carried but never advanced.
+ * u = p/(m_s c); qw = q_s * w; a direction with n[d] == 1 is invariant: no ghosts, no
+ * derivative, its coordinate is carried but never advanced.
+ *
+ * Particle store ("struct of arrays", fp32).  The caller hands over ABSOLUTE
+ * positions in [0, n[d]*dx[d]).  Absolute fp32 coordinates have an ulp of up to 6e-5 cells on a
+ * 1024-cell axis, which is not enough to keep the deposited current within 1e-5 of the fp64
+ * scheme over several steps, so the first psc_particles_sort converts the position columns IN
+ * PLACE to the internal form: in-cell offsets in [0,1) (units of cells) plus one int32 cell key per
+ * particle kept in the workspace (psc_particles_keys).  The columns stay in internal form until
+ * psc_particles_export converts them back to absolute coordinates (psc_step_host does so before
+ * copying out).  psc_particles_form tells which form the current columns are in.
  *
  * Field layout: each of E, B, J is float[3][ez][ey][ex] with ex = n[0] + 2*g (1 if n[0] == 1)
  * etc., x fastest; interior cell i is stored at i + g.  Yee staggering (PAPER.md:141-143,
@@ -81,7 +90,7 @@ typedef struct {
 /* One set of particle columns (structure of arrays), each of length >= n.
  * `id` may be NULL in both sets (then no id is carried). */
 typedef struct {
-  float *x, *y, *z;    /* positions x^{n+1/2} */
+  float *x, *y, *z;    /* positions x^{n+1/2}: absolute, or in-cell offsets (internal form) */
   float *ux, *uy, *uz; /* u^n = p/(m c) */
   float *qw;           /* q_s * w */
   int32_t *species;    /* 0 .. n_species-1 */
@@ -111,16 +120,18 @@ int psc_bind_particles(psc_ctx *ctx, int64_t n, const psc_particle_cols *primary
 
 /* Cell-key counting sort.  key = block-major, cell-minor; stable (ascending
  * input index inside a key).  Afterwards the CURRENT column set (psc_particles_current) holds
- * the particles in sorted order; the two sets swap roles.  Arbitrary input order is accepted;
- * when the list is the previous sort's output advanced by one psc_push_particles, a cheaper
- * path that exploits "a particle moves at most one cell per step" is taken --
- * the result is identical. */
+ * the particles in sorted order and in internal form; the two sets swap roles.  Arbitrary input
+ * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))); from
+ * internal-form columns (the previous sort's output advanced by psc_push_particles) the push has
+ * already left each particle's new key -- its cell moved by at most one per direction
+ * -- so the sort does not read positions at all. */
 int psc_particles_sort(psc_ctx *ctx, void *stream);
 
 /* The particle loop of Fig. 8 in one pass over the particles
  * (PAPER.md:603): zero J; per particle gather E,B at x^{n+1/2} (Eq. 11), Boris push
  * p^n -> p^{n+1} (Eq. 27-28), x^{n+1/2} -> x^{n+3/2} (Eq. 26), charge-conserving deposit of
- * j^{n+1}, periodic wrap.  Requires a sorted list (PSC_ERR_NOT_SORTED).
+ * j^{n+1}, periodic wrap (on the integer cell index).  Requires a sorted list
+ * in internal form, i.e. psc_particles_sort directly before (PSC_ERR_NOT_SORTED).
  * J ghosts are NOT folded on return (psc_exchange_j). */
 int psc_push_particles(psc_ctx *ctx, void *stream);
 
@@ -147,13 +158,23 @@ int psc_step(psc_ctx *ctx, void *stream);
 int psc_step_host(psc_ctx *ctx, void *stream, int64_t n, const psc_particle_cols *host,
                   float *hostE, float *hostB, float *hostJ, int nsteps);
 
-/* Inspection.  Device pointers into the workspace, valid until the next sort:
- * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i), perm[n] (sorted slot s holds
- * input particle perm[s]), cell_offsets[n_keys+1] (exclusive scan of the key histogram). */
-int psc_sort_result(const psc_ctx *ctx, const int32_t **cell_idx, const int32_t **perm,
+/* Inspection of the last sort.  Device pointers into the workspace, valid until the next sort:
+ * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i; computed on `stream` by this
+ * call), perm[n] (sorted slot s holds input particle perm[s]), cell_offsets[n_keys+1]
+ * (exclusive scan of the key histogram). */
+int psc_sort_result(psc_ctx *ctx, void *stream, const int32_t **cell_idx, const int32_t **perm,
                     const int32_t **cell_offsets, int64_t *n_keys);
-/* The column set that currently holds the particles. */
+/* The column set that currently holds the particles (positions in the form psc_particles_form
+ * reports). */
 int psc_particles_current(const psc_ctx *ctx, psc_particle_cols *out);
+/* 0: absolute positions, 1: internal form (in-cell offsets + keys). */
+int psc_particles_form(const psc_ctx *ctx);
+/* Internal form only: key[n] of the current particles (cell key as defined by the sort; the cell
+ * a particle's offset refers to).  Device pointer into the workspace. */
+int psc_particles_keys(const psc_ctx *ctx, const int32_t **key);
+/* Converts the current columns back to absolute positions x = (cell + offset) * dx, in place
+ * (one fp32 rounding).  The list counts as unsorted afterwards.  No-op on absolute columns. */
+int psc_particles_export(psc_ctx *ctx, void *stream);
 /* Synchronises `stream`, returns and keeps the sticky flags. */
 int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);
 /* Kernels and memsets/copies this context has enqueued so far (host counter). */

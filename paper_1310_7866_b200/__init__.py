@@ -21,7 +21,8 @@ EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
     "psc_field_elems", "psc_bind_particles", "psc_particles_sort", "psc_push_particles",
     "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step", "psc_step_host",
-    "psc_sort_result", "psc_particles_current", "psc_status", "psc_launch_count",
+    "psc_sort_result", "psc_particles_current", "psc_particles_form", "psc_particles_keys",
+    "psc_particles_export", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_strerror", "psc_version",
 ]
 
@@ -80,8 +81,12 @@ def lib():
         L.psc_fill_ghosts.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.psc_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(PscCols),
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
-        L.psc_sort_result.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
-                                      C.POINTER(C.c_void_p), C.POINTER(C.c_int64)]
+        L.psc_sort_result.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                      C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                      C.POINTER(C.c_int64)]
+        L.psc_particles_form.argtypes = [C.c_void_p]
+        L.psc_particles_keys.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.psc_particles_export.argtypes = [C.c_void_p, C.c_void_p]
         L.psc_particles_current.argtypes = [C.c_void_p, C.POINTER(PscCols)]
         L.psc_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32)]
         L.psc_launch_count.argtypes = [C.c_void_p]
@@ -206,13 +211,25 @@ class Psc:
                                         int(nsteps)), "psc_step_host")
 
     # -- inspection ------------------------------------------------------------------------------
-    def sort_result(self):
+    def sort_result(self, stream=None):
         """raw device pointers (cell_idx, perm, cell_offsets) and n_keys"""
         ci, pm, co = C.c_void_p(), C.c_void_p(), C.c_void_p()
         nk = C.c_int64()
-        self._check(lib().psc_sort_result(self._h, C.byref(ci), C.byref(pm), C.byref(co), C.byref(nk)),
-                    "psc_sort_result")
+        self._check(lib().psc_sort_result(self._h, _stream(stream), C.byref(ci), C.byref(pm),
+                                          C.byref(co), C.byref(nk)), "psc_sort_result")
         return ci.value, pm.value, co.value, int(nk.value)
+
+    def particles_form(self):
+        return int(lib().psc_particles_form(self._h))
+
+    def particles_keys(self):
+        """raw device pointer of the current particles' cell keys (internal form only)"""
+        k = C.c_void_p()
+        self._check(lib().psc_particles_keys(self._h, C.byref(k)), "psc_particles_keys")
+        return k.value
+
+    def particles_export(self, stream=None):
+        self._check(lib().psc_particles_export(self._h, _stream(stream)), "psc_particles_export")
 
     def particles_current(self):
         """raw device pointers of the column set that currently holds the particles"""

@@ -143,6 +143,7 @@ size_t psc_workspace_bytes(const psc_ctx *c, int64_t max_particles) {
 int psc_bind_workspace(psc_ctx *c, void *ws, size_t bytes) {
   if (!c || !ws) return PSC_ERR_INVALID_ARG;
   if (((uintptr_t)ws) & 255) return PSC_ERR_ALIGN;
+  if (c->have_particles && c->form == PSC_FORM_REL) return PSC_ERR_INVALID_ARG;  // keys live in ws
   c->ws = ws;
   c->ws_bytes = bytes;
   c->ws_cap = -1;
@@ -187,6 +188,8 @@ int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const 
   c->np = n;
   c->have_particles = 1;
   c->state = PSC_STATE_UNSORTED;
+  c->form = PSC_FORM_ABS;
+  c->kcur = 0;
   c->have_sort_result = 0;
   if (c->ws) {
     if (c->ws_bytes < psc_workspace_bytes(c, n)) {
@@ -209,7 +212,7 @@ int psc_particles_sort(psc_ctx *c, void *stream) {
 int psc_push_particles(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
-  if (c->state != PSC_STATE_SORTED) return PSC_ERR_NOT_SORTED;
+  if (c->state != PSC_STATE_SORTED || c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
   const int rc = c->gd.order == 1 ? psc_push_order1(c, (cudaStream_t)stream)
                                   : psc_push_order2(c, (cudaStream_t)stream);
   if (rc == PSC_OK) c->state = PSC_STATE_UNSORTED;
@@ -271,6 +274,7 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
     PSC_CUDA_TRY(c, cudaMemcpyAsync(c->E, hE, fb, cudaMemcpyHostToDevice, s));
     PSC_CUDA_TRY(c, cudaMemcpyAsync(c->B, hB, fb, cudaMemcpyHostToDevice, s));
     c->state = PSC_STATE_UNSORTED;
+    c->form = PSC_FORM_ABS;
     c->launches += 11;
   }
   for (int i = 0; i < nsteps; i++) {
@@ -278,6 +282,8 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
     if (rc) return rc;
   }
   {
+    const int rc = psc_particles_export(c, stream);
+    if (rc) return rc;
     Cols &d = c->cols[c->cur];
     void *dst[] = {h->x, h->y, h->z, h->ux, h->uy, h->uz, h->qw, h->species, h->id};
     const void *src[] = {d.x, d.y, d.z, d.ux, d.uy, d.uz, d.qw, d.sp, d.id};
@@ -292,15 +298,36 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
   return PSC_OK;
 }
 
-int psc_sort_result(const psc_ctx *c, const int32_t **cell_idx, const int32_t **perm,
+int psc_sort_result(psc_ctx *c, void *stream, const int32_t **cell_idx, const int32_t **perm,
                     const int32_t **cell_offsets, int64_t *n_keys) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_sort_result) return PSC_ERR_NOT_SORTED;
-  if (cell_idx) *cell_idx = c->cell_idx;
+  if (cell_idx) {
+    const int rc = psc_sort_cell_idx(c, (cudaStream_t)stream);
+    if (rc) return rc;
+    *cell_idx = c->cell_idx;
+  }
   if (perm) *perm = c->perm;
   if (cell_offsets) *cell_offsets = c->cell_offsets;
   if (n_keys) *n_keys = c->gd.nkeys;
   return PSC_OK;
+}
+
+int psc_particles_form(const psc_ctx *c) { return c ? c->form : PSC_ERR_INVALID_ARG; }
+
+int psc_particles_keys(const psc_ctx *c, const int32_t **key) {
+  if (!c || !key) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
+  *key = c->key[c->kcur];
+  return PSC_OK;
+}
+
+int psc_particles_export(psc_ctx *c, void *stream) {
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles) return PSC_ERR_NOT_BOUND;
+  if (c->form == PSC_FORM_ABS) return PSC_OK;
+  return psc_particles_to_abs(c, (cudaStream_t)stream);
 }
 
 int psc_particles_current(const psc_ctx *c, psc_particle_cols *out) {

@@ -35,6 +35,7 @@ struct Cols {
 };
 
 enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1 };
+enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
 
 struct psc_ctx {
   GridDesc gd;
@@ -45,12 +46,14 @@ struct psc_ctx {
   int64_t np;
   int have_particles, have_fields;
   int state;
+  int form;        // PSC_FORM_ABS: absolute positions; PSC_FORM_REL: in-cell offsets + key[kcur]
+  int kcur;        // which key buffer belongs to the current column set
   int have_sort_result;
   // workspace carve-up (all device pointers)
   void *ws;
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
-  int32_t *key, *perm, *cell_idx, *cell_offsets, *cursor, *scan_tmp, *big_list;
+  int32_t *key[2], *perm, *cell_idx, *cell_offsets, *cursor, *scan_tmp, *big_list;
   uint32_t *d_flags;  // owned: 16 words; [0] sticky flags, [1] big-segment counter
   int64_t launches;
   int last_err;
@@ -89,6 +92,8 @@ int psc_fields_fold(psc_ctx *c, float *F, cudaStream_t s);
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n);
 int psc_sort_carve(psc_ctx *c, int64_t n);
 int psc_sort_run(psc_ctx *c, cudaStream_t s);
+int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s);
+int psc_particles_to_abs(psc_ctx *c, cudaStream_t s);
 // push1.cu / push2.cu
 int psc_push_order1(psc_ctx *c, cudaStream_t s);
 int psc_push_order2(psc_ctx *c, cudaStream_t s);

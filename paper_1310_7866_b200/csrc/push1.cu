@@ -7,6 +7,13 @@
 // cell-ordered particle range with coalesced column loads, accumulates current in a shared
 // J tile (tile + 1 low / 2 high halo nodes) and flushes the tile to global J once.
 //
+// Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction +
+// the cell key.  The move is b = a + v dt/dx; a particle that leaves its cell (b < 0 or b >= 1;
+// at most one cell per direction) gets offset b -/+ 1 and the key of the
+// neighbouring cell, looked up in per-direction tables that hold the periodic wrap -- the
+// single-GPU form of the particle exchange.  The new key is what the next sort
+// consumes; no floor(), no float->int conversion and no absolute coordinate appear here.
+//
 // The VB current is the exact flux of a b0-shaped cloud moving on the straight line
 // x^{n+1/2} -> x^{n+3/2}; it is evaluated by splitting the line at the cell faces it crosses
 // (at most one per direction because dt <= dx/2).  For a segment a -> b inside one cell, with
@@ -146,13 +153,35 @@ __device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TileGeo
 
 template <bool D3>
 __global__ void __launch_bounds__(PUSH_THREADS, 3)
-k_push1(GridDesc gd, Cols p, const int *__restrict__ cell_offsets, const float *__restrict__ E,
-        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
+k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell_offsets,
+        const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
+        uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   TileGeom<D3> tg;
   tg.init(gd, blockIdx.x);
   float *sF = smem;                // [6][fvol]: Ex Ey Ez Bx By Bz
   float *sJ = smem + 6 * tg.fvol;  // [3][jvol]
+  int *sLut = (int *)(sJ + 3 * tg.jvol);  // [cpb]: cell in tile -> lx | ly << 10 | lz << 20
+  int *sKx = sLut + gd.cpb;               // key contribution of local x coordinate -1 .. bs0
+  int *sKy = sKx + gd.bs[0] + 2;
+  int *sKz = sKy + gd.bs[1] + 2;
+
+  for (int i = threadIdx.x; i < gd.cpb; i += blockDim.x) {
+    const int lx = i % gd.bs[0], t = i / gd.bs[0];
+    sLut[i] = lx | ((t % gd.bs[1]) << 10) | ((t / gd.bs[1]) << 20);
+  }
+  for (int i = threadIdx.x; i < gd.bs[0] + gd.bs[1] + gd.bs[2] + 6; i += blockDim.x) {
+    int d = 0, l = i;
+    if (l >= gd.bs[0] + 2) { l -= gd.bs[0] + 2; d = 1; }
+    if (d == 1 && l >= gd.bs[1] + 2) { l -= gd.bs[1] + 2; d = 2; }
+    int c = tg.o[d] + l - 1;  // global cell coordinate, wrapped periodically
+    if (c < 0) c += gd.n[d];
+    if (c >= gd.n[d]) c -= gd.n[d];
+    const int b = c / gd.bs[d], ll = c - b * gd.bs[d];
+    const int bstride = d == 0 ? 1 : d == 1 ? gd.nb[0] : gd.nb[0] * gd.nb[1];
+    const int lstride = d == 0 ? 1 : d == 1 ? gd.bs[0] : gd.bs[0] * gd.bs[1];
+    sKx[i] = b * bstride * gd.cpb + ll * lstride;
+  }
 
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
@@ -170,33 +199,22 @@ k_push1(GridDesc gd, Cols p, const int *__restrict__ cell_offsets, const float *
   const float *sEx = sF, *sEy = sF + tg.fvol, *sEz = sF + 2 * tg.fvol;
   const float *sBx = sF + 3 * tg.fvol, *sBy = sF + 4 * tg.fvol, *sBz = sF + 5 * tg.fvol;
   uint32_t bad = 0;
+  const int kbase = blockIdx.x * gd.cpb;
 
   for (int a = p0 + threadIdx.x; a < p1; a += blockDim.x) {
-    float x = 0.f, ax = 0.f;
-    int lx = 0;
-    const float y = ld_stream(p.y + a), z = ld_stream(p.z + a);
+    float ax = 0.f;
+    const float ay = ld_stream(p.y + a), az = ld_stream(p.z + a);
     float ux = ld_stream(p.ux + a), uy = ld_stream(p.uy + a), uz = ld_stream(p.uz + a);
     const float qw = ld_stream(p.qw + a);
     const int sp = ld_stream(p.sp + a);
-    if (D3) x = ld_stream(p.x + a);
-
-    // cell and in-cell offsets (same fp32 product + floor as the sort)
-    const float yi = __fmul_rn(y, gd.inv_dx[1]), zi = __fmul_rn(z, gd.inv_dx[2]);
-    const float cyf = floorf(yi), czf = floorf(zi);
-    const float ay = yi - cyf, az = zi - czf;
-    int ly = (int)cyf - tg.o[1], lz = (int)czf - tg.o[2];
-    bool in_tile = ly >= 0 && ly < gd.bs[1] && lz >= 0 && lz < gd.bs[2];
-    if (D3) {
-      const float xi = __fmul_rn(x, gd.inv_dx[0]);
-      const float cxf = floorf(xi);
-      ax = xi - cxf;
-      lx = (int)cxf - tg.o[0];
-      in_tile = in_tile && lx >= 0 && lx < gd.bs[0];
-    }
-    if (!in_tile) {  // not the sorted list this kernel was promised: flag, leave untouched
+    const int lc = ld_stream(key + a) - kbase;
+    if (D3) ax = ld_stream(p.x + a);
+    if (lc < 0 || lc >= gd.cpb) {  // not the sorted list this kernel was promised: flag, skip
       bad |= PSC_F_NOT_IN_TILE;
       continue;
     }
+    const int packed = sLut[lc];
+    const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
 
     // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) ----------
     Stencil1 sx, sy, sz;
@@ -256,21 +274,32 @@ k_push1(GridDesc gd, Cols p, const int *__restrict__ cell_offsets, const float *
       }
     }
 
-    // ---- store; periodic wrap is the single-GPU particle exchange -----------
-    const float y1 = wrap_periodic(fmaf(gd.dt, vy, y), gd.L[1]);
-    const float z1 = wrap_periodic(fmaf(gd.dt, vz, z), gd.L[2]);
-    if (D3) {
-      const float x1 = wrap_periodic(fmaf(gd.dt, vx, x), gd.L[0]);
-      st_stream(p.x + a, x1);
-      if (!(fabsf(x1) <= gd.L[0])) bad |= PSC_F_NAN;
+    // ---- new offset + new key (periodic wrap lives in the key tables) -----------------------
+    {
+      float by_ = ay + ddy, bz_ = az + ddz;
+      const int sy = by_ >= 1.f ? 1 : (by_ < 0.f ? -1 : 0);
+      const int sz = bz_ >= 1.f ? 1 : (bz_ < 0.f ? -1 : 0);
+      by_ = fminf(fmaxf(by_ - (float)sy, 0.f), 0.99999994f);
+      bz_ = fminf(fmaxf(bz_ - (float)sz, 0.f), 0.99999994f);
+      int nk = sKy[ly + sy + 1] + sKz[lz + sz + 1];
+      if (D3) {
+        float bx_ = ax + ddx;
+        const int sx = bx_ >= 1.f ? 1 : (bx_ < 0.f ? -1 : 0);
+        bx_ = fminf(fmaxf(bx_ - (float)sx, 0.f), 0.99999994f);
+        nk += sKx[lx + sx + 1];
+        st_stream(p.x + a, bx_);
+        if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
+      } else {
+        nk += sKx[1];
+      }
+      st_stream(p.y + a, by_);
+      st_stream(p.z + a, bz_);
+      st_stream(p.ux + a, ux);
+      st_stream(p.uy + a, uy);
+      st_stream(p.uz + a, uz);
+      __stcs(key + a, nk);
+      if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
-    st_stream(p.y + a, y1);
-    st_stream(p.z + a, z1);
-    st_stream(p.ux + a, ux);
-    st_stream(p.uy + a, uy);
-    st_stream(p.uz + a, uz);
-    if (!(fabsf(y1) <= gd.L[1]) || !(fabsf(z1) <= gd.L[2]) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
-      bad |= PSC_F_NAN;
   }
   if (bad) atomicOr(flags, bad);
   __syncthreads();
@@ -304,16 +333,17 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       fvol *= gd.bs[d] + 2;
       jvol *= gd.bs[d] + 3;
     }
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol) * sizeof(float);
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + gd.cpb + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6) * sizeof(float);
+  if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &p = c->cols[c->cur];
   const int threads = c->opt_threads > 0 ? c->opt_threads : PUSH_THREADS;
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
   } else {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
   }
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

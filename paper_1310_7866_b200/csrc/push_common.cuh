@@ -23,14 +23,6 @@ __device__ __forceinline__ void boris_push(float &ux, float &uy, float &uz, floa
   uz = fmaf(h, ez, plz);
 }
 
-// periodic wrap into [0, L) (A14): x - L or x + L may round to exactly L
-__device__ __forceinline__ float wrap_periodic(float x, float L) {
-  if (x < 0.0f) x += L;
-  if (x >= L) x -= L;
-  if (x >= L) x = 0.0f;
-  return x;
-}
-
 // streaming (read-once / write-once) particle column accesses: keep them out of L1
 __device__ __forceinline__ float ld_stream(const float *p) { return __ldcs(p); }
 __device__ __forceinline__ int ld_stream(const int *p) { return __ldcs(p); }

@@ -3,9 +3,10 @@
 // One key orders by block ("supercell") and by cell inside the block at once:
 //   key = block_index * cells_per_block + cell_in_block.
 // A counting sort is O(N + M).  The B200 form:
-//   1. k_keys     key + natural cell index per particle, histogram over keys with
-//                 warp-aggregated atomics (lanes holding the same key elect one lane that adds
-//                 the group's size; on a cell-ordered list a warp issues 1-2 atomics, not 32);
+//   1. k_keys     (absolute positions in) key per particle from floor(fl32(x * 1/dx)), or
+//      k_hist     (internal form in) the keys the push left behind; either way a histogram over
+//                 keys with warp-aggregated atomics (lanes holding the same key elect one lane
+//                 that adds the group's size; on a cell-ordered list a warp issues 1-2 atomics);
 //   2. scan       exclusive prefix sum of the histogram -> cell_offsets (three small kernels);
 //   3. k_scatter  slot = cursor[key] + rank, again warp-aggregated; writes the permutation;
 //   4. k_segsort  the atomics hand out slots in arbitrary order ACROSS warps, so every key's
@@ -15,7 +16,8 @@
 //                 unique stable counting sort, bit-exact against any stable reference;
 //   5. k_reorder  out[s] = in[perm[s]] for every column (coalesced writes; the reads are nearly
 //                 coalesced when the list is a previous sort's output advanced by one push,
-//                 because a particle moves at most one cell per step).
+//                 because a particle moves at most one cell per step).  Positions
+//                 leave this kernel in the internal form (in-cell offset; the cell is the key).
 #include <limits.h>
 
 #include "psc_internal.cuh"
@@ -36,8 +38,8 @@ __device__ __forceinline__ unsigned lanemask_lt() {
 
 __global__ void __launch_bounds__(SORT_THREADS)
 k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict__ y,
-       const float *__restrict__ z, int *__restrict__ key, int *__restrict__ cell_idx,
-       int *__restrict__ hist, uint32_t *__restrict__ flags) {
+       const float *__restrict__ z, int *__restrict__ key, int *__restrict__ hist,
+       uint32_t *__restrict__ flags) {
   const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   const int nround = ((n + 31) / 32) * 32;
@@ -68,10 +70,70 @@ k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict_
       const int l0 = c[0] - b0 * gd.bs[0], l1 = c[1] - b1 * gd.bs[1], l2 = c[2] - b2 * gd.bs[2];
       k = ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
       key[a] = k;
-      cell_idx[a] = (c[2] * gd.n[1] + c[1]) * gd.n[0] + c[0];
     }
     const unsigned grp = __match_any_sync(0xffffffffu, k);
     if (valid && (grp & lanemask_lt()) == 0) atomicAdd(&hist[k], __popc(grp));
+  }
+}
+
+// histogram of keys that already exist (internal form: the push wrote them)
+__global__ void __launch_bounds__(SORT_THREADS)
+k_hist(int n, int nkeys, const int *__restrict__ key, int *__restrict__ hist,
+       uint32_t *__restrict__ flags) {
+  const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
+  const int stride = gridDim.x * blockDim.x;
+  const int nround = ((n + 31) / 32) * 32;
+  for (int a = a0; a < nround; a += stride) {
+    const bool valid = a < n;
+    int k = -1 - (int)(threadIdx.x & 31);
+    if (valid) {
+      k = key[a];
+      if (k < 0 || k >= nkeys) {  // cannot happen unless the caller scribbled over the workspace
+        atomicOr(flags, PSC_F_OOB);
+        k = 0;
+      }
+    }
+    const unsigned grp = __match_any_sync(0xffffffffu, k);
+    if (valid && (grp & lanemask_lt()) == 0) atomicAdd(&hist[k], __popc(grp));
+  }
+}
+
+// key -> cell coordinates
+__device__ __forceinline__ void key_to_cell(const GridDesc &gd, int k, int c[3]) {
+  const int b = k / gd.cpb, l = k - b * gd.cpb;
+  const int b0 = b % gd.nb[0], br = b / gd.nb[0];
+  const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
+  const int l0 = l % gd.bs[0], lr = l / gd.bs[0];
+  const int l1 = lr % gd.bs[1], l2 = lr / gd.bs[1];
+  c[0] = b0 * gd.bs[0] + l0;
+  c[1] = b1 * gd.bs[1] + l1;
+  c[2] = b2 * gd.bs[2] + l2;
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_cell_idx(GridDesc gd, int n, const int *__restrict__ key, int *__restrict__ cell_idx) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n) return;
+  int c[3];
+  key_to_cell(gd, key[a], c);
+  cell_idx[a] = (c[2] * gd.n[1] + c[1]) * gd.n[0] + c[0];
+}
+
+// internal form -> absolute positions, in place: x = (cell + offset) * dx
+__global__ void __launch_bounds__(SORT_THREADS)
+k_to_abs(GridDesc gd, int n, const int *__restrict__ key, float *__restrict__ x,
+         float *__restrict__ y, float *__restrict__ z) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= n) return;
+  int c[3];
+  key_to_cell(gd, key[a], c);
+  float *pos[3] = {x, y, z};
+#pragma unroll
+  for (int d = 0; d < 3; d++) {
+    if (gd.n[d] == 1) continue;
+    float v = ((float)c[d] + pos[d][a]) * gd.dx[d];
+    if (v >= gd.L[d]) v = nextafterf(gd.L[d], 0.f);  // rounding must not leave [0, L)
+    pos[d][a] = v;
   }
 }
 
@@ -293,18 +355,27 @@ k_segsort_big(const int *__restrict__ offs, int *__restrict__ perm,
   }
 }
 
+// FROM_ABS: the input columns hold absolute positions -> write in-cell offsets
+template <bool FROM_ABS>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_reorder(int n, const int *__restrict__ perm, Cols in, Cols out) {
+k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out,
+          const int *__restrict__ key_in, int *__restrict__ key_out) {
   const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   for (int s = s0; s < n; s += stride) {
     const int p = perm[s];
-    const float x = in.x[p], y = in.y[p], z = in.z[p];
+    float x = in.x[p], y = in.y[p], z = in.z[p];
     const float ux = in.ux[p], uy = in.uy[p], uz = in.uz[p];
     const float qw = in.qw[p];
     const int sp = in.sp[p];
+    const int k = key_in[p];
     int id = 0;
     if (in.id) id = in.id[p];
+    if (FROM_ABS) {  // same fp32 product + floor as k_keys; clamped like there
+      if (gd.n[0] > 1) { const float xi = __fmul_rn(x, gd.inv_dx[0]); x = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
+      if (gd.n[1] > 1) { const float xi = __fmul_rn(y, gd.inv_dx[1]); y = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
+      if (gd.n[2] > 1) { const float xi = __fmul_rn(z, gd.inv_dx[2]); z = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
+    }
     out.x[s] = x;
     out.y[s] = y;
     out.z[s] = z;
@@ -313,6 +384,7 @@ k_reorder(int n, const int *__restrict__ perm, Cols in, Cols out) {
     out.uz[s] = uz;
     out.qw[s] = qw;
     out.sp[s] = sp;
+    key_out[s] = k;
     if (in.id) out.id[s] = id;
   }
 }
@@ -324,7 +396,7 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
   size_t b = 0;
-  b += 3 * align_up((size_t)n * 4, 256);                      // key, perm, cell_idx
+  b += 4 * align_up((size_t)n * 4, 256);                      // key[2], perm, cell_idx
   b += 2 * align_up((nk + 1) * 4, 256);                       // cell_offsets, cursor
   b += align_up((nk / SCAN_TILE + 3) * 4, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
@@ -339,7 +411,8 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
     p += align_up(bytes, 256);
     return r;
   };
-  c->key = (int32_t *)take((size_t)n * 4);
+  c->key[0] = (int32_t *)take((size_t)n * 4);
+  c->key[1] = (int32_t *)take((size_t)n * 4);
   c->perm = (int32_t *)take((size_t)n * 4);
   c->cell_idx = (int32_t *)take((size_t)n * 4);
   c->cell_offsets = (int32_t *)take((nk + 1) * 4);
@@ -358,11 +431,14 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
   const Cols &out = c->cols[c->cur ^ 1];
   const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
 
+  int32_t *key_in = c->key[c->kcur], *key_out = c->key[c->kcur ^ 1];
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
   c->launches += 2;
-  k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, c->key, c->cell_idx, c->cursor,
-                                          c->d_flags);
+  if (c->form == PSC_FORM_ABS)
+    k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, key_in, c->cursor, c->d_flags);
+  else
+    k_hist<<<pblocks, SORT_THREADS, 0, s>>>(n, nk, key_in, c->cursor, c->d_flags);
   PSC_LAUNCH_CHECK(c);
   const int sblocks = (int)cdiv64(nk, SCAN_TILE);
   k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, c->cell_offsets, c->scan_tmp);
@@ -371,7 +447,7 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
   PSC_LAUNCH_CHECK(c);
   k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->cursor, c->scan_tmp, sblocks);
   PSC_LAUNCH_CHECK(c);
-  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, c->key, c->cursor, c->perm);
+  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, key_in, c->cursor, c->perm);
   PSC_LAUNCH_CHECK(c);
   const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
   k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->perm, c->big_list,
@@ -388,10 +464,36 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
                                                               c->d_flags + 1);
     PSC_LAUNCH_CHECK(c);
   }
-  k_reorder<<<pblocks, SORT_THREADS, 0, s>>>(n, c->perm, in, out);
+  if (c->form == PSC_FORM_ABS)
+    k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
+  else
+    k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
   PSC_LAUNCH_CHECK(c);
   c->cur ^= 1;
+  c->kcur ^= 1;
+  c->form = PSC_FORM_REL;
   c->state = PSC_STATE_SORTED;
   c->have_sort_result = 1;
+  return PSC_OK;
+}
+
+// cell_idx[a] of the last sort's INPUT particles (their keys are in the non-current key buffer)
+int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s) {
+  const int n = (int)c->np;
+  if (n == 0) return PSC_OK;
+  k_cell_idx<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key[c->kcur ^ 1], c->cell_idx);
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}
+
+int psc_particles_to_abs(psc_ctx *c, cudaStream_t s) {
+  const int n = (int)c->np;
+  if (n) {
+    const Cols &p = c->cols[c->cur];
+    k_to_abs<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key[c->kcur], p.x, p.y, p.z);
+    PSC_LAUNCH_CHECK(c);
+  }
+  c->form = PSC_FORM_ABS;
+  c->state = PSC_STATE_UNSORTED;
   return PSC_OK;
 }

@@ -55,16 +55,18 @@ class Simulation:
         assert s["x"].data_ptr() == ptr
         return {c: (None if t is None else t[: self.np]) for c, t in s.items()}
 
+    def _ws_view(self, ptr, count):
+        off = ptr - self.ws.data_ptr()
+        return self.ws[off: off + 4 * count].view(torch.int32)
+
+    def keys(self):
+        """cell keys of the current particles (internal form), int32 tensor viewing the workspace"""
+        return self._ws_view(self.psc.particles_keys(), self.np)
+
     def sort_result(self):
         """(cell_idx[n], perm[n], cell_offsets[n_keys+1]) as int32 tensors viewing the workspace"""
         ci, pm, co, nk = self.psc.sort_result()
-        base = self.ws.data_ptr()
-
-        def view(ptr, count):
-            off = ptr - base
-            return self.ws[off: off + 4 * count].view(torch.int32)
-
-        return view(ci, self.np), view(pm, self.np), view(co, nk + 1)
+        return self._ws_view(ci, self.np), self._ws_view(pm, self.np), self._ws_view(co, nk + 1)
 
     def step(self, nsteps=1):
         for _ in range(nsteps):

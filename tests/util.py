@@ -21,9 +21,41 @@ def oracle_state(pl):
     return st, E, B
 
 
-def gpu_cols(sim):
+def gpu_cols(sim, export=True):
+    """the current particle columns as numpy arrays; export=True first converts the internal form
+    (in-cell offsets) back to absolute fp32 positions through psc_particles_export"""
+    if export:
+        sim.psc.particles_export()
     cur = sim.current()
     return {k: v.cpu().numpy() for k, v in cur.items() if v is not None}
+
+
+def key_to_cell(key, n, block):
+    """inverse of the sort key of PAPER.md:593 as the oracle defines it:
+    key = block_index * cells_per_block + cell_in_block, both x-fastest"""
+    n = np.asarray(n)
+    bs = np.asarray(block)
+    nb = n // bs
+    cpb = int(bs.prod())
+    b, l = key // cpb, key % cpb
+    bc = (b % nb[0], (b // nb[0]) % nb[1], b // (nb[0] * nb[1]))
+    lc = (l % bs[0], (l // bs[0]) % bs[1], l // (bs[0] * bs[1]))
+    return [bc[d] * bs[d] + lc[d] for d in range(3)]
+
+
+def gpu_positions_f64(sim, block=(0, 0, 0)):
+    """positions of the current particles in fp64 from the internal form (cell + offset) * dx --
+    no export rounding; invariant coordinates are returned as stored"""
+    assert sim.psc.particles_form() == 1
+    cur = sim.current()
+    key = sim.keys().cpu().numpy().astype(np.int64)
+    pl = sim.plasma
+    cells = key_to_cell(key, pl.n, library_block(pl.n, block))
+    out = []
+    for d, c in enumerate(("x", "y", "z")):
+        o = cur[c].cpu().numpy().astype(np.float64)
+        out.append(np.ascontiguousarray(o if pl.n[d] == 1 else (cells[d] + o) * pl.dx[d]))
+    return out
 
 
 def periodic_dist(a, b, L):
@@ -42,6 +74,17 @@ def rel_maxnorm(got, ref):
             continue
         worst = max(worst, err / den)
     return worst
+
+
+def rel_fieldnorm(got, ref):
+    """max |got - ref| over all components / max |ref| over all components: the north_star's
+    'relative to the field's max-norm' read literally (a vector field has one max-norm)"""
+    den = np.abs(ref).max()
+    err = np.abs(got.astype(np.float64) - ref).max()
+    if den == 0.0:
+        assert err == 0.0
+        return 0.0
+    return err / den
 
 
 def smooth_fields(pl, amp, seed):
