@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- particle-updates/s of the full PIC step (psc_step, Fig. 8 of arXiv:1310.7866) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl psc|reference]
+
+One "step" is one psc_step over the whole synthetic plasma (sort -> B half -> fused gather/push/
+deposit -> B half -> J exchange -> E), all particles and fields resident in HBM.  The default
+workload is BASELINE.json configs[1] (2-d thermal plasma, 1x1024x1024 cells, 100 particles per
+cell per species, 209 715 200 particles); the particle arrays (6.7 GB per column set) exceed the
+126 MB L2 many times over, so no explicit L2 flush is needed between steps.
+
+Rank layout: the path does not shard (replicas only), so with --gpus N
+every rank steps its own replica, seeded per rank; value = particles of all ranks * K / max time.
+
+The JSON line carries
+  value        device-resident whole-job throughput, CUDA events around the K steps, max over ranks
+  e2e          the same metric through psc_step_host with pinned HOST buffers: every step copies
+               all particle columns + E, B to the device, steps once, and copies particles, E, B, J
+               back (bytes counted from the buffers)
+  roofline     the fused gather-push-deposit kernel: algorithmic bytes / CUDA-event duration of
+               the kernel launch (psc_profile brackets, on the launching stream, inside the timed
+               region) against MEASURED_PEAKS.json's copy bandwidth
+  cpu_baseline the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded
+               sample of the same workload (rank 0, N = 1 only)
+--impl reference times only the oracle (there is no reference code).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "particle-updates/sec per full PIC step"
+UNIT = "particle-updates/s"
+WORKLOADS = {
+    1: "config1: 2-d yz thermal plasma 1x64x64, 16 ppc/species, order 1",
+    2: "config2: 2-d yz thermal plasma 1x1024x1024, 100 ppc/species (209715200 particles), order 1",
+    3: "config3: 2-d yz double Harris sheet 1x512x1024, 10..110 ppc/species, order 1",
+    4: "config4: 3-d thermal plasma 128^3, 50 ppc/species (209715200 particles), order 1",
+    5: "config5: 3-d relativistic beam-plasma 64x64x256, 80 ppc, order 2 (TSC)",
+}
+# algorithmic bytes per particle of the fused kernel
+PUSH_BYTES = {2: 48, 3: 56}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons of one GPU, sampled every 200 ms while running"""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [v.strip() for v in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(cfg, sample_grid, nsteps):
+    """the fp64 oracle on a bounded sample of the workload -> (updates/s, threads, particles)"""
+    import numpy as np
+
+    import psc_inputs
+    from oracle.psc_oracle import Oracle
+
+    pl = psc_inputs.make_config(cfg, scale=sample_grid)
+    orc = Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m)
+    f64 = lambda t: np.ascontiguousarray(t.cpu().numpy().astype(np.float64))
+    E, B, J = f64(pl.E), f64(pl.B), orc.zeros_field()
+    cols = [f64(getattr(pl, k)) for k in ("x", "y", "z", "ux", "uy", "uz", "qw")]
+    sp = np.ascontiguousarray(pl.species.numpy())
+    state = (orc, E, B, J, cols, sp)
+    t0 = time.perf_counter()
+    orc.step(E, B, J, *cols, sp, nsteps)
+    dt = time.perf_counter() - t0
+    return pl.n_particles * nsteps / dt, orc.num_threads(), pl.n_particles, state
+
+
+def sample_grids(cfg):
+    if cfg in (1, 2):
+        return [(1, 256, 256), (1, 128, 128), (1, 64, 64), (1, 32, 32)]
+    if cfg == 3:
+        return [(1, 128, 256), (1, 64, 128), (1, 32, 64)]
+    if cfg == 4:
+        return [(32, 32, 32), (16, 16, 16), (8, 8, 8)]
+    return [(16, 16, 64), (8, 8, 32), (8, 8, 16)]
+
+
+def ppc_of(cfg):
+    return {1: 32, 2: 200, 3: 28, 4: 100, 5: 80}[cfg]
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, each step a bounded sample of the workload"""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import numpy as np  # noqa: F401
+
+    total = args.steps + args.warmup
+    grids = sample_grids(args.config)
+    grid = grids[-1]
+    for g in grids:  # largest sample that keeps the whole run near two minutes at ~3e6 updates/s
+        if g[0] * g[1] * g[2] * ppc_of(args.config) * total <= 3.5e8:
+            grid = g
+            break
+    import psc_inputs
+    from oracle.psc_oracle import Oracle
+
+    pl = psc_inputs.make_config(args.config, scale=grid)
+    orc = Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m)
+    import numpy as np
+    f64 = lambda t: np.ascontiguousarray(t.cpu().numpy().astype(np.float64))
+    E, B, J = f64(pl.E), f64(pl.B), orc.zeros_field()
+    cols = [f64(getattr(pl, k)) for k in ("x", "y", "z", "ux", "uy", "uz", "qw")]
+    sp = np.ascontiguousarray(pl.species.numpy())
+    if args.warmup:
+        orc.step(E, B, J, *cols, sp, args.warmup)
+    t0 = time.perf_counter()
+    orc.step(E, B, J, *cols, sp, args.steps)
+    dt = time.perf_counter() - t0
+    val = pl.n_particles * args.steps / dt
+    sample = "grid %dx%dx%d of the same recipe, %d particles per step" % (grid + (pl.n_particles,))
+    out = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": WORKLOADS[args.config], "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(out), flush=True)
+    return 0
+
+
+def run_psc(args):
+    import torch
+    import torch.distributed as dist
+
+    import psc_inputs
+    from paper_1310_7866_b200 import COLUMNS
+    from paper_1310_7866_b200.harness import Simulation
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: there is no CPU fallback"
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    scale = tuple(int(v) for v in args.scale.split("x")) if args.scale else None
+    t_gen = time.perf_counter()
+    pl = psc_inputs.make_config(args.config, device=dev, scale=scale)
+    if world > 1:  # replicas: same recipe, rank-dependent seed offset is not needed for timing
+        pass
+    sim = Simulation(pl, device=dev, with_id=False)
+    npart = sim.np
+    ndim = sum(1 for v in pl.n if v > 1)
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t_gen
+    psc = sim.psc
+    psc.set_option("profile", 1)
+
+    # ---- device-resident: W warm-up steps, K timed steps ---------------------------------------
+    for _ in range(args.warmup):
+        psc.step()
+    barrier()
+    psc.profile()          # reset the phase accumulators
+    l0 = psc.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(args.steps):
+        psc.step()
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    launches = psc.launch_count() - l0
+    prof = psc.profile()
+    flags = psc.status()
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = npart * world * args.steps / (ms_max * 1e-3)
+
+    # ---- roofline of the fused gather-push-deposit kernel ------------------------------------
+    peak, peak_src = peaks()
+    push_ms, push_n = prof["push"]
+    push_avg = push_ms / max(push_n, 1)
+    bytes_pp = PUSH_BYTES[ndim]
+    achieved = bytes_pp * npart / (push_avg * 1e-3) / 1e9 if push_n else 0.0
+    roofline = {"bound": "hbm", "kernel": "k_push%d" % pl.order, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
+                "share_of_step": push_ms / ms if ms else None}
+    tr = os.path.join(ROOT, "profiles", "traffic_config%d.json" % args.config)
+    if os.path.exists(tr) and scale is None:  # dram bytes per launch from the committed ncu capture
+        with open(tr) as f:
+            roofline["traffic"] = json.load(f).get("dram_bytes_per_launch")
+    phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
+
+    # ---- end to end through psc_step_host with pinned host buffers -----------------------------
+    e2e = None
+    if not args.no_e2e:
+        sim.psc.particles_export()
+        cur = sim.current()
+        host = {}
+        for c in COLUMNS:
+            tns = cur[c]
+            host[c] = None if tns is None else torch.empty(tns.shape, dtype=tns.dtype, pin_memory=True)
+            if tns is not None:
+                host[c].copy_(tns)
+        hE = torch.empty(sim.E.shape, dtype=torch.float32, pin_memory=True).copy_(sim.E)
+        hB = torch.empty(sim.B.shape, dtype=torch.float32, pin_memory=True).copy_(sim.B)
+        hJ = torch.empty(sim.J.shape, dtype=torch.float32, pin_memory=True)
+        torch.cuda.synchronize()
+        pbytes = sum(h.numel() * h.element_size() for h in host.values() if h is not None)
+        fbytes = hE.numel() * 4
+        h2d, d2h = pbytes + 2 * fbytes, pbytes + 3 * fbytes
+        ksteps = max(1, min(args.steps, args.e2e_steps))
+        psc.step_host(npart, host, hE, hB, hJ, 1)     # warm-up (pages, first-touch)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(ksteps):
+            psc.step_host(npart, host, hE, hB, hJ, 1)
+        e1.record()
+        barrier()
+        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": npart * world * ksteps / (float(te.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
+               "api": "psc_step_host (pinned host columns + fields in, particles + E,B,J out)"}
+        flags |= psc.status()
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config] + (" [grid %s]" % args.scale if scale else ""),
+                   "particles_per_gpu": npart, "grid": list(pl.n), "order": pl.order,
+                   "parallelism": "replicas" if world > 1 else "single-gpu",
+                   "l2": "inputs exceed L2 (particle columns %.2f GB vs 126 MB)" % (npart * 32 / 1e9)
+                   if npart * 32 > 4 * 126e6 else "inputs smaller than L2 (small config)",
+                   "setup_s": round(t_gen, 1)},
+        "clocks": clocks, "gpu_launches": launches, "status_flags": flags,
+        "phase_ms": phases, "roofline": roofline, "e2e": e2e,
+    }
+
+    # ---- the oracle on the host cores (rank 0, N = 1 only) --------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu:
+        grid = sample_grids(args.config)[0 if not args.quick_cpu else -1]
+        rate, threads, nsamp, _ = oracle_rate(args.config, grid, args.cpu_steps)
+        out["cpu_baseline"] = {
+            "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "grid %dx%dx%d of the same recipe (%d particles), %d steps"
+                      % (grid + (nsamp, args.cpu_steps))}
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0 if flags == 0 else 1
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="psc", choices=["psc", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--scale", default=None, help="NXxNYxNZ: smaller grid of the same recipe (debug)")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-steps", type=int, default=2)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--quick-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "psc":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_psc(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

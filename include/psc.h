@@ -181,6 +181,25 @@ int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);
 int64_t psc_launch_count(const psc_ctx *ctx);
 /* Last CUDA runtime error code seen by this context (0 if none). */
 int psc_last_cuda_error(const psc_ctx *ctx);
+/* Per-phase device timing.  After psc_set_option(ctx, "profile", 1) every call brackets its
+ * phases with CUDA events recorded on the call's stream (no synchronisation while running; a full
+ * event ring is drained with one cudaEventSynchronize).  psc_profile synchronises `stream`, adds
+ * the elapsed milliseconds of every completed bracket to ms[PSC_PH_COUNT] and the number of
+ * brackets to count[PSC_PH_COUNT] (host arrays), and resets the accumulators.  PSC_PH_SORT spans
+ * the whole psc_particles_sort (PSC_PH_SORT_* are its parts); PSC_PH_PUSH is the fused
+ * gather-push-deposit kernel launch alone. */
+#define PSC_PH_SORT 0
+#define PSC_PH_PUSH 1
+#define PSC_PH_J_ZERO 2
+#define PSC_PH_FIELD_B 3
+#define PSC_PH_J_EXCHANGE 4
+#define PSC_PH_FIELD_E 5
+#define PSC_PH_SORT_COUNT 6
+#define PSC_PH_SORT_SCAN 7
+#define PSC_PH_SORT_RANK 8
+#define PSC_PH_SORT_REORDER 9
+#define PSC_PH_COUNT 16
+int psc_profile(psc_ctx *ctx, void *stream, double *ms, int64_t *count);
 /* Selects kernel variants for experiments; 0 = default.  Host only. */
 int psc_set_option(psc_ctx *ctx, const char *name, int64_t value);
 const char *psc_strerror(int code);

@@ -16,6 +16,9 @@ PSC_OK = 0
 PSC_E, PSC_B, PSC_J = 0, 1, 2
 PSC_F_OOB, PSC_F_MOVED_GT_1CELL, PSC_F_NAN, PSC_F_NOT_IN_TILE = 1, 2, 4, 8
 PSC_GHOST = 2
+PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
+          "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9}
+PSC_PH_COUNT = 16
 
 EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
@@ -23,7 +26,7 @@ EXPORTS = [
     "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step", "psc_step_host",
     "psc_sort_result", "psc_particles_current", "psc_particles_form", "psc_particles_keys",
     "psc_particles_export", "psc_status", "psc_launch_count",
-    "psc_last_cuda_error", "psc_set_option", "psc_strerror", "psc_version",
+    "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
 ]
 
 COLUMNS = ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id")
@@ -92,6 +95,7 @@ def lib():
         L.psc_launch_count.argtypes = [C.c_void_p]
         L.psc_launch_count.restype = C.c_int64
         L.psc_last_cuda_error.argtypes = [C.c_void_p]
+        L.psc_profile.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         L.psc_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
         L.psc_strerror.argtypes = [C.c_int]
         L.psc_strerror.restype = C.c_char_p
@@ -241,6 +245,13 @@ class Psc:
         f = C.c_uint32()
         self._check(lib().psc_status(self._h, _stream(stream), C.byref(f)), "psc_status")
         return int(f.value)
+
+    def profile(self, stream=None):
+        """{phase: (total ms, brackets)} since the last call (needs set_option("profile", 1))"""
+        ms = (C.c_double * PSC_PH_COUNT)()
+        cnt = (C.c_int64 * PSC_PH_COUNT)()
+        self._check(lib().psc_profile(self._h, _stream(stream), ms, cnt), "psc_profile")
+        return {k: (float(ms[i]), int(cnt[i])) for k, i in PHASES.items()}
 
     def launch_count(self):
         return int(lib().psc_launch_count(self._h))

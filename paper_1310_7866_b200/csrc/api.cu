@@ -19,7 +19,36 @@ Cols to_cols(const psc_particle_cols *c) {
   return o;
 }
 
+void prof_drain(psc_ctx *c, int ph) {
+  Prof &pr = c->prof;
+  const int n = pr.used[ph];
+  if (n == 0) return;
+  cudaEventSynchronize(pr.ev[ph][n - 1][1]);
+  for (int i = 0; i < n; i++) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, pr.ev[ph][i][0], pr.ev[ph][i][1]) == cudaSuccess) {
+      pr.ms[ph] += (double)ms;
+      pr.cnt[ph]++;
+    }
+  }
+  pr.used[ph] = 0;
+}
+
 }  // namespace
+
+void psc_prof_begin(psc_ctx *c, int ph, cudaStream_t s) {
+  Prof &pr = c->prof;
+  if (!pr.on) return;
+  if (pr.used[ph] == PSC_PROF_RING) prof_drain(c, ph);
+  cudaEventRecord(pr.ev[ph][pr.used[ph]][0], s);
+}
+
+void psc_prof_end(psc_ctx *c, int ph, cudaStream_t s) {
+  Prof &pr = c->prof;
+  if (!pr.on) return;
+  cudaEventRecord(pr.ev[ph][pr.used[ph]][1], s);
+  pr.used[ph]++;
+}
 
 extern "C" {
 
@@ -131,6 +160,12 @@ int psc_create(const psc_params *p, psc_ctx **out) {
 
 void psc_destroy(psc_ctx *c) {
   if (!c) return;
+  if (c->prof.have_events)
+    for (int ph = 0; ph < PSC_PH_COUNT; ph++)
+      for (int i = 0; i < PSC_PROF_RING; i++) {
+        cudaEventDestroy(c->prof.ev[ph][i][0]);
+        cudaEventDestroy(c->prof.ev[ph][i][1]);
+      }
   if (c->d_flags) cudaFree(c->d_flags);
   free(c);
 }
@@ -206,6 +241,7 @@ int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const 
 int psc_particles_sort(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  ProfScope ps(c, PSC_PH_SORT, (cudaStream_t)stream);
   return psc_sort_run(c, (cudaStream_t)stream);
 }
 
@@ -222,8 +258,14 @@ int psc_push_particles(psc_ctx *c, void *stream) {
 int psc_push_fields(psc_ctx *c, int which, float frac, void *stream) {
   if (!c || !(frac > 0.f)) return PSC_ERR_INVALID_ARG;
   if (!c->have_fields) return PSC_ERR_NOT_BOUND;
-  if (which == PSC_B) return psc_fields_push_b(c, frac, (cudaStream_t)stream);
-  if (which == PSC_E) return psc_fields_push_e(c, frac, (cudaStream_t)stream);
+  if (which == PSC_B) {
+    ProfScope ps(c, PSC_PH_FIELD_B, (cudaStream_t)stream);
+    return psc_fields_push_b(c, frac, (cudaStream_t)stream);
+  }
+  if (which == PSC_E) {
+    ProfScope ps(c, PSC_PH_FIELD_E, (cudaStream_t)stream);
+    return psc_fields_push_e(c, frac, (cudaStream_t)stream);
+  }
   return PSC_ERR_INVALID_ARG;
 }
 
@@ -238,6 +280,7 @@ int psc_fill_ghosts(psc_ctx *c, int which, void *stream) {
 int psc_exchange_j(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_fields) return PSC_ERR_NOT_BOUND;
+  ProfScope ps(c, PSC_PH_J_EXCHANGE, (cudaStream_t)stream);
   int rc = psc_fields_fold(c, c->J, (cudaStream_t)stream);
   if (rc) return rc;
   return psc_fields_fill_ghosts(c, c->J, (cudaStream_t)stream);
@@ -347,6 +390,19 @@ int psc_status(psc_ctx *c, void *stream, uint32_t *flags) {
   return PSC_OK;
 }
 
+int psc_profile(psc_ctx *c, void *stream, double *ms, int64_t *count) {
+  if (!c || !ms || !count) return PSC_ERR_INVALID_ARG;
+  PSC_CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+  for (int ph = 0; ph < PSC_PH_COUNT; ph++) {
+    prof_drain(c, ph);
+    ms[ph] = c->prof.ms[ph];
+    count[ph] = c->prof.cnt[ph];
+    c->prof.ms[ph] = 0.0;
+    c->prof.cnt[ph] = 0;
+  }
+  return PSC_OK;
+}
+
 int64_t psc_launch_count(const psc_ctx *c) { return c ? c->launches : 0; }
 int psc_last_cuda_error(const psc_ctx *c) { return c ? c->last_err : 0; }
 
@@ -354,7 +410,19 @@ int psc_set_option(psc_ctx *c, const char *name, int64_t value) {
   if (!c || !name) return PSC_ERR_INVALID_ARG;
   if (!strcmp(name, "push_variant")) c->opt_push_variant = (int)value;
   else if (!strcmp(name, "threads")) c->opt_threads = (int)value;
-  else if (!strcmp(name, "clear_flags")) {
+  else if (!strcmp(name, "profile")) {
+    Prof &pr = c->prof;
+    if (value && !pr.have_events) {
+      for (int ph = 0; ph < PSC_PH_COUNT; ph++)
+        for (int i = 0; i < PSC_PROF_RING; i++)
+          for (int k = 0; k < 2; k++)
+            if (cudaEventCreate(&pr.ev[ph][i][k]) != cudaSuccess) return PSC_ERR_CUDA;
+      pr.have_events = 1;
+    }
+    if (!value)
+      for (int ph = 0; ph < PSC_PH_COUNT; ph++) prof_drain(c, ph);
+    pr.on = value != 0;
+  } else if (!strcmp(name, "clear_flags")) {
     if (cudaMemset(c->d_flags, 0, 4) != cudaSuccess) return PSC_ERR_CUDA;
   } else return PSC_ERR_INVALID_ARG;
   return PSC_OK;

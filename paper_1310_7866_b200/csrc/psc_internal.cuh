@@ -37,8 +37,20 @@ struct Cols {
 enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1 };
 enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
 
+// per-phase CUDA-event timing (psc_profile): a ring of start/stop pairs per phase
+constexpr int PSC_PROF_RING = 64;
+struct Prof {
+  int on;
+  int have_events;
+  cudaEvent_t ev[PSC_PH_COUNT][PSC_PROF_RING][2];
+  int used[PSC_PH_COUNT];
+  double ms[PSC_PH_COUNT];
+  int64_t cnt[PSC_PH_COUNT];
+};
+
 struct psc_ctx {
   GridDesc gd;
+  Prof prof;
   float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
   float *E, *B, *J;
   Cols cols[2];
@@ -82,6 +94,15 @@ struct psc_ctx {
   } while (0)
 
 static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// api.cu: phase brackets (no-ops unless profiling is on)
+void psc_prof_begin(psc_ctx *c, int phase, cudaStream_t s);
+void psc_prof_end(psc_ctx *c, int phase, cudaStream_t s);
+struct ProfScope {
+  psc_ctx *c; int ph; cudaStream_t s;
+  ProfScope(psc_ctx *c_, int ph_, cudaStream_t s_) : c(c_), ph(ph_), s(s_) { psc_prof_begin(c, ph, s); }
+  ~ProfScope() { psc_prof_end(c, ph, s); }
+};
 
 // fields.cu
 int psc_fields_push_b(psc_ctx *c, float frac, cudaStream_t s);

@@ -324,8 +324,11 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const bool d3 = gd.n[0] > 1 && gd.n[1] > 1 && gd.n[2] > 1;
   const bool d2yz = gd.n[0] == 1 && gd.n[1] > 1 && gd.n[2] > 1;
   if (!d3 && !d2yz) return PSC_ERR_UNSUPPORTED;  // 2-d runs are yz-plane runs
-  PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
-  c->launches++;
+  {
+    ProfScope ps(c, PSC_PH_J_ZERO, s);
+    PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
+    c->launches++;
+  }
   if (c->np == 0) return PSC_OK;
   int fvol = 1, jvol = 1;
   for (int d = 0; d < 3; d++)
@@ -338,6 +341,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &p = c->cols[c->cur];
   const int threads = c->opt_threads > 0 ? c->opt_threads : PUSH_THREADS;
+  ProfScope ps(c, PSC_PH_PUSH, s);
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);

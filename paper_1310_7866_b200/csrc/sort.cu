@@ -435,11 +435,14 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
   c->launches += 2;
+  psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
   if (c->form == PSC_FORM_ABS)
     k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, key_in, c->cursor, c->d_flags);
   else
     k_hist<<<pblocks, SORT_THREADS, 0, s>>>(n, nk, key_in, c->cursor, c->d_flags);
   PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_COUNT, s);
+  psc_prof_begin(c, PSC_PH_SORT_SCAN, s);
   const int sblocks = (int)cdiv64(nk, SCAN_TILE);
   k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, c->cell_offsets, c->scan_tmp);
   PSC_LAUNCH_CHECK(c);
@@ -447,6 +450,8 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
   PSC_LAUNCH_CHECK(c);
   k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->cursor, c->scan_tmp, sblocks);
   PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_SCAN, s);
+  psc_prof_begin(c, PSC_PH_SORT_RANK, s);
   k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, key_in, c->cursor, c->perm);
   PSC_LAUNCH_CHECK(c);
   const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
@@ -464,11 +469,14 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
                                                               c->d_flags + 1);
     PSC_LAUNCH_CHECK(c);
   }
+  psc_prof_end(c, PSC_PH_SORT_RANK, s);
+  psc_prof_begin(c, PSC_PH_SORT_REORDER, s);
   if (c->form == PSC_FORM_ABS)
     k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
   else
     k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
   PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_REORDER, s);
   c->cur ^= 1;
   c->kcur ^= 1;
   c->form = PSC_FORM_REL;
