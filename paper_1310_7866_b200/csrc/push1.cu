@@ -151,12 +151,182 @@ __device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TileGeo
   }
 }
 
+// ---- warp-level reduction of the home-cell currents -------------------------------------------
+// The particle list is cell-ordered, so the 32 lanes of a warp mostly sit in ONE cell and their
+// first trajectory segment deposits onto the same 8 (2-d) / 12 (3-d) J points.  Summing those in
+// registers and issuing one shared-memory add per point per warp replaces 32-way conflicting
+// atomics (shared fp32 atomicAdd is a compare-and-swap loop on sm_100a: ATOMS.CAST.SPIN) by
+// shuffles.  The reduction halves the number of live values at every butterfly stage
+// ("transpose-reduce"): 9 shuffles for 8 values, 13 for 12, instead of 5 per value.
+
+__device__ __forceinline__ float xadd(bool up, float lo, float hi, int m) {
+  // lanes with `up` keep hi and hand lo to their partner; the others keep lo and hand over hi
+  return (up ? hi : lo) + __shfl_xor_sync(0xffffffffu, up ? lo : hi, m);
+}
+
+// returns, in every lane, the warp total of v[(lane >> 2) & 7]
+__device__ __forceinline__ float warp_reduce8(const float (&v)[8], int lane) {
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4;
+  float w[4], u[2];
+#pragma unroll
+  for (int i = 0; i < 4; i++) w[i] = xadd(b4, v[i], v[i + 4], 16);
+#pragma unroll
+  for (int i = 0; i < 2; i++) u[i] = xadd(b3, w[i], w[i + 2], 8);
+  float t = xadd(b2, u[0], u[1], 4);
+  t += __shfl_xor_sync(0xffffffffu, t, 2);
+  t += __shfl_xor_sync(0xffffffffu, t, 1);
+  return t;
+}
+
+// returns the warp total of v[red12_index(lane)]
+__device__ __forceinline__ int red12_index(int lane) {
+  return ((lane & 16) ? 6 : 0) + ((lane & 8) ? 3 : 0) + ((lane & 2) ? 2 : ((lane & 4) ? 1 : 0));
+}
+__device__ __forceinline__ float warp_reduce12(const float (&v)[12], int lane) {
+  const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
+  float w[6], u[3];
+#pragma unroll
+  for (int i = 0; i < 6; i++) w[i] = xadd(b4, v[i], v[i + 6], 16);
+#pragma unroll
+  for (int i = 0; i < 3; i++) u[i] = xadd(b3, w[i], w[i + 3], 8);
+  const float t0 = xadd(b2, u[0], u[1], 4);
+  const float t1 = u[2] + __shfl_xor_sync(0xffffffffu, u[2], 4);
+  float r = xadd(b1, t0, t1, 2);
+  r += __shfl_xor_sync(0xffffffffu, r, 1);
+  return r;
+}
+
+// in-cell VB currents of one segment a -> b (both in the coordinates of the segment's cell), in
+// the order the reductions and the per-lane J offsets use:
+//   3-d: jx{(y,z),(y+1,z),(y,z+1),(y+1,z+1)}  jy{(z,x),(z+1,x),(z,x+1),(z+1,x+1)}
+//        jz{(x,y),(x+1,y),(x,y+1),(x+1,y+1)}
+//   2-d: jx{(y,z),(y+1,z),(y,z+1),(y+1,z+1)}  jy{z,z+1}  jz{y,y+1}
+template <bool D3>
+__device__ __forceinline__ void vb_values(float (&v)[D3 ? 12 : 8], float ax, float ay, float az,
+                                          float bx, float by, float bz, float tau, float fx,
+                                          float fy, float fz, float qvx) {
+  const float my = 0.5f * (ay + by), mz = 0.5f * (az + bz);
+  const float dy = by - ay, dz = bz - az;
+  if (D3) {
+    const float mx = 0.5f * (ax + bx), dx = bx - ax;
+    {
+      const float c = fx * dx, h = dy * dz * (1.0f / 12.0f);
+      v[0] = c * ((1.f - my) * (1.f - mz) + h);
+      v[1] = c * (my * (1.f - mz) - h);
+      v[2] = c * ((1.f - my) * mz - h);
+      v[3] = c * (my * mz + h);
+    }
+    {
+      const float c = fy * dy, h = dz * dx * (1.0f / 12.0f);
+      v[4] = c * ((1.f - mz) * (1.f - mx) + h);
+      v[5] = c * (mz * (1.f - mx) - h);
+      v[6] = c * ((1.f - mz) * mx - h);
+      v[7] = c * (mz * mx + h);
+    }
+    {
+      const float c = fz * dz, h = dx * dy * (1.0f / 12.0f);
+      v[8] = c * ((1.f - mx) * (1.f - my) + h);
+      v[9] = c * (mx * (1.f - my) - h);
+      v[10] = c * ((1.f - mx) * my - h);
+      v[11] = c * (mx * my + h);
+    }
+  } else {
+    {
+      const float c = qvx * tau, h = dy * dz * (1.0f / 12.0f);
+      v[0] = c * ((1.f - my) * (1.f - mz) + h);
+      v[1] = c * (my * (1.f - mz) - h);
+      v[2] = c * ((1.f - my) * mz - h);
+      v[3] = c * (my * mz + h);
+    }
+    {
+      const float c = fy * dy;
+      v[4] = c * (1.f - mz);
+      v[5] = c * mz;
+    }
+    {
+      const float c = fz * dz;
+      v[6] = c * (1.f - my);
+      v[7] = c * my;
+    }
+  }
+}
+
+// Walks the straight line a -> a + dd (cells; at most one face crossing per direction because
+// dt <= dx/2) and deposits every segment from number `first_seg` on with
+// shared-memory atomics.  first_seg = 1 is the slow path of the kernel below: segment 0 (inside
+// the home cell) has already gone through the warp reduction.
+template <bool D3>
+__device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TileGeom<D3> &tg, int lx,
+                                        int ly, int lz, float ax, float ay, float az, float ddx,
+                                        float ddy, float ddz, float fx, float fy, float fz,
+                                        float qvx, int first_seg) {
+  const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
+  const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+  const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+  const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+  float tx = sxd ? ((sxd > 0 ? 1.f - ax : -ax) / ddx) : 2.f;
+  float ty = syd ? ((syd > 0 ? 1.f - ay : -ay) / ddy) : 2.f;
+  float tz = szd ? ((szd > 0 ? 1.f - az : -az) / ddz) : 2.f;
+  float px = ax, py = ay, pz = az;  // segment start, in origin-cell coordinates
+  int rx = 0, ry = 0, rz = 0;       // current cell relative to the origin cell
+  float tprev = 0.f;
+#pragma unroll 1
+  for (int seg = 0; seg < (D3 ? 4 : 3); seg++) {
+    const float t = fminf(fminf(tx, ty), fminf(tz, 1.f));
+    const int which = (t >= 1.f) ? 3 : (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
+    float qx = ax + t * ddx, qy = ay + t * ddy, qz = az + t * ddz;  // segment end
+    if (which == 3) {
+      qx = endx; qy = endy; qz = endz;
+    } else if (which == 0) {
+      qx = sxd > 0 ? (float)(rx + 1) : (float)rx;
+    } else if (which == 1) {
+      qy = syd > 0 ? (float)(ry + 1) : (float)ry;
+    } else {
+      qz = szd > 0 ? (float)(rz + 1) : (float)rz;
+    }
+    if (seg >= first_seg)
+      vb_segment<D3>(sJ, tg, lx + rx, ly + ry, lz + rz, px - rx, py - ry, pz - rz, qx - rx, qy - ry,
+                     qz - rz, t - tprev, fx, fy, fz, qvx);
+    if (which == 3) break;
+    if (which == 0) { rx += sxd; tx = 2.f; }
+    else if (which == 1) { ry += syd; ty = 2.f; }
+    else { rz += szd; tz = 2.f; }
+    px = qx; py = qy; pz = qz;
+    tprev = t;
+  }
+}
+
+constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
+constexpr int QW = 8;      // words per entry
+
+template <bool D3>
+__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TileGeom<D3> &tg,
+                                            const GridDesc &gd, const int *__restrict__ sLut,
+                                            const float *__restrict__ q, int start, int n, int lane) {
+  if (lane < n) {
+    const int e = start + lane;
+    const int lc = __float_as_int(q[0 * QCAP + e]);
+    const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
+    const float ddx = q[4 * QCAP + e], ddy = q[5 * QCAP + e], ddz = q[6 * QCAP + e];
+    const float qw = q[7 * QCAP + e];
+    const int packed = sLut[lc];
+    const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
+    // 2-d: the x slots carry (unused, v_x): the out-of-plane current needs the velocity
+    const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
+    const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
+    vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
+                qvx, 1);
+  }
+  __syncwarp();
+}
+
 template <bool D3>
 __global__ void __launch_bounds__(PUSH_THREADS, 3)
 k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell_offsets,
         const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
         uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
+  constexpr int NV = D3 ? 12 : 8;
   TileGeom<D3> tg;
   tg.init(gd, blockIdx.x);
   float *sF = smem;                // [6][fvol]: Ex Ey Ez Bx By Bz
@@ -165,6 +335,9 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
   int *sKx = sLut + gd.cpb;               // key contribution of local x coordinate -1 .. bs0
   int *sKy = sKx + gd.bs[0] + 2;
   int *sKz = sKy + gd.bs[1] + 2;
+  float *sQ = (float *)(sKz + gd.bs[2] + 2);  // [warps][QW][QCAP]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  float *myQ = sQ + warp * (QW * QCAP);
 
   for (int i = threadIdx.x; i < gd.cpb; i += blockDim.x) {
     const int lx = i % gd.bs[0], t = i / gd.bs[0];
@@ -201,18 +374,49 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
   uint32_t bad = 0;
   const int kbase = blockIdx.x * gd.cpb;
 
-  for (int a = p0 + threadIdx.x; a < p1; a += blockDim.x) {
-    float ax = 0.f;
-    const float ay = ld_stream(p.y + a), az = ld_stream(p.z + a);
-    float ux = ld_stream(p.ux + a), uy = ld_stream(p.uy + a), uz = ld_stream(p.uz + a);
-    const float qw = ld_stream(p.qw + a);
-    const int sp = ld_stream(p.sp + a);
-    const int lc = ld_stream(key + a) - kbase;
-    if (D3) ax = ld_stream(p.x + a);
-    if (lc < 0 || lc >= gd.cpb) {  // not the sorted list this kernel was promised: flag, skip
-      bad |= PSC_F_NOT_IN_TILE;
-      continue;
+  // which reduced value this lane ends up holding, and the J point (relative to the cell's
+  // (lx+1, ly+1, lz+1) tile node) it belongs to
+  int my_off;
+  bool writer;
+  {
+    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1], jv = tg.jvol;
+    if (D3) {
+      const int idx = red12_index(lane);
+      const int off[12] = {0, s1, s2, s1 + s2, jv, jv + s2, jv + 1, jv + s2 + 1,
+                           2 * jv, 2 * jv + 1, 2 * jv + s1, 2 * jv + s1 + 1};
+      my_off = off[idx];
+      writer = (lane & 1) == 0 && !((lane & 2) && (lane & 4));
+    } else {
+      const int idx = (lane >> 2) & 7;
+      const int off[8] = {0, 1, s2, s2 + 1, jv, jv + s2, 2 * jv, 2 * jv + 1};
+      my_off = off[idx];
+      writer = (lane & 3) == 0;
     }
+  }
+  int qcnt = 0;  // warp-uniform: entries in this warp's queue
+
+  for (int base = p0 + warp * 32; base < p1; base += nwarps * 32) {
+    const int a = base + lane;
+    const bool act = a < p1;
+    float ax = 0.f, ay = 0.f, az = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
+    int sp = 0, lc = 0;
+    if (act) {
+      ay = ld_stream(p.y + a);
+      az = ld_stream(p.z + a);
+      ux = ld_stream(p.ux + a);
+      uy = ld_stream(p.uy + a);
+      uz = ld_stream(p.uz + a);
+      qw = ld_stream(p.qw + a);
+      sp = ld_stream(p.sp + a);
+      lc = ld_stream(key + a) - kbase;
+      if (D3) ax = ld_stream(p.x + a);
+      if (lc < 0 || lc >= gd.cpb) {  // not the sorted list this kernel was promised: flag, drop
+        bad |= PSC_F_NOT_IN_TILE;
+        lc = 0;
+        qw = 0.f;
+      }
+    }
+    lc = __shfl_sync(0xffffffffu, lc, act ? lane : 0);  // idle tail lanes: lane 0's cell, no charge
     const int packed = sLut[lc];
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
 
@@ -234,59 +438,89 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
     const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
     const float ddx = D3 ? vx * gd.dt_dx[0] : 0.f;  // displacement in cells
     const float ddy = vy * gd.dt_dx[1], ddz = vz * gd.dt_dx[2];
+    const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
+    const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+    const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+    const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+    const bool cross = (sxd | syd | szd) != 0;
 
-    // ---- Villasenor-Buneman deposit -----------------------------------------------------------
+    // ---- Villasenor-Buneman deposit: segment 0 (inside the home cell) ------------------------
     {
       const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
       const float qvx = qw * gd.inv_dV * vx;
-      const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
-      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
-      float tx = sxd ? ((sxd > 0 ? 1.f - ax : -ax) / ddx) : 2.f;
-      float ty = syd ? ((syd > 0 ? 1.f - ay : -ay) / ddy) : 2.f;
-      float tz = szd ? ((szd > 0 ? 1.f - az : -az) / ddz) : 2.f;
-      float px = ax, py = ay, pz = az;  // segment start, in origin-cell coordinates
-      int rx = 0, ry = 0, rz = 0;       // current cell relative to the origin cell
-      float tprev = 0.f;
-#pragma unroll 1
-      for (int seg = 0; seg < (D3 ? 4 : 3); seg++) {
-        const float t = fminf(fminf(tx, ty), fminf(tz, 1.f));
-        const int which = (t >= 1.f) ? 3 : (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
-        float qx = ax + t * ddx, qy = ay + t * ddy, qz = az + t * ddz;  // segment end
-        if (which == 3) {
-          qx = endx; qy = endy; qz = endz;
-        } else if (which == 0) {
-          qx = sxd > 0 ? (float)(rx + 1) : (float)rx;
-        } else if (which == 1) {
-          qy = syd > 0 ? (float)(ry + 1) : (float)ry;
-        } else {
-          qz = szd > 0 ? (float)(rz + 1) : (float)rz;
+      float qx = endx, qy = endy, qz = endz, t = 1.f;
+      if (cross) {  // same arithmetic as vb_walk's first iteration
+        const float tx = sxd ? ((sxd > 0 ? 1.f - ax : -ax) / ddx) : 2.f;
+        const float ty = syd ? ((syd > 0 ? 1.f - ay : -ay) / ddy) : 2.f;
+        const float tz = szd ? ((szd > 0 ? 1.f - az : -az) / ddz) : 2.f;
+        t = fminf(fminf(tx, ty), fminf(tz, 1.f));
+        if (t < 1.f) {
+          const int which = (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
+          qx = ax + t * ddx; qy = ay + t * ddy; qz = az + t * ddz;
+          if (which == 0) qx = sxd > 0 ? 1.f : 0.f;
+          else if (which == 1) qy = syd > 0 ? 1.f : 0.f;
+          else qz = szd > 0 ? 1.f : 0.f;
         }
-        vb_segment<D3>(sJ, tg, lx + rx, ly + ry, lz + rz, px - rx, py - ry, pz - rz, qx - rx,
-                       qy - ry, qz - rz, t - tprev, fx, fy, fz, qvx);
-        if (which == 3) break;
-        if (which == 0) { rx += sxd; tx = 2.f; }
-        else if (which == 1) { ry += syd; ty = 2.f; }
-        else { rz += szd; tz = 2.f; }
-        px = qx; py = qy; pz = qz;
-        tprev = t;
+      }
+      float v[NV];
+      vb_values<D3>(v, ax, ay, az, qx, qy, qz, t, fx, fy, fz, qvx);
+      // one reduction per distinct cell among the lanes (cell-ordered list: usually one or two)
+      unsigned todo = 0xffffffffu;
+      while (todo) {
+        const int cl = __shfl_sync(0xffffffffu, lc, __ffs(todo) - 1);
+        const bool in = lc == cl;
+        const unsigned m = __ballot_sync(0xffffffffu, in);
+        float r;
+        if (m == 0xffffffffu) {
+          if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(v), lane);
+          else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(v), lane);
+        } else {
+          float w[NV];
+#pragma unroll
+          for (int i = 0; i < NV; i++) w[i] = in ? v[i] : 0.f;
+          if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(w), lane);
+          else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(w), lane);
+        }
+        if (writer) {
+          const int pk = sLut[cl];
+          const int cx = pk & 1023, cy = (pk >> 10) & 1023, cz = pk >> 20;
+          const int node = D3 ? ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1)
+                              : (cz + 1) * tg.je[1] + (cy + 1);
+          atomicAdd(&sJ[node + my_off], r);
+        }
+        todo &= ~m;
+      }
+      // the rest of a trajectory that leaves its cell goes through the per-warp queue
+      const unsigned cm = __ballot_sync(0xffffffffu, cross);
+      if (cm) {
+        if (cross) {
+          const int e = qcnt + __popc(cm & ((1u << lane) - 1u));
+          myQ[0 * QCAP + e] = __int_as_float(lc);
+          myQ[1 * QCAP + e] = D3 ? ax : 0.f;
+          myQ[2 * QCAP + e] = ay;
+          myQ[3 * QCAP + e] = az;
+          myQ[4 * QCAP + e] = D3 ? ddx : vx;
+          myQ[5 * QCAP + e] = ddy;
+          myQ[6 * QCAP + e] = ddz;
+          myQ[7 * QCAP + e] = qw;
+        }
+        qcnt += __popc(cm);
+        __syncwarp();
+        if (qcnt >= 32) {
+          qcnt -= 32;
+          drain_queue<D3>(sJ, tg, gd, sLut, myQ, qcnt, 32, lane);
+        }
       }
     }
 
     // ---- new offset + new key (periodic wrap lives in the key tables) -----------------------
-    {
-      float by_ = ay + ddy, bz_ = az + ddz;
-      const int sy = by_ >= 1.f ? 1 : (by_ < 0.f ? -1 : 0);
-      const int sz = bz_ >= 1.f ? 1 : (bz_ < 0.f ? -1 : 0);
-      by_ = fminf(fmaxf(by_ - (float)sy, 0.f), 0.99999994f);
-      bz_ = fminf(fmaxf(bz_ - (float)sz, 0.f), 0.99999994f);
-      int nk = sKy[ly + sy + 1] + sKz[lz + sz + 1];
+    if (act) {
+      float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+      float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+      int nk = sKy[ly + syd + 1] + sKz[lz + szd + 1];
       if (D3) {
-        float bx_ = ax + ddx;
-        const int sx = bx_ >= 1.f ? 1 : (bx_ < 0.f ? -1 : 0);
-        bx_ = fminf(fmaxf(bx_ - (float)sx, 0.f), 0.99999994f);
-        nk += sKx[lx + sx + 1];
+        float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
+        nk += sKx[lx + sxd + 1];
         st_stream(p.x + a, bx_);
         if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
       } else {
@@ -301,6 +535,7 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
       if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
   }
+  if (qcnt) drain_queue<D3>(sJ, tg, gd, sLut, myQ, 0, qcnt, lane);
   if (bad) atomicOr(flags, bad);
   __syncthreads();
 
@@ -336,11 +571,12 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       fvol *= gd.bs[d] + 2;
       jvol *= gd.bs[d] + 3;
     }
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + gd.cpb + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6) * sizeof(float);
+  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH_THREADS;
+  if (threads < 32 || threads > PUSH_THREADS) return PSC_ERR_INVALID_ARG;
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + gd.cpb + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6 + (threads / 32) * QW * QCAP) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &p = c->cols[c->cur];
-  const int threads = c->opt_threads > 0 ? c->opt_threads : PUSH_THREADS;
   ProfScope ps(c, PSC_PH_PUSH, s);
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
