@@ -259,10 +259,14 @@ def run_psc(args):
                 "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                 "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
                 "share_of_step": push_ms / ms if ms else None}
-    tr = os.path.join(ROOT, "profiles", "traffic_config%d.json" % args.config)
-    if os.path.exists(tr) and scale is None:  # dram bytes per launch from the committed ncu capture
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch from the committed ncu captures
+    if os.path.exists(tr) and scale is None:
+        import csv
         with open(tr) as f:
-            roofline["traffic"] = json.load(f).get("dram_bytes_per_launch")
+            for row in csv.DictReader(f):     # the last row of this config + kernel wins
+                if int(row["config"]) == args.config and row["kernel"] == roofline["kernel"]:
+                    roofline["traffic"] = float(row["dram_bytes_per_launch"])
+                    roofline["traffic_commit"] = row["commit"]
     phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
 
     # ---- end to end through psc_step_host with pinned host buffers -----------------------------
