@@ -1,8 +1,474 @@
-// push2.cu -- second-order particles (b2 gather + Esirkepov deposit); see below.
+// push2.cu -- the fused particle loop of Fig. 8 for second-order
+// particles: gather E,B with b2 (TSC) weights (Eq. 11, 31), Boris push
+// (Eq. 27-28), move (Eq. 26), Esirkepov charge-conserving deposit, periodic wrap.
+//
+// One thread block per sort block ("supercell"); a warp takes one CELL at a time
+// and walks that cell's particle range in chunks of 32, so the cell -- and with it every tile
+// address that does not depend on the in-cell offset -- is warp-uniform.
+//
+// Stencils, relative to the particle's cell l and its in-cell offset a in [0,1) (A13,
+// A15).  Because dt <= dx/2 a particle moves less than half a cell, so the node nearest to the
+// old AND to the new position is l or l+1, and all b2 weights of both positions live on the four
+// nodes l-1 .. l+2:
+//   S0[k] = b2(a - k), S1[k] = b2(a + d - k), k = -1..2, DS = S1 - S0   (d = displacement, cells)
+// Esirkepov's density decomposition on those nodes, for component c with transverse e, f:
+//   W_c[i][je][jf] = DS_c[i] (S0_e S0_f + DS_e S0_f / 2 + S0_e DS_f / 2 + DS_e DS_f / 3)
+//                  = DS_c[i] ((S0_e + DS_e/2)(S0_f + DS_f/2) + DS_e DS_f / 12)
+//   j_c(i+1/2, je, jf) = j_c(i-1/2, je, jf) - (qw/dV)(dx_c/dt) W_c[i][je][jf],  i = -1, 0, 1
+// (the running sum starts from 0 below the stencil and returns to 0 above it because
+// sum_i DS[i] = 0).  Along the invariant direction of a 2-d run the current is
+// (qw/dV) v_x * bracket.  That is 3 x 48 (3-d) or 16 + 12 + 12 (2-d) current values per
+// particle at FIXED offsets from the cell: the 32 lanes' values are summed with a butterfly
+// "transpose-reduce" (each stage halves the number of live values per lane) and every lane adds
+// its one or two totals to the shared-memory J tile -- no same-address atomic conflicts.
+#include <limits.h>
+
 #include "push_common.cuh"
 
+namespace {
+
+constexpr int PUSH2_THREADS = 256;
+
+// b2 weights of the three points nearest to a sample at distance h in [-1/2, 1/2) from the
+// middle point (Eq. 31): points -1, 0, +1.
+__device__ __forceinline__ void tsc3(float h, float &wm, float &w0, float &wp) {
+  const float a = 0.5f - h, b = 0.5f + h;
+  wm = 0.5f * a * a;
+  w0 = 0.75f - h * h;
+  wp = 0.5f * b * b;
+}
+
+// b2 weights of offset a in (-1/2, 3/2) on the nodes -1, 0, 1, 2 relative to the cell
+__device__ __forceinline__ void tsc4(float a, float (&S)[4]) {
+  const bool up = a >= 0.5f;
+  float wm, w0, wp;
+  tsc3(up ? a - 1.0f : a, wm, w0, wp);
+  S[0] = up ? 0.f : wm;
+  S[1] = up ? wm : w0;
+  S[2] = up ? w0 : wp;
+  S[3] = up ? wp : 0.f;
+}
+
+__device__ __forceinline__ float xadd2(bool up, float lo, float hi, int m) {
+  return (up ? hi : lo) + __shfl_xor_sync(0xffffffffu, up ? lo : hi, m);
+}
+
+// Butterfly transpose-reduce of N per-lane values over the warp.  After the five stages lane L
+// holds, in r[0..R), the warp totals of the values with index red_index<N>(L, j) (or padding).
+template <int N>
+struct RedShape {
+  static constexpr int H1 = (N + 1) / 2, H2 = (H1 + 1) / 2, H3 = (H2 + 1) / 2, H4 = (H3 + 1) / 2,
+                       H5 = (H4 + 1) / 2;
+  static constexpr int R = H5;  // values per lane at the end
+};
+
+template <int N, int H>
+__device__ __forceinline__ void red_stage(const float (&in)[N], float (&out)[H], bool up, int m) {
+#pragma unroll
+  for (int i = 0; i < H; i++) out[i] = xadd2(up, in[i], (i + H < N) ? in[i + H] : 0.f, m);
+}
+
+template <int N>
+__device__ __forceinline__ void warp_reduce_n(const float (&v)[N], float (&r)[RedShape<N>::R],
+                                              int lane) {
+  using S = RedShape<N>;
+  float a[S::H1], b[S::H2], c[S::H3], d[S::H4];
+  red_stage<N, S::H1>(v, a, lane & 16, 16);
+  red_stage<S::H1, S::H2>(a, b, lane & 8, 8);
+  red_stage<S::H2, S::H3>(b, c, lane & 4, 4);
+  red_stage<S::H3, S::H4>(c, d, lane & 2, 2);
+  red_stage<S::H4, S::H5>(d, r, lane & 1, 1);
+}
+
+// index (0..N-1) of the value whose total lane `lane` holds in r[j], or -1 for padding
+template <int N>
+__device__ __forceinline__ int red_index(int lane, int j) {
+  using S = RedShape<N>;
+  const int cnt[5] = {N, S::H1, S::H2, S::H3, S::H4};
+  const int half[5] = {S::H1, S::H2, S::H3, S::H4, S::H5};
+  const int bit[5] = {16, 8, 4, 2, 1};
+  int idx = j;  // index inside the last level
+  bool ok = true;
+#pragma unroll
+  for (int l = 4; l >= 0; l--) {
+    if (lane & bit[l]) idx += half[l];
+    ok = ok && idx < cnt[l];
+  }
+  return ok ? idx : -1;
+}
+
+template <bool D3>
+struct Geom2 {
+  int o[3];     // first cell of the tile
+  int te[3];    // tile extents (fields and J alike): bs + 3 points, local point t <-> node o + t - 1
+  int tvol;
+  __device__ __forceinline__ void init(const GridDesc &gd, int tile) {
+    const int b0 = tile % gd.nb[0];
+    const int r = tile / gd.nb[0];
+    const int b1 = r % gd.nb[1], b2 = r / gd.nb[1];
+    o[0] = b0 * gd.bs[0];
+    o[1] = b1 * gd.bs[1];
+    o[2] = b2 * gd.bs[2];
+    te[0] = D3 ? gd.bs[0] + 3 : 1;
+    te[1] = gd.bs[1] + 3;
+    te[2] = gd.bs[2] + 3;
+    tvol = te[0] * te[1] * te[2];
+  }
+};
+
+// 1-d gather stencils of one particle along one direction
+struct Sten2 {
+  int tn;           // first tile point of the node-centred stencil (l + (a >= 1/2))
+  float wn[3];      // node-centred weights
+  float ws[3];      // half-staggered weights; first tile point is l
+  __device__ __forceinline__ void set(int l, float a) {
+    const bool up = a >= 0.5f;
+    tn = l + (up ? 1 : 0);
+    tsc3(up ? a - 1.0f : a, wn[0], wn[1], wn[2]);
+    tsc3(a - 0.5f, ws[0], ws[1], ws[2]);
+  }
+};
+
+template <bool D3, bool SX, bool SY, bool SZ>
+__device__ __forceinline__ float gather2(const float *__restrict__ F, const Geom2<D3> &tg, int lx,
+                                         int ly, int lz, const Sten2 &sx, const Sten2 &sy,
+                                         const Sten2 &sz) {
+  const int ty = SY ? ly : sy.tn, tz = SZ ? lz : sz.tn;
+  const float *wy = SY ? sy.ws : sy.wn, *wz = SZ ? sz.ws : sz.wn;
+  float acc = 0.f;
+  if (D3) {
+    const int tx = SX ? lx : sx.tn;
+    const float *wx = SX ? sx.ws : sx.wn;
+    const float *q = F + (tz * tg.te[1] + ty) * tg.te[0] + tx;
+    const int s1 = tg.te[0], s2 = tg.te[0] * tg.te[1];
+#pragma unroll
+    for (int kz = 0; kz < 3; kz++) {
+      float az = 0.f;
+#pragma unroll
+      for (int ky = 0; ky < 3; ky++) {
+        const float *row = q + kz * s2 + ky * s1;
+        const float ay = wx[0] * row[0] + wx[1] * row[1] + wx[2] * row[2];
+        az = fmaf(wy[ky], ay, az);
+      }
+      acc = fmaf(wz[kz], az, acc);
+    }
+  } else {
+    const float *q = F + tz * tg.te[1] + ty;
+    const int s2 = tg.te[1];
+#pragma unroll
+    for (int kz = 0; kz < 3; kz++) {
+      const float *row = q + kz * s2;
+      const float ay = wy[0] * row[0] + wy[1] * row[1] + wy[2] * row[2];
+      acc = fmaf(wz[kz], ay, acc);
+    }
+  }
+  return acc;
+}
+
+// value layouts of the per-particle current values handed to the reduction
+//   3-d, component c (transverse e, f cyclic): v[(jf * 4 + je) * 3 + i]   (48 values)
+//   2-d: jx: v[jz * 4 + jy] (16);  jy: v[jz * 3 + i] (12, flux along y);  jz: v[jy * 3 + i] (12)
+// tile offset (relative to the cell's own point (lx+1, ly+1, lz+1)) of value `idx`
+template <bool D3>
+__device__ __forceinline__ int value_offset(const Geom2<D3> &tg, int comp, int idx) {
+  const int s[3] = {1, tg.te[0], tg.te[0] * tg.te[1]};
+  if (idx < 0) return INT_MIN;
+  if (D3) {
+    const int e = (comp + 1) % 3, f = (comp + 2) % 3;
+    const int i = idx % 3, je = (idx / 3) % 4, jf = idx / 12;
+    return comp * tg.tvol + (i - 1) * s[comp] + (je - 1) * s[e] + (jf - 1) * s[f];
+  }
+  if (comp == 0) return ((idx / 4) - 1) * s[2] + ((idx % 4) - 1) * s[1];
+  if (comp == 1) return tg.tvol + ((idx / 3) - 1) * s[2] + ((idx % 3) - 1) * s[1];
+  return 2 * tg.tvol + ((idx % 3) - 1) * s[2] + ((idx / 3) - 1) * s[1];
+}
+
+template <int N>
+__device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const float (&v)[N],
+                                            const int (&off)[2], int lane) {
+  float r[RedShape<N>::R];
+  warp_reduce_n<N>(v, r, lane);
+  static_assert(RedShape<N>::R <= 2, "two totals per lane at most");
+#pragma unroll
+  for (int j = 0; j < RedShape<N>::R; j++)
+    if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
+}
+
+template <bool D3>
+__global__ void __launch_bounds__(PUSH2_THREADS, 2)
+k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell_offsets,
+        const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
+        uint32_t *__restrict__ flags) {
+  extern __shared__ float smem[];
+  Geom2<D3> tg;
+  tg.init(gd, blockIdx.x);
+  float *sF = smem;                // [6][tvol]
+  float *sJ = smem + 6 * tg.tvol;  // [3][tvol]
+  int *sKx = (int *)(sJ + 3 * tg.tvol);  // key contribution of local coordinate -1 .. bs
+  int *sKy = sKx + gd.bs[0] + 2;
+  int *sKz = sKy + gd.bs[1] + 2;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+
+  for (int i = threadIdx.x; i < gd.bs[0] + gd.bs[1] + gd.bs[2] + 6; i += blockDim.x) {
+    int d = 0, l = i;
+    if (l >= gd.bs[0] + 2) { l -= gd.bs[0] + 2; d = 1; }
+    if (d == 1 && l >= gd.bs[1] + 2) { l -= gd.bs[1] + 2; d = 2; }
+    int c = tg.o[d] + l - 1;
+    if (c < 0) c += gd.n[d];
+    if (c >= gd.n[d]) c -= gd.n[d];
+    const int b = c / gd.bs[d], ll = c - b * gd.bs[d];
+    const int bstride = d == 0 ? 1 : d == 1 ? gd.nb[0] : gd.nb[0] * gd.nb[1];
+    const int lstride = d == 0 ? 1 : d == 1 ? gd.bs[0] : gd.bs[0] * gd.bs[1];
+    sKx[i] = b * bstride * gd.cpb + ll * lstride;
+  }
+  for (int i = threadIdx.x; i < 6 * tg.tvol; i += blockDim.x) {
+    const int c = i / tg.tvol, r = i - c * tg.tvol;
+    const int tx = r % tg.te[0], t = r / tg.te[0];
+    const int ty = t % tg.te[1], tz = t / tg.te[1];
+    const int gx = D3 ? tg.o[0] + tx - 1 + gd.g[0] : 0;
+    const int gy = tg.o[1] + ty - 1 + gd.g[1], gz = tg.o[2] + tz - 1 + gd.g[2];
+    const int gi = (gz * gd.ext[1] + gy) * gd.ext[0] + gx;
+    sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
+  }
+  for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) sJ[i] = 0.f;
+
+  // which totals this lane holds after each reduction, as J-tile offsets from the cell's point
+  constexpr int NX = D3 ? 48 : 16, NY = D3 ? 48 : 12, NZ = D3 ? 48 : 12;
+  int offx[2], offy[2], offz[2];
+#pragma unroll
+  for (int j = 0; j < 2; j++) {
+    offx[j] = j < RedShape<NX>::R ? value_offset<D3>(tg, 0, red_index<NX>(lane, j)) : INT_MIN;
+    offy[j] = j < RedShape<NY>::R ? value_offset<D3>(tg, 1, red_index<NY>(lane, j)) : INT_MIN;
+    offz[j] = j < RedShape<NZ>::R ? value_offset<D3>(tg, 2, red_index<NZ>(lane, j)) : INT_MIN;
+  }
+  __syncthreads();
+
+  const float *sEx = sF, *sEy = sF + tg.tvol, *sEz = sF + 2 * tg.tvol;
+  const float *sBx = sF + 3 * tg.tvol, *sBy = sF + 4 * tg.tvol, *sBz = sF + 5 * tg.tvol;
+  const int kbase = blockIdx.x * gd.cpb;
+  uint32_t bad = 0;
+
+  for (int ci = warp; ci < gd.cpb; ci += nwarps) {
+    const int p0 = cell_offsets[kbase + ci], p1 = cell_offsets[kbase + ci + 1];
+    if (p0 >= p1) continue;
+    const int lx = ci % gd.bs[0], lt = ci / gd.bs[0];
+    const int ly = lt % gd.bs[1], lz = lt / gd.bs[1];
+    float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
+                            : (lz + 1) * tg.te[1] + (ly + 1));
+    for (int base = p0; base < p1; base += 32) {
+      const int a = base + lane;
+      const bool act = a < p1;
+      float ax = 0.25f, ay = 0.25f, az = 0.25f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
+      int sp = 0;
+      if (act) {
+        ay = ld_stream(p.y + a);
+        az = ld_stream(p.z + a);
+        ux = ld_stream(p.ux + a);
+        uy = ld_stream(p.uy + a);
+        uz = ld_stream(p.uz + a);
+        qw = ld_stream(p.qw + a);
+        sp = ld_stream(p.sp + a);
+        if (D3) ax = ld_stream(p.x + a);
+        if (ld_stream(key + a) != kbase + ci) {  // not the sorted list this kernel was promised
+          bad |= PSC_F_NOT_IN_TILE;
+          qw = 0.f;
+        }
+      }
+      // ---- gather (Eq. 11 with b2 weights; each component from its own Yee points) ---------
+      Sten2 sx, sy, sz;
+      sx.set(lx, ax);
+      sy.set(ly, ay);
+      sz.set(lz, az);
+      const float ex = gather2<D3, true, false, false>(sEx, tg, lx, ly, lz, sx, sy, sz);
+      const float ey = gather2<D3, false, true, false>(sEy, tg, lx, ly, lz, sx, sy, sz);
+      const float ez = gather2<D3, false, false, true>(sEz, tg, lx, ly, lz, sx, sy, sz);
+      const float bx = gather2<D3, false, true, true>(sBx, tg, lx, ly, lz, sx, sy, sz);
+      const float by = gather2<D3, true, false, true>(sBy, tg, lx, ly, lz, sx, sy, sz);
+      const float bz = gather2<D3, true, true, false>(sBz, tg, lx, ly, lz, sx, sy, sz);
+
+      // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
+      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, gd.qmh[sp]);
+      const float ig = rsqrtf(1.0f + ux * ux + uy * uy + uz * uz);
+      const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
+      const float endx = D3 ? ax + vx * gd.dt_dx[0] : ax;
+      const float endy = ay + vy * gd.dt_dx[1], endz = az + vz * gd.dt_dx[2];
+
+      // ---- Esirkepov deposit ------------------------------------------------------------------
+      {
+        float S0[4], S1[4];
+        float Ym[4], Yd[4], Zm[4], Zd[4];  // S0 + DS/2 and DS along y, z
+        float Ay[3], Az[3];                // running sums -f * DS along y, z
+        tsc4(ay, S0);
+        tsc4(endy, S1);
+        {
+          const float f = qw * gd.cur[1];
+          float run = 0.f;
+#pragma unroll
+          for (int k = 0; k < 4; k++) {
+            Yd[k] = S1[k] - S0[k];
+            Ym[k] = S0[k] + 0.5f * Yd[k];
+            if (k < 3) { run -= f * Yd[k]; Ay[k] = run; }
+          }
+        }
+        tsc4(az, S0);
+        tsc4(endz, S1);
+        {
+          const float f = qw * gd.cur[2];
+          float run = 0.f;
+#pragma unroll
+          for (int k = 0; k < 4; k++) {
+            Zd[k] = S1[k] - S0[k];
+            Zm[k] = S0[k] + 0.5f * Zd[k];
+            if (k < 3) { run -= f * Zd[k]; Az[k] = run; }
+          }
+        }
+        if (D3) {
+          float Xm[4], Xd[4], Ax[3];
+          tsc4(ax, S0);
+          tsc4(endx, S1);
+          {
+            const float f = qw * gd.cur[0];
+            float run = 0.f;
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+              Xd[k] = S1[k] - S0[k];
+              Xm[k] = S0[k] + 0.5f * Xd[k];
+              if (k < 3) { run -= f * Xd[k]; Ax[k] = run; }
+            }
+          }
+          float v[48];
+          // jx: transverse e = y, f = z
+#pragma unroll
+          for (int jf = 0; jf < 4; jf++)
+#pragma unroll
+            for (int je = 0; je < 4; je++) {
+              const float br = fmaf(Ym[je], Zm[jf], Yd[je] * Zd[jf] * (1.0f / 12.0f));
+#pragma unroll
+              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Ax[i] * br;
+            }
+          add_reduced<48>(cellJ, v, offx, lane);
+          // jy: e = z, f = x
+#pragma unroll
+          for (int jf = 0; jf < 4; jf++)
+#pragma unroll
+            for (int je = 0; je < 4; je++) {
+              const float br = fmaf(Zm[je], Xm[jf], Zd[je] * Xd[jf] * (1.0f / 12.0f));
+#pragma unroll
+              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Ay[i] * br;
+            }
+          add_reduced<48>(cellJ, v, offy, lane);
+          // jz: e = x, f = y
+#pragma unroll
+          for (int jf = 0; jf < 4; jf++)
+#pragma unroll
+            for (int je = 0; je < 4; je++) {
+              const float br = fmaf(Xm[je], Ym[jf], Xd[je] * Yd[jf] * (1.0f / 12.0f));
+#pragma unroll
+              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Az[i] * br;
+            }
+          add_reduced<48>(cellJ, v, offz, lane);
+        } else {
+          const float qvx = qw * gd.inv_dV * vx;
+          {
+            float v[16];
+#pragma unroll
+            for (int jz = 0; jz < 4; jz++)
+#pragma unroll
+              for (int jy = 0; jy < 4; jy++)
+                v[jz * 4 + jy] = qvx * fmaf(Ym[jy], Zm[jz], Yd[jy] * Zd[jz] * (1.0f / 12.0f));
+            add_reduced<16>(cellJ, v, offx, lane);
+          }
+          {
+            float v[12];
+#pragma unroll
+            for (int jz = 0; jz < 4; jz++)
+#pragma unroll
+              for (int i = 0; i < 3; i++) v[jz * 3 + i] = Ay[i] * Zm[jz];
+            add_reduced<12>(cellJ, v, offy, lane);
+          }
+          {
+            float v[12];
+#pragma unroll
+            for (int jy = 0; jy < 4; jy++)
+#pragma unroll
+              for (int i = 0; i < 3; i++) v[jy * 3 + i] = Az[i] * Ym[jy];
+            add_reduced<12>(cellJ, v, offz, lane);
+          }
+        }
+      }
+
+      // ---- new offset + new key (periodic wrap lives in the key tables) ---------------------
+      if (act) {
+        const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+        const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+        const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+        const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+        const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+        int nk = sKy[ly + syd + 1] + sKz[lz + szd + 1];
+        if (D3) {
+          const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
+          nk += sKx[lx + sxd + 1];
+          st_stream(p.x + a, bx_);
+          if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
+        } else {
+          nk += sKx[1];
+        }
+        st_stream(p.y + a, by_);
+        st_stream(p.z + a, bz_);
+        st_stream(p.ux + a, ux);
+        st_stream(p.uy + a, uy);
+        st_stream(p.uz + a, uz);
+        __stcs(key + a, nk);
+        if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
+          bad |= PSC_F_NAN;
+      }
+    }
+  }
+  if (bad) atomicOr(flags, bad);
+  __syncthreads();
+
+  // ---- flush the J tile to global J -----------------------------------------------------------
+  for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) {
+    const float v = sJ[i];
+    if (v == 0.f) continue;
+    const int c = i / tg.tvol, r = i - c * tg.tvol;
+    const int tx = r % tg.te[0], t = r / tg.te[0];
+    const int ty = t % tg.te[1], tz = t / tg.te[1];
+    const int gx = D3 ? tg.o[0] + tx - 1 + gd.g[0] : 0;
+    const int gy = tg.o[1] + ty - 1 + gd.g[1], gz = tg.o[2] + tz - 1 + gd.g[2];
+    atomicAdd(&J[c * gd.comp + (gz * gd.ext[1] + gy) * gd.ext[0] + gx], v);
+  }
+}
+
+}  // namespace
+
 int psc_push_order2(psc_ctx *c, cudaStream_t s) {
-  (void)c;
-  (void)s;
-  return PSC_ERR_UNSUPPORTED;
+  const GridDesc &gd = c->gd;
+  const bool d3 = gd.n[0] > 1 && gd.n[1] > 1 && gd.n[2] > 1;
+  const bool d2yz = gd.n[0] == 1 && gd.n[1] > 1 && gd.n[2] > 1;
+  if (!d3 && !d2yz) return PSC_ERR_UNSUPPORTED;  // 2-d runs are yz-plane runs (A25)
+  {
+    ProfScope ps(c, PSC_PH_J_ZERO, s);
+    PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
+    c->launches++;
+  }
+  if (c->np == 0) return PSC_OK;
+  int tvol = 1;
+  for (int d = 0; d < 3; d++)
+    if (gd.n[d] > 1) tvol *= gd.bs[d] + 3;
+  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH2_THREADS;
+  if (threads < 32 || threads > PUSH2_THREADS) return PSC_ERR_INVALID_ARG;
+  const size_t smem = (size_t)(9 * tvol + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6) * sizeof(float);
+  if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  const Cols &p = c->cols[c->cur];
+  ProfScope ps(c, PSC_PH_PUSH, s);
+  if (d3) {
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+  } else {
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+  }
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
 }

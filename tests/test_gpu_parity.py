@@ -32,6 +32,12 @@ def _small(kind):
         return psc_inputs.thermal((12, 20, 8), 5, seed=12, name="ragged3d")
     if kind == "harris":
         return psc_inputs.make_config(3, scale=(1, 32, 128))
+    if kind == "beam":                                          # config 5 recipe, order 2, 80/cell
+        return psc_inputs.make_config(5, scale=(8, 8, 32))
+    if kind == "3d-ragged-o2":
+        return psc_inputs.thermal((12, 20, 8), 5, seed=13, order=2, name="ragged3d-o2")
+    if kind == "2d-o2":                                         # order 2 in the yz plane (NEXT #2)
+        return psc_inputs.thermal((1, 24, 40), 9, seed=14, order=2, name="ragged2d-o2")
     raise ValueError(kind)
 
 
@@ -190,7 +196,9 @@ def _push_once(kind, block, amp=0.05):
 @pytest.mark.parametrize("kind,block", [("2d", (0, 0, 0)), ("2d-ragged", (1, 4, 8)),
                                         ("2d-ragged", (1, 24, 40)), ("3d", (0, 0, 0)),
                                         ("3d-ragged", (2, 4, 2)), ("3d-ragged", (1, 1, 1)),
-                                        ("harris", (1, 8, 8))])
+                                        ("harris", (1, 8, 8)), ("beam", (0, 0, 0)),
+                                        ("3d-ragged-o2", (2, 4, 2)), ("3d-ragged-o2", (1, 1, 1)),
+                                        ("2d-o2", (0, 0, 0)), ("2d-o2", (1, 3, 5))])
 def test_push_particles_matches_oracle(kind, block):
     pl, sim, orc, cols0, st, sp, J = _push_once(kind, block)
     got = gpu_cols(sim)
@@ -211,7 +219,7 @@ def test_push_particles_matches_oracle(kind, block):
     assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
 
 
-@pytest.mark.parametrize("kind", ["2d", "3d"])
+@pytest.mark.parametrize("kind", ["2d", "3d", "beam", "2d-o2"])
 def test_gpu_continuity_residual(kind):
     """(rho^{n+3/2} - rho^{n+1/2})/dt + div- j^{n+1} = 0 (Eq. 25) with the GPU's J and the GPU's
     stored fp32 positions, evaluated by the oracle's rho / div-; normalised by max|rho_s|/dt of one
@@ -231,7 +239,7 @@ def test_gpu_continuity_residual(kind):
 # ------------------------------------------------------------------------------------------------
 # closed loop: 10 psc_step, particles matched by id
 
-@pytest.mark.parametrize("kind", ["2d", "3d", "harris"])
+@pytest.mark.parametrize("kind", ["2d", "3d", "harris", "beam", "2d-o2"])
 def test_ten_steps_match_oracle(kind):
     pl = _small(kind)
     sim = _sim(pl)
