@@ -215,7 +215,7 @@ def run_psc(args):
     pl = psc_inputs.make_config(args.config, device=dev, scale=scale)
     if world > 1:  # replicas: same recipe, rank-dependent seed offset is not needed for timing
         pass
-    sim = Simulation(pl, device=dev, with_id=False)
+    sim = Simulation(pl, device=dev, with_id=False, with_x=pl.n[0] > 1)
     npart = sim.np
     ndim = sum(1 for v in pl.n if v > 1)
     torch.cuda.synchronize()

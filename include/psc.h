@@ -88,7 +88,8 @@ typedef struct {
 } psc_params;
 
 /* One set of particle columns (structure of arrays), each of length >= n.
- * `id` may be NULL in both sets (then no id is carried). */
+ * `id` may be NULL in both sets (then no id is carried).  In a 2-d (yz) run `x`, the coordinate
+ * along the invariant direction, may be NULL in both sets (then it is not carried either). */
 typedef struct {
   float *x, *y, *z;    /* positions x^{n+1/2}: absolute, or in-cell offsets (internal form) */
   float *ux, *uy, *uz; /* u^n = p/(m c) */
@@ -121,17 +122,22 @@ int psc_bind_particles(psc_ctx *ctx, int64_t n, const psc_particle_cols *primary
 /* Cell-key counting sort.  key = block-major, cell-minor; stable (ascending
  * input index inside a key).  Afterwards the CURRENT column set (psc_particles_current) holds
  * the particles in sorted order and in internal form; the two sets swap roles.  Arbitrary input
- * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))); from
- * internal-form columns (the previous sort's output advanced by psc_push_particles) the push has
- * already left each particle's new key -- its cell moved by at most one per direction
- * -- so the sort does not read positions at all. */
+ * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))).  A list
+ * that is the previous sort's output advanced by psc_push_particles is sorted from what the push
+ * left behind -- per particle the one-byte direction code of its move (a particle moves at most
+ * one cell per direction and step: 9 / 27 destination classes) and per cell the
+ * count of each code -- so the sort itself reads no particle column; the physical
+ * reorder that this call's contract demands is one more pass (psc_step leaves it to the next
+ * push's load instead). */
 int psc_particles_sort(psc_ctx *ctx, void *stream);
 
 /* The particle loop of Fig. 8 in one pass over the particles
  * (PAPER.md:603): zero J; per particle gather E,B at x^{n+1/2} (Eq. 11), Boris push
  * p^n -> p^{n+1} (Eq. 27-28), x^{n+1/2} -> x^{n+3/2} (Eq. 26), charge-conserving deposit of
  * j^{n+1}, periodic wrap (on the integer cell index).  Requires a sorted list
- * in internal form, i.e. psc_particles_sort directly before (PSC_ERR_NOT_SORTED).
+ * in internal form, i.e. psc_particles_sort directly before (PSC_ERR_NOT_SORTED).  Out of
+ * place: the advanced particles are written to the OTHER column set, which becomes the current
+ * one (psc_particles_current), in the order of the sorted list.
  * J ghosts are NOT folded on return (psc_exchange_j). */
 int psc_push_particles(psc_ctx *ctx, void *stream);
 
@@ -148,7 +154,9 @@ int psc_fill_ghosts(psc_ctx *ctx, int which, void *stream);
 
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
- * u^{n+1}. */
+ * u^{n+1}.  Same results as the calls above in that order; from the second step on the sort
+ * only builds the index (permutation + cell offsets) and the particle loop reorders on load
+ * (PAPER.md:603), so every particle column is read once and written once per step. */
 int psc_step(psc_ctx *ctx, void *stream);
 
 /* End-to-end form with HOST buffers: copies the host particle columns (n particles) and host
@@ -158,7 +166,8 @@ int psc_step(psc_ctx *ctx, void *stream);
 int psc_step_host(psc_ctx *ctx, void *stream, int64_t n, const psc_particle_cols *host,
                   float *hostE, float *hostB, float *hostJ, int nsteps);
 
-/* Inspection of the last sort.  Device pointers into the workspace, valid until the next sort:
+/* Inspection of the last sort.  Device pointers into the workspace, valid until the next sort
+ * or push:
  * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i; computed on `stream` by this
  * call), perm[n] (sorted slot s holds input particle perm[s]), cell_offsets[n_keys+1]
  * (exclusive scan of the key histogram). */
@@ -170,8 +179,9 @@ int psc_particles_current(const psc_ctx *ctx, psc_particle_cols *out);
 /* 0: absolute positions, 1: internal form (in-cell offsets + keys). */
 int psc_particles_form(const psc_ctx *ctx);
 /* Internal form only: key[n] of the current particles (cell key as defined by the sort; the cell
- * a particle's offset refers to).  Device pointer into the workspace. */
-int psc_particles_keys(const psc_ctx *ctx, const int32_t **key);
+ * a particle's offset refers to), computed on `stream` by this call from the cell offsets and
+ * the direction codes.  Device pointer into the workspace, valid until the next call. */
+int psc_particles_keys(psc_ctx *ctx, void *stream, const int32_t **key);
 /* Converts the current columns back to absolute positions x = (cell + offset) * dx, in place
  * (one fp32 rounding).  The list counts as unsorted afterwards.  No-op on absolute columns. */
 int psc_particles_export(psc_ctx *ctx, void *stream);

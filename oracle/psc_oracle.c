@@ -618,3 +618,44 @@ int orc_sort(const orc_params *p, int64_t n, const float *x, const float *y, con
   free(count);
   return 0;
 }
+
+/* The same stable counting sort with the cell of every particle GIVEN as integer
+ * coordinates -- used on a list that a push has advanced: which cell a particle is in is then a
+ * decision the GPU path has already taken in its own precision (where
+ * floating point decides an integer, both sides take that decision in the kernel's precision), and
+ * what is compared is everything that follows from it: keys, offsets, the stable permutation.
+ * Returns 0, or -1 if a cell lies outside the grid.                                             */
+int orc_sort_cells(const orc_params *p, int64_t n, const int32_t *cx, const int32_t *cy,
+                   const int32_t *cz, int32_t *cell_idx, int32_t *key, int32_t *perm,
+                   int32_t *cell_offsets) {
+  const int64_t nk = ncells(p);
+  const int32_t *cc[3] = {cx, cy, cz};
+  int nb[3], bs[3];
+  for (int d = 0; d < 3; d++) {
+    bs[d] = p->block[d];
+    nb[d] = p->n[d] / bs[d];
+  }
+  int64_t *count = (int64_t *)calloc(nk + 1, sizeof(int64_t));
+  for (int64_t a = 0; a < n; a++) {
+    int c[3];
+    for (int d = 0; d < 3; d++) {
+      c[d] = cc[d][a];
+      if (c[d] < 0 || c[d] >= p->n[d]) {
+        free(count);
+        return -1;
+      }
+    }
+    const int b[3] = {c[0] / bs[0], c[1] / bs[1], c[2] / bs[2]};
+    const int l[3] = {c[0] % bs[0], c[1] % bs[1], c[2] % bs[2]};
+    const int64_t kk = (((int64_t)b[2] * nb[1] + b[1]) * nb[0] + b[0]) * ((int64_t)bs[0] * bs[1] * bs[2]) +
+                       ((int64_t)l[2] * bs[1] + l[1]) * bs[0] + l[0];
+    key[a] = (int32_t)kk;
+    cell_idx[a] = (int32_t)(((int64_t)c[2] * p->n[1] + c[1]) * p->n[0] + c[0]);
+    count[kk + 1]++;
+  }
+  for (int64_t a = 0; a < nk; a++) count[a + 1] += count[a];
+  for (int64_t a = 0; a <= nk; a++) cell_offsets[a] = (int32_t)count[a];
+  for (int64_t a = 0; a < n; a++) perm[count[key[a]]++] = (int32_t)a; /* stable (A17) */
+  free(count);
+  return 0;
+}

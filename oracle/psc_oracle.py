@@ -51,6 +51,7 @@ def lib():
         _lib = C.CDLL(build())
         _lib.orc_num_threads.restype = C.c_int
         _lib.orc_sort.restype = C.c_int
+        _lib.orc_sort_cells.restype = C.c_int
     return _lib
 
 
@@ -182,4 +183,18 @@ class Oracle:
                             _i(cell_idx), _i(key), _i(perm), _i(offs))
         if rc != 0:
             raise ValueError("orc_sort: particle outside the domain")
+        return cell_idx, key, perm, offs
+
+    def sort_cells(self, cx, cy, cz):
+        """int32 cell coordinates in -> (cell_idx, key, perm, cell_offsets), all int32."""
+        n = cx.shape[0]
+        nk = self.n[0] * self.n[1] * self.n[2]
+        cell_idx = np.zeros(n, dtype=np.int32)
+        key = np.zeros(n, dtype=np.int32)
+        perm = np.zeros(n, dtype=np.int32)
+        offs = np.zeros(nk + 1, dtype=np.int32)
+        rc = lib().orc_sort_cells(C.byref(self.p), C.c_int64(n), _i(cx), _i(cy), _i(cz),
+                                  _i(cell_idx), _i(key), _i(perm), _i(offs))
+        if rc != 0:
+            raise ValueError("orc_sort_cells: cell outside the grid")
         return cell_idx, key, perm, offs

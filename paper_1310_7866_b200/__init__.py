@@ -88,7 +88,7 @@ def lib():
                                       C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                       C.POINTER(C.c_int64)]
         L.psc_particles_form.argtypes = [C.c_void_p]
-        L.psc_particles_keys.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.psc_particles_keys.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]
         L.psc_particles_export.argtypes = [C.c_void_p, C.c_void_p]
         L.psc_particles_current.argtypes = [C.c_void_p, C.POINTER(PscCols)]
         L.psc_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32)]
@@ -226,10 +226,10 @@ class Psc:
     def particles_form(self):
         return int(lib().psc_particles_form(self._h))
 
-    def particles_keys(self):
+    def particles_keys(self, stream=None):
         """raw device pointer of the current particles' cell keys (internal form only)"""
         k = C.c_void_p()
-        self._check(lib().psc_particles_keys(self._h, C.byref(k)), "psc_particles_keys")
+        self._check(lib().psc_particles_keys(self._h, _stream(stream), C.byref(k)), "psc_particles_keys")
         return k.value
 
     def particles_export(self, stream=None):

@@ -7,8 +7,9 @@
 
 namespace {
 
-bool cols_complete(const psc_particle_cols *c) {
-  return c->x && c->y && c->z && c->ux && c->uy && c->uz && c->qw && c->species;
+// x may be NULL when x is the invariant direction of a 2-d run (then it is not carried)
+bool cols_complete(const psc_ctx *ctx, const psc_particle_cols *c) {
+  return (c->x || ctx->gd.n[0] == 1) && c->y && c->z && c->ux && c->uy && c->uz && c->qw && c->species;
 }
 
 Cols to_cols(const psc_particle_cols *c) {
@@ -136,6 +137,7 @@ int psc_create(const psc_params *p, psc_ctx **out) {
   gd.ntiles = gd.nb[0] * gd.nb[1] * gd.nb[2];
   gd.order = p->order;
   gd.nsp = p->n_species;
+  gd.nd = is3d ? 27 : 9;
   for (int s = 0; s < p->n_species; s++) {
     c->q[s] = p->q[s];
     c->m[s] = p->m[s];
@@ -211,8 +213,9 @@ int psc_bind_fields(psc_ctx *c, float *E, float *B, float *J) {
 
 int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const psc_particle_cols *b) {
   if (!c || !a || !b || n < 0 || n > 0x7fffff00LL) return PSC_ERR_INVALID_ARG;
-  if (!cols_complete(a) || !cols_complete(b)) return PSC_ERR_INVALID_ARG;
+  if (!cols_complete(c, a) || !cols_complete(c, b)) return PSC_ERR_INVALID_ARG;
   if ((a->id == nullptr) != (b->id == nullptr)) return PSC_ERR_INVALID_ARG;
+  if ((a->x == nullptr) != (b->x == nullptr)) return PSC_ERR_INVALID_ARG;
   const void *ptrs[] = {a->x, a->y, a->z, a->ux, a->uy, a->uz, a->qw, a->species, a->id,
                         b->x, b->y, b->z, b->ux, b->uy, b->uz, b->qw, b->species, b->id};
   for (const void *p : ptrs)
@@ -224,7 +227,7 @@ int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const 
   c->have_particles = 1;
   c->state = PSC_STATE_UNSORTED;
   c->form = PSC_FORM_ABS;
-  c->kcur = 0;
+  c->ocur = 0;
   c->have_sort_result = 0;
   if (c->ws) {
     if (c->ws_bytes < psc_workspace_bytes(c, n)) {
@@ -241,18 +244,47 @@ int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const 
 int psc_particles_sort(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
-  ProfScope ps(c, PSC_PH_SORT, (cudaStream_t)stream);
-  return psc_sort_run(c, (cudaStream_t)stream);
+  cudaStream_t s = (cudaStream_t)stream;
+  ProfScope ps(c, PSC_PH_SORT, s);
+  int rc = PSC_OK;
+  if (c->state == PSC_STATE_PUSHED) rc = psc_sort_index(c, s);  // steady state: keys/indices only
+  if (rc == PSC_OK && c->state == PSC_STATE_INDEXED) return psc_sort_materialize(c, s);
+  if (rc) return rc;
+  return psc_sort_general(c, s);
+}
+
+// the sort as psc_step uses it: after a push only the index sort runs, and the physical reorder
+// is left to the next push's load
+static int sort_lazy(psc_ctx *c, cudaStream_t s) {
+  if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  ProfScope ps(c, PSC_PH_SORT, s);
+  if (c->state == PSC_STATE_PUSHED) return psc_sort_index(c, s);
+  if (c->state == PSC_STATE_INDEXED || c->state == PSC_STATE_SORTED) return PSC_OK;
+  return psc_sort_general(c, s);
 }
 
 int psc_push_particles(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
-  if (c->state != PSC_STATE_SORTED || c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
-  const int rc = c->gd.order == 1 ? psc_push_order1(c, (cudaStream_t)stream)
-                                  : psc_push_order2(c, (cudaStream_t)stream);
-  if (rc == PSC_OK) c->state = PSC_STATE_UNSORTED;
-  return rc;
+  if ((c->state != PSC_STATE_SORTED && c->state != PSC_STATE_INDEXED) || c->form != PSC_FORM_REL)
+    return PSC_ERR_NOT_SORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  {
+    ProfScope ps(c, PSC_PH_J_ZERO, s);
+    PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * c->gd.comp * sizeof(float), s));
+    c->launches++;
+  }
+  if (c->np == 0) {  // nothing to push: every cell keeps zero particles
+    PSC_CUDA_TRY(c, cudaMemsetAsync(c->dircnt, 0, (size_t)c->gd.nkeys * c->gd.nd * 4, s));
+    c->launches++;
+  } else {
+    const int rc = c->gd.order == 1 ? psc_push_order1(c, s) : psc_push_order2(c, s);
+    if (rc) return rc;
+  }
+  c->cur ^= 1;  // the kernel wrote the other column set
+  c->state = PSC_STATE_PUSHED;
+  c->have_sort_result = 0;
+  return PSC_OK;
 }
 
 int psc_push_fields(psc_ctx *c, int which, float frac, void *stream) {
@@ -291,7 +323,8 @@ int psc_exchange_j(psc_ctx *c, void *stream) {
 // update (ghost points are computed like their images), add_and_fill_ghosts_j is psc_exchange_j.
 int psc_step(psc_ctx *c, void *stream) {
   int rc;
-  if ((rc = psc_particles_sort(c, stream))) return rc;
+  if (!c) return PSC_ERR_INVALID_ARG;
+  if ((rc = sort_lazy(c, (cudaStream_t)stream))) return rc;
   if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^n -> B^{n+1/2}
   if ((rc = psc_push_particles(c, stream))) return rc;            // p, x, j^{n+1}
   if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^{n+1/2} -> B^{n+1}
@@ -304,12 +337,13 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
                   float *hB, float *hJ, int nsteps) {
   if (!c || !h || !hE || !hB || nsteps < 0) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->have_fields || !c->ws) return PSC_ERR_NOT_BOUND;
-  if (n != c->np || !cols_complete(h)) return PSC_ERR_INVALID_ARG;
+  if (n != c->np || !cols_complete(c, h)) return PSC_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)stream;
   const size_t fb = (size_t)3 * c->gd.comp * 4, pb = (size_t)n * 4;
   {
     Cols &d = c->cols[c->cur];
     if ((d.id != nullptr) != (h->id != nullptr)) return PSC_ERR_INVALID_ARG;
+    if ((d.x != nullptr) != (h->x != nullptr)) return PSC_ERR_INVALID_ARG;
     const void *src[] = {h->x, h->y, h->z, h->ux, h->uy, h->uz, h->qw, h->species, h->id};
     void *dst[] = {d.x, d.y, d.z, d.ux, d.uy, d.uz, d.qw, d.sp, d.id};
     for (int i = 0; i < 9; i++)
@@ -318,6 +352,7 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
     PSC_CUDA_TRY(c, cudaMemcpyAsync(c->B, hB, fb, cudaMemcpyHostToDevice, s));
     c->state = PSC_STATE_UNSORTED;
     c->form = PSC_FORM_ABS;
+    c->have_sort_result = 0;
     c->launches += 11;
   }
   for (int i = 0; i < nsteps; i++) {
@@ -351,18 +386,20 @@ int psc_sort_result(psc_ctx *c, void *stream, const int32_t **cell_idx, const in
     *cell_idx = c->cell_idx;
   }
   if (perm) *perm = c->perm;
-  if (cell_offsets) *cell_offsets = c->cell_offsets;
+  if (cell_offsets) *cell_offsets = c->offs[c->ocur];
   if (n_keys) *n_keys = c->gd.nkeys;
   return PSC_OK;
 }
 
 int psc_particles_form(const psc_ctx *c) { return c ? c->form : PSC_ERR_INVALID_ARG; }
 
-int psc_particles_keys(const psc_ctx *c, const int32_t **key) {
+int psc_particles_keys(psc_ctx *c, void *stream, const int32_t **key) {
   if (!c || !key) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
   if (c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
-  *key = c->key[c->kcur];
+  const int rc = psc_sort_current_keys(c, (cudaStream_t)stream);
+  if (rc) return rc;
+  *key = c->curkey;
   return PSC_OK;
 }
 

@@ -25,6 +25,7 @@ struct GridDesc {
   int ntiles;        // number of blocks
   int order;
   int nsp;
+  int nd;            // direction codes of a move: 9 (2-d) or 27 (3-d); see dir_code()
   float qmh[PSC_MAX_SPECIES];  // q_s dt / (2 m_s), the Boris h
 };
 
@@ -34,8 +35,23 @@ struct Cols {
   int32_t *id;
 };
 
-enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1 };
+// Where the particle list is in the sort / push cycle (internal form unless UNSORTED):
+//   UNSORTED  absolute positions in arbitrary order (after bind or export)
+//   SORTED    the current column set is physically in sorted order; offs[ocur] = cell offsets
+//   PUSHED    the current set is in the slot order of offs[ocur], every particle carries the
+//             direction code of its move (dcode) and dircnt holds the per-cell code counts
+//   INDEXED   the current set is still in the OLD slot order (offs[ocur^1]); perm and
+//             offs[ocur] describe the new sorted order (reorder happens on the next load)
+enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1, PSC_STATE_PUSHED = 2, PSC_STATE_INDEXED = 3 };
 enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
+
+// Direction code of a move by (sx, sy, sz) in {-1,0,1}^3 cells (a particle moves at
+// most one cell per step, so 9 (2-d) / 27 (3-d) destination classes exist).  2-d (yz plane):
+// (sy+1) + 3 (sz+1), "stay" = 4; 3-d: (sx+1) + 3 (sy+1) + 9 (sz+1), "stay" = 13.
+template <bool D3>
+__host__ __device__ __forceinline__ int dir_code(int sx, int sy, int sz) {
+  return D3 ? (sx + 1) + 3 * (sy + 1) + 9 * (sz + 1) : (sy + 1) + 3 * (sz + 1);
+}
 
 // per-phase CUDA-event timing (psc_profile): a ring of start/stop pairs per phase
 constexpr int PSC_PROF_RING = 64;
@@ -58,14 +74,15 @@ struct psc_ctx {
   int64_t np;
   int have_particles, have_fields;
   int state;
-  int form;        // PSC_FORM_ABS: absolute positions; PSC_FORM_REL: in-cell offsets + key[kcur]
-  int kcur;        // which key buffer belongs to the current column set
-  int have_sort_result;
+  int form;        // PSC_FORM_ABS: absolute positions; PSC_FORM_REL: in-cell offsets
+  int ocur;        // offs[ocur]: offsets of the latest sort
+  int have_sort_result;  // 0: none; 1: key[] holds the input keys; 2: input keys = old offs + dcode
   // workspace carve-up (all device pointers)
   void *ws;
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
-  int32_t *key[2], *perm, *cell_idx, *cell_offsets, *cursor, *scan_tmp, *big_list;
+  int32_t *key, *curkey, *perm, *cell_idx, *offs[2], *cursor, *scan_tmp, *big_list, *dircnt;
+  uint8_t *dcode;
   uint32_t *d_flags;  // owned: 16 words; [0] sticky flags, [1] big-segment counter
   int64_t launches;
   int last_err;
@@ -112,8 +129,11 @@ int psc_fields_fold(psc_ctx *c, float *F, cudaStream_t s);
 // sort.cu
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n);
 int psc_sort_carve(psc_ctx *c, int64_t n);
-int psc_sort_run(psc_ctx *c, cudaStream_t s);
+int psc_sort_general(psc_ctx *c, cudaStream_t s);      // UNSORTED | SORTED -> SORTED
+int psc_sort_index(psc_ctx *c, cudaStream_t s);        // PUSHED -> INDEXED
+int psc_sort_materialize(psc_ctx *c, cudaStream_t s);  // INDEXED -> SORTED
 int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s);
+int psc_sort_current_keys(psc_ctx *c, cudaStream_t s);  // key[] := keys of the current particles
 int psc_particles_to_abs(psc_ctx *c, cudaStream_t s);
 // push1.cu / push2.cu
 int psc_push_order1(psc_ctx *c, cudaStream_t s);

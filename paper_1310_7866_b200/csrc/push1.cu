@@ -3,9 +3,20 @@
 // move (Eq. 26), Villasenor-Buneman charge-conserving deposit, periodic wrap.
 //
 // One thread block per sort block ("supercell"): the block stages the E/B values
-// its cells can touch (tile + 1 halo point each side) in shared memory, walks the block's
-// cell-ordered particle range with coalesced column loads, accumulates current in a shared
-// J tile (tile + 1 low / 2 high halo nodes) and flushes the tile to global J once.
+// its cells can touch (tile + 1 halo point each side) in shared memory and accumulates current
+// in a shared J tile (tile + 1 low / 2 high halo nodes) that is flushed to global J once.  A
+// warp takes one CELL at a time and walks that cell's slots in chunks of 32, so the cell -- and
+// with it every tile address that does not depend on the in-cell offset -- is warp-uniform, the
+// gather reads are shared-memory broadcasts, and the currents of the trajectories that stay
+// inside the cell (the great majority) are summed in registers over the whole cell and
+// reduced across the warp once per cell.
+//
+// This is the single particle loop of PAPER.md:603 ("only one loop each time step that reads
+// and writes all particle data"): slot s of the new sorted order loads particle perm[s] of the
+// old list (reorder on load; perm comes from the index sort of sort.cu and is the identity after
+// a physical sort), and the kernel writes the advanced particle to slot s of the OTHER column
+// set together with the one-byte direction code of its move; per cell it writes the count of
+// each code.  Those two are all the next sort reads.
 //
 // Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction +
 // the cell key.  The move is b = a + v dt/dx; a particle that leaves its cell (b < 0 or b >= 1;
@@ -51,48 +62,6 @@ struct TileGeom {
     jvol = je[0] * je[1] * je[2];
   }
 };
-
-// b1 stencil along one direction for in-cell offset a in [0,1) of tile-local cell l:
-// node-centred quantity: points l, l+1 with weights 1-a, a;
-// half-staggered quantity (sampled at l+1/2): points l-1, l or l, l+1.
-struct Stencil1 {
-  int in, is;      // first point (index into the field tile, halo included)
-  float fn, fs;    // weight of the second point
-  __device__ __forceinline__ void set(int l, float a) {
-    in = l + 1;
-    fn = a;
-    const bool lo = a < 0.5f;
-    is = lo ? l : l + 1;
-    fs = lo ? a + 0.5f : a - 0.5f;
-  }
-};
-
-template <bool D3, bool SX, bool SY, bool SZ>
-__device__ __forceinline__ float gather1(const float *__restrict__ F, const TileGeom<D3> &tg,
-                                         const Stencil1 &sx, const Stencil1 &sy,
-                                         const Stencil1 &sz) {
-  const int iy = SY ? sy.is : sy.in, iz = SZ ? sz.is : sz.in;
-  const float fy = SY ? sy.fs : sy.fn, fz = SZ ? sz.fs : sz.fn;
-  if (D3) {
-    const int ix = SX ? sx.is : sx.in;
-    const float fx = SX ? sx.fs : sx.fn;
-    const float *q = F + (iz * tg.fe[1] + iy) * tg.fe[0] + ix;
-    const int s1 = tg.fe[0], s2 = tg.fe[0] * tg.fe[1];
-    const float v00 = q[0] + fx * (q[1] - q[0]);
-    const float v10 = q[s1] + fx * (q[s1 + 1] - q[s1]);
-    const float v01 = q[s2] + fx * (q[s2 + 1] - q[s2]);
-    const float v11 = q[s2 + s1] + fx * (q[s2 + s1 + 1] - q[s2 + s1]);
-    const float w0 = v00 + fy * (v10 - v00);
-    const float w1 = v01 + fy * (v11 - v01);
-    return w0 + fz * (w1 - w0);
-  } else {
-    const float *q = F + iz * tg.fe[1] + iy;
-    const int s2 = tg.fe[1];
-    const float w0 = q[0] + fy * (q[1] - q[0]);
-    const float w1 = q[s2] + fy * (q[s2 + 1] - q[s2]);
-    return w0 + fz * (w1 - w0);
-  }
-}
 
 // one VB segment in the cell with tile-local coordinates (cx,cy,cz); a*, b* in-cell start/end
 template <bool D3>
@@ -301,61 +270,63 @@ constexpr int QW = 8;      // words per entry
 
 template <bool D3>
 __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TileGeom<D3> &tg,
-                                            const GridDesc &gd, const int *__restrict__ sLut,
-                                            const float *__restrict__ q, int start, int n, int lane) {
+                                            const GridDesc &gd, const float *__restrict__ q,
+                                            int start, int n, int lane) {
   if (lane < n) {
     const int e = start + lane;
-    const int lc = __float_as_int(q[0 * QCAP + e]);
+    const int packed = __float_as_int(q[0 * QCAP + e]);
     const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
     const float ddx = q[4 * QCAP + e], ddy = q[5 * QCAP + e], ddz = q[6 * QCAP + e];
     const float qw = q[7 * QCAP + e];
-    const int packed = sLut[lc];
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
     // 2-d: the x slots carry (unused, v_x): the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
     const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
     vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
-                qvx, 1);
+                qvx, 0);
   }
   __syncwarp();
 }
 
+// b1 gather of one component (Eq. 11; each component from its own staggered
+// points).  q points at the first stencil point, f* are the weights of the second point.
+template <bool D3>
+__device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, int s2, float fx,
+                                         float fy, float fz) {
+  if (D3) {
+    const float v00 = fmaf(fx, q[1] - q[0], q[0]);
+    const float v10 = fmaf(fx, q[s1 + 1] - q[s1], q[s1]);
+    const float v01 = fmaf(fx, q[s2 + 1] - q[s2], q[s2]);
+    const float v11 = fmaf(fx, q[s2 + s1 + 1] - q[s2 + s1], q[s2 + s1]);
+    const float w0 = fmaf(fy, v10 - v00, v00);
+    const float w1 = fmaf(fy, v11 - v01, v01);
+    return fmaf(fz, w1 - w0, w0);
+  } else {
+    const float w0 = fmaf(fy, q[1] - q[0], q[0]);
+    const float w1 = fmaf(fy, q[s2 + 1] - q[s2], q[s2]);
+    return fmaf(fz, w1 - w0, w0);
+  }
+}
+
 template <bool D3>
 __global__ void __launch_bounds__(PUSH_THREADS, 3)
-k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell_offsets,
+k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
+        const int *__restrict__ offs, uint8_t *__restrict__ dcode, int *__restrict__ dircnt,
         const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
         uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   constexpr int NV = D3 ? 12 : 8;
   TileGeom<D3> tg;
   tg.init(gd, blockIdx.x);
-  float *sF = smem;                // [6][fvol]: Ex Ey Ez Bx By Bz
-  float *sJ = smem + 6 * tg.fvol;  // [3][jvol]
-  int *sLut = (int *)(sJ + 3 * tg.jvol);  // [cpb]: cell in tile -> lx | ly << 10 | lz << 20
-  int *sKx = sLut + gd.cpb;               // key contribution of local x coordinate -1 .. bs0
-  int *sKy = sKx + gd.bs[0] + 2;
-  int *sKz = sKy + gd.bs[1] + 2;
-  float *sQ = (float *)(sKz + gd.bs[2] + 2);  // [warps][QW][QCAP]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  float *sF = smem;                           // [6][fvol]: Ex Ey Ez Bx By Bz
+  float *sJ = smem + 6 * tg.fvol;             // [3][jvol]
+  float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
+  int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
+  float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QW][QCAP]
   float *myQ = sQ + warp * (QW * QCAP);
 
-  for (int i = threadIdx.x; i < gd.cpb; i += blockDim.x) {
-    const int lx = i % gd.bs[0], t = i / gd.bs[0];
-    sLut[i] = lx | ((t % gd.bs[1]) << 10) | ((t / gd.bs[1]) << 20);
-  }
-  for (int i = threadIdx.x; i < gd.bs[0] + gd.bs[1] + gd.bs[2] + 6; i += blockDim.x) {
-    int d = 0, l = i;
-    if (l >= gd.bs[0] + 2) { l -= gd.bs[0] + 2; d = 1; }
-    if (d == 1 && l >= gd.bs[1] + 2) { l -= gd.bs[1] + 2; d = 2; }
-    int c = tg.o[d] + l - 1;  // global cell coordinate, wrapped periodically
-    if (c < 0) c += gd.n[d];
-    if (c >= gd.n[d]) c -= gd.n[d];
-    const int b = c / gd.bs[d], ll = c - b * gd.bs[d];
-    const int bstride = d == 0 ? 1 : d == 1 ? gd.nb[0] : gd.nb[0] * gd.nb[1];
-    const int lstride = d == 0 ? 1 : d == 1 ? gd.bs[0] : gd.bs[0] * gd.bs[1];
-    sKx[i] = b * bstride * gd.cpb + ll * lstride;
-  }
-
+  if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
     const int lx = r % tg.fe[0], t = r / tg.fe[0];
@@ -366,13 +337,15 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
     sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
   }
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
+  DirCount<D3> dirs;
+  dirs.init(sDir + warp * 32, lane);
   __syncthreads();
 
-  const int p0 = cell_offsets[blockIdx.x * gd.cpb], p1 = cell_offsets[(blockIdx.x + 1) * gd.cpb];
-  const float *sEx = sF, *sEy = sF + tg.fvol, *sEz = sF + 2 * tg.fvol;
-  const float *sBx = sF + 3 * tg.fvol, *sBy = sF + 4 * tg.fvol, *sBz = sF + 5 * tg.fvol;
+  const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   uint32_t bad = 0;
   const int kbase = blockIdx.x * gd.cpb;
+  const unsigned lt = lanemask_lt_();
+  const float cdx = D3 ? gd.dt_dx[0] : 0.f, cdy = gd.dt_dx[1], cdz = gd.dt_dx[2];
 
   // which reduced value this lane ends up holding, and the J point (relative to the cell's
   // (lx+1, ly+1, lz+1) tile node) it belongs to
@@ -395,108 +368,79 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
-  for (int base = p0 + warp * 32; base < p1; base += nwarps * 32) {
-    const int a = base + lane;
-    const bool act = a < p1;
-    float ax = 0.f, ay = 0.f, az = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
-    int sp = 0, lc = 0;
-    if (act) {
-      ay = ld_stream(p.y + a);
-      az = ld_stream(p.z + a);
-      ux = ld_stream(p.ux + a);
-      uy = ld_stream(p.uy + a);
-      uz = ld_stream(p.uz + a);
-      qw = ld_stream(p.qw + a);
-      sp = ld_stream(p.sp + a);
-      lc = ld_stream(key + a) - kbase;
-      if (D3) ax = ld_stream(p.x + a);
-      if (lc < 0 || lc >= gd.cpb) {  // not the sorted list this kernel was promised: flag, drop
-        bad |= PSC_F_NOT_IN_TILE;
-        lc = 0;
-        qw = 0.f;
-      }
-    }
-    lc = __shfl_sync(0xffffffffu, lc, act ? lane : 0);  // idle tail lanes: lane 0's cell, no charge
-    const int packed = sLut[lc];
-    const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
-
-    // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) ----------
-    Stencil1 sx, sy, sz;
-    sx.set(lx, ax);
-    sy.set(ly, ay);
-    sz.set(lz, az);
-    const float ex = gather1<D3, true, false, false>(sEx, tg, sx, sy, sz);
-    const float ey = gather1<D3, false, true, false>(sEy, tg, sx, sy, sz);
-    const float ez = gather1<D3, false, false, true>(sEz, tg, sx, sy, sz);
-    const float bx = gather1<D3, false, true, true>(sBx, tg, sx, sy, sz);
-    const float by = gather1<D3, true, false, true>(sBy, tg, sx, sy, sz);
-    const float bz = gather1<D3, true, true, false>(sBz, tg, sx, sy, sz);
-
-    // ---- Boris (Eq. 27-28) and move (Eq. 26) ------------------------------------------------
-    boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, gd.qmh[sp]);
-    const float ig = rsqrtf(1.0f + ux * ux + uy * uy + uz * uz);
-    const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
-    const float ddx = D3 ? vx * gd.dt_dx[0] : 0.f;  // displacement in cells
-    const float ddy = vy * gd.dt_dx[1], ddz = vz * gd.dt_dx[2];
-    const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
-    const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-    const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-    const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
-    const bool cross = (sxd | syd | szd) != 0;
-
-    // ---- Villasenor-Buneman deposit: segment 0 (inside the home cell) ------------------------
-    {
-      const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
-      const float qvx = qw * gd.inv_dV * vx;
-      float qx = endx, qy = endy, qz = endz, t = 1.f;
-      if (cross) {  // same arithmetic as vb_walk's first iteration
-        const float tx = sxd ? ((sxd > 0 ? 1.f - ax : -ax) / ddx) : 2.f;
-        const float ty = syd ? ((syd > 0 ? 1.f - ay : -ay) / ddy) : 2.f;
-        const float tz = szd ? ((szd > 0 ? 1.f - az : -az) / ddz) : 2.f;
-        t = fminf(fminf(tx, ty), fminf(tz, 1.f));
-        if (t < 1.f) {
-          const int which = (tx <= ty && tx <= tz) ? 0 : (ty <= tz ? 1 : 2);
-          qx = ax + t * ddx; qy = ay + t * ddy; qz = az + t * ddz;
-          if (which == 0) qx = sxd > 0 ? 1.f : 0.f;
-          else if (which == 1) qy = syd > 0 ? 1.f : 0.f;
-          else qz = szd > 0 ? 1.f : 0.f;
-        }
-      }
-      float v[NV];
-      vb_values<D3>(v, ax, ay, az, qx, qy, qz, t, fx, fy, fz, qvx);
-      // one reduction per distinct cell among the lanes (cell-ordered list: usually one or two)
-      unsigned todo = 0xffffffffu;
-      while (todo) {
-        const int cl = __shfl_sync(0xffffffffu, lc, __ffs(todo) - 1);
-        const bool in = lc == cl;
-        const unsigned m = __ballot_sync(0xffffffffu, in);
-        float r;
-        if (m == 0xffffffffu) {
-          if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(v), lane);
-          else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(v), lane);
-        } else {
-          float w[NV];
+  for (int ci = warp; ci < gd.cpb; ci += nwarps) {
+    const int p0 = offs[kbase + ci], p1 = offs[kbase + ci + 1];
+    const int lx = ci % gd.bs[0], lt_ = ci / gd.bs[0];
+    const int ly = lt_ % gd.bs[1], lz = lt_ / gd.bs[1];
+    const int packed = lx | (ly << 10) | (lz << 20);
+    // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
+    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
+                               : (lz + 1) * tg.fe[1] + (ly + 1));
+    float acc[NV];
 #pragma unroll
-          for (int i = 0; i < NV; i++) w[i] = in ? v[i] : 0.f;
-          if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(w), lane);
-          else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(w), lane);
-        }
-        if (writer) {
-          const int pk = sLut[cl];
-          const int cx = pk & 1023, cy = (pk >> 10) & 1023, cz = pk >> 20;
-          const int node = D3 ? ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1)
-                              : (cz + 1) * tg.je[1] + (cy + 1);
-          atomicAdd(&sJ[node + my_off], r);
-        }
-        todo &= ~m;
+    for (int i = 0; i < NV; i++) acc[i] = 0.f;
+
+    for (int base = p0; base < p1; base += 32) {
+      const int s = base + lane;
+      const bool act = s < p1;
+      float ax = 0.f, ay = 0.f, az = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
+      int sp = 0, p = s;
+      if (act) {
+        if (perm) p = ld_stream(perm + s);
+        ay = ld_stream(in.y + p);
+        az = ld_stream(in.z + p);
+        ux = ld_stream(in.ux + p);
+        uy = ld_stream(in.uy + p);
+        uz = ld_stream(in.uz + p);
+        qw = ld_stream(in.qw + p);
+        sp = ld_stream(in.sp + p);
+        if (D3) ax = ld_stream(in.x + p);
       }
-      // the rest of a trajectory that leaves its cell goes through the per-warp queue
+
+      // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) --------
+      // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l
+      // (a < 1/2, weight a + 1/2) or l, l+1 (weight a - 1/2)
+      const bool hy = ay >= 0.5f, hz = az >= 0.5f, hx = D3 && ax >= 0.5f;
+      const float gy = hy ? ay - 0.5f : ay + 0.5f, gz = hz ? az - 0.5f : az + 0.5f;
+      const float gx = hx ? ax - 0.5f : ax + 0.5f;
+      const int oy = hy ? 0 : -fs1, oz = hz ? 0 : -fs2, ox = (!D3 || hx) ? 0 : -1;
+      const float ex = gather1<D3>(cF + ox, fs1, fs2, gx, ay, az);
+      const float ey = gather1<D3>(cF + fvol + oy, fs1, fs2, ax, gy, az);
+      const float ez = gather1<D3>(cF + 2 * fvol + oz, fs1, fs2, ax, ay, gz);
+      const float bx = gather1<D3>(cF + 3 * fvol + oy + oz, fs1, fs2, ax, gy, gz);
+      const float by = gather1<D3>(cF + 4 * fvol + ox + oz, fs1, fs2, gx, ay, gz);
+      const float bz = gather1<D3>(cF + 5 * fvol + ox + oy, fs1, fs2, gx, gy, az);
+
+      // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
+      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
+      const float ig = rsqrtf(fmaf(ux, ux, fmaf(uy, uy, fmaf(uz, uz, 1.0f))));
+      const float vx = ux * ig;
+      const float ddx = D3 ? vx * cdx : 0.f;  // displacement in cells
+      const float ddy = (uy * ig) * cdy, ddz = (uz * ig) * cdz;
+      const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
+      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      const int dc = dir_code<D3>(sxd, syd, szd);
+      const bool cross = act && dc != DirCount<D3>::STAY;
+
+      // ---- Villasenor-Buneman deposit ---------------------------------------------------------
+      // a trajectory that stays in the cell is one segment: its currents go to the per-cell
+      // register sums; one that leaves goes through the per-warp queue (all its segments)
+      {
+        const float qs = cross ? 0.f : qw;
+        float v[NV];
+        vb_values<D3>(v, ax, ay, az, endx, endy, endz, 1.f, qs * gd.cur[0], qs * gd.cur[1],
+                      qs * gd.cur[2], qs * gd.inv_dV * vx);
+#pragma unroll
+        for (int i = 0; i < NV; i++) acc[i] += v[i];
+      }
       const unsigned cm = __ballot_sync(0xffffffffu, cross);
       if (cm) {
         if (cross) {
-          const int e = qcnt + __popc(cm & ((1u << lane) - 1u));
-          myQ[0 * QCAP + e] = __int_as_float(lc);
-          myQ[1 * QCAP + e] = D3 ? ax : 0.f;
+          const int e = qcnt + __popc(cm & lt);
+          myQ[0 * QCAP + e] = __int_as_float(packed);
+          myQ[1 * QCAP + e] = ax;
           myQ[2 * QCAP + e] = ay;
           myQ[3 * QCAP + e] = az;
           myQ[4 * QCAP + e] = D3 ? ddx : vx;
@@ -508,34 +452,49 @@ k_push1(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
         __syncwarp();
         if (qcnt >= 32) {
           qcnt -= 32;
-          drain_queue<D3>(sJ, tg, gd, sLut, myQ, qcnt, 32, lane);
+          drain_queue<D3>(sJ, tg, gd, myQ, qcnt, 32, lane);
         }
+      }
+      dirs.add(act, dc);
+
+      // ---- store slot s of the other column set: new offset, momentum, direction code -----
+      if (act) {
+        const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+        const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+        if (D3) {
+          const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
+          st_stream(out.x + s, bx_);
+          if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
+        } else if (in.x) {
+          st_stream(out.x + s, ld_stream(in.x + p));  // invariant coordinate: carried
+        }
+        st_stream(out.y + s, by_);
+        st_stream(out.z + s, bz_);
+        st_stream(out.ux + s, ux);
+        st_stream(out.uy + s, uy);
+        st_stream(out.uz + s, uz);
+        st_stream(out.qw + s, qw);
+        st_stream(out.sp + s, sp);
+        if (in.id) st_stream(out.id + s, ld_stream(in.id + p));
+        dcode[s] = (uint8_t)dc;
+        if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
       }
     }
 
-    // ---- new offset + new key (periodic wrap lives in the key tables) -----------------------
-    if (act) {
-      float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-      float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-      int nk = sKy[ly + syd + 1] + sKz[lz + szd + 1];
-      if (D3) {
-        float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
-        nk += sKx[lx + sxd + 1];
-        st_stream(p.x + a, bx_);
-        if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
-      } else {
-        nk += sKx[1];
+    // ---- the cell's in-cell currents: one warp reduction, one shared add per J point -------
+    if (p1 > p0) {
+      float r;
+      if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
+      else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(acc), lane);
+      if (writer) {
+        const int node = D3 ? ((lz + 1) * tg.je[1] + (ly + 1)) * tg.je[0] + (lx + 1)
+                            : (lz + 1) * tg.je[1] + (ly + 1);
+        atomicAdd(&sJ[node + my_off], r);
       }
-      st_stream(p.y + a, by_);
-      st_stream(p.z + a, bz_);
-      st_stream(p.ux + a, ux);
-      st_stream(p.uy + a, uy);
-      st_stream(p.uz + a, uz);
-      __stcs(key + a, nk);
-      if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
+    dirs.cell_done(dircnt, kbase + ci, lane);
   }
-  if (qcnt) drain_queue<D3>(sJ, tg, gd, sLut, myQ, 0, qcnt, lane);
+  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, 0, qcnt, lane);
   if (bad) atomicOr(flags, bad);
   __syncthreads();
 
@@ -559,12 +518,6 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const bool d3 = gd.n[0] > 1 && gd.n[1] > 1 && gd.n[2] > 1;
   const bool d2yz = gd.n[0] == 1 && gd.n[1] > 1 && gd.n[2] > 1;
   if (!d3 && !d2yz) return PSC_ERR_UNSUPPORTED;  // 2-d runs are yz-plane runs
-  {
-    ProfScope ps(c, PSC_PH_J_ZERO, s);
-    PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
-    c->launches++;
-  }
-  if (c->np == 0) return PSC_OK;
   int fvol = 1, jvol = 1;
   for (int d = 0; d < 3; d++)
     if (gd.n[d] > 1) {
@@ -573,17 +526,19 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     }
   const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH_THREADS;
   if (threads < 32 || threads > PUSH_THREADS) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + gd.cpb + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6 + (threads / 32) * QW * QCAP) * sizeof(float);
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP)) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
-  const Cols &p = c->cols[c->cur];
+  const Cols &in = c->cols[c->cur];
+  const Cols &out = c->cols[c->cur ^ 1];
+  const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
   ProfScope ps(c, PSC_PH_PUSH, s);
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
   } else {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
   }
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

@@ -196,31 +196,22 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
 
 template <bool D3>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
-k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell_offsets,
-        const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
-        uint32_t *__restrict__ flags) {
+k_push2(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
+        const int *__restrict__ cell_offsets, uint8_t *__restrict__ dcode,
+        int *__restrict__ dircnt, const float *__restrict__ E, const float *__restrict__ B,
+        float *__restrict__ J, uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   Geom2<D3> tg;
   tg.init(gd, blockIdx.x);
   float *sF = smem;                // [6][tvol]
   float *sJ = smem + 6 * tg.tvol;  // [3][tvol]
-  int *sKx = (int *)(sJ + 3 * tg.tvol);  // key contribution of local coordinate -1 .. bs
-  int *sKy = sKx + gd.bs[0] + 2;
-  int *sKz = sKy + gd.bs[1] + 2;
+  float *sH = sJ + 3 * tg.tvol;               // [8]: Boris h per species
+  int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
 
-  for (int i = threadIdx.x; i < gd.bs[0] + gd.bs[1] + gd.bs[2] + 6; i += blockDim.x) {
-    int d = 0, l = i;
-    if (l >= gd.bs[0] + 2) { l -= gd.bs[0] + 2; d = 1; }
-    if (d == 1 && l >= gd.bs[1] + 2) { l -= gd.bs[1] + 2; d = 2; }
-    int c = tg.o[d] + l - 1;
-    if (c < 0) c += gd.n[d];
-    if (c >= gd.n[d]) c -= gd.n[d];
-    const int b = c / gd.bs[d], ll = c - b * gd.bs[d];
-    const int bstride = d == 0 ? 1 : d == 1 ? gd.nb[0] : gd.nb[0] * gd.nb[1];
-    const int lstride = d == 0 ? 1 : d == 1 ? gd.bs[0] : gd.bs[0] * gd.bs[1];
-    sKx[i] = b * bstride * gd.cpb + ll * lstride;
-  }
+  if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
+  DirCount<D3> dirs;
+  dirs.init(sDir + warp * 32, lane);
   for (int i = threadIdx.x; i < 6 * tg.tvol; i += blockDim.x) {
     const int c = i / tg.tvol, r = i - c * tg.tvol;
     const int tx = r % tg.te[0], t = r / tg.te[0];
@@ -250,7 +241,6 @@ k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
 
   for (int ci = warp; ci < gd.cpb; ci += nwarps) {
     const int p0 = cell_offsets[kbase + ci], p1 = cell_offsets[kbase + ci + 1];
-    if (p0 >= p1) continue;
     const int lx = ci % gd.bs[0], lt = ci / gd.bs[0];
     const int ly = lt % gd.bs[1], lz = lt / gd.bs[1];
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
@@ -259,20 +249,17 @@ k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
       const int a = base + lane;
       const bool act = a < p1;
       float ax = 0.25f, ay = 0.25f, az = 0.25f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
-      int sp = 0;
+      int sp = 0, p = a;
       if (act) {
-        ay = ld_stream(p.y + a);
-        az = ld_stream(p.z + a);
-        ux = ld_stream(p.ux + a);
-        uy = ld_stream(p.uy + a);
-        uz = ld_stream(p.uz + a);
-        qw = ld_stream(p.qw + a);
-        sp = ld_stream(p.sp + a);
-        if (D3) ax = ld_stream(p.x + a);
-        if (ld_stream(key + a) != kbase + ci) {  // not the sorted list this kernel was promised
-          bad |= PSC_F_NOT_IN_TILE;
-          qw = 0.f;
-        }
+        if (perm) p = ld_stream(perm + a);  // reorder on load
+        ay = ld_stream(in.y + p);
+        az = ld_stream(in.z + p);
+        ux = ld_stream(in.ux + p);
+        uy = ld_stream(in.uy + p);
+        uz = ld_stream(in.uz + p);
+        qw = ld_stream(in.qw + p);
+        sp = ld_stream(in.sp + p);
+        if (D3) ax = ld_stream(in.x + p);
       }
       // ---- gather (Eq. 11 with b2 weights; each component from its own Yee points) ---------
       Sten2 sx, sy, sz;
@@ -287,7 +274,7 @@ k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
       const float bz = gather2<D3, true, true, false>(sBz, tg, lx, ly, lz, sx, sy, sz);
 
       // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
-      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, gd.qmh[sp]);
+      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
       const float ig = rsqrtf(1.0f + ux * ux + uy * uy + uz * uz);
       const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
       const float endx = D3 ? ax + vx * gd.dt_dx[0] : ax;
@@ -397,32 +384,36 @@ k_push2(GridDesc gd, Cols p, int *__restrict__ key, const int *__restrict__ cell
         }
       }
 
-      // ---- new offset + new key (periodic wrap lives in the key tables) ---------------------
+      // ---- store slot a of the other column set: new offset, momentum, direction code -----
+      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      const int dc = dir_code<D3>(sxd, syd, szd);
+      dirs.add(act, dc);
       if (act) {
-        const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-        const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-        const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
         const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
         const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-        int nk = sKy[ly + syd + 1] + sKz[lz + szd + 1];
         if (D3) {
           const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
-          nk += sKx[lx + sxd + 1];
-          st_stream(p.x + a, bx_);
+          st_stream(out.x + a, bx_);
           if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
-        } else {
-          nk += sKx[1];
+        } else if (in.x) {
+          st_stream(out.x + a, ld_stream(in.x + p));  // invariant coordinate: carried
         }
-        st_stream(p.y + a, by_);
-        st_stream(p.z + a, bz_);
-        st_stream(p.ux + a, ux);
-        st_stream(p.uy + a, uy);
-        st_stream(p.uz + a, uz);
-        __stcs(key + a, nk);
+        st_stream(out.y + a, by_);
+        st_stream(out.z + a, bz_);
+        st_stream(out.ux + a, ux);
+        st_stream(out.uy + a, uy);
+        st_stream(out.uz + a, uz);
+        st_stream(out.qw + a, qw);
+        st_stream(out.sp + a, sp);
+        if (in.id) st_stream(out.id + a, ld_stream(in.id + p));
+        dcode[a] = (uint8_t)dc;
         if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
           bad |= PSC_F_NAN;
       }
     }
+    dirs.cell_done(dircnt, kbase + ci, lane);
   }
   if (bad) atomicOr(flags, bad);
   __syncthreads();
@@ -447,27 +438,23 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const bool d3 = gd.n[0] > 1 && gd.n[1] > 1 && gd.n[2] > 1;
   const bool d2yz = gd.n[0] == 1 && gd.n[1] > 1 && gd.n[2] > 1;
   if (!d3 && !d2yz) return PSC_ERR_UNSUPPORTED;  // 2-d runs are yz-plane runs (A25)
-  {
-    ProfScope ps(c, PSC_PH_J_ZERO, s);
-    PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * gd.comp * sizeof(float), s));
-    c->launches++;
-  }
-  if (c->np == 0) return PSC_OK;
   int tvol = 1;
   for (int d = 0; d < 3; d++)
     if (gd.n[d] > 1) tvol *= gd.bs[d] + 3;
   const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH2_THREADS;
   if (threads < 32 || threads > PUSH2_THREADS) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(9 * tvol + gd.bs[0] + gd.bs[1] + gd.bs[2] + 6) * sizeof(float);
+  const size_t smem = (size_t)(9 * tvol + PSC_MAX_SPECIES + (threads / 32) * 32) * sizeof(float);
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
-  const Cols &p = c->cols[c->cur];
+  const Cols &in = c->cols[c->cur];
+  const Cols &out = c->cols[c->cur ^ 1];
+  const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
   ProfScope ps(c, PSC_PH_PUSH, s);
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
   } else {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, p, c->key[c->kcur], c->cell_offsets, c->E, c->B, c->J, c->d_flags);
+    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
   }
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

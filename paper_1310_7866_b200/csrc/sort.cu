@@ -1,23 +1,35 @@
-// sort.cu -- cell-key counting sort of the particle list (PAPER.md:585-597).
+// sort.cu -- cell-key counting sort of the particle list (PAPER.md:585-603).
 //
 // One key orders by block ("supercell") and by cell inside the block at once:
 //   key = block_index * cells_per_block + cell_in_block.
-// A counting sort is O(N + M).  The B200 form:
-//   1. k_keys     (absolute positions in) key per particle from floor(fl32(x * 1/dx)), or
-//      k_hist     (internal form in) the keys the push left behind; either way a histogram over
-//                 keys with warp-aggregated atomics (lanes holding the same key elect one lane
-//                 that adds the group's size; on a cell-ordered list a warp issues 1-2 atomics);
-//   2. scan       exclusive prefix sum of the histogram -> cell_offsets (three small kernels);
+// A counting sort is O(N + M).  Two forms:
+//
+// GENERAL (arbitrary input order; the first sort of a run, from absolute positions):
+//   1. k_keys     key per particle from floor(fl32(x * 1/dx)) (k_hist: keys already known), and a
+//                 histogram over keys with warp-aggregated atomics;
+//   2. scan       exclusive prefix sum of the histogram -> cell offsets (three small kernels);
 //   3. k_scatter  slot = cursor[key] + rank, again warp-aggregated; writes the permutation;
 //   4. k_segsort  the atomics hand out slots in arbitrary order ACROSS warps, so every key's
-//                 segment of `perm` is sorted ascending (bitonic network, in registers / shared
-//                 memory; segments are ~ particles-per-cell long).  A set of distinct input
-//                 indices in ascending order IS the stable order, hence the result is the
-//                 unique stable counting sort, bit-exact against any stable reference;
-//   5. k_reorder  out[s] = in[perm[s]] for every column (coalesced writes; the reads are nearly
-//                 coalesced when the list is a previous sort's output advanced by one push,
-//                 because a particle moves at most one cell per step).  Positions
-//                 leave this kernel in the internal form (in-cell offset; the cell is the key).
+//                 segment of `perm` is sorted ascending: a set of distinct input indices in
+//                 ascending order IS the stable order, hence the result is the unique stable
+//                 counting sort, bit-exact against any stable reference;
+//   5. k_reorder  out[s] = in[perm[s]] for every column; positions leave in the internal form.
+//
+// INDEX (steady state: "a particle moves at most one cell per step", "the
+// sort only touches keys/indices", "reorder on load"): the list is the previous sort's output
+// advanced by one push, which left per particle a one-byte direction code (one of 9 / 27
+// destination classes) and per cell the count of each code.  Then
+//   1. k_dest_hist  new count of cell k = sum over its 9 / 27 neighbour source cells of the
+//                   count of the code that points at k;
+//   2. scan         -> new cell offsets;
+//   3. k_dir_base   stable order inside a destination cell = ascending old slot = ascending
+//                   source-cell key, then slot order inside the source cell: first slot of every
+//                   (source cell, code) group by a running sum over the sources in key order;
+//   4. k_rank       one warp per source cell walks its slots in order and hands out
+//                   consecutive slots per code (ballot + popc for the stayers, lane order for the
+//                   few leavers) -> perm.  Reads 1 byte, writes 4 bytes per particle.
+// No particle column is touched: the next push loads particle perm[s] for slot s (reorder on
+// load).  psc_particles_sort, whose contract is a physically sorted list, adds k_reorder.
 #include <limits.h>
 
 #include "psc_internal.cuh"
@@ -358,17 +370,15 @@ k_segsort_big(const int *__restrict__ offs, int *__restrict__ perm,
 // FROM_ABS: the input columns hold absolute positions -> write in-cell offsets
 template <bool FROM_ABS>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out,
-          const int *__restrict__ key_in, int *__restrict__ key_out) {
+k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out) {
   const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   for (int s = s0; s < n; s += stride) {
     const int p = perm[s];
-    float x = in.x[p], y = in.y[p], z = in.z[p];
+    float x = in.x ? in.x[p] : 0.f, y = in.y[p], z = in.z[p];
     const float ux = in.ux[p], uy = in.uy[p], uz = in.uz[p];
     const float qw = in.qw[p];
     const int sp = in.sp[p];
-    const int k = key_in[p];
     int id = 0;
     if (in.id) id = in.id[p];
     if (FROM_ABS) {  // same fp32 product + floor as k_keys; clamped like there
@@ -376,7 +386,7 @@ k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out,
       if (gd.n[1] > 1) { const float xi = __fmul_rn(y, gd.inv_dx[1]); y = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
       if (gd.n[2] > 1) { const float xi = __fmul_rn(z, gd.inv_dx[2]); z = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
     }
-    out.x[s] = x;
+    if (in.x) out.x[s] = x;
     out.y[s] = y;
     out.z[s] = z;
     out.ux[s] = ux;
@@ -384,9 +394,145 @@ k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out,
     out.uz[s] = uz;
     out.qw[s] = qw;
     out.sp[s] = sp;
-    key_out[s] = k;
     if (in.id) out.id[s] = id;
   }
+}
+
+
+// ---- index sort of a pushed list -------------------------------------------------------------
+
+__device__ __forceinline__ int cell_to_key(const GridDesc &gd, const int c[3]) {
+  const int b0 = c[0] / gd.bs[0], b1 = c[1] / gd.bs[1], b2 = c[2] / gd.bs[2];
+  const int l0 = c[0] - b0 * gd.bs[0], l1 = c[1] - b1 * gd.bs[1], l2 = c[2] - b2 * gd.bs[2];
+  return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
+}
+
+__device__ __forceinline__ int wrap(int c, int n) { return c < 0 ? c + n : (c >= n ? c - n : c); }
+
+// key of the neighbour of cell c[] in direction code dc (periodic)
+template <bool D3>
+__device__ __forceinline__ int neighbour_key(const GridDesc &gd, const int c[3], int dc, int sign) {
+  int s[3];
+  if (D3) {
+    s[0] = dc % 3 - 1;
+    s[1] = (dc / 3) % 3 - 1;
+    s[2] = dc / 9 - 1;
+  } else {
+    s[0] = 0;
+    s[1] = dc % 3 - 1;
+    s[2] = dc / 3 - 1;
+  }
+  int q[3];
+#pragma unroll
+  for (int d = 0; d < 3; d++) q[d] = wrap(c[d] + sign * s[d], gd.n[d]);
+  return cell_to_key(gd, q);
+}
+
+// hist[k] = particles that will be in cell k: source cell (k - dir) sends count[dir]
+template <bool D3>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_dest_hist(GridDesc gd, const int *__restrict__ dircnt, int *__restrict__ hist) {
+  constexpr int ND = D3 ? 27 : 9;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= gd.nkeys) return;
+  int c[3];
+  key_to_cell(gd, k, c);
+  int tot = 0;
+#pragma unroll
+  for (int dc = 0; dc < ND; dc++) tot += dircnt[neighbour_key<D3>(gd, c, dc, -1) * ND + dc];
+  hist[k] = tot;
+}
+
+// dircnt[src][dc] (count) -> first new slot of the (src, dc) group, in place
+template <bool D3>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ offs_new) {
+  constexpr int ND = D3 ? 27 : 9;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= gd.nkeys) return;
+  int c[3];
+  key_to_cell(gd, k, c);
+  int sk[ND], cnt[ND];
+#pragma unroll
+  for (int dc = 0; dc < ND; dc++) {
+    sk[dc] = neighbour_key<D3>(gd, c, dc, -1);
+    cnt[dc] = dircnt[sk[dc] * ND + dc];
+  }
+  const int o = offs_new[k];
+#pragma unroll
+  for (int i = 0; i < ND; i++) {
+    int b = o;
+#pragma unroll
+    for (int j = 0; j < ND; j++) b += (sk[j] < sk[i]) ? cnt[j] : 0;
+    dircnt[sk[i] * ND + i] = b;
+  }
+}
+
+// one warp per source cell: perm[new slot] = old slot
+template <bool D3>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_rank(int nkeys, const int *__restrict__ offs_old, const uint8_t *__restrict__ dcode,
+       const int *__restrict__ dirbase, int *__restrict__ perm, uint32_t *__restrict__ flags) {
+  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
+  __shared__ int sb[SORT_THREADS / 32][32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int warps = gridDim.x * (SORT_THREADS / 32);
+  const unsigned lt = lanemask_lt();
+  for (int k = blockIdx.x * (SORT_THREADS / 32) + w; k < nkeys; k += warps) {
+    const int p0 = offs_old[k], p1 = offs_old[k + 1];
+    if (p0 >= p1) continue;
+    const int b = lane < ND ? dirbase[k * ND + lane] : 0;
+    sb[w][lane] = b;
+    int bstay = __shfl_sync(0xffffffffu, b, STAY);
+    __syncwarp();
+    for (int base = p0; base < p1; base += 32) {
+      const int s = base + lane;
+      const bool act = s < p1;
+      int dc = act ? (int)dcode[s] : STAY;
+      if (dc >= ND) {  // cannot happen unless the caller scribbled over the workspace
+        atomicOr(flags, PSC_F_OOB);
+        dc = STAY;
+      }
+      const bool stay = act && dc == STAY;
+      const unsigned m = __ballot_sync(0xffffffffu, stay);
+      int slot = bstay + __popc(m & lt);
+      bstay += __popc(m);
+      unsigned lv = __ballot_sync(0xffffffffu, act && !stay);
+      while (lv) {  // the few leavers, in lane order (= slot order: stable)
+        const int l = __ffs(lv) - 1;
+        lv &= lv - 1;
+        if (lane == l) {
+          slot = sb[w][dc];
+          sb[w][dc] = slot + 1;
+        }
+        __syncwarp();
+      }
+      if (act) perm[slot] = s;
+    }
+    __syncwarp();
+  }
+}
+
+// key of the particle in slot s of a list laid out by `offs`: the slot's cell, moved by the
+// particle's direction code if there is one
+template <bool D3>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const uint8_t *__restrict__ dcode,
+            int *__restrict__ key) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  int lo = 0, hi = gd.nkeys;  // largest k with offs[k] <= s (and offs[k+1] > s)
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (offs[mid] <= s) lo = mid; else hi = mid;
+  }
+  int k = lo;
+  if (dcode) {
+    int c[3];
+    key_to_cell(gd, k, c);
+    k = neighbour_key<D3>(gd, c, (int)dcode[s], +1);
+  }
+  key[s] = k;
 }
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -396,8 +542,10 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
   size_t b = 0;
-  b += 4 * align_up((size_t)n * 4, 256);                      // key[2], perm, cell_idx
-  b += 2 * align_up((nk + 1) * 4, 256);                       // cell_offsets, cursor
+  b += 4 * align_up((size_t)n * 4, 256);                      // key, perm, cell_idx, curkey
+  b += align_up((size_t)n, 256);                              // dcode
+  b += 3 * align_up((nk + 1) * 4, 256);                       // offs[2], cursor
+  b += align_up(nk * 27 * 4, 256);                            // dircnt
   b += align_up((nk / SCAN_TILE + 3) * 4, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
   return b;
@@ -411,52 +559,94 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
     p += align_up(bytes, 256);
     return r;
   };
-  c->key[0] = (int32_t *)take((size_t)n * 4);
-  c->key[1] = (int32_t *)take((size_t)n * 4);
+  c->key = (int32_t *)take((size_t)n * 4);
+  c->curkey = (int32_t *)take((size_t)n * 4);
   c->perm = (int32_t *)take((size_t)n * 4);
   c->cell_idx = (int32_t *)take((size_t)n * 4);
-  c->cell_offsets = (int32_t *)take((nk + 1) * 4);
+  c->dcode = (uint8_t *)take((size_t)n);
+  c->offs[0] = (int32_t *)take((nk + 1) * 4);
+  c->offs[1] = (int32_t *)take((nk + 1) * 4);
   c->cursor = (int32_t *)take((nk + 1) * 4);
+  c->dircnt = (int32_t *)take(nk * 27 * 4);
   c->scan_tmp = (int32_t *)take((nk / SCAN_TILE + 3) * 4);
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
   if ((size_t)(p - (char *)c->ws) > c->ws_bytes) return PSC_ERR_WORKSPACE;
   return PSC_OK;
 }
 
-int psc_sort_run(psc_ctx *c, cudaStream_t s) {
+namespace {
+
+inline bool is3d(const GridDesc &gd) { return gd.n[0] > 1; }
+
+// exclusive scan of the histogram in c->cursor -> out (and cursor := out)
+int run_scan(psc_ctx *c, int32_t *out, cudaStream_t s) {
+  const int nk = c->gd.nkeys;
+  ProfScope ps(c, PSC_PH_SORT_SCAN, s);
+  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
+  k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, out, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_tmp<<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, out, c->cursor, c->scan_tmp, sblocks);
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}
+
+int slot_keys(psc_ctx *c, const int32_t *offs, const uint8_t *dcode, int32_t *key, cudaStream_t s) {
+  const int n = (int)c->np;
+  if (n == 0) return PSC_OK;
+  const int blocks = (int)cdiv64(n, SORT_THREADS);
+  if (is3d(c->gd)) k_slot_keys<true><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dcode, key);
+  else k_slot_keys<false><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dcode, key);
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}
+
+}  // namespace
+
+// key[] (c->curkey) := keys of the current particles, in their current order
+int psc_sort_current_keys(psc_ctx *c, cudaStream_t s) {
+  switch (c->state) {
+    case PSC_STATE_SORTED: return slot_keys(c, c->offs[c->ocur], nullptr, c->curkey, s);
+    case PSC_STATE_PUSHED: return slot_keys(c, c->offs[c->ocur], c->dcode, c->curkey, s);
+    case PSC_STATE_INDEXED: return slot_keys(c, c->offs[c->ocur ^ 1], c->dcode, c->curkey, s);
+    default: return PSC_ERR_NOT_SORTED;
+  }
+}
+
+// general counting sort: arbitrary order in, physically sorted list out
+int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const GridDesc &gd = c->gd;
   const int n = (int)c->np;
   const int nk = gd.nkeys;
   const Cols &in = c->cols[c->cur];
   const Cols &out = c->cols[c->cur ^ 1];
   const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
+  int32_t *offs_new = c->offs[c->ocur ^ 1];
 
-  int32_t *key_in = c->key[c->kcur], *key_out = c->key[c->kcur ^ 1];
+  if (c->form == PSC_FORM_REL) {  // a sorted list sorted again: keys from the slots
+    const int rc = slot_keys(c, c->offs[c->ocur], nullptr, c->key, s);
+    if (rc) return rc;
+  }
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
   c->launches += 2;
   psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
   if (c->form == PSC_FORM_ABS)
-    k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, key_in, c->cursor, c->d_flags);
+    k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, c->key, c->cursor, c->d_flags);
   else
-    k_hist<<<pblocks, SORT_THREADS, 0, s>>>(n, nk, key_in, c->cursor, c->d_flags);
+    k_hist<<<pblocks, SORT_THREADS, 0, s>>>(n, nk, c->key, c->cursor, c->d_flags);
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_COUNT, s);
-  psc_prof_begin(c, PSC_PH_SORT_SCAN, s);
-  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
-  k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, c->cell_offsets, c->scan_tmp);
-  PSC_LAUNCH_CHECK(c);
-  k_scan_tmp<<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
-  PSC_LAUNCH_CHECK(c);
-  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->cursor, c->scan_tmp, sblocks);
-  PSC_LAUNCH_CHECK(c);
-  psc_prof_end(c, PSC_PH_SORT_SCAN, s);
+  {
+    const int rc = run_scan(c, offs_new, s);
+    if (rc) return rc;
+  }
   psc_prof_begin(c, PSC_PH_SORT_RANK, s);
-  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, key_in, c->cursor, c->perm);
+  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, c->key, c->cursor, c->perm);
   PSC_LAUNCH_CHECK(c);
   const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
-  k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, c->cell_offsets, c->perm, c->big_list,
-                                            c->d_flags + 1);
+  k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, offs_new, c->perm, c->big_list, c->d_flags + 1);
   PSC_LAUNCH_CHECK(c);
   if (n > WARP_SEG_CAP) {
     static bool attr_set = false;
@@ -465,31 +655,77 @@ int psc_sort_run(psc_ctx *c, cudaStream_t s) {
                                            BIG_SMEM_CAP * 4));
       attr_set = true;
     }
-    k_segsort_big<<<c->sm_count, 1024, BIG_SMEM_CAP * 4, s>>>(c->cell_offsets, c->perm, c->big_list,
+    k_segsort_big<<<c->sm_count, 1024, BIG_SMEM_CAP * 4, s>>>(offs_new, c->perm, c->big_list,
                                                               c->d_flags + 1);
     PSC_LAUNCH_CHECK(c);
   }
   psc_prof_end(c, PSC_PH_SORT_RANK, s);
   psc_prof_begin(c, PSC_PH_SORT_REORDER, s);
-  if (c->form == PSC_FORM_ABS)
-    k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
-  else
-    k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out, key_in, key_out);
+  if (c->form == PSC_FORM_ABS) k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out);
+  else k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out);
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_REORDER, s);
   c->cur ^= 1;
-  c->kcur ^= 1;
+  c->ocur ^= 1;
   c->form = PSC_FORM_REL;
   c->state = PSC_STATE_SORTED;
   c->have_sort_result = 1;
   return PSC_OK;
 }
 
-// cell_idx[a] of the last sort's INPUT particles (their keys are in the non-current key buffer)
+// index sort of a pushed list: new offsets + perm from the direction codes; no column moves
+int psc_sort_index(psc_ctx *c, cudaStream_t s) {
+  const GridDesc &gd = c->gd;
+  const int nk = gd.nkeys;
+  const int32_t *offs_old = c->offs[c->ocur];
+  int32_t *offs_new = c->offs[c->ocur ^ 1];
+  const int cblocks = (int)cdiv64(nk, SORT_THREADS);
+  const bool d3 = is3d(gd);
+  psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
+  if (d3) k_dest_hist<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->cursor);
+  else k_dest_hist<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->cursor);
+  PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_COUNT, s);
+  {
+    const int rc = run_scan(c, offs_new, s);
+    if (rc) return rc;
+  }
+  psc_prof_begin(c, PSC_PH_SORT_RANK, s);
+  if (d3) k_dir_base<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, offs_new);
+  else k_dir_base<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, offs_new);
+  PSC_LAUNCH_CHECK(c);
+  const int rblocks = (int)min((int64_t)c->sm_count * 32, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
+  if (d3) k_rank<true><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_old, c->dcode, c->dircnt, c->perm, c->d_flags);
+  else k_rank<false><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_old, c->dcode, c->dircnt, c->perm, c->d_flags);
+  PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_RANK, s);
+  c->ocur ^= 1;
+  c->state = PSC_STATE_INDEXED;
+  c->have_sort_result = 2;
+  return PSC_OK;
+}
+
+// INDEXED -> SORTED: the physical reorder the next push would otherwise do on load
+int psc_sort_materialize(psc_ctx *c, cudaStream_t s) {
+  const int n = (int)c->np;
+  const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
+  ProfScope ps(c, PSC_PH_SORT_REORDER, s);
+  k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(c->gd, n, c->perm, c->cols[c->cur], c->cols[c->cur ^ 1]);
+  PSC_LAUNCH_CHECK(c);
+  c->cur ^= 1;
+  c->state = PSC_STATE_SORTED;
+  return PSC_OK;
+}
+
+// cell_idx[a] of the last sort's INPUT particles
 int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s) {
   const int n = (int)c->np;
   if (n == 0) return PSC_OK;
-  k_cell_idx<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key[c->kcur ^ 1], c->cell_idx);
+  if (c->have_sort_result == 2) {  // index sort: input key = old slot's cell moved by the code
+    const int rc = slot_keys(c, c->offs[c->ocur ^ 1], c->dcode, c->key, s);
+    if (rc) return rc;
+  }
+  k_cell_idx<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key, c->cell_idx);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
@@ -497,11 +733,14 @@ int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s) {
 int psc_particles_to_abs(psc_ctx *c, cudaStream_t s) {
   const int n = (int)c->np;
   if (n) {
+    const int rc = psc_sort_current_keys(c, s);
+    if (rc) return rc;
     const Cols &p = c->cols[c->cur];
-    k_to_abs<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key[c->kcur], p.x, p.y, p.z);
+    k_to_abs<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->curkey, p.x, p.y, p.z);
     PSC_LAUNCH_CHECK(c);
   }
   c->form = PSC_FORM_ABS;
   c->state = PSC_STATE_UNSORTED;
+  c->have_sort_result = 0;
   return PSC_OK;
 }

@@ -10,7 +10,7 @@ from . import COLUMNS, PSC_B, PSC_E, PSC_GHOST, Psc
 
 
 class Simulation:
-    def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True):
+    def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True, with_x=True):
         self.device = torch.device(device)
         self.plasma = plasma
         self.psc = Psc(plasma.n, plasma.dx, plasma.dt, plasma.order, plasma.q, plasma.m, block)
@@ -28,8 +28,8 @@ class Simulation:
         for k in range(2):
             s = {}
             for c in COLUMNS:
-                if c == "id" and not with_id:
-                    s[c] = None
+                if (c == "id" and not with_id) or (c == "x" and not with_x):
+                    s[c] = None       # optional columns (include/psc.h): not carried
                     continue
                 dt = torch.int32 if c in ("species", "id") else torch.float32
                 s[c] = torch.empty(max(self.np, 1), dtype=dt, device=dev)
@@ -50,9 +50,9 @@ class Simulation:
 
     def current(self):
         """the column set (dict of tensors, trimmed to n particles) that holds the particles now"""
-        ptr = self.psc.particles_current()["x"]
-        s = self.sets[0] if self.sets[0]["x"].data_ptr() == ptr else self.sets[1]
-        assert s["x"].data_ptr() == ptr
+        ptr = self.psc.particles_current()["y"]
+        s = self.sets[0] if self.sets[0]["y"].data_ptr() == ptr else self.sets[1]
+        assert s["y"].data_ptr() == ptr
         return {c: (None if t is None else t[: self.np]) for c, t in s.items()}
 
     def _ws_view(self, ptr, count):

@@ -7,7 +7,7 @@ import pytest
 import torch
 
 import psc_inputs
-from tests.util import (gpu_cols, gpu_positions_f64, library_block, oracle_for, oracle_sorted_state, oracle_state,
+from tests.util import (gpu_cols, gpu_positions_f64, key_to_cell, library_block, oracle_for, oracle_sorted_state, oracle_state,
                         periodic_dist, rel_fieldnorm, rel_maxnorm, smooth_fields)
 
 pytestmark = pytest.mark.gpu
@@ -126,6 +126,91 @@ def test_sort_bit_exact(kind, block):
         assert np.array_equal(after[k], v[perm]), k
 
 
+@pytest.mark.parametrize("kind,block", [("2d", (0, 0, 0)), ("2d-ragged", (1, 4, 8)), ("2d-ragged", (1, 24, 40)),
+                                        ("3d", (0, 0, 0)), ("3d-ragged", (2, 4, 2)), ("3d-ragged", (1, 1, 1)),
+                                        ("harris", (1, 8, 8)), ("beam", (0, 0, 0))])
+def test_index_sort_bit_exact(kind, block):
+    """steady state: the sort of a list a push has advanced works from the direction codes the
+    push left (index sort).  The cells the particles are in are the GPU's own
+    decision (its fp32 move); given those, keys, offsets and the stable permutation must equal
+    the oracle's counting sort bit for bit -- three sort/push rounds, the last through psc_step's
+    lazy form (reorder on load)."""
+    pl = _small(kind)
+    smooth_fields(pl, 0.05, seed=21)
+    sim = _sim(pl, block=block)
+    lb = library_block(pl.n, block)
+    orc = oracle_for(pl, block=lb)
+    sim.psc.particles_sort()
+    for it in range(3):
+        if it < 2:
+            sim.psc.push_particles()
+        else:
+            sim.psc.step()                       # (list is sorted: push only)
+            sim.psc.step()                       # index sort + push with reorder on load
+        before = {k: v.copy() for k, v in gpu_cols(sim, export=False).items()}
+        cells = [np.ascontiguousarray(v.astype(np.int32)) for v in
+                 key_to_cell(sim.keys().cpu().numpy().astype(np.int64), pl.n, lb)]
+        cell_idx, key, perm, offs = orc.sort_cells(*cells)
+        assert np.array_equal(key, sim.keys().cpu().numpy())
+        moved = int((np.diff(key) < 0).sum())
+        assert moved > 0                         # the push really un-sorted the list
+        sim.psc.particles_sort()
+        assert sim.psc.status() == 0
+        g_ci, g_pm, g_co = (t.cpu().numpy() for t in sim.sort_result())
+        assert np.array_equal(g_co, offs)
+        assert np.array_equal(g_pm, perm)
+        assert np.array_equal(g_ci, cell_idx)
+        after = gpu_cols(sim, export=False)
+        for k, v in before.items():
+            assert np.array_equal(after[k], v[perm]), k
+        assert np.array_equal(sim.keys().cpu().numpy(), key[perm])
+
+
+def test_step_equals_explicit_calls():
+    """psc_step (index sort + reorder on load) gives the same state as the explicit sequence
+    psc_particles_sort, psc_push_fields, psc_push_particles, ... of Fig. 8: particle columns
+    bit for bit after the first step (same arithmetic on the same values), within rounding of
+    the atomically summed J afterwards"""
+    pl = _small("2d")
+    a, b = _sim(pl), _sim(pl)
+    for it in range(4):
+        a.psc.step()
+        b.psc.particles_sort()
+        b.psc.push_fields(1, 0.5)
+        b.psc.push_particles()
+        b.psc.push_fields(1, 0.5)
+        b.psc.exchange_j()
+        b.psc.push_fields(0, 1.0)
+        ca, cb = gpu_cols(a, export=False), gpu_cols(b, export=False)
+        ka, kb = a.keys().cpu().numpy(), b.keys().cpu().numpy()
+        ia, ib = np.argsort(ca["id"], kind="stable"), np.argsort(cb["id"], kind="stable")
+        if it == 0:
+            for k in ca:
+                assert np.array_equal(ca[k][ia], cb[k][ib]), k
+            assert np.array_equal(ka[ia], kb[ib])
+        else:
+            for k in ("ux", "uy", "uz"):
+                assert np.abs(ca[k][ia] - cb[k][ib]).max() < 1e-6
+        assert (a.J - b.J).abs().max() <= 1e-5 * b.J.abs().max()
+    assert a.psc.status() == 0 and b.psc.status() == 0
+
+
+def test_invariant_coordinate_is_optional():
+    """2-d run with x == NULL (not carried): same y, z, u as with x bound"""
+    from paper_1310_7866_b200.harness import Simulation
+    pl = _small("2d-ragged")
+    a = Simulation(pl)
+    b = Simulation(pl, with_x=False)
+    a.step(3)
+    b.step(3)
+    ca, cb = gpu_cols(a, export=False), gpu_cols(b, export=False)
+    assert "x" not in cb
+    ia, ib = np.argsort(ca["id"], kind="stable"), np.argsort(cb["id"], kind="stable")
+    for k in ("y", "z", "ux", "uy", "uz", "qw", "species"):
+        assert np.allclose(ca[k][ia], cb[k][ib], rtol=0, atol=1e-6), k
+    assert b.psc.status() == 0
+
+
 def test_sort_degenerate_cases():
     # empty list
     pl = psc_inputs.thermal((1, 8, 8), 1, seed=3)
@@ -133,9 +218,12 @@ def test_sort_degenerate_cases():
         setattr(pl, k, getattr(pl, k)[:0])
     sim = _sim(pl)
     sim.psc.particles_sort()
-    sim.psc.push_particles()
-    assert sim.psc.status() == 0
     assert int(sim.sort_result()[2].abs().max()) == 0
+    sim.psc.push_particles()
+    sim.psc.particles_sort()                     # index sort of an empty pushed list
+    assert int(sim.sort_result()[2].abs().max()) == 0
+    sim.step(2)
+    assert sim.psc.status() == 0
     # everything in very few cells: segments of ~3000 (shared-memory block sort) and ~70000
     # (in-place global sort) particles
     for count in (3000, 70000):

@@ -306,6 +306,35 @@ def test_sort_against_numpy_stable_argsort(n, block):
     assert np.all(np.diff(blk) >= 0)
 
 
+@pytest.mark.parametrize("n,block", [((1, 16, 24), (1, 4, 8)), ((8, 12, 16), (4, 4, 4))])
+def test_sort_cells_against_numpy_stable_argsort(n, block):
+    """the sort with integer cells given: same keys / offsets / stable permutation as numpy's
+    stable argsort of the block-major key, and identical to sort() on positions in those cells"""
+    rng = np.random.default_rng(4)
+    npart = 4000
+    orc = Oracle(n, (1.0, 1.0, 1.0), 0.3, 1, [-1.0], [1.0], block=block)
+    c = [rng.integers(0, n[d], npart).astype(np.int32) for d in range(3)]
+    cell_idx, key, perm, offs = orc.sort_cells(*c)
+    c64 = [v.astype(np.int64) for v in c]
+    assert np.array_equal(cell_idx, (c64[2] * n[1] + c64[1]) * n[0] + c64[0])
+    nb = [n[d] // block[d] for d in range(3)]
+    b = [c64[d] // block[d] for d in range(3)]
+    l = [c64[d] % block[d] for d in range(3)]
+    want_key = ((b[2] * nb[1] + b[1]) * nb[0] + b[0]) * (block[0] * block[1] * block[2]) \
+        + (l[2] * block[1] + l[1]) * block[0] + l[0]
+    assert np.array_equal(key, want_key)
+    assert np.array_equal(perm, np.argsort(want_key, kind="stable"))
+    hist = np.bincount(want_key, minlength=n[0] * n[1] * n[2])
+    assert np.array_equal(offs, np.concatenate([[0], np.cumsum(hist)]))
+    pos = [(c[d] + rng.random(npart) * 0.99).astype(np.float32) for d in range(3)]
+    for got, want in zip(orc.sort(*pos), (cell_idx, key, perm, offs)):
+        assert np.array_equal(got, want)
+    with pytest.raises(ValueError):
+        bad = c[2].copy()
+        bad[7] = n[2]
+        orc.sort_cells(c[0], c[1], bad)
+
+
 def test_sort_rejects_out_of_domain():
     orc = Oracle((1, 8, 8), (1.0, 1.0, 1.0), 0.3, 1, [-1.0], [1.0], block=(1, 4, 4))
     z = np.array([8.0], dtype=np.float32)
