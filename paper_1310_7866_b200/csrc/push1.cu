@@ -38,7 +38,7 @@
 
 namespace {
 
-constexpr int PUSH_THREADS = 256;
+
 
 template <bool D3>
 struct TileGeom {
@@ -308,8 +308,8 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
   }
 }
 
-template <bool D3>
-__global__ void __launch_bounds__(PUSH_THREADS, 3)
+template <bool D3, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         const int *__restrict__ offs, uint8_t *__restrict__ dcode, int *__restrict__ dircnt,
         const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
@@ -325,6 +325,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
   float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QW][QCAP]
   float *myQ = sQ + warp * (QW * QCAP);
+  int *sOffs = (int *)(sQ + nwarps * (QW * QCAP));  // [cpb + 1]: slot ranges of the tile's cells
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
@@ -337,13 +338,17 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
     sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
   }
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
+  const int kbase = blockIdx.x * gd.cpb;
+  for (int i = threadIdx.x; i <= gd.cpb; i += blockDim.x) sOffs[i] = offs[kbase + i];
   DirCount<D3> dirs;
   dirs.init(sDir + warp * 32, lane);
   __syncthreads();
+  for (int i = threadIdx.x; i < gd.cpb; i += blockDim.x)  // empty cells send nothing anywhere
+    if (sOffs[i + 1] == sOffs[i])
+      for (int d = 0; d < DirCount<D3>::ND; d++) dircnt[(kbase + i) * DirCount<D3>::ND + d] = 0;
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   uint32_t bad = 0;
-  const int kbase = blockIdx.x * gd.cpb;
   const unsigned lt = lanemask_lt_();
   const float cdx = D3 ? gd.dt_dx[0] : 0.f, cdy = gd.dt_dx[1], cdz = gd.dt_dx[2];
 
@@ -368,34 +373,95 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
-  for (int ci = warp; ci < gd.cpb; ci += nwarps) {
-    const int p0 = offs[kbase + ci], p1 = offs[kbase + ci + 1];
-    const int lx = ci % gd.bs[0], lt_ = ci / gd.bs[0];
-    const int ly = lt_ % gd.bs[1], lz = lt_ / gd.bs[1];
-    const int packed = lx | (ly << 10) | (lz << 20);
-    // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
-    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
-                               : (lz + 1) * tg.fe[1] + (ly + 1));
-    float acc[NV];
-#pragma unroll
-    for (int i = 0; i < NV; i++) acc[i] = 0.f;
-
-    for (int base = p0; base < p1; base += 32) {
-      const int s = base + lane;
-      const bool act = s < p1;
-      float ax = 0.f, ay = 0.f, az = 0.f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
-      int sp = 0, p = s;
-      if (act) {
-        if (perm) p = ld_stream(perm + s);
-        ay = ld_stream(in.y + p);
-        az = ld_stream(in.z + p);
-        ux = ld_stream(in.ux + p);
-        uy = ld_stream(in.uy + p);
-        uz = ld_stream(in.uz + p);
-        qw = ld_stream(in.qw + p);
-        sp = ld_stream(in.sp + p);
-        if (D3) ax = ld_stream(in.x + p);
+  // The warp's work is the sequence of 32-slot chunks of its cells (cells warp, warp + nwarps,
+  // ...; empty cells skipped).  It is software-pipelined: the columns of chunk t+1 are loaded
+  // (through perm: reorder on load) before chunk t is computed, and perm of chunk t+2 with them,
+  // so that a DRAM round trip is hidden behind one chunk of arithmetic.
+  struct It {
+    int ci, base, p1;
+    bool ok;
+  };
+  auto adv = [&](It &it) {
+    it.base += 32;
+    while (it.base >= it.p1) {
+      it.ci += nwarps;
+      if (it.ci >= gd.cpb) {
+        it.ok = false;
+        return;
       }
+      it.base = sOffs[it.ci];
+      it.p1 = sOffs[it.ci + 1];
+    }
+  };
+  struct Raw {
+    float ax, ay, az, ux, uy, uz, qw, cx;
+    int sp, id;
+  };
+  auto load_perm = [&](const It &it) -> int {
+    const int s = it.base + lane;
+    return (perm && s < it.p1) ? ld_stream(perm + s) : s;
+  };
+  auto load_cols = [&](Raw &r, const It &it, int p) {
+    r.ax = r.ay = r.az = r.ux = r.uy = r.uz = r.qw = r.cx = 0.f;
+    r.sp = r.id = 0;
+    if (it.base + lane < it.p1) {
+      r.ay = __ldg(in.y + p);
+      r.az = __ldg(in.z + p);
+      r.ux = __ldg(in.ux + p);
+      r.uy = __ldg(in.uy + p);
+      r.uz = __ldg(in.uz + p);
+      r.qw = __ldg(in.qw + p);
+      r.sp = __ldg(in.sp + p);
+      if (D3) r.ax = __ldg(in.x + p);
+      else if (in.x) r.cx = __ldg(in.x + p);  // invariant coordinate: carried
+      if (in.id) r.id = __ldg(in.id + p);
+    }
+  };
+
+  It a = {warp - nwarps, 0, 0, true};
+  adv(a);
+  It pp = a;
+  Raw nx;
+  int pA = 0, pP = 0;
+  if (a.ok) {
+    pA = load_perm(a);
+    load_cols(nx, a, pA);
+    adv(pp);
+    if (pp.ok) pP = load_perm(pp);
+  }
+  int cur_ci = -1, lx = 0, ly = 0, lz = 0, packed = 0;
+  const float *cF = sF;
+  float acc[NV];
+
+  while (a.ok) {
+    const It c = a;
+    const Raw cur = nx;
+    adv(a);
+    pA = pP;
+    if (a.ok) load_cols(nx, a, pA);
+    if (pp.ok) {
+      adv(pp);
+      if (pp.ok) pP = load_perm(pp);
+    }
+    if (c.ci != cur_ci) {  // first chunk of a cell
+      cur_ci = c.ci;
+      lx = c.ci % gd.bs[0];
+      const int lt_ = c.ci / gd.bs[0];
+      ly = lt_ % gd.bs[1];
+      lz = lt_ / gd.bs[1];
+      packed = lx | (ly << 10) | (lz << 20);
+      // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
+      cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
+                    : (lz + 1) * tg.fe[1] + (ly + 1));
+#pragma unroll
+      for (int i = 0; i < NV; i++) acc[i] = 0.f;
+    }
+    {
+      const int s = c.base + lane;
+      const bool act = s < c.p1;
+      const float ax = cur.ax, ay = cur.ay, az = cur.az, qw = cur.qw;
+      float ux = cur.ux, uy = cur.uy, uz = cur.uz;
+      const int sp = cur.sp;
 
       // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) --------
       // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l
@@ -466,7 +532,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
           st_stream(out.x + s, bx_);
           if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
         } else if (in.x) {
-          st_stream(out.x + s, ld_stream(in.x + p));  // invariant coordinate: carried
+          st_stream(out.x + s, cur.cx);  // invariant coordinate: carried
         }
         st_stream(out.y + s, by_);
         st_stream(out.z + s, bz_);
@@ -475,14 +541,15 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         st_stream(out.uz + s, uz);
         st_stream(out.qw + s, qw);
         st_stream(out.sp + s, sp);
-        if (in.id) st_stream(out.id + s, ld_stream(in.id + p));
+        if (in.id) st_stream(out.id + s, cur.id);
         dcode[s] = (uint8_t)dc;
         if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
       }
     }
 
-    // ---- the cell's in-cell currents: one warp reduction, one shared add per J point -------
-    if (p1 > p0) {
+    // ---- last chunk of the cell: its in-cell currents take one warp reduction and one shared
+    // add per J point; its direction-code counts go to the index sort
+    if (!a.ok || a.ci != c.ci) {
       float r;
       if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
       else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(acc), lane);
@@ -491,8 +558,8 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
                             : (lz + 1) * tg.je[1] + (ly + 1);
         atomicAdd(&sJ[node + my_off], r);
       }
+      dirs.cell_done(dircnt, kbase + c.ci, lane);
     }
-    dirs.cell_done(dircnt, kbase + ci, lane);
   }
   if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, 0, qcnt, lane);
   if (bad) atomicOr(flags, bad);
@@ -524,22 +591,37 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       fvol *= gd.bs[d] + 2;
       jvol *= gd.bs[d] + 3;
     }
-  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH_THREADS;
-  if (threads < 32 || threads > PUSH_THREADS) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP)) * sizeof(float);
+  const int vthreads = c->opt_push_variant == 3 ? 256 : 128;
+  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : vthreads;
+  if (threads < 32 || threads > vthreads) return PSC_ERR_INVALID_ARG;
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP) + gd.cpb + 1) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &in = c->cols[c->cur];
   const Cols &out = c->cols[c->cur ^ 1];
   const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
   ProfScope ps(c, PSC_PH_PUSH, s);
+#define PSC_LAUNCH_PUSH1(D3_, T_, B_)                                                              \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, T_, B_>,                                     \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    k_push1<D3_, T_, B_><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur],     \
+                                                          c->dcode, c->dircnt, c->E, c->B, c->J,   \
+                                                          c->d_flags);                             \
+  } while (0)
+  const int v = c->opt_push_variant;
   if (d3) {
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
+    if (v == 1) PSC_LAUNCH_PUSH1(true, 128, 6);
+    else if (v == 2) PSC_LAUNCH_PUSH1(true, 128, 4);
+    else if (v == 3) PSC_LAUNCH_PUSH1(true, 256, 3);
+    else PSC_LAUNCH_PUSH1(true, 128, 5);
   } else {
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push1<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
+    if (v == 1) PSC_LAUNCH_PUSH1(false, 128, 6);
+    else if (v == 2) PSC_LAUNCH_PUSH1(false, 128, 4);
+    else if (v == 3) PSC_LAUNCH_PUSH1(false, 256, 3);
+    else PSC_LAUNCH_PUSH1(false, 128, 5);
   }
+#undef PSC_LAUNCH_PUSH1
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
