@@ -40,32 +40,40 @@ namespace {
 
 
 
-template <bool D3>
+// Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
+// library defaults, 8x8 in 2-d and 4x4x4 in 3-d), known at compile time so that every tile
+// extent, stride and shared-memory offset folds into an immediate; CBS == 0: run-time block.
+template <bool D3, int CBS>
 struct TileGeom {
   int o[3];        // first cell of the tile (global cell coordinates)
+  int bs[3], cpb;  // block size in cells, cells per block
   int fe[3], fvol; // field tile extents (bs+2 | 1), volume
   int je[3], jvol; // J tile extents (bs+3 | 1), volume
   __device__ __forceinline__ void init(const GridDesc &gd, int tile) {
+    bs[0] = CBS ? (D3 ? CBS : 1) : gd.bs[0];
+    bs[1] = CBS ? CBS : gd.bs[1];
+    bs[2] = CBS ? CBS : gd.bs[2];
+    cpb = bs[0] * bs[1] * bs[2];
     const int b0 = tile % gd.nb[0];
     const int r = tile / gd.nb[0];
     const int b1 = r % gd.nb[1], b2 = r / gd.nb[1];
-    o[0] = b0 * gd.bs[0];
-    o[1] = b1 * gd.bs[1];
-    o[2] = b2 * gd.bs[2];
-    fe[0] = D3 ? gd.bs[0] + 2 : 1;
-    fe[1] = gd.bs[1] + 2;
-    fe[2] = gd.bs[2] + 2;
-    je[0] = D3 ? gd.bs[0] + 3 : 1;
-    je[1] = gd.bs[1] + 3;
-    je[2] = gd.bs[2] + 3;
+    o[0] = b0 * bs[0];
+    o[1] = b1 * bs[1];
+    o[2] = b2 * bs[2];
+    fe[0] = D3 ? bs[0] + 2 : 1;
+    fe[1] = bs[1] + 2;
+    fe[2] = bs[2] + 2;
+    je[0] = D3 ? bs[0] + 3 : 1;
+    je[1] = bs[1] + 3;
+    je[2] = bs[2] + 3;
     fvol = fe[0] * fe[1] * fe[2];
     jvol = je[0] * je[1] * je[2];
   }
 };
 
 // one VB segment in the cell with tile-local coordinates (cx,cy,cz); a*, b* in-cell start/end
-template <bool D3>
-__device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TileGeom<D3> &tg, int cx,
+template <bool D3, class TG>
+__device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TG &tg, int cx,
                                            int cy, int cz, float ax, float ay, float az, float bx,
                                            float by, float bz, float tau, float fx, float fy,
                                            float fz, float qvx) {
@@ -224,8 +232,8 @@ __device__ __forceinline__ void vb_values(float (&v)[D3 ? 12 : 8], float ax, flo
 // dt <= dx/2) and deposits every segment from number `first_seg` on with
 // shared-memory atomics.  first_seg = 1 is the slow path of the kernel below: segment 0 (inside
 // the home cell) has already gone through the warp reduction.
-template <bool D3>
-__device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TileGeom<D3> &tg, int lx,
+template <bool D3, class TG>
+__device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, int lx,
                                         int ly, int lz, float ax, float ay, float az, float ddx,
                                         float ddy, float ddz, float fx, float fy, float fz,
                                         float qvx, int first_seg) {
@@ -268,8 +276,8 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TileGeom<D
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
 constexpr int QW = 8;      // words per entry
 
-template <bool D3>
-__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TileGeom<D3> &tg,
+template <bool D3, class TG>
+__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg,
                                             const GridDesc &gd, const float *__restrict__ q,
                                             int start, int n, int lane) {
   if (lane < n) {
@@ -308,7 +316,7 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
   }
 }
 
-template <bool D3, int THREADS, int MINB>
+template <bool D3, int CBS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         const int *__restrict__ offs, uint8_t *__restrict__ dcode, int *__restrict__ dircnt,
@@ -316,7 +324,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   constexpr int NV = D3 ? 12 : 8;
-  TileGeom<D3> tg;
+  TileGeom<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   float *sF = smem;                           // [6][fvol]: Ex Ey Ez Bx By Bz
@@ -338,14 +346,13 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
     sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
   }
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
-  const int kbase = blockIdx.x * gd.cpb;
-  for (int i = threadIdx.x; i <= gd.cpb; i += blockDim.x) sOffs[i] = offs[kbase + i];
-  DirCount<D3> dirs;
-  dirs.init(sDir + warp * 32, lane);
+  const int kbase = blockIdx.x * tg.cpb;
+  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) sOffs[i] = offs[kbase + i];
+  sDir[warp * 32 + lane] = 0;
   __syncthreads();
-  for (int i = threadIdx.x; i < gd.cpb; i += blockDim.x)  // empty cells send nothing anywhere
+  for (int i = threadIdx.x; i < tg.cpb; i += blockDim.x)  // empty cells send nothing anywhere
     if (sOffs[i + 1] == sOffs[i])
-      for (int d = 0; d < DirCount<D3>::ND; d++) dircnt[(kbase + i) * DirCount<D3>::ND + d] = 0;
+      for (int d = 0; d < (D3 ? 27 : 9); d++) dircnt[(kbase + i) * (D3 ? 27 : 9) + d] = 0;
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   uint32_t bad = 0;
@@ -385,7 +392,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
     it.base += 32;
     while (it.base >= it.p1) {
       it.ci += nwarps;
-      if (it.ci >= gd.cpb) {
+      if (it.ci >= tg.cpb) {
         it.ok = false;
         return;
       }
@@ -423,6 +430,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   It pp = a;
   Raw nx;
   int pA = 0, pP = 0;
+  int ncross = 0;  // warp-uniform: leavers of the current cell so far
   if (a.ok) {
     pA = load_perm(a);
     load_cols(nx, a, pA);
@@ -436,19 +444,19 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   while (a.ok) {
     const It c = a;
     const Raw cur = nx;
-    adv(a);
+    a = pp;  // chunk t+1 (what the perm iterator pointed at)
     pA = pP;
-    if (a.ok) load_cols(nx, a, pA);
-    if (pp.ok) {
+    if (a.ok) {
+      load_cols(nx, a, pA);
       adv(pp);
       if (pp.ok) pP = load_perm(pp);
     }
     if (c.ci != cur_ci) {  // first chunk of a cell
       cur_ci = c.ci;
-      lx = c.ci % gd.bs[0];
-      const int lt_ = c.ci / gd.bs[0];
-      ly = lt_ % gd.bs[1];
-      lz = lt_ / gd.bs[1];
+      lx = c.ci % tg.bs[0];
+      const int lt_ = c.ci / tg.bs[0];
+      ly = lt_ % tg.bs[1];
+      lz = lt_ / tg.bs[1];
       packed = lx | (ly << 10) | (lz << 20);
       // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
       cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
@@ -488,7 +496,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
       const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
       const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
       const int dc = dir_code<D3>(sxd, syd, szd);
-      const bool cross = act && dc != DirCount<D3>::STAY;
+      const bool cross = act && dc != (D3 ? 13 : 4);
 
       // ---- Villasenor-Buneman deposit ---------------------------------------------------------
       // a trajectory that stays in the cell is one segment: its currents go to the per-cell
@@ -514,14 +522,15 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
           myQ[6 * QCAP + e] = ddz;
           myQ[7 * QCAP + e] = qw;
         }
+        if (cross) atomicAdd(&sDir[warp * 32 + dc], 1);
         qcnt += __popc(cm);
+        ncross += __popc(cm);
         __syncwarp();
         if (qcnt >= 32) {
           qcnt -= 32;
           drain_queue<D3>(sJ, tg, gd, myQ, qcnt, 32, lane);
         }
       }
-      dirs.add(act, dc);
 
       // ---- store slot s of the other column set: new offset, momentum, direction code -----
       if (act) {
@@ -558,7 +567,18 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
                             : (lz + 1) * tg.je[1] + (ly + 1);
         atomicAdd(&sJ[node + my_off], r);
       }
-      dirs.cell_done(dircnt, kbase + c.ci, lane);
+      // direction-code counts of the cell: the leavers were counted above, the rest stayed
+      {
+        constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
+        int *row = sDir + warp * 32;
+        if (lane < ND) {
+          const int p0c = sOffs[c.ci];
+          dircnt[(kbase + c.ci) * ND + lane] = lane == STAY ? (c.p1 - p0c) - ncross : row[lane];
+          row[lane] = 0;
+        }
+        ncross = 0;
+        __syncwarp();
+      }
     }
   }
   if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, 0, qcnt, lane);
@@ -591,7 +611,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       fvol *= gd.bs[d] + 2;
       jvol *= gd.bs[d] + 3;
     }
-  const int vthreads = c->opt_push_variant == 3 ? 256 : 128;
+  const int vthreads = 128;
   const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : vthreads;
   if (threads < 32 || threads > vthreads) return PSC_ERR_INVALID_ARG;
   const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP) + gd.cpb + 1) * sizeof(float);
@@ -601,25 +621,23 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const Cols &out = c->cols[c->cur ^ 1];
   const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
   ProfScope ps(c, PSC_PH_PUSH, s);
-#define PSC_LAUNCH_PUSH1(D3_, T_, B_)                                                              \
+#define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, T_, B_>,                                     \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_>,                               \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    k_push1<D3_, T_, B_><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur],     \
-                                                          c->dcode, c->dircnt, c->E, c->B, c->J,   \
-                                                          c->d_flags);                             \
+    k_push1<D3_, CBS_, T_, B_><<<gd.ntiles, threads, smem, s>>>(                                   \
+        gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);   \
   } while (0)
   const int v = c->opt_push_variant;
   if (d3) {
-    if (v == 1) PSC_LAUNCH_PUSH1(true, 128, 6);
-    else if (v == 2) PSC_LAUNCH_PUSH1(true, 128, 4);
-    else if (v == 3) PSC_LAUNCH_PUSH1(true, 256, 3);
-    else PSC_LAUNCH_PUSH1(true, 128, 5);
+    const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4 && v != 2;
+    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4);
+    else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
   } else {
-    if (v == 1) PSC_LAUNCH_PUSH1(false, 128, 6);
-    else if (v == 2) PSC_LAUNCH_PUSH1(false, 128, 4);
-    else if (v == 3) PSC_LAUNCH_PUSH1(false, 256, 3);
-    else PSC_LAUNCH_PUSH1(false, 128, 5);
+    const bool def = gd.bs[1] == 8 && gd.bs[2] == 8 && v != 2;
+    if (def && v == 1) PSC_LAUNCH_PUSH1(false, 8, 128, 6);
+    else if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
+    else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
   }
 #undef PSC_LAUNCH_PUSH1
   PSC_LAUNCH_CHECK(c);
