@@ -246,11 +246,7 @@ int psc_particles_sort(psc_ctx *c, void *stream) {
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
   cudaStream_t s = (cudaStream_t)stream;
   ProfScope ps(c, PSC_PH_SORT, s);
-  int rc = PSC_OK;
-  if (c->state == PSC_STATE_PUSHED) rc = psc_sort_index(c, s);  // steady state: keys/indices only
-  if (rc == PSC_OK && c->state == PSC_STATE_INDEXED) return psc_sort_materialize(c, s);
-  if (rc) return rc;
-  return psc_sort_general(c, s);
+  return psc_sort_general(c, s);  // the physically sorted, stable list this call promises
 }
 
 // the sort as psc_step uses it: after a push only the index sort runs, and the physical reorder

@@ -38,10 +38,14 @@ struct Cols {
 // Where the particle list is in the sort / push cycle (internal form unless UNSORTED):
 //   UNSORTED  absolute positions in arbitrary order (after bind or export)
 //   SORTED    the current column set is physically in sorted order; offs[ocur] = cell offsets
-//   PUSHED    the current set is in the slot order of offs[ocur], every particle carries the
-//             direction code of its move (dcode) and dircnt holds the per-cell code counts
-//   INDEXED   the current set is still in the OLD slot order (offs[ocur^1]); perm and
-//             offs[ocur] describe the new sorted order (reorder happens on the next load)
+//   PUSHED    the current set is the list a push wrote: cell k's particles of BEFORE the push in
+//             [offs[ocur][k], offs[ocur][k+1]), its stayers first (dircnt[k][STAY] of them), then
+//             its leavers, each leaver with the direction code of its move in dcode[slot];
+//             dircnt holds the per-cell code counts
+//   INDEXED   the current set is still that written list (layout offs[ocur^1]); offs[ocur] are
+//             the cell offsets of the new order, nstay / aoffs / alist say where each cell's
+//             particles are (a run of stayers + listed arrivals; reorder happens on the next
+//             load); dircnt[k][dc != STAY] now hold arrival-list bases
 enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1, PSC_STATE_PUSHED = 2, PSC_STATE_INDEXED = 3 };
 enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
 
@@ -76,12 +80,14 @@ struct psc_ctx {
   int state;
   int form;        // PSC_FORM_ABS: absolute positions; PSC_FORM_REL: in-cell offsets
   int ocur;        // offs[ocur]: offsets of the latest sort
-  int have_sort_result;  // 0: none; 1: key[] holds the input keys; 2: input keys = old offs + dcode
+  int have_sort_result;  // 0: none; 1: key[] holds the input keys of the last general sort
   // workspace carve-up (all device pointers)
   void *ws;
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
-  int32_t *key, *curkey, *perm, *cell_idx, *offs[2], *cursor, *scan_tmp, *big_list, *dircnt;
+  int32_t *key, *curkey, *perm, *cell_idx, *offs[2], *cursor, *big_list, *dircnt;
+  int32_t *alist, *aoffs, *nstay;  // index sort: arrival list, its per-cell offsets, stayers per cell
+  long long *pack, *packloc, *scan_tmp;
   uint8_t *dcode;
   uint32_t *d_flags;  // owned: 16 words; [0] sticky flags, [1] big-segment counter
   int64_t launches;
@@ -129,9 +135,8 @@ int psc_fields_fold(psc_ctx *c, float *F, cudaStream_t s);
 // sort.cu
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n);
 int psc_sort_carve(psc_ctx *c, int64_t n);
-int psc_sort_general(psc_ctx *c, cudaStream_t s);      // UNSORTED | SORTED -> SORTED
+int psc_sort_general(psc_ctx *c, cudaStream_t s);      // any state -> SORTED (stable)
 int psc_sort_index(psc_ctx *c, cudaStream_t s);        // PUSHED -> INDEXED
-int psc_sort_materialize(psc_ctx *c, cudaStream_t s);  // INDEXED -> SORTED
 int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s);
 int psc_sort_current_keys(psc_ctx *c, cudaStream_t s);  // key[] := keys of the current particles
 int psc_particles_to_abs(psc_ctx *c, cudaStream_t s);

@@ -12,11 +12,12 @@
 // reduced across the warp once per cell.
 //
 // This is the single particle loop of PAPER.md:603 ("only one loop each time step that reads
-// and writes all particle data"): slot s of the new sorted order loads particle perm[s] of the
-// old list (reorder on load; perm comes from the index sort of sort.cu and is the identity after
-// a physical sort), and the kernel writes the advanced particle to slot s of the OTHER column
-// set together with the one-byte direction code of its move; per cell it writes the count of
-// each code.  Those two are all the next sort reads.
+// and writes all particle data"): a cell's particles are loaded as one contiguous run (the
+// stayers of the previous step) plus a short indexed list of arrivals (reorder on load; both
+// from the index sort of sort.cu), and the advanced particles are written to the cell's segment
+// of the OTHER column set -- those that stay in the cell compacted at the front, the leavers at
+// the back with the one-byte direction code of their move; per cell the kernel writes the count
+// of each code.  The leavers' codes and the counts are all the next sort reads.
 //
 // Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction +
 // the cell key.  The move is b = a + v dt/dx; a particle that leaves its cell (b < 0 or b >= 1;
@@ -275,6 +276,8 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
 
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
 constexpr int QW = 8;      // words per entry
+constexpr int NST = 4;        // chunks in the per-warp column ring (NST - 1 in flight)
+constexpr int RING_COLS = 9;  // y z ux uy uz qw species [x] [id]
 
 template <bool D3, class TG>
 __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg,
@@ -318,10 +321,8 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
 
 template <bool D3, int CBS, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
-        const int *__restrict__ offs, uint8_t *__restrict__ dcode, int *__restrict__ dircnt,
-        const float *__restrict__ E, const float *__restrict__ B, float *__restrict__ J,
-        uint32_t *__restrict__ flags) {
+k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
+        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   constexpr int NV = D3 ? 12 : 8;
   TileGeom<D3, CBS> tg;
@@ -333,7 +334,14 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
   float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QW][QCAP]
   float *myQ = sQ + warp * (QW * QCAP);
-  int *sOffs = (int *)(sQ + nwarps * (QW * QCAP));  // [cpb + 1]: slot ranges of the tile's cells
+  float *myRing = sQ + nwarps * (QW * QCAP) + warp * (NST * RING_COLS * 32);  // [NST][RING_COLS][32]
+  int *sIn = (int *)(sQ + nwarps * (QW * QCAP + NST * RING_COLS * 32));  // [cpb]: first input slot of each cell's run
+  int *sNs = sIn + tg.cpb;                         // [cpb]: length of that run
+  int *sA = sNs + tg.cpb;                          // [cpb + 1]: first arrival-list entry
+  int *sOut = sA + tg.cpb + 1;                     // [cpb + 1]: output segments
+  uint8_t *__restrict__ dcode = pls.dcode;
+  int *__restrict__ dircnt = pls.dircnt;
+  const int *__restrict__ alist = pls.alist;
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
@@ -347,11 +355,19 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   }
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
   const int kbase = blockIdx.x * tg.cpb;
-  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) sOffs[i] = offs[kbase + i];
+  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
+    const int o = pls.offs_in[kbase + i];
+    if (i < tg.cpb) {
+      sIn[i] = o;
+      sNs[i] = pls.nstay ? pls.nstay[kbase + i] : pls.offs_in[kbase + i + 1] - o;
+    }
+    sA[i] = pls.aoffs ? pls.aoffs[kbase + i] : 0;
+    sOut[i] = pls.offs_out[kbase + i];
+  }
   sDir[warp * 32 + lane] = 0;
   __syncthreads();
   for (int i = threadIdx.x; i < tg.cpb; i += blockDim.x)  // empty cells send nothing anywhere
-    if (sOffs[i + 1] == sOffs[i])
+    if (sOut[i + 1] == sOut[i])
       for (int d = 0; d < (D3 ? 27 : 9); d++) dircnt[(kbase + i) * (D3 ? 27 : 9) + d] = 0;
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
@@ -380,12 +396,14 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
-  // The warp's work is the sequence of 32-slot chunks of its cells (cells warp, warp + nwarps,
-  // ...; empty cells skipped).  It is software-pipelined: the columns of chunk t+1 are loaded
-  // (through perm: reorder on load) before chunk t is computed, and perm of chunk t+2 with them,
-  // so that a DRAM round trip is hidden behind one chunk of arithmetic.
+  // The warp's work is the sequence of 32-particle chunks of its cells (cells warp, warp +
+  // nwarps, ...; empty cells skipped).  Particle v of a cell is slot sIn + v of the input columns
+  // if v < sNs (the cell's stayer run), else slot alist[sA + v - sNs] (an arrival: reorder on
+  // load).  The loop is software-pipelined: the columns of chunk t+1 are loaded before chunk t is
+  // computed, and the list entries of chunk t+2 with them, so that a DRAM round trip is hidden
+  // behind one chunk of arithmetic.
   struct It {
-    int ci, base, p1;
+    int ci, base, p1;  // cell, first particle of the chunk, particles in the cell
     bool ok;
   };
   auto adv = [&](It &it) {
@@ -396,8 +414,8 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         it.ok = false;
         return;
       }
-      it.base = sOffs[it.ci];
-      it.p1 = sOffs[it.ci + 1];
+      it.base = 0;
+      it.p1 = sOut[it.ci + 1] - sOut[it.ci];
     }
   };
   struct Raw {
@@ -405,52 +423,81 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
     int sp, id;
   };
   auto load_perm = [&](const It &it) -> int {
-    const int s = it.base + lane;
-    return (perm && s < it.p1) ? ld_stream(perm + s) : s;
+    const int v = it.base + lane, ns = sNs[it.ci];
+    return (v >= ns && v < it.p1) ? ld_stream(alist + (sA[it.ci] + v - ns)) : sIn[it.ci] + v;
   };
-  auto load_cols = [&](Raw &r, const It &it, int p) {
-    r.ax = r.ay = r.az = r.ux = r.uy = r.uz = r.qw = r.cx = 0.f;
-    r.sp = r.id = 0;
-    if (it.base + lane < it.p1) {
-      r.ay = __ldg(in.y + p);
-      r.az = __ldg(in.z + p);
-      r.ux = __ldg(in.ux + p);
-      r.uy = __ldg(in.uy + p);
-      r.uz = __ldg(in.uz + p);
-      r.qw = __ldg(in.qw + p);
-      r.sp = __ldg(in.sp + p);
-      if (D3) r.ax = __ldg(in.x + p);
-      else if (in.x) r.cx = __ldg(in.x + p);  // invariant coordinate: carried
-      if (in.id) r.id = __ldg(in.id + p);
+  // Particle columns travel through a per-warp shared-memory ring of NST chunks filled with
+  // asynchronous 4-byte copies (cp.async; each lane copies and later reads its own element, so no
+  // cross-lane synchronisation is involved): NST - 1 chunks of loads are in flight per warp
+  // without holding registers, which is what hides the DRAM latency at 20 warps per SM.
+  // Lanes past the end of the cell copy zero bytes, i.e. get zero-filled slots.
+  const bool has_x = D3 || in.x != nullptr, has_id = in.id != nullptr;
+  auto issue = [&](const It &it, int p, int stage) {
+    const bool v = it.base + lane < it.p1;
+    const int q = v ? p : 0;
+    float *r = myRing + stage * (RING_COLS * 32) + lane;
+    cp_async4(r + 0 * 32, in.y + q, v);
+    cp_async4(r + 1 * 32, in.z + q, v);
+    cp_async4(r + 2 * 32, in.ux + q, v);
+    cp_async4(r + 3 * 32, in.uy + q, v);
+    cp_async4(r + 4 * 32, in.uz + q, v);
+    cp_async4(r + 5 * 32, in.qw + q, v);
+    cp_async4(r + 6 * 32, in.sp + q, v);
+    if (has_x) cp_async4(r + 7 * 32, in.x + q, v);
+    if (has_id) cp_async4(r + 8 * 32, in.id + q, v);
+  };
+  auto fetch = [&](Raw &r_, int stage) {
+    const float *r = myRing + stage * (RING_COLS * 32) + lane;
+    r_.ay = r[0 * 32];
+    r_.az = r[1 * 32];
+    r_.ux = r[2 * 32];
+    r_.uy = r[3 * 32];
+    r_.uz = r[4 * 32];
+    r_.qw = r[5 * 32];
+    r_.sp = __float_as_int(r[6 * 32]);
+    r_.ax = r_.cx = 0.f;
+    if (has_x) {
+      const float t = r[7 * 32];
+      if (D3) r_.ax = t; else r_.cx = t;
     }
+    r_.id = has_id ? __float_as_int(r[8 * 32]) : 0;
   };
 
-  It a = {warp - nwarps, 0, 0, true};
+  It a = {warp - nwarps, 0, 0, true};  // the chunk to compute
   adv(a);
-  It pp = a;
-  Raw nx;
-  int pA = 0, pP = 0;
-  int ncross = 0;  // warp-uniform: leavers of the current cell so far
-  if (a.ok) {
-    pA = load_perm(a);
-    load_cols(nx, a, pA);
-    adv(pp);
-    if (pp.ok) pP = load_perm(pp);
+  It pr = a;                           // the chunk to issue loads for (NST - 1 ahead)
+  int pPr = 0;
+  if (pr.ok) pPr = load_perm(pr);
+  int stage_p = 0, stage_c = 0;
+#pragma unroll 1
+  for (int k = 0; k < NST - 1; k++) {
+    if (pr.ok) {
+      issue(pr, pPr, stage_p);
+      adv(pr);
+      if (pr.ok) pPr = load_perm(pr);
+    }
+    cp_async_commit();
+    stage_p++;
   }
+  int ncross = 0, nst = 0;  // warp-uniform: leavers / stayers of the current cell so far
   int cur_ci = -1, lx = 0, ly = 0, lz = 0, packed = 0;
   const float *cF = sF;
   float acc[NV];
 
   while (a.ok) {
     const It c = a;
-    const Raw cur = nx;
-    a = pp;  // chunk t+1 (what the perm iterator pointed at)
-    pA = pP;
-    if (a.ok) {
-      load_cols(nx, a, pA);
-      adv(pp);
-      if (pp.ok) pP = load_perm(pp);
+    if (pr.ok) {
+      issue(pr, pPr, stage_p);
+      adv(pr);
+      if (pr.ok) pPr = load_perm(pr);  // list entries one more chunk ahead
     }
+    cp_async_commit();
+    stage_p = stage_p + 1 == NST ? 0 : stage_p + 1;
+    cp_async_wait<NST - 1>();
+    Raw cur;
+    fetch(cur, stage_c);
+    stage_c = stage_c + 1 == NST ? 0 : stage_c + 1;
+    adv(a);  // a: the next chunk (tells whether this one ends its cell)
     if (c.ci != cur_ci) {  // first chunk of a cell
       cur_ci = c.ci;
       lx = c.ci % tg.bs[0];
@@ -465,8 +512,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
       for (int i = 0; i < NV; i++) acc[i] = 0.f;
     }
     {
-      const int s = c.base + lane;
-      const bool act = s < c.p1;
+      const bool act = c.base + lane < c.p1;
       const float ax = cur.ax, ay = cur.ay, az = cur.az, qw = cur.qw;
       float ux = cur.ux, uy = cur.uy, uz = cur.uz;
       const int sp = cur.sp;
@@ -510,6 +556,11 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         for (int i = 0; i < NV; i++) acc[i] += v[i];
       }
       const unsigned cm = __ballot_sync(0xffffffffu, cross);
+      const unsigned sm = __ballot_sync(0xffffffffu, act && !cross);
+      // output slot: stayers fill the cell's segment from the front, leavers from the back
+      const int s = cross ? sOut[c.ci + 1] - 1 - ncross - __popc(cm & lt)
+                          : sOut[c.ci] + nst + __popc(sm & lt);
+      nst += __popc(sm);
       if (cm) {
         if (cross) {
           const int e = qcnt + __popc(cm & lt);
@@ -551,7 +602,7 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         st_stream(out.qw + s, qw);
         st_stream(out.sp + s, sp);
         if (in.id) st_stream(out.id + s, cur.id);
-        dcode[s] = (uint8_t)dc;
+        if (cross) dcode[s] = (uint8_t)dc;
         if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
       }
     }
@@ -572,11 +623,11 @@ k_push1(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
         int *row = sDir + warp * 32;
         if (lane < ND) {
-          const int p0c = sOffs[c.ci];
-          dircnt[(kbase + c.ci) * ND + lane] = lane == STAY ? (c.p1 - p0c) - ncross : row[lane];
+          dircnt[(kbase + c.ci) * ND + lane] = lane == STAY ? nst : row[lane];
           row[lane] = 0;
         }
         ncross = 0;
+        nst = 0;
         __syncwarp();
       }
     }
@@ -614,19 +665,19 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const int vthreads = 128;
   const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : vthreads;
   if (threads < 32 || threads > vthreads) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP) + gd.cpb + 1) * sizeof(float);
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP + NST * RING_COLS * 32) + 4 * gd.cpb + 2) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &in = c->cols[c->cur];
   const Cols &out = c->cols[c->cur ^ 1];
-  const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
+  const PushLists pls = psc_push_lists(c);
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_>,                               \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
     k_push1<D3_, CBS_, T_, B_><<<gd.ntiles, threads, smem, s>>>(                                   \
-        gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);   \
+        gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                           \
   } while (0)
   const int v = c->opt_push_variant;
   if (d3) {

@@ -196,10 +196,8 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
 
 template <bool D3>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
-k_push2(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
-        const int *__restrict__ cell_offsets, uint8_t *__restrict__ dcode,
-        int *__restrict__ dircnt, const float *__restrict__ E, const float *__restrict__ B,
-        float *__restrict__ J, uint32_t *__restrict__ flags) {
+k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
+        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
   Geom2<D3> tg;
   tg.init(gd, blockIdx.x);
@@ -239,19 +237,29 @@ k_push2(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
   const int kbase = blockIdx.x * gd.cpb;
   uint32_t bad = 0;
 
+  uint8_t *__restrict__ dcode = pls.dcode;
+  int *__restrict__ dircnt = pls.dircnt;
+  const unsigned lanes_lt = lanemask_lt_();
+
   for (int ci = warp; ci < gd.cpb; ci += nwarps) {
-    const int p0 = cell_offsets[kbase + ci], p1 = cell_offsets[kbase + ci + 1];
+    // the cell's particles: its run of stayers of the previous step, then its listed arrivals
+    // (reorder on load); its output segment: stayers from the front, leavers from the back
+    const int in0 = pls.offs_in[kbase + ci];
+    const int ns = pls.nstay ? pls.nstay[kbase + ci] : pls.offs_in[kbase + ci + 1] - in0;
+    const int a0 = pls.aoffs ? pls.aoffs[kbase + ci] : 0;
+    int ofront = pls.offs_out[kbase + ci], oback = pls.offs_out[kbase + ci + 1] - 1;
+    const int np_cell = oback + 1 - ofront;  // stayers + arrivals
     const int lx = ci % gd.bs[0], lt = ci / gd.bs[0];
     const int ly = lt % gd.bs[1], lz = lt / gd.bs[1];
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
-    for (int base = p0; base < p1; base += 32) {
-      const int a = base + lane;
-      const bool act = a < p1;
+    for (int base = 0; base < np_cell; base += 32) {
+      const int v = base + lane;
+      const bool act = v < np_cell;
       float ax = 0.25f, ay = 0.25f, az = 0.25f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
-      int sp = 0, p = a;
+      int sp = 0, p = in0 + v;
       if (act) {
-        if (perm) p = ld_stream(perm + a);  // reorder on load
+        if (v >= ns) p = ld_stream(pls.alist + (a0 + v - ns));  // reorder on load
         ay = ld_stream(in.y + p);
         az = ld_stream(in.z + p);
         ux = ld_stream(in.ux + p);
@@ -390,6 +398,12 @@ k_push2(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
       const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
       const int dc = dir_code<D3>(sxd, syd, szd);
       dirs.add(act, dc);
+      const bool leave = act && dc != DirCount<D3>::STAY;
+      const unsigned lm = __ballot_sync(0xffffffffu, leave);
+      const unsigned sm = __ballot_sync(0xffffffffu, act && !leave);
+      const int a = leave ? oback - __popc(lm & lanes_lt) : ofront + __popc(sm & lanes_lt);
+      ofront += __popc(sm);
+      oback -= __popc(lm);
       if (act) {
         const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
         const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
@@ -408,7 +422,7 @@ k_push2(GridDesc gd, Cols in, Cols out, const int *__restrict__ perm,
         st_stream(out.qw + a, qw);
         st_stream(out.sp + a, sp);
         if (in.id) st_stream(out.id + a, ld_stream(in.id + p));
-        dcode[a] = (uint8_t)dc;
+        if (leave) dcode[a] = (uint8_t)dc;
         if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
           bad |= PSC_F_NAN;
       }
@@ -447,14 +461,14 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &in = c->cols[c->cur];
   const Cols &out = c->cols[c->cur ^ 1];
-  const int *perm = c->state == PSC_STATE_INDEXED ? c->perm : nullptr;
+  const PushLists pls = psc_push_lists(c);
   ProfScope ps(c, PSC_PH_PUSH, s);
   if (d3) {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
+    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J, c->d_flags);
   } else {
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, perm, c->offs[c->ocur], c->dcode, c->dircnt, c->E, c->B, c->J, c->d_flags);
+    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J, c->d_flags);
   }
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

@@ -29,10 +29,54 @@ __device__ __forceinline__ int ld_stream(const int *p) { return __ldcs(p); }
 __device__ __forceinline__ void st_stream(float *p, float v) { __stcs(p, v); }
 __device__ __forceinline__ void st_stream(int *p, int v) { __stcs(p, v); }
 
+// asynchronous 4-byte global -> shared copy (LDGSTS); valid == false copies nothing and
+// zero-fills the destination (src-size 0)
+__device__ __forceinline__ void cp_async4(void *smem_dst, const void *gsrc, bool valid) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const int sz = valid ? 4 : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(d), "l"(gsrc), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
 __device__ __forceinline__ unsigned lanemask_lt_() {
   unsigned m;
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
+}
+
+// The particle lists a push kernel reads and writes (sort.cu "INDEX" form).
+// Input: cell k's particles are the run [offs_in[k], offs_in[k] + nstay[k]) of the input columns
+// (the stayers of the previous push) plus the arrivals alist[aoffs[k] .. aoffs[k+1]) (slots of
+// the input columns).  Output: cell k's segment [offs_out[k], offs_out[k+1]) of the other column
+// set, the particles that stay in k compacted at its front, the leavers at its back with their
+// direction code in dcode[slot]; dircnt[k][*] = how many took each direction.
+struct PushLists {
+  const int *offs_in;
+  const int *nstay;     // nullptr: the whole segment (a physically sorted list)
+  const int *aoffs;     // nullptr: no arrivals
+  const int *alist;
+  const int *offs_out;
+  uint8_t *dcode;
+  int *dircnt;
+};
+
+// SORTED: every segment is one run, written back to the same layout; INDEXED: the written list
+// (layout offs[ocur^1]) is read through nstay / aoffs / alist into the new layout offs[ocur].
+static inline PushLists psc_push_lists(const psc_ctx *c) {
+  PushLists l;
+  const bool indexed = c->state == PSC_STATE_INDEXED;
+  l.offs_in = indexed ? c->offs[c->ocur ^ 1] : c->offs[c->ocur];
+  l.nstay = indexed ? c->nstay : nullptr;
+  l.aoffs = indexed ? c->aoffs : nullptr;
+  l.alist = c->alist;
+  l.offs_out = c->offs[c->ocur];
+  l.dcode = c->dcode;
+  l.dircnt = c->dircnt;
+  return l;
 }
 
 // Per-warp bookkeeping of the direction codes of one cell's particles (9 / 27

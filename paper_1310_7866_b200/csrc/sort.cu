@@ -17,19 +17,25 @@
 //
 // INDEX (steady state: "a particle moves at most one cell per step", "the
 // sort only touches keys/indices", "reorder on load"): the list is the previous sort's output
-// advanced by one push, which left per particle a one-byte direction code (one of 9 / 27
-// destination classes) and per cell the count of each code.  Then
-//   1. k_dest_hist  new count of cell k = sum over its 9 / 27 neighbour source cells of the
-//                   count of the code that points at k;
-//   2. scan         -> new cell offsets;
-//   3. k_dir_base   stable order inside a destination cell = ascending old slot = ascending
-//                   source-cell key, then slot order inside the source cell: first slot of every
-//                   (source cell, code) group by a running sum over the sources in key order;
-//   4. k_rank       one warp per source cell walks its slots in order and hands out
-//                   consecutive slots per code (ballot + popc for the stayers, lane order for the
-//                   few leavers) -> perm.  Reads 1 byte, writes 4 bytes per particle.
-// No particle column is touched: the next push loads particle perm[s] for slot s (reorder on
-// load).  psc_particles_sort, whose contract is a physically sorted list, adds k_reorder.
+// advanced by one push.  The push wrote every cell's particles back into a segment of the cell's
+// size, the STAYERS (still in the cell: the great majority) compacted at the front and the
+// LEAVERS at the back, each leaver with the one-byte direction code of its move (one of 9 / 27
+// destination classes), and per cell the count of each code.  So the particles of a cell of the
+// NEXT step are one contiguous run (its stayers) plus a short list of arrivals, and the sort
+// works on cells and leavers only:
+//   1. k_dest_hist  per cell: stayers, arrivals (sum over the 8 / 26 neighbour source cells of
+//                   the count of the code that points here);
+//   2. scan         one pass over (total, arrivals) packed in 64 bits -> new cell offsets and
+//                   offsets into the arrival list;
+//   3. k_dir_base   first arrival-list slot of every (source cell, code) group: sources in key
+//                   order, i.e. ascending slot of the written list;
+//   4. k_rank       one warp per source cell walks its LEAVER region and writes the slots of
+//                   the leavers into the arrival list.
+// No particle column is touched and nothing per stayer is read or written: the next push loads
+// the stayer run directly and the arrivals through the list (reorder on load).  The order this
+// gives inside a cell (stayers, then arrivals) is a valid cell sort but not the stable one
+// (A17); psc_particles_sort, whose contract is the physically sorted, stable list,
+// runs the general form on the keys of the written list instead.
 #include <limits.h>
 
 #include "psc_internal.cuh"
@@ -149,40 +155,45 @@ k_to_abs(GridDesc gd, int n, const int *__restrict__ key, float *__restrict__ x,
   }
 }
 
-// ---- exclusive scan of hist[0..m) -> out[0..m], out[m] = total; also cursor := out -----------
+// ---- exclusive scan of in[0..m) -> out[0..m], out[m] = total -----------------------------------
+// T = int: one histogram (general sort; cursor := out as well).  T = long long: two histograms
+// packed as (hi << 32) | lo and scanned in one pass (index sort: hi = particles per cell, lo =
+// arrivals per cell; both totals are < 2^31, so the low half never carries into the high half);
+// the last kernel unpacks them into out (hi) and out_lo.
 
-__global__ void __launch_bounds__(SORT_THREADS)
-k_scan_local(int m, const int *__restrict__ in, int *__restrict__ out, int *__restrict__ tmp) {
-  __shared__ int wsum[SORT_THREADS / 32];
-  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
-  int v[SCAN_ITEMS];
-  int s = 0;
-#pragma unroll
-  for (int i = 0; i < SCAN_ITEMS; i++) {
-    v[i] = (base + i < m) ? in[base + i] : 0;
-    s += v[i];
-  }
-  // inclusive scan of s across the block
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int inc = s;
+template <typename T>
+__device__ __forceinline__ T warp_inclusive(T v, int lane) {
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
-    const int t = __shfl_up_sync(0xffffffffu, inc, o);
-    if (lane >= o) inc += t;
+    const T t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += t;
   }
+  return v;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_scan_local(int m, const T *__restrict__ in, T *__restrict__ out, T *__restrict__ tmp) {
+  __shared__ T wsum[SORT_THREADS / 32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  T v[SCAN_ITEMS];
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++) {
+    v[i] = (base + i < m) ? in[base + i] : (T)0;
+    s += v[i];
+  }
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const T inc = warp_inclusive(s, lane);
   if (lane == 31) wsum[w] = inc;
   __syncthreads();
   if (w == 0) {
-    int t = lane < SORT_THREADS / 32 ? wsum[lane] : 0;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int u = __shfl_up_sync(0xffffffffu, t, o);
-      if (lane >= o) t += u;
-    }
+    T t = lane < SORT_THREADS / 32 ? wsum[lane] : (T)0;
+    t = warp_inclusive(t, lane);
     if (lane < SORT_THREADS / 32) wsum[lane] = t;
   }
   __syncthreads();
-  int run = inc - s + (w ? wsum[w - 1] : 0);
+  T run = inc - s + (w ? wsum[w - 1] : (T)0);
 #pragma unroll
   for (int i = 0; i < SCAN_ITEMS; i++) {
     if (base + i < m) out[base + i] = run;
@@ -192,35 +203,23 @@ k_scan_local(int m, const int *__restrict__ in, int *__restrict__ out, int *__re
 }
 
 // single block: exclusive scan of tmp[0..nb) in place, tmp[nb] = total
-__global__ void __launch_bounds__(1024) k_scan_tmp(int nb, int *__restrict__ tmp) {
-  __shared__ int wsum[32];
-  __shared__ int carry_s;
+template <typename T>
+__global__ void __launch_bounds__(1024) k_scan_tmp(int nb, T *__restrict__ tmp) {
+  __shared__ T wsum[32];
+  __shared__ T carry_s;
   if (threadIdx.x == 0) carry_s = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (int base = 0; base < nb; base += 1024) {
     const int i = base + threadIdx.x;
-    const int v = i < nb ? tmp[i] : 0;
-    int inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
+    const T v = i < nb ? tmp[i] : (T)0;
+    const T inc = warp_inclusive(v, lane);
     if (lane == 31) wsum[w] = inc;
     __syncthreads();
-    if (w == 0) {
-      int t = wsum[lane];
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int u = __shfl_up_sync(0xffffffffu, t, o);
-        if (lane >= o) t += u;
-      }
-      wsum[lane] = t;
-    }
+    if (w == 0) wsum[lane] = warp_inclusive(wsum[lane], lane);
     __syncthreads();
-    const int carry = carry_s;
-    const int exc = carry + inc - v + (w ? wsum[w - 1] : 0);
+    const T carry = carry_s;
+    const T exc = carry + inc - v + (w ? wsum[w - 1] : (T)0);
     if (i < nb) tmp[i] = exc;
     __syncthreads();
     if (threadIdx.x == 1023) carry_s = exc + v;
@@ -242,6 +241,25 @@ k_scan_add(int m, int *__restrict__ out, int *__restrict__ cursor, const int *__
       cursor[base + i] = v;
     }
   if (blockIdx.x == 0 && threadIdx.x == 0) out[m] = tmp[nb];
+}
+
+// packed form: loc[] holds the block-local packed scan; out := high halves, out_lo := low halves
+__global__ void __launch_bounds__(SORT_THREADS)
+k_scan_add2(int m, const long long *__restrict__ loc, int *__restrict__ out,
+            int *__restrict__ out_lo, const long long *__restrict__ tmp, int nb) {
+  const long long add = tmp[blockIdx.x];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+#pragma unroll
+  for (int i = 0; i < SCAN_ITEMS; i++)
+    if (base + i < m) {
+      const long long v = loc[base + i] + add;
+      out[base + i] = (int)(v >> 32);
+      out_lo[base + i] = (int)(v & 0xffffffffLL);
+    }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    out[m] = (int)(tmp[nb] >> 32);
+    out_lo[m] = (int)(tmp[nb] & 0xffffffffLL);
+  }
 }
 
 __global__ void __launch_bounds__(SORT_THREADS)
@@ -428,39 +446,47 @@ __device__ __forceinline__ int neighbour_key(const GridDesc &gd, const int c[3],
   return cell_to_key(gd, q);
 }
 
-// hist[k] = particles that will be in cell k: source cell (k - dir) sends count[dir]
+// per destination cell k: stayers (its own STAY count), arrivals (source cell k - dir sends
+// count[dir]); pack[k] = (stayers + arrivals) << 32 | arrivals for the packed scan
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_dest_hist(GridDesc gd, const int *__restrict__ dircnt, int *__restrict__ hist) {
-  constexpr int ND = D3 ? 27 : 9;
+k_dest_hist(GridDesc gd, const int *__restrict__ dircnt, int *__restrict__ nstay,
+            long long *__restrict__ pack) {
+  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= gd.nkeys) return;
   int c[3];
   key_to_cell(gd, k, c);
-  int tot = 0;
+  int na = 0;
 #pragma unroll
-  for (int dc = 0; dc < ND; dc++) tot += dircnt[neighbour_key<D3>(gd, c, dc, -1) * ND + dc];
-  hist[k] = tot;
+  for (int dc = 0; dc < ND; dc++)
+    if (dc != STAY) na += dircnt[neighbour_key<D3>(gd, c, dc, -1) * ND + dc];
+  const int ns = dircnt[k * ND + STAY];
+  nstay[k] = ns;
+  pack[k] = ((long long)(ns + na) << 32) | (long long)na;
 }
 
-// dircnt[src][dc] (count) -> first new slot of the (src, dc) group, in place
+// dircnt[src][dc] (count, dc != STAY) -> first arrival-list slot of the (src, dc) group, in
+// place: the arrivals of a cell are ordered by source key (= by slot in the written list)
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ offs_new) {
-  constexpr int ND = D3 ? 27 : 9;
+k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ aoffs) {
+  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= gd.nkeys) return;
+  if (aoffs[k + 1] == aoffs[k]) return;  // no arrivals: every group is empty, its base unused
   int c[3];
   key_to_cell(gd, k, c);
   int sk[ND], cnt[ND];
 #pragma unroll
   for (int dc = 0; dc < ND; dc++) {
     sk[dc] = neighbour_key<D3>(gd, c, dc, -1);
-    cnt[dc] = dircnt[sk[dc] * ND + dc];
+    cnt[dc] = dc == STAY ? 0 : dircnt[sk[dc] * ND + dc];
   }
-  const int o = offs_new[k];
+  const int o = aoffs[k];
 #pragma unroll
   for (int i = 0; i < ND; i++) {
+    if (i == STAY) continue;
     int b = o;
 #pragma unroll
     for (int j = 0; j < ND; j++) b += (sk[j] < sk[i]) ? cnt[j] : 0;
@@ -468,57 +494,51 @@ k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ offs_n
   }
 }
 
-// one warp per source cell: perm[new slot] = old slot
+// one warp per source cell: walks the cell's leaver region of the written list (behind its
+// stayers) and writes each leaver's slot into its group of the arrival list
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_rank(int nkeys, const int *__restrict__ offs_old, const uint8_t *__restrict__ dcode,
-       const int *__restrict__ dirbase, int *__restrict__ perm, uint32_t *__restrict__ flags) {
+k_rank(int nkeys, const int *__restrict__ offs_w, const uint8_t *__restrict__ dcode,
+       const int *__restrict__ dirbase, int *__restrict__ alist, uint32_t *__restrict__ flags) {
   constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
   __shared__ int sb[SORT_THREADS / 32][32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int warps = gridDim.x * (SORT_THREADS / 32);
   const unsigned lt = lanemask_lt();
   for (int k = blockIdx.x * (SORT_THREADS / 32) + w; k < nkeys; k += warps) {
-    const int p0 = offs_old[k], p1 = offs_old[k + 1];
-    if (p0 >= p1) continue;
     const int b = lane < ND ? dirbase[k * ND + lane] : 0;
+    const int p0 = offs_w[k] + __shfl_sync(0xffffffffu, b, STAY), p1 = offs_w[k + 1];
+    if (p0 >= p1) continue;
     sb[w][lane] = b;
-    int bstay = __shfl_sync(0xffffffffu, b, STAY);
     __syncwarp();
     for (int base = p0; base < p1; base += 32) {
       const int s = base + lane;
-      const bool act = s < p1;
+      bool act = s < p1;
       int dc = act ? (int)dcode[s] : STAY;
-      if (dc >= ND) {  // cannot happen unless the caller scribbled over the workspace
+      if (act && (dc >= ND || dc == STAY)) {  // cannot happen unless the workspace was scribbled over
         atomicOr(flags, PSC_F_OOB);
-        dc = STAY;
+        act = false;
       }
-      const bool stay = act && dc == STAY;
-      const unsigned m = __ballot_sync(0xffffffffu, stay);
-      int slot = bstay + __popc(m & lt);
-      bstay += __popc(m);
-      unsigned lv = __ballot_sync(0xffffffffu, act && !stay);
-      while (lv) {  // the few leavers, in lane order (= slot order: stable)
-        const int l = __ffs(lv) - 1;
-        lv &= lv - 1;
-        if (lane == l) {
-          slot = sb[w][dc];
-          sb[w][dc] = slot + 1;
-        }
-        __syncwarp();
-      }
-      if (act) perm[slot] = s;
+      const unsigned peers = __match_any_sync(0xffffffffu, act ? dc : 64 + lane);
+      int slot = 0;
+      if (act) slot = sb[w][dc] + __popc(peers & lt);
+      __syncwarp();
+      if (act && (peers & lt) == 0) sb[w][dc] += __popc(peers);
+      __syncwarp();
+      if (act) alist[slot] = s;
     }
     __syncwarp();
   }
 }
 
 // key of the particle in slot s of a list laid out by `offs`: the slot's cell, moved by the
-// particle's direction code if there is one
+// particle's direction code if the slot lies in the cell's leaver region (behind the
+// dirtab[cell][STAY] stayers; dirtab == nullptr: a sorted list, nobody has moved)
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const uint8_t *__restrict__ dcode,
-            int *__restrict__ key) {
+k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const int *__restrict__ dirtab,
+            const uint8_t *__restrict__ dcode, int *__restrict__ key) {
+  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
   const int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   int lo = 0, hi = gd.nkeys;  // largest k with offs[k] <= s (and offs[k+1] > s)
@@ -527,10 +547,12 @@ k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const uint8_t *__r
     if (offs[mid] <= s) lo = mid; else hi = mid;
   }
   int k = lo;
-  if (dcode) {
+  if (dirtab && s >= offs[k] + dirtab[k * ND + STAY]) {
     int c[3];
     key_to_cell(gd, k, c);
-    k = neighbour_key<D3>(gd, c, (int)dcode[s], +1);
+    int dc = (int)dcode[s];
+    if (dc >= ND) dc = STAY;
+    k = neighbour_key<D3>(gd, c, dc, +1);
   }
   key[s] = k;
 }
@@ -542,11 +564,12 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
   size_t b = 0;
-  b += 4 * align_up((size_t)n * 4, 256);                      // key, perm, cell_idx, curkey
+  b += 5 * align_up((size_t)n * 4, 256);                      // key, curkey, perm, cell_idx, alist
   b += align_up((size_t)n, 256);                              // dcode
-  b += 3 * align_up((nk + 1) * 4, 256);                       // offs[2], cursor
+  b += 5 * align_up((nk + 1) * 4, 256);                       // offs[2], cursor, aoffs, nstay
+  b += 2 * align_up((nk + 1) * 8, 256);                       // pack, packloc
   b += align_up(nk * 27 * 4, 256);                            // dircnt
-  b += align_up((nk / SCAN_TILE + 3) * 4, 256);               // scan_tmp
+  b += align_up((nk / SCAN_TILE + 3) * 8, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
   return b;
 }
@@ -563,12 +586,17 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
   c->curkey = (int32_t *)take((size_t)n * 4);
   c->perm = (int32_t *)take((size_t)n * 4);
   c->cell_idx = (int32_t *)take((size_t)n * 4);
+  c->alist = (int32_t *)take((size_t)n * 4);
   c->dcode = (uint8_t *)take((size_t)n);
   c->offs[0] = (int32_t *)take((nk + 1) * 4);
   c->offs[1] = (int32_t *)take((nk + 1) * 4);
   c->cursor = (int32_t *)take((nk + 1) * 4);
+  c->aoffs = (int32_t *)take((nk + 1) * 4);
+  c->nstay = (int32_t *)take((nk + 1) * 4);
+  c->pack = (long long *)take((nk + 1) * 8);
+  c->packloc = (long long *)take((nk + 1) * 8);
   c->dircnt = (int32_t *)take(nk * 27 * 4);
-  c->scan_tmp = (int32_t *)take((nk / SCAN_TILE + 3) * 4);
+  c->scan_tmp = (long long *)take((nk / SCAN_TILE + 3) * 8);
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
   if ((size_t)(p - (char *)c->ws) > c->ws_bytes) return PSC_ERR_WORKSPACE;
   return PSC_OK;
@@ -583,21 +611,44 @@ int run_scan(psc_ctx *c, int32_t *out, cudaStream_t s) {
   const int nk = c->gd.nkeys;
   ProfScope ps(c, PSC_PH_SORT_SCAN, s);
   const int sblocks = (int)cdiv64(nk, SCAN_TILE);
-  k_scan_local<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, out, c->scan_tmp);
+  int *tmp = (int *)c->scan_tmp;
+  k_scan_local<int><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, out, tmp);
   PSC_LAUNCH_CHECK(c);
-  k_scan_tmp<<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
+  k_scan_tmp<int><<<1, 1024, 0, s>>>(sblocks, tmp);
   PSC_LAUNCH_CHECK(c);
-  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, out, c->cursor, c->scan_tmp, sblocks);
+  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, out, c->cursor, tmp, sblocks);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
 
-int slot_keys(psc_ctx *c, const int32_t *offs, const uint8_t *dcode, int32_t *key, cudaStream_t s) {
+// packed scan of c->pack -> out_hi (cell offsets), out_lo (arrival-list offsets)
+int run_scan2(psc_ctx *c, int32_t *out_hi, int32_t *out_lo, cudaStream_t s) {
+  const int nk = c->gd.nkeys;
+  ProfScope ps(c, PSC_PH_SORT_SCAN, s);
+  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
+  k_scan_local<long long><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->pack, c->packloc, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_tmp<long long><<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_add2<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->packloc, out_hi, out_lo, c->scan_tmp, sblocks);
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}
+
+// key[s] of the particles of the current column set, in their current order
+int slot_keys(psc_ctx *c, int32_t *key, cudaStream_t s) {
   const int n = (int)c->np;
   if (n == 0) return PSC_OK;
+  const int32_t *offs, *dirtab = nullptr;
+  switch (c->state) {
+    case PSC_STATE_SORTED: offs = c->offs[c->ocur]; break;
+    case PSC_STATE_PUSHED: offs = c->offs[c->ocur]; dirtab = c->dircnt; break;
+    case PSC_STATE_INDEXED: offs = c->offs[c->ocur ^ 1]; dirtab = c->dircnt; break;
+    default: return PSC_ERR_NOT_SORTED;
+  }
   const int blocks = (int)cdiv64(n, SORT_THREADS);
-  if (is3d(c->gd)) k_slot_keys<true><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dcode, key);
-  else k_slot_keys<false><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dcode, key);
+  if (is3d(c->gd)) k_slot_keys<true><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dirtab, c->dcode, key);
+  else k_slot_keys<false><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dirtab, c->dcode, key);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
@@ -605,16 +656,9 @@ int slot_keys(psc_ctx *c, const int32_t *offs, const uint8_t *dcode, int32_t *ke
 }  // namespace
 
 // key[] (c->curkey) := keys of the current particles, in their current order
-int psc_sort_current_keys(psc_ctx *c, cudaStream_t s) {
-  switch (c->state) {
-    case PSC_STATE_SORTED: return slot_keys(c, c->offs[c->ocur], nullptr, c->curkey, s);
-    case PSC_STATE_PUSHED: return slot_keys(c, c->offs[c->ocur], c->dcode, c->curkey, s);
-    case PSC_STATE_INDEXED: return slot_keys(c, c->offs[c->ocur ^ 1], c->dcode, c->curkey, s);
-    default: return PSC_ERR_NOT_SORTED;
-  }
-}
+int psc_sort_current_keys(psc_ctx *c, cudaStream_t s) { return slot_keys(c, c->curkey, s); }
 
-// general counting sort: arbitrary order in, physically sorted list out
+// general counting sort: arbitrary order in, physically sorted (stable) list out
 int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const GridDesc &gd = c->gd;
   const int n = (int)c->np;
@@ -622,12 +666,13 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const Cols &in = c->cols[c->cur];
   const Cols &out = c->cols[c->cur ^ 1];
   const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
-  int32_t *offs_new = c->offs[c->ocur ^ 1];
 
-  if (c->form == PSC_FORM_REL) {  // a sorted list sorted again: keys from the slots
-    const int rc = slot_keys(c, c->offs[c->ocur], nullptr, c->key, s);
+  if (c->form == PSC_FORM_REL) {  // a sorted or pushed list sorted again: keys from the slots
+    const int rc = slot_keys(c, c->key, s);
     if (rc) return rc;
+    if (c->state == PSC_STATE_INDEXED) c->ocur ^= 1;  // back to the layout of the written list
   }
+  int32_t *offs_new = c->offs[c->ocur ^ 1];
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
   c->launches += 2;
@@ -673,58 +718,43 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   return PSC_OK;
 }
 
-// index sort of a pushed list: new offsets + perm from the direction codes; no column moves
+// index sort of a pushed list: new cell offsets + the arrival list from the per-cell direction
+// counts and the leavers' direction codes; no column moves
 int psc_sort_index(psc_ctx *c, cudaStream_t s) {
   const GridDesc &gd = c->gd;
   const int nk = gd.nkeys;
-  const int32_t *offs_old = c->offs[c->ocur];
+  const int32_t *offs_w = c->offs[c->ocur];  // layout of the written list
   int32_t *offs_new = c->offs[c->ocur ^ 1];
   const int cblocks = (int)cdiv64(nk, SORT_THREADS);
   const bool d3 = is3d(gd);
   psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
-  if (d3) k_dest_hist<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->cursor);
-  else k_dest_hist<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->cursor);
+  if (d3) k_dest_hist<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->nstay, c->pack);
+  else k_dest_hist<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->nstay, c->pack);
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_COUNT, s);
   {
-    const int rc = run_scan(c, offs_new, s);
+    const int rc = run_scan2(c, offs_new, c->aoffs, s);
     if (rc) return rc;
   }
   psc_prof_begin(c, PSC_PH_SORT_RANK, s);
-  if (d3) k_dir_base<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, offs_new);
-  else k_dir_base<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, offs_new);
+  if (d3) k_dir_base<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
+  else k_dir_base<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
   PSC_LAUNCH_CHECK(c);
   const int rblocks = (int)min((int64_t)c->sm_count * 32, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
-  if (d3) k_rank<true><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_old, c->dcode, c->dircnt, c->perm, c->d_flags);
-  else k_rank<false><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_old, c->dcode, c->dircnt, c->perm, c->d_flags);
+  if (d3) k_rank<true><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
+  else k_rank<false><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_RANK, s);
   c->ocur ^= 1;
   c->state = PSC_STATE_INDEXED;
-  c->have_sort_result = 2;
+  c->have_sort_result = 0;
   return PSC_OK;
 }
 
-// INDEXED -> SORTED: the physical reorder the next push would otherwise do on load
-int psc_sort_materialize(psc_ctx *c, cudaStream_t s) {
-  const int n = (int)c->np;
-  const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
-  ProfScope ps(c, PSC_PH_SORT_REORDER, s);
-  k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(c->gd, n, c->perm, c->cols[c->cur], c->cols[c->cur ^ 1]);
-  PSC_LAUNCH_CHECK(c);
-  c->cur ^= 1;
-  c->state = PSC_STATE_SORTED;
-  return PSC_OK;
-}
-
-// cell_idx[a] of the last sort's INPUT particles
+// cell_idx[a] of the last (general) sort's INPUT particles
 int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s) {
   const int n = (int)c->np;
   if (n == 0) return PSC_OK;
-  if (c->have_sort_result == 2) {  // index sort: input key = old slot's cell moved by the code
-    const int rc = slot_keys(c, c->offs[c->ocur ^ 1], c->dcode, c->key, s);
-    if (rc) return rc;
-  }
   k_cell_idx<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key, c->cell_idx);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

@@ -7,7 +7,7 @@ import pytest
 import torch
 
 import psc_inputs
-from tests.util import (gpu_cols, gpu_positions_f64, key_to_cell, library_block, oracle_for, oracle_sorted_state, oracle_state,
+from tests.util import (gpu_cols, gpu_positions_f64, key_to_cell, library_block, oracle_for, oracle_sorted_state, oracle_state, order_by_id,
                         periodic_dist, rel_fieldnorm, rel_maxnorm, smooth_fields)
 
 pytestmark = pytest.mark.gpu
@@ -290,6 +290,8 @@ def _push_once(kind, block, amp=0.05):
 def test_push_particles_matches_oracle(kind, block):
     pl, sim, orc, cols0, st, sp, J = _push_once(kind, block)
     got = gpu_cols(sim)
+    o = order_by_id(got["id"], cols0["id"])       # the push regroups inside each cell's segment
+    got = {k: v[o] for k, v in got.items()}
     L = [pl.n[d] * pl.dx[d] for d in range(3)]
     for d, c in enumerate(("x", "y", "z")):
         if pl.n[d] == 1:
@@ -315,6 +317,8 @@ def test_gpu_continuity_residual(kind):
     pl, sim, orc, cols0, st, sp, J = _push_once(kind, (0, 0, 0), amp=0.05)
     f64 = lambda a: np.ascontiguousarray(a.astype(np.float64))
     x1, y1, z1 = gpu_positions_f64(sim)            # internal form: no export rounding
+    o = order_by_id(sim.current()["id"].cpu().numpy(), cols0["id"])
+    x1, y1, z1 = (np.ascontiguousarray(v[o]) for v in (x1, y1, z1))
     rho0 = orc.rho(f64(cols0["x"]), f64(cols0["y"]), f64(cols0["z"]), f64(cols0["qw"]))
     rho1 = orc.rho(x1, y1, z1, f64(cols0["qw"]))
     Jg = np.ascontiguousarray(sim.interior(sim.J).cpu().numpy().astype(np.float64))

@@ -58,6 +58,16 @@ def gpu_positions_f64(sim, block=(0, 0, 0)):
     return out
 
 
+def order_by_id(got_id, ref_id):
+    """index array o with got_id[o] == ref_id: the push writes every cell's segment with the
+    stayers in front and the leavers behind, so lists are compared particle by particle via id"""
+    pos = np.empty(len(got_id), dtype=np.int64)
+    pos[got_id] = np.arange(len(got_id))
+    o = pos[ref_id]
+    assert np.array_equal(got_id[o], ref_id)
+    return o
+
+
 def periodic_dist(a, b, L):
     d = np.abs(a.astype(np.float64) - b.astype(np.float64))
     return np.minimum(d, L - d)
