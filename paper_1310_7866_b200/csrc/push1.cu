@@ -319,7 +319,8 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
   }
 }
 
-template <bool D3, int CBS, int THREADS, int MINB>
+// XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id)
+template <bool D3, int CBS, int THREADS, int MINB, bool XC>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
         const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
@@ -431,7 +432,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   // cross-lane synchronisation is involved): NST - 1 chunks of loads are in flight per warp
   // without holding registers, which is what hides the DRAM latency at 20 warps per SM.
   // Lanes past the end of the cell copy zero bytes, i.e. get zero-filled slots.
-  const bool has_x = D3 || in.x != nullptr, has_id = in.id != nullptr;
+  const bool has_x = D3 || (XC && in.x != nullptr), has_id = XC && in.id != nullptr;
   auto issue = [&](const It &it, int p, int stage) {
     const bool v = it.base + lane < it.p1;
     const int q = v ? p : 0;
@@ -533,7 +534,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
 
       // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
       boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
-      const float ig = rsqrtf(fmaf(ux, ux, fmaf(uy, uy, fmaf(uz, uz, 1.0f))));
+      const float ig = rsqrt_ge1(fmaf(ux, ux, fmaf(uy, uy, fmaf(uz, uz, 1.0f))));
       const float vx = ux * ig;
       const float ddx = D3 ? vx * cdx : 0.f;  // displacement in cells
       const float ddy = (uy * ig) * cdy, ddz = (uz * ig) * cdz;
@@ -591,7 +592,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
           const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
           st_stream(out.x + s, bx_);
           if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
-        } else if (in.x) {
+        } else if (has_x) {
           st_stream(out.x + s, cur.cx);  // invariant coordinate: carried
         }
         st_stream(out.y + s, by_);
@@ -601,7 +602,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
         st_stream(out.uz + s, uz);
         st_stream(out.qw + s, qw);
         st_stream(out.sp + s, sp);
-        if (in.id) st_stream(out.id + s, cur.id);
+        if (has_id) st_stream(out.id + s, cur.id);
         if (cross) dcode[s] = (uint8_t)dc;
         if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
       }
@@ -674,20 +675,26 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_>,                               \
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    k_push1<D3_, CBS_, T_, B_><<<gd.ntiles, threads, smem, s>>>(                                   \
-        gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                           \
+    if (xc) {                                                                                      \
+      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, true>,                       \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+      k_push1<D3_, CBS_, T_, B_, true><<<gd.ntiles, threads, smem, s>>>(                           \
+          gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                         \
+    } else {                                                                                       \
+      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, false>,                      \
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+      k_push1<D3_, CBS_, T_, B_, false><<<gd.ntiles, threads, smem, s>>>(                          \
+          gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                         \
+    }                                                                                              \
   } while (0)
-  const int v = c->opt_push_variant;
+  const bool xc = in.id != nullptr || (!d3 && in.x != nullptr);
   if (d3) {
-    const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4 && v != 2;
+    const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4 && c->opt_push_variant != 2;
     if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4);
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
   } else {
-    const bool def = gd.bs[1] == 8 && gd.bs[2] == 8 && v != 2;
-    if (def && v == 1) PSC_LAUNCH_PUSH1(false, 8, 128, 6);
-    else if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
+    const bool def = gd.bs[1] == 8 && gd.bs[2] == 8 && c->opt_push_variant != 2;
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
   }
 #undef PSC_LAUNCH_PUSH1

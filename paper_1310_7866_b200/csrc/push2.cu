@@ -283,7 +283,7 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
 
       // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
       boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
-      const float ig = rsqrtf(1.0f + ux * ux + uy * uy + uz * uz);
+      const float ig = rsqrt_ge1(1.0f + ux * ux + uy * uy + uz * uz);
       const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
       const float endx = D3 ? ax + vx * gd.dt_dx[0] : ax;
       const float endy = ay + vy * gd.dt_dx[1], endz = az + vz * gd.dt_dx[2];

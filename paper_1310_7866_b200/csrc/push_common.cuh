@@ -2,15 +2,28 @@
 #pragma once
 #include "psc_internal.cuh"
 
+// 1/sqrt(x) and 1/x for x >= 1 (1 + |u|^2, 1 + |t|^2): the bare MUFU approximations (2 ulp /
+// 1 ulp), without the denormal-range scaling rsqrtf() and division wrap around them
+__device__ __forceinline__ float rsqrt_ge1(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ float rcp_ge1(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
 // Boris rotation, PAPER.md:171-179 (Eq. 27-28): half electric kick, magnetic rotation with
 // gamma taken after the first half kick ("We follow Boris"; A6), half electric kick.
 // h = q dt / (2 m).  u is u = p/(m c).
 __device__ __forceinline__ void boris_push(float &ux, float &uy, float &uz, float ex, float ey,
                                            float ez, float bx, float by, float bz, float h) {
   const float umx = fmaf(h, ex, ux), umy = fmaf(h, ey, uy), umz = fmaf(h, ez, uz);
-  const float ig = h * rsqrtf(fmaf(umx, umx, fmaf(umy, umy, fmaf(umz, umz, 1.0f))));
+  const float ig = h * rsqrt_ge1(fmaf(umx, umx, fmaf(umy, umy, fmaf(umz, umz, 1.0f))));
   const float tx = bx * ig, ty = by * ig, tz = bz * ig;
-  const float sf = __fdividef(2.0f, fmaf(tx, tx, fmaf(ty, ty, fmaf(tz, tz, 1.0f))));
+  const float sf = 2.0f * rcp_ge1(fmaf(tx, tx, fmaf(ty, ty, fmaf(tz, tz, 1.0f))));
   const float sx = tx * sf, sy = ty * sf, sz = tz * sf;
   const float upx = fmaf(umy, tz, fmaf(-umz, ty, umx));
   const float upy = fmaf(umz, tx, fmaf(-umx, tz, umy));
