@@ -39,13 +39,13 @@ struct Cols {
 //   UNSORTED  absolute positions in arbitrary order (after bind or export)
 //   SORTED    the current column set is physically in sorted order; offs[ocur] = cell offsets
 //   PUSHED    the current set is the list a push wrote: cell k's particles of BEFORE the push in
-//             [offs[ocur][k], offs[ocur][k+1]), its stayers first (dircnt[k][STAY] of them), then
+//             [offs[ocur][k], offs[ocur][k+1]), its stayers first (dircnt[STAY][k] of them), then
 //             its leavers, each leaver with the direction code of its move in dcode[slot];
 //             dircnt holds the per-cell code counts
 //   INDEXED   the current set is still that written list (layout offs[ocur^1]); offs[ocur] are
 //             the cell offsets of the new order, nstay / aoffs / alist say where each cell's
 //             particles are (a run of stayers + listed arrivals; reorder happens on the next
-//             load); dircnt[k][dc != STAY] now hold arrival-list bases
+//             load); dircnt[dc != STAY][k] now hold arrival-list bases
 enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1, PSC_STATE_PUSHED = 2, PSC_STATE_INDEXED = 3 };
 enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
 

@@ -369,7 +369,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   __syncthreads();
   for (int i = threadIdx.x; i < tg.cpb; i += blockDim.x)  // empty cells send nothing anywhere
     if (sOut[i + 1] == sOut[i])
-      for (int d = 0; d < (D3 ? 27 : 9); d++) dircnt[(kbase + i) * (D3 ? 27 : 9) + d] = 0;
+      for (int d = 0; d < (D3 ? 27 : 9); d++) dircnt[d * gd.nkeys + kbase + i] = 0;
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   uint32_t bad = 0;
@@ -624,7 +624,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
         constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
         int *row = sDir + warp * 32;
         if (lane < ND) {
-          dircnt[(kbase + c.ci) * ND + lane] = lane == STAY ? nst : row[lane];
+          dircnt[lane * gd.nkeys + kbase + c.ci] = lane == STAY ? nst : row[lane];
           row[lane] = 0;
         }
         ncross = 0;

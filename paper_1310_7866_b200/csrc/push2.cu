@@ -427,7 +427,7 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
           bad |= PSC_F_NAN;
       }
     }
-    dirs.cell_done(dircnt, kbase + ci, lane);
+    dirs.cell_done(dircnt, kbase + ci, gd.nkeys, lane);
   }
   if (bad) atomicOr(flags, bad);
   __syncthreads();

@@ -66,7 +66,8 @@ __device__ __forceinline__ unsigned lanemask_lt_() {
 // (the stayers of the previous push) plus the arrivals alist[aoffs[k] .. aoffs[k+1]) (slots of
 // the input columns).  Output: cell k's segment [offs_out[k], offs_out[k+1]) of the other column
 // set, the particles that stay in k compacted at its front, the leavers at its back with their
-// direction code in dcode[slot]; dircnt[k][*] = how many took each direction.
+// direction code in dcode[slot]; dircnt[dc][k] = how many of cell k took direction dc
+// (direction-major, so that the per-cell kernels of the index sort read it coalesced).
 struct PushLists {
   const int *offs_in;
   const int *nstay;     // nullptr: the whole segment (a physically sorted list)
@@ -112,10 +113,10 @@ struct DirCount {
     nstay += __popc(__ballot_sync(0xffffffffu, act && stay));
     if (act && !stay) atomicAdd(&row[dc], 1);
   }
-  __device__ __forceinline__ void cell_done(int *__restrict__ dircnt, int key, int lane) {
+  __device__ __forceinline__ void cell_done(int *__restrict__ dircnt, int key, int nkeys, int lane) {
     __syncwarp();
     if (lane < ND) {
-      dircnt[key * ND + lane] = row[lane] + (lane == STAY ? nstay : 0);
+      dircnt[lane * nkeys + key] = row[lane] + (lane == STAY ? nstay : 0);
       row[lane] = 0;
     }
     nstay = 0;

@@ -27,8 +27,8 @@
 //                   the count of the code that points here);
 //   2. scan         one pass over (total, arrivals) packed in 64 bits -> new cell offsets and
 //                   offsets into the arrival list;
-//   3. k_dir_base   first arrival-list slot of every (source cell, code) group: sources in key
-//                   order, i.e. ascending slot of the written list;
+//   3. k_dir_base   first arrival-list slot of every (source cell, code) group: a cell's
+//                   arrivals are grouped by the direction they came from;
 //   4. k_rank       one warp per source cell walks its LEAVER region and writes the slots of
 //                   the leavers into the arrival list.
 // No particle column is touched and nothing per stayer is read or written: the next push loads
@@ -427,24 +427,35 @@ __device__ __forceinline__ int cell_to_key(const GridDesc &gd, const int c[3]) {
 
 __device__ __forceinline__ int wrap(int c, int n) { return c < 0 ? c + n : (c >= n ? c - n : c); }
 
-// key of the neighbour of cell c[] in direction code dc (periodic)
-template <bool D3>
-__device__ __forceinline__ int neighbour_key(const GridDesc &gd, const int c[3], int dc, int sign) {
-  int s[3];
-  if (D3) {
-    s[0] = dc % 3 - 1;
-    s[1] = (dc / 3) % 3 - 1;
-    s[2] = dc / 9 - 1;
-  } else {
-    s[0] = 0;
-    s[1] = dc % 3 - 1;
-    s[2] = dc / 3 - 1;
-  }
-  int q[3];
+// Keys of the 9 / 27 neighbours of a cell without a division per neighbour: the key is a sum of
+// one term per direction, key = sum_d (b_d * bstride_d * cpb + l_d * lstride_d), so three
+// candidate terms per direction (cell - 1, cell, cell + 1, periodic) give every neighbour by
+// three additions.
+struct NbKeys {
+  int t[3][3];
+  __device__ __forceinline__ void init(const GridDesc &gd, const int c[3]) {
+    int bstride = gd.cpb, lstride = 1;
 #pragma unroll
-  for (int d = 0; d < 3; d++) q[d] = wrap(c[d] + sign * s[d], gd.n[d]);
-  return cell_to_key(gd, q);
-}
+    for (int d = 0; d < 3; d++) {
+#pragma unroll
+      for (int s = -1; s <= 1; s++) {
+        const int q = wrap(c[d] + s, gd.n[d]);
+        const int b = q / gd.bs[d];
+        t[d][s + 1] = b * bstride + (q - b * gd.bs[d]) * lstride;
+      }
+      bstride *= gd.nb[d];
+      lstride *= gd.bs[d];
+    }
+  }
+  // neighbour in direction code dc (sign = +1) or the cell that reaches this one by dc (-1)
+  template <bool D3>
+  __device__ __forceinline__ int key(int dc, int sign) const {
+    const int s0 = D3 ? dc % 3 - 1 : 0;
+    const int s1 = D3 ? (dc / 3) % 3 - 1 : dc % 3 - 1;
+    const int s2 = D3 ? dc / 9 - 1 : dc / 3 - 1;
+    return t[0][sign * s0 + 1] + t[1][sign * s1 + 1] + t[2][sign * s2 + 1];
+  }
+};
 
 // per destination cell k: stayers (its own STAY count), arrivals (source cell k - dir sends
 // count[dir]); pack[k] = (stayers + arrivals) << 32 | arrivals for the packed scan
@@ -457,75 +468,101 @@ k_dest_hist(GridDesc gd, const int *__restrict__ dircnt, int *__restrict__ nstay
   if (k >= gd.nkeys) return;
   int c[3];
   key_to_cell(gd, k, c);
+  NbKeys nb;
+  nb.init(gd, c);
   int na = 0;
 #pragma unroll
   for (int dc = 0; dc < ND; dc++)
-    if (dc != STAY) na += dircnt[neighbour_key<D3>(gd, c, dc, -1) * ND + dc];
-  const int ns = dircnt[k * ND + STAY];
+    if (dc != STAY) na += dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)];
+  const int ns = dircnt[STAY * gd.nkeys + k];
   nstay[k] = ns;
   pack[k] = ((long long)(ns + na) << 32) | (long long)na;
 }
 
-// dircnt[src][dc] (count, dc != STAY) -> first arrival-list slot of the (src, dc) group, in
-// place: the arrivals of a cell are ordered by source key (= by slot in the written list)
+// dircnt[dc][src] (count, dc != STAY) -> first arrival-list slot of the (src, dc) group, in
+// place: the arrivals of a cell are ordered by the direction they came from
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
 k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ aoffs) {
   constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= gd.nkeys) return;
-  if (aoffs[k + 1] == aoffs[k]) return;  // no arrivals: every group is empty, its base unused
+  int o = aoffs[k];
+  if (aoffs[k + 1] == o) return;  // no arrivals: every group is empty, its base unused
   int c[3];
   key_to_cell(gd, k, c);
-  int sk[ND], cnt[ND];
+  NbKeys nb;
+  nb.init(gd, c);
+  int cnt[ND];  // all loads first: the stores below may alias them as far as the compiler knows
+#pragma unroll
+  for (int dc = 0; dc < ND; dc++) cnt[dc] = dc == STAY ? 0 : dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)];
 #pragma unroll
   for (int dc = 0; dc < ND; dc++) {
-    sk[dc] = neighbour_key<D3>(gd, c, dc, -1);
-    cnt[dc] = dc == STAY ? 0 : dircnt[sk[dc] * ND + dc];
-  }
-  const int o = aoffs[k];
-#pragma unroll
-  for (int i = 0; i < ND; i++) {
-    if (i == STAY) continue;
-    int b = o;
-#pragma unroll
-    for (int j = 0; j < ND; j++) b += (sk[j] < sk[i]) ? cnt[j] : 0;
-    dircnt[sk[i] * ND + i] = b;
+    if (dc == STAY) continue;
+    dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)] = o;
+    o += cnt[dc];
   }
 }
 
-// one warp per source cell: walks the cell's leaver region of the written list (behind its
-// stayers) and writes each leaver's slot into its group of the arrival list
+// A warp per source cell walks the cell's leaver region of the written list (behind its
+// stayers) and writes each leaver's slot into its group of the arrival list.  A region is a
+// handful of entries and every step is a dependent global load, so a warp works on RANK_U cells
+// at once: their table rows, then their first code chunks, are loaded back to back.
+constexpr int RANK_U = 4;
+
 template <bool D3>
 __global__ void __launch_bounds__(SORT_THREADS)
 k_rank(int nkeys, const int *__restrict__ offs_w, const uint8_t *__restrict__ dcode,
        const int *__restrict__ dirbase, int *__restrict__ alist, uint32_t *__restrict__ flags) {
   constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  __shared__ int sb[SORT_THREADS / 32][32];
+  __shared__ int sb[SORT_THREADS / 32][RANK_U][32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int warps = gridDim.x * (SORT_THREADS / 32);
   const unsigned lt = lanemask_lt();
-  for (int k = blockIdx.x * (SORT_THREADS / 32) + w; k < nkeys; k += warps) {
-    const int b = lane < ND ? dirbase[k * ND + lane] : 0;
-    const int p0 = offs_w[k] + __shfl_sync(0xffffffffu, b, STAY), p1 = offs_w[k + 1];
-    if (p0 >= p1) continue;
-    sb[w][lane] = b;
+  for (int k0 = (blockIdx.x * (SORT_THREADS / 32) + w) * RANK_U; k0 < nkeys; k0 += warps * RANK_U) {
+    int p0[RANK_U], p1[RANK_U], dc0[RANK_U];
+#pragma unroll
+    for (int j = 0; j < RANK_U; j++) {
+      const int k = k0 + j;
+      const bool ok = k < nkeys;
+      const int b = (ok && lane < ND) ? dirbase[lane * nkeys + k] : 0;
+      sb[w][j][lane] = b;
+      p0[j] = (ok ? offs_w[k] : 0) + __shfl_sync(0xffffffffu, b, STAY);
+      p1[j] = ok ? offs_w[k + 1] : 0;
+    }
+#pragma unroll
+    for (int j = 0; j < RANK_U; j++) dc0[j] = p0[j] + lane < p1[j] ? (int)dcode[p0[j] + lane] : STAY;
     __syncwarp();
-    for (int base = p0; base < p1; base += 32) {
-      const int s = base + lane;
-      bool act = s < p1;
-      int dc = act ? (int)dcode[s] : STAY;
-      if (act && (dc >= ND || dc == STAY)) {  // cannot happen unless the workspace was scribbled over
-        atomicOr(flags, PSC_F_OOB);
-        act = false;
+#pragma unroll
+    for (int j = 0; j < RANK_U; j++) {
+      for (int base = p0[j]; base < p1[j]; base += 32) {
+        const int s = base + lane;
+        bool act = s < p1[j];
+        int dc = base == p0[j] ? dc0[j] : (act ? (int)dcode[s] : STAY);
+        if (act && (dc >= ND || dc == STAY)) {  // cannot happen unless the workspace was scribbled over
+          atomicOr(flags, PSC_F_OOB);
+          act = false;
+        }
+        // rank inside the (cell, code) group: one ballot per distinct code present (a few);
+        // match.any would do it in one instruction but is an order of magnitude slower here
+        int rank = 0, cnt = 0;
+        unsigned rem = __ballot_sync(0xffffffffu, act);
+        while (rem) {
+          const int d = __shfl_sync(0xffffffffu, dc, __ffs(rem) - 1);
+          const unsigned m = __ballot_sync(0xffffffffu, act && dc == d);
+          if (act && dc == d) {
+            rank = __popc(m & lt);
+            cnt = __popc(m);
+          }
+          rem &= ~m;
+        }
+        int slot = 0;
+        if (act) slot = sb[w][j][dc] + rank;
+        __syncwarp();
+        if (act && rank == 0) sb[w][j][dc] += cnt;
+        __syncwarp();
+        if (act) alist[slot] = s;
       }
-      const unsigned peers = __match_any_sync(0xffffffffu, act ? dc : 64 + lane);
-      int slot = 0;
-      if (act) slot = sb[w][dc] + __popc(peers & lt);
-      __syncwarp();
-      if (act && (peers & lt) == 0) sb[w][dc] += __popc(peers);
-      __syncwarp();
-      if (act) alist[slot] = s;
     }
     __syncwarp();
   }
@@ -547,12 +584,14 @@ k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const int *__restr
     if (offs[mid] <= s) lo = mid; else hi = mid;
   }
   int k = lo;
-  if (dirtab && s >= offs[k] + dirtab[k * ND + STAY]) {
+  if (dirtab && s >= offs[k] + dirtab[STAY * gd.nkeys + k]) {
     int c[3];
     key_to_cell(gd, k, c);
     int dc = (int)dcode[s];
     if (dc >= ND) dc = STAY;
-    k = neighbour_key<D3>(gd, c, dc, +1);
+    NbKeys nb;
+    nb.init(gd, c);
+    k = nb.key<D3>(dc, +1);
   }
   key[s] = k;
 }
@@ -740,7 +779,7 @@ int psc_sort_index(psc_ctx *c, cudaStream_t s) {
   if (d3) k_dir_base<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
   else k_dir_base<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
   PSC_LAUNCH_CHECK(c);
-  const int rblocks = (int)min((int64_t)c->sm_count * 32, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
+  const int rblocks = (int)min((int64_t)c->sm_count * 32, max((int64_t)1, cdiv64(nk, (SORT_THREADS / 32) * 4)));
   if (d3) k_rank<true><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
   else k_rank<false><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
   PSC_LAUNCH_CHECK(c);
