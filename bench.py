@@ -109,6 +109,23 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(ms, world, device="cpu"):
+    """the slowest rank's time: every multi-GPU number is the max over ranks (device timing)"""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(particles_per_rank, world, steps, ms_max):
+    """whole-job particle updates per second: replicas of equal size, the slowest rank's time"""
+    return particles_per_rank * world * steps / (ms_max * 1e-3)
+
+
 def oracle_rate(cfg, sample_grid, nsteps):
     """the fp64 oracle on a bounded sample of the workload -> (updates/s, threads, particles)"""
     import numpy as np
@@ -245,11 +262,8 @@ def run_psc(args):
     launches = psc.launch_count() - l0
     prof = psc.profile()
     flags = psc.status()
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = npart * world * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, dev)
+    value = job_throughput(npart, world, args.steps, ms_max)
 
     # ---- roofline of the fused gather-push-deposit kernel ------------------------------------
     peak, peak_src = peaks()
@@ -298,10 +312,8 @@ def run_psc(args):
             psc.step_host(npart, host, hE, hB, hJ, 1)
         e1.record()
         barrier()
-        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": npart * world * ksteps / (float(te.item()) * 1e-3), "unit": UNIT,
+        te = max_over_ranks(e0.elapsed_time(e1), world, dev)
+        e2e = {"value": job_throughput(npart, world, ksteps, te), "unit": UNIT,
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
                "api": "psc_step_host (pinned host columns + fields in, particles + E,B,J out)"}
         flags |= psc.status()

@@ -122,13 +122,11 @@ int psc_bind_particles(psc_ctx *ctx, int64_t n, const psc_particle_cols *primary
 /* Cell-key counting sort.  key = block-major, cell-minor; stable (ascending
  * input index inside a key).  Afterwards the CURRENT column set (psc_particles_current) holds
  * the particles in sorted order and in internal form; the two sets swap roles.  Arbitrary input
- * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))).  A list
- * that is the previous sort's output advanced by psc_push_particles is sorted from what the push
- * left behind -- per particle the one-byte direction code of its move (a particle moves at most
- * one cell per direction and step: 9 / 27 destination classes) and per cell the
- * count of each code -- so the sort itself reads no particle column; the physical
- * reorder that this call's contract demands is one more pass (psc_step leaves it to the next
- * push's load instead). */
+ * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))); from a
+ * list in internal form (sorted, or advanced by psc_push_particles) they come from the slot's
+ * cell and, for the particles that left it, the one-byte direction code the push recorded.
+ * psc_sort_result describes this call's permutation.  psc_step does NOT run this full sort in
+ * the steady state: see psc_step. */
 int psc_particles_sort(psc_ctx *ctx, void *stream);
 
 /* The particle loop of Fig. 8 in one pass over the particles
@@ -137,7 +135,10 @@ int psc_particles_sort(psc_ctx *ctx, void *stream);
  * j^{n+1}, periodic wrap (on the integer cell index).  Requires a sorted list
  * in internal form, i.e. psc_particles_sort directly before (PSC_ERR_NOT_SORTED).  Out of
  * place: the advanced particles are written to the OTHER column set, which becomes the current
- * one (psc_particles_current), in the order of the sorted list.
+ * one (psc_particles_current).  Every cell's particles are written back into that cell's
+ * segment of the list, those that stay in the cell first, those that left it (a particle moves
+ * at most one cell per direction and step) behind them: the list is then no longer
+ * sorted, psc_particles_keys tells the cell of every particle.
  * J ghosts are NOT folded on return (psc_exchange_j). */
 int psc_push_particles(psc_ctx *ctx, void *stream);
 
@@ -154,9 +155,13 @@ int psc_fill_ghosts(psc_ctx *ctx, int which, void *stream);
 
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
- * u^{n+1}.  Same results as the calls above in that order; from the second step on the sort
- * only builds the index (permutation + cell offsets) and the particle loop reorders on load
- * (PAPER.md:603), so every particle column is read once and written once per step. */
+ * u^{n+1}.  Same fields and the same set of particles (up to the rounding of the atomically
+ * summed J) as the calls above in that order.  From the second step on the sort works on cells
+ * and cell-leavers only: it builds new cell offsets and, per cell, the list of
+ * arriving particles from the 9 / 27 direction classes the previous push recorded; the particle
+ * loop loads a cell's stayers as one run and its arrivals through that list (reorder on load),
+ * so every particle column is read once and written once per step.  Inside a cell the order is
+ * then "stayers, arrivals" instead of the stable order psc_particles_sort gives. */
 int psc_step(psc_ctx *ctx, void *stream);
 
 /* End-to-end form with HOST buffers: copies the host particle columns (n particles) and host
@@ -166,8 +171,8 @@ int psc_step(psc_ctx *ctx, void *stream);
 int psc_step_host(psc_ctx *ctx, void *stream, int64_t n, const psc_particle_cols *host,
                   float *hostE, float *hostB, float *hostJ, int nsteps);
 
-/* Inspection of the last sort.  Device pointers into the workspace, valid until the next sort
- * or push:
+/* Inspection of the last psc_particles_sort.  Device pointers into the workspace, valid until
+ * the next sort or push:
  * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i; computed on `stream` by this
  * call), perm[n] (sorted slot s holds input particle perm[s]), cell_offsets[n_keys+1]
  * (exclusive scan of the key histogram). */
@@ -180,7 +185,7 @@ int psc_particles_current(const psc_ctx *ctx, psc_particle_cols *out);
 int psc_particles_form(const psc_ctx *ctx);
 /* Internal form only: key[n] of the current particles (cell key as defined by the sort; the cell
  * a particle's offset refers to), computed on `stream` by this call from the cell offsets and
- * the direction codes.  Device pointer into the workspace, valid until the next call. */
+ * the leavers' direction codes.  Device pointer into the workspace, valid until the next call. */
 int psc_particles_keys(psc_ctx *ctx, void *stream, const int32_t **key);
 /* Converts the current columns back to absolute positions x = (cell + offset) * dx, in place
  * (one fp32 rounding).  The list counts as unsorted afterwards.  No-op on absolute columns. */

@@ -363,6 +363,45 @@ def test_ten_steps_match_oracle(kind):
     assert rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B) < 10 * TOL
 
 
+@pytest.mark.parametrize("order", [1, 2])
+def test_index_path_mass_migration(order):
+    """steady-state sort (cells + leavers only) under stress: a cold drifting slab in which whole
+    cells empty out and refill (v dt/dx = 0.3 along y, 0.15 along z, |v| = 0.95 c: two fifths of
+    the particles change cell every step, cells receive > 32 arrivals, cells start with zero
+    stayers), most of the grid empty.  Eight psc_step against the oracle, matched by id; keys agree with positions."""
+    pl = psc_inputs.thermal((1, 16, 24), 40, seed=17, order=order, name="slab")
+    keep = (pl.y >= 3.0) & (pl.y < 6.0) & (pl.species == 0)     # a slab three cells thick, one species
+    for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species"):
+        setattr(pl, k, getattr(pl, k)[keep].contiguous())
+    n = pl.y.numel()
+    pl.id = torch.arange(n, dtype=torch.int32)
+    vy, vz = 0.3 * pl.dx[1] / pl.dt, 0.15 * pl.dx[2] / pl.dt   # cells per step -> velocity
+    gam = 1.0 / np.sqrt(1.0 - vy * vy - vz * vz)
+    pl.ux = torch.zeros(n); pl.uy = torch.full((n,), float(gam * vy)); pl.uz = torch.full((n,), float(gam * vz))
+    pl.qw = pl.qw * 1e-3                                        # nearly a test-particle beam
+    sim = _sim(pl)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    lb = library_block(pl.n)
+    for it in range(8):
+        orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], 1)
+        sim.step(1)
+        assert sim.psc.status() == 0
+        # the cell each particle is filed under is the cell its position is in
+        _, py, pz = gpu_positions_f64(sim)
+        cells = key_to_cell(sim.keys().cpu().numpy().astype(np.int64), pl.n, lb)
+        assert np.array_equal(np.floor(py / pl.dx[1]).astype(np.int64), cells[1])
+        assert np.array_equal(np.floor(pz / pl.dx[2]).astype(np.int64), cells[2])
+        ids = sim.current()["id"].cpu().numpy()
+        assert np.array_equal(np.sort(ids), np.arange(n))      # nobody lost, nobody duplicated
+        o = order_by_id(ids, st["id"])
+        L = [pl.n[d] * pl.dx[d] for d in range(3)]
+        assert (periodic_dist(py[o], st["y"], L[1]) / L[1]).max() < TOL
+        assert (periodic_dist(pz[o], st["z"], L[2]) / L[2]).max() < TOL
+        assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+
+
 def test_step_host_end_to_end():
     """psc_step_host (host buffers in, host buffers out) equals the device-resident path"""
     pl = _small("2d")
