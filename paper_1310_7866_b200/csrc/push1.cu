@@ -694,7 +694,8 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8 && c->opt_push_variant != 2;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
+    if (def && c->opt_push_variant == 1) PSC_LAUNCH_PUSH1(false, 8, 128, 6);
+    else if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
   }
 #undef PSC_LAUNCH_PUSH1
