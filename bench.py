@@ -49,6 +49,8 @@ WORKLOADS = {
 }
 # algorithmic bytes per particle of the fused kernel
 PUSH_BYTES = {2: 48, 3: 56}
+# k_push2: smsp__inst_executed.sum / particles of the committed capture (profiles/r1d_push_kernels_ncu.md)
+PUSH2_WARP_INST_PER_PARTICLE = 6.25e9 / 83886080
 
 
 def peaks():
@@ -301,6 +303,18 @@ def run_psc(args):
                 "unit": "GB/s", "frac": achieved / peak, "traffic": None,
                 "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
                 "share_of_step": push_ms / ms if ms else None}
+    if pl.order == 2 and push_n:
+        # the order-2 kernel is bound by plain ALU/FMA issue, not by HBM:
+        # achieved = warp instructions per particle (ncu smsp__inst_executed.sum of the committed
+        # capture / particles) * particles / kernel time; peak = SMs * 4 schedulers * SM clock
+        props = torch.cuda.get_device_properties(dev)
+        sm_clock_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
+        peak_inst = props.multi_processor_count * 4 * sm_clock_ghz          # G warp-inst/s
+        ach_inst = PUSH2_WARP_INST_PER_PARTICLE * npart / (push_avg * 1e-3) / 1e9
+        roofline.update({"bound": "alu", "achieved": ach_inst, "peak": peak_inst, "unit": "Gwarp-inst/s",
+                         "frac": ach_inst / peak_inst, "hbm_achieved_gbs": achieved, "hbm_frac": achieved / peak,
+                         "peak_source": "148 SMs x 4 schedulers x max SM clock (1 warp instruction per scheduler and cycle)",
+                         "warp_inst_per_particle": PUSH2_WARP_INST_PER_PARTICLE})
     tr = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch from the committed ncu captures
     if os.path.exists(tr) and scale is None:
         import csv
