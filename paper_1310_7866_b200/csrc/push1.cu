@@ -39,6 +39,11 @@
 
 namespace {
 
+constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
+constexpr int QW = 8;      // words per entry
+constexpr int QROWS3 = 12; // rows of the queue in 3-d: the drain reuses drained slots as scratch [NV]
+constexpr int NST = 4;        // chunks in the per-warp column ring (NST - 1 in flight)
+constexpr int RING_COLS = 9;  // y z ux uy uz qw species [x] [id]
 
 
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
@@ -71,63 +76,6 @@ struct TileGeom {
     jvol = je[0] * je[1] * je[2];
   }
 };
-
-// one VB segment in the cell with tile-local coordinates (cx,cy,cz); a*, b* in-cell start/end
-template <bool D3, class TG>
-__device__ __forceinline__ void vb_segment(float *__restrict__ sJ, const TG &tg, int cx,
-                                           int cy, int cz, float ax, float ay, float az, float bx,
-                                           float by, float bz, float tau, float fx, float fy,
-                                           float fz, float qvx) {
-  const float my = 0.5f * (ay + by), mz = 0.5f * (az + bz);
-  const float dy = by - ay, dz = bz - az;
-  float *jx = sJ, *jy = sJ + tg.jvol, *jz = sJ + 2 * tg.jvol;
-  if (D3) {
-    const float mx = 0.5f * (ax + bx), dx = bx - ax;
-    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1];
-    const int base = ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1);
-    {
-      const float c = fx * dx, h = dy * dz * (1.0f / 12.0f);
-      atomicAdd(&jx[base], c * ((1.f - my) * (1.f - mz) + h));
-      atomicAdd(&jx[base + s1], c * (my * (1.f - mz) - h));
-      atomicAdd(&jx[base + s2], c * ((1.f - my) * mz - h));
-      atomicAdd(&jx[base + s1 + s2], c * (my * mz + h));
-    }
-    {
-      const float c = fy * dy, h = dz * dx * (1.0f / 12.0f);
-      atomicAdd(&jy[base], c * ((1.f - mz) * (1.f - mx) + h));
-      atomicAdd(&jy[base + s2], c * (mz * (1.f - mx) - h));
-      atomicAdd(&jy[base + 1], c * ((1.f - mz) * mx - h));
-      atomicAdd(&jy[base + s2 + 1], c * (mz * mx + h));
-    }
-    {
-      const float c = fz * dz, h = dx * dy * (1.0f / 12.0f);
-      atomicAdd(&jz[base], c * ((1.f - mx) * (1.f - my) + h));
-      atomicAdd(&jz[base + 1], c * (mx * (1.f - my) - h));
-      atomicAdd(&jz[base + s1], c * ((1.f - mx) * my - h));
-      atomicAdd(&jz[base + s1 + 1], c * (mx * my + h));
-    }
-  } else {
-    const int s2 = tg.je[1];
-    const int base = (cz + 1) * tg.je[1] + (cy + 1);
-    {
-      const float c = qvx * tau, h = dy * dz * (1.0f / 12.0f);
-      atomicAdd(&jx[base], c * ((1.f - my) * (1.f - mz) + h));
-      atomicAdd(&jx[base + 1], c * (my * (1.f - mz) - h));
-      atomicAdd(&jx[base + s2], c * ((1.f - my) * mz - h));
-      atomicAdd(&jx[base + s2 + 1], c * (my * mz + h));
-    }
-    {
-      const float c = fy * dy;
-      atomicAdd(&jy[base], c * (1.f - mz));
-      atomicAdd(&jy[base + s2], c * mz);
-    }
-    {
-      const float c = fz * dz;
-      atomicAdd(&jz[base], c * (1.f - my));
-      atomicAdd(&jz[base + 1], c * my);
-    }
-  }
-}
 
 // ---- warp-level reduction of the home-cell currents -------------------------------------------
 // The particle list is cell-ordered, so the 32 lanes of a warp mostly sit in ONE cell and their
@@ -230,14 +178,22 @@ __device__ __forceinline__ void vb_values(float (&v)[D3 ? 12 : 8], float ax, flo
 }
 
 // Walks the straight line a -> a + dd (cells; at most one face crossing per direction because
-// dt <= dx/2) and deposits every segment from number `first_seg` on with
-// shared-memory atomics.  first_seg = 1 is the slow path of the kernel below: segment 0 (inside
-// the home cell) has already gone through the warp reduction.
+// dt <= dx/2) and deposits every segment -- the slow path of the kernel below,
+// taken by the trajectories that leave their cell.
+// The segments' currents are added with shared-memory atomics, which are compare-and-swap loops
+// for fp32 (ATOMS.CAST.SPIN) and therefore pay for every same-address collision inside the
+// warp.  The trajectories drained together come from a few cells and cross the same faces, i.e.
+// hit the same J points in the same order; so each lane walks its NV values in a different
+// rotation (start = lane mod NV): the values go through a lane-private scratch column `scr`
+// ([NV][QCAP], the drained queue slots) and are picked with the rotated index, the point offsets
+// from the table `rel` ([NV], the order of vb_values).
 template <bool D3, class TG>
 __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, int lx,
                                         int ly, int lz, float ax, float ay, float az, float ddx,
                                         float ddy, float ddz, float fx, float fy, float fz,
-                                        float qvx, int first_seg) {
+                                        float qvx, const int *__restrict__ rel,
+                                        float *__restrict__ scr, int rot) {
+  constexpr int NV = D3 ? 12 : 8;
   const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
   const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
   const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
@@ -262,9 +218,21 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
     } else {
       qz = szd > 0 ? (float)(rz + 1) : (float)rz;
     }
-    if (seg >= first_seg)
-      vb_segment<D3>(sJ, tg, lx + rx, ly + ry, lz + rz, px - rx, py - ry, pz - rz, qx - rx, qy - ry,
-                     qz - rz, t - tprev, fx, fy, fz, qvx);
+    {
+      float v[NV];
+      vb_values<D3>(v, px - rx, py - ry, pz - rz, qx - rx, qy - ry, qz - rz, t - tprev, fx, fy, fz, qvx);
+      const int cx = lx + rx, cy = ly + ry, cz = lz + rz;
+      float *node = sJ + (D3 ? ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1)
+                             : (cz + 1) * tg.je[1] + (cy + 1));
+#pragma unroll
+      for (int i = 0; i < NV; i++) scr[i * QCAP] = v[i];
+      int idx = rot;
+#pragma unroll
+      for (int j = 0; j < NV; j++) {
+        atomicAdd(node + rel[idx], scr[idx * QCAP]);
+        idx = idx + 1 == NV ? 0 : idx + 1;
+      }
+    }
     if (which == 3) break;
     if (which == 0) { rx += sxd; tx = 2.f; }
     else if (which == 1) { ry += syd; ty = 2.f; }
@@ -274,15 +242,11 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
   }
 }
 
-constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
-constexpr int QW = 8;      // words per entry
-constexpr int NST = 4;        // chunks in the per-warp column ring (NST - 1 in flight)
-constexpr int RING_COLS = 9;  // y z ux uy uz qw species [x] [id]
 
 template <bool D3, class TG>
 __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg,
-                                            const GridDesc &gd, const float *__restrict__ q,
-                                            int start, int n, int lane) {
+                                            const GridDesc &gd, float *__restrict__ q,
+                                            const int *__restrict__ rel, int start, int n, int lane) {
   if (lane < n) {
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
@@ -294,7 +258,7 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
     const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
     vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
-                qvx, 0);
+                qvx, rel, q + e, lane % (D3 ? 12 : 8));
   }
   __syncwarp();
 }
@@ -333,10 +297,12 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   float *sJ = smem + 6 * tg.fvol;             // [3][jvol]
   float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
   int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
-  float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QW][QCAP]
-  float *myQ = sQ + warp * (QW * QCAP);
-  float *myRing = sQ + nwarps * (QW * QCAP) + warp * (NST * RING_COLS * 32);  // [NST][RING_COLS][32]
-  int *sIn = (int *)(sQ + nwarps * (QW * QCAP + NST * RING_COLS * 32));  // [cpb]: first input slot of each cell's run
+  constexpr int QR = D3 ? QROWS3 : QW;        // queue rows (>= NV: drained slots serve as scratch)
+  float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QR][QCAP]
+  float *myQ = sQ + warp * (QR * QCAP);
+  float *myRing = sQ + nwarps * (QR * QCAP) + warp * (NST * RING_COLS * 32);  // [NST][RING_COLS][32]
+  int *sRel = (int *)(sQ + nwarps * (QR * QCAP + NST * RING_COLS * 32));  // [12]: J points of vb_values
+  int *sIn = sRel + 12;                            // [cpb]: first input slot of each cell's run
   int *sNs = sIn + tg.cpb;                         // [cpb]: length of that run
   int *sA = sNs + tg.cpb;                          // [cpb + 1]: first arrival-list entry
   int *sOut = sA + tg.cpb + 1;                     // [cpb + 1]: output segments
@@ -345,6 +311,13 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   const int *__restrict__ alist = pls.alist;
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
+  if (threadIdx.x < NV) {  // J points of the NV in-cell currents, relative to the cell's node
+    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1], jv = tg.jvol;
+    const int off3[12] = {0, s1, s2, s1 + s2, jv, jv + s2, jv + 1, jv + s2 + 1,
+                          2 * jv, 2 * jv + 1, 2 * jv + s1, 2 * jv + s1 + 1};
+    const int off2[8] = {0, 1, s2, s2 + 1, jv, jv + s2, 2 * jv, 2 * jv + 1};
+    sRel[threadIdx.x] = D3 ? off3[threadIdx.x] : off2[threadIdx.x & 7];
+  }
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
     const int lx = r % tg.fe[0], t = r / tg.fe[0];
@@ -380,20 +353,12 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   // (lx+1, ly+1, lz+1) tile node) it belongs to
   int my_off;
   bool writer;
-  {
-    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1], jv = tg.jvol;
-    if (D3) {
-      const int idx = red12_index(lane);
-      const int off[12] = {0, s1, s2, s1 + s2, jv, jv + s2, jv + 1, jv + s2 + 1,
-                           2 * jv, 2 * jv + 1, 2 * jv + s1, 2 * jv + s1 + 1};
-      my_off = off[idx];
-      writer = (lane & 1) == 0 && !((lane & 2) && (lane & 4));
-    } else {
-      const int idx = (lane >> 2) & 7;
-      const int off[8] = {0, 1, s2, s2 + 1, jv, jv + s2, 2 * jv, 2 * jv + 1};
-      my_off = off[idx];
-      writer = (lane & 3) == 0;
-    }
+  if (D3) {
+    my_off = sRel[red12_index(lane)];
+    writer = (lane & 1) == 0 && !((lane & 2) && (lane & 4));
+  } else {
+    my_off = sRel[(lane >> 2) & 7];
+    writer = (lane & 3) == 0;
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
@@ -580,7 +545,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
         __syncwarp();
         if (qcnt >= 32) {
           qcnt -= 32;
-          drain_queue<D3>(sJ, tg, gd, myQ, qcnt, 32, lane);
+          drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
         }
       }
 
@@ -633,7 +598,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       }
     }
   }
-  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, 0, qcnt, lane);
+  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, sRel, 0, qcnt, lane);
   if (bad) atomicOr(flags, bad);
   __syncthreads();
 
@@ -666,7 +631,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const int vthreads = 128;
   const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : vthreads;
   if (threads < 32 || threads > vthreads) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + QW * QCAP + NST * RING_COLS * 32) + 4 * gd.cpb + 2) * sizeof(float);
+  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + (d3 ? QROWS3 : QW) * QCAP + NST * RING_COLS * 32) + 12 + 4 * gd.cpb + 2) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const Cols &in = c->cols[c->cur];
