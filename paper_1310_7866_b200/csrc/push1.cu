@@ -177,6 +177,55 @@ __device__ __forceinline__ void vb_values(float (&v)[D3 ? 12 : 8], float ax, flo
   }
 }
 
+// The same in-cell currents, accumulated as MOMENTS: with e, f the two transverse midpoints of a
+// component and c its prefactor, the four values are c((1-e)(1-f)+h), c(e(1-f)-h), c((1-e)f-h),
+// c(ef+h), i.e. linear in M0 = c, M1 = c e, M2 = c f, M3 = c (e f + h):
+//   v_a = M0 - M1 - M2 + M3, v_b = M1 - M3, v_c = M2 - M3, v_d = M3
+// (2-d in-plane components: c(1-m), c m from N0 = c, N1 = c m).  Summing the moments over a
+// cell's particles and converting once per cell (moments_to_values) costs 7 instead of 16
+// operations per particle and component.  acc uses the slots of the values it turns into.
+template <bool D3>
+__device__ __forceinline__ void vb_moments(float (&acc)[D3 ? 12 : 8], float ax, float ay, float az,
+                                           float bx, float by, float bz, float fx, float fy,
+                                           float fz, float qvx) {
+  const float my = 0.5f * (ay + by), mz = 0.5f * (az + bz);
+  const float dy = by - ay, dz = bz - az;
+  auto add4 = [](float *m, float c, float e, float f, float dd) {
+    m[0] += c;
+    m[1] = fmaf(c, e, m[1]);
+    m[2] = fmaf(c, f, m[2]);
+    m[3] = fmaf(c, fmaf(e, f, dd * (1.0f / 12.0f)), m[3]);
+  };
+  if (D3) {
+    const float mx = 0.5f * (ax + bx), dx = bx - ax;
+    add4(acc + 0, fx * dx, my, mz, dy * dz);
+    add4(acc + 4, fy * dy, mz, mx, dz * dx);
+    add4(acc + 8, fz * dz, mx, my, dx * dy);
+  } else {
+    add4(acc + 0, qvx, my, mz, dy * dz);
+    const float cy = fy * dy, cz = fz * dz;
+    acc[4] += cy;
+    acc[5] = fmaf(cy, mz, acc[5]);
+    acc[6] += cz;
+    acc[7] = fmaf(cz, my, acc[7]);
+  }
+}
+
+template <bool D3>
+__device__ __forceinline__ void moments_to_values(float (&acc)[D3 ? 12 : 8]) {
+#pragma unroll
+  for (int b = 0; b < (D3 ? 12 : 4); b += 4) {
+    const float m0 = acc[b], m1 = acc[b + 1], m2 = acc[b + 2], m3 = acc[b + 3];
+    acc[b] = (m0 - m1) - (m2 - m3);
+    acc[b + 1] = m1 - m3;
+    acc[b + 2] = m2 - m3;
+  }
+  if (!D3) {
+    acc[4] -= acc[5];
+    acc[6] -= acc[7];
+  }
+}
+
 // Walks the straight line a -> a + dd (cells; at most one face crossing per direction because
 // dt <= dx/2) and deposits every segment -- the slow path of the kernel below,
 // taken by the trajectories that leave their cell.
@@ -515,11 +564,8 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       // register sums; one that leaves goes through the per-warp queue (all its segments)
       {
         const float qs = cross ? 0.f : qw;
-        float v[NV];
-        vb_values<D3>(v, ax, ay, az, endx, endy, endz, 1.f, qs * gd.cur[0], qs * gd.cur[1],
-                      qs * gd.cur[2], qs * gd.inv_dV * vx);
-#pragma unroll
-        for (int i = 0; i < NV; i++) acc[i] += v[i];
+        vb_moments<D3>(acc, ax, ay, az, endx, endy, endz, qs * gd.cur[0], qs * gd.cur[1],
+                       qs * gd.cur[2], qs * gd.inv_dV * vx);
       }
       const unsigned cm = __ballot_sync(0xffffffffu, cross);
       const unsigned sm = __ballot_sync(0xffffffffu, act && !cross);
@@ -577,6 +623,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     // add per J point; its direction-code counts go to the index sort
     if (!a.ok || a.ci != c.ci) {
       float r;
+      moments_to_values<D3>(acc);
       if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
       else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(acc), lane);
       if (writer) {
