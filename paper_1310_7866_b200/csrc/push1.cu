@@ -420,6 +420,8 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   struct It {
     int ci, base, p1;  // cell, first particle of the chunk, particles in the cell
     bool ok;
+    int ns, in0;       // the cell's stayer run: length, first input slot (per-cell constants kept
+                       // in registers: the load/store path of the SM is the scarce resource)
   };
   auto adv = [&](It &it) {
     it.base += 32;
@@ -431,6 +433,8 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       }
       it.base = 0;
       it.p1 = sOut[it.ci + 1] - sOut[it.ci];
+      it.ns = sNs[it.ci];
+      it.in0 = sIn[it.ci];
     }
   };
   struct Raw {
@@ -438,8 +442,8 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     int sp, id;
   };
   auto load_perm = [&](const It &it) -> int {
-    const int v = it.base + lane, ns = sNs[it.ci];
-    return (v >= ns && v < it.p1) ? ld_stream(alist + (sA[it.ci] + v - ns)) : sIn[it.ci] + v;
+    const int v = it.base + lane;
+    return (v >= it.ns && v < it.p1) ? ld_stream(alist + (sA[it.ci] + v - it.ns)) : it.in0 + v;
   };
   // Particle columns travel through a per-warp shared-memory ring of NST chunks filled with
   // asynchronous 4-byte copies (cp.async; each lane copies and later reads its own element, so no
@@ -478,7 +482,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     r_.id = has_id ? __float_as_int(r[8 * 32]) : 0;
   };
 
-  It a = {warp - nwarps, 0, 0, true};  // the chunk to compute
+  It a = {warp - nwarps, 0, 0, true, 0, 0};  // the chunk to compute
   adv(a);
   It pr = a;                           // the chunk to issue loads for (NST - 1 ahead)
   int pPr = 0;
@@ -496,6 +500,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   }
   int ncross = 0, nst = 0;  // warp-uniform: leavers / stayers of the current cell so far
   int cur_ci = -1, lx = 0, ly = 0, lz = 0, packed = 0;
+  int oF = 0, oB = 0;  // the cell's output segment: first slot, last slot
   const float *cF = sF;
   float acc[NV];
 
@@ -520,6 +525,8 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       ly = lt_ % tg.bs[1];
       lz = lt_ / tg.bs[1];
       packed = lx | (ly << 10) | (lz << 20);
+      oF = sOut[c.ci];
+      oB = sOut[c.ci + 1] - 1;
       // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
       cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
                     : (lz + 1) * tg.fe[1] + (ly + 1));
@@ -570,8 +577,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       const unsigned cm = __ballot_sync(0xffffffffu, cross);
       const unsigned sm = __ballot_sync(0xffffffffu, act && !cross);
       // output slot: stayers fill the cell's segment from the front, leavers from the back
-      const int s = cross ? sOut[c.ci + 1] - 1 - ncross - __popc(cm & lt)
-                          : sOut[c.ci] + nst + __popc(sm & lt);
+      const int s = cross ? oB - ncross - __popc(cm & lt) : oF + nst + __popc(sm & lt);
       nst += __popc(sm);
       if (cm) {
         if (cross) {
