@@ -149,7 +149,8 @@ k_to_abs(GridDesc gd, int n, const int *__restrict__ key, float *__restrict__ x,
 #pragma unroll
   for (int d = 0; d < 3; d++) {
     if (gd.n[d] == 1) continue;
-    float v = ((float)c[d] + pos[d][a]) * gd.dx[d];
+    // formed in fp64 and rounded once (this pass runs once per export, not per step)
+    float v = __double2float_rn(((double)c[d] + (double)pos[d][a]) * (double)gd.dx[d]);
     if (v >= gd.L[d]) v = nextafterf(gd.L[d], 0.f);  // rounding must not leave [0, L)
     pos[d][a] = v;
   }
@@ -399,10 +400,18 @@ k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out) {
     const int sp = in.sp[p];
     int id = 0;
     if (in.id) id = in.id[p];
-    if (FROM_ABS) {  // same fp32 product + floor as k_keys; clamped like there
-      if (gd.n[0] > 1) { const float xi = __fmul_rn(x, gd.inv_dx[0]); x = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
-      if (gd.n[1] > 1) { const float xi = __fmul_rn(y, gd.inv_dx[1]); y = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
-      if (gd.n[2] > 1) { const float xi = __fmul_rn(z, gd.inv_dx[2]); z = fminf(fmaxf(xi - floorf(xi), 0.f), 0.99999994f); }
+    if (FROM_ABS) {
+      // the cell is decided as in k_keys (fp32 product with 1/dx, floor); the offset is then
+      // (x - cell dx) / dx with the difference formed by one FMA, i.e. accurate to fp32 RELATIVE
+      // precision of the offset also when dx is not a power of two (x * (1/dx) - cell would carry
+      // the absolute rounding error of x / dx, ~1e-6 cells at x / dx ~ 20)
+      auto rel = [&](float v, int d) {
+        const float c = floorf(__fmul_rn(v, gd.inv_dx[d]));
+        return fminf(fmaxf(fmaf(-c, gd.dx[d], v) * gd.inv_dx[d], 0.f), 0.99999994f);
+      };
+      if (gd.n[0] > 1) x = rel(x, 0);
+      if (gd.n[1] > 1) y = rel(y, 1);
+      if (gd.n[2] > 1) z = rel(z, 2);
     }
     if (in.x) out.x[s] = x;
     out.y[s] = y;

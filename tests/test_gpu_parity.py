@@ -38,6 +38,20 @@ def _small(kind):
         return psc_inputs.thermal((12, 20, 8), 5, seed=13, order=2, name="ragged3d-o2")
     if kind == "2d-o2":                                         # order 2 in the yz plane (NEXT #2)
         return psc_inputs.thermal((1, 24, 40), 9, seed=14, order=2, name="ragged2d-o2")
+    if kind in ("2d-aniso", "2d-aniso-o2", "3d-aniso", "3d-aniso-o2"):
+        # anisotropic cells (dx != dy != dz != 1), four species, per-particle random weights
+        d3 = kind.startswith("3d")
+        pl = psc_inputs.thermal((12, 20, 8) if d3 else (1, 24, 40), 5 if d3 else 7,
+                                dx=(0.8, 1.25, 0.5) if d3 else (1.0, 0.5, 2.0), seed=31 + d3,
+                                order=2 if kind.endswith("o2") else 1, name=kind)
+        g = torch.Generator().manual_seed(77)
+        n = pl.qw.numel()
+        pl.qw = (pl.qw * (0.5 + torch.rand(n, generator=g))).float()
+        pl.q = list(pl.q) + [-2.0, 3.0]
+        pl.m = list(pl.m) + [4.0, 50.0]
+        flip = torch.rand(n, generator=g) < 0.3        # a third of the particles become species 2 / 3
+        pl.species = torch.where(flip, pl.species + 2, pl.species).to(torch.int32)
+        return pl
     raise ValueError(kind)
 
 
@@ -286,7 +300,9 @@ def _push_once(kind, block, amp=0.05):
                                         ("3d-ragged", (2, 4, 2)), ("3d-ragged", (1, 1, 1)),
                                         ("harris", (1, 8, 8)), ("beam", (0, 0, 0)),
                                         ("3d-ragged-o2", (2, 4, 2)), ("3d-ragged-o2", (1, 1, 1)),
-                                        ("2d-o2", (0, 0, 0)), ("2d-o2", (1, 3, 5))])
+                                        ("2d-o2", (0, 0, 0)), ("2d-o2", (1, 3, 5)),
+                                        ("2d-aniso", (0, 0, 0)), ("2d-aniso-o2", (1, 4, 8)),
+                                        ("3d-aniso", (0, 0, 0)), ("3d-aniso-o2", (2, 4, 2))])
 def test_push_particles_matches_oracle(kind, block):
     pl, sim, orc, cols0, st, sp, J = _push_once(kind, block)
     got = gpu_cols(sim)
@@ -309,7 +325,7 @@ def test_push_particles_matches_oracle(kind, block):
     assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
 
 
-@pytest.mark.parametrize("kind", ["2d", "3d", "beam", "2d-o2"])
+@pytest.mark.parametrize("kind", ["2d", "3d", "beam", "2d-o2", "2d-aniso", "3d-aniso-o2"])
 def test_gpu_continuity_residual(kind):
     """(rho^{n+3/2} - rho^{n+1/2})/dt + div- j^{n+1} = 0 (Eq. 25) with the GPU's J and the GPU's
     stored fp32 positions, evaluated by the oracle's rho / div-; normalised by max|rho_s|/dt of one
@@ -331,7 +347,7 @@ def test_gpu_continuity_residual(kind):
 # ------------------------------------------------------------------------------------------------
 # closed loop: 10 psc_step, particles matched by id
 
-@pytest.mark.parametrize("kind", ["2d", "3d", "harris", "beam", "2d-o2"])
+@pytest.mark.parametrize("kind", ["2d", "3d", "harris", "beam", "2d-o2", "2d-aniso-o2", "3d-aniso"])
 def test_ten_steps_match_oracle(kind):
     pl = _small(kind)
     sim = _sim(pl)
