@@ -1,0 +1,102 @@
+"""Error behaviour of the C ABI on a device and degenerate inputs of the particle loop."""
+import ctypes as C
+
+import numpy as np
+import pytest
+import torch
+
+import paper_1310_7866_b200 as psc
+import psc_inputs
+from tests.util import gpu_cols, oracle_for, oracle_state, order_by_id, periodic_dist, rel_maxnorm
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+def _sim(pl, **kw):
+    from paper_1310_7866_b200.harness import Simulation
+
+    return Simulation(pl, **kw)
+
+
+def test_call_order_and_binding_errors():
+    pl = psc_inputs.thermal((1, 8, 8), 2, seed=5)
+    sim = _sim(pl)
+    L, h = psc.lib(), sim.psc._h
+    assert L.psc_push_particles(h, None) == -3                  # PSC_ERR_NOT_SORTED: no sort yet
+    sim.psc.particles_sort()
+    sim.psc.push_particles()
+    assert L.psc_push_particles(h, None) == -3                  # pushed list: sort again first
+    sim.psc.particles_sort()
+    assert L.psc_push_fields(h, 7, C.c_float(0.5), None) == -1  # which must be PSC_E or PSC_B
+    assert L.psc_push_fields(h, 1, C.c_float(0.0), None) == -1  # frac > 0
+    assert L.psc_fill_ghosts(h, 9, None) == -1
+    # a workspace that is too small / misaligned is refused
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    assert L.psc_bind_workspace(h, C.c_void_p(small.data_ptr() + 8), C.c_size_t(1016)) == -5   # PSC_ERR_ALIGN
+    sim.psc.particles_export()                                  # (keys live in the workspace)
+    assert L.psc_bind_workspace(h, C.c_void_p(small.data_ptr()), C.c_size_t(1024)) == -8       # PSC_ERR_WORKSPACE
+    assert sim.psc.status() == 0
+
+
+def test_unbound_context_reports_not_bound():
+    pl = psc_inputs.thermal((1, 8, 8), 1, seed=5)
+    p = psc.Psc(pl.n, pl.dx, pl.dt, 1, pl.q, pl.m, (0, 0, 0))
+    L = psc.lib()
+    assert L.psc_step(p._h, None) == -2                         # PSC_ERR_NOT_BOUND
+    assert L.psc_particles_sort(p._h, None) == -2
+    assert L.psc_push_fields(p._h, 1, C.c_float(0.5), None) == -2
+
+
+@pytest.mark.parametrize("order", [1, 2])
+def test_eight_species_and_particles_on_faces(order):
+    """PSC_MAX_SPECIES species (one neutral, one heavy), particles placed exactly on cell faces,
+    on the domain origin and one ulp below the upper edge; five steps against the oracle."""
+    pl = psc_inputs.thermal((1, 16, 12), 6, seed=41, order=order, name="faces")
+    n = pl.y.numel()
+    g = torch.Generator().manual_seed(3)
+    pl.q = [-1.0, 1.0, 0.0, 2.0, -3.0, 1.0, -1.0, 0.5]
+    pl.m = [1.0, 100.0, 1.0, 4.0, 9.0, 1836.0, 2.0, 0.7]
+    pl.species = torch.randint(0, 8, (n,), generator=g, dtype=torch.int32)
+    k = n // 4
+    pl.y[:k] = torch.floor(pl.y[:k])                            # exactly on faces
+    pl.z[k:2 * k] = torch.floor(pl.z[k:2 * k])
+    pl.y[0], pl.z[0] = 0.0, 0.0
+    pl.y[1] = float(np.nextafter(np.float32(16.0), np.float32(0.0)))
+    pl.z[2] = float(np.nextafter(np.float32(12.0), np.float32(0.0)))
+    sim = _sim(pl)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], 5)
+    sim.step(5)
+    assert sim.psc.status() == 0
+    got = gpu_cols(sim)
+    o = order_by_id(got["id"], st["id"])
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for d, c in ((1, "y"), (2, "z")):
+        assert (periodic_dist(got[c][o], st[c], L[d]) / L[d]).max() < TOL
+    assert np.array_equal(got["species"][o], st["species"])
+    for c in ("ux", "uy", "uz"):
+        assert np.abs(got[c][o] - st[c]).max() < TOL * 0.1
+    assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
+
+
+def test_step_host_without_optional_columns():
+    """psc_step_host in bench.py's configuration (no x, no id) equals the device-resident run"""
+    pl = psc_inputs.thermal((1, 16, 16), 4, seed=9)
+    a = _sim(pl, with_id=False, with_x=False)
+    a.step(2)
+    ref = gpu_cols(a)
+    b = _sim(pl, with_id=False, with_x=False)
+    host = {k: (None if k in ("x", "id") else getattr(pl, k).clone().pin_memory())
+            for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id")}
+    hE, hB = b.E.cpu().pin_memory(), b.B.cpu().pin_memory()
+    hJ = torch.zeros_like(hE).pin_memory()
+    b.psc.step_host(pl.n_particles, host, hE, hB, hJ, nsteps=2)
+    # no id to match by: compare per-cell-independent aggregates and the fields
+    for k in ("ux", "uy", "uz", "qw"):
+        assert abs(float(host[k].double().sum()) - float(ref[k].astype(np.float64).sum())) <= 1e-6 * np.abs(ref[k]).sum()
+    assert np.array_equal(np.sort(host["species"].numpy()), np.sort(ref["species"]))
+    assert (hE - a.E.cpu()).abs().max() <= 1e-5 * a.E.abs().max().cpu()
