@@ -63,9 +63,10 @@ extern "C" {
 
 /* sticky device flags (psc_status) */
 #define PSC_F_OOB 1u            /* a particle position outside [0, n*dx) was seen by the sort */
-#define PSC_F_MOVED_GT_1CELL 2u /* a particle moved more than one cell in a step */
+#define PSC_F_MOVED_GT_1CELL 2u /* reserved: a move of more than one cell cannot occur,
+                                   psc_create enforces dt <= dx/2 and |v| < c, so |move| < 1/2 cell;
+                                   non-finite momenta raise PSC_F_NAN instead */
 #define PSC_F_NAN 4u            /* a non-finite position or momentum was produced */
-#define PSC_F_NOT_IN_TILE 8u    /* push found a particle outside the block its sort slot belongs to */
 
 #define PSC_MAX_SPECIES 8
 #define PSC_GHOST 2
@@ -215,7 +216,10 @@ int psc_last_cuda_error(const psc_ctx *ctx);
 #define PSC_PH_SORT_REORDER 9
 #define PSC_PH_COUNT 16
 int psc_profile(psc_ctx *ctx, void *stream, double *ms, int64_t *count);
-/* Selects kernel variants for experiments; 0 = default.  Host only. */
+/* Host-side switches: "profile" (0/1: per-phase event timing), "clear_flags" (reset the sticky
+ * device flags), and for experiments "push_variant" (0 default; 1: 2-d default tile at 6 blocks
+ * per SM; 2: run-time tile geometry) and "threads" (threads per block of the particle kernels,
+ * multiple of 32, 0 = default).  Unknown names return PSC_ERR_INVALID_ARG. */
 int psc_set_option(psc_ctx *ctx, const char *name, int64_t value);
 const char *psc_strerror(int code);
 const char *psc_version(void);

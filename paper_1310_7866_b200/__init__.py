@@ -14,7 +14,7 @@ from . import build as _build
 
 PSC_OK = 0
 PSC_E, PSC_B, PSC_J = 0, 1, 2
-PSC_F_OOB, PSC_F_MOVED_GT_1CELL, PSC_F_NAN, PSC_F_NOT_IN_TILE = 1, 2, 4, 8
+PSC_F_OOB, PSC_F_MOVED_GT_1CELL, PSC_F_NAN = 1, 2, 4
 PSC_GHOST = 2
 PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
           "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9}

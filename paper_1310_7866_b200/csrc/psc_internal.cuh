@@ -94,7 +94,8 @@ struct psc_ctx {
   int last_err;
   int sm_count;
   // options
-  int opt_push_variant, opt_threads, opt_fuse_ghosts;
+  int opt_push_variant;  // 0: default; 1: 2-d default tile at 6 blocks/SM; 2: run-time tile geometry
+  int opt_threads;       // threads per block of the particle kernels (0: default)
 };
 
 #define PSC_CUDA_TRY(ctx, expr)                   \

@@ -19,12 +19,12 @@
 // the back with the one-byte direction code of their move; per cell the kernel writes the count
 // of each code.  The leavers' codes and the counts are all the next sort reads.
 //
-// Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction +
-// the cell key.  The move is b = a + v dt/dx; a particle that leaves its cell (b < 0 or b >= 1;
-// at most one cell per direction) gets offset b -/+ 1 and the key of the
-// neighbouring cell, looked up in per-direction tables that hold the periodic wrap -- the
-// single-GPU form of the particle exchange.  The new key is what the next sort
-// consumes; no floor(), no float->int conversion and no absolute coordinate appear here.
+// Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction;
+// the cell is implied by the segment.  The move is b = a + v dt/dx; a particle that leaves its
+// cell (b < 0 or b >= 1; at most one cell per direction) is stored with offset
+// b -/+ 1 and the direction code of the move; the index sort turns code + source cell into the
+// destination cell with the periodic wrap -- the single-GPU form of the particle exchange
+// (PAPER.md:403).  No floor(), no float->int conversion and no absolute coordinate appear here.
 //
 // The VB current is the exact flux of a b0-shaped cloud moving on the straight line
 // x^{n+1/2} -> x^{n+3/2}; it is evaluated by splitting the line at the cell faces it crosses
@@ -441,7 +441,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     float ax, ay, az, ux, uy, uz, qw, cx;
     int sp, id;
   };
-  auto load_perm = [&](const It &it) -> int {
+  auto load_slot = [&](const It &it) -> int {
     const int v = it.base + lane;
     return (v >= it.ns && v < it.p1) ? ld_stream(alist + (sA[it.ci] + v - it.ns)) : it.in0 + v;
   };
@@ -486,14 +486,14 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   adv(a);
   It pr = a;                           // the chunk to issue loads for (NST - 1 ahead)
   int pPr = 0;
-  if (pr.ok) pPr = load_perm(pr);
+  if (pr.ok) pPr = load_slot(pr);
   int stage_p = 0, stage_c = 0;
 #pragma unroll 1
   for (int k = 0; k < NST - 1; k++) {
     if (pr.ok) {
       issue(pr, pPr, stage_p);
       adv(pr);
-      if (pr.ok) pPr = load_perm(pr);
+      if (pr.ok) pPr = load_slot(pr);
     }
     cp_async_commit();
     stage_p++;
@@ -509,7 +509,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     if (pr.ok) {
       issue(pr, pPr, stage_p);
       adv(pr);
-      if (pr.ok) pPr = load_perm(pr);  // list entries one more chunk ahead
+      if (pr.ok) pPr = load_slot(pr);  // list entries one more chunk ahead
     }
     cp_async_commit();
     stage_p = stage_p + 1 == NST ? 0 : stage_p + 1;
