@@ -120,7 +120,9 @@ int psc_create(const psc_params *p, psc_ctx **out) {
     gd.bs[d] = bs;
     gd.nb[d] = p->n[d] / bs;
   }
-  if (tot * 3 > 0x7fffffffLL || nk > 0x3fffffffLL) {
+  // 32-bit indexing: 3 field components, and the per-cell direction table of the index sort
+  // (27 entries per cell)
+  if (tot * 3 > 0x7fffffffLL || nk * 27 > 0x7fffffffLL) {
     free(c);
     return PSC_ERR_INVALID_ARG;
   }
