@@ -97,21 +97,29 @@ __device__ __forceinline__ int red_index(int lane, int j) {
   return ok ? idx : -1;
 }
 
-template <bool D3>
+// CBS != 0: the sort block is CBS cells along every active direction (the library defaults, 8x8
+// in 2-d and 4x4x4 in 3-d), so every tile extent and stride folds into an immediate; CBS == 0:
+// run-time block.
+template <bool D3, int CBS>
 struct Geom2 {
   int o[3];     // first cell of the tile
+  int bs[3], cpb;
   int te[3];    // tile extents (fields and J alike): bs + 3 points, local point t <-> node o + t - 1
   int tvol;
   __device__ __forceinline__ void init(const GridDesc &gd, int tile) {
+    bs[0] = CBS ? (D3 ? CBS : 1) : gd.bs[0];
+    bs[1] = CBS ? CBS : gd.bs[1];
+    bs[2] = CBS ? CBS : gd.bs[2];
+    cpb = bs[0] * bs[1] * bs[2];
     const int b0 = tile % gd.nb[0];
     const int r = tile / gd.nb[0];
     const int b1 = r % gd.nb[1], b2 = r / gd.nb[1];
-    o[0] = b0 * gd.bs[0];
-    o[1] = b1 * gd.bs[1];
-    o[2] = b2 * gd.bs[2];
-    te[0] = D3 ? gd.bs[0] + 3 : 1;
-    te[1] = gd.bs[1] + 3;
-    te[2] = gd.bs[2] + 3;
+    o[0] = b0 * bs[0];
+    o[1] = b1 * bs[1];
+    o[2] = b2 * bs[2];
+    te[0] = D3 ? bs[0] + 3 : 1;
+    te[1] = bs[1] + 3;
+    te[2] = bs[2] + 3;
     tvol = te[0] * te[1] * te[2];
   }
 };
@@ -129,8 +137,8 @@ struct Sten2 {
   }
 };
 
-template <bool D3, bool SX, bool SY, bool SZ>
-__device__ __forceinline__ float gather2(const float *__restrict__ F, const Geom2<D3> &tg, int lx,
+template <bool D3, bool SX, bool SY, bool SZ, class TG>
+__device__ __forceinline__ float gather2(const float *__restrict__ F, const TG &tg, int lx,
                                          int ly, int lz, const Sten2 &sx, const Sten2 &sy,
                                          const Sten2 &sz) {
   const int ty = SY ? ly : sy.tn, tz = SZ ? lz : sz.tn;
@@ -169,8 +177,8 @@ __device__ __forceinline__ float gather2(const float *__restrict__ F, const Geom
 //   3-d, component c (transverse e, f cyclic): v[(jf * 4 + je) * 3 + i]   (48 values)
 //   2-d: jx: v[jz * 4 + jy] (16);  jy: v[jz * 3 + i] (12, flux along y);  jz: v[jy * 3 + i] (12)
 // tile offset (relative to the cell's own point (lx+1, ly+1, lz+1)) of value `idx`
-template <bool D3>
-__device__ __forceinline__ int value_offset(const Geom2<D3> &tg, int comp, int idx) {
+template <bool D3, class TG>
+__device__ __forceinline__ int value_offset(const TG &tg, int comp, int idx) {
   const int s[3] = {1, tg.te[0], tg.te[0] * tg.te[1]};
   if (idx < 0) return INT_MIN;
   if (D3) {
@@ -194,12 +202,12 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
     if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
 }
 
-template <bool D3>
+template <bool D3, int CBS>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
 k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
         const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
   extern __shared__ float smem[];
-  Geom2<D3> tg;
+  Geom2<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   float *sF = smem;                // [6][tvol]
   float *sJ = smem + 6 * tg.tvol;  // [3][tvol]
@@ -234,14 +242,14 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
 
   const float *sEx = sF, *sEy = sF + tg.tvol, *sEz = sF + 2 * tg.tvol;
   const float *sBx = sF + 3 * tg.tvol, *sBy = sF + 4 * tg.tvol, *sBz = sF + 5 * tg.tvol;
-  const int kbase = blockIdx.x * gd.cpb;
+  const int kbase = blockIdx.x * tg.cpb;
   uint32_t bad = 0;
 
   uint8_t *__restrict__ dcode = pls.dcode;
   int *__restrict__ dircnt = pls.dircnt;
   const unsigned lanes_lt = lanemask_lt_();
 
-  for (int ci = warp; ci < gd.cpb; ci += nwarps) {
+  for (int ci = warp; ci < tg.cpb; ci += nwarps) {
     // the cell's particles: its run of stayers of the previous step, then its listed arrivals
     // (reorder on load); its output segment: stayers from the front, leavers from the back
     const int in0 = pls.offs_in[kbase + ci];
@@ -249,8 +257,8 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     const int a0 = pls.aoffs ? pls.aoffs[kbase + ci] : 0;
     int ofront = pls.offs_out[kbase + ci], oback = pls.offs_out[kbase + ci + 1] - 1;
     const int np_cell = oback + 1 - ofront;  // stayers + arrivals
-    const int lx = ci % gd.bs[0], lt = ci / gd.bs[0];
-    const int ly = lt % gd.bs[1], lz = lt / gd.bs[1];
+    const int lx = ci % tg.bs[0], lt = ci / tg.bs[0];
+    const int ly = lt % tg.bs[1], lz = lt / tg.bs[1];
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
     for (int base = 0; base < np_cell; base += 32) {
@@ -463,13 +471,22 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const Cols &out = c->cols[c->cur ^ 1];
   const PushLists pls = psc_push_lists(c);
   ProfScope ps(c, PSC_PH_PUSH, s);
+#define PSC_LAUNCH_PUSH2(D3_, CBS_)                                                                 \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_>,                                       \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    k_push2<D3_, CBS_><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J,        \
+                                                        c->d_flags);                               \
+  } while (0)
+  const bool generic = c->opt_push_variant == 2;
   if (d3) {
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<true><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J, c->d_flags);
+    if (!generic && gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4) PSC_LAUNCH_PUSH2(true, 4);
+    else PSC_LAUNCH_PUSH2(true, 0);
   } else {
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_push2<false><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J, c->d_flags);
+    if (!generic && gd.bs[1] == 8 && gd.bs[2] == 8) PSC_LAUNCH_PUSH2(false, 8);
+    else PSC_LAUNCH_PUSH2(false, 0);
   }
+#undef PSC_LAUNCH_PUSH2
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
