@@ -50,7 +50,7 @@ WORKLOADS = {
 # algorithmic bytes per particle of the fused kernel
 PUSH_BYTES = {2: 48, 3: 56}
 # k_push2: smsp__inst_executed.sum / particles of the committed capture (profiles/r1e_push_kernels_ncu.md)
-PUSH2_WARP_INST_PER_PARTICLE = 6.2496e9 / 83886080
+PUSH2_WARP_INST_PER_PARTICLE = 5.5695e9 / 83886080
 
 
 def peaks():
