@@ -375,6 +375,10 @@ def run_psc(args):
     # ---- the oracle on the host cores (rank 0, N = 1 only) --------------------------------------
     if rank == 0 and world == 1 and not args.no_cpu:
         grid = sample_grids(args.config)[0 if not args.quick_cpu else -1]
+        if args.cpu_steps <= 0:  # about 10 s of oracle work on this sample (rough rates per config)
+            est = {1: 4.5e7, 2: 4.5e7, 3: 2.9e7, 4: 2.9e7, 5: 5e6}[args.config]
+            nsample = grid[0] * grid[1] * grid[2] * ppc_of(args.config)
+            args.cpu_steps = max(2, min(200, int(10.0 * est / nsample)))
         rate, threads, nsamp, _ = oracle_rate(args.config, grid, args.cpu_steps)
         out["cpu_baseline"] = {
             "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
@@ -396,7 +400,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--scale", default=None, help="NXxNYxNZ: smaller grid of the same recipe (debug)")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-steps", type=int, default=2)
+    ap.add_argument("--cpu-steps", type=int, default=0, help="oracle steps on the CPU sample (0: about 10 s of work)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick-cpu", action="store_true")
