@@ -190,25 +190,33 @@ class Psc:
 
     # -- the hot path ----------------------------------------------------------------------------
     def particles_sort(self, stream=None):
+        """psc_particles_sort: stable cell-key counting sort (include/psc.h)"""
         self._check(lib().psc_particles_sort(self._h, _stream(stream)), "psc_particles_sort")
 
     def push_particles(self, stream=None):
+        """psc_push_particles: fused gather (Eq. 11) - Boris (Eq. 27-28) - move (Eq. 26) -
+        charge-conserving deposit, the particle loop of Fig. 8"""
         self._check(lib().psc_push_particles(self._h, _stream(stream)), "psc_push_particles")
 
     def push_fields(self, which, frac, stream=None):
+        """psc_push_fields: Yee FDTD update of E or B over frac*dt (Eq. 17-18)"""
         self._check(lib().psc_push_fields(self._h, int(which), float(frac), _stream(stream)),
                     "psc_push_fields")
 
     def exchange_j(self, stream=None):
+        """psc_exchange_j: add_and_fill_ghosts_j of Fig. 8 on one GPU"""
         self._check(lib().psc_exchange_j(self._h, _stream(stream)), "psc_exchange_j")
 
     def fill_ghosts(self, which, stream=None):
+        """psc_fill_ghosts: ghosts := periodic images"""
         self._check(lib().psc_fill_ghosts(self._h, int(which), _stream(stream)), "psc_fill_ghosts")
 
     def step(self, stream=None):
+        """psc_step: one time step in the order of Fig. 8"""
         self._check(lib().psc_step(self._h, _stream(stream)), "psc_step")
 
     def step_host(self, n, host_cols, hE, hB, hJ=None, nsteps=1, stream=None):
+        """psc_step_host: the same with HOST buffers (copies in, nsteps psc_step, copies out)"""
         h = _cols(host_cols)
         self._check(lib().psc_step_host(self._h, _stream(stream), int(n), C.byref(h), hE.data_ptr(),
                                         hB.data_ptr(), None if hJ is None else hJ.data_ptr(),
