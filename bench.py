@@ -38,7 +38,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "particle-updates/sec per full PIC step"
+# BASELINE.json's metric string; its second half is the `roofline` object of the line
+METRIC = "particle-updates/sec per full PIC step on 1 B200; push+deposit HBM GB/s vs peak"
 UNIT = "particle-updates/s"
 WORKLOADS = {
     1: "config1: 2-d yz thermal plasma 1x64x64, 16 ppc/species, order 1",
