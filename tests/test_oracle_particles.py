@@ -436,3 +436,100 @@ def test_energy_drift_bounded_config1_1000_steps():
     g1 = orc.div_minus(E) - orc.rho(cols[0], cols[1], cols[2], cols[6])
     assert np.abs(g1 - g0).max() < 1e-12
     assert np.abs(orc.div_plus(B)).max() < 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# diagnostics: energies and rho on nodes -- pinned directly
+
+def test_energy_closed_forms():
+    """orc_energy against closed forms that separate every factor: one particle of known u, w,
+    m_s gives w m_s (gamma - 1) exactly; uniform E / B give 1/2 |E|^2 V and 1/2 |B|^2 V; a
+    two-species list fails if m_s, the weight w = qw / q_s or the -1 of (gamma - 1) is dropped."""
+    n, dx = (3, 4, 5), (0.5, 1.25, 2.0)
+    q, m = [-1.0, 2.0], [1.0, 7.0]
+    orc = Oracle(n, dx, 0.1, 1, q, m)
+    V = np.prod([n[d] * dx[d] for d in range(3)])
+    Z = orc.zeros_field()
+    # one particle, species 1 (q = 2, m = 7), weight w = 3  =>  qw = 6
+    u = np.array([[0.3], [-1.2], [2.0]])
+    g = np.sqrt(1.0 + (u ** 2).sum())
+    en = orc.energy(Z, Z, _c(u[0]), _c(u[1]), _c(u[2]), _c(np.array([6.0])), np.array([1], dtype=np.int32))
+    assert en[0] == 0.0 and en[1] == 0.0
+    assert abs(en[2] - 3.0 * 7.0 * (g - 1.0)) < 1e-13 * en[2]
+    # a particle at rest carries no kinetic energy (gamma - 1, not gamma)
+    z1 = _c(np.zeros(1))
+    assert orc.energy(Z, Z, z1, z1, z1, _c(np.array([6.0])), np.array([1], dtype=np.int32))[2] == 0.0
+    # uniform fields: 1/2 |E|^2 V, 1/2 |B|^2 V, each in its own slot
+    E, B = _uniform_fields(orc, (0.3, -0.4, 1.2), (2.0, 0.5, -0.25))
+    en = orc.energy(E, B, z1[:0], z1[:0], z1[:0], z1[:0], np.zeros(0, dtype=np.int32))
+    assert abs(en[0] - 0.5 * (0.09 + 0.16 + 1.44) * V) < 1e-12 * V
+    assert abs(en[1] - 0.5 * (4.0 + 0.25 + 0.0625) * V) < 1e-12 * V
+    assert en[2] == 0.0
+    # a single non-zero field value: E^2 dV / 2 with dV = dx dy dz (not V, not 1)
+    E1 = orc.zeros_field()
+    E1[1, 2, 3, 1] = 3.0
+    assert abs(orc.energy(E1, Z, z1[:0], z1[:0], z1[:0], z1[:0], np.zeros(0, dtype=np.int32))[0]
+               - 0.5 * 9.0 * np.prod(dx)) < 1e-13
+    # two species, different weights: sum_p (qw_p / q_s) m_s (gamma_p - 1), term by term in numpy
+    rng = np.random.default_rng(11)
+    npart = 50
+    sp = (np.arange(npart) % 2).astype(np.int32)
+    w = 0.5 + rng.random(npart)
+    qw = _c(np.where(sp == 0, q[0], q[1]) * w)
+    uu = [_c(rng.standard_normal(npart) * 1.5) for _ in range(3)]
+    gam = np.sqrt(1.0 + uu[0] ** 2 + uu[1] ** 2 + uu[2] ** 2)
+    want = (w * np.where(sp == 0, m[0], m[1]) * (gam - 1.0)).sum()
+    got = orc.energy(Z, Z, *uu, qw, sp)[2]
+    assert abs(got - want) < 1e-12 * want
+    # non-relativistic limit: w m u^2 / 2
+    us = _c(np.array([1e-4]))
+    en = orc.energy(Z, Z, us, z1, z1, _c(np.array([-2.0])), np.array([0], dtype=np.int32))
+    assert abs(en[2] - 2.0 * 1.0 * 0.5e-8) < 1e-8 * en[2]
+
+
+@pytest.mark.parametrize("order,n", [(1, (5, 4, 6)), (1, (1, 6, 5)), (2, (6, 6, 7)), (2, (1, 7, 6))])
+@pytest.mark.parametrize("npart", [1, 8])
+def test_rho_equals_brute_force(order, n, npart):
+    """orc_rho (stencil form) == the definition: b1 / b2 of the minimum-image distance to EVERY node
+    (Eq. 29-31), on 1-8 particles incl. positions next to the periodic seam; total
+    charge sum rho dV = sum qw; a particle sitting on a node puts the closed-form weight there."""
+    dx = (1.0, 0.9, 1.2)
+    rng = np.random.default_rng(17 * order + npart + n[0])
+    orc = Oracle(n, dx, 0.2, order, [-1.0, 1.0], [1.0, 4.0])
+    bf = BruteForce(n, dx, 0.2, order, [-1.0, 1.0], [1.0, 4.0])
+    pos, _, qw, _ = _small_plasma(rng, n, dx, npart, 0.1)
+    for d in range(3):                       # first particle hugs the upper seam, last the lower
+        pos[d][0] = n[d] * dx[d] * (1.0 - 1e-9)
+        pos[d][-1] = n[d] * dx[d] * 1e-9 if npart > 1 else pos[d][-1]
+    got = orc.rho(*pos, qw)
+    want = bf.rho(np.stack(pos, axis=1), qw)
+    assert np.abs(got - want).max() < 1e-13 * np.abs(want).max()
+    assert abs(got.sum() * np.prod(dx) - qw.sum()) < 1e-13 * np.abs(qw).sum()
+    # one particle exactly on node (i,j,k): weight 1 (b1) or 3/4 per active direction (b2)
+    node = [min(2, n[d] - 1) for d in range(3)]
+    p1 = [_c(np.array([node[d] * dx[d]])) for d in range(3)]
+    r1 = orc.rho(*p1, _c(np.array([2.5])))
+    nact = sum(1 for d in range(3) if n[d] > 1)
+    w0 = 1.0 if order == 1 else 0.75 ** nact
+    assert abs(r1[node[2], node[1], node[0]] - 2.5 / np.prod(dx) * w0) < 1e-13
+    if order == 1:
+        assert np.count_nonzero(r1) == 1
+
+
+def test_wrap_lands_on_upper_edge():
+    """A14: a position that rounds to exactly L after the periodic shift is stored as 0, so that
+    floor(x / dx) stays in [0, n).  x0 = 0 moving down by less than half an ulp of L gives
+    x1 + L == L in fp64."""
+    n, dx = (1, 8, 8), (1.0, 1.0, 1.0)
+    orc = Oracle(n, dx, 0.3, 1, [-1.0], [1.0])
+    Z = orc.zeros_field()
+    J = orc.zeros_field()
+    x = _c(np.array([0.0])); y = _c(np.array([0.0])); z = _c(np.array([3.5]))
+    ux = _c(np.zeros(1)); uy = _c(np.array([-1e-18])); uz = _c(np.array([1e-18]))
+    orc.push_particles(Z, Z, J, x, y, z, ux, uy, uz, _c(np.array([-1.0])), np.zeros(1, dtype=np.int32))
+    assert y[0] == 0.0 and 0.0 <= z[0] < 8.0 and z[0] == 3.5
+    # and the ordinary cases on both sides of the seam
+    y[:] = 0.1; uy[:] = -2.0; z[:] = 7.9; uz[:] = 2.0
+    orc.push_particles(Z, Z, J, x, y, z, ux, uy, uz, _c(np.array([-1.0])), np.zeros(1, dtype=np.int32))
+    g = np.sqrt(1 + 8.0)
+    assert abs(y[0] - (0.1 - 0.3 * 2.0 / g + 8.0)) < 1e-14 and abs(z[0] - (7.9 + 0.3 * 2.0 / g - 8.0)) < 1e-14
