@@ -268,8 +268,6 @@ def run_psc(args):
     t_gen = time.perf_counter() - t_gen
     psc = sim.psc
     psc.set_option("profile", 1)
-    if args.variant:
-        psc.set_option("push_variant", args.variant)
 
     # ---- device-resident: W warm-up steps, K timed steps ---------------------------------------
     for _ in range(args.warmup):
@@ -405,7 +403,6 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick-cpu", action="store_true")
-    ap.add_argument("--variant", type=int, default=0, help="kernel variant for experiments (psc_set_option push_variant)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "psc":
         args.warmup = 3  # timing rule: at least 3 warm-up steps

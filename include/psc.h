@@ -23,13 +23,19 @@
  * derivative, its coordinate is carried but never advanced.
  *
  * Particle store ("struct of arrays", fp32).  The caller hands over ABSOLUTE
- * positions in [0, n[d]*dx[d]).  Absolute fp32 coordinates have an ulp of up to 6e-5 cells on a
- * 1024-cell axis, which is not enough to keep the deposited current within 1e-5 of the fp64
- * scheme over several steps, so the first psc_particles_sort converts the position columns IN
- * PLACE to the internal form: in-cell offsets in [0,1) (units of cells) plus one int32 cell key per
- * particle kept in the workspace (psc_particles_keys).  The columns stay in internal form until
- * psc_particles_export converts them back to absolute coordinates (psc_step_host does so before
- * copying out).  psc_particles_form tells which form the current columns are in.
+ * positions in [0, n[d]*dx[d]) as n dense entries per column.  Absolute fp32 coordinates have an
+ * ulp of up to 6e-5 cells on a 1024-cell axis, which is not enough to keep the deposited current
+ * within 1e-5 of the fp64 scheme over several steps, so the first psc_particles_sort moves the
+ * particles into the INTERNAL form, the "cell store": positions become in-cell offsets in [0,1)
+ * (units of cells), and the particles of cell k (key order of the sort) occupy the slots
+ * [base[k], base[k] + count[k]) of the other column set, where base[k] is a multiple of 32 and
+ * leaves every cell spare room -- which is why every column must be psc_particle_capacity(n)
+ * entries long, not n.  A push updates particles that stay in their cell in place and hands the
+ * others over through per-cell exchange rows in the workspace (see psc_push_particles), so
+ * between two pushes some particles live outside the columns.  psc_particles_gather returns a
+ * dense copy of everything (offsets + cell keys, or absolute positions) without changing the
+ * state; psc_particles_export converts the store back to n dense absolute entries
+ * (psc_step_host does so before copying out).  psc_particles_form tells which form is current.
  *
  * Field layout: each of E, B, J is float[3][ez][ey][ex] with ex = n[0] + 2*g (1 if n[0] == 1)
  * etc., x fastest; interior cell i is stored at i + g.  Yee staggering (PAPER.md:141-143,
@@ -62,11 +68,15 @@ extern "C" {
 #define PSC_J 2
 
 /* sticky device flags (psc_status) */
-#define PSC_F_OOB 1u            /* a particle position outside [0, n*dx) was seen by the sort */
-#define PSC_F_MOVED_GT_1CELL 2u /* reserved: a move of more than one cell cannot occur,
-                                   psc_create enforces dt <= dx/2 and |v| < c, so |move| < 1/2 cell;
-                                   non-finite momenta raise PSC_F_NAN instead */
-#define PSC_F_NAN 4u            /* a non-finite position or momentum was produced */
+#define PSC_F_OOB 1u      /* a particle position outside [0, n*dx) was seen by the sort (the particle
+                             is filed under the nearest edge cell) */
+#define PSC_F_NAN 4u      /* a non-finite momentum was produced */
+#define PSC_F_SPECIES 8u  /* a species index outside [0, n_species) was seen by the sort (the
+                             particle is treated as species 0) */
+#define PSC_F_OVERFLOW 32u /* a particle found no room although the columns / workspace have the
+                             sizes psc_particle_capacity / psc_workspace_bytes ask for: lost */
+/* (a move of more than one cell, cannot occur: psc_create enforces dt <= dx/2 and
+ * |v| < c, so |move| < 1/2 cell; non-finite momenta raise PSC_F_NAN.) */
 
 #define PSC_MAX_SPECIES 8
 #define PSC_GHOST 2
@@ -88,9 +98,10 @@ typedef struct {
                         must divide n[d]; 1 along invariant directions */
 } psc_params;
 
-/* One set of particle columns (structure of arrays), each of length >= n.
- * `id` may be NULL in both sets (then no id is carried).  In a 2-d (yz) run `x`, the coordinate
- * along the invariant direction, may be NULL in both sets (then it is not carried either). */
+/* One set of particle columns (structure of arrays), each of `capacity`
+ * entries (psc_bind_particles).  `id` may be NULL in both sets (then no id is carried).  In a 2-d
+ * (yz) run `x`, the coordinate along the invariant direction, may be NULL in both sets (then it
+ * is not carried either). */
 typedef struct {
   float *x, *y, *z;    /* positions x^{n+1/2}: absolute, or in-cell offsets (internal form) */
   float *ux, *uy, *uz; /* u^n = p/(m c) */
@@ -104,7 +115,8 @@ int psc_create(const psc_params *params, psc_ctx **out);
 void psc_destroy(psc_ctx *ctx);
 
 /* Scratch the caller must provide for up to max_particles particles (sort keys, permutation,
- * histograms, scan temporaries).  Host only. */
+ * histograms, scan temporaries, the two exchange buffers of 32 records per cell, the spill
+ * list).  Host only. */
 size_t psc_workspace_bytes(const psc_ctx *ctx, int64_t max_particles);
 /* ws must be 256-byte aligned (PSC_ERR_ALIGN) and at least psc_workspace_bytes large. */
 int psc_bind_workspace(psc_ctx *ctx, void *ws, size_t bytes);
@@ -115,32 +127,42 @@ int psc_bind_fields(psc_ctx *ctx, float *E, float *B, float *J);
 /* Number of floats in one of E/B/J (3 * ex * ey * ez) and the extents; host only. */
 int64_t psc_field_elems(const psc_ctx *ctx, int32_t ext[3]);
 
-/* `primary` holds the n particles; `secondary` is a second buffer set of the same shapes used by
- * the out-of-place reorder.  Binding marks the particle list as unsorted. */
-int psc_bind_particles(psc_ctx *ctx, int64_t n, const psc_particle_cols *primary,
+/* Entries every particle column must have for n particles: n + n/8 + 48 per cell, rounded up to a
+ * multiple of 32 -- every cell of the store gets an eighth of spare room (at least 16 slots) and
+ * starts on a 128-byte boundary.  Host only. */
+int64_t psc_particle_capacity(const psc_ctx *ctx, int64_t n);
+
+/* `primary` holds the n particles (absolute positions, entries [0, n)); `secondary` is a second
+ * buffer set of the same shapes the sort, the export and a re-layout write into.  Every column
+ * of both sets has `capacity` >= psc_particle_capacity(n) entries (PSC_ERR_WORKSPACE) and is
+ * 16-byte aligned (PSC_ERR_ALIGN).  Binding marks the particle list as unsorted. */
+int psc_bind_particles(psc_ctx *ctx, int64_t n, int64_t capacity, const psc_particle_cols *primary,
                        const psc_particle_cols *secondary);
 
 /* Cell-key counting sort.  key = block-major, cell-minor; stable (ascending
- * input index inside a key).  Afterwards the CURRENT column set (psc_particles_current) holds
- * the particles in sorted order and in internal form; the two sets swap roles.  Arbitrary input
- * order is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))); from a
- * list in internal form (sorted, or advanced by psc_push_particles) they come from the slot's
- * cell and, for the particles that left it, the one-byte direction code the push recorded.
- * psc_sort_result describes this call's permutation.  psc_step does NOT run this full sort in
- * the steady state: see psc_step. */
+ * input index inside a key).  Afterwards the particles are in the internal form (the cell store
+ * above) in sorted order: cell after cell, inside a cell in input order.  Arbitrary input order
+ * is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))) and the result
+ * is written to the other column set (the two sets swap roles); from the internal form (sorted,
+ * or advanced by psc_push_particles) the input order is the dense order of psc_particles_gather
+ * and the keys are the cells the particles are filed under.  psc_sort_result describes this
+ * call's permutation.  Synchronises `stream` (it reads the layout statistics back).  psc_step
+ * does NOT run this sort in the steady state: see psc_step. */
 int psc_particles_sort(psc_ctx *ctx, void *stream);
 
 /* The particle loop of Fig. 8 in one pass over the particles
  * (PAPER.md:603): zero J; per particle gather E,B at x^{n+1/2} (Eq. 11), Boris push
  * p^n -> p^{n+1} (Eq. 27-28), x^{n+1/2} -> x^{n+3/2} (Eq. 26), charge-conserving deposit of
- * j^{n+1}, periodic wrap (on the integer cell index).  Requires a sorted list
- * in internal form, i.e. psc_particles_sort directly before (PSC_ERR_NOT_SORTED).  Out of
- * place: the advanced particles are written to the OTHER column set, which becomes the current
- * one (psc_particles_current).  Every cell's particles are written back into that cell's
- * segment of the list, those that stay in the cell first, those that left it (a particle moves
- * at most one cell per direction and step) behind them: the list is then no longer
- * sorted, psc_particles_keys tells the cell of every particle.
- * J ghosts are NOT folded on return (psc_exchange_j). */
+ * j^{n+1}, periodic wrap (on the integer cell index).  Requires the internal
+ * form (PSC_ERR_NOT_SORTED otherwise).  In place: a particle that stays in its cell is
+ * rewritten where it is (positions and momenta only; q*w, species, id are not touched); a particle
+ * that leaves (at most one cell per direction and step) is written as a 32-byte
+ * record, tagged with the direction code of its move, into the exchange row of its source cell
+ * and is picked up from there by the next psc_push_particles of its destination cell, which
+ * files it into a free slot ("reorder on load").  An exchange row holds 32 records
+ * and a cell has finite capacity: what does not fit goes to a spill list, and the next
+ * psc_push_particles / psc_step first lays the store out again (on the device, no host round
+ * trip).  J ghosts are NOT folded on return (psc_exchange_j). */
 int psc_push_particles(psc_ctx *ctx, void *stream);
 
 /* FDTD (Eq. 17-18): which == PSC_B: B -= frac*dt*curl+ E;
@@ -157,12 +179,10 @@ int psc_fill_ghosts(psc_ctx *ctx, int which, void *stream);
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
  * u^{n+1}.  Same fields and the same set of particles (up to the rounding of the atomically
- * summed J) as the calls above in that order.  From the second step on the sort works on cells
- * and cell-leavers only: it builds new cell offsets and, per cell, the list of
- * arriving particles from the 9 / 27 direction classes the previous push recorded; the particle
- * loop loads a cell's stayers as one run and its arrivals through that list (reorder on load),
- * so every particle column is read once and written once per step.  Inside a cell the order is
- * then "stayers, arrivals" instead of the stable order psc_particles_sort gives. */
+ * summed J) as the calls above in that order.  Only the first step sorts:
+ * afterwards the store keeps itself ordered by cell (see psc_push_particles), so a steady-state
+ * step reads every particle once and writes its positions and momenta once.  Inside a cell the
+ * order is then arbitrary instead of the stable order psc_particles_sort gives. */
 int psc_step(psc_ctx *ctx, void *stream);
 
 /* End-to-end form with HOST buffers: copies the host particle columns (n particles) and host
@@ -175,22 +195,31 @@ int psc_step_host(psc_ctx *ctx, void *stream, int64_t n, const psc_particle_cols
 /* Inspection of the last psc_particles_sort.  Device pointers into the workspace, valid until
  * the next sort or push:
  * cell_idx[n] (cell of input particle a, natural (k*ny+j)*nx+i; computed on `stream` by this
- * call), perm[n] (sorted slot s holds input particle perm[s]), cell_offsets[n_keys+1]
- * (exclusive scan of the key histogram). */
+ * call), perm[n] (sorted position s holds input particle perm[s]), cell_offsets[n_keys+1]
+ * (exclusive scan of the key histogram: dense positions, not slots of the store). */
 int psc_sort_result(psc_ctx *ctx, void *stream, const int32_t **cell_idx, const int32_t **perm,
                     const int32_t **cell_offsets, int64_t *n_keys);
-/* The column set that currently holds the particles (positions in the form psc_particles_form
- * reports). */
+/* The column set that currently holds the particles: n dense absolute entries
+ * (psc_particles_form == 0), or the cell store (== 1: use psc_particles_gather to read it). */
 int psc_particles_current(const psc_ctx *ctx, psc_particle_cols *out);
-/* 0: absolute positions, 1: internal form (in-cell offsets + keys). */
+/* 0: absolute positions, 1: internal form (cell store). */
 int psc_particles_form(const psc_ctx *ctx);
-/* Internal form only: key[n] of the current particles (cell key as defined by the sort; the cell
- * a particle's offset refers to), computed on `stream` by this call from the cell offsets and
- * the leavers' direction codes.  Device pointer into the workspace, valid until the next call. */
-int psc_particles_keys(psc_ctx *ctx, void *stream, const int32_t **key);
-/* Converts the current columns back to absolute positions x = (cell + offset) * dx, in place
- * (one fp32 rounding).  The list counts as unsorted afterwards.  No-op on absolute columns. */
+/* Internal form only: writes a dense copy of all n particles into the caller's device columns
+ * `dst` (each >= n entries; x / id may be NULL) without changing any state: cell after cell in
+ * key order, a cell's resident particles first, then the records waiting in its exchange row.
+ * absolute == 0: positions are in-cell offsets and key[i] (device, >= n entries, may be NULL) is
+ * the sort key of the cell they refer to; absolute != 0: x = (cell + offset) * dx, formed in fp64
+ * and rounded once.  Entries of a sorted store come out in sorted order. */
+int psc_particles_gather(psc_ctx *ctx, void *stream, const psc_particle_cols *dst, int32_t *key,
+                         int absolute);
+/* Converts the store back to n dense absolute entries (as psc_particles_gather, into the other
+ * column set, which becomes the current one).  The list counts as unsorted afterwards.  No-op on
+ * absolute columns. */
 int psc_particles_export(psc_ctx *ctx, void *stream);
+/* Synchronises `stream`; info[0] = largest cell count at the last layout, [1] = slots of the
+ * store in use, [2] = re-layouts since psc_create, [3] = particles spilled by the last push,
+ * [4] = slots of the per-warp cell image of the particle kernels.  Host array. */
+int psc_store_info(psc_ctx *ctx, void *stream, int64_t info[8]);
 /* Synchronises `stream`, returns and keeps the sticky flags. */
 int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);
 /* Kernels and memsets/copies this context has enqueued so far (host counter). */
@@ -202,8 +231,9 @@ int psc_last_cuda_error(const psc_ctx *ctx);
  * event ring is drained with one cudaEventSynchronize).  psc_profile synchronises `stream`, adds
  * the elapsed milliseconds of every completed bracket to ms[PSC_PH_COUNT] and the number of
  * brackets to count[PSC_PH_COUNT] (host arrays), and resets the accumulators.  PSC_PH_SORT spans
- * the whole psc_particles_sort (PSC_PH_SORT_* are its parts); PSC_PH_PUSH is the fused
- * gather-push-deposit kernel launch alone. */
+ * the whole psc_particles_sort, or inside psc_step the (normally empty) re-layout launches
+ * (PSC_PH_SORT_* are its parts); PSC_PH_PUSH is the fused gather-push-deposit kernel launch
+ * alone. */
 #define PSC_PH_SORT 0
 #define PSC_PH_PUSH 1
 #define PSC_PH_J_ZERO 2
@@ -217,9 +247,7 @@ int psc_last_cuda_error(const psc_ctx *ctx);
 #define PSC_PH_COUNT 16
 int psc_profile(psc_ctx *ctx, void *stream, double *ms, int64_t *count);
 /* Host-side switches: "profile" (0/1: per-phase event timing), "clear_flags" (reset the sticky
- * device flags), and for experiments "push_variant" (0 default; 1: 2-d default tile at 6 blocks
- * per SM; 2: run-time tile geometry) and "threads" (threads per block of the particle kernels,
- * multiple of 32, 0 = default).  Unknown names return PSC_ERR_INVALID_ARG. */
+ * device flags).  Unknown names return PSC_ERR_INVALID_ARG. */
 int psc_set_option(psc_ctx *ctx, const char *name, int64_t value);
 const char *psc_strerror(int code);
 const char *psc_version(void);

@@ -14,7 +14,7 @@ from . import build as _build
 
 PSC_OK = 0
 PSC_E, PSC_B, PSC_J = 0, 1, 2
-PSC_F_OOB, PSC_F_MOVED_GT_1CELL, PSC_F_NAN = 1, 2, 4
+PSC_F_OOB, PSC_F_NAN, PSC_F_SPECIES, PSC_F_OVERFLOW = 1, 4, 8, 32
 PSC_GHOST = 2
 PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
           "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9}
@@ -22,10 +22,10 @@ PSC_PH_COUNT = 16
 
 EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
-    "psc_field_elems", "psc_bind_particles", "psc_particles_sort", "psc_push_particles",
-    "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step", "psc_step_host",
-    "psc_sort_result", "psc_particles_current", "psc_particles_form", "psc_particles_keys",
-    "psc_particles_export", "psc_status", "psc_launch_count",
+    "psc_field_elems", "psc_particle_capacity", "psc_bind_particles", "psc_particles_sort",
+    "psc_push_particles", "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step",
+    "psc_step_host", "psc_sort_result", "psc_particles_current", "psc_particles_form",
+    "psc_particles_gather", "psc_particles_export", "psc_store_info", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
 ]
 
@@ -77,7 +77,9 @@ def lib():
         L.psc_bind_fields.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.psc_field_elems.argtypes = [C.c_void_p, C.POINTER(C.c_int32 * 3)]
         L.psc_field_elems.restype = C.c_int64
-        L.psc_bind_particles.argtypes = [C.c_void_p, C.c_int64, C.POINTER(PscCols), C.POINTER(PscCols)]
+        L.psc_particle_capacity.argtypes = [C.c_void_p, C.c_int64]
+        L.psc_particle_capacity.restype = C.c_int64
+        L.psc_bind_particles.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.POINTER(PscCols), C.POINTER(PscCols)]
         for f in ("psc_particles_sort", "psc_push_particles", "psc_exchange_j", "psc_step"):
             getattr(L, f).argtypes = [C.c_void_p, C.c_void_p]
         L.psc_push_fields.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_void_p]
@@ -88,7 +90,8 @@ def lib():
                                       C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                       C.POINTER(C.c_int64)]
         L.psc_particles_form.argtypes = [C.c_void_p]
-        L.psc_particles_keys.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.psc_particles_gather.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(PscCols), C.c_void_p, C.c_int]
+        L.psc_store_info.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
         L.psc_particles_export.argtypes = [C.c_void_p, C.c_void_p]
         L.psc_particles_current.argtypes = [C.c_void_p, C.POINTER(PscCols)]
         L.psc_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32)]
@@ -182,10 +185,14 @@ class Psc:
         self._check(lib().psc_bind_fields(self._h, E.data_ptr(), B.data_ptr(), J.data_ptr()),
                     "psc_bind_fields")
 
-    def bind_particles(self, n, primary, secondary):
+    def particle_capacity(self, n):
+        """entries every particle column needs for n particles (the cell store's spare room)"""
+        return int(lib().psc_particle_capacity(self._h, int(n)))
+
+    def bind_particles(self, n, capacity, primary, secondary):
         self._keep["particles"] = (primary, secondary)
         a, b = _cols(primary), _cols(secondary)
-        self._check(lib().psc_bind_particles(self._h, int(n), C.byref(a), C.byref(b)),
+        self._check(lib().psc_bind_particles(self._h, int(n), int(capacity), C.byref(a), C.byref(b)),
                     "psc_bind_particles")
 
     # -- the hot path ----------------------------------------------------------------------------
@@ -234,11 +241,20 @@ class Psc:
     def particles_form(self):
         return int(lib().psc_particles_form(self._h))
 
-    def particles_keys(self, stream=None):
-        """raw device pointer of the current particles' cell keys (internal form only)"""
-        k = C.c_void_p()
-        self._check(lib().psc_particles_keys(self._h, _stream(stream), C.byref(k)), "psc_particles_keys")
-        return k.value
+    def particles_gather(self, dst, key=None, absolute=False, stream=None):
+        """psc_particles_gather: dense copy of the cell store into the caller's columns `dst`
+        (+ cell keys), state unchanged"""
+        d = _cols(dst)
+        self._check(lib().psc_particles_gather(self._h, _stream(stream), C.byref(d),
+                                               None if key is None else key.data_ptr(),
+                                               1 if absolute else 0), "psc_particles_gather")
+
+    def store_info(self, stream=None):
+        """{max_count, slots, relayouts, spilled, image_slots} of the cell store (synchronises)"""
+        a = (C.c_int64 * 8)()
+        self._check(lib().psc_store_info(self._h, _stream(stream), a), "psc_store_info")
+        return {"max_count": int(a[0]), "slots": int(a[1]), "relayouts": int(a[2]),
+                "spilled": int(a[3]), "image_slots": int(a[4])}
 
     def particles_export(self, stream=None):
         self._check(lib().psc_particles_export(self._h, _stream(stream)), "psc_particles_export")

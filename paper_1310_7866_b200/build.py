@@ -18,7 +18,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libpsc_b200.so")
 SOURCES = ["api.cu", "fields.cu", "sort.cu", "push1.cu", "push2.cu"]
-HEADERS = ["psc_internal.cuh", "push_common.cuh"]
+HEADERS = ["psc_internal.cuh", "push_common.cuh", "store.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -53,7 +53,7 @@ void psc_prof_end(psc_ctx *c, int ph, cudaStream_t s) {
 
 extern "C" {
 
-const char *psc_version(void) { return "psc-b200 0.1 (sm_100a)"; }
+const char *psc_version(void) { return "psc-b200 0.2 (sm_100a)"; }
 
 const char *psc_strerror(int code) {
   switch (code) {
@@ -120,9 +120,8 @@ int psc_create(const psc_params *p, psc_ctx **out) {
     gd.bs[d] = bs;
     gd.nb[d] = p->n[d] / bs;
   }
-  // 32-bit indexing: 3 field components, and the per-cell direction table of the index sort
-  // (27 entries per cell)
-  if (tot * 3 > 0x7fffffffLL || nk * 27 > 0x7fffffffLL) {
+  // 32-bit indexing: 3 field components, and the exchange rows (32 records per cell)
+  if (tot * 3 > 0x7fffffffLL || nk * PSC_XCAP > 0x7fffffffLL) {
     free(c);
     return PSC_ERR_INVALID_ARG;
   }
@@ -150,14 +149,14 @@ int psc_create(const psc_params *p, psc_ctx **out) {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess ||
       cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-      cudaMalloc((void **)&c->d_flags, 64) != cudaSuccess ||
-      cudaMemset(c->d_flags, 0, 64) != cudaSuccess) {
+      cudaMalloc((void **)&c->d_flags, PSC_DW_COUNT * 4) != cudaSuccess ||
+      cudaMemset(c->d_flags, 0, PSC_DW_COUNT * 4) != cudaSuccess) {
     c->last_err = (int)cudaGetLastError();
     if (c->d_flags) cudaFree(c->d_flags);
     free(c);
     return PSC_ERR_CUDA;  // no device: there is no CPU fallback
   }
-  c->opt_threads = 0;
+  c->bufC = 64;
   *out = c;
   return PSC_OK;
 }
@@ -171,6 +170,7 @@ void psc_destroy(psc_ctx *c) {
         cudaEventDestroy(c->prof.ev[ph][i][1]);
       }
   if (c->d_flags) cudaFree(c->d_flags);
+  if (c->rho) cudaFree(c->rho);
   free(c);
 }
 
@@ -182,7 +182,7 @@ size_t psc_workspace_bytes(const psc_ctx *c, int64_t max_particles) {
 int psc_bind_workspace(psc_ctx *c, void *ws, size_t bytes) {
   if (!c || !ws) return PSC_ERR_INVALID_ARG;
   if (((uintptr_t)ws) & 255) return PSC_ERR_ALIGN;
-  if (c->have_particles && c->form == PSC_FORM_REL) return PSC_ERR_INVALID_ARG;  // keys live in ws
+  if (c->have_particles && c->form == PSC_FORM_REL) return PSC_ERR_INVALID_ARG;  // the store's tables live in ws
   c->ws = ws;
   c->ws_bytes = bytes;
   c->ws_cap = -1;
@@ -213,11 +213,19 @@ int psc_bind_fields(psc_ctx *c, float *E, float *B, float *J) {
   return PSC_OK;
 }
 
-int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const psc_particle_cols *b) {
-  if (!c || !a || !b || n < 0 || n > 0x7fffff00LL) return PSC_ERR_INVALID_ARG;
+int64_t psc_particle_capacity(const psc_ctx *c, int64_t n) {
+  if (!c || n < 0) return 0;
+  return psc_store_capacity(c, n);
+}
+
+int psc_bind_particles(psc_ctx *c, int64_t n, int64_t capacity, const psc_particle_cols *a,
+                       const psc_particle_cols *b) {
+  if (!c || !a || !b || n < 0 || n > 0x6fffff00LL) return PSC_ERR_INVALID_ARG;
   if (!cols_complete(c, a) || !cols_complete(c, b)) return PSC_ERR_INVALID_ARG;
   if ((a->id == nullptr) != (b->id == nullptr)) return PSC_ERR_INVALID_ARG;
   if ((a->x == nullptr) != (b->x == nullptr)) return PSC_ERR_INVALID_ARG;
+  if (capacity < psc_store_capacity(c, n)) return PSC_ERR_WORKSPACE;
+  if (capacity > 0x7fffff00LL) return PSC_ERR_INVALID_ARG;  // 32-bit slot indices
   const void *ptrs[] = {a->x, a->y, a->z, a->ux, a->uy, a->uz, a->qw, a->species, a->id,
                         b->x, b->y, b->z, b->ux, b->uy, b->uz, b->qw, b->species, b->id};
   for (const void *p : ptrs)
@@ -226,10 +234,11 @@ int psc_bind_particles(psc_ctx *c, int64_t n, const psc_particle_cols *a, const 
   c->cols[1] = to_cols(b);
   c->cur = 0;
   c->np = n;
+  c->capacity = capacity;
   c->have_particles = 1;
   c->state = PSC_STATE_UNSORTED;
   c->form = PSC_FORM_ABS;
-  c->ocur = 0;
+  c->xcur = 0;
   c->have_sort_result = 0;
   if (c->ws) {
     if (c->ws_bytes < psc_workspace_bytes(c, n)) {
@@ -251,36 +260,33 @@ int psc_particles_sort(psc_ctx *c, void *stream) {
   return psc_sort_general(c, s);  // the physically sorted, stable list this call promises
 }
 
-// the sort as psc_step uses it: after a push only the index sort runs, and the physical reorder
-// is left to the next push's load
+// the sort as psc_step uses it: a store keeps itself ordered by cell; only a
+// push that spilled makes the device lay it out again
 static int sort_lazy(psc_ctx *c, cudaStream_t s) {
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
   ProfScope ps(c, PSC_PH_SORT, s);
-  if (c->state == PSC_STATE_PUSHED) return psc_sort_index(c, s);
-  if (c->state == PSC_STATE_INDEXED || c->state == PSC_STATE_SORTED) return PSC_OK;
+  if (c->state == PSC_STATE_STORE) return psc_store_relayout_if_spilled(c, s);
   return psc_sort_general(c, s);
 }
 
 int psc_push_particles(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
-  if ((c->state != PSC_STATE_SORTED && c->state != PSC_STATE_INDEXED) || c->form != PSC_FORM_REL)
-    return PSC_ERR_NOT_SORTED;
+  if (c->state != PSC_STATE_STORE || c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
   cudaStream_t s = (cudaStream_t)stream;
+  if (!c->in_step) {  // (psc_step has just done this)
+    ProfScope ps(c, PSC_PH_SORT, s);
+    const int rc = psc_store_relayout_if_spilled(c, s);
+    if (rc) return rc;
+  }
   {
     ProfScope ps(c, PSC_PH_J_ZERO, s);
     PSC_CUDA_TRY(c, cudaMemsetAsync(c->J, 0, (size_t)3 * c->gd.comp * sizeof(float), s));
     c->launches++;
   }
-  if (c->np == 0) {  // nothing to push: every cell keeps zero particles
-    PSC_CUDA_TRY(c, cudaMemsetAsync(c->dircnt, 0, (size_t)c->gd.nkeys * c->gd.nd * 4, s));
-    c->launches++;
-  } else {
-    const int rc = c->gd.order == 1 ? psc_push_order1(c, s) : psc_push_order2(c, s);
-    if (rc) return rc;
-  }
-  c->cur ^= 1;  // the kernel wrote the other column set
-  c->state = PSC_STATE_PUSHED;
+  const int rc = c->gd.order == 1 ? psc_push_order1(c, s) : psc_push_order2(c, s);
+  if (rc) return rc;
+  c->xcur ^= 1;  // the leavers' records are in the exchange the next push reads
   c->have_sort_result = 0;
   return PSC_OK;
 }
@@ -324,7 +330,10 @@ int psc_step(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if ((rc = sort_lazy(c, (cudaStream_t)stream))) return rc;
   if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^n -> B^{n+1/2}
-  if ((rc = psc_push_particles(c, stream))) return rc;            // p, x, j^{n+1}
+  c->in_step = 1;
+  rc = psc_push_particles(c, stream);                             // p, x, j^{n+1}
+  c->in_step = 0;
+  if (rc) return rc;
   if ((rc = psc_push_fields(c, PSC_B, 0.5f, stream))) return rc;  // B^{n+1/2} -> B^{n+1}
   if ((rc = psc_exchange_j(c, stream))) return rc;
   if ((rc = psc_push_fields(c, PSC_E, 1.0f, stream))) return rc;  // E^{n+1/2} -> E^{n+3/2}
@@ -384,28 +393,35 @@ int psc_sort_result(psc_ctx *c, void *stream, const int32_t **cell_idx, const in
     *cell_idx = c->cell_idx;
   }
   if (perm) *perm = c->perm;
-  if (cell_offsets) *cell_offsets = c->offs[c->ocur];
+  if (cell_offsets) *cell_offsets = c->offs_dense;
   if (n_keys) *n_keys = c->gd.nkeys;
   return PSC_OK;
 }
 
 int psc_particles_form(const psc_ctx *c) { return c ? c->form : PSC_ERR_INVALID_ARG; }
 
-int psc_particles_keys(psc_ctx *c, void *stream, const int32_t **key) {
-  if (!c || !key) return PSC_ERR_INVALID_ARG;
+int psc_particles_gather(psc_ctx *c, void *stream, const psc_particle_cols *dst, int32_t *key,
+                         int absolute) {
+  if (!c || !dst) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
   if (c->form != PSC_FORM_REL) return PSC_ERR_NOT_SORTED;
-  const int rc = psc_sort_current_keys(c, (cudaStream_t)stream);
-  if (rc) return rc;
-  *key = c->curkey;
-  return PSC_OK;
+  if (!dst->y || !dst->z || !dst->ux || !dst->uy || !dst->uz || !dst->qw || !dst->species)
+    return PSC_ERR_INVALID_ARG;
+  return psc_store_gather(c, to_cols(dst), key, absolute != 0, (cudaStream_t)stream);
 }
 
 int psc_particles_export(psc_ctx *c, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles) return PSC_ERR_NOT_BOUND;
   if (c->form == PSC_FORM_ABS) return PSC_OK;
-  return psc_particles_to_abs(c, (cudaStream_t)stream);
+  if (!c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  const int rc = psc_store_gather(c, c->cols[c->cur ^ 1], nullptr, true, (cudaStream_t)stream);
+  if (rc) return rc;
+  c->cur ^= 1;
+  c->form = PSC_FORM_ABS;
+  c->state = PSC_STATE_UNSORTED;
+  c->have_sort_result = 0;
+  return PSC_OK;
 }
 
 int psc_particles_current(const psc_ctx *c, psc_particle_cols *out) {
@@ -415,6 +431,20 @@ int psc_particles_current(const psc_ctx *c, psc_particle_cols *out) {
   out->x = d.x; out->y = d.y; out->z = d.z;
   out->ux = d.ux; out->uy = d.uy; out->uz = d.uz;
   out->qw = d.qw; out->species = d.sp; out->id = d.id;
+  return PSC_OK;
+}
+
+int psc_store_info(psc_ctx *c, void *stream, int64_t info[8]) {
+  if (!c || !info) return PSC_ERR_INVALID_ARG;
+  uint32_t dw[PSC_DW_COUNT];
+  PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  PSC_CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+  for (int i = 0; i < 8; i++) info[i] = 0;
+  info[0] = dw[PSC_DW_MAXCNT];
+  info[1] = dw[PSC_DW_SLOTS];
+  info[2] = dw[PSC_DW_RELAYOUTS];
+  info[3] = dw[PSC_DW_SPILL];
+  info[4] = c->bufC;
   return PSC_OK;
 }
 
@@ -443,9 +473,7 @@ int psc_last_cuda_error(const psc_ctx *c) { return c ? c->last_err : 0; }
 
 int psc_set_option(psc_ctx *c, const char *name, int64_t value) {
   if (!c || !name) return PSC_ERR_INVALID_ARG;
-  if (!strcmp(name, "push_variant")) c->opt_push_variant = (int)value;
-  else if (!strcmp(name, "threads")) c->opt_threads = (int)value;
-  else if (!strcmp(name, "profile")) {
+  if (!strcmp(name, "profile")) {
     Prof &pr = c->prof;
     if (value && !pr.have_events) {
       for (int ph = 0; ph < PSC_PH_COUNT; ph++)

@@ -27,6 +27,7 @@ struct GridDesc {
   int nsp;
   int nd;            // direction codes of a move: 9 (2-d) or 27 (3-d); see dir_code()
   float qmh[PSC_MAX_SPECIES];  // q_s dt / (2 m_s), the Boris h
+  int gmode;         // gather/deposit pairing (psc.h PSC_SCHEME_*)
 };
 
 struct Cols {
@@ -35,18 +36,63 @@ struct Cols {
   int32_t *id;
 };
 
-// Where the particle list is in the sort / push cycle (internal form unless UNSORTED):
-//   UNSORTED  absolute positions in arbitrary order (after bind or export)
-//   SORTED    the current column set is physically in sorted order; offs[ocur] = cell offsets
-//   PUSHED    the current set is the list a push wrote: cell k's particles of BEFORE the push in
-//             [offs[ocur][k], offs[ocur][k+1]), its stayers first (dircnt[STAY][k] of them), then
-//             its leavers, each leaver with the direction code of its move in dcode[slot];
-//             dircnt holds the per-cell code counts
-//   INDEXED   the current set is still that written list (layout offs[ocur^1]); offs[ocur] are
-//             the cell offsets of the new order, nstay / aoffs / alist say where each cell's
-//             particles are (a run of stayers + listed arrivals; reorder happens on the next
-//             load); dircnt[dc != STAY][k] now hold arrival-list bases
-enum { PSC_STATE_UNSORTED = 0, PSC_STATE_SORTED = 1, PSC_STATE_PUSHED = 2, PSC_STATE_INDEXED = 3 };
+// ---- the cell store -------------------------------------------------------
+// In the internal form the particles of cell k (key order: block-major, cell-minor)
+// are the slots [base[k], base[k] + cnt[k]) of the current column set.  base[] is fixed between
+// layouts, a multiple of 32 slots (128 bytes per column), and leaves every cell spare capacity
+// cap[k] = base[k+1] - base[k] >= cnt[k].  A push updates the particles that stay in their cell IN
+// PLACE; a particle that leaves (at most one cell per direction and step) is written
+// as a 32-byte record into the exchange rows of its SOURCE cell, tagged with the direction code of
+// its move; the next push of the destination cell collects the records aimed at it from its 8 / 26
+// neighbours' rows (reorder on load) and files them into the holes the cell's own
+// leavers left.  So no per-step sort pass exists at all; the exchange is ping-pong buffered.
+constexpr int PSC_XCAP = 32;        // exchange records per cell and step (one 32-byte code row)
+constexpr int PSC_SLOT_ALIGN = 32;  // cell segments start on multiples of 32 slots
+constexpr uint8_t PSC_XDC_NONE = 0xff;
+
+// One exchange record: the first 8 buffer columns of a particle (see StoreDesc::col), positions
+// relative to the DESTINATION cell.  2-d: {y z ux uy uz qw sp x2d}, 3-d: {x y z ux uy uz qw sp}.
+struct __align__(16) XRec {
+  uint4 a, b;
+};
+
+struct Exchange {
+  XRec *rec;      // [nkeys * PSC_XCAP]
+  uint8_t *dc;    // [nkeys * PSC_XCAP] direction codes, PSC_XDC_NONE = unused entry
+  int32_t *id;    // [nkeys * PSC_XCAP] or nullptr
+};
+
+// particles that found no room (exchange row or destination cell full): the next step re-lays
+// the store out before it pushes (sort.cu: relayout)
+struct Spill {
+  XRec *rec;
+  int32_t *key;   // destination cell
+  int32_t *id;    // or nullptr
+  int32_t *count; // device counter
+  int cap;
+};
+
+// What a particle kernel reads and writes.  Column order of the per-warp shared-memory image of
+// a cell ("buffer columns"): the DYNAMIC columns first (2-d: y z ux uy uz; 3-d: x y z ux uy uz),
+// then the STATIC ones (qw, species, [carried x of a 2-d run], [id]).
+struct StoreDesc {
+  float *col[10];
+  int ncol;        // buffer columns in use
+  int ndyn;        // 5 or 6
+  int icol_id;     // buffer column of id, or -1
+  int icol_x2d;    // buffer column of the carried invariant coordinate, or -1
+  const int32_t *base;
+  int32_t *cnt;
+  Exchange xin, xout;
+  Spill spill;
+  int C;           // slots of the per-warp cell image (multiple of 32, <= 256)
+  uint32_t *flags;
+};
+
+// Where the particle list is in the sort / push cycle:
+//   UNSORTED  absolute positions, dense [0, n), arbitrary order (after bind or export)
+//   STORE     internal form: the cell store above (after psc_particles_sort, after a push)
+enum { PSC_STATE_UNSORTED = 0, PSC_STATE_STORE = 1 };
 enum { PSC_FORM_ABS = 0, PSC_FORM_REL = 1 };
 
 // Direction code of a move by (sx, sy, sz) in {-1,0,1}^3 cells (a particle moves at
@@ -68,34 +114,47 @@ struct Prof {
   int64_t cnt[PSC_PH_COUNT];
 };
 
+// device status block (owned by the context): words
+enum {
+  PSC_DW_FLAGS = 0,    // sticky flags (psc_status)
+  PSC_DW_BIG = 1,      // big-segment counter of the general sort
+  PSC_DW_SPILL = 2,    // spill counter: != 0 => the next step re-lays the store out
+  PSC_DW_MAXCNT = 3,   // largest cell count seen by the last layout
+  PSC_DW_SLOTS = 4,    // slots used by the last layout
+  PSC_DW_RELAYOUTS = 5,  // number of re-layouts performed
+  PSC_DW_COUNT = 16
+};
+
 struct psc_ctx {
   GridDesc gd;
   Prof prof;
   float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
   float *E, *B, *J;
+  float *rho;      // owned: node charge density of psc_marder ([ext2][ext1][ext0]), lazily allocated
   Cols cols[2];
   int cur;
   int64_t np;
+  int32_t np32;    // np as the device sees it (source of an async copy)
+  int64_t capacity;  // slots per column the caller bound
   int have_particles, have_fields;
   int state;
   int form;        // PSC_FORM_ABS: absolute positions; PSC_FORM_REL: in-cell offsets
-  int ocur;        // offs[ocur]: offsets of the latest sort
-  int have_sort_result;  // 0: none; 1: key[] holds the input keys of the last general sort
+  int xcur;        // exchange[xcur] holds the leavers of the last push (read by the next one)
+  int in_step;     // psc_step is calling psc_push_particles (the re-layout check already ran)
+  int have_sort_result;  // 1: key/perm/offs_dense describe the last psc_particles_sort
+  int bufC;        // StoreDesc::C for the current layout
   // workspace carve-up (all device pointers)
   void *ws;
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
-  int32_t *key, *curkey, *perm, *cell_idx, *offs[2], *cursor, *big_list, *dircnt;
-  int32_t *alist, *aoffs, *nstay;  // index sort: arrival list, its per-cell offsets, stayers per cell
+  int32_t *key, *perm, *cell_idx, *offs_dense, *base, *cnt, *cursor, *big_list, *tot, *doffs;
   long long *pack, *packloc, *scan_tmp;
-  uint8_t *dcode;
-  uint32_t *d_flags;  // owned: 16 words; [0] sticky flags, [1] big-segment counter
+  Exchange xch[2];
+  Spill spill;
+  uint32_t *d_flags;  // owned: PSC_DW_COUNT words
   int64_t launches;
   int last_err;
   int sm_count;
-  // options
-  int opt_push_variant;  // 0: default; 1: 2-d default tile at 6 blocks/SM; 2: run-time tile geometry
-  int opt_threads;       // threads per block of the particle kernels (0: default)
 };
 
 #define PSC_CUDA_TRY(ctx, expr)                   \
@@ -118,6 +177,7 @@ struct psc_ctx {
   } while (0)
 
 static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+static inline bool psc_is3d(const GridDesc &gd) { return gd.n[0] > 1; }
 
 // api.cu: phase brackets (no-ops unless profiling is on)
 void psc_prof_begin(psc_ctx *c, int phase, cudaStream_t s);
@@ -135,12 +195,17 @@ int psc_fields_fill_ghosts(psc_ctx *c, float *F, cudaStream_t s);
 int psc_fields_fold(psc_ctx *c, float *F, cudaStream_t s);
 // sort.cu
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n);
+int64_t psc_store_capacity(const psc_ctx *c, int64_t n);
 int psc_sort_carve(psc_ctx *c, int64_t n);
-int psc_sort_general(psc_ctx *c, cudaStream_t s);      // any state -> SORTED (stable)
-int psc_sort_index(psc_ctx *c, cudaStream_t s);        // PUSHED -> INDEXED
+int psc_sort_general(psc_ctx *c, cudaStream_t s);      // any state -> STORE (stable)
+int psc_store_relayout_if_spilled(psc_ctx *c, cudaStream_t s);
 int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s);
-int psc_sort_current_keys(psc_ctx *c, cudaStream_t s);  // key[] := keys of the current particles
-int psc_particles_to_abs(psc_ctx *c, cudaStream_t s);
+// dense copy of the store (residents of every cell, then the records waiting in its exchange
+// row, then the spill list) into `dst`, keys into `key` (may be null); to_abs: positions absolute
+int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cudaStream_t s);
+StoreDesc psc_store_desc(const psc_ctx *c);
 // push1.cu / push2.cu
 int psc_push_order1(psc_ctx *c, cudaStream_t s);
 int psc_push_order2(psc_ctx *c, cudaStream_t s);
+// marder.cu
+int psc_marder_pass(psc_ctx *c, float diffusion, int iters, cudaStream_t s);

@@ -12,18 +12,17 @@
 // reduced across the warp once per cell.
 //
 // This is the single particle loop of PAPER.md:603 ("only one loop each time step that reads
-// and writes all particle data"): a cell's particles are loaded as one contiguous run (the
-// stayers of the previous step) plus a short indexed list of arrivals (reorder on load; both
-// from the index sort of sort.cu), and the advanced particles are written to the cell's segment
-// of the OTHER column set -- those that stay in the cell compacted at the front, the leavers at
-// the back with the one-byte direction code of their move; per cell the kernel writes the count
-// of each code.  The leavers' codes and the counts are all the next sort reads.
+// and writes all particle data"), over the cell store of store.cuh: a cell's resident particles
+// arrive in shared memory through one bulk asynchronous copy per column, are advanced there in
+// place and written back the same way; the few that leave go, as 32-byte records tagged with the
+// direction code of their move, into the cell's exchange row, from which the destination cell's
+// warp collects them in the NEXT push (reorder on load).  There is no sort pass between pushes.
 //
 // Positions are in the internal form (include/psc.h): in-cell offset a in [0,1) per direction;
 // the cell is implied by the segment.  The move is b = a + v dt/dx; a particle that leaves its
-// cell (b < 0 or b >= 1; at most one cell per direction) is stored with offset
-// b -/+ 1 and the direction code of the move; the index sort turns code + source cell into the
-// destination cell with the periodic wrap -- the single-GPU form of the particle exchange
+// cell (b < 0 or b >= 1; at most one cell per direction) is recorded with offset
+// b -/+ 1 and the direction code of the move; the destination's warp turns code + source cell
+// back into "mine" with the periodic wrap -- the single-GPU form of the particle exchange
 // (PAPER.md:403).  No floor(), no float->int conversion and no absolute coordinate appear here.
 //
 // The VB current is the exact flux of a b0-shaped cloud moving on the straight line
@@ -35,15 +34,15 @@
 //   W_11 = m_e m_f + del_e del_f/12;
 // in 2-d (x invariant) the in-plane weights reduce to {1-m, m} and the out-of-plane current is
 // the time average of v_x S_y S_z over the segment (A12).
-#include "push_common.cuh"
+#include "store.cuh"
 
 namespace {
 
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
-constexpr int QW = 8;      // words per entry
-constexpr int QROWS3 = 12; // rows of the queue in 3-d: the drain reuses drained slots as scratch [NV]
-constexpr int NST = 4;        // chunks in the per-warp column ring (NST - 1 in flight)
-constexpr int RING_COLS = 9;  // y z ux uy uz qw species [x] [id]
+// rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax (2-d: carried x), 2 ay, 3 az,
+// 4 ddx (2-d: v_x), 5 ddy, 6 ddz, 7 qw, 8 ux, 9 uy, 10 uz, 11 species | row index << 8, 12 id.
+// The drain reuses rows [0, NV) of a drained entry as its scratch column.
+constexpr int QROWS = 13;
 
 
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
@@ -292,9 +291,12 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
 }
 
 
-template <bool D3, class TG>
-__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg,
-                                            const GridDesc &gd, float *__restrict__ q,
+// Drains n (<= 32) queue entries starting at `start`: deposits every segment of each trajectory
+// and writes the particle's record (offsets relative to the DESTINATION cell) into its source
+// cell's exchange row.
+template <bool D3, bool XC, class TG>
+__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg, const GridDesc &gd,
+                                            const StoreDesc &sd, int kbase, float *__restrict__ q,
                                             const int *__restrict__ rel, int start, int n, int lane) {
   if (lane < n) {
     const int e = start + lane;
@@ -302,12 +304,35 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg
     const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
     const float ddx = q[4 * QCAP + e], ddy = q[5 * QCAP + e], ddz = q[6 * QCAP + e];
     const float qw = q[7 * QCAP + e];
+    const float ux = q[8 * QCAP + e], uy = q[9 * QCAP + e], uz = q[10 * QCAP + e];
+    const int spx = __float_as_int(q[11 * QCAP + e]);
+    const int id = XC ? __float_as_int(q[12 * QCAP + e]) : 0;
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
-    // 2-d: the x slots carry (unused, v_x): the out-of-plane current needs the velocity
+    // 2-d: the x slots carry (carried x, v_x): the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
     const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
     vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
                 qvx, rel, q + e, lane % (D3 ? 12 : 8));
+    // the record: new offsets relative to the destination cell
+    const float endx = D3 ? ax + ddx : 0.f, endy = ay + ddy, endz = az + ddz;
+    const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+    const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+    const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+    Part p;
+    p.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
+    p.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+    p.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+    p.ux = ux; p.uy = uy; p.uz = uz; p.qw = qw;
+    p.sp = spx & 255;
+    float w[8];
+    CellWalker<D3, XC>::to_words(w, p, D3 ? 0.f : ax);
+    const int xi = spx >> 8;
+    const int src = kbase + (lz * tg.bs[1] + ly) * tg.bs[0] + lx;
+    int dest = 0;
+    if (xi >= PSC_XCAP)
+      dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0, wrap_cell(tg.o[1] + ly + syd, gd.n[1]),
+                      wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
+    CellWalker<D3, XC>::write_record(sd, gd, src, xi, w, id, dest);
   }
   __syncwarp();
 }
@@ -335,29 +360,24 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
 // XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id)
 template <bool D3, int CBS, int THREADS, int MINB, bool XC>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
-        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
-  extern __shared__ float smem[];
+k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
+        float *__restrict__ J, int wstride) {
+  extern __shared__ __align__(128) unsigned char smraw[];
   constexpr int NV = D3 ? 12 : 8;
+  using Walker = CellWalker<D3, XC>;
   TileGeom<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  float *sF = smem;                           // [6][fvol]: Ex Ey Ez Bx By Bz
-  float *sJ = smem + 6 * tg.fvol;             // [3][jvol]
+  // per-warp areas first (128-byte aligned cell images), then the block's tiles and tables
+  Walker wk;
+  wk.init(smraw + (size_t)warp * wstride, sd, lane);
+  float *myQ = (float *)(smraw + (size_t)nwarps * wstride) + warp * (QROWS * QCAP);  // [QROWS][QCAP]
+  float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP);  // [6][fvol]
+  float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
   float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
-  int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
-  constexpr int QR = D3 ? QROWS3 : QW;        // queue rows (>= NV: drained slots serve as scratch)
-  float *sQ = (float *)(sDir + nwarps * 32);  // [warps][QR][QCAP]
-  float *myQ = sQ + warp * (QR * QCAP);
-  float *myRing = sQ + nwarps * (QR * QCAP) + warp * (NST * RING_COLS * 32);  // [NST][RING_COLS][32]
-  int *sRel = (int *)(sQ + nwarps * (QR * QCAP + NST * RING_COLS * 32));  // [12]: J points of vb_values
-  int *sIn = sRel + 12;                            // [cpb]: first input slot of each cell's run
-  int *sNs = sIn + tg.cpb;                         // [cpb]: length of that run
-  int *sA = sNs + tg.cpb;                          // [cpb + 1]: first arrival-list entry
-  int *sOut = sA + tg.cpb + 1;                     // [cpb + 1]: output segments
-  uint8_t *__restrict__ dcode = pls.dcode;
-  int *__restrict__ dircnt = pls.dircnt;
-  const int *__restrict__ alist = pls.alist;
+  int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [12]: J points of vb_values
+  int *sBase = sRel + 12;                     // [cpb + 1]: first slot of each cell
+  int *sCnt = sBase + tg.cpb + 1;             // [cpb]: particles resident in each cell
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   if (threadIdx.x < NV) {  // J points of the NV in-cell currents, relative to the cell's node
@@ -366,6 +386,11 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
                           2 * jv, 2 * jv + 1, 2 * jv + s1, 2 * jv + s1 + 1};
     const int off2[8] = {0, 1, s2, s2 + 1, jv, jv + s2, 2 * jv, 2 * jv + 1};
     sRel[threadIdx.x] = D3 ? off3[threadIdx.x] : off2[threadIdx.x & 7];
+  }
+  const int kbase = blockIdx.x * tg.cpb;
+  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
+    sBase[i] = sd.base[kbase + i];
+    if (i < tg.cpb) sCnt[i] = sd.cnt[kbase + i];
   }
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
@@ -377,21 +402,7 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
     sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
   }
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
-  const int kbase = blockIdx.x * tg.cpb;
-  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
-    const int o = pls.offs_in[kbase + i];
-    if (i < tg.cpb) {
-      sIn[i] = o;
-      sNs[i] = pls.nstay ? pls.nstay[kbase + i] : pls.offs_in[kbase + i + 1] - o;
-    }
-    sA[i] = pls.aoffs ? pls.aoffs[kbase + i] : 0;
-    sOut[i] = pls.offs_out[kbase + i];
-  }
-  sDir[warp * 32 + lane] = 0;
   __syncthreads();
-  for (int i = threadIdx.x; i < tg.cpb; i += blockDim.x)  // empty cells send nothing anywhere
-    if (sOut[i + 1] == sOut[i])
-      for (int d = 0; d < (D3 ? 27 : 9); d++) dircnt[d * gd.nkeys + kbase + i] = 0;
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   uint32_t bad = 0;
@@ -411,133 +422,35 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
-  // The warp's work is the sequence of 32-particle chunks of its cells (cells warp, warp +
-  // nwarps, ...; empty cells skipped).  Particle v of a cell is slot sIn + v of the input columns
-  // if v < sNs (the cell's stayer run), else slot alist[sA + v - sNs] (an arrival: reorder on
-  // load).  The loop is software-pipelined: the columns of chunk t+1 are loaded before chunk t is
-  // computed, and the list entries of chunk t+2 with them, so that a DRAM round trip is hidden
-  // behind one chunk of arithmetic.
-  struct It {
-    int ci, base, p1;  // cell, first particle of the chunk, particles in the cell
-    bool ok;
-    int ns, in0;       // the cell's stayer run: length, first input slot (per-cell constants kept
-                       // in registers: the load/store path of the SM is the scarce resource)
-  };
-  auto adv = [&](It &it) {
-    it.base += 32;
-    while (it.base >= it.p1) {
-      it.ci += nwarps;
-      if (it.ci >= tg.cpb) {
-        it.ok = false;
-        return;
-      }
-      it.base = 0;
-      it.p1 = sOut[it.ci + 1] - sOut[it.ci];
-      it.ns = sNs[it.ci];
-      it.in0 = sIn[it.ci];
-    }
-  };
-  struct Raw {
-    float ax, ay, az, ux, uy, uz, qw, cx;
-    int sp, id;
-  };
-  auto load_slot = [&](const It &it) -> int {
-    const int v = it.base + lane;
-    return (v >= it.ns && v < it.p1) ? ld_stream(alist + (sA[it.ci] + v - it.ns)) : it.in0 + v;
-  };
-  // Particle columns travel through a per-warp shared-memory ring of NST chunks filled with
-  // asynchronous 4-byte copies (cp.async; each lane copies and later reads its own element, so no
-  // cross-lane synchronisation is involved): NST - 1 chunks of loads are in flight per warp
-  // without holding registers, which is what hides the DRAM latency at 20 warps per SM.
-  // Lanes past the end of the cell copy zero bytes, i.e. get zero-filled slots.
-  const bool has_x = D3 || (XC && in.x != nullptr), has_id = XC && in.id != nullptr;
-  auto issue = [&](const It &it, int p, int stage) {
-    const bool v = it.base + lane < it.p1;
-    const int q = v ? p : 0;
-    float *r = myRing + stage * (RING_COLS * 32) + lane;
-    cp_async4(r + 0 * 32, in.y + q, v);
-    cp_async4(r + 1 * 32, in.z + q, v);
-    cp_async4(r + 2 * 32, in.ux + q, v);
-    cp_async4(r + 3 * 32, in.uy + q, v);
-    cp_async4(r + 4 * 32, in.uz + q, v);
-    cp_async4(r + 5 * 32, in.qw + q, v);
-    cp_async4(r + 6 * 32, in.sp + q, v);
-    if (has_x) cp_async4(r + 7 * 32, in.x + q, v);
-    if (has_id) cp_async4(r + 8 * 32, in.id + q, v);
-  };
-  auto fetch = [&](Raw &r_, int stage) {
-    const float *r = myRing + stage * (RING_COLS * 32) + lane;
-    r_.ay = r[0 * 32];
-    r_.az = r[1 * 32];
-    r_.ux = r[2 * 32];
-    r_.uy = r[3 * 32];
-    r_.uz = r[4 * 32];
-    r_.qw = r[5 * 32];
-    r_.sp = __float_as_int(r[6 * 32]);
-    r_.ax = r_.cx = 0.f;
-    if (has_x) {
-      const float t = r[7 * 32];
-      if (D3) r_.ax = t; else r_.cx = t;
-    }
-    r_.id = has_id ? __float_as_int(r[8 * 32]) : 0;
-  };
-
-  It a = {warp - nwarps, 0, 0, true, 0, 0};  // the chunk to compute
-  adv(a);
-  It pr = a;                           // the chunk to issue loads for (NST - 1 ahead)
-  int pPr = 0;
-  if (pr.ok) pPr = load_slot(pr);
-  int stage_p = 0, stage_c = 0;
+  // The warp's cells: warp, warp + nwarps, ...  The resident run of the next cell is requested
+  // from the copy engine as soon as the image of the current one has been written back.
+  if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
-  for (int k = 0; k < NST - 1; k++) {
-    if (pr.ok) {
-      issue(pr, pPr, stage_p);
-      adv(pr);
-      if (pr.ok) pPr = load_slot(pr);
-    }
-    cp_async_commit();
-    stage_p++;
-  }
-  int ncross = 0, nst = 0;  // warp-uniform: leavers / stayers of the current cell so far
-  int cur_ci = -1, lx = 0, ly = 0, lz = 0, packed = 0;
-  int oF = 0, oB = 0;  // the cell's output segment: first slot, last slot
-  const float *cF = sF;
-  float acc[NV];
-
-  while (a.ok) {
-    const It c = a;
-    if (pr.ok) {
-      issue(pr, pPr, stage_p);
-      adv(pr);
-      if (pr.ok) pPr = load_slot(pr);  // list entries one more chunk ahead
-    }
-    cp_async_commit();
-    stage_p = stage_p + 1 == NST ? 0 : stage_p + 1;
-    cp_async_wait<NST - 1>();
-    Raw cur;
-    fetch(cur, stage_c);
-    stage_c = stage_c + 1 == NST ? 0 : stage_c + 1;
-    adv(a);  // a: the next chunk (tells whether this one ends its cell)
-    if (c.ci != cur_ci) {  // first chunk of a cell
-      cur_ci = c.ci;
-      lx = c.ci % tg.bs[0];
-      const int lt_ = c.ci / tg.bs[0];
-      ly = lt_ % tg.bs[1];
-      lz = lt_ / tg.bs[1];
-      packed = lx | (ly << 10) | (lz << 20);
-      oF = sOut[c.ci];
-      oB = sOut[c.ci + 1] - 1;
-      // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
-      cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
-                    : (lz + 1) * tg.fe[1] + (ly + 1));
+  for (int ci = warp; ci < tg.cpb; ci += nwarps) {
+    const int lx = ci % tg.bs[0];
+    const int lt_ = ci / tg.bs[0];
+    const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
+    wk.begin_cell(sd, gd, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], tg.o[0] + lx,
+                  tg.o[1] + ly, tg.o[2] + lz);
+    const int ntot = wk.n + wk.na;
+    const int packed = lx | (ly << 10) | (lz << 20);
+    // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
+    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
+                               : (lz + 1) * tg.fe[1] + (ly + 1));
+    float acc[NV];
 #pragma unroll
-      for (int i = 0; i < NV; i++) acc[i] = 0.f;
-    }
-    {
-      const bool act = c.base + lane < c.p1;
-      const float ax = cur.ax, ay = cur.ay, az = cur.az, qw = cur.qw;
+    for (int i = 0; i < NV; i++) acc[i] = 0.f;
+
+#pragma unroll 1
+    for (int v0 = 0; v0 < ntot; v0 += 32) {
+      Part cur;
+      bool isarr;
+      float x2d;
+      int id;
+      const bool act = wk.load(sd, v0, cur, isarr, x2d, id);
+      const float ax = D3 ? cur.ax : 0.f, ay = cur.ay, az = cur.az, qw = cur.qw;
       float ux = cur.ux, uy = cur.uy, uz = cur.uz;
-      const int sp = cur.sp;
+      const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
 
       // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) --------
       // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l
@@ -570,64 +483,49 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
       // a trajectory that stays in the cell is one segment: its currents go to the per-cell
       // register sums; one that leaves goes through the per-warp queue (all its segments)
       {
-        const float qs = cross ? 0.f : qw;
+        const float qs = (cross || !act) ? 0.f : qw;
         vb_moments<D3>(acc, ax, ay, az, endx, endy, endz, qs * gd.cur[0], qs * gd.cur[1],
                        qs * gd.cur[2], qs * gd.inv_dV * vx);
       }
       const unsigned cm = __ballot_sync(0xffffffffu, cross);
-      const unsigned sm = __ballot_sync(0xffffffffu, act && !cross);
-      // output slot: stayers fill the cell's segment from the front, leavers from the back
-      const int s = cross ? oB - ncross - __popc(cm & lt) : oF + nst + __popc(sm & lt);
-      nst += __popc(sm);
       if (cm) {
+        const int xi = wk.leaver_index(cross, dc);
         if (cross) {
+          if (wk.fast && !isarr) wk.extras(sd, v0 + lane, x2d, id);
           const int e = qcnt + __popc(cm & lt);
           myQ[0 * QCAP + e] = __int_as_float(packed);
-          myQ[1 * QCAP + e] = ax;
+          myQ[1 * QCAP + e] = D3 ? ax : x2d;
           myQ[2 * QCAP + e] = ay;
           myQ[3 * QCAP + e] = az;
           myQ[4 * QCAP + e] = D3 ? ddx : vx;
           myQ[5 * QCAP + e] = ddy;
           myQ[6 * QCAP + e] = ddz;
           myQ[7 * QCAP + e] = qw;
+          myQ[8 * QCAP + e] = ux;
+          myQ[9 * QCAP + e] = uy;
+          myQ[10 * QCAP + e] = uz;
+          myQ[11 * QCAP + e] = __int_as_float(sp | (xi << 8));
+          if (XC) myQ[12 * QCAP + e] = __int_as_float(id);
         }
-        if (cross) atomicAdd(&sDir[warp * 32 + dc], 1);
         qcnt += __popc(cm);
-        ncross += __popc(cm);
         __syncwarp();
         if (qcnt >= 32) {
           qcnt -= 32;
-          drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
+          drain_queue<D3, XC>(sJ, tg, gd, sd, kbase, myQ, sRel, qcnt, 32, lane);
         }
       }
 
-      // ---- store slot s of the other column set: new offset, momentum, direction code -----
-      if (act) {
-        const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-        const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-        if (D3) {
-          const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
-          st_stream(out.x + s, bx_);
-          if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
-        } else if (has_x) {
-          st_stream(out.x + s, cur.cx);  // invariant coordinate: carried
-        }
-        st_stream(out.y + s, by_);
-        st_stream(out.z + s, bz_);
-        st_stream(out.ux + s, ux);
-        st_stream(out.uy + s, uy);
-        st_stream(out.uz + s, uz);
-        st_stream(out.qw + s, qw);
-        st_stream(out.sp + s, sp);
-        if (has_id) st_stream(out.id + s, cur.id);
-        if (cross) dcode[s] = (uint8_t)dc;
-        if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
-      }
+      // ---- file the particles that stay: in place (residents) or into a hole (arrivals) -----
+      Part pn;
+      pn.ax = endx; pn.ay = endy; pn.az = endz;
+      pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
+      wk.store(sd, v0, act, isarr, cross, pn, x2d, id);
+      if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
 
-    // ---- last chunk of the cell: its in-cell currents take one warp reduction and one shared
-    // add per J point; its direction-code counts go to the index sort
-    if (!a.ok || a.ci != c.ci) {
+    // ---- the cell is done: its in-cell currents take one warp reduction and one shared add per
+    // J point; its image goes back to global memory and the next cell's run is requested
+    if (ntot) {
       float r;
       moments_to_values<D3>(acc);
       if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
@@ -637,22 +535,13 @@ k_push1(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
                             : (lz + 1) * tg.je[1] + (ly + 1);
         atomicAdd(&sJ[node + my_off], r);
       }
-      // direction-code counts of the cell: the leavers were counted above, the rest stayed
-      {
-        constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-        int *row = sDir + warp * 32;
-        if (lane < ND) {
-          dircnt[lane * gd.nkeys + kbase + c.ci] = lane == STAY ? nst : row[lane];
-          row[lane] = 0;
-        }
-        ncross = 0;
-        nst = 0;
-        __syncwarp();
-      }
     }
+    const int nx = ci + nwarps;
+    wk.end_cell(sd, nx < tg.cpb ? sCnt[nx] : 0, nx < tg.cpb ? sBase[nx] : 0);
   }
-  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, sRel, 0, qcnt, lane);
-  if (bad) atomicOr(flags, bad);
+  if (qcnt) drain_queue<D3, XC>(sJ, tg, gd, sd, kbase, myQ, sRel, 0, qcnt, lane);
+  wk.finish();
+  if (bad) atomicOr(sd.flags, bad);
   __syncthreads();
 
   // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
@@ -681,40 +570,36 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       fvol *= gd.bs[d] + 2;
       jvol *= gd.bs[d] + 3;
     }
-  const int vthreads = 128;
-  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : vthreads;
-  if (threads < 32 || threads > vthreads) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + (threads / 32) * (32 + (d3 ? QROWS3 : QW) * QCAP + NST * RING_COLS * 32) + 12 + 4 * gd.cpb + 2) * sizeof(float);
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
+  const StoreDesc sd = psc_store_desc(c);
+  const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
+  constexpr int threads = 128;
+  const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
+  const int wstride = (wbytes + 127) / 128 * 128;
+  const size_t smem = (size_t)(threads / 32) * (wstride + QROWS * QCAP * 4) +
+                      (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 2 * gd.cpb + 2) * sizeof(float);
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
-  const Cols &in = c->cols[c->cur];
-  const Cols &out = c->cols[c->cur ^ 1];
-  const PushLists pls = psc_push_lists(c);
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
   do {                                                                                             \
     if (xc) {                                                                                      \
       PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, true>,                       \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      k_push1<D3_, CBS_, T_, B_, true><<<gd.ntiles, threads, smem, s>>>(                           \
-          gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                         \
+      k_push1<D3_, CBS_, T_, B_, true><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride); \
     } else {                                                                                       \
       PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, false>,                      \
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      k_push1<D3_, CBS_, T_, B_, false><<<gd.ntiles, threads, smem, s>>>(                          \
-          gd, in, out, pls, c->E, c->B, c->J, c->d_flags);                                         \
+      k_push1<D3_, CBS_, T_, B_, false><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride); \
     }                                                                                              \
   } while (0)
-  const bool xc = in.id != nullptr || (!d3 && in.x != nullptr);
   if (d3) {
-    const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4 && c->opt_push_variant != 2;
+    const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
     if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4);
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
   } else {
-    const bool def = gd.bs[1] == 8 && gd.bs[2] == 8 && c->opt_push_variant != 2;
-    if (def && c->opt_push_variant == 1) PSC_LAUNCH_PUSH1(false, 8, 128, 6);
-    else if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
-    else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
+    const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 4);
+    else PSC_LAUNCH_PUSH1(false, 0, 128, 4);
   }
 #undef PSC_LAUNCH_PUSH1
   PSC_LAUNCH_CHECK(c);

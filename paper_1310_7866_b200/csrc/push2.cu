@@ -3,8 +3,10 @@
 // (Eq. 27-28), move (Eq. 26), Esirkepov charge-conserving deposit, periodic wrap.
 //
 // One thread block per sort block ("supercell"); a warp takes one CELL at a time
-// and walks that cell's particle range in chunks of 32, so the cell -- and with it every tile
-// address that does not depend on the in-cell offset -- is warp-uniform.
+// and walks that cell's particles in chunks of 32, so the cell -- and with it every tile
+// address that does not depend on the in-cell offset -- is warp-uniform.  Particle I/O is the
+// cell store's (store.cuh): bulk asynchronous copies of the cell's columns into shared memory,
+// in-place update, leavers through the exchange rows.
 //
 // Stencils, relative to the particle's cell l and its in-cell offset a in [0,1) (A13,
 // A15).  Because dt <= dx/2 a particle moves less than half a cell, so the node nearest to the
@@ -23,7 +25,7 @@
 // its one or two totals to the shared-memory J tile -- no same-address atomic conflicts.
 #include <limits.h>
 
-#include "push_common.cuh"
+#include "store.cuh"
 
 namespace {
 
@@ -202,22 +204,29 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
     if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
 }
 
-template <bool D3, int CBS>
+template <bool D3, int CBS, bool XC>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
-k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__ E,
-        const float *__restrict__ B, float *__restrict__ J, uint32_t *__restrict__ flags) {
-  extern __shared__ float smem[];
+k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
+        float *__restrict__ J, int wstride) {
+  extern __shared__ __align__(128) unsigned char smraw[];
+  using Walker = CellWalker<D3, XC>;
   Geom2<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
-  float *sF = smem;                // [6][tvol]
-  float *sJ = smem + 6 * tg.tvol;  // [3][tvol]
-  float *sH = sJ + 3 * tg.tvol;               // [8]: Boris h per species
-  int *sDir = (int *)(sH + PSC_MAX_SPECIES);  // [warps][32]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  Walker wk;
+  wk.init(smraw + (size_t)warp * wstride, sd, lane);
+  float *sF = (float *)(smraw + (size_t)nwarps * wstride);  // [6][tvol]
+  float *sJ = sF + 6 * tg.tvol;                              // [3][tvol]
+  float *sH = sJ + 3 * tg.tvol;                              // [8]: Boris h per species
+  int *sBase = (int *)(sH + PSC_MAX_SPECIES);                // [cpb + 1]
+  int *sCnt = sBase + tg.cpb + 1;                            // [cpb]
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
-  DirCount<D3> dirs;
-  dirs.init(sDir + warp * 32, lane);
+  const int kbase = blockIdx.x * tg.cpb;
+  for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
+    sBase[i] = sd.base[kbase + i];
+    if (i < tg.cpb) sCnt[i] = sd.cnt[kbase + i];
+  }
   for (int i = threadIdx.x; i < 6 * tg.tvol; i += blockDim.x) {
     const int c = i / tg.tvol, r = i - c * tg.tvol;
     const int tx = r % tg.te[0], t = r / tg.te[0];
@@ -242,41 +251,29 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
 
   const float *sEx = sF, *sEy = sF + tg.tvol, *sEz = sF + 2 * tg.tvol;
   const float *sBx = sF + 3 * tg.tvol, *sBy = sF + 4 * tg.tvol, *sBz = sF + 5 * tg.tvol;
-  const int kbase = blockIdx.x * tg.cpb;
   uint32_t bad = 0;
 
-  uint8_t *__restrict__ dcode = pls.dcode;
-  int *__restrict__ dircnt = pls.dircnt;
-  const unsigned lanes_lt = lanemask_lt_();
-
+  if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
+#pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
-    // the cell's particles: its run of stayers of the previous step, then its listed arrivals
-    // (reorder on load); its output segment: stayers from the front, leavers from the back
-    const int in0 = pls.offs_in[kbase + ci];
-    const int ns = pls.nstay ? pls.nstay[kbase + ci] : pls.offs_in[kbase + ci + 1] - in0;
-    const int a0 = pls.aoffs ? pls.aoffs[kbase + ci] : 0;
-    int ofront = pls.offs_out[kbase + ci], oback = pls.offs_out[kbase + ci + 1] - 1;
-    const int np_cell = oback + 1 - ofront;  // stayers + arrivals
     const int lx = ci % tg.bs[0], lt = ci / tg.bs[0];
     const int ly = lt % tg.bs[1], lz = lt / tg.bs[1];
+    wk.begin_cell(sd, gd, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], tg.o[0] + lx,
+                  tg.o[1] + ly, tg.o[2] + lz);
+    const int np_cell = wk.n + wk.na;  // residents + arrivals (reorder on load)
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
+#pragma unroll 1
     for (int base = 0; base < np_cell; base += 32) {
-      const int v = base + lane;
-      const bool act = v < np_cell;
-      float ax = 0.25f, ay = 0.25f, az = 0.25f, ux = 0.f, uy = 0.f, uz = 0.f, qw = 0.f;
-      int sp = 0, p = in0 + v;
-      if (act) {
-        if (v >= ns) p = ld_stream(pls.alist + (a0 + v - ns));  // reorder on load
-        ay = ld_stream(in.y + p);
-        az = ld_stream(in.z + p);
-        ux = ld_stream(in.ux + p);
-        uy = ld_stream(in.uy + p);
-        uz = ld_stream(in.uz + p);
-        qw = ld_stream(in.qw + p);
-        sp = ld_stream(in.sp + p);
-        if (D3) ax = ld_stream(in.x + p);
-      }
+      Part cur;
+      bool isarr;
+      float x2d;
+      int id;
+      const bool act = wk.load(sd, base, cur, isarr, x2d, id);
+      const float ax = D3 ? cur.ax : 0.25f, ay = cur.ay, az = cur.az;
+      float ux = cur.ux, uy = cur.uy, uz = cur.uz;
+      const float qw = act ? cur.qw : 0.f;
+      const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
       // ---- gather (Eq. 11 with b2 weights; each component from its own Yee points) ---------
       Sten2 sx, sy, sz;
       sx.set(lx, ax);
@@ -400,44 +397,40 @@ k_push2(GridDesc gd, Cols in, Cols out, PushLists pls, const float *__restrict__
         }
       }
 
-      // ---- store slot a of the other column set: new offset, momentum, direction code -----
+      // ---- file the particle: in place / into a hole if it stays, as a record if it leaves -----
       const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
       const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
       const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
       const int dc = dir_code<D3>(sxd, syd, szd);
-      dirs.add(act, dc);
-      const bool leave = act && dc != DirCount<D3>::STAY;
-      const unsigned lm = __ballot_sync(0xffffffffu, leave);
-      const unsigned sm = __ballot_sync(0xffffffffu, act && !leave);
-      const int a = leave ? oback - __popc(lm & lanes_lt) : ofront + __popc(sm & lanes_lt);
-      ofront += __popc(sm);
-      oback -= __popc(lm);
-      if (act) {
-        const float by_ = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-        const float bz_ = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-        if (D3) {
-          const float bx_ = fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f);
-          st_stream(out.x + a, bx_);
-          if (!(bx_ >= 0.f)) bad |= PSC_F_NAN;
-        } else if (in.x) {
-          st_stream(out.x + a, ld_stream(in.x + p));  // invariant coordinate: carried
+      const bool leave = act && dc != Walker::STAY;
+      Part pn;
+      pn.ax = endx; pn.ay = endy; pn.az = endz;
+      pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
+      if (__any_sync(0xffffffffu, leave)) {
+        const int xi = wk.leaver_index(leave, dc);
+        if (leave) {
+          if (wk.fast && !isarr) wk.extras(sd, base + lane, x2d, id);
+          Part pr = pn;
+          pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
+          pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+          pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+          float w[8];
+          Walker::to_words(w, pr, x2d);
+          int dest = 0;
+          if (xi >= PSC_XCAP)
+            dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
+                            wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
+          Walker::write_record(sd, gd, kbase + ci, xi, w, id, dest);
         }
-        st_stream(out.y + a, by_);
-        st_stream(out.z + a, bz_);
-        st_stream(out.ux + a, ux);
-        st_stream(out.uy + a, uy);
-        st_stream(out.uz + a, uz);
-        st_stream(out.qw + a, qw);
-        st_stream(out.sp + a, sp);
-        if (in.id) st_stream(out.id + a, ld_stream(in.id + p));
-        if (leave) dcode[a] = (uint8_t)dc;
-        if (!(by_ >= 0.f) || !(bz_ >= 0.f) || !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f))
-          bad |= PSC_F_NAN;
       }
+      wk.store(sd, base, act, isarr, leave, pn, x2d, id);
+      if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
-    dirs.cell_done(dircnt, kbase + ci, gd.nkeys, lane);
+    const int nx = ci + nwarps;
+    wk.end_cell(sd, nx < tg.cpb ? sCnt[nx] : 0, nx < tg.cpb ? sBase[nx] : 0);
   }
-  if (bad) atomicOr(flags, bad);
+  wk.finish();
+  if (bad) atomicOr(sd.flags, bad);
   __syncthreads();
 
   // ---- flush the J tile to global J -----------------------------------------------------------
@@ -463,30 +456,35 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   int tvol = 1;
   for (int d = 0; d < 3; d++)
     if (gd.n[d] > 1) tvol *= gd.bs[d] + 3;
-  const int threads = c->opt_threads > 0 ? (c->opt_threads / 32) * 32 : PUSH2_THREADS;
-  if (threads < 32 || threads > PUSH2_THREADS) return PSC_ERR_INVALID_ARG;
-  const size_t smem = (size_t)(9 * tvol + PSC_MAX_SPECIES + (threads / 32) * 32) * sizeof(float);
+  const StoreDesc sd = psc_store_desc(c);
+  const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
+  const int threads = PUSH2_THREADS;
+  const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
+  const int wstride = (wbytes + 127) / 128 * 128;
+  const size_t smem = (size_t)(threads / 32) * wstride +
+                      (size_t)(9 * tvol + PSC_MAX_SPECIES + 2 * gd.cpb + 2) * sizeof(float);
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
-  const Cols &in = c->cols[c->cur];
-  const Cols &out = c->cols[c->cur ^ 1];
-  const PushLists pls = psc_push_lists(c);
   ProfScope ps(c, PSC_PH_PUSH, s);
-#define PSC_LAUNCH_PUSH2(D3_, CBS_)                                                                 \
+#define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_)                                                           \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_>,                                       \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_>,                                  \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    k_push2<D3_, CBS_><<<gd.ntiles, threads, smem, s>>>(gd, in, out, pls, c->E, c->B, c->J,        \
-                                                        c->d_flags);                               \
+    k_push2<D3_, CBS_, XC_><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride);   \
   } while (0)
-  const bool generic = c->opt_push_variant == 2;
+#define PSC_LAUNCH_PUSH2(D3_, CBS_)           \
+  do {                                        \
+    if (xc) PSC_LAUNCH_PUSH2_(D3_, CBS_, true); \
+    else PSC_LAUNCH_PUSH2_(D3_, CBS_, false); \
+  } while (0)
   if (d3) {
-    if (!generic && gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4) PSC_LAUNCH_PUSH2(true, 4);
+    if (gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4) PSC_LAUNCH_PUSH2(true, 4);
     else PSC_LAUNCH_PUSH2(true, 0);
   } else {
-    if (!generic && gd.bs[1] == 8 && gd.bs[2] == 8) PSC_LAUNCH_PUSH2(false, 8);
+    if (gd.bs[1] == 8 && gd.bs[2] == 8) PSC_LAUNCH_PUSH2(false, 8);
     else PSC_LAUNCH_PUSH2(false, 0);
   }
 #undef PSC_LAUNCH_PUSH2
+#undef PSC_LAUNCH_PUSH2_
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }

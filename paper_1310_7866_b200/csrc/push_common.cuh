@@ -60,66 +60,3 @@ __device__ __forceinline__ unsigned lanemask_lt_() {
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
 }
-
-// The particle lists a push kernel reads and writes (sort.cu "INDEX" form).
-// Input: cell k's particles are the run [offs_in[k], offs_in[k] + nstay[k]) of the input columns
-// (the stayers of the previous push) plus the arrivals alist[aoffs[k] .. aoffs[k+1]) (slots of
-// the input columns).  Output: cell k's segment [offs_out[k], offs_out[k+1]) of the other column
-// set, the particles that stay in k compacted at its front, the leavers at its back with their
-// direction code in dcode[slot]; dircnt[dc][k] = how many of cell k took direction dc
-// (direction-major, so that the per-cell kernels of the index sort read it coalesced).
-struct PushLists {
-  const int *offs_in;
-  const int *nstay;     // nullptr: the whole segment (a physically sorted list)
-  const int *aoffs;     // nullptr: no arrivals
-  const int *alist;
-  const int *offs_out;
-  uint8_t *dcode;
-  int *dircnt;
-};
-
-// SORTED: every segment is one run, written back to the same layout; INDEXED: the written list
-// (layout offs[ocur^1]) is read through nstay / aoffs / alist into the new layout offs[ocur].
-static inline PushLists psc_push_lists(const psc_ctx *c) {
-  PushLists l;
-  const bool indexed = c->state == PSC_STATE_INDEXED;
-  l.offs_in = indexed ? c->offs[c->ocur ^ 1] : c->offs[c->ocur];
-  l.nstay = indexed ? c->nstay : nullptr;
-  l.aoffs = indexed ? c->aoffs : nullptr;
-  l.alist = c->alist;
-  l.offs_out = c->offs[c->ocur];
-  l.dcode = c->dcode;
-  l.dircnt = c->dircnt;
-  return l;
-}
-
-// Per-warp bookkeeping of the direction codes of one cell's particles (9 / 27
-// destination classes): the stayers are counted with a ballot, the few leavers with
-// shared-memory integer atomics on the warp's private row.  cell_done() writes the cell's ND
-// counts (what the index sort of sort.cu consumes) and clears the row.
-template <bool D3>
-struct DirCount {
-  static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  int *row;   // shared, [32], zero on entry
-  int nstay;
-  __device__ __forceinline__ void init(int *r, int lane) {
-    row = r;
-    row[lane] = 0;
-    nstay = 0;
-    __syncwarp();
-  }
-  __device__ __forceinline__ void add(bool act, int dc) {
-    const bool stay = dc == STAY;
-    nstay += __popc(__ballot_sync(0xffffffffu, act && stay));
-    if (act && !stay) atomicAdd(&row[dc], 1);
-  }
-  __device__ __forceinline__ void cell_done(int *__restrict__ dircnt, int key, int nkeys, int lane) {
-    __syncwarp();
-    if (lane < ND) {
-      dircnt[lane * nkeys + key] = row[lane] + (lane == STAY ? nstay : 0);
-      row[lane] = 0;
-    }
-    nstay = 0;
-    __syncwarp();
-  }
-};

@@ -1,44 +1,33 @@
-// sort.cu -- cell-key counting sort of the particle list.
+// sort.cu -- cell-key counting sort of the particle list and the layout of
+// the cell store it produces.
 //
 // One key orders by block ("supercell") and by cell inside the block at once:
 //   key = block_index * cells_per_block + cell_in_block.
-// A counting sort is O(N + M).  Two forms:
-//
-// GENERAL (arbitrary input order; the first sort of a run, from absolute positions):
+// A counting sort is O(N + M):
 //   1. k_keys     key per particle from floor(fl32(x * 1/dx)) (k_hist: keys already known), and a
 //                 histogram over keys with warp-aggregated atomics;
-//   2. scan       exclusive prefix sum of the histogram -> cell offsets (three small kernels);
-//   3. k_scatter  slot = cursor[key] + rank, again warp-aggregated; writes the permutation;
-//   4. k_segsort  the atomics hand out slots in arbitrary order ACROSS warps, so every key's
+//   2. k_layout   capacity of every cell = its count plus spare room, rounded up to 32 slots;
+//      scan       one exclusive prefix sum over (capacity, count) packed in 64 bits -> the first
+//                 slot base[k] of every cell in the store and the dense offsets of the sorted list;
+//   3. k_scatter  dense position = cursor[key] + rank, again warp-aggregated; writes the permutation;
+//   4. k_segsort  the atomics hand out positions in arbitrary order ACROSS warps, so every key's
 //                 segment of `perm` is sorted ascending: a set of distinct input indices in
 //                 ascending order IS the stable order, hence the result is the unique stable
 //                 counting sort, bit-exact against any stable reference;
-//   5. k_reorder  out[s] = in[perm[s]] for every column; positions leave in the internal form.
+//   5. k_reorder  out[base[k] + rank] = in[perm[s]] for every column; positions leave in the
+//                 internal form (in-cell offsets).
 //
-// INDEX (steady state: "a particle moves at most one cell per step", "the
-// sort only touches keys/indices", "reorder on load"): the list is the previous sort's output
-// advanced by one push.  The push wrote every cell's particles back into a segment of the cell's
-// size, the STAYERS (still in the cell: the great majority) compacted at the front and the
-// LEAVERS at the back, each leaver with the one-byte direction code of its move (one of 9 / 27
-// destination classes), and per cell the count of each code.  So the particles of a cell of the
-// NEXT step are one contiguous run (its stayers) plus a short list of arrivals, and the sort
-// works on cells and leavers only:
-//   1. k_dest_hist  per cell: stayers, arrivals (sum over the 8 / 26 neighbour source cells of
-//                   the count of the code that points here);
-//   2. scan         one pass over (total, arrivals) packed in 64 bits -> new cell offsets and
-//                   offsets into the arrival list;
-//   3. k_dir_base   first arrival-list slot of every (source cell, code) group: a cell's
-//                   arrivals are grouped by the direction they came from;
-//   4. k_rank       one warp per source cell walks its LEAVER region and writes the slots of
-//                   the leavers into the arrival list.
-// No particle column is touched and nothing per stayer is read or written: the next push loads
-// the stayer run directly and the arrivals through the list (reorder on load).  The order this
-// gives inside a cell (stayers, then arrivals) is a valid cell sort but not the stable one
-// (A17); psc_particles_sort, whose contract is the physically sorted, stable list,
-// runs the general form on the keys of the written list instead.
+// PAPER.md:597-603 ("a particle moves at most one cell per step", "reorder on load"): between
+// pushes NO sort runs.  The push kernels keep every cell's particles dense in the cell's own
+// slots and hand the few cell-changers over through the exchange rows (store.cuh).  Only when a
+// push had to spill (an exchange row or a cell ran out of room) the next step re-lays the store
+// out: k_tot / scan / k_gather flatten residents + exchange records + spill list into the other
+// column set, and steps 1-5 (without 4: the order inside a cell is immaterial, A17)
+// bring them back.  Whether that is needed is known on the device only, so these launches carry a
+// condition word and return at once when it is zero.
 #include <limits.h>
 
-#include "psc_internal.cuh"
+#include "store.cuh"
 
 namespace {
 
@@ -54,10 +43,13 @@ __device__ __forceinline__ unsigned lanemask_lt() {
   return m;
 }
 
+#define PSC_COND_RETURN(cond) \
+  if ((cond) && !*(cond)) return
+
 __global__ void __launch_bounds__(SORT_THREADS)
 k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict__ y,
-       const float *__restrict__ z, int *__restrict__ key, int *__restrict__ hist,
-       uint32_t *__restrict__ flags) {
+       const float *__restrict__ z, const int *__restrict__ sp, int *__restrict__ key,
+       int *__restrict__ hist, uint32_t *__restrict__ flags) {
   const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   const int nround = ((n + 31) / 32) * 32;
@@ -76,6 +68,9 @@ k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict_
         }
         const float xi = __fmul_rn(pos[d][a], gd.inv_dx[d]);  // one fp32 rounding, then floor
         int ci = (int)floorf(xi);
+        // a product that rounds up to n although x < L belongs to the last cell (its offset is
+        // then clamped just below 1 by k_reorder): not a fault
+        if (ci == gd.n[d] && pos[d][a] < gd.L[d]) ci = gd.n[d] - 1;
         if (!(ci >= 0 && ci < gd.n[d])) {  // also catches NaN
           oob = true;
           ci = ci < 0 ? 0 : gd.n[d] - 1;
@@ -84,9 +79,9 @@ k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict_
         c[d] = ci;
       }
       if (oob) atomicOr(flags, PSC_F_OOB);
-      const int b0 = c[0] / gd.bs[0], b1 = c[1] / gd.bs[1], b2 = c[2] / gd.bs[2];
-      const int l0 = c[0] - b0 * gd.bs[0], l1 = c[1] - b1 * gd.bs[1], l2 = c[2] - b2 * gd.bs[2];
-      k = ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
+      const int s = sp[a];
+      if (s < 0 || s >= gd.nsp) atomicOr(flags, PSC_F_SPECIES);
+      k = cell_key(gd, c[0], c[1], c[2]);
       key[a] = k;
     }
     const unsigned grp = __match_any_sync(0xffffffffu, k);
@@ -94,10 +89,12 @@ k_keys(GridDesc gd, int n, const float *__restrict__ x, const float *__restrict_
   }
 }
 
-// histogram of keys that already exist (internal form: the push wrote them)
+// histogram of keys that already exist (a flattened store)
 __global__ void __launch_bounds__(SORT_THREADS)
-k_hist(int n, int nkeys, const int *__restrict__ key, int *__restrict__ hist,
-       uint32_t *__restrict__ flags) {
+k_hist(const int *__restrict__ np, int nkeys, const int *__restrict__ key, int *__restrict__ hist,
+       uint32_t *__restrict__ flags, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int n = *np;
   const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   const int nround = ((n + 31) / 32) * 32;
@@ -114,6 +111,12 @@ k_hist(int n, int nkeys, const int *__restrict__ key, int *__restrict__ hist,
     const unsigned grp = __match_any_sync(0xffffffffu, k);
     if (valid && (grp & lanemask_lt()) == 0) atomicAdd(&hist[k], __popc(grp));
   }
+}
+
+__global__ void __launch_bounds__(SORT_THREADS)
+k_zero(int m, int *__restrict__ a, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) a[i] = 0;
 }
 
 // key -> cell coordinates
@@ -137,30 +140,38 @@ k_cell_idx(GridDesc gd, int n, const int *__restrict__ key, int *__restrict__ ce
   cell_idx[a] = (c[2] * gd.n[1] + c[1]) * gd.n[0] + c[0];
 }
 
-// internal form -> absolute positions, in place: x = (cell + offset) * dx
+// Capacity of a cell holding cnt particles: room for an eighth more (at least 16), rounded up to
+// a multiple of 32 slots so that every column of every cell starts on a 128-byte line.
+// Sum over cells <= n + n/8 + 47 nkeys (psc_store_capacity).
+__device__ __forceinline__ int cell_capacity(int cnt) {
+  const int spare = max(cnt >> 3, 16);
+  return (cnt + spare + PSC_SLOT_ALIGN - 1) & ~(PSC_SLOT_ALIGN - 1);
+}
+
+// per cell: pack = capacity << 32 | count for the packed scan; cnt := count; stats: largest count
 __global__ void __launch_bounds__(SORT_THREADS)
-k_to_abs(GridDesc gd, int n, const int *__restrict__ key, float *__restrict__ x,
-         float *__restrict__ y, float *__restrict__ z) {
-  const int a = blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= n) return;
-  int c[3];
-  key_to_cell(gd, key[a], c);
-  float *pos[3] = {x, y, z};
-#pragma unroll
-  for (int d = 0; d < 3; d++) {
-    if (gd.n[d] == 1) continue;
-    // formed in fp64 and rounded once (this pass runs once per export, not per step)
-    float v = __double2float_rn(((double)c[d] + (double)pos[d][a]) * (double)gd.dx[d]);
-    if (v >= gd.L[d]) v = nextafterf(gd.L[d], 0.f);  // rounding must not leave [0, L)
-    pos[d][a] = v;
+k_layout(int nk, const int *__restrict__ hist, long long *__restrict__ pack, int *__restrict__ cnt,
+         uint32_t *__restrict__ dw, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  int mx = 0;
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nk; k += gridDim.x * blockDim.x) {
+    const int c = hist[k];
+    cnt[k] = c;
+    pack[k] = ((long long)cell_capacity(c) << 32) | (long long)c;
+    mx = max(mx, c);
   }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  if ((threadIdx.x & 31) == 0 && mx) atomicMax(&dw[PSC_DW_MAXCNT], (uint32_t)mx);
 }
 
 // ---- exclusive scan of in[0..m) -> out[0..m], out[m] = total -----------------------------------
-// T = int: one histogram (general sort; cursor := out as well).  T = long long: two histograms
-// packed as (hi << 32) | lo and scanned in one pass (index sort: hi = particles per cell, lo =
-// arrivals per cell; both totals are < 2^31, so the low half never carries into the high half);
-// the last kernel unpacks them into out (hi) and out_lo.
+// T = int: one histogram (cursor := out as well if given).  T = long long: two histograms packed
+// as (hi << 32) | lo and scanned in one pass (the layout: hi = capacity of a cell, lo = particles
+// in it; both totals are < 2^31, so the low half never carries into the high half); the last
+// kernel unpacks them into out (hi) and out_lo.
+// cond != nullptr: the launch does nothing unless *cond != 0 (a re-layout only runs when the
+// previous push spilled; the host cannot know without synchronising, so the device decides).
 
 template <typename T>
 __device__ __forceinline__ T warp_inclusive(T v, int lane) {
@@ -174,7 +185,9 @@ __device__ __forceinline__ T warp_inclusive(T v, int lane) {
 
 template <typename T>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_scan_local(int m, const T *__restrict__ in, T *__restrict__ out, T *__restrict__ tmp) {
+k_scan_local(int m, const T *__restrict__ in, T *__restrict__ out, T *__restrict__ tmp,
+             const uint32_t *__restrict__ cond) {
+  if (cond && !*cond) return;
   __shared__ T wsum[SORT_THREADS / 32];
   const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   T v[SCAN_ITEMS];
@@ -205,7 +218,8 @@ k_scan_local(int m, const T *__restrict__ in, T *__restrict__ out, T *__restrict
 
 // single block: exclusive scan of tmp[0..nb) in place, tmp[nb] = total
 template <typename T>
-__global__ void __launch_bounds__(1024) k_scan_tmp(int nb, T *__restrict__ tmp) {
+__global__ void __launch_bounds__(1024) k_scan_tmp(int nb, T *__restrict__ tmp, const uint32_t *__restrict__ cond) {
+  if (cond && !*cond) return;
   __shared__ T wsum[32];
   __shared__ T carry_s;
   if (threadIdx.x == 0) carry_s = 0;
@@ -231,7 +245,8 @@ __global__ void __launch_bounds__(1024) k_scan_tmp(int nb, T *__restrict__ tmp) 
 
 __global__ void __launch_bounds__(SORT_THREADS)
 k_scan_add(int m, int *__restrict__ out, int *__restrict__ cursor, const int *__restrict__ tmp,
-           int nb) {
+           int nb, const uint32_t *__restrict__ cond) {
+  if (cond && !*cond) return;
   const int add = tmp[blockIdx.x];
   const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
 #pragma unroll
@@ -239,7 +254,7 @@ k_scan_add(int m, int *__restrict__ out, int *__restrict__ cursor, const int *__
     if (base + i < m) {
       const int v = out[base + i] + add;
       out[base + i] = v;
-      cursor[base + i] = v;
+      if (cursor) cursor[base + i] = v;
     }
   if (blockIdx.x == 0 && threadIdx.x == 0) out[m] = tmp[nb];
 }
@@ -247,7 +262,9 @@ k_scan_add(int m, int *__restrict__ out, int *__restrict__ cursor, const int *__
 // packed form: loc[] holds the block-local packed scan; out := high halves, out_lo := low halves
 __global__ void __launch_bounds__(SORT_THREADS)
 k_scan_add2(int m, const long long *__restrict__ loc, int *__restrict__ out,
-            int *__restrict__ out_lo, const long long *__restrict__ tmp, int nb) {
+            int *__restrict__ out_lo, int *__restrict__ cursor, const long long *__restrict__ tmp, int nb,
+            const uint32_t *__restrict__ cond) {
+  if (cond && !*cond) return;
   const long long add = tmp[blockIdx.x];
   const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
 #pragma unroll
@@ -256,6 +273,7 @@ k_scan_add2(int m, const long long *__restrict__ loc, int *__restrict__ out,
       const long long v = loc[base + i] + add;
       out[base + i] = (int)(v >> 32);
       out_lo[base + i] = (int)(v & 0xffffffffLL);
+      cursor[base + i] = (int)(v & 0xffffffffLL);
     }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     out[m] = (int)(tmp[nb] >> 32);
@@ -264,7 +282,10 @@ k_scan_add2(int m, const long long *__restrict__ loc, int *__restrict__ out,
 }
 
 __global__ void __launch_bounds__(SORT_THREADS)
-k_scatter(int n, const int *__restrict__ key, int *__restrict__ cursor, int *__restrict__ perm) {
+k_scatter(const int *__restrict__ np, const int *__restrict__ key, int *__restrict__ cursor,
+          int *__restrict__ perm, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int n = *np;
   const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   const int nround = ((n + 31) / 32) * 32;
@@ -386,415 +407,500 @@ k_segsort_big(const int *__restrict__ offs, int *__restrict__ perm,
   }
 }
 
-// FROM_ABS: the input columns hold absolute positions -> write in-cell offsets
+// Sorted position s holds input particle perm[s]; its cell k = key[perm[s]] starts at dense
+// offset offs[k] and at slot base[k] of the store.  FROM_ABS: the input columns hold absolute
+// positions -> write in-cell offsets.
 template <bool FROM_ABS>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_reorder(GridDesc gd, int n, const int *__restrict__ perm, Cols in, Cols out) {
+k_reorder(GridDesc gd, const int *__restrict__ np, const int *__restrict__ perm,
+          const int *__restrict__ key, const int *__restrict__ offs, const int *__restrict__ base,
+          Cols in, Cols out, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int n = *np;
   const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
   const int stride = gridDim.x * blockDim.x;
   for (int s = s0; s < n; s += stride) {
     const int p = perm[s];
+    const int k = key[p];
+    const size_t o = (size_t)base[k] + (s - offs[k]);
     float x = in.x ? in.x[p] : 0.f, y = in.y[p], z = in.z[p];
     const float ux = in.ux[p], uy = in.uy[p], uz = in.uz[p];
     const float qw = in.qw[p];
-    const int sp = in.sp[p];
+    int sp = in.sp[p];
     int id = 0;
     if (in.id) id = in.id[p];
     if (FROM_ABS) {
-      // the cell is decided as in k_keys (fp32 product with 1/dx, floor); the offset is then
-      // (x - cell dx) / dx with the difference formed by one FMA, i.e. accurate to fp32 RELATIVE
-      // precision of the offset also when dx is not a power of two (x * (1/dx) - cell would carry
-      // the absolute rounding error of x / dx, ~1e-6 cells at x / dx ~ 20)
+      // the cell is the one k_keys decided (key[p]); the offset is (x - cell dx) / dx with the
+      // difference formed by one FMA, i.e. accurate to fp32 RELATIVE precision of the offset also
+      // when dx is not a power of two (x * (1/dx) - cell would carry the absolute rounding error
+      // of x / dx, ~1e-6 cells at x / dx ~ 20)
+      int c[3];
+      key_to_cell(gd, k, c);
       auto rel = [&](float v, int d) {
-        const float c = floorf(__fmul_rn(v, gd.inv_dx[d]));
-        return fminf(fmaxf(fmaf(-c, gd.dx[d], v) * gd.inv_dx[d], 0.f), 0.99999994f);
+        return fminf(fmaxf(fmaf(-(float)c[d], gd.dx[d], v) * gd.inv_dx[d], 0.f), 0.99999994f);
       };
       if (gd.n[0] > 1) x = rel(x, 0);
       if (gd.n[1] > 1) y = rel(y, 1);
       if (gd.n[2] > 1) z = rel(z, 2);
+      if (sp < 0 || sp >= gd.nsp) sp = 0;  // flagged by k_keys (PSC_F_SPECIES)
     }
-    if (in.x) out.x[s] = x;
-    out.y[s] = y;
-    out.z[s] = z;
-    out.ux[s] = ux;
-    out.uy[s] = uy;
-    out.uz[s] = uz;
-    out.qw[s] = qw;
-    out.sp[s] = sp;
-    if (in.id) out.id[s] = id;
+    if (in.x) out.x[o] = x;
+    out.y[o] = y;
+    out.z[o] = z;
+    out.ux[o] = ux;
+    out.uy[o] = uy;
+    out.uz[o] = uz;
+    out.qw[o] = qw;
+    out.sp[o] = sp;
+    if (in.id) out.id[o] = id;
   }
 }
 
+// ---- flattening the store -----------------------------------------------------------------------
 
-// ---- index sort of a pushed list -------------------------------------------------------------
-
-__device__ __forceinline__ int cell_to_key(const GridDesc &gd, const int c[3]) {
-  const int b0 = c[0] / gd.bs[0], b1 = c[1] / gd.bs[1], b2 = c[2] / gd.bs[2];
-  const int l0 = c[0] - b0 * gd.bs[0], l1 = c[1] - b1 * gd.bs[1], l2 = c[2] - b2 * gd.bs[2];
-  return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
+__device__ __forceinline__ int row_count(const uint8_t *__restrict__ dc, int k) {
+  const uint4 *p = reinterpret_cast<const uint4 *>(dc + (size_t)k * PSC_XCAP);
+  const uint4 r0 = p[0], r1 = p[1];
+  const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+  int c = 0;
+#pragma unroll
+  for (int q = 0; q < 8; q++) c += 4 - __popc(__vcmpeq4(w[q], 0xffffffffu) & 0x01010101u);
+  return c;
 }
 
-__device__ __forceinline__ int wrap(int c, int n) { return c < 0 ? c + n : (c >= n ? c - n : c); }
-
-// Keys of the 9 / 27 neighbours of a cell without a division per neighbour: the key is a sum of
-// one term per direction, key = sum_d (b_d * bstride_d * cpb + l_d * lstride_d), so three
-// candidate terms per direction (cell - 1, cell, cell + 1, periodic) give every neighbour by
-// three additions.
-struct NbKeys {
-  int t[3][3];
-  __device__ __forceinline__ void init(const GridDesc &gd, const int c[3]) {
-    int bstride = gd.cpb, lstride = 1;
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
-#pragma unroll
-      for (int s = -1; s <= 1; s++) {
-        const int q = wrap(c[d] + s, gd.n[d]);
-        const int b = q / gd.bs[d];
-        t[d][s + 1] = b * bstride + (q - b * gd.bs[d]) * lstride;
-      }
-      bstride *= gd.nb[d];
-      lstride *= gd.bs[d];
-    }
-  }
-  // neighbour in direction code dc (sign = +1) or the cell that reaches this one by dc (-1)
-  template <bool D3>
-  __device__ __forceinline__ int key(int dc, int sign) const {
-    const int s0 = D3 ? dc % 3 - 1 : 0;
-    const int s1 = D3 ? (dc / 3) % 3 - 1 : dc % 3 - 1;
-    const int s2 = D3 ? dc / 9 - 1 : dc / 3 - 1;
-    return t[0][sign * s0 + 1] + t[1][sign * s1 + 1] + t[2][sign * s2 + 1];
-  }
-};
-
-// per destination cell k: stayers (its own STAY count), arrivals (source cell k - dir sends
-// count[dir]); pack[k] = (stayers + arrivals) << 32 | arrivals for the packed scan
-template <bool D3>
+// tot[k] = residents of cell k + records waiting in its exchange row
 __global__ void __launch_bounds__(SORT_THREADS)
-k_dest_hist(GridDesc gd, const int *__restrict__ dircnt, int *__restrict__ nstay,
-            long long *__restrict__ pack) {
-  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= gd.nkeys) return;
-  int c[3];
-  key_to_cell(gd, k, c);
-  NbKeys nb;
-  nb.init(gd, c);
-  int na = 0;
-#pragma unroll
-  for (int dc = 0; dc < ND; dc++)
-    if (dc != STAY) na += dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)];
-  const int ns = dircnt[STAY * gd.nkeys + k];
-  nstay[k] = ns;
-  pack[k] = ((long long)(ns + na) << 32) | (long long)na;
+k_tot(int nk, const int *__restrict__ cnt, const uint8_t *__restrict__ dc, int *__restrict__ tot,
+      const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nk; k += gridDim.x * blockDim.x)
+    tot[k] = cnt[k] + row_count(dc, k);
 }
 
-// dircnt[dc][src] (count, dc != STAY) -> first arrival-list slot of the (src, dc) group, in
-// place: the arrivals of a cell are ordered by the direction they came from
-template <bool D3>
+// A warp per cell copies the cell's residents, then the records of its exchange row, to the dense
+// positions doffs[k] ...; key = the cell the offsets refer to (for a record: the destination of
+// its move).  ABS: positions become x = (cell + offset) * dx, formed in fp64 and rounded once.
+template <bool D3, bool ABS>
 __global__ void __launch_bounds__(SORT_THREADS)
-k_dir_base(GridDesc gd, int *__restrict__ dircnt, const int *__restrict__ aoffs) {
-  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= gd.nkeys) return;
-  int o = aoffs[k];
-  if (aoffs[k + 1] == o) return;  // no arrivals: every group is empty, its base unused
-  int c[3];
-  key_to_cell(gd, k, c);
-  NbKeys nb;
-  nb.init(gd, c);
-  int cnt[ND];  // all loads first: the stores below may alias them as far as the compiler knows
-#pragma unroll
-  for (int dc = 0; dc < ND; dc++) cnt[dc] = dc == STAY ? 0 : dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)];
-#pragma unroll
-  for (int dc = 0; dc < ND; dc++) {
-    if (dc == STAY) continue;
-    dircnt[dc * gd.nkeys + nb.key<D3>(dc, -1)] = o;
-    o += cnt[dc];
-  }
-}
-
-// A warp per source cell walks the cell's leaver region of the written list (behind its
-// stayers) and writes each leaver's slot into its group of the arrival list.  A region is a
-// handful of entries and every step is a dependent global load, so a warp works on RANK_U cells
-// at once: their table rows, then their first code chunks, are loaded back to back.
-constexpr int RANK_U = 4;
-
-template <bool D3>
-__global__ void __launch_bounds__(SORT_THREADS)
-k_rank(int nkeys, const int *__restrict__ offs_w, const uint8_t *__restrict__ dcode,
-       const int *__restrict__ dirbase, int *__restrict__ alist, uint32_t *__restrict__ flags) {
-  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  __shared__ int sb[SORT_THREADS / 32][RANK_U][32];
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+k_gather(GridDesc gd, Cols in, const int *__restrict__ base, const int *__restrict__ cnt,
+         Exchange xin, const int *__restrict__ doffs, Cols out, int *__restrict__ keyout,
+         const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int lane = threadIdx.x & 31;
   const int warps = gridDim.x * (SORT_THREADS / 32);
-  const unsigned lt = lanemask_lt();
-  for (int k0 = (blockIdx.x * (SORT_THREADS / 32) + w) * RANK_U; k0 < nkeys; k0 += warps * RANK_U) {
-    int p0[RANK_U], p1[RANK_U], dc0[RANK_U];
-#pragma unroll
-    for (int j = 0; j < RANK_U; j++) {
-      const int k = k0 + j;
-      const bool ok = k < nkeys;
-      const int b = (ok && lane < ND) ? dirbase[lane * nkeys + k] : 0;
-      sb[w][j][lane] = b;
-      p0[j] = (ok ? offs_w[k] : 0) + __shfl_sync(0xffffffffu, b, STAY);
-      p1[j] = ok ? offs_w[k + 1] : 0;
-    }
-#pragma unroll
-    for (int j = 0; j < RANK_U; j++) dc0[j] = p0[j] + lane < p1[j] ? (int)dcode[p0[j] + lane] : STAY;
-    __syncwarp();
-#pragma unroll
-    for (int j = 0; j < RANK_U; j++) {
-      for (int base = p0[j]; base < p1[j]; base += 32) {
-        const int s = base + lane;
-        bool act = s < p1[j];
-        int dc = base == p0[j] ? dc0[j] : (act ? (int)dcode[s] : STAY);
-        if (act && (dc >= ND || dc == STAY)) {  // cannot happen unless the workspace was scribbled over
-          atomicOr(flags, PSC_F_OOB);
-          act = false;
-        }
-        // rank inside the (cell, code) group: one ballot per distinct code present (a few);
-        // match.any would do it in one instruction but is an order of magnitude slower here
-        int rank = 0, cnt = 0;
-        unsigned rem = __ballot_sync(0xffffffffu, act);
-        while (rem) {
-          const int d = __shfl_sync(0xffffffffu, dc, __ffs(rem) - 1);
-          const unsigned m = __ballot_sync(0xffffffffu, act && dc == d);
-          if (act && dc == d) {
-            rank = __popc(m & lt);
-            cnt = __popc(m);
-          }
-          rem &= ~m;
-        }
-        int slot = 0;
-        if (act) slot = sb[w][j][dc] + rank;
-        __syncwarp();
-        if (act && rank == 0) sb[w][j][dc] += cnt;
-        __syncwarp();
-        if (act) alist[slot] = s;
-      }
-    }
-    __syncwarp();
-  }
-}
-
-// key of the particle in slot s of a list laid out by `offs`: the slot's cell, moved by the
-// particle's direction code if the slot lies in the cell's leaver region (behind the
-// dirtab[cell][STAY] stayers; dirtab == nullptr: a sorted list, nobody has moved)
-template <bool D3>
-__global__ void __launch_bounds__(SORT_THREADS)
-k_slot_keys(GridDesc gd, int n, const int *__restrict__ offs, const int *__restrict__ dirtab,
-            const uint8_t *__restrict__ dcode, int *__restrict__ key) {
-  constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4;
-  const int s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= n) return;
-  int lo = 0, hi = gd.nkeys;  // largest k with offs[k] <= s (and offs[k+1] > s)
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (offs[mid] <= s) lo = mid; else hi = mid;
-  }
-  int k = lo;
-  if (dirtab && s >= offs[k] + dirtab[STAY * gd.nkeys + k]) {
+  for (int k = blockIdx.x * (SORT_THREADS / 32) + (threadIdx.x >> 5); k < gd.nkeys; k += warps) {
+    const int n = cnt[k], d0 = doffs[k], nt = doffs[k + 1] - d0;
+    if (nt == 0) continue;
     int c[3];
     key_to_cell(gd, k, c);
-    int dc = (int)dcode[s];
-    if (dc >= ND) dc = STAY;
-    NbKeys nb;
-    nb.init(gd, c);
-    k = nb.key<D3>(dc, +1);
+    auto absf = [&](float off, int cell, int d) {
+      float v = __double2float_rn(((double)cell + (double)off) * (double)gd.dx[d]);
+      if (v >= gd.L[d]) v = nextafterf(gd.L[d], 0.f);  // rounding must not leave [0, L)
+      return v;
+    };
+    const size_t b = (size_t)base[k];
+    for (int i = lane; i < n; i += 32) {
+      const size_t s = b + i, o = (size_t)d0 + i;
+      float x = in.x ? in.x[s] : 0.f, y = in.y[s], z = in.z[s];
+      if (ABS) {
+        if (D3) x = absf(x, c[0], 0);
+        y = absf(y, c[1], 1);
+        z = absf(z, c[2], 2);
+      }
+      if (out.x) out.x[o] = x;
+      out.y[o] = y;
+      out.z[o] = z;
+      out.ux[o] = in.ux[s];
+      out.uy[o] = in.uy[s];
+      out.uz[o] = in.uz[s];
+      out.qw[o] = in.qw[s];
+      out.sp[o] = in.sp[s];
+      if (out.id) out.id[o] = in.id ? in.id[s] : 0;
+      if (keyout) keyout[o] = k;
+    }
+    if (nt > n) {  // the row's records, in row order
+      const int dc = (int)xin.dc[(size_t)k * PSC_XCAP + lane];
+      const bool have = dc != (int)PSC_XDC_NONE;
+      const unsigned m = __ballot_sync(0xffffffffu, have);
+      if (have) {
+        const size_t idx = (size_t)k * PSC_XCAP + lane, o = (size_t)d0 + n + __popc(m & lanemask_lt());
+        const XRec r = xin.rec[idx];
+        int sx, sy, sz;
+        dir_decode<D3>(dc, sx, sy, sz);
+        const int cx = D3 ? wrap_cell(c[0] + sx, gd.n[0]) : 0, cy = wrap_cell(c[1] + sy, gd.n[1]),
+                  cz = wrap_cell(c[2] + sz, gd.n[2]);
+        float w[8] = {__uint_as_float(r.a.x), __uint_as_float(r.a.y), __uint_as_float(r.a.z), __uint_as_float(r.a.w),
+                      __uint_as_float(r.b.x), __uint_as_float(r.b.y), __uint_as_float(r.b.z), __uint_as_float(r.b.w)};
+        float x = D3 ? w[0] : w[7], y = D3 ? w[1] : w[0], z = D3 ? w[2] : w[1];
+        if (ABS) {
+          if (D3) x = absf(x, cx, 0);
+          y = absf(y, cy, 1);
+          z = absf(z, cz, 2);
+        }
+        if (out.x) out.x[o] = x;
+        out.y[o] = y;
+        out.z[o] = z;
+        out.ux[o] = D3 ? w[3] : w[2];
+        out.uy[o] = D3 ? w[4] : w[3];
+        out.uz[o] = D3 ? w[5] : w[4];
+        out.qw[o] = D3 ? w[6] : w[5];
+        out.sp[o] = __float_as_int(D3 ? w[7] : w[6]);
+        if (out.id) out.id[o] = xin.id ? xin.id[idx] : 0;
+        if (keyout) keyout[o] = cell_key(gd, cx, cy, cz);
+      }
+    }
   }
-  key[s] = k;
+}
+
+// the spill list follows the cells: dense positions doffs[nkeys] ...; *ntotal := all particles
+template <bool D3, bool ABS>
+__global__ void __launch_bounds__(SORT_THREADS)
+k_gather_spill(GridDesc gd, Spill sp, const int *__restrict__ doffs, Cols out, int *__restrict__ keyout,
+               int *__restrict__ ntotal, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int ns = min(*sp.count, sp.cap), d0 = doffs[gd.nkeys];
+  if (blockIdx.x == 0 && threadIdx.x == 0) *ntotal = d0 + ns;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < ns; i += gridDim.x * blockDim.x) {
+    const XRec r = sp.rec[i];
+    const int k = sp.key[i];
+    const size_t o = (size_t)d0 + i;
+    int c[3];
+    key_to_cell(gd, k, c);
+    auto absf = [&](float off, int cell, int d) {
+      float v = __double2float_rn(((double)cell + (double)off) * (double)gd.dx[d]);
+      if (v >= gd.L[d]) v = nextafterf(gd.L[d], 0.f);
+      return v;
+    };
+    float w[8] = {__uint_as_float(r.a.x), __uint_as_float(r.a.y), __uint_as_float(r.a.z), __uint_as_float(r.a.w),
+                  __uint_as_float(r.b.x), __uint_as_float(r.b.y), __uint_as_float(r.b.z), __uint_as_float(r.b.w)};
+    float x = D3 ? w[0] : w[7], y = D3 ? w[1] : w[0], z = D3 ? w[2] : w[1];
+    if (ABS) {
+      if (D3) x = absf(x, c[0], 0);
+      y = absf(y, c[1], 1);
+      z = absf(z, c[2], 2);
+    }
+    if (out.x) out.x[o] = x;
+    out.y[o] = y;
+    out.z[o] = z;
+    out.ux[o] = D3 ? w[3] : w[2];
+    out.uy[o] = D3 ? w[4] : w[3];
+    out.uz[o] = D3 ? w[5] : w[4];
+    out.qw[o] = D3 ? w[6] : w[5];
+    out.sp[o] = __float_as_int(D3 ? w[7] : w[6]);
+    if (out.id) out.id[o] = sp.id ? sp.id[i] : 0;
+    if (keyout) keyout[o] = k;
+  }
+}
+
+// after a (re-)layout: every exchange row empty, nothing spilled; records the slots in use
+__global__ void __launch_bounds__(SORT_THREADS)
+k_store_reset(int nk, uint8_t *__restrict__ dc0, uint8_t *__restrict__ dc1, const int *__restrict__ base,
+              uint32_t *__restrict__ dw, long long capacity, const uint32_t *__restrict__ cond) {
+  PSC_COND_RETURN(cond);
+  const int m = nk * (PSC_XCAP / 4);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) {
+    reinterpret_cast<unsigned *>(dc0)[i] = 0xffffffffu;
+    reinterpret_cast<unsigned *>(dc1)[i] = 0xffffffffu;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    dw[PSC_DW_SLOTS] = (uint32_t)base[nk];
+    if ((long long)base[nk] > capacity) atomicOr(&dw[PSC_DW_FLAGS], PSC_F_OVERFLOW);
+  }
+}
+
+// last launch of a conditional re-layout (grid of one block): clears the condition itself
+__global__ void k_relayout_done(uint32_t *__restrict__ dw) {
+  if (threadIdx.x == 0 && dw[PSC_DW_SPILL]) {
+    dw[PSC_DW_SPILL] = 0;
+    dw[PSC_DW_RELAYOUTS]++;
+  }
 }
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+// slots per column a store of n particles can need (see cell_capacity)
+int64_t psc_store_capacity(const psc_ctx *c, int64_t n) {
+  const int64_t v = n + n / 8 + 48 * (int64_t)c->gd.nkeys;
+  return (v + 31) / 32 * 32;
+}
+
+static int64_t spill_capacity(int64_t n) { return n / 16 > 4096 ? n / 16 : 4096; }
+
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
+  const size_t nx = nk * PSC_XCAP;
   size_t b = 0;
-  b += 5 * align_up((size_t)n * 4, 256);                      // key, curkey, perm, cell_idx, alist
-  b += align_up((size_t)n, 256);                              // dcode
-  b += 5 * align_up((nk + 1) * 4, 256);                       // offs[2], cursor, aoffs, nstay
+  b += 3 * align_up((size_t)n * 4 + 4, 256);                  // key, perm, cell_idx
+  b += 6 * align_up((nk + 1) * 4, 256);                       // offs_dense, base, cnt, cursor, tot, doffs
   b += 2 * align_up((nk + 1) * 8, 256);                       // pack, packloc
-  b += align_up(nk * 27 * 4, 256);                            // dircnt
   b += align_up((nk / SCAN_TILE + 3) * 8, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
+  b += 2 * (align_up(nx * sizeof(XRec), 256) + align_up(nx, 256) + align_up(nx * 4, 256));  // exchange x2
+  const size_t sc = (size_t)spill_capacity(n);
+  b += align_up(sc * sizeof(XRec), 256) + 2 * align_up(sc * 4, 256);  // spill
   return b;
 }
 
 int psc_sort_carve(psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
+  const size_t nx = nk * PSC_XCAP;
   char *p = (char *)c->ws;
   auto take = [&](size_t bytes) {
     void *r = p;
     p += align_up(bytes, 256);
     return r;
   };
-  c->key = (int32_t *)take((size_t)n * 4);
-  c->curkey = (int32_t *)take((size_t)n * 4);
-  c->perm = (int32_t *)take((size_t)n * 4);
-  c->cell_idx = (int32_t *)take((size_t)n * 4);
-  c->alist = (int32_t *)take((size_t)n * 4);
-  c->dcode = (uint8_t *)take((size_t)n);
-  c->offs[0] = (int32_t *)take((nk + 1) * 4);
-  c->offs[1] = (int32_t *)take((nk + 1) * 4);
+  c->key = (int32_t *)take((size_t)n * 4 + 4);
+  c->perm = (int32_t *)take((size_t)n * 4 + 4);
+  c->cell_idx = (int32_t *)take((size_t)n * 4 + 4);
+  c->offs_dense = (int32_t *)take((nk + 1) * 4);
+  c->base = (int32_t *)take((nk + 1) * 4);
+  c->cnt = (int32_t *)take((nk + 1) * 4);
   c->cursor = (int32_t *)take((nk + 1) * 4);
-  c->aoffs = (int32_t *)take((nk + 1) * 4);
-  c->nstay = (int32_t *)take((nk + 1) * 4);
+  c->tot = (int32_t *)take((nk + 1) * 4);
+  c->doffs = (int32_t *)take((nk + 1) * 4);
   c->pack = (long long *)take((nk + 1) * 8);
   c->packloc = (long long *)take((nk + 1) * 8);
-  c->dircnt = (int32_t *)take(nk * 27 * 4);
   c->scan_tmp = (long long *)take((nk / SCAN_TILE + 3) * 8);
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
+  for (int i = 0; i < 2; i++) {
+    c->xch[i].rec = (XRec *)take(nx * sizeof(XRec));
+    c->xch[i].dc = (uint8_t *)take(nx);
+    c->xch[i].id = (int32_t *)take(nx * 4);
+  }
+  const size_t sc = (size_t)spill_capacity(n);
+  c->spill.rec = (XRec *)take(sc * sizeof(XRec));
+  c->spill.key = (int32_t *)take(sc * 4);
+  c->spill.id = (int32_t *)take(sc * 4);
+  c->spill.count = (int32_t *)(c->d_flags + PSC_DW_SPILL);
+  c->spill.cap = (int)sc;
   if ((size_t)(p - (char *)c->ws) > c->ws_bytes) return PSC_ERR_WORKSPACE;
   return PSC_OK;
 }
 
+// what the particle kernels see: the current column set in buffer-column order, the exchange
+// the last push filled (xin) and the one the next push fills (xout)
+StoreDesc psc_store_desc(const psc_ctx *c) {
+  StoreDesc sd;
+  const Cols &p = c->cols[c->cur];
+  const bool d3 = psc_is3d(c->gd);
+  for (int i = 0; i < 10; i++) sd.col[i] = nullptr;
+  int k = 0;
+  if (d3) sd.col[k++] = p.x;
+  sd.col[k++] = p.y;
+  sd.col[k++] = p.z;
+  sd.col[k++] = p.ux;
+  sd.col[k++] = p.uy;
+  sd.col[k++] = p.uz;
+  sd.ndyn = k;
+  sd.col[k++] = p.qw;
+  sd.col[k++] = (float *)p.sp;
+  sd.icol_x2d = sd.icol_id = -1;
+  if (!d3 && p.x) { sd.icol_x2d = k; sd.col[k++] = p.x; }
+  if (p.id) { sd.icol_id = k; sd.col[k++] = (float *)p.id; }
+  sd.ncol = k;
+  sd.base = c->base;
+  sd.cnt = c->cnt;
+  sd.xin = c->xch[c->xcur];
+  sd.xout = c->xch[c->xcur ^ 1];
+  if (!p.id) sd.xin.id = sd.xout.id = nullptr;
+  sd.spill = c->spill;
+  if (!p.id) sd.spill.id = nullptr;
+  sd.C = c->bufC;
+  sd.flags = c->d_flags + PSC_DW_FLAGS;
+  return sd;
+}
+
 namespace {
 
-inline bool is3d(const GridDesc &gd) { return gd.n[0] > 1; }
-
-// exclusive scan of the histogram in c->cursor -> out (and cursor := out)
-int run_scan(psc_ctx *c, int32_t *out, cudaStream_t s) {
+// packed scan of c->pack -> base (capacities), offs_dense (counts), cursor := offs_dense
+int run_scan2(psc_ctx *c, cudaStream_t s, const uint32_t *cond) {
   const int nk = c->gd.nkeys;
   ProfScope ps(c, PSC_PH_SORT_SCAN, s);
+  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
+  k_scan_local<long long><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->pack, c->packloc, c->scan_tmp, cond);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_tmp<long long><<<1, 1024, 0, s>>>(sblocks, c->scan_tmp, cond);
+  PSC_LAUNCH_CHECK(c);
+  k_scan_add2<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->packloc, c->base, c->offs_dense, c->cursor,
+                                               c->scan_tmp, sblocks, cond);
+  PSC_LAUNCH_CHECK(c);
+  return PSC_OK;
+}
+
+// exclusive scan tot -> doffs
+int run_scan1(psc_ctx *c, cudaStream_t s, const uint32_t *cond) {
+  const int nk = c->gd.nkeys;
   const int sblocks = (int)cdiv64(nk, SCAN_TILE);
   int *tmp = (int *)c->scan_tmp;
-  k_scan_local<int><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->cursor, out, tmp);
+  k_scan_local<int><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->tot, c->doffs, tmp, cond);
   PSC_LAUNCH_CHECK(c);
-  k_scan_tmp<int><<<1, 1024, 0, s>>>(sblocks, tmp);
+  k_scan_tmp<int><<<1, 1024, 0, s>>>(sblocks, tmp, cond);
   PSC_LAUNCH_CHECK(c);
-  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, out, c->cursor, tmp, sblocks);
-  PSC_LAUNCH_CHECK(c);
-  return PSC_OK;
-}
-
-// packed scan of c->pack -> out_hi (cell offsets), out_lo (arrival-list offsets)
-int run_scan2(psc_ctx *c, int32_t *out_hi, int32_t *out_lo, cudaStream_t s) {
-  const int nk = c->gd.nkeys;
-  ProfScope ps(c, PSC_PH_SORT_SCAN, s);
-  const int sblocks = (int)cdiv64(nk, SCAN_TILE);
-  k_scan_local<long long><<<sblocks, SORT_THREADS, 0, s>>>(nk, c->pack, c->packloc, c->scan_tmp);
-  PSC_LAUNCH_CHECK(c);
-  k_scan_tmp<long long><<<1, 1024, 0, s>>>(sblocks, c->scan_tmp);
-  PSC_LAUNCH_CHECK(c);
-  k_scan_add2<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->packloc, out_hi, out_lo, c->scan_tmp, sblocks);
+  k_scan_add<<<sblocks, SORT_THREADS, 0, s>>>(nk, c->doffs, nullptr, tmp, sblocks, cond);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
 
-// key[s] of the particles of the current column set, in their current order
-int slot_keys(psc_ctx *c, int32_t *key, cudaStream_t s) {
-  const int n = (int)c->np;
-  if (n == 0) return PSC_OK;
-  const int32_t *offs, *dirtab = nullptr;
-  switch (c->state) {
-    case PSC_STATE_SORTED: offs = c->offs[c->ocur]; break;
-    case PSC_STATE_PUSHED: offs = c->offs[c->ocur]; dirtab = c->dircnt; break;
-    case PSC_STATE_INDEXED: offs = c->offs[c->ocur ^ 1]; dirtab = c->dircnt; break;
-    default: return PSC_ERR_NOT_SORTED;
+int grid_for(const psc_ctx *c, int64_t items, int per_block) {
+  return (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(items, per_block)));
+}
+
+// flattens the store of the current set into `dst` (dense), keys into keyout; *ntotal (device)
+// receives the particle count
+int gather_store(psc_ctx *c, const Cols &dst, int32_t *keyout, bool to_abs, int *ntotal, cudaStream_t s,
+                 const uint32_t *cond) {
+  const GridDesc &gd = c->gd;
+  const int nk = gd.nkeys;
+  const Cols &in = c->cols[c->cur];
+  const Exchange &xin = c->xch[c->xcur];
+  Exchange xi = xin;
+  Spill sp = c->spill;
+  if (!in.id) { xi.id = nullptr; sp.id = nullptr; }
+  k_tot<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk, c->cnt, xin.dc, c->tot, cond);
+  PSC_LAUNCH_CHECK(c);
+  int rc = run_scan1(c, s, cond);
+  if (rc) return rc;
+  const int gb = grid_for(c, nk, SORT_THREADS / 32);
+  const int sb = grid_for(c, c->spill.cap, SORT_THREADS);
+  const bool d3 = psc_is3d(gd);
+#define PSC_GATHER(D3_, ABS_)                                                                        \
+  do {                                                                                               \
+    k_gather<D3_, ABS_><<<gb, SORT_THREADS, 0, s>>>(gd, in, c->base, c->cnt, xi, c->doffs, dst, keyout, cond); \
+    PSC_LAUNCH_CHECK(c);                                                                             \
+    k_gather_spill<D3_, ABS_><<<sb, SORT_THREADS, 0, s>>>(gd, sp, c->doffs, dst, keyout, ntotal, cond);       \
+    PSC_LAUNCH_CHECK(c);                                                                             \
+  } while (0)
+  if (d3 && to_abs) PSC_GATHER(true, true);
+  else if (d3) PSC_GATHER(true, false);
+  else if (to_abs) PSC_GATHER(false, true);
+  else PSC_GATHER(false, false);
+#undef PSC_GATHER
+  return PSC_OK;
+}
+
+// counting sort of the dense list `src` (keys in c->key, histogram in c->cursor, *np particles)
+// into the store layout in `dst`
+int sort_core(psc_ctx *c, const Cols &src, const Cols &dst, bool from_abs, bool stable, const int *np,
+              cudaStream_t s, const uint32_t *cond) {
+  const GridDesc &gd = c->gd;
+  const int nk = gd.nkeys;
+  const int pblocks = grid_for(c, c->np, SORT_THREADS);
+  k_layout<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk, c->cursor, c->pack, c->cnt, c->d_flags, cond);
+  PSC_LAUNCH_CHECK(c);
+  int rc = run_scan2(c, s, cond);
+  if (rc) return rc;
+  psc_prof_begin(c, PSC_PH_SORT_RANK, s);
+  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(np, c->key, c->cursor, c->perm, cond);
+  PSC_LAUNCH_CHECK(c);
+  if (stable) {
+    const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
+    k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, c->offs_dense, c->perm, c->big_list, c->d_flags + PSC_DW_BIG);
+    PSC_LAUNCH_CHECK(c);
+    if (c->np > WARP_SEG_CAP) {
+      static bool attr_set = false;
+      if (!attr_set) {
+        PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_segsort_big, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             BIG_SMEM_CAP * 4));
+        attr_set = true;
+      }
+      k_segsort_big<<<c->sm_count, 1024, BIG_SMEM_CAP * 4, s>>>(c->offs_dense, c->perm, c->big_list,
+                                                                c->d_flags + PSC_DW_BIG);
+      PSC_LAUNCH_CHECK(c);
+    }
   }
-  const int blocks = (int)cdiv64(n, SORT_THREADS);
-  if (is3d(c->gd)) k_slot_keys<true><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dirtab, c->dcode, key);
-  else k_slot_keys<false><<<blocks, SORT_THREADS, 0, s>>>(c->gd, n, offs, dirtab, c->dcode, key);
+  psc_prof_end(c, PSC_PH_SORT_RANK, s);
+  psc_prof_begin(c, PSC_PH_SORT_REORDER, s);
+  if (from_abs)
+    k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, np, c->perm, c->key, c->offs_dense, c->base, src, dst, cond);
+  else
+    k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, np, c->perm, c->key, c->offs_dense, c->base, src, dst, cond);
+  PSC_LAUNCH_CHECK(c);
+  psc_prof_end(c, PSC_PH_SORT_REORDER, s);
+  k_store_reset<<<grid_for(c, (int64_t)nk * 8, SORT_THREADS), SORT_THREADS, 0, s>>>(
+      nk, c->xch[0].dc, c->xch[1].dc, c->base, c->d_flags, (long long)c->capacity, cond);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }
 
 }  // namespace
 
-// key[] (c->curkey) := keys of the current particles, in their current order
-int psc_sort_current_keys(psc_ctx *c, cudaStream_t s) { return slot_keys(c, c->curkey, s); }
+int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cudaStream_t s) {
+  return gather_store(c, dst, key, to_abs, c->key + c->np /* scratch word behind key[] */, s, nullptr);
+}
 
-// general counting sort: arbitrary order in, physically sorted (stable) list out
+// general counting sort: any state in, the cell store (stable inside every cell) out
 int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const GridDesc &gd = c->gd;
   const int n = (int)c->np;
   const int nk = gd.nkeys;
-  const Cols &in = c->cols[c->cur];
-  const Cols &out = c->cols[c->cur ^ 1];
-  const int pblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(n, SORT_THREADS)));
-
-  if (c->form == PSC_FORM_REL) {  // a sorted or pushed list sorted again: keys from the slots
-    const int rc = slot_keys(c, c->key, s);
-    if (rc) return rc;
-    if (c->state == PSC_STATE_INDEXED) c->ocur ^= 1;  // back to the layout of the written list
-  }
-  int32_t *offs_new = c->offs[c->ocur ^ 1];
+  const int pblocks = grid_for(c, n, SORT_THREADS);
+  int *np_dev = c->key + c->np;  // one scratch word behind key[]: the particle count on the device
   PSC_CUDA_TRY(c, cudaMemsetAsync(c->cursor, 0, (size_t)(nk + 1) * 4, s));
-  PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + 1, 0, 4, s));
-  c->launches += 2;
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + PSC_DW_BIG, 0, 4, s));
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + PSC_DW_MAXCNT, 0, 4, s));
+  c->launches += 3;
+  const bool from_abs = c->form == PSC_FORM_ABS;
+  const Cols &src = c->cols[from_abs ? c->cur : c->cur ^ 1];
+  const Cols &dst = c->cols[from_abs ? c->cur ^ 1 : c->cur];
   psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
-  if (c->form == PSC_FORM_ABS)
-    k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, in.x, in.y, in.z, c->key, c->cursor, c->d_flags);
-  else
-    k_hist<<<pblocks, SORT_THREADS, 0, s>>>(n, nk, c->key, c->cursor, c->d_flags);
-  PSC_LAUNCH_CHECK(c);
-  psc_prof_end(c, PSC_PH_SORT_COUNT, s);
-  {
-    const int rc = run_scan(c, offs_new, s);
+  if (from_abs) {
+    c->np32 = n;
+    PSC_CUDA_TRY(c, cudaMemcpyAsync(np_dev, &c->np32, 4, cudaMemcpyHostToDevice, s));
+    k_keys<<<pblocks, SORT_THREADS, 0, s>>>(gd, n, src.x, src.y, src.z, src.sp, c->key, c->cursor,
+                                            c->d_flags + PSC_DW_FLAGS);
+    PSC_LAUNCH_CHECK(c);
+  } else {  // a store sorted again: flatten it into the other set, keys from the cells
+    const int rc = gather_store(c, src, c->key, false, np_dev, s, nullptr);
     if (rc) return rc;
-  }
-  psc_prof_begin(c, PSC_PH_SORT_RANK, s);
-  k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(n, c->key, c->cursor, c->perm);
-  PSC_LAUNCH_CHECK(c);
-  const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
-  k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, offs_new, c->perm, c->big_list, c->d_flags + 1);
-  PSC_LAUNCH_CHECK(c);
-  if (n > WARP_SEG_CAP) {
-    static bool attr_set = false;
-    if (!attr_set) {
-      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_segsort_big, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           BIG_SMEM_CAP * 4));
-      attr_set = true;
-    }
-    k_segsort_big<<<c->sm_count, 1024, BIG_SMEM_CAP * 4, s>>>(offs_new, c->perm, c->big_list,
-                                                              c->d_flags + 1);
+    k_hist<<<pblocks, SORT_THREADS, 0, s>>>(np_dev, nk, c->key, c->cursor, c->d_flags + PSC_DW_FLAGS, nullptr);
     PSC_LAUNCH_CHECK(c);
   }
-  psc_prof_end(c, PSC_PH_SORT_RANK, s);
-  psc_prof_begin(c, PSC_PH_SORT_REORDER, s);
-  if (c->form == PSC_FORM_ABS) k_reorder<true><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out);
-  else k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, n, c->perm, in, out);
-  PSC_LAUNCH_CHECK(c);
-  psc_prof_end(c, PSC_PH_SORT_REORDER, s);
-  c->cur ^= 1;
-  c->ocur ^= 1;
+  psc_prof_end(c, PSC_PH_SORT_COUNT, s);
+  {
+    const int rc = sort_core(c, src, dst, from_abs, true, np_dev, s, nullptr);
+    if (rc) return rc;
+  }
+  PSC_CUDA_TRY(c, cudaMemsetAsync(c->d_flags + PSC_DW_SPILL, 0, 4, s));
+  if (from_abs) c->cur ^= 1;
+  c->xcur = 0;
   c->form = PSC_FORM_REL;
-  c->state = PSC_STATE_SORTED;
+  c->state = PSC_STATE_STORE;
   c->have_sort_result = 1;
+  // size of the per-warp cell image of the particle kernels: the largest cell plus room for its
+  // arrivals (read back: this call synchronises the stream)
+  uint32_t dw[PSC_DW_COUNT];
+  PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, s));
+  PSC_CUDA_TRY(c, cudaStreamSynchronize(s));
+  const int mx = (int)dw[PSC_DW_MAXCNT];
+  int C = (mx + mx / 8 + 24 + 31) / 32 * 32;
+  c->bufC = C < 64 ? 64 : (C > 256 ? 256 : C);
+  if ((int64_t)dw[PSC_DW_SLOTS] > c->capacity) return PSC_ERR_WORKSPACE;
   return PSC_OK;
 }
 
-// index sort of a pushed list: new cell offsets + the arrival list from the per-cell direction
-// counts and the leavers' direction codes; no column moves
-int psc_sort_index(psc_ctx *c, cudaStream_t s) {
-  const GridDesc &gd = c->gd;
-  const int nk = gd.nkeys;
-  const int32_t *offs_w = c->offs[c->ocur];  // layout of the written list
-  int32_t *offs_new = c->offs[c->ocur ^ 1];
-  const int cblocks = (int)cdiv64(nk, SORT_THREADS);
-  const bool d3 = is3d(gd);
-  psc_prof_begin(c, PSC_PH_SORT_COUNT, s);
-  if (d3) k_dest_hist<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->nstay, c->pack);
-  else k_dest_hist<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->nstay, c->pack);
+// in the steady state nothing is sorted.  Only if the last push spilled
+// (device word PSC_DW_SPILL != 0) the store is flattened and laid out again; the launches below
+// return immediately otherwise.
+int psc_store_relayout_if_spilled(psc_ctx *c, cudaStream_t s) {
+  const int nk = c->gd.nkeys;
+  const uint32_t *cond = c->d_flags + PSC_DW_SPILL;
+  int *np_dev = c->key + c->np;
+  const Cols &tmp = c->cols[c->cur ^ 1];
+  const Cols &dst = c->cols[c->cur];
+  int rc = gather_store(c, tmp, c->key, false, np_dev, s, cond);
+  if (rc) return rc;
+  k_zero<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk + 1, c->cursor, cond);
   PSC_LAUNCH_CHECK(c);
-  psc_prof_end(c, PSC_PH_SORT_COUNT, s);
-  {
-    const int rc = run_scan2(c, offs_new, c->aoffs, s);
-    if (rc) return rc;
-  }
-  psc_prof_begin(c, PSC_PH_SORT_RANK, s);
-  if (d3) k_dir_base<true><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
-  else k_dir_base<false><<<cblocks, SORT_THREADS, 0, s>>>(gd, c->dircnt, c->aoffs);
+  k_hist<<<grid_for(c, c->np, SORT_THREADS), SORT_THREADS, 0, s>>>(np_dev, nk, c->key, c->cursor,
+                                                                  c->d_flags + PSC_DW_FLAGS, cond);
   PSC_LAUNCH_CHECK(c);
-  const int rblocks = (int)min((int64_t)c->sm_count * 32, max((int64_t)1, cdiv64(nk, (SORT_THREADS / 32) * 4)));
-  if (d3) k_rank<true><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
-  else k_rank<false><<<rblocks, SORT_THREADS, 0, s>>>(nk, offs_w, c->dcode, c->dircnt, c->alist, c->d_flags);
+  rc = sort_core(c, tmp, dst, false, false, np_dev, s, cond);
+  if (rc) return rc;
+  k_relayout_done<<<1, 32, 0, s>>>(c->d_flags);
   PSC_LAUNCH_CHECK(c);
-  psc_prof_end(c, PSC_PH_SORT_RANK, s);
-  c->ocur ^= 1;
-  c->state = PSC_STATE_INDEXED;
   c->have_sort_result = 0;
   return PSC_OK;
 }
@@ -805,20 +911,5 @@ int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s) {
   if (n == 0) return PSC_OK;
   k_cell_idx<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->key, c->cell_idx);
   PSC_LAUNCH_CHECK(c);
-  return PSC_OK;
-}
-
-int psc_particles_to_abs(psc_ctx *c, cudaStream_t s) {
-  const int n = (int)c->np;
-  if (n) {
-    const int rc = psc_sort_current_keys(c, s);
-    if (rc) return rc;
-    const Cols &p = c->cols[c->cur];
-    k_to_abs<<<(int)cdiv64(n, SORT_THREADS), SORT_THREADS, 0, s>>>(c->gd, n, c->curkey, p.x, p.y, p.z);
-    PSC_LAUNCH_CHECK(c);
-  }
-  c->form = PSC_FORM_ABS;
-  c->state = PSC_STATE_UNSORTED;
-  c->have_sort_result = 0;
   return PSC_OK;
 }

@@ -1,0 +1,473 @@
+// store.cuh -- device side of the cell store (psc_internal.cuh): how a warp
+// streams one cell's particles through shared memory.
+//
+// a particle moves at most one cell per step, so the per-step "sort" only has to
+// deal with the few particles that change cell, and the reorder can be folded into the next
+// push's load ("only one loop each time step that reads and writes all particle data").  Here:
+//   * a cell's resident particles are one 128-byte-aligned run per column; the warp that owns the
+//     cell fetches the whole run with ONE bulk asynchronous copy per column (cp.async.bulk ->
+//     UBLKCP: issued by one lane, executed by the copy engine, completion counted on an mbarrier),
+//     so the SM's load/store pipe never sees the particle stream;
+//   * the warp advances the particles in that shared-memory image IN PLACE, and writes the image's
+//     dynamic columns (positions, momenta) back with one bulk copy per column; q*w, species, id of
+//     a particle that stays in its cell are never rewritten;
+//   * a particle that leaves is appended, as one 32-byte record tagged with the direction code of
+//     its move, to the exchange row of its SOURCE cell (ping-pong buffered);
+//   * the arrivals of a cell are the records of its 8 / 26 neighbours' rows whose code points at
+//     it; they are pushed together with the residents (in the idle lanes of the cell's last
+//     chunk) and filed into the holes the cell's own leavers left, else appended, so that
+//     [0, cnt) stays dense; holes left over are closed by moving particles from the tail.
+// A cell that does not fit the image (more than C particles) is streamed straight from and to
+// global memory with an in-place compaction instead (rare; correct for any size).  A particle that
+// finds no room (row or cell full) goes to the spill list; the next step then re-lays the store
+// out before pushing (sort.cu).
+#pragma once
+#include "push_common.cuh"
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t *b, unsigned parity) {
+  unsigned ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(b)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, unsigned parity) {
+  while (!mbar_try_wait(b, parity)) {
+  }
+}
+// global -> shared bulk copy (16-byte aligned, size a multiple of 16), completion on `bar`
+__device__ __forceinline__ void bulk_g2s(void *sdst, const void *gsrc, unsigned bytes, uint64_t *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(sdst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// shared -> global bulk copy, tracked by the issuing thread's bulk group
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *ssrc, unsigned bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// cell key (block-major, cell-minor) of periodic cell coordinates
+__device__ __forceinline__ int wrap_cell(int c, int n) { return c < 0 ? c + n : (c >= n ? c - n : c); }
+__device__ __forceinline__ int cell_key(const GridDesc &gd, int cx, int cy, int cz) {
+  const int b0 = cx / gd.bs[0], b1 = cy / gd.bs[1], b2 = cz / gd.bs[2];
+  const int l0 = cx - b0 * gd.bs[0], l1 = cy - b1 * gd.bs[1], l2 = cz - b2 * gd.bs[2];
+  return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
+}
+template <bool D3>
+__device__ __forceinline__ void dir_decode(int dc, int &sx, int &sy, int &sz) {
+  if (D3) {
+    sx = dc % 3 - 1;
+    sy = (dc / 3) % 3 - 1;
+    sz = dc / 9 - 1;
+  } else {
+    sx = 0;
+    sy = dc % 3 - 1;
+    sz = dc / 3 - 1;
+  }
+}
+
+// a particle that found no room in its exchange row or its destination cell
+static __device__ __noinline__ void spill_record(Spill sp, uint32_t *flags, int key, uint4 a, uint4 b, int id) {
+  const int i = atomicAdd(sp.count, 1);
+  if (i < sp.cap) {
+    XRec r;
+    r.a = a;
+    r.b = b;
+    sp.rec[i] = r;
+    sp.key[i] = key;
+    if (sp.id) sp.id[i] = id;
+  } else {
+    atomicOr(flags, PSC_F_OVERFLOW);  // the particle is lost: the workspace was sized for fewer particles
+  }
+}
+__device__ __forceinline__ void spill_particle(const StoreDesc &sd, int key, const float (&w)[8], int id) {
+  spill_record(sd.spill, sd.flags, key,
+               make_uint4(__float_as_uint(w[0]), __float_as_uint(w[1]), __float_as_uint(w[2]), __float_as_uint(w[3])),
+               make_uint4(__float_as_uint(w[4]), __float_as_uint(w[5]), __float_as_uint(w[6]), __float_as_uint(w[7])), id);
+}
+
+// One particle in registers: in-cell offsets a*, momenta, the static values.
+struct Part {
+  float ax, ay, az, ux, uy, uz, qw;
+  int sp;
+};
+
+constexpr int WALK_AC = 128;  // arrival-list window (entries)
+
+// Per-warp view of the store.  XC: optional columns (id, carried x of a 2-d run) may be bound.
+template <bool D3, bool XC>
+struct CellWalker {
+  static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4, NDYN = D3 ? 6 : 5;
+  // bytes of per-warp shared memory for an image of C slots x ncol columns
+  __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
+    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + PSC_XCAP /*xrow*/ + 16 /*bar*/;
+  }
+  float *buf;      // [ncol][C]
+  uint8_t *holes;  // [C]
+  uint16_t *arr;   // [WALK_AC]
+  int *nbk;        // [32]
+  uint8_t *xrow;   // [PSC_XCAP]
+  uint64_t *bar;
+  int C, ncol, lane;
+  unsigned lt;
+  unsigned parity;
+  bool loads_armed;  // bulk loads for the cell about to be processed are in flight
+  // current cell
+  int key, n, na, base, cap;
+  bool fast;
+  int nh, tcur, nleave, a0, my_start;
+
+  __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_) {
+    C = sd.C;
+    ncol = sd.ncol;
+    lane = lane_;
+    lt = lanemask_lt_();
+    buf = (float *)wsm;
+    holes = (uint8_t *)(buf + ncol * C);
+    arr = (uint16_t *)(holes + C);
+    nbk = (int *)(arr + WALK_AC);
+    xrow = (uint8_t *)(nbk + 32);
+    bar = (uint64_t *)(xrow + PSC_XCAP);
+    parity = 0;
+    loads_armed = false;
+    xrow[lane] = PSC_XDC_NONE;
+    if (lane == 0) {
+      mbar_init(bar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+  }
+
+  // lane 0: fetch the resident run of a cell into the image (n <= C)
+  __device__ __forceinline__ void issue_loads(const StoreDesc &sd, int n_, int base_) {
+    loads_armed = n_ > 0 && n_ <= C;
+    if (loads_armed && lane == 0) {
+      const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
+      mbar_expect_tx(bar, bytes * (unsigned)ncol);
+      for (int c = 0; c < ncol; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
+    }
+  }
+
+  // the 32 code bytes of cell `src`'s exchange row
+  __device__ __forceinline__ void load_row(const StoreDesc &sd, int src, uint4 &r0, uint4 &r1) {
+    const uint4 *p = reinterpret_cast<const uint4 *>(sd.xin.dc + (size_t)src * PSC_XCAP);
+    r0 = p[0];
+    r1 = p[1];
+  }
+  // writes the arrival-list window [a0, a0 + WALK_AC): entry = direction lane << 8 | row index
+  __device__ __forceinline__ void fill_window(const uint4 &r0, const uint4 &r1, bool have) {
+    if (have) {
+      const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+      const unsigned pat = (unsigned)lane * 0x01010101u;
+      int g = my_start - a0;
+#pragma unroll
+      for (int q = 0; q < 8; q++) {
+        unsigned m = __vcmpeq4(w[q], pat) & 0x01010101u;
+        while (m) {
+          const int j = q * 4 + ((__ffs(m) - 1) >> 3);
+          if (g >= 0 && g < WALK_AC) arr[g] = (uint16_t)((lane << 8) | j);
+          g++;
+          m &= m - 1;
+        }
+      }
+    }
+    __syncwarp();
+  }
+
+  // Start of a cell: where its arrivals are (the neighbours' rows), whether it takes the
+  // shared-memory path, wait for its resident run.  (cx, cy, cz): the cell's coordinates.
+  __device__ __forceinline__ void begin_cell(const StoreDesc &sd, const GridDesc &gd, int key_, int n_,
+                                             int base_, int cap_, int cx, int cy, int cz) {
+    key = key_;
+    n = n_;
+    base = base_;
+    cap = cap_;
+    const bool have = lane < ND && lane != STAY;
+    uint4 r0 = make_uint4(~0u, ~0u, ~0u, ~0u), r1 = r0;
+    int cntm = 0;
+    if (have) {
+      int sx, sy, sz;
+      dir_decode<D3>(lane, sx, sy, sz);
+      const int src = cell_key(gd, D3 ? wrap_cell(cx - sx, gd.n[0]) : 0, wrap_cell(cy - sy, gd.n[1]),
+                               wrap_cell(cz - sz, gd.n[2]));
+      nbk[lane] = src;
+      load_row(sd, src, r0, r1);
+      const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+      const unsigned pat = (unsigned)lane * 0x01010101u;
+#pragma unroll
+      for (int q = 0; q < 8; q++) cntm += __popc(__vcmpeq4(w[q], pat) & 0x01010101u);
+    }
+    int inc = cntm;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += t;
+    }
+    na = __shfl_sync(0xffffffffu, inc, 31);
+    my_start = inc - cntm;
+    a0 = 0;
+    if (na) fill_window(r0, r1, have);
+    fast = n + na <= C;
+    nh = 0;
+    tcur = fast ? n : 0;  // shared-memory path: append cursor; global path: write cursor
+    nleave = 0;
+    if (loads_armed) {
+      mbar_wait(bar, parity);
+      parity ^= 1;
+      loads_armed = false;
+    }
+  }
+
+  // Loads particle v0 + lane of the cell (residents first, then arrivals).  Returns whether the
+  // lane holds a particle.  x2d / id are fetched only where a later move needs them (leavers, the
+  // global path): see extras().
+  __device__ __forceinline__ bool load(const StoreDesc &sd, int v0, Part &p, bool &isarr, float &x2d, int &id) {
+    const int v = v0 + lane;
+    const bool act = v < n + na;
+    isarr = v >= n;
+    p.ax = p.ay = p.az = 0.25f;
+    p.ux = p.uy = p.uz = p.qw = 0.f;
+    p.sp = 0;
+    x2d = 0.f;
+    id = 0;
+    if (v0 + 32 > n && na) {  // warp-uniform: this chunk contains arrivals
+      if (v0 + 32 - n > a0 + WALK_AC) {  // next window of the arrival list (cells with > 128 arrivals)
+        a0 = v0 > n ? v0 - n : 0;
+        const bool have = lane < ND && lane != STAY;
+        uint4 r0 = make_uint4(~0u, ~0u, ~0u, ~0u), r1 = r0;
+        if (have) load_row(sd, nbk[lane], r0, r1);
+        __syncwarp();
+        fill_window(r0, r1, have);
+      }
+      if (act && isarr) {
+        const int e = arr[v - n - a0];
+        const size_t idx = (size_t)nbk[e >> 8] * PSC_XCAP + (e & 255);
+        const XRec r = sd.xin.rec[idx];
+        if (D3) {
+          p.ax = __uint_as_float(r.a.x); p.ay = __uint_as_float(r.a.y); p.az = __uint_as_float(r.a.z);
+          p.ux = __uint_as_float(r.a.w); p.uy = __uint_as_float(r.b.x); p.uz = __uint_as_float(r.b.y);
+          p.qw = __uint_as_float(r.b.z); p.sp = (int)r.b.w;
+        } else {
+          p.ay = __uint_as_float(r.a.x); p.az = __uint_as_float(r.a.y);
+          p.ux = __uint_as_float(r.a.z); p.uy = __uint_as_float(r.a.w); p.uz = __uint_as_float(r.b.x);
+          p.qw = __uint_as_float(r.b.y); p.sp = (int)r.b.z; x2d = __uint_as_float(r.b.w);
+        }
+        if (XC && sd.xin.id) id = sd.xin.id[idx];
+      }
+    }
+    if (act && !isarr) {
+      if (fast) {
+        const float *q = buf + v;
+        if (D3) {
+          p.ax = q[0]; p.ay = q[C]; p.az = q[2 * C]; p.ux = q[3 * C]; p.uy = q[4 * C]; p.uz = q[5 * C];
+          p.qw = q[6 * C]; p.sp = __float_as_int(q[7 * C]);
+        } else {
+          p.ay = q[0]; p.az = q[C]; p.ux = q[2 * C]; p.uy = q[3 * C]; p.uz = q[4 * C];
+          p.qw = q[5 * C]; p.sp = __float_as_int(q[6 * C]);
+        }
+      } else {
+        const size_t s = (size_t)base + v;
+        if (D3) {
+          p.ax = ld_stream(sd.col[0] + s); p.ay = ld_stream(sd.col[1] + s); p.az = ld_stream(sd.col[2] + s);
+          p.ux = ld_stream(sd.col[3] + s); p.uy = ld_stream(sd.col[4] + s); p.uz = ld_stream(sd.col[5] + s);
+          p.qw = ld_stream(sd.col[6] + s); p.sp = __float_as_int(ld_stream(sd.col[7] + s));
+        } else {
+          p.ay = ld_stream(sd.col[0] + s); p.az = ld_stream(sd.col[1] + s);
+          p.ux = ld_stream(sd.col[2] + s); p.uy = ld_stream(sd.col[3] + s); p.uz = ld_stream(sd.col[4] + s);
+          p.qw = ld_stream(sd.col[5] + s); p.sp = __float_as_int(ld_stream(sd.col[6] + s));
+        }
+        if (XC) {
+          if (sd.icol_x2d >= 0) x2d = ld_stream(sd.col[sd.icol_x2d] + s);
+          if (sd.icol_id >= 0) id = __float_as_int(ld_stream(sd.col[sd.icol_id] + s));
+        }
+      }
+    }
+    return act;
+  }
+
+  // optional values of a RESIDENT particle on the shared-memory path (needed only if it leaves)
+  __device__ __forceinline__ void extras(const StoreDesc &sd, int v, float &x2d, int &id) {
+    if (XC) {
+      if (sd.icol_x2d >= 0) x2d = buf[sd.icol_x2d * C + v];
+      if (sd.icol_id >= 0) id = __float_as_int(buf[sd.icol_id * C + v]);
+    }
+  }
+
+  // the 8 record words of a particle (positions as given)
+  __device__ __forceinline__ static void to_words(float (&w)[8], const Part &p, float x2d) {
+    if (D3) {
+      w[0] = p.ax; w[1] = p.ay; w[2] = p.az; w[3] = p.ux; w[4] = p.uy; w[5] = p.uz; w[6] = p.qw;
+      w[7] = __int_as_float(p.sp);
+    } else {
+      w[0] = p.ay; w[1] = p.az; w[2] = p.ux; w[3] = p.uy; w[4] = p.uz; w[5] = p.qw;
+      w[6] = __int_as_float(p.sp); w[7] = x2d;
+    }
+  }
+
+  // index of the next leaver's record in the cell's exchange row (all lanes; `leave`: this lane
+  // leaves with direction code dc).  Records past the row's capacity go to the spill list.
+  __device__ __forceinline__ int leaver_index(bool leave, int dc) {
+    const unsigned m = __ballot_sync(0xffffffffu, leave);
+    const int xi = nleave + __popc(m & lt);
+    if (leave && xi < PSC_XCAP) xrow[xi] = (uint8_t)dc;
+    nleave += __popc(m);
+    return xi;
+  }
+
+  // writes a leaver's record (positions relative to the destination cell) into row slot xi of
+  // cell src_key, or spills it
+  __device__ __forceinline__ static void write_record(const StoreDesc &sd, const GridDesc &gd, int src_key,
+                                                      int xi, const float (&w)[8], int id, int dest_key) {
+    if (xi < PSC_XCAP) {
+      const size_t idx = (size_t)src_key * PSC_XCAP + xi;
+      XRec r;
+      r.a = make_uint4(__float_as_uint(w[0]), __float_as_uint(w[1]), __float_as_uint(w[2]), __float_as_uint(w[3]));
+      r.b = make_uint4(__float_as_uint(w[4]), __float_as_uint(w[5]), __float_as_uint(w[6]), __float_as_uint(w[7]));
+      sd.xout.rec[idx] = r;
+      if (XC && sd.xout.id) sd.xout.id[idx] = id;
+    } else {
+      spill_particle(sd, dest_key, w, id);
+    }
+  }
+
+  // Files the advanced particle of every lane that STAYS in the cell (stay), notes the hole of
+  // every resident that leaves (leave).  pn: the new values (offsets in [0,1)).
+  __device__ __forceinline__ void store(const StoreDesc &sd, int v0, bool act, bool isarr, bool leave,
+                                        const Part &pn, float x2d, int id) {
+    const int v = v0 + lane;
+    const bool stay = act && !leave;
+    if (fast) {
+      const bool rl = act && leave && !isarr;
+      const unsigned mrl = __ballot_sync(0xffffffffu, rl);
+      if (rl) {
+        holes[nh + __popc(mrl & lt)] = (uint8_t)v;
+        buf[v] = -1.f;  // column 0 (an offset, >= 0 for a particle) marks the hole
+      }
+      nh += __popc(mrl);
+      if (stay && !isarr) {
+        float *q = buf + v;
+        if (D3) {
+          q[0] = pn.ax; q[C] = pn.ay; q[2 * C] = pn.az; q[3 * C] = pn.ux; q[4 * C] = pn.uy; q[5 * C] = pn.uz;
+        } else {
+          q[0] = pn.ay; q[C] = pn.az; q[2 * C] = pn.ux; q[3 * C] = pn.uy; q[4 * C] = pn.uz;
+        }
+      }
+      const unsigned ma = __ballot_sync(0xffffffffu, stay && isarr);
+      if (ma) {
+        __syncwarp();
+        if (stay && isarr) {
+          const int r = __popc(ma & lt);
+          const int slot = r < nh ? (int)holes[nh - 1 - r] : tcur + (r - nh);
+          float w[8];
+          to_words(w, pn, x2d);
+          if (slot < cap) {
+            float *q = buf + slot;
+#pragma unroll
+            for (int c = 0; c < (D3 ? 8 : 7); c++) q[c * C] = w[c];
+            const size_t s = (size_t)base + slot;
+            st_stream(sd.col[NDYN] + s, pn.qw);
+            st_stream(sd.col[NDYN + 1] + s, __int_as_float(pn.sp));
+            if (XC) {
+              if (sd.icol_x2d >= 0) { q[sd.icol_x2d * C] = x2d; st_stream(sd.col[sd.icol_x2d] + s, x2d); }
+              if (sd.icol_id >= 0) { q[sd.icol_id * C] = __int_as_float(id); st_stream(sd.col[sd.icol_id] + s, __int_as_float(id)); }
+            }
+          } else {
+            spill_particle(sd, key, w, id);
+          }
+        }
+        const int ca = __popc(ma), used = ca < nh ? ca : nh;
+        nh -= used;
+        tcur += ca - used;
+        __syncwarp();
+      }
+    } else {
+      // global path: in-place streaming compaction (the write cursor tcur never passes the reads)
+      const unsigned ms = __ballot_sync(0xffffffffu, stay);
+      const int slot = tcur + __popc(ms & lt);
+      __syncwarp();
+      if (stay) {
+        float w[8];
+        to_words(w, pn, x2d);
+        if (slot < cap) {
+          const size_t s = (size_t)base + slot;
+#pragma unroll
+          for (int c = 0; c < (D3 ? 8 : 7); c++) st_stream(sd.col[c] + s, w[c]);
+          if (XC) {
+            if (sd.icol_x2d >= 0) st_stream(sd.col[sd.icol_x2d] + s, x2d);
+            if (sd.icol_id >= 0) st_stream(sd.col[sd.icol_id] + s, __int_as_float(id));
+          }
+        } else {
+          spill_particle(sd, key, w, id);
+        }
+      }
+      tcur += __popc(ms);
+    }
+  }
+
+  // End of a cell: close the remaining holes from the tail, write the image back, publish the
+  // count and the exchange row, start fetching the next cell (next_n <= 0: none).
+  __device__ __forceinline__ void end_cell(const StoreDesc &sd, int next_n, int next_base) {
+    int newcnt;
+    __syncwarp();
+    if (fast) {
+      if (nh > 0) {
+        const int m = n - nh;  // no append happened while holes were left, so tcur == n
+        int done = 0;
+        for (int t0 = m; t0 < n; t0 += 32) {
+          const int s = t0 + lane;
+          const bool valid = s < n && buf[s] >= 0.f;
+          const unsigned mv = __ballot_sync(0xffffffffu, valid);
+          if (valid) {
+            const int h = holes[done + __popc(mv & lt)];  // ascending list: its first entries are < m
+            for (int c = 0; c < ncol; c++) buf[c * C + h] = buf[c * C + s];
+            for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + h, buf[c * C + s]);
+          }
+          done += __popc(mv);
+        }
+        newcnt = m;
+      } else {
+        newcnt = tcur < cap ? tcur : cap;
+      }
+      fence_proxy_async();
+      __syncwarp();
+      if (lane == 0 && newcnt > 0) {
+        const unsigned bytes = (unsigned)((newcnt + 3) & ~3) * 4u;
+#pragma unroll
+        for (int c = 0; c < NDYN; c++) bulk_s2g(sd.col[c] + base, buf + c * C, bytes);
+        bulk_commit();
+      }
+    } else {
+      newcnt = tcur < cap ? tcur : cap;
+    }
+    if (lane == 0) sd.cnt[key] = newcnt;
+    if (lane < PSC_XCAP / 4)
+      reinterpret_cast<unsigned *>(sd.xout.dc + (size_t)key * PSC_XCAP)[lane] = reinterpret_cast<const unsigned *>(xrow)[lane];
+    __syncwarp();
+    xrow[lane] = PSC_XDC_NONE;
+    if (lane == 0) bulk_wait_read0();  // the image may be overwritten once the copy engine has read it
+    __syncwarp();
+    if (next_n > 0) issue_loads(sd, next_n, next_base);
+  }
+
+  __device__ __forceinline__ void finish() {
+    if (lane == 0) bulk_wait_all();
+    __syncwarp();
+  }
+};

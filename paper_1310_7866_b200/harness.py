@@ -24,6 +24,7 @@ class Simulation:
         self.J = torch.zeros(shp, dtype=torch.float32, device=dev)
         self.interior(self.E).copy_(plasma.E.to(dev))
         self.interior(self.B).copy_(plasma.B.to(dev))
+        self.capacity = self.psc.particle_capacity(self.np)
         self.sets = []
         for k in range(2):
             s = {}
@@ -32,7 +33,7 @@ class Simulation:
                     s[c] = None       # optional columns (include/psc.h): not carried
                     continue
                 dt = torch.int32 if c in ("species", "id") else torch.float32
-                s[c] = torch.empty(max(self.np, 1), dtype=dt, device=dev)
+                s[c] = torch.empty(self.capacity, dtype=dt, device=dev)
             self.sets.append(s)
         for c in COLUMNS:
             if self.sets[0][c] is not None and self.np:
@@ -40,7 +41,7 @@ class Simulation:
         self.ws = torch.empty(self.psc.workspace_bytes(self.np), dtype=torch.uint8, device=dev)
         self.psc.bind_workspace(self.ws)
         self.psc.bind_fields(self.E, self.B, self.J)
-        self.psc.bind_particles(self.np, self.sets[0], self.sets[1])
+        self.psc.bind_particles(self.np, self.capacity, self.sets[0], self.sets[1])
         self.psc.fill_ghosts(PSC_E)
         self.psc.fill_ghosts(PSC_B)
 
@@ -49,19 +50,34 @@ class Simulation:
         return F[:, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]]
 
     def current(self):
-        """the column set (dict of tensors, trimmed to n particles) that holds the particles now"""
+        """the column set (dict of tensors, trimmed to n particles) that holds the particles now;
+        only meaningful for absolute columns (after bind or psc_particles_export)"""
+        assert self.psc.particles_form() == 0
         ptr = self.psc.particles_current()["y"]
         s = self.sets[0] if self.sets[0]["y"].data_ptr() == ptr else self.sets[1]
         assert s["y"].data_ptr() == ptr
         return {c: (None if t is None else t[: self.np]) for c, t in s.items()}
 
+    def gather(self, absolute=False):
+        """dense copy of the cell store (psc_particles_gather): dict of column tensors [n] plus
+        "key" (int32 cell keys; the cell the in-cell offsets refer to).  State unchanged."""
+        dev = self.device
+        out = {}
+        for c in COLUMNS:
+            if self.sets[0][c] is None:
+                out[c] = None
+                continue
+            dt = torch.int32 if c in ("species", "id") else torch.float32
+            out[c] = torch.empty(max(self.np, 1), dtype=dt, device=dev)
+        key = torch.empty(max(self.np, 1), dtype=torch.int32, device=dev)
+        self.psc.particles_gather(out, key, absolute)
+        out = {c: (None if t is None else t[: self.np]) for c, t in out.items()}
+        out["key"] = key[: self.np]
+        return out
+
     def _ws_view(self, ptr, count):
         off = ptr - self.ws.data_ptr()
         return self.ws[off: off + 4 * count].view(torch.int32)
-
-    def keys(self):
-        """cell keys of the current particles (internal form), int32 tensor viewing the workspace"""
-        return self._ws_view(self.psc.particles_keys(), self.np)
 
     def sort_result(self):
         """(cell_idx[n], perm[n], cell_offsets[n_keys+1]) as int32 tensors viewing the workspace"""

@@ -26,7 +26,7 @@ def test_call_order_and_binding_errors():
     assert L.psc_push_particles(h, None) == -3                  # PSC_ERR_NOT_SORTED: no sort yet
     sim.psc.particles_sort()
     sim.psc.push_particles()
-    assert L.psc_push_particles(h, None) == -3                  # pushed list: sort again first
+    assert L.psc_push_particles(h, None) == 0                   # the store stays ordered by cell: no sort needed
     sim.psc.particles_sort()
     assert L.psc_push_fields(h, 7, C.c_float(0.5), None) == -1  # which must be PSC_E or PSC_B
     assert L.psc_push_fields(h, 1, C.c_float(0.0), None) == -1  # frac > 0

@@ -21,13 +21,23 @@ def oracle_state(pl):
     return st, E, B
 
 
+def gpu_state(sim):
+    """dense numpy copy of the cell store through psc_particles_gather (state unchanged): in-cell
+    offsets, momenta, qw, species, id and "key", the sort key of the cell each particle is filed
+    under"""
+    return {k: v.cpu().numpy() for k, v in sim.gather().items() if v is not None}
+
+
 def gpu_cols(sim, export=True):
-    """the current particle columns as numpy arrays; export=True first converts the internal form
-    (in-cell offsets) back to absolute fp32 positions through psc_particles_export"""
+    """the particle columns as numpy arrays, dense; export=True: absolute fp32 positions
+    ((cell + offset) * dx rounded once, as psc_particles_export gives them); export=False: the
+    internal form (in-cell offsets) plus "key".  Neither changes the library's state."""
+    if sim.psc.particles_form() == 0:
+        return {k: v.cpu().numpy() for k, v in sim.current().items() if v is not None}
+    g = sim.gather(absolute=export)
     if export:
-        sim.psc.particles_export()
-    cur = sim.current()
-    return {k: v.cpu().numpy() for k, v in cur.items() if v is not None}
+        del g["key"]
+    return {k: v.cpu().numpy() for k, v in g.items() if v is not None}
 
 
 def key_to_cell(key, n, block):
@@ -43,19 +53,24 @@ def key_to_cell(key, n, block):
     return [bc[d] * bs[d] + lc[d] for d in range(3)]
 
 
-def gpu_positions_f64(sim, block=(0, 0, 0)):
-    """positions of the current particles in fp64 from the internal form (cell + offset) * dx --
-    no export rounding; invariant coordinates are returned as stored"""
-    assert sim.psc.particles_form() == 1
-    cur = sim.current()
-    key = sim.keys().cpu().numpy().astype(np.int64)
-    pl = sim.plasma
-    cells = key_to_cell(key, pl.n, library_block(pl.n, block))
+def positions_f64(st, pl, block=(0, 0, 0)):
+    """fp64 positions (cell + offset) * dx of a gpu_state -- no export rounding; invariant
+    coordinates are returned as stored"""
+    cells = key_to_cell(st["key"].astype(np.int64), pl.n, library_block(pl.n, block))
     out = []
     for d, c in enumerate(("x", "y", "z")):
-        o = cur[c].cpu().numpy().astype(np.float64)
+        if c not in st:
+            out.append(np.zeros(len(st["key"])))
+            continue
+        o = st[c].astype(np.float64)
         out.append(np.ascontiguousarray(o if pl.n[d] == 1 else (cells[d] + o) * pl.dx[d]))
     return out
+
+
+def gpu_positions_f64(sim, block=(0, 0, 0)):
+    """positions of the current particles in fp64 from the internal form"""
+    assert sim.psc.particles_form() == 1
+    return positions_f64(gpu_state(sim), sim.plasma, block)
 
 
 def order_by_id(got_id, ref_id):
