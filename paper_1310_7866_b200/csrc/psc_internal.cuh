@@ -46,9 +46,9 @@ struct Cols {
 // its move; the next push of the destination cell collects the records aimed at it from its 8 / 26
 // neighbours' rows (reorder on load) and files them into the holes the cell's own
 // leavers left.  So no per-step sort pass exists at all; the exchange is ping-pong buffered.
-constexpr int PSC_XCAP = 32;        // exchange records per cell and step (one 32-byte code row)
+constexpr int PSC_XCAP = 32;        // exchange records per cell and step (one bit each in a header word)
+constexpr int PSC_XW2 = 16, PSC_XW3 = 32;  // header words per row (2-d: 9 direction codes, 3-d: 27)
 constexpr int PSC_SLOT_ALIGN = 32;  // cell segments start on multiples of 32 slots
-constexpr uint8_t PSC_XDC_NONE = 0xff;
 
 // One exchange record: the first 8 buffer columns of a particle (see StoreDesc::col), positions
 // relative to the DESTINATION cell.  2-d: {y z ux uy uz qw sp x2d}, 3-d: {x y z ux uy uz qw sp}.
@@ -57,9 +57,9 @@ struct __align__(16) XRec {
 };
 
 struct Exchange {
-  XRec *rec;      // [nkeys * PSC_XCAP]
-  uint8_t *dc;    // [nkeys * PSC_XCAP] direction codes, PSC_XDC_NONE = unused entry
-  int32_t *id;    // [nkeys * PSC_XCAP] or nullptr
+  XRec *rec;       // [nkeys * PSC_XCAP]
+  uint32_t *mask;  // [nkeys * XW] row headers: mask[k * XW + dc] bit i <=> record i of row k moved by code dc
+  int32_t *id;     // [nkeys * PSC_XCAP] or nullptr
 };
 
 // particles that found no room (exchange row or destination cell full): the next step re-lays

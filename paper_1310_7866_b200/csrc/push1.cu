@@ -39,10 +39,10 @@
 namespace {
 
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
-// rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax (2-d: carried x), 2 ay, 3 az,
-// 4 ddx (2-d: v_x), 5 ddy, 6 ddz, 7 qw, 8 ux, 9 uy, 10 uz, 11 species | row index << 8, 12 id.
-// The drain reuses rows [0, NV) of a drained entry as its scratch column.
-constexpr int QROWS = 13;
+// rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 ddx (2-d: v_x),
+// 5 ddy, 6 ddz, 7 qw.  The drain reuses rows [0, NV) of a drained entry as its scratch column,
+// hence 12 rows in 3-d.
+constexpr int QROWS2 = 8, QROWS3 = 12;
 
 
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
@@ -291,48 +291,23 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
 }
 
 
-// Drains n (<= 32) queue entries starting at `start`: deposits every segment of each trajectory
-// and writes the particle's record (offsets relative to the DESTINATION cell) into its source
-// cell's exchange row.
-template <bool D3, bool XC, class TG>
+// Drains n (<= 32) queue entries starting at `start`: deposits every segment of each trajectory.
+template <bool D3, class TG>
 __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg, const GridDesc &gd,
-                                            const StoreDesc &sd, int kbase, float *__restrict__ q,
-                                            const int *__restrict__ rel, int start, int n, int lane) {
+                                            float *__restrict__ q, const int *__restrict__ rel,
+                                            int start, int n, int lane) {
   if (lane < n) {
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
     const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
     const float ddx = q[4 * QCAP + e], ddy = q[5 * QCAP + e], ddz = q[6 * QCAP + e];
     const float qw = q[7 * QCAP + e];
-    const float ux = q[8 * QCAP + e], uy = q[9 * QCAP + e], uz = q[10 * QCAP + e];
-    const int spx = __float_as_int(q[11 * QCAP + e]);
-    const int id = XC ? __float_as_int(q[12 * QCAP + e]) : 0;
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
-    // 2-d: the x slots carry (carried x, v_x): the out-of-plane current needs the velocity
+    // 2-d: the ddx slot carries v_x: the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
     const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
     vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
                 qvx, rel, q + e, lane % (D3 ? 12 : 8));
-    // the record: new offsets relative to the destination cell
-    const float endx = D3 ? ax + ddx : 0.f, endy = ay + ddy, endz = az + ddz;
-    const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-    const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-    const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
-    Part p;
-    p.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
-    p.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-    p.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-    p.ux = ux; p.uy = uy; p.uz = uz; p.qw = qw;
-    p.sp = spx & 255;
-    float w[8];
-    CellWalker<D3, XC>::to_words(w, p, D3 ? 0.f : ax);
-    const int xi = spx >> 8;
-    const int src = kbase + (lz * tg.bs[1] + ly) * tg.bs[0] + lx;
-    int dest = 0;
-    if (xi >= PSC_XCAP)
-      dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0, wrap_cell(tg.o[1] + ly + syd, gd.n[1]),
-                      wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-    CellWalker<D3, XC>::write_record(sd, gd, src, xi, w, id, dest);
   }
   __syncwarp();
 }
@@ -369,15 +344,25 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   // per-warp areas first (128-byte aligned cell images), then the block's tiles and tables
-  Walker wk;
-  wk.init(smraw + (size_t)warp * wstride, sd, lane);
+  constexpr int QROWS = D3 ? QROWS3 : QROWS2;
   float *myQ = (float *)(smraw + (size_t)nwarps * wstride) + warp * (QROWS * QCAP);  // [QROWS][QCAP]
   float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP);  // [6][fvol]
   float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
   float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
   int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [12]: J points of vb_values
-  int *sBase = sRel + 12;                     // [cpb + 1]: first slot of each cell
+  int *sNbT = sRel + 12;                      // [27]: first key of the 3^3 neighbouring tiles
+  int *sBase = sNbT + 27;                     // [cpb + 1]: first slot of each cell
   int *sCnt = sBase + tg.cpb + 1;             // [cpb]: particles resident in each cell
+  Walker wk;
+  wk.init(smraw + (size_t)warp * wstride, sd, lane, sNbT);
+  if (threadIdx.x < 27) {  // periodic neighbour tiles (the single-GPU particle exchange)
+    const int t = threadIdx.x;
+    const int b0 = blockIdx.x % gd.nb[0], br = blockIdx.x / gd.nb[0];
+    const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
+    const int n0 = wrap_cell(b0 + t % 3 - 1, gd.nb[0]), n1 = wrap_cell(b1 + (t / 3) % 3 - 1, gd.nb[1]),
+              n2 = wrap_cell(b2 + t / 9 - 1, gd.nb[2]);
+    sNbT[t] = ((n2 * gd.nb[1] + n1) * gd.nb[0] + (D3 ? n0 : 0)) * tg.cpb;
+  }
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   if (threadIdx.x < NV) {  // J points of the NV in-cell currents, relative to the cell's node
@@ -430,8 +415,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int lx = ci % tg.bs[0];
     const int lt_ = ci / tg.bs[0];
     const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
-    wk.begin_cell(sd, gd, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], tg.o[0] + lx,
-                  tg.o[1] + ly, tg.o[2] + lz);
+    wk.begin_cell(sd, tg, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], lx, ly, lz);
     const int ntot = wk.n + wk.na;
     const int packed = lx | (ly << 10) | (lz << 20);
     // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
@@ -491,27 +475,36 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       if (cm) {
         const int xi = wk.leaver_index(cross, dc);
         if (cross) {
+          // the particle's record goes to this cell's exchange row (offsets relative to the
+          // destination cell), its trajectory to the queue
           if (wk.fast && !isarr) wk.extras(sd, v0 + lane, x2d, id);
+          Part pr;
+          pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
+          pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+          pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+          pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
+          float w[8];
+          Walker::to_words(w, pr, x2d);
+          int dest = 0;
+          if (xi >= PSC_XCAP)
+            dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
+                            wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
+          Walker::write_record(sd, gd, kbase + ci, xi, w, id, dest);
           const int e = qcnt + __popc(cm & lt);
           myQ[0 * QCAP + e] = __int_as_float(packed);
-          myQ[1 * QCAP + e] = D3 ? ax : x2d;
+          myQ[1 * QCAP + e] = ax;
           myQ[2 * QCAP + e] = ay;
           myQ[3 * QCAP + e] = az;
           myQ[4 * QCAP + e] = D3 ? ddx : vx;
           myQ[5 * QCAP + e] = ddy;
           myQ[6 * QCAP + e] = ddz;
           myQ[7 * QCAP + e] = qw;
-          myQ[8 * QCAP + e] = ux;
-          myQ[9 * QCAP + e] = uy;
-          myQ[10 * QCAP + e] = uz;
-          myQ[11 * QCAP + e] = __int_as_float(sp | (xi << 8));
-          if (XC) myQ[12 * QCAP + e] = __int_as_float(id);
         }
         qcnt += __popc(cm);
         __syncwarp();
         if (qcnt >= 32) {
           qcnt -= 32;
-          drain_queue<D3, XC>(sJ, tg, gd, sd, kbase, myQ, sRel, qcnt, 32, lane);
+          drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
         }
       }
 
@@ -539,7 +532,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int nx = ci + nwarps;
     wk.end_cell(sd, nx < tg.cpb ? sCnt[nx] : 0, nx < tg.cpb ? sBase[nx] : 0);
   }
-  if (qcnt) drain_queue<D3, XC>(sJ, tg, gd, sd, kbase, myQ, sRel, 0, qcnt, lane);
+  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, sRel, 0, qcnt, lane);
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
   __syncthreads();
@@ -576,8 +569,8 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   constexpr int threads = 128;
   const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
   const int wstride = (wbytes + 127) / 128 * 128;
-  const size_t smem = (size_t)(threads / 32) * (wstride + QROWS * QCAP * 4) +
-                      (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 2 * gd.cpb + 2) * sizeof(float);
+  const size_t smem = (size_t)(threads / 32) * (wstride + (d3 ? QROWS3 : QROWS2) * QCAP * 4) +
+                      (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 27 + 2 * gd.cpb + 2) * sizeof(float);
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
@@ -598,8 +591,8 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 4);
-    else PSC_LAUNCH_PUSH1(false, 0, 128, 4);
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
+    else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
   }
 #undef PSC_LAUNCH_PUSH1
   PSC_LAUNCH_CHECK(c);

@@ -213,13 +213,22 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   Geom2<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-  Walker wk;
-  wk.init(smraw + (size_t)warp * wstride, sd, lane);
   float *sF = (float *)(smraw + (size_t)nwarps * wstride);  // [6][tvol]
   float *sJ = sF + 6 * tg.tvol;                              // [3][tvol]
   float *sH = sJ + 3 * tg.tvol;                              // [8]: Boris h per species
-  int *sBase = (int *)(sH + PSC_MAX_SPECIES);                // [cpb + 1]
+  int *sNbT = (int *)(sH + PSC_MAX_SPECIES);                 // [27]: first key of the 3^3 neighbouring tiles
+  int *sBase = sNbT + 27;                                    // [cpb + 1]
   int *sCnt = sBase + tg.cpb + 1;                            // [cpb]
+  Walker wk;
+  wk.init(smraw + (size_t)warp * wstride, sd, lane, sNbT);
+  if (threadIdx.x < 27) {  // periodic neighbour tiles (the single-GPU particle exchange)
+    const int t = threadIdx.x;
+    const int b0 = blockIdx.x % gd.nb[0], br = blockIdx.x / gd.nb[0];
+    const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
+    const int n0 = wrap_cell(b0 + t % 3 - 1, gd.nb[0]), n1 = wrap_cell(b1 + (t / 3) % 3 - 1, gd.nb[1]),
+              n2 = wrap_cell(b2 + t / 9 - 1, gd.nb[2]);
+    sNbT[t] = ((n2 * gd.nb[1] + n1) * gd.nb[0] + (D3 ? n0 : 0)) * tg.cpb;
+  }
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   const int kbase = blockIdx.x * tg.cpb;
@@ -258,8 +267,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
     const int lx = ci % tg.bs[0], lt = ci / tg.bs[0];
     const int ly = lt % tg.bs[1], lz = lt / tg.bs[1];
-    wk.begin_cell(sd, gd, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], tg.o[0] + lx,
-                  tg.o[1] + ly, tg.o[2] + lz);
+    wk.begin_cell(sd, tg, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], lx, ly, lz);
     const int np_cell = wk.n + wk.na;  // residents + arrivals (reorder on load)
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
@@ -462,7 +470,7 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
   const int wstride = (wbytes + 127) / 128 * 128;
   const size_t smem = (size_t)(threads / 32) * wstride +
-                      (size_t)(9 * tvol + PSC_MAX_SPECIES + 2 * gd.cpb + 2) * sizeof(float);
+                      (size_t)(9 * tvol + PSC_MAX_SPECIES + 27 + 2 * gd.cpb + 2) * sizeof(float);
   if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_)                                                           \

@@ -458,23 +458,20 @@ k_reorder(GridDesc gd, const int *__restrict__ np, const int *__restrict__ perm,
 
 // ---- flattening the store -----------------------------------------------------------------------
 
-__device__ __forceinline__ int row_count(const uint8_t *__restrict__ dc, int k) {
-  const uint4 *p = reinterpret_cast<const uint4 *>(dc + (size_t)k * PSC_XCAP);
-  const uint4 r0 = p[0], r1 = p[1];
-  const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
-  int c = 0;
-#pragma unroll
-  for (int q = 0; q < 8; q++) c += 4 - __popc(__vcmpeq4(w[q], 0xffffffffu) & 0x01010101u);
-  return c;
+// records waiting in the exchange row of cell k: the union of its per-direction masks
+__device__ __forceinline__ unsigned row_union(const uint32_t *__restrict__ mask, int k, int xw, int nd) {
+  unsigned u = 0;
+  for (int d = 0; d < nd; d++) u |= mask[(size_t)k * xw + d];
+  return u;
 }
 
 // tot[k] = residents of cell k + records waiting in its exchange row
 __global__ void __launch_bounds__(SORT_THREADS)
-k_tot(int nk, const int *__restrict__ cnt, const uint8_t *__restrict__ dc, int *__restrict__ tot,
-      const uint32_t *__restrict__ cond) {
+k_tot(int nk, int xw, int nd, const int *__restrict__ cnt, const uint32_t *__restrict__ mask,
+      int *__restrict__ tot, const uint32_t *__restrict__ cond) {
   PSC_COND_RETURN(cond);
   for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nk; k += gridDim.x * blockDim.x)
-    tot[k] = cnt[k] + row_count(dc, k);
+    tot[k] = cnt[k] + __popc(row_union(mask, k, xw, nd));
 }
 
 // A warp per cell copies the cell's residents, then the records of its exchange row, to the dense
@@ -518,9 +515,13 @@ k_gather(GridDesc gd, Cols in, const int *__restrict__ base, const int *__restri
       if (out.id) out.id[o] = in.id ? in.id[s] : 0;
       if (keyout) keyout[o] = k;
     }
-    if (nt > n) {  // the row's records, in row order
-      const int dc = (int)xin.dc[(size_t)k * PSC_XCAP + lane];
-      const bool have = dc != (int)PSC_XDC_NONE;
+    if (nt > n) {  // the row's records, in row order: lane = record index
+      constexpr int XW = D3 ? PSC_XW3 : PSC_XW2, ND = D3 ? 27 : 9;
+      const unsigned mine = lane < ND ? xin.mask[(size_t)k * XW + lane] : 0u;
+      int dc = -1;
+      for (int d = 0; d < ND; d++)
+        if ((__shfl_sync(0xffffffffu, mine, d) >> lane) & 1u) dc = d;
+      const bool have = dc >= 0;
       const unsigned m = __ballot_sync(0xffffffffu, have);
       if (have) {
         const size_t idx = (size_t)k * PSC_XCAP + lane, o = (size_t)d0 + n + __popc(m & lanemask_lt());
@@ -594,13 +595,13 @@ k_gather_spill(GridDesc gd, Spill sp, const int *__restrict__ doffs, Cols out, i
 
 // after a (re-)layout: every exchange row empty, nothing spilled; records the slots in use
 __global__ void __launch_bounds__(SORT_THREADS)
-k_store_reset(int nk, uint8_t *__restrict__ dc0, uint8_t *__restrict__ dc1, const int *__restrict__ base,
+k_store_reset(int nk, int xw, uint32_t *__restrict__ m0, uint32_t *__restrict__ m1, const int *__restrict__ base,
               uint32_t *__restrict__ dw, long long capacity, const uint32_t *__restrict__ cond) {
   PSC_COND_RETURN(cond);
-  const int m = nk * (PSC_XCAP / 4);
+  const int m = nk * xw;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) {
-    reinterpret_cast<unsigned *>(dc0)[i] = 0xffffffffu;
-    reinterpret_cast<unsigned *>(dc1)[i] = 0xffffffffu;
+    m0[i] = 0u;
+    m1[i] = 0u;
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     dw[PSC_DW_SLOTS] = (uint32_t)base[nk];
@@ -637,7 +638,7 @@ size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   b += 2 * align_up((nk + 1) * 8, 256);                       // pack, packloc
   b += align_up((nk / SCAN_TILE + 3) * 8, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
-  b += 2 * (align_up(nx * sizeof(XRec), 256) + align_up(nx, 256) + align_up(nx * 4, 256));  // exchange x2
+  b += 2 * (align_up(nx * sizeof(XRec), 256) + align_up(nk * PSC_XW3 * 4, 256) + align_up(nx * 4, 256));  // exchange x2
   const size_t sc = (size_t)spill_capacity(n);
   b += align_up(sc * sizeof(XRec), 256) + 2 * align_up(sc * 4, 256);  // spill
   return b;
@@ -667,7 +668,7 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
   for (int i = 0; i < 2; i++) {
     c->xch[i].rec = (XRec *)take(nx * sizeof(XRec));
-    c->xch[i].dc = (uint8_t *)take(nx);
+    c->xch[i].mask = (uint32_t *)take(nk * PSC_XW3 * 4);
     c->xch[i].id = (int32_t *)take(nx * 4);
   }
   const size_t sc = (size_t)spill_capacity(n);
@@ -759,7 +760,8 @@ int gather_store(psc_ctx *c, const Cols &dst, int32_t *keyout, bool to_abs, int 
   Exchange xi = xin;
   Spill sp = c->spill;
   if (!in.id) { xi.id = nullptr; sp.id = nullptr; }
-  k_tot<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk, c->cnt, xin.dc, c->tot, cond);
+  k_tot<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, gd.nd, c->cnt,
+                                                              xin.mask, c->tot, cond);
   PSC_LAUNCH_CHECK(c);
   int rc = run_scan1(c, s, cond);
   if (rc) return rc;
@@ -819,8 +821,9 @@ int sort_core(psc_ctx *c, const Cols &src, const Cols &dst, bool from_abs, bool 
     k_reorder<false><<<pblocks, SORT_THREADS, 0, s>>>(gd, np, c->perm, c->key, c->offs_dense, c->base, src, dst, cond);
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_REORDER, s);
-  k_store_reset<<<grid_for(c, (int64_t)nk * 8, SORT_THREADS), SORT_THREADS, 0, s>>>(
-      nk, c->xch[0].dc, c->xch[1].dc, c->base, c->d_flags, (long long)c->capacity, cond);
+  k_store_reset<<<grid_for(c, (int64_t)nk * 16, SORT_THREADS), SORT_THREADS, 0, s>>>(
+      nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, c->xch[0].mask, c->xch[1].mask, c->base, c->d_flags,
+      (long long)c->capacity, cond);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }

@@ -11,10 +11,11 @@
 //   * the warp advances the particles in that shared-memory image IN PLACE, and writes the image's
 //     dynamic columns (positions, momenta) back with one bulk copy per column; q*w, species, id of
 //     a particle that stays in its cell are never rewritten;
-//   * a particle that leaves is appended, as one 32-byte record tagged with the direction code of
-//     its move, to the exchange row of its SOURCE cell (ping-pong buffered);
-//   * the arrivals of a cell are the records of its 8 / 26 neighbours' rows whose code points at
-//     it; they are pushed together with the residents (in the idle lanes of the cell's last
+//   * a particle that leaves is appended, as one 32-byte record, to the exchange row of its
+//     SOURCE cell (ping-pong buffered); the row's header holds one 32-bit mask per direction code
+//     (9 / 27 destination classes) saying which records moved that way;
+//   * the arrivals of a cell are the records of its 8 / 26 neighbours' rows whose direction points
+//     at it: one 4-byte header load per neighbour finds them; they are pushed together with the residents (in the idle lanes of the cell's last
 //     chunk) and filed into the holes the cell's own leavers left, else appended, so that
 //     [0, cnt) stays dense; holes left over are closed by moving particles from the tail.
 // A cell that does not fit the image (more than C particles) is streamed straight from and to
@@ -115,17 +116,20 @@ constexpr int WALK_AC = 128;  // arrival-list window (entries)
 template <bool D3, bool XC>
 struct CellWalker {
   static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4, NDYN = D3 ? 6 : 5;
+  static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
   // bytes of per-warp shared memory for an image of C slots x ncol columns
   __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
-    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + PSC_XCAP /*xrow*/ + 16 /*bar*/;
+    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ + 16 /*bar*/;
   }
   float *buf;      // [ncol][C]
   uint8_t *holes;  // [C]
   uint16_t *arr;   // [WALK_AC]
   int *nbk;        // [32]
-  uint8_t *xrow;   // [PSC_XCAP]
+  unsigned *xrow;  // [32]: per direction code, which of the cell's records so far moved that way
   uint64_t *bar;
+  const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
   int C, ncol, lane;
+  int sx, sy, sz;  // the direction this lane looks at when a cell collects its arrivals (lane = code)
   unsigned lt;
   unsigned parity;
   bool loads_armed;  // bulk loads for the cell about to be processed are in flight
@@ -134,20 +138,22 @@ struct CellWalker {
   bool fast;
   int nh, tcur, nleave, a0, my_start;
 
-  __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_) {
+  __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_, const int *nbt_) {
     C = sd.C;
-    ncol = sd.ncol;
+    ncol = XC ? sd.ncol : (D3 ? 8 : 7);
     lane = lane_;
+    nbt = nbt_;
+    dir_decode<D3>(lane < ND ? lane : STAY, sx, sy, sz);
     lt = lanemask_lt_();
     buf = (float *)wsm;
     holes = (uint8_t *)(buf + ncol * C);
     arr = (uint16_t *)(holes + C);
     nbk = (int *)(arr + WALK_AC);
-    xrow = (uint8_t *)(nbk + 32);
-    bar = (uint64_t *)(xrow + PSC_XCAP);
+    xrow = (unsigned *)(nbk + 32);
+    bar = (uint64_t *)(xrow + 32);
     parity = 0;
     loads_armed = false;
-    xrow[lane] = PSC_XDC_NONE;
+    xrow[lane] = 0u;
     if (lane == 0) {
       mbar_init(bar, 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -161,59 +167,57 @@ struct CellWalker {
     if (loads_armed && lane == 0) {
       const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
       mbar_expect_tx(bar, bytes * (unsigned)ncol);
-      for (int c = 0; c < ncol; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
+      if (XC) {
+        for (int c = 0; c < ncol; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
+      } else {
+#pragma unroll
+        for (int c = 0; c < (D3 ? 8 : 7); c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
+      }
     }
   }
 
-  // the 32 code bytes of cell `src`'s exchange row
-  __device__ __forceinline__ void load_row(const StoreDesc &sd, int src, uint4 &r0, uint4 &r1) {
-    const uint4 *p = reinterpret_cast<const uint4 *>(sd.xin.dc + (size_t)src * PSC_XCAP);
-    r0 = p[0];
-    r1 = p[1];
-  }
   // writes the arrival-list window [a0, a0 + WALK_AC): entry = direction lane << 8 | row index
-  __device__ __forceinline__ void fill_window(const uint4 &r0, const uint4 &r1, bool have) {
-    if (have) {
-      const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
-      const unsigned pat = (unsigned)lane * 0x01010101u;
-      int g = my_start - a0;
-#pragma unroll
-      for (int q = 0; q < 8; q++) {
-        unsigned m = __vcmpeq4(w[q], pat) & 0x01010101u;
-        while (m) {
-          const int j = q * 4 + ((__ffs(m) - 1) >> 3);
-          if (g >= 0 && g < WALK_AC) arr[g] = (uint16_t)((lane << 8) | j);
-          g++;
-          m &= m - 1;
-        }
-      }
+  __device__ __forceinline__ void fill_window(unsigned mask) {
+    int g = my_start - a0;
+    while (mask) {
+      const int j = __ffs(mask) - 1;
+      if (g >= 0 && g < WALK_AC) arr[g] = (uint16_t)((lane << 8) | j);
+      g++;
+      mask &= mask - 1;
     }
     __syncwarp();
   }
 
-  // Start of a cell: where its arrivals are (the neighbours' rows), whether it takes the
-  // shared-memory path, wait for its resident run.  (cx, cy, cz): the cell's coordinates.
-  __device__ __forceinline__ void begin_cell(const StoreDesc &sd, const GridDesc &gd, int key_, int n_,
-                                             int base_, int cap_, int cx, int cy, int cz) {
+  // key of the cell that reaches cell (lx, ly, lz) of this tile by a move in this lane's direction
+  template <class TG>
+  __device__ __forceinline__ int source_key(const TG &tg, int lx, int ly, int lz) const {
+    int qx = lx - sx, qy = ly - sy, qz = lz - sz;
+    const int tx = D3 ? (qx < 0 ? -1 : (qx >= tg.bs[0] ? 1 : 0)) : 0;
+    const int ty = qy < 0 ? -1 : (qy >= tg.bs[1] ? 1 : 0);
+    const int tz = qz < 0 ? -1 : (qz >= tg.bs[2] ? 1 : 0);
+    qx -= tx * tg.bs[0];
+    qy -= ty * tg.bs[1];
+    qz -= tz * tg.bs[2];
+    return nbt[(tz + 1) * 9 + (ty + 1) * 3 + (tx + 1)] + (qz * tg.bs[1] + qy) * tg.bs[0] + qx;
+  }
+
+  // Start of a cell: where its arrivals are (the neighbours' row headers), whether it takes the
+  // shared-memory path, wait for its resident run.  (lx, ly, lz): the cell inside the tile.
+  template <class TG>
+  __device__ __forceinline__ void begin_cell(const StoreDesc &sd, const TG &tg, int key_, int n_,
+                                             int base_, int cap_, int lx, int ly, int lz) {
     key = key_;
     n = n_;
     base = base_;
     cap = cap_;
     const bool have = lane < ND && lane != STAY;
-    uint4 r0 = make_uint4(~0u, ~0u, ~0u, ~0u), r1 = r0;
-    int cntm = 0;
+    unsigned mask = 0;
     if (have) {
-      int sx, sy, sz;
-      dir_decode<D3>(lane, sx, sy, sz);
-      const int src = cell_key(gd, D3 ? wrap_cell(cx - sx, gd.n[0]) : 0, wrap_cell(cy - sy, gd.n[1]),
-                               wrap_cell(cz - sz, gd.n[2]));
+      const int src = source_key(tg, lx, ly, lz);
       nbk[lane] = src;
-      load_row(sd, src, r0, r1);
-      const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
-      const unsigned pat = (unsigned)lane * 0x01010101u;
-#pragma unroll
-      for (int q = 0; q < 8; q++) cntm += __popc(__vcmpeq4(w[q], pat) & 0x01010101u);
+      mask = sd.xin.mask[(size_t)src * XW + lane];
     }
+    const int cntm = __popc(mask);
     int inc = cntm;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -223,7 +227,7 @@ struct CellWalker {
     na = __shfl_sync(0xffffffffu, inc, 31);
     my_start = inc - cntm;
     a0 = 0;
-    if (na) fill_window(r0, r1, have);
+    if (na) fill_window(mask);
     fast = n + na <= C;
     nh = 0;
     tcur = fast ? n : 0;  // shared-memory path: append cursor; global path: write cursor
@@ -251,10 +255,9 @@ struct CellWalker {
       if (v0 + 32 - n > a0 + WALK_AC) {  // next window of the arrival list (cells with > 128 arrivals)
         a0 = v0 > n ? v0 - n : 0;
         const bool have = lane < ND && lane != STAY;
-        uint4 r0 = make_uint4(~0u, ~0u, ~0u, ~0u), r1 = r0;
-        if (have) load_row(sd, nbk[lane], r0, r1);
+        const unsigned mask = have ? sd.xin.mask[(size_t)nbk[lane] * XW + lane] : 0u;
         __syncwarp();
-        fill_window(r0, r1, have);
+        fill_window(mask);
       }
       if (act && isarr) {
         const int e = arr[v - n - a0];
@@ -326,7 +329,7 @@ struct CellWalker {
   __device__ __forceinline__ int leaver_index(bool leave, int dc) {
     const unsigned m = __ballot_sync(0xffffffffu, leave);
     const int xi = nleave + __popc(m & lt);
-    if (leave && xi < PSC_XCAP) xrow[xi] = (uint8_t)dc;
+    if (leave && xi < PSC_XCAP) atomicOr(&xrow[dc], 1u << xi);
     nleave += __popc(m);
     return xi;
   }
@@ -457,10 +460,9 @@ struct CellWalker {
       newcnt = tcur < cap ? tcur : cap;
     }
     if (lane == 0) sd.cnt[key] = newcnt;
-    if (lane < PSC_XCAP / 4)
-      reinterpret_cast<unsigned *>(sd.xout.dc + (size_t)key * PSC_XCAP)[lane] = reinterpret_cast<const unsigned *>(xrow)[lane];
+    if (lane < XW) sd.xout.mask[(size_t)key * XW + lane] = xrow[lane];
     __syncwarp();
-    xrow[lane] = PSC_XDC_NONE;
+    xrow[lane] = 0u;
     if (lane == 0) bulk_wait_read0();  // the image may be overwritten once the copy engine has read it
     __syncwarp();
     if (next_n > 0) issue_loads(sd, next_n, next_base);
