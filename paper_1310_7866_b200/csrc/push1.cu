@@ -39,8 +39,8 @@
 namespace {
 
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
-// rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 ddx (2-d: v_x),
-// 5 ddy, 6 ddz, 7 qw.  The drain reuses rows [0, NV) of a drained entry as its scratch column,
+// rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 endx (2-d: v_x),
+// 5 endy, 6 endz, 7 qw.  The drain reuses rows [0, NV) of a drained entry as its scratch column,
 // hence 12 rows in 3-d.
 constexpr int QROWS2 = 8, QROWS3 = 12;
 
@@ -225,7 +225,7 @@ __device__ __forceinline__ void moments_to_values(float (&acc)[D3 ? 12 : 8]) {
   }
 }
 
-// Walks the straight line a -> a + dd (cells; at most one face crossing per direction because
+// Walks the straight line a -> end (cells; at most one face crossing per direction because
 // dt <= dx/2) and deposits every segment -- the slow path of the kernel below,
 // taken by the trajectories that leave their cell.
 // The segments' currents are added with shared-memory atomics, which are compare-and-swap loops
@@ -237,12 +237,12 @@ __device__ __forceinline__ void moments_to_values(float (&acc)[D3 ? 12 : 8]) {
 // from the table `rel` ([NV], the order of vb_values).
 template <bool D3, class TG>
 __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, int lx,
-                                        int ly, int lz, float ax, float ay, float az, float ddx,
-                                        float ddy, float ddz, float fx, float fy, float fz,
+                                        int ly, int lz, float ax, float ay, float az, float endx,
+                                        float endy, float endz, float fx, float fy, float fz,
                                         float qvx, const int *__restrict__ rel,
                                         float *__restrict__ scr, int rot) {
   constexpr int NV = D3 ? 12 : 8;
-  const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
+  const float ddx = endx - ax, ddy = endy - ay, ddz = endz - az;
   const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
   const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
   const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
@@ -300,13 +300,13 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
     const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
-    const float ddx = q[4 * QCAP + e], ddy = q[5 * QCAP + e], ddz = q[6 * QCAP + e];
+    const float ex = q[4 * QCAP + e], ey = q[5 * QCAP + e], ez = q[6 * QCAP + e];
     const float qw = q[7 * QCAP + e];
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
-    // 2-d: the ddx slot carries v_x: the out-of-plane current needs the velocity
+    // 2-d: the endx slot carries v_x: the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
-    const float qvx = D3 ? 0.f : qw * gd.inv_dV * ddx;
-    vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ddx : 0.f, ddy, ddz, fx, fy, fz,
+    const float qvx = D3 ? 0.f : qw * gd.inv_dV * ex;
+    vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ex : 0.f, ey, ez, fx, fy, fz,
                 qvx, rel, q + e, lane % (D3 ? 12 : 8));
   }
   __syncwarp();
@@ -407,6 +407,72 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
 
+  // One particle: gather (Eq. 11 with b1 weights; each component from its own Yee points:
+  // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l (a < 1/2, weight
+  // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28), velocity.
+  auto kick = [&](const float *cF, float ax, float ay, float az, float &ux, float &uy, float &uz, int sp) {
+    const bool hy = ay >= 0.5f, hz = az >= 0.5f, hx = D3 && ax >= 0.5f;
+    const float gy = hy ? ay - 0.5f : ay + 0.5f, gz = hz ? az - 0.5f : az + 0.5f;
+    const float gx = hx ? ax - 0.5f : ax + 0.5f;
+    const int oy = hy ? 0 : -fs1, oz = hz ? 0 : -fs2, ox = (!D3 || hx) ? 0 : -1;
+    const float ex = gather1<D3>(cF + ox, fs1, fs2, gx, ay, az);
+    const float ey = gather1<D3>(cF + fvol + oy, fs1, fs2, ax, gy, az);
+    const float ez = gather1<D3>(cF + 2 * fvol + oz, fs1, fs2, ax, ay, gz);
+    const float bx = gather1<D3>(cF + 3 * fvol + oy + oz, fs1, fs2, ax, gy, gz);
+    const float by = gather1<D3>(cF + 4 * fvol + ox + oz, fs1, fs2, gx, ay, gz);
+    const float bz = gather1<D3>(cF + 5 * fvol + ox + oy, fs1, fs2, gx, gy, az);
+    boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp & (PSC_MAX_SPECIES - 1)]);
+  };
+  // The move x^{n+1/2} -> x^{n+3/2} (Eq. 26) in cells, written with explicit roundings: the pass
+  // over a cell's leavers recomputes it from the stored momentum and must get the same bits.
+  auto move = [&](float ax, float ay, float az, float ux, float uy, float uz, float &vx, float &endx,
+                  float &endy, float &endz) {
+    const float ig = rsqrt_ge1(__fmaf_rn(ux, ux, __fmaf_rn(uy, uy, __fmaf_rn(uz, uz, 1.0f))));
+    vx = __fmul_rn(ux, ig);
+    endx = D3 ? __fmaf_rn(vx, cdx, ax) : 0.f;
+    endy = __fmaf_rn(__fmul_rn(uy, ig), cdy, ay);
+    endz = __fmaf_rn(__fmul_rn(uz, ig), cdz, az);
+  };
+  // a trajectory that leaves its cell: its record goes to the cell's exchange row (offsets
+  // relative to the destination cell), its current through the queue (all its segments)
+  auto depart = [&](bool cross, int xi, int packed, int lx, int ly, int lz, float ax, float ay, float az,
+                    float endx, float endy, float endz, float vx, float ux, float uy, float uz, float qw,
+                    int sp, float x2d, int id) {
+    const unsigned cm = __ballot_sync(0xffffffffu, cross);
+    if (cross) {
+      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      Part pr;
+      pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
+      pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+      pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+      pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
+      float w[8];
+      Walker::to_words(w, pr, x2d);
+      int dest = 0;
+      if (xi >= PSC_XCAP)
+        dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
+                        wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
+      wk.emit(sd, gd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+      const int e = qcnt + __popc(cm & lt);
+      myQ[0 * QCAP + e] = __int_as_float(packed);
+      myQ[1 * QCAP + e] = ax;
+      myQ[2 * QCAP + e] = ay;
+      myQ[3 * QCAP + e] = az;
+      myQ[4 * QCAP + e] = D3 ? endx : vx;
+      myQ[5 * QCAP + e] = endy;
+      myQ[6 * QCAP + e] = endz;
+      myQ[7 * QCAP + e] = qw;
+    }
+    qcnt += __popc(cm);
+    __syncwarp();
+    if (qcnt >= 32) {
+      qcnt -= 32;
+      drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
+    }
+  };
+
   // The warp's cells: warp, warp + nwarps, ...  The resident run of the next cell is requested
   // from the copy engine as soon as the image of the current one has been written back.
   if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
@@ -425,8 +491,30 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
 #pragma unroll
     for (int i = 0; i < NV; i++) acc[i] = 0.f;
 
+    // ---- full chunks of residents of the cell image: no bounds, no arrivals ---------------------
+    const int nfull = wk.fast ? (wk.n & ~31) : 0;
 #pragma unroll 1
-    for (int v0 = 0; v0 < ntot; v0 += 32) {
+    for (int v0 = 0; v0 < nfull; v0 += 32) {
+      Part p;
+      wk.load_image(v0 + lane, p);
+      kick(cF, p.ax, p.ay, p.az, p.ux, p.uy, p.uz, p.sp);
+      float vx;
+      Part pn = p;
+      move(p.ax, p.ay, p.az, p.ux, p.uy, p.uz, vx, pn.ax, pn.ay, pn.az);
+      const bool stay = (!D3 || (pn.ax >= 0.f && pn.ax < 1.f)) && pn.ay >= 0.f && pn.ay < 1.f &&
+                        pn.az >= 0.f && pn.az < 1.f;
+      // Villasenor-Buneman: a trajectory that stays in the cell is one segment, summed in registers
+      const float qs = stay ? p.qw : 0.f;
+      vb_moments<D3>(acc, p.ax, p.ay, p.az, pn.ax, pn.ay, pn.az, qs * gd.cur[0], qs * gd.cur[1],
+                     qs * gd.cur[2], qs * gd.inv_dV * vx);
+      wk.store_image(v0, true, !stay, pn);
+    }
+
+    // ---- the rest: the last residents, the arrivals (reorder on load), cells on the global path
+    bool leavers_done = !wk.fast;
+    int v0 = nfull;
+#pragma unroll 1
+    do {
       Part cur;
       bool isarr;
       float x2d;
@@ -435,86 +523,49 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       const float ax = D3 ? cur.ax : 0.f, ay = cur.ay, az = cur.az, qw = cur.qw;
       float ux = cur.ux, uy = cur.uy, uz = cur.uz;
       const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
-
-      // ---- gather (Eq. 11 with b1 weights; each component from its own Yee points) --------
-      // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l
-      // (a < 1/2, weight a + 1/2) or l, l+1 (weight a - 1/2)
-      const bool hy = ay >= 0.5f, hz = az >= 0.5f, hx = D3 && ax >= 0.5f;
-      const float gy = hy ? ay - 0.5f : ay + 0.5f, gz = hz ? az - 0.5f : az + 0.5f;
-      const float gx = hx ? ax - 0.5f : ax + 0.5f;
-      const int oy = hy ? 0 : -fs1, oz = hz ? 0 : -fs2, ox = (!D3 || hx) ? 0 : -1;
-      const float ex = gather1<D3>(cF + ox, fs1, fs2, gx, ay, az);
-      const float ey = gather1<D3>(cF + fvol + oy, fs1, fs2, ax, gy, az);
-      const float ez = gather1<D3>(cF + 2 * fvol + oz, fs1, fs2, ax, ay, gz);
-      const float bx = gather1<D3>(cF + 3 * fvol + oy + oz, fs1, fs2, ax, gy, gz);
-      const float by = gather1<D3>(cF + 4 * fvol + ox + oz, fs1, fs2, gx, ay, gz);
-      const float bz = gather1<D3>(cF + 5 * fvol + ox + oy, fs1, fs2, gx, gy, az);
-
-      // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
-      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
-      const float ig = rsqrt_ge1(fmaf(ux, ux, fmaf(uy, uy, fmaf(uz, uz, 1.0f))));
-      const float vx = ux * ig;
-      const float ddx = D3 ? vx * cdx : 0.f;  // displacement in cells
-      const float ddy = (uy * ig) * cdy, ddz = (uz * ig) * cdz;
-      const float endx = ax + ddx, endy = ay + ddy, endz = az + ddz;
-      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
-      const int dc = dir_code<D3>(sxd, syd, szd);
-      const bool cross = act && dc != (D3 ? 13 : 4);
-
-      // ---- Villasenor-Buneman deposit ---------------------------------------------------------
-      // a trajectory that stays in the cell is one segment: its currents go to the per-cell
-      // register sums; one that leaves goes through the per-warp queue (all its segments)
+      kick(cF, ax, ay, az, ux, uy, uz, sp);
+      float vx, endx, endy, endz;
+      move(ax, ay, az, ux, uy, uz, vx, endx, endy, endz);
+      const bool stay = (!D3 || (endx >= 0.f && endx < 1.f)) && endy >= 0.f && endy < 1.f &&
+                        endz >= 0.f && endz < 1.f;
+      const bool cross = act && !stay;
       {
         const float qs = (cross || !act) ? 0.f : qw;
         vb_moments<D3>(acc, ax, ay, az, endx, endy, endz, qs * gd.cur[0], qs * gd.cur[1],
                        qs * gd.cur[2], qs * gd.inv_dV * vx);
       }
-      const unsigned cm = __ballot_sync(0xffffffffu, cross);
-      if (cm) {
-        const int xi = wk.leaver_index(cross, dc);
-        if (cross) {
-          // the particle's record goes to this cell's exchange row (offsets relative to the
-          // destination cell), its trajectory to the queue
-          if (wk.fast && !isarr) wk.extras(sd, v0 + lane, x2d, id);
-          Part pr;
-          pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
-          pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-          pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-          pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
-          float w[8];
-          Walker::to_words(w, pr, x2d);
-          int dest = 0;
-          if (xi >= PSC_XCAP)
-            dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
-                            wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-          Walker::write_record(sd, gd, kbase + ci, xi, w, id, dest);
-          const int e = qcnt + __popc(cm & lt);
-          myQ[0 * QCAP + e] = __int_as_float(packed);
-          myQ[1 * QCAP + e] = ax;
-          myQ[2 * QCAP + e] = ay;
-          myQ[3 * QCAP + e] = az;
-          myQ[4 * QCAP + e] = D3 ? ddx : vx;
-          myQ[5 * QCAP + e] = ddy;
-          myQ[6 * QCAP + e] = ddz;
-          myQ[7 * QCAP + e] = qw;
-        }
-        qcnt += __popc(cm);
-        __syncwarp();
-        if (qcnt >= 32) {
-          qcnt -= 32;
-          drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
-        }
-      }
-
-      // ---- file the particles that stay: in place (residents) or into a hole (arrivals) -----
       Part pn;
       pn.ax = endx; pn.ay = endy; pn.az = endz;
       pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
-      wk.store(sd, v0, act, isarr, cross, pn, x2d, id);
-      if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
-    }
+      if (wk.fast) wk.store_image(v0, act && !isarr, cross, pn);
+      if (!leavers_done) {
+        // all residents of the image are advanced: the cell's leavers, 32 at a time
+        leavers_done = true;
+        const int nl = wk.nh;
+#pragma unroll 1
+        for (int i0 = 0; i0 < nl; i0 += 32) {
+          const bool al = i0 + lane < nl;
+          Part q;
+          float qx2d = 0.f;
+          int qid = 0;
+          q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
+          if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
+          float qvx, qex, qey, qez;
+          move(D3 ? q.ax : 0.f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
+          depart(al, i0 + lane, packed, lx, ly, lz, D3 ? q.ax : 0.f, q.ay, q.az, qex, qey, qez, qvx, q.ux,
+                 q.uy, q.uz, q.qw, q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
+        }
+        wk.nleave = nl;
+      }
+      // arrivals that leave again at once, and every leaver of a cell on the global path
+      const bool late = cross && (isarr || !wk.fast);
+      if (__any_sync(0xffffffffu, late)) {
+        const int xi = wk.leaver_slot(late);
+        depart(late, xi, packed, lx, ly, lz, ax, ay, az, endx, endy, endz, vx, ux, uy, uz, qw, sp, x2d, id);
+      }
+      wk.place(sd, v0, act, isarr, cross, pn, x2d, id);
+      v0 += 32;
+    } while (v0 < ntot);
 
     // ---- the cell is done: its in-cell currents take one warp reduction and one shared add per
     // J point; its image goes back to global memory and the next cell's run is requested
@@ -523,6 +574,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       moments_to_values<D3>(acc);
       if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
       else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(acc), lane);
+      if (!(fabsf(r) < 3.0e38f)) bad |= PSC_F_NAN;  // a non-finite momentum poisons the cell's sums
       if (writer) {
         const int node = D3 ? ((lz + 1) * tg.je[1] + (ly + 1)) * tg.je[0] + (lx + 1)
                             : (lz + 1) * tg.je[1] + (ly + 1);

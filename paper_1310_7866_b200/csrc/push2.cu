@@ -262,6 +262,40 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   const float *sBx = sF + 3 * tg.tvol, *sBy = sF + 4 * tg.tvol, *sBz = sF + 5 * tg.tvol;
   uint32_t bad = 0;
 
+  // The move x^{n+1/2} -> x^{n+3/2} (Eq. 26) in cells, written with explicit roundings: the pass
+  // over a cell's leavers recomputes it from the stored momentum and must get the same bits.
+  const float cdx = D3 ? gd.dt_dx[0] : 0.f, cdy = gd.dt_dx[1], cdz = gd.dt_dx[2];
+  auto move = [&](float ax, float ay, float az, float ux, float uy, float uz, float &vx, float &endx,
+                  float &endy, float &endz) {
+    const float ig = rsqrt_ge1(__fmaf_rn(ux, ux, __fmaf_rn(uy, uy, __fmaf_rn(uz, uz, 1.0f))));
+    vx = __fmul_rn(ux, ig);
+    endx = D3 ? __fmaf_rn(vx, cdx, ax) : ax;
+    endy = __fmaf_rn(__fmul_rn(uy, ig), cdy, ay);
+    endz = __fmaf_rn(__fmul_rn(uz, ig), cdz, az);
+  };
+  // a particle that leaves its cell: its record (offsets relative to the destination cell) goes
+  // to the cell's exchange row
+  auto depart = [&](bool leave, int xi, int lx, int ly, int lz, float endx, float endy, float endz,
+                    float ux, float uy, float uz, float qw, int sp, float x2d, int id) {
+    if (leave) {
+      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
+      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
+      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      Part pr;
+      pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
+      pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
+      pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+      pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
+      float w[8];
+      Walker::to_words(w, pr, x2d);
+      int dest = 0;
+      if (xi >= PSC_XCAP)
+        dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
+                        wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
+      wk.emit(sd, gd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+    }
+  };
+
   if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
@@ -271,6 +305,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int np_cell = wk.n + wk.na;  // residents + arrivals (reorder on load)
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
+    bool leavers_done = !wk.fast;
 #pragma unroll 1
     for (int base = 0; base < np_cell; base += 32) {
       Part cur;
@@ -296,10 +331,8 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
 
       // ---- Boris (Eq. 27-28) and move (Eq. 26) ----------------------------------------------
       boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp]);
-      const float ig = rsqrt_ge1(1.0f + ux * ux + uy * uy + uz * uz);
-      const float vx = ux * ig, vy = uy * ig, vz = uz * ig;
-      const float endx = D3 ? ax + vx * gd.dt_dx[0] : ax;
-      const float endy = ay + vy * gd.dt_dx[1], endz = az + vz * gd.dt_dx[2];
+      float vx, endx, endy, endz;
+      move(ax, ay, az, ux, uy, uz, vx, endx, endy, endz);
 
       // ---- Esirkepov deposit ------------------------------------------------------------------
       {
@@ -406,32 +439,40 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       }
 
       // ---- file the particle: in place / into a hole if it stays, as a record if it leaves -----
-      const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
-      const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
-      const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
-      const int dc = dir_code<D3>(sxd, syd, szd);
-      const bool leave = act && dc != Walker::STAY;
+      const bool stay = (!D3 || (endx >= 0.f && endx < 1.f)) && endy >= 0.f && endy < 1.f &&
+                        endz >= 0.f && endz < 1.f;
+      const bool leave = act && !stay;
       Part pn;
       pn.ax = endx; pn.ay = endy; pn.az = endz;
       pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
-      if (__any_sync(0xffffffffu, leave)) {
-        const int xi = wk.leaver_index(leave, dc);
-        if (leave) {
-          if (wk.fast && !isarr) wk.extras(sd, base + lane, x2d, id);
-          Part pr = pn;
-          pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
-          pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
-          pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
-          float w[8];
-          Walker::to_words(w, pr, x2d);
-          int dest = 0;
-          if (xi >= PSC_XCAP)
-            dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
-                            wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-          Walker::write_record(sd, gd, kbase + ci, xi, w, id, dest);
+      if (wk.fast) wk.store_image(base, act && !isarr, leave, pn);
+      if (!leavers_done && base + 32 >= wk.n) {
+        // all residents of the image are advanced: the records of the cell's leavers, 32 at a
+        // time (their deposit is done: Esirkepov's stencil covers the move across the face)
+        leavers_done = true;
+        const int nl = wk.nh;
+#pragma unroll 1
+        for (int i0 = 0; i0 < nl; i0 += 32) {
+          const bool al = i0 + lane < nl;
+          Part q;
+          float qx2d = 0.f;
+          int qid = 0;
+          q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
+          if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
+          float qvx, qex, qey, qez;
+          move(D3 ? q.ax : 0.25f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
+          depart(al, i0 + lane, lx, ly, lz, qex, qey, qez, q.ux, q.uy, q.uz, q.qw,
+                 q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
         }
+        wk.nleave = nl;
       }
-      wk.store(sd, base, act, isarr, leave, pn, x2d, id);
+      // arrivals that leave again at once, and every leaver of a cell on the global path
+      const bool late = leave && (isarr || !wk.fast);
+      if (__any_sync(0xffffffffu, late)) {
+        const int xi = wk.leaver_slot(late);
+        depart(late, xi, lx, ly, lz, endx, endy, endz, ux, uy, uz, qw, sp, x2d, id);
+      }
+      wk.place(sd, base, act, isarr, leave, pn, x2d, id);
       if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
     const int nx = ci + nwarps;

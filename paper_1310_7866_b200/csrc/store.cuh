@@ -10,7 +10,10 @@
 //     so the SM's load/store pipe never sees the particle stream;
 //   * the warp advances the particles in that shared-memory image IN PLACE, and writes the image's
 //     dynamic columns (positions, momenta) back with one bulk copy per column; q*w, species, id of
-//     a particle that stays in its cell are never rewritten;
+//     a particle that stays in its cell are never rewritten.  A resident that leaves keeps its OLD
+//     offsets in the image next to its NEW momentum and is only noted in the hole list; once all
+//     residents of the cell are done, one pass over that list (32 leavers at a time instead of one
+//     or two per chunk) recomputes the move bit-identically, writes the records and deposits;
 //   * a particle that leaves is appended, as one 32-byte record, to the exchange row of its
 //     SOURCE cell (ping-pong buffered); the row's header holds one 32-bit mask per direction code
 //     (9 / 27 destination classes) saying which records moved that way;
@@ -119,13 +122,14 @@ struct CellWalker {
   static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
   // bytes of per-warp shared memory for an image of C slots x ncol columns
   __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
-    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ + 16 /*bar*/;
+    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ + 12 * 4 /*hbm*/ + 16 /*bar*/;
   }
   float *buf;      // [ncol][C]
   uint8_t *holes;  // [C]
   uint16_t *arr;   // [WALK_AC]
   int *nbk;        // [32]
   unsigned *xrow;  // [32]: per direction code, which of the cell's records so far moved that way
+  unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole (its resident left)
   uint64_t *bar;
   const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
   int C, ncol, lane;
@@ -150,7 +154,8 @@ struct CellWalker {
     arr = (uint16_t *)(holes + C);
     nbk = (int *)(arr + WALK_AC);
     xrow = (unsigned *)(nbk + 32);
-    bar = (uint64_t *)(xrow + 32);
+    hbm = xrow + 32;
+    bar = (uint64_t *)(hbm + 12);
     parity = 0;
     loads_armed = false;
     xrow[lane] = 0u;
@@ -305,6 +310,59 @@ struct CellWalker {
     return act;
   }
 
+  // resident v of the image (shared-memory path), no bounds check
+  __device__ __forceinline__ void load_image(int v, Part &p) const {
+    const float *q = buf + v;
+    if (D3) {
+      p.ax = q[0]; p.ay = q[C]; p.az = q[2 * C]; p.ux = q[3 * C]; p.uy = q[4 * C]; p.uz = q[5 * C];
+      p.qw = q[6 * C]; p.sp = __float_as_int(q[7 * C]);
+    } else {
+      p.ax = 0.f;
+      p.ay = q[0]; p.az = q[C]; p.ux = q[2 * C]; p.uy = q[3 * C]; p.uz = q[4 * C];
+      p.qw = q[5 * C]; p.sp = __float_as_int(q[6 * C]);
+    }
+  }
+
+  // Files resident v0 + lane of the image after its push: the momentum always, the offsets only if
+  // it stays; a leaver keeps its old offsets and is noted as a hole (see leaver()).
+  __device__ __forceinline__ void store_image(int v0, bool act, bool leave, const Part &pn) {
+    const int v = v0 + lane;
+    const unsigned mrl = __ballot_sync(0xffffffffu, act && leave);
+    if (act) {
+      float *q = buf + v;
+      if (D3) {
+        if (!leave) { q[0] = pn.ax; q[C] = pn.ay; q[2 * C] = pn.az; }
+        q[3 * C] = pn.ux; q[4 * C] = pn.uy; q[5 * C] = pn.uz;
+      } else {
+        if (!leave) { q[0] = pn.ay; q[C] = pn.az; }
+        q[2 * C] = pn.ux; q[3 * C] = pn.uy; q[4 * C] = pn.uz;
+      }
+      if (leave) holes[nh + __popc(mrl & lt)] = (uint8_t)v;
+    }
+    if (lane == 0) hbm[v0 >> 5] = mrl;
+    nh += __popc(mrl);
+  }
+
+  // leaver i of the hole list: its image values (OLD offsets, NEW momentum) and optional columns
+  __device__ __forceinline__ int leaver(const StoreDesc &sd, int i, Part &p, float &x2d, int &id) const {
+    const int h = holes[i];
+    load_image(h, p);
+    x2d = 0.f;
+    id = 0;
+    if (XC) {
+      if (sd.icol_x2d >= 0) x2d = buf[sd.icol_x2d * C + h];
+      if (sd.icol_id >= 0) id = __float_as_int(buf[sd.icol_id * C + h]);
+    }
+    return h;
+  }
+
+  // writes record xi of the current cell's row (moved by direction code dc), or spills it
+  __device__ __forceinline__ void emit(const StoreDesc &sd, const GridDesc &gd, int xi, int dc,
+                                       const float (&w)[8], int id, int dest_key) {
+    if (xi < PSC_XCAP) atomicOr(&xrow[dc], 1u << xi);
+    write_record(sd, gd, key, xi, w, id, dest_key);
+  }
+
   // optional values of a RESIDENT particle on the shared-memory path (needed only if it leaves)
   __device__ __forceinline__ void extras(const StoreDesc &sd, int v, float &x2d, int &id) {
     if (XC) {
@@ -325,11 +383,10 @@ struct CellWalker {
   }
 
   // index of the next leaver's record in the cell's exchange row (all lanes; `leave`: this lane
-  // leaves with direction code dc).  Records past the row's capacity go to the spill list.
-  __device__ __forceinline__ int leaver_index(bool leave, int dc) {
+  // leaves).  Records past the row's capacity go to the spill list (emit()).
+  __device__ __forceinline__ int leaver_slot(bool leave) {
     const unsigned m = __ballot_sync(0xffffffffu, leave);
     const int xi = nleave + __popc(m & lt);
-    if (leave && xi < PSC_XCAP) atomicOr(&xrow[dc], 1u << xi);
     nleave += __popc(m);
     return xi;
   }
@@ -350,34 +407,21 @@ struct CellWalker {
     }
   }
 
-  // Files the advanced particle of every lane that STAYS in the cell (stay), notes the hole of
-  // every resident that leaves (leave).  pn: the new values (offsets in [0,1)).
-  __device__ __forceinline__ void store(const StoreDesc &sd, int v0, bool act, bool isarr, bool leave,
+  // General form (any chunk; both paths), second half: after the residents of the chunk went
+  // through store_image() and -- on the shared-memory path -- the cell's leavers were processed,
+  // an ARRIVAL that stays is filed into a hole of the list, else appended.  Global path: every
+  // particle of the chunk that stays is compacted to the front of the cell.  pn: the new values.
+  __device__ __forceinline__ void place(const StoreDesc &sd, int v0, bool act, bool isarr, bool leave,
                                         const Part &pn, float x2d, int id) {
-    const int v = v0 + lane;
     const bool stay = act && !leave;
     if (fast) {
-      const bool rl = act && leave && !isarr;
-      const unsigned mrl = __ballot_sync(0xffffffffu, rl);
-      if (rl) {
-        holes[nh + __popc(mrl & lt)] = (uint8_t)v;
-        buf[v] = -1.f;  // column 0 (an offset, >= 0 for a particle) marks the hole
-      }
-      nh += __popc(mrl);
-      if (stay && !isarr) {
-        float *q = buf + v;
-        if (D3) {
-          q[0] = pn.ax; q[C] = pn.ay; q[2 * C] = pn.az; q[3 * C] = pn.ux; q[4 * C] = pn.uy; q[5 * C] = pn.uz;
-        } else {
-          q[0] = pn.ay; q[C] = pn.az; q[2 * C] = pn.ux; q[3 * C] = pn.uy; q[4 * C] = pn.uz;
-        }
-      }
       const unsigned ma = __ballot_sync(0xffffffffu, stay && isarr);
       if (ma) {
         __syncwarp();
         if (stay && isarr) {
           const int r = __popc(ma & lt);
           const int slot = r < nh ? (int)holes[nh - 1 - r] : tcur + (r - nh);
+          if (r < nh) atomicAnd(&hbm[slot >> 5], ~(1u << (slot & 31)));
           float w[8];
           to_words(w, pn, x2d);
           if (slot < cap) {
@@ -435,7 +479,7 @@ struct CellWalker {
         int done = 0;
         for (int t0 = m; t0 < n; t0 += 32) {
           const int s = t0 + lane;
-          const bool valid = s < n && buf[s] >= 0.f;
+          const bool valid = s < n && !((hbm[s >> 5] >> (s & 31)) & 1u);
           const unsigned mv = __ballot_sync(0xffffffffu, valid);
           if (valid) {
             const int h = holes[done + __popc(mv & lt)];  // ascending list: its first entries are < m
