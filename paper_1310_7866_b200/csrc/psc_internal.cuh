@@ -86,6 +86,7 @@ struct StoreDesc {
   Exchange xin, xout;
   Spill spill;
   int C;           // slots of the per-warp cell image (multiple of 32, <= 256)
+  int32_t *bigflag;  // [ntiles]: the image launch left a cell of this tile to the BIG launch
   uint32_t *flags;
 };
 
@@ -147,7 +148,7 @@ struct psc_ctx {
   void *ws;
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
-  int32_t *key, *perm, *cell_idx, *offs_dense, *base, *cnt, *cursor, *big_list, *tot, *doffs;
+  int32_t *key, *perm, *cell_idx, *offs_dense, *base, *cnt, *cursor, *big_list, *tot, *doffs, *bigflag;
   long long *pack, *packloc, *scan_tmp;
   Exchange xch[2];
   Spill spill;

@@ -332,14 +332,17 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
   }
 }
 
-// XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id)
-template <bool D3, int CBS, int THREADS, int MINB, bool XC>
+// XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id).
+// BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
+// launch for the tiles in which the first one had to leave a cell out.
+template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
   extern __shared__ __align__(128) unsigned char smraw[];
+  if (BIG && !sd.bigflag[blockIdx.x]) return;
   constexpr int NV = D3 ? 12 : 8;
-  using Walker = CellWalker<D3, XC>;
+  using Walker = CellWalker<D3, XC, BIG>;
   TileGeom<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
@@ -363,7 +366,6 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
               n2 = wrap_cell(b2 + t / 9 - 1, gd.nb[2]);
     sNbT[t] = ((n2 * gd.nb[1] + n1) * gd.nb[0] + (D3 ? n0 : 0)) * tg.cpb;
   }
-
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
   if (threadIdx.x < NV) {  // J points of the NV in-cell currents, relative to the cell's node
     const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1], jv = tg.jvol;
@@ -406,10 +408,11 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     writer = (lane & 3) == 0;
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
+  bool left_out = false;  // this warp met a cell that does not fit the image
 
   // One particle: gather (Eq. 11 with b1 weights; each component from its own Yee points:
   // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l (a < 1/2, weight
-  // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28), velocity.
+  // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28).
   auto kick = [&](const float *cF, float ax, float ay, float az, float &ux, float &uy, float &uz, int sp) {
     const bool hy = ay >= 0.5f, hz = az >= 0.5f, hx = D3 && ax >= 0.5f;
     const float gy = hy ? ay - 0.5f : ay + 0.5f, gz = hz ? az - 0.5f : az + 0.5f;
@@ -454,7 +457,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       if (xi >= PSC_XCAP)
         dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
                         wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-      wk.emit(sd, gd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+      wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
       const int e = qcnt + __popc(cm & lt);
       myQ[0 * QCAP + e] = __int_as_float(packed);
       myQ[1 * QCAP + e] = ax;
@@ -473,15 +476,28 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     }
   };
 
-  // The warp's cells: warp, warp + nwarps, ...  The resident run of the next cell is requested
-  // from the copy engine as soon as the image of the current one has been written back.
+  // The warp's cells: warp, warp + nwarps, ...  The header words that tell a cell's arrivals are
+  // requested one cell ahead; the resident run of the next cell is requested from the copy engine
+  // as soon as the image of the current one has been written back.
+  int src_next;
+  unsigned mask_next = wk.fetch_mask(sd, tg, warp, src_next);
   if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
+    const int nx = ci + nwarps;
+    const int next_n = nx < tg.cpb ? sCnt[nx] : 0, next_base = nx < tg.cpb ? sBase[nx] : 0;
+    const unsigned mask = mask_next;
+    const int src = src_next;
+    mask_next = wk.fetch_mask(sd, tg, nx, src_next);
+    wk.begin_cell(kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], mask, src);
+    if (wk.fits == BIG) {  // the other launch's cell
+      left_out = true;
+      wk.skip_cell(sd, next_n, next_base);
+      continue;
+    }
     const int lx = ci % tg.bs[0];
     const int lt_ = ci / tg.bs[0];
     const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
-    wk.begin_cell(sd, tg, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], lx, ly, lz);
     const int ntot = wk.n + wk.na;
     const int packed = lx | (ly << 10) | (lz << 20);
     // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
@@ -491,81 +507,76 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
 #pragma unroll
     for (int i = 0; i < NV; i++) acc[i] = 0.f;
 
-    // ---- full chunks of residents of the cell image: no bounds, no arrivals ---------------------
-    const int nfull = wk.fast ? (wk.n & ~31) : 0;
+    if (!BIG) {
+      // ---- image path: every particle of the cell, arrivals included, is a slot of the image ----
+      if (wk.na) wk.stage_arrivals(sd);
+      bool landed = false;
 #pragma unroll 1
-    for (int v0 = 0; v0 < nfull; v0 += 32) {
-      Part p;
-      wk.load_image(v0 + lane, p);
-      kick(cF, p.ax, p.ay, p.az, p.ux, p.uy, p.uz, p.sp);
-      float vx;
-      Part pn = p;
-      move(p.ax, p.ay, p.az, p.ux, p.uy, p.uz, vx, pn.ax, pn.ay, pn.az);
-      const bool stay = (!D3 || (pn.ax >= 0.f && pn.ax < 1.f)) && pn.ay >= 0.f && pn.ay < 1.f &&
-                        pn.az >= 0.f && pn.az < 1.f;
-      // Villasenor-Buneman: a trajectory that stays in the cell is one segment, summed in registers
-      const float qs = stay ? p.qw : 0.f;
-      vb_moments<D3>(acc, p.ax, p.ay, p.az, pn.ax, pn.ay, pn.az, qs * gd.cur[0], qs * gd.cur[1],
-                     qs * gd.cur[2], qs * gd.inv_dV * vx);
-      wk.store_image(v0, true, !stay, pn);
-    }
-
-    // ---- the rest: the last residents, the arrivals (reorder on load), cells on the global path
-    bool leavers_done = !wk.fast;
-    int v0 = nfull;
+      for (int v0 = 0; v0 < ntot; v0 += 32) {
+        if (!landed && v0 + 32 > wk.n) {
+          wk.arrivals_landed();
+          landed = true;
+        }
+        const bool act = v0 + lane < ntot;
+        Part p;
+        wk.load_image(v0 + lane, p);
+        kick(cF, p.ax, p.ay, p.az, p.ux, p.uy, p.uz, p.sp);
+        float vx;
+        Part pn = p;
+        move(p.ax, p.ay, p.az, p.ux, p.uy, p.uz, vx, pn.ax, pn.ay, pn.az);
+        const bool stay = (!D3 || (pn.ax >= 0.f && pn.ax < 1.f)) && pn.ay >= 0.f && pn.ay < 1.f &&
+                          pn.az >= 0.f && pn.az < 1.f;
+        // Villasenor-Buneman: a trajectory that stays in the cell is one segment, summed in registers
+        const float qs = stay ? p.qw : 0.f;
+        vb_moments<D3>(acc, p.ax, p.ay, p.az, pn.ax, pn.ay, pn.az, qs * gd.cur[0], qs * gd.cur[1],
+                       qs * gd.cur[2], qs * gd.inv_dV * vx);
+        wk.store_image(v0, act, !stay, pn);
+      }
+      // ---- the cell's leavers, 32 at a time: records + the currents of their trajectories ------
+      const int nl = wk.nh;
 #pragma unroll 1
-    do {
-      Part cur;
-      bool isarr;
-      float x2d;
-      int id;
-      const bool act = wk.load(sd, v0, cur, isarr, x2d, id);
-      const float ax = D3 ? cur.ax : 0.f, ay = cur.ay, az = cur.az, qw = cur.qw;
-      float ux = cur.ux, uy = cur.uy, uz = cur.uz;
-      const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
-      kick(cF, ax, ay, az, ux, uy, uz, sp);
-      float vx, endx, endy, endz;
-      move(ax, ay, az, ux, uy, uz, vx, endx, endy, endz);
-      const bool stay = (!D3 || (endx >= 0.f && endx < 1.f)) && endy >= 0.f && endy < 1.f &&
-                        endz >= 0.f && endz < 1.f;
-      const bool cross = act && !stay;
-      {
+      for (int i0 = 0; i0 < nl; i0 += 32) {
+        const bool al = i0 + lane < nl;
+        Part q;
+        float qx2d = 0.f;
+        int qid = 0;
+        q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
+        if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
+        float qvx, qex, qey, qez;
+        move(D3 ? q.ax : 0.f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
+        depart(al, i0 + lane, packed, lx, ly, lz, D3 ? q.ax : 0.f, q.ay, q.az, qex, qey, qez, qvx, q.ux,
+               q.uy, q.uz, q.qw, q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
+      }
+    } else {
+      // ---- global path: residents from the columns, arrivals from the rows, compaction in place
+#pragma unroll 1
+      for (int v0 = 0; v0 < ntot; v0 += 32) {
+        Part cur;
+        float x2d;
+        int id;
+        const bool act = wk.load_global(sd, v0, cur, x2d, id);
+        const float ax = D3 ? cur.ax : 0.f, ay = cur.ay, az = cur.az, qw = cur.qw;
+        float ux = cur.ux, uy = cur.uy, uz = cur.uz;
+        const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
+        kick(cF, ax, ay, az, ux, uy, uz, sp);
+        float vx, endx, endy, endz;
+        move(ax, ay, az, ux, uy, uz, vx, endx, endy, endz);
+        const bool stay = (!D3 || (endx >= 0.f && endx < 1.f)) && endy >= 0.f && endy < 1.f &&
+                          endz >= 0.f && endz < 1.f;
+        const bool cross = act && !stay;
         const float qs = (cross || !act) ? 0.f : qw;
         vb_moments<D3>(acc, ax, ay, az, endx, endy, endz, qs * gd.cur[0], qs * gd.cur[1],
                        qs * gd.cur[2], qs * gd.inv_dV * vx);
-      }
-      Part pn;
-      pn.ax = endx; pn.ay = endy; pn.az = endz;
-      pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
-      if (wk.fast) wk.store_image(v0, act && !isarr, cross, pn);
-      if (!leavers_done) {
-        // all residents of the image are advanced: the cell's leavers, 32 at a time
-        leavers_done = true;
-        const int nl = wk.nh;
-#pragma unroll 1
-        for (int i0 = 0; i0 < nl; i0 += 32) {
-          const bool al = i0 + lane < nl;
-          Part q;
-          float qx2d = 0.f;
-          int qid = 0;
-          q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
-          if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
-          float qvx, qex, qey, qez;
-          move(D3 ? q.ax : 0.f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
-          depart(al, i0 + lane, packed, lx, ly, lz, D3 ? q.ax : 0.f, q.ay, q.az, qex, qey, qez, qvx, q.ux,
-                 q.uy, q.uz, q.qw, q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
+        if (__any_sync(0xffffffffu, cross)) {
+          const int xi = wk.leaver_slot(cross);
+          depart(cross, xi, packed, lx, ly, lz, ax, ay, az, endx, endy, endz, vx, ux, uy, uz, qw, sp, x2d, id);
         }
-        wk.nleave = nl;
+        Part pn;
+        pn.ax = endx; pn.ay = endy; pn.az = endz;
+        pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
+        wk.store_global(sd, act && stay, pn, x2d, id);
       }
-      // arrivals that leave again at once, and every leaver of a cell on the global path
-      const bool late = cross && (isarr || !wk.fast);
-      if (__any_sync(0xffffffffu, late)) {
-        const int xi = wk.leaver_slot(late);
-        depart(late, xi, packed, lx, ly, lz, ax, ay, az, endx, endy, endz, vx, ux, uy, uz, qw, sp, x2d, id);
-      }
-      wk.place(sd, v0, act, isarr, cross, pn, x2d, id);
-      v0 += 32;
-    } while (v0 < ntot);
+    }
 
     // ---- the cell is done: its in-cell currents take one warp reduction and one shared add per
     // J point; its image goes back to global memory and the next cell's run is requested
@@ -581,13 +592,14 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         atomicAdd(&sJ[node + my_off], r);
       }
     }
-    const int nx = ci + nwarps;
-    wk.end_cell(sd, nx < tg.cpb ? sCnt[nx] : 0, nx < tg.cpb ? sBase[nx] : 0);
+    if (BIG) wk.end_global(sd);
+    else wk.end_image(sd, next_n, next_base);
   }
   if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, sRel, 0, qcnt, lane);
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
-  __syncthreads();
+  const int any_left = __syncthreads_or(left_out ? 1 : 0);
+  if (!BIG && threadIdx.x == 0) sd.bigflag[blockIdx.x] = any_left;
 
   // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) {
@@ -619,22 +631,33 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const StoreDesc sd = psc_store_desc(c);
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
   constexpr int threads = 128;
-  const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
-  const int wstride = (wbytes + 127) / 128 * 128;
-  const size_t smem = (size_t)(threads / 32) * (wstride + (d3 ? QROWS3 : QROWS2) * QCAP * 4) +
-                      (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 27 + 2 * gd.cpb + 2) * sizeof(float);
-  if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 27 + 2 * gd.cpb + 2) * sizeof(float);
+  const size_t qbytes = (size_t)(d3 ? QROWS3 : QROWS2) * QCAP * 4;
+  auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
+  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.C, sd.ncol)
+                               : CellWalker<false, true, false>::smem_bytes(sd.C, sd.ncol));
+  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.C, sd.ncol));
+  const size_t smem_img = (size_t)(threads / 32) * (ws_img + qbytes) + tile_bytes;
+  const size_t smem_big = (size_t)(threads / 32) * (ws_big + qbytes) + tile_bytes;
+  if (smem_img > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   ProfScope ps(c, PSC_PH_PUSH, s);
+#define PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, XC_, BIG_, SMEM_, WS_)                                  \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_>,                    \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
+    k_push1<D3_, CBS_, T_, B_, XC_, BIG_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    PSC_LAUNCH_CHECK(c);                                                                           \
+  } while (0)
+  // the image launch, then the launch for the cells it had to leave out (its blocks return at
+  // once for every other tile)
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
   do {                                                                                             \
     if (xc) {                                                                                      \
-      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, true>,                       \
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      k_push1<D3_, CBS_, T_, B_, true><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride); \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, true, false, smem_img, ws_img);                         \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, true, true, smem_big, ws_big);                           \
     } else {                                                                                       \
-      PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, false>,                      \
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      k_push1<D3_, CBS_, T_, B_, false><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride); \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, smem_img, ws_img);                        \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, smem_big, ws_big);                          \
     }                                                                                              \
   } while (0)
   if (d3) {
@@ -647,6 +670,6 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
   }
 #undef PSC_LAUNCH_PUSH1
-  PSC_LAUNCH_CHECK(c);
+#undef PSC_LAUNCH_PUSH1_
   return PSC_OK;
 }

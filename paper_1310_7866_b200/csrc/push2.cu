@@ -204,12 +204,15 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
     if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
 }
 
-template <bool D3, int CBS, bool XC>
+// BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
+// launch for the tiles in which the first one had to leave a cell out.
+template <bool D3, int CBS, bool XC, bool BIG>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
 k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
   extern __shared__ __align__(128) unsigned char smraw[];
-  using Walker = CellWalker<D3, XC>;
+  if (BIG && !sd.bigflag[blockIdx.x]) return;
+  using Walker = CellWalker<D3, XC, BIG>;
   Geom2<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
@@ -292,27 +295,50 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       if (xi >= PSC_XCAP)
         dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
                         wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-      wk.emit(sd, gd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+      wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
     }
   };
 
+  bool left_out = false;  // this warp met a cell that does not fit the image
+  int src_next;
+  unsigned mask_next = wk.fetch_mask(sd, tg, warp, src_next);
   if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
+    const int nx = ci + nwarps;
+    const int next_n = nx < tg.cpb ? sCnt[nx] : 0, next_base = nx < tg.cpb ? sBase[nx] : 0;
+    const unsigned mask = mask_next;
+    const int src = src_next;
+    mask_next = wk.fetch_mask(sd, tg, nx, src_next);
+    wk.begin_cell(kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], mask, src);
+    if (wk.fits == BIG) {  // the other launch's cell
+      left_out = true;
+      wk.skip_cell(sd, next_n, next_base);
+      continue;
+    }
     const int lx = ci % tg.bs[0], lt = ci / tg.bs[0];
     const int ly = lt % tg.bs[1], lz = lt / tg.bs[1];
-    wk.begin_cell(sd, tg, kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], lx, ly, lz);
     const int np_cell = wk.n + wk.na;  // residents + arrivals (reorder on load)
     float *cellJ = sJ + (D3 ? ((lz + 1) * tg.te[1] + (ly + 1)) * tg.te[0] + (lx + 1)
                             : (lz + 1) * tg.te[1] + (ly + 1));
-    bool leavers_done = !wk.fast;
+    if (!BIG && wk.na) wk.stage_arrivals(sd);
+    bool landed = false;
 #pragma unroll 1
     for (int base = 0; base < np_cell; base += 32) {
       Part cur;
-      bool isarr;
-      float x2d;
-      int id;
-      const bool act = wk.load(sd, base, cur, isarr, x2d, id);
+      float x2d = 0.f;
+      int id = 0;
+      bool act;
+      if (BIG) {
+        act = wk.load_global(sd, base, cur, x2d, id);
+      } else {
+        if (!landed && base + 32 > wk.n) {
+          wk.arrivals_landed();
+          landed = true;
+        }
+        act = base + lane < np_cell;
+        wk.load_image(base + lane, cur);
+      }
       const float ax = D3 ? cur.ax : 0.25f, ay = cur.ay, az = cur.az;
       float ux = cur.ux, uy = cur.uy, uz = cur.uz;
       const float qw = act ? cur.qw : 0.f;
@@ -438,49 +464,50 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         }
       }
 
-      // ---- file the particle: in place / into a hole if it stays, as a record if it leaves -----
+      // ---- file the particle: in place if it stays; a leaver is noted (image path) or recorded
       const bool stay = (!D3 || (endx >= 0.f && endx < 1.f)) && endy >= 0.f && endy < 1.f &&
                         endz >= 0.f && endz < 1.f;
       const bool leave = act && !stay;
       Part pn;
       pn.ax = endx; pn.ay = endy; pn.az = endz;
       pn.ux = ux; pn.uy = uy; pn.uz = uz; pn.qw = qw; pn.sp = sp;
-      if (wk.fast) wk.store_image(base, act && !isarr, leave, pn);
-      if (!leavers_done && base + 32 >= wk.n) {
-        // all residents of the image are advanced: the records of the cell's leavers, 32 at a
-        // time (their deposit is done: Esirkepov's stencil covers the move across the face)
-        leavers_done = true;
-        const int nl = wk.nh;
-#pragma unroll 1
-        for (int i0 = 0; i0 < nl; i0 += 32) {
-          const bool al = i0 + lane < nl;
-          Part q;
-          float qx2d = 0.f;
-          int qid = 0;
-          q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
-          if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
-          float qvx, qex, qey, qez;
-          move(D3 ? q.ax : 0.25f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
-          depart(al, i0 + lane, lx, ly, lz, qex, qey, qez, q.ux, q.uy, q.uz, q.qw,
-                 q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
+      if (BIG) {
+        if (__any_sync(0xffffffffu, leave)) {
+          const int xi = wk.leaver_slot(leave);
+          depart(leave, xi, lx, ly, lz, endx, endy, endz, ux, uy, uz, qw, sp, x2d, id);
         }
-        wk.nleave = nl;
+        wk.store_global(sd, act && stay, pn, x2d, id);
+      } else {
+        wk.store_image(base, act, leave, pn);
       }
-      // arrivals that leave again at once, and every leaver of a cell on the global path
-      const bool late = leave && (isarr || !wk.fast);
-      if (__any_sync(0xffffffffu, late)) {
-        const int xi = wk.leaver_slot(late);
-        depart(late, xi, lx, ly, lz, endx, endy, endz, ux, uy, uz, qw, sp, x2d, id);
-      }
-      wk.place(sd, base, act, isarr, leave, pn, x2d, id);
       if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
     }
-    const int nx = ci + nwarps;
-    wk.end_cell(sd, nx < tg.cpb ? sCnt[nx] : 0, nx < tg.cpb ? sBase[nx] : 0);
+    if (BIG) {
+      wk.end_global(sd);
+    } else {
+      // the records of the cell's leavers, 32 at a time (their deposit is done: Esirkepov's
+      // stencil covers the move across the face)
+      const int nl = wk.nh;
+#pragma unroll 1
+      for (int i0 = 0; i0 < nl; i0 += 32) {
+        const bool al = i0 + lane < nl;
+        Part q;
+        float qx2d = 0.f;
+        int qid = 0;
+        q.ax = q.ay = q.az = 0.25f; q.ux = q.uy = q.uz = q.qw = 0.f; q.sp = 0;
+        if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
+        float qvx, qex, qey, qez;
+        move(D3 ? q.ax : 0.25f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
+        depart(al, i0 + lane, lx, ly, lz, qex, qey, qez, q.ux, q.uy, q.uz, q.qw,
+               q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
+      }
+      wk.end_image(sd, next_n, next_base);
+    }
   }
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
-  __syncthreads();
+  const int any_left = __syncthreads_or(left_out ? 1 : 0);
+  if (!BIG && threadIdx.x == 0) sd.bigflag[blockIdx.x] = any_left;
 
   // ---- flush the J tile to global J -----------------------------------------------------------
   for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) {
@@ -508,22 +535,31 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const StoreDesc sd = psc_store_desc(c);
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
   const int threads = PUSH2_THREADS;
-  const int wbytes = d3 ? CellWalker<true, true>::smem_bytes(sd.C, sd.ncol) : CellWalker<false, true>::smem_bytes(sd.C, sd.ncol);
-  const int wstride = (wbytes + 127) / 128 * 128;
-  const size_t smem = (size_t)(threads / 32) * wstride +
-                      (size_t)(9 * tvol + PSC_MAX_SPECIES + 27 + 2 * gd.cpb + 2) * sizeof(float);
-  if (smem > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
+  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.C, sd.ncol)
+                               : CellWalker<false, true, false>::smem_bytes(sd.C, sd.ncol));
+  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.C, sd.ncol));
+  const size_t tile_bytes = (size_t)(9 * tvol + PSC_MAX_SPECIES + 27 + 2 * gd.cpb + 2) * sizeof(float);
+  const size_t smem_img = (size_t)(threads / 32) * ws_img + tile_bytes;
+  const size_t smem_big = (size_t)(threads / 32) * ws_big + tile_bytes;
+  if (smem_img > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   ProfScope ps(c, PSC_PH_PUSH, s);
-#define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_)                                                           \
+#define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_, BIG_, SMEM_, WS_)                                         \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_>,                                  \
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    k_push2<D3_, CBS_, XC_><<<gd.ntiles, threads, smem, s>>>(gd, sd, c->E, c->B, c->J, wstride);   \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_, BIG_>,                            \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
+    k_push2<D3_, CBS_, XC_, BIG_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
-#define PSC_LAUNCH_PUSH2(D3_, CBS_)           \
-  do {                                        \
-    if (xc) PSC_LAUNCH_PUSH2_(D3_, CBS_, true); \
-    else PSC_LAUNCH_PUSH2_(D3_, CBS_, false); \
+#define PSC_LAUNCH_PUSH2(D3_, CBS_)                                       \
+  do {                                                                    \
+    if (xc) {                                                             \
+      PSC_LAUNCH_PUSH2_(D3_, CBS_, true, false, smem_img, ws_img);        \
+      PSC_LAUNCH_PUSH2_(D3_, CBS_, true, true, smem_big, ws_big);         \
+    } else {                                                              \
+      PSC_LAUNCH_PUSH2_(D3_, CBS_, false, false, smem_img, ws_img);       \
+      PSC_LAUNCH_PUSH2_(D3_, CBS_, false, true, smem_big, ws_big);        \
+    }                                                                     \
   } while (0)
   if (d3) {
     if (gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4) PSC_LAUNCH_PUSH2(true, 4);
@@ -534,6 +570,5 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   }
 #undef PSC_LAUNCH_PUSH2
 #undef PSC_LAUNCH_PUSH2_
-  PSC_LAUNCH_CHECK(c);
   return PSC_OK;
 }

@@ -638,6 +638,7 @@ size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   b += 2 * align_up((nk + 1) * 8, 256);                       // pack, packloc
   b += align_up((nk / SCAN_TILE + 3) * 8, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
+  b += align_up((size_t)c->gd.ntiles * 4, 256);               // bigflag
   b += 2 * (align_up(nx * sizeof(XRec), 256) + align_up(nk * PSC_XW3 * 4, 256) + align_up(nx * 4, 256));  // exchange x2
   const size_t sc = (size_t)spill_capacity(n);
   b += align_up(sc * sizeof(XRec), 256) + 2 * align_up(sc * 4, 256);  // spill
@@ -666,6 +667,7 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
   c->packloc = (long long *)take((nk + 1) * 8);
   c->scan_tmp = (long long *)take((nk / SCAN_TILE + 3) * 8);
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
+  c->bigflag = (int32_t *)take((size_t)c->gd.ntiles * 4);
   for (int i = 0; i < 2; i++) {
     c->xch[i].rec = (XRec *)take(nx * sizeof(XRec));
     c->xch[i].mask = (uint32_t *)take(nk * PSC_XW3 * 4);
@@ -710,6 +712,7 @@ StoreDesc psc_store_desc(const psc_ctx *c) {
   sd.spill = c->spill;
   if (!p.id) sd.spill.id = nullptr;
   sd.C = c->bufC;
+  sd.bigflag = c->bigflag;
   sd.flags = c->d_flags + PSC_DW_FLAGS;
   return sd;
 }

@@ -18,13 +18,17 @@
 //     SOURCE cell (ping-pong buffered); the row's header holds one 32-bit mask per direction code
 //     (9 / 27 destination classes) saying which records moved that way;
 //   * the arrivals of a cell are the records of its 8 / 26 neighbours' rows whose direction points
-//     at it: one 4-byte header load per neighbour finds them; they are pushed together with the residents (in the idle lanes of the cell's last
-//     chunk) and filed into the holes the cell's own leavers left, else appended, so that
-//     [0, cnt) stays dense; holes left over are closed by moving particles from the tail.
-// A cell that does not fit the image (more than C particles) is streamed straight from and to
-// global memory with an in-place compaction instead (rare; correct for any size).  A particle that
-// finds no room (row or cell full) goes to the spill list; the next step then re-lays the store
-// out before pushing (sort.cu).
+//     at it: one 4-byte header load per neighbour finds them (requested one cell ahead), and
+//     asynchronous 4-byte copies (cp.async) drop their words into the image BEHIND the residents
+//     while the residents are being pushed -- from then on an arrival is a particle of the cell
+//     like any other (reorder on load);
+//   * at the end of the cell the holes the leavers left are closed by moving particles from the
+//     tail of the image, so that [0, cnt) stays dense.
+// A cell that does not fit the image (more than C particles incl. arrivals) is left to a second
+// launch of the same kernel in its BIG form, which streams such cells straight from and to global
+// memory with an in-place compaction (rare; correct for any size; tiles without such a cell leave
+// at once).  A particle that finds no room (row or cell full) goes to the spill list; the next
+// step then re-lays the store out before pushing (sort.cu).
 #pragma once
 #include "push_common.cuh"
 
@@ -116,20 +120,23 @@ struct Part {
 constexpr int WALK_AC = 128;  // arrival-list window (entries)
 
 // Per-warp view of the store.  XC: optional columns (id, carried x of a 2-d run) may be bound.
-template <bool D3, bool XC>
+// BIG == false: the shared-memory image path (cells with n + arrivals <= C; others are skipped
+// and reported); BIG == true: the global-memory path for exactly those others.
+template <bool D3, bool XC, bool BIG>
 struct CellWalker {
-  static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4, NDYN = D3 ? 6 : 5;
+  static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4, NDYN = D3 ? 6 : 5, NREC = D3 ? 8 : 7;
   static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
   // bytes of per-warp shared memory for an image of C slots x ncol columns
   __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
-    return ncol * C * 4 + C /*holes*/ + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ + 12 * 4 /*hbm*/ + 16 /*bar*/;
+    return (BIG ? 0 : ncol * C * 4 + C /*holes*/) + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ +
+           12 * 4 /*hbm*/ + 16 /*bar*/;
   }
   float *buf;      // [ncol][C]
-  uint8_t *holes;  // [C]
-  uint16_t *arr;   // [WALK_AC]
-  int *nbk;        // [32]
+  uint8_t *holes;  // [C]: slots of the image whose particle left, ascending
+  uint16_t *arr;   // [WALK_AC]: arrival a -> direction lane << 8 | record index in that neighbour's row
+  int *nbk;        // [32]: key of the neighbour cell a lane looks at
   unsigned *xrow;  // [32]: per direction code, which of the cell's records so far moved that way
-  unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole (its resident left)
+  unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole
   uint64_t *bar;
   const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
   int C, ncol, lane;
@@ -139,19 +146,19 @@ struct CellWalker {
   bool loads_armed;  // bulk loads for the cell about to be processed are in flight
   // current cell
   int key, n, na, base, cap;
-  bool fast;
+  bool fits;         // n + na <= C: the cell takes the image path
   int nh, tcur, nleave, a0, my_start;
 
   __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_, const int *nbt_) {
     C = sd.C;
-    ncol = XC ? sd.ncol : (D3 ? 8 : 7);
+    ncol = XC ? sd.ncol : NREC;
     lane = lane_;
     nbt = nbt_;
     dir_decode<D3>(lane < ND ? lane : STAY, sx, sy, sz);
     lt = lanemask_lt_();
     buf = (float *)wsm;
-    holes = (uint8_t *)(buf + ncol * C);
-    arr = (uint16_t *)(holes + C);
+    holes = (uint8_t *)(buf + (BIG ? 0 : ncol * C));
+    arr = (uint16_t *)(holes + (BIG ? 0 : C));
     nbk = (int *)(arr + WALK_AC);
     xrow = (unsigned *)(nbk + 32);
     hbm = xrow + 32;
@@ -159,7 +166,7 @@ struct CellWalker {
     parity = 0;
     loads_armed = false;
     xrow[lane] = 0u;
-    if (lane == 0) {
+    if (!BIG && lane == 0) {
       mbar_init(bar, 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -168,6 +175,7 @@ struct CellWalker {
 
   // lane 0: fetch the resident run of a cell into the image (n <= C)
   __device__ __forceinline__ void issue_loads(const StoreDesc &sd, int n_, int base_) {
+    if (BIG) return;
     loads_armed = n_ > 0 && n_ <= C;
     if (loads_armed && lane == 0) {
       const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
@@ -176,21 +184,9 @@ struct CellWalker {
         for (int c = 0; c < ncol; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
       } else {
 #pragma unroll
-        for (int c = 0; c < (D3 ? 8 : 7); c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
+        for (int c = 0; c < NREC; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
       }
     }
-  }
-
-  // writes the arrival-list window [a0, a0 + WALK_AC): entry = direction lane << 8 | row index
-  __device__ __forceinline__ void fill_window(unsigned mask) {
-    int g = my_start - a0;
-    while (mask) {
-      const int j = __ffs(mask) - 1;
-      if (g >= 0 && g < WALK_AC) arr[g] = (uint16_t)((lane << 8) | j);
-      g++;
-      mask &= mask - 1;
-    }
-    __syncwarp();
   }
 
   // key of the cell that reaches cell (lx, ly, lz) of this tile by a move in this lane's direction
@@ -206,22 +202,37 @@ struct CellWalker {
     return nbt[(tz + 1) * 9 + (ty + 1) * 3 + (tx + 1)] + (qz * tg.bs[1] + qy) * tg.bs[0] + qx;
   }
 
-  // Start of a cell: where its arrivals are (the neighbours' row headers), whether it takes the
-  // shared-memory path, wait for its resident run.  (lx, ly, lz): the cell inside the tile.
+  // The header word this lane needs to find the arrivals of cell ci of the tile (its neighbour in
+  // this lane's direction, that direction's mask): requested one cell ahead of begin_cell().
   template <class TG>
-  __device__ __forceinline__ void begin_cell(const StoreDesc &sd, const TG &tg, int key_, int n_,
-                                             int base_, int cap_, int lx, int ly, int lz) {
+  __device__ __forceinline__ unsigned fetch_mask(const StoreDesc &sd, const TG &tg, int ci, int &src) const {
+    src = 0;
+    if (!(lane < ND && lane != STAY) || ci >= tg.cpb) return 0u;
+    const int lx = ci % tg.bs[0], t = ci / tg.bs[0];
+    src = source_key(tg, lx, t % tg.bs[1], t / tg.bs[1]);
+    return sd.xin.mask[(size_t)src * XW + lane];
+  }
+
+  // writes the arrival-list window [a0, a0 + WALK_AC): entry = direction lane << 8 | record index
+  __device__ __forceinline__ void fill_window(unsigned mask) {
+    int g = my_start - a0;
+    while (mask) {
+      const int j = __ffs(mask) - 1;
+      if (g >= 0 && g < WALK_AC) arr[g] = (uint16_t)((lane << 8) | j);
+      g++;
+      mask &= mask - 1;
+    }
+    __syncwarp();
+  }
+
+  // Start of a cell: its arrivals (from the neighbours' header words), whether it fits the image;
+  // waits for its resident run.
+  __device__ __forceinline__ void begin_cell(int key_, int n_, int base_, int cap_, unsigned mask, int src) {
     key = key_;
     n = n_;
     base = base_;
     cap = cap_;
-    const bool have = lane < ND && lane != STAY;
-    unsigned mask = 0;
-    if (have) {
-      const int src = source_key(tg, lx, ly, lz);
-      nbk[lane] = src;
-      mask = sd.xin.mask[(size_t)src * XW + lane];
-    }
+    nbk[lane] = src;
     const int cntm = __popc(mask);
     int inc = cntm;
 #pragma unroll
@@ -232,85 +243,53 @@ struct CellWalker {
     na = __shfl_sync(0xffffffffu, inc, 31);
     my_start = inc - cntm;
     a0 = 0;
-    if (na) fill_window(mask);
-    fast = n + na <= C;
+    fits = n + na <= C && na <= WALK_AC;
+    if (na && fits != BIG) fill_window(mask);
     nh = 0;
-    tcur = fast ? n : 0;  // shared-memory path: append cursor; global path: write cursor
+    tcur = 0;
     nleave = 0;
-    if (loads_armed) {
+    if (!BIG && loads_armed) {
       mbar_wait(bar, parity);
       parity ^= 1;
       loads_armed = false;
     }
   }
 
-  // Loads particle v0 + lane of the cell (residents first, then arrivals).  Returns whether the
-  // lane holds a particle.  x2d / id are fetched only where a later move needs them (leavers, the
-  // global path): see extras().
-  __device__ __forceinline__ bool load(const StoreDesc &sd, int v0, Part &p, bool &isarr, float &x2d, int &id) {
-    const int v = v0 + lane;
-    const bool act = v < n + na;
-    isarr = v >= n;
-    p.ax = p.ay = p.az = 0.25f;
-    p.ux = p.uy = p.uz = p.qw = 0.f;
-    p.sp = 0;
-    x2d = 0.f;
-    id = 0;
-    if (v0 + 32 > n && na) {  // warp-uniform: this chunk contains arrivals
-      if (v0 + 32 - n > a0 + WALK_AC) {  // next window of the arrival list (cells with > 128 arrivals)
-        a0 = v0 > n ? v0 - n : 0;
-        const bool have = lane < ND && lane != STAY;
-        const unsigned mask = have ? sd.xin.mask[(size_t)nbk[lane] * XW + lane] : 0u;
-        __syncwarp();
-        fill_window(mask);
-      }
-      if (act && isarr) {
-        const int e = arr[v - n - a0];
-        const size_t idx = (size_t)nbk[e >> 8] * PSC_XCAP + (e & 255);
-        const XRec r = sd.xin.rec[idx];
-        if (D3) {
-          p.ax = __uint_as_float(r.a.x); p.ay = __uint_as_float(r.a.y); p.az = __uint_as_float(r.a.z);
-          p.ux = __uint_as_float(r.a.w); p.uy = __uint_as_float(r.b.x); p.uz = __uint_as_float(r.b.y);
-          p.qw = __uint_as_float(r.b.z); p.sp = (int)r.b.w;
-        } else {
-          p.ay = __uint_as_float(r.a.x); p.az = __uint_as_float(r.a.y);
-          p.ux = __uint_as_float(r.a.z); p.uy = __uint_as_float(r.a.w); p.uz = __uint_as_float(r.b.x);
-          p.qw = __uint_as_float(r.b.y); p.sp = (int)r.b.z; x2d = __uint_as_float(r.b.w);
-        }
-        if (XC && sd.xin.id) id = sd.xin.id[idx];
+  // ---- image path ---------------------------------------------------------------------------------
+
+  // The arrivals' record words go to the image slots [n, n + na) behind the residents, by
+  // asynchronous 4-byte copies (a lane per arrival); wait with arrivals_landed().
+  __device__ __forceinline__ void stage_arrivals(const StoreDesc &sd) {
+    for (int a = lane; a < na; a += 32) {
+      const int e = arr[a];
+      const size_t idx = (size_t)nbk[e >> 8] * PSC_XCAP + (e & 255);
+      const float *r = reinterpret_cast<const float *>(sd.xin.rec + idx);
+      float *q = buf + n + a;
+#pragma unroll
+      for (int w = 0; w < NREC; w++) cp_async4(q + w * C, r + w, true);
+      if (XC) {
+        if (sd.icol_x2d >= 0) cp_async4(q + sd.icol_x2d * C, r + 7, true);
+        if (sd.icol_id >= 0) cp_async4(q + sd.icol_id * C, sd.xin.id + idx, true);
       }
     }
-    if (act && !isarr) {
-      if (fast) {
-        const float *q = buf + v;
-        if (D3) {
-          p.ax = q[0]; p.ay = q[C]; p.az = q[2 * C]; p.ux = q[3 * C]; p.uy = q[4 * C]; p.uz = q[5 * C];
-          p.qw = q[6 * C]; p.sp = __float_as_int(q[7 * C]);
-        } else {
-          p.ay = q[0]; p.az = q[C]; p.ux = q[2 * C]; p.uy = q[3 * C]; p.uz = q[4 * C];
-          p.qw = q[5 * C]; p.sp = __float_as_int(q[6 * C]);
-        }
-      } else {
-        const size_t s = (size_t)base + v;
-        if (D3) {
-          p.ax = ld_stream(sd.col[0] + s); p.ay = ld_stream(sd.col[1] + s); p.az = ld_stream(sd.col[2] + s);
-          p.ux = ld_stream(sd.col[3] + s); p.uy = ld_stream(sd.col[4] + s); p.uz = ld_stream(sd.col[5] + s);
-          p.qw = ld_stream(sd.col[6] + s); p.sp = __float_as_int(ld_stream(sd.col[7] + s));
-        } else {
-          p.ay = ld_stream(sd.col[0] + s); p.az = ld_stream(sd.col[1] + s);
-          p.ux = ld_stream(sd.col[2] + s); p.uy = ld_stream(sd.col[3] + s); p.uz = ld_stream(sd.col[4] + s);
-          p.qw = ld_stream(sd.col[5] + s); p.sp = __float_as_int(ld_stream(sd.col[6] + s));
-        }
-        if (XC) {
-          if (sd.icol_x2d >= 0) x2d = ld_stream(sd.col[sd.icol_x2d] + s);
-          if (sd.icol_id >= 0) id = __float_as_int(ld_stream(sd.col[sd.icol_id] + s));
-        }
-      }
+    cp_async_commit();
+  }
+  // Before the first chunk that touches slots >= n: the arrivals are in the image, and the slots
+  // between the last particle and the end of its chunk hold a harmless particle (at rest, no
+  // charge) instead of whatever the copies left there.
+  __device__ __forceinline__ void arrivals_landed() {
+    cp_async_wait<0>();
+    const int T = n + na;
+    const int s = T + lane;
+    if (s < ((T + 31) & ~31)) {
+      float *q = buf + s;
+#pragma unroll
+      for (int c = 0; c < NREC; c++) q[c * C] = (c < (D3 ? 3 : 2)) ? 0.25f : 0.f;
     }
-    return act;
+    __syncwarp();
   }
 
-  // resident v of the image (shared-memory path), no bounds check
+  // particle v of the image, no bounds check
   __device__ __forceinline__ void load_image(int v, Part &p) const {
     const float *q = buf + v;
     if (D3) {
@@ -323,7 +302,7 @@ struct CellWalker {
     }
   }
 
-  // Files resident v0 + lane of the image after its push: the momentum always, the offsets only if
+  // Files particle v0 + lane of the image after its push: the momentum always, the offsets only if
   // it stays; a leaver keeps its old offsets and is noted as a hole (see leaver()).
   __device__ __forceinline__ void store_image(int v0, bool act, bool leave, const Part &pn) {
     const int v = v0 + lane;
@@ -344,7 +323,7 @@ struct CellWalker {
   }
 
   // leaver i of the hole list: its image values (OLD offsets, NEW momentum) and optional columns
-  __device__ __forceinline__ int leaver(const StoreDesc &sd, int i, Part &p, float &x2d, int &id) const {
+  __device__ __forceinline__ void leaver(const StoreDesc &sd, int i, Part &p, float &x2d, int &id) const {
     const int h = holes[i];
     load_image(h, p);
     x2d = 0.f;
@@ -353,23 +332,71 @@ struct CellWalker {
       if (sd.icol_x2d >= 0) x2d = buf[sd.icol_x2d * C + h];
       if (sd.icol_id >= 0) id = __float_as_int(buf[sd.icol_id * C + h]);
     }
-    return h;
   }
 
-  // writes record xi of the current cell's row (moved by direction code dc), or spills it
-  __device__ __forceinline__ void emit(const StoreDesc &sd, const GridDesc &gd, int xi, int dc,
-                                       const float (&w)[8], int id, int dest_key) {
-    if (xi < PSC_XCAP) atomicOr(&xrow[dc], 1u << xi);
-    write_record(sd, gd, key, xi, w, id, dest_key);
-  }
-
-  // optional values of a RESIDENT particle on the shared-memory path (needed only if it leaves)
-  __device__ __forceinline__ void extras(const StoreDesc &sd, int v, float &x2d, int &id) {
-    if (XC) {
-      if (sd.icol_x2d >= 0) x2d = buf[sd.icol_x2d * C + v];
-      if (sd.icol_id >= 0) id = __float_as_int(buf[sd.icol_id * C + v]);
+  // End of a cell on the image path: close the holes from the tail of the image, write the image's
+  // dynamic columns back, the static ones where a particle is new in its slot; publish the count
+  // and the exchange row; start fetching the next cell (next_n <= 0: none).
+  __device__ __forceinline__ void end_image(const StoreDesc &sd, int next_n, int next_base) {
+    __syncwarp();
+    const int T = n + na;
+    int newcnt = T - nh;
+    if (nh > 0) {
+      int done = 0;
+      for (int t0 = newcnt; t0 < T; t0 += 32) {
+        const int s = t0 + lane;
+        const bool valid = s < T && !((hbm[s >> 5] >> (s & 31)) & 1u);
+        const unsigned mv = __ballot_sync(0xffffffffu, valid);
+        if (valid) {
+          const int h = holes[done + __popc(mv & lt)];  // ascending list: its first entries are < newcnt
+          for (int c = 0; c < ncol; c++) buf[c * C + h] = buf[c * C + s];
+          if (h < n)
+            for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + h, buf[c * C + s]);
+        }
+        done += __popc(mv);
+      }
+      __syncwarp();
     }
+    if (newcnt > cap) {  // no room for all arrivals: the excess spills (and forces a re-layout)
+      for (int s = cap + lane; s < newcnt; s += 32) {
+        float w[8];
+#pragma unroll
+        for (int c = 0; c < NREC; c++) w[c] = buf[c * C + s];
+        if (!D3) w[7] = (XC && sd.icol_x2d >= 0) ? buf[sd.icol_x2d * C + s] : 0.f;
+        spill_particle(sd, key, w, (XC && sd.icol_id >= 0) ? __float_as_int(buf[sd.icol_id * C + s]) : 0);
+      }
+      newcnt = cap;
+    }
+    // arrivals that ended up behind the old residents: their static columns are new in global memory
+    for (int s = n + lane; s < newcnt; s += 32)
+      for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + s, buf[c * C + s]);
+    fence_proxy_async();
+    __syncwarp();
+    if (lane == 0 && newcnt > 0) {
+      const unsigned bytes = (unsigned)((newcnt + 3) & ~3) * 4u;
+#pragma unroll
+      for (int c = 0; c < NDYN; c++) bulk_s2g(sd.col[c] + base, buf + c * C, bytes);
+      bulk_commit();
+    }
+    publish(sd, newcnt);
+    if (lane == 0) bulk_wait_read0();  // the image may be overwritten once the copy engine has read it
+    __syncwarp();
+    if (next_n > 0) issue_loads(sd, next_n, next_base);
   }
+
+  // a cell this launch leaves to the other one: nothing changes, only the next fetch starts
+  __device__ __forceinline__ void skip_cell(const StoreDesc &sd, int next_n, int next_base) {
+    if (next_n > 0) issue_loads(sd, next_n, next_base);
+  }
+
+  __device__ __forceinline__ void publish(const StoreDesc &sd, int newcnt) {
+    if (lane == 0) sd.cnt[key] = newcnt;
+    if (lane < XW) sd.xout.mask[(size_t)key * XW + lane] = xrow[lane];
+    __syncwarp();
+    xrow[lane] = 0u;
+  }
+
+  // ---- records ------------------------------------------------------------------------------------
 
   // the 8 record words of a particle (positions as given)
   __device__ __forceinline__ static void to_words(float (&w)[8], const Part &p, float x2d) {
@@ -382,21 +409,13 @@ struct CellWalker {
     }
   }
 
-  // index of the next leaver's record in the cell's exchange row (all lanes; `leave`: this lane
-  // leaves).  Records past the row's capacity go to the spill list (emit()).
-  __device__ __forceinline__ int leaver_slot(bool leave) {
-    const unsigned m = __ballot_sync(0xffffffffu, leave);
-    const int xi = nleave + __popc(m & lt);
-    nleave += __popc(m);
-    return xi;
-  }
-
-  // writes a leaver's record (positions relative to the destination cell) into row slot xi of
-  // cell src_key, or spills it
-  __device__ __forceinline__ static void write_record(const StoreDesc &sd, const GridDesc &gd, int src_key,
-                                                      int xi, const float (&w)[8], int id, int dest_key) {
+  // writes record xi of the current cell's row (moved by direction code dc; positions relative
+  // to the destination cell), or spills it if the row is full
+  __device__ __forceinline__ void emit(const StoreDesc &sd, int xi, int dc, const float (&w)[8], int id,
+                                       int dest_key) {
     if (xi < PSC_XCAP) {
-      const size_t idx = (size_t)src_key * PSC_XCAP + xi;
+      atomicOr(&xrow[dc], 1u << xi);
+      const size_t idx = (size_t)key * PSC_XCAP + xi;
       XRec r;
       r.a = make_uint4(__float_as_uint(w[0]), __float_as_uint(w[1]), __float_as_uint(w[2]), __float_as_uint(w[3]));
       r.b = make_uint4(__float_as_uint(w[4]), __float_as_uint(w[5]), __float_as_uint(w[6]), __float_as_uint(w[7]));
@@ -407,113 +426,100 @@ struct CellWalker {
     }
   }
 
-  // General form (any chunk; both paths), second half: after the residents of the chunk went
-  // through store_image() and -- on the shared-memory path -- the cell's leavers were processed,
-  // an ARRIVAL that stays is filed into a hole of the list, else appended.  Global path: every
-  // particle of the chunk that stays is compacted to the front of the cell.  pn: the new values.
-  __device__ __forceinline__ void place(const StoreDesc &sd, int v0, bool act, bool isarr, bool leave,
-                                        const Part &pn, float x2d, int id) {
-    const bool stay = act && !leave;
-    if (fast) {
-      const unsigned ma = __ballot_sync(0xffffffffu, stay && isarr);
-      if (ma) {
+  // ---- global path (BIG) --------------------------------------------------------------------------
+
+  // Loads particle v0 + lane of the cell (residents from the columns, then arrivals from the
+  // neighbours' rows).  Returns whether the lane holds a particle.
+  __device__ __forceinline__ bool load_global(const StoreDesc &sd, int v0, Part &p, float &x2d, int &id) {
+    const int v = v0 + lane;
+    const bool act = v < n + na;
+    p.ax = p.ay = p.az = 0.25f;
+    p.ux = p.uy = p.uz = p.qw = 0.f;
+    p.sp = 0;
+    x2d = 0.f;
+    id = 0;
+    if (v0 + 32 > n && na) {  // warp-uniform: this chunk contains arrivals
+      if (v0 + 32 - n > a0 + WALK_AC) {  // next window of the arrival list
+        a0 = v0 > n ? v0 - n : 0;
+        const bool have = lane < ND && lane != STAY;
+        const unsigned mask = have ? sd.xin.mask[(size_t)nbk[lane] * XW + lane] : 0u;
         __syncwarp();
-        if (stay && isarr) {
-          const int r = __popc(ma & lt);
-          const int slot = r < nh ? (int)holes[nh - 1 - r] : tcur + (r - nh);
-          if (r < nh) atomicAnd(&hbm[slot >> 5], ~(1u << (slot & 31)));
-          float w[8];
-          to_words(w, pn, x2d);
-          if (slot < cap) {
-            float *q = buf + slot;
-#pragma unroll
-            for (int c = 0; c < (D3 ? 8 : 7); c++) q[c * C] = w[c];
-            const size_t s = (size_t)base + slot;
-            st_stream(sd.col[NDYN] + s, pn.qw);
-            st_stream(sd.col[NDYN + 1] + s, __int_as_float(pn.sp));
-            if (XC) {
-              if (sd.icol_x2d >= 0) { q[sd.icol_x2d * C] = x2d; st_stream(sd.col[sd.icol_x2d] + s, x2d); }
-              if (sd.icol_id >= 0) { q[sd.icol_id * C] = __int_as_float(id); st_stream(sd.col[sd.icol_id] + s, __int_as_float(id)); }
-            }
-          } else {
-            spill_particle(sd, key, w, id);
-          }
-        }
-        const int ca = __popc(ma), used = ca < nh ? ca : nh;
-        nh -= used;
-        tcur += ca - used;
-        __syncwarp();
+        fill_window(mask);
       }
-    } else {
-      // global path: in-place streaming compaction (the write cursor tcur never passes the reads)
-      const unsigned ms = __ballot_sync(0xffffffffu, stay);
-      const int slot = tcur + __popc(ms & lt);
-      __syncwarp();
-      if (stay) {
-        float w[8];
-        to_words(w, pn, x2d);
-        if (slot < cap) {
-          const size_t s = (size_t)base + slot;
-#pragma unroll
-          for (int c = 0; c < (D3 ? 8 : 7); c++) st_stream(sd.col[c] + s, w[c]);
-          if (XC) {
-            if (sd.icol_x2d >= 0) st_stream(sd.col[sd.icol_x2d] + s, x2d);
-            if (sd.icol_id >= 0) st_stream(sd.col[sd.icol_id] + s, __int_as_float(id));
-          }
+      if (act && v >= n) {
+        const int e = arr[v - n - a0];
+        const size_t idx = (size_t)nbk[e >> 8] * PSC_XCAP + (e & 255);
+        const XRec r = sd.xin.rec[idx];
+        if (D3) {
+          p.ax = __uint_as_float(r.a.x); p.ay = __uint_as_float(r.a.y); p.az = __uint_as_float(r.a.z);
+          p.ux = __uint_as_float(r.a.w); p.uy = __uint_as_float(r.b.x); p.uz = __uint_as_float(r.b.y);
+          p.qw = __uint_as_float(r.b.z); p.sp = (int)r.b.w;
         } else {
-          spill_particle(sd, key, w, id);
+          p.ay = __uint_as_float(r.a.x); p.az = __uint_as_float(r.a.y);
+          p.ux = __uint_as_float(r.a.z); p.uy = __uint_as_float(r.a.w); p.uz = __uint_as_float(r.b.x);
+          p.qw = __uint_as_float(r.b.y); p.sp = (int)r.b.z; x2d = __uint_as_float(r.b.w);
         }
+        if (XC && sd.xin.id) id = sd.xin.id[idx];
       }
-      tcur += __popc(ms);
     }
+    if (act && v < n) {
+      const size_t s = (size_t)base + v;
+      if (D3) {
+        p.ax = ld_stream(sd.col[0] + s); p.ay = ld_stream(sd.col[1] + s); p.az = ld_stream(sd.col[2] + s);
+        p.ux = ld_stream(sd.col[3] + s); p.uy = ld_stream(sd.col[4] + s); p.uz = ld_stream(sd.col[5] + s);
+        p.qw = ld_stream(sd.col[6] + s); p.sp = __float_as_int(ld_stream(sd.col[7] + s));
+      } else {
+        p.ay = ld_stream(sd.col[0] + s); p.az = ld_stream(sd.col[1] + s);
+        p.ux = ld_stream(sd.col[2] + s); p.uy = ld_stream(sd.col[3] + s); p.uz = ld_stream(sd.col[4] + s);
+        p.qw = ld_stream(sd.col[5] + s); p.sp = __float_as_int(ld_stream(sd.col[6] + s));
+      }
+      if (XC) {
+        if (sd.icol_x2d >= 0) x2d = ld_stream(sd.col[sd.icol_x2d] + s);
+        if (sd.icol_id >= 0) id = __float_as_int(ld_stream(sd.col[sd.icol_id] + s));
+      }
+    }
+    return act;
   }
 
-  // End of a cell: close the remaining holes from the tail, write the image back, publish the
-  // count and the exchange row, start fetching the next cell (next_n <= 0: none).
-  __device__ __forceinline__ void end_cell(const StoreDesc &sd, int next_n, int next_base) {
-    int newcnt;
+  // index of the next leaver's record in the cell's exchange row (all lanes)
+  __device__ __forceinline__ int leaver_slot(bool leave) {
+    const unsigned m = __ballot_sync(0xffffffffu, leave);
+    const int xi = nleave + __popc(m & lt);
+    nleave += __popc(m);
+    return xi;
+  }
+
+  // every particle of the chunk that stays is compacted to the front of the cell, in place (the
+  // write cursor tcur never passes the reads); pn: the new values
+  __device__ __forceinline__ void store_global(const StoreDesc &sd, bool stay, const Part &pn, float x2d, int id) {
+    const unsigned ms = __ballot_sync(0xffffffffu, stay);
+    const int slot = tcur + __popc(ms & lt);
     __syncwarp();
-    if (fast) {
-      if (nh > 0) {
-        const int m = n - nh;  // no append happened while holes were left, so tcur == n
-        int done = 0;
-        for (int t0 = m; t0 < n; t0 += 32) {
-          const int s = t0 + lane;
-          const bool valid = s < n && !((hbm[s >> 5] >> (s & 31)) & 1u);
-          const unsigned mv = __ballot_sync(0xffffffffu, valid);
-          if (valid) {
-            const int h = holes[done + __popc(mv & lt)];  // ascending list: its first entries are < m
-            for (int c = 0; c < ncol; c++) buf[c * C + h] = buf[c * C + s];
-            for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + h, buf[c * C + s]);
-          }
-          done += __popc(mv);
-        }
-        newcnt = m;
-      } else {
-        newcnt = tcur < cap ? tcur : cap;
-      }
-      fence_proxy_async();
-      __syncwarp();
-      if (lane == 0 && newcnt > 0) {
-        const unsigned bytes = (unsigned)((newcnt + 3) & ~3) * 4u;
+    if (stay) {
+      float w[8];
+      to_words(w, pn, x2d);
+      if (slot < cap) {
+        const size_t s = (size_t)base + slot;
 #pragma unroll
-        for (int c = 0; c < NDYN; c++) bulk_s2g(sd.col[c] + base, buf + c * C, bytes);
-        bulk_commit();
+        for (int c = 0; c < NREC; c++) st_stream(sd.col[c] + s, w[c]);
+        if (XC) {
+          if (sd.icol_x2d >= 0) st_stream(sd.col[sd.icol_x2d] + s, x2d);
+          if (sd.icol_id >= 0) st_stream(sd.col[sd.icol_id] + s, __int_as_float(id));
+        }
+      } else {
+        spill_particle(sd, key, w, id);
       }
-    } else {
-      newcnt = tcur < cap ? tcur : cap;
     }
-    if (lane == 0) sd.cnt[key] = newcnt;
-    if (lane < XW) sd.xout.mask[(size_t)key * XW + lane] = xrow[lane];
+    tcur += __popc(ms);
+  }
+
+  __device__ __forceinline__ void end_global(const StoreDesc &sd) {
     __syncwarp();
-    xrow[lane] = 0u;
-    if (lane == 0) bulk_wait_read0();  // the image may be overwritten once the copy engine has read it
-    __syncwarp();
-    if (next_n > 0) issue_loads(sd, next_n, next_base);
+    publish(sd, tcur < cap ? tcur : cap);
   }
 
   __device__ __forceinline__ void finish() {
-    if (lane == 0) bulk_wait_all();
+    if (!BIG && lane == 0) bulk_wait_all();
     __syncwarp();
   }
 };
