@@ -85,7 +85,7 @@ struct StoreDesc {
   int32_t *cnt;
   Exchange xin, xout;
   Spill spill;
-  int C;           // slots of the per-warp cell image (multiple of 32, <= 256)
+  int imgC;        // slots of the per-warp cell image (multiple of 32, <= 256)
   int32_t *bigflag;  // [ntiles]: the image launch left a cell of this tile to the BIG launch
   uint32_t *flags;
 };

@@ -335,14 +335,14 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
 // XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id).
 // BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
 // launch for the tiles in which the first one had to leave a cell out.
-template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG>
+template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG, int CT>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
   extern __shared__ __align__(128) unsigned char smraw[];
   if (BIG && !sd.bigflag[blockIdx.x]) return;
   constexpr int NV = D3 ? 12 : 8;
-  using Walker = CellWalker<D3, XC, BIG>;
+  using Walker = CellWalker<D3, XC, BIG, CT>;
   TileGeom<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
@@ -634,40 +634,44 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 27 + 2 * gd.cpb + 2) * sizeof(float);
   const size_t qbytes = (size_t)(d3 ? QROWS3 : QROWS2) * QCAP * 4;
   auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
-  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.C, sd.ncol)
-                               : CellWalker<false, true, false>::smem_bytes(sd.C, sd.ncol));
-  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.C, sd.ncol));
+  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)
+                               : CellWalker<false, true, false>::smem_bytes(sd.imgC, sd.ncol));
+  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.imgC, sd.ncol));
   const size_t smem_img = (size_t)(threads / 32) * (ws_img + qbytes) + tile_bytes;
   const size_t smem_big = (size_t)(threads / 32) * (ws_big + qbytes) + tile_bytes;
   if (smem_img > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   ProfScope ps(c, PSC_PH_PUSH, s);
-#define PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, XC_, BIG_, SMEM_, WS_)                                  \
+#define PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, XC_, BIG_, CT_, SMEM_, WS_)                             \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_>,                    \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_>,               \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, CBS_, T_, B_, XC_, BIG_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the image launch, then the launch for the cells it had to leave out (its blocks return at
-  // once for every other tile)
-#define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_)                                                        \
+  // once for every other tile).  The library's default tiles without optional columns get the
+  // image stride as a compile-time constant.
+#define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_, FAST_)                                                 \
   do {                                                                                             \
     if (xc) {                                                                                      \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, true, false, smem_img, ws_img);                         \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, true, true, smem_big, ws_big);                           \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, true, false, 0, smem_img, ws_img);                      \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, true, true, 0, smem_big, ws_big);                        \
     } else {                                                                                       \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, smem_img, ws_img);                        \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, smem_big, ws_big);                          \
+      if (FAST_ && sd.imgC == 256) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 256, smem_img, ws_img); \
+      else if (FAST_ && sd.imgC == 192) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 192, smem_img, ws_img); \
+      else if (FAST_ && sd.imgC == 128) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 128, smem_img, ws_img); \
+      else PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 0, smem_img, ws_img);                \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_big, ws_big);                       \
     }                                                                                              \
   } while (0)
   if (d3) {
     const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
-    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4);
-    else PSC_LAUNCH_PUSH1(true, 0, 128, 4);
+    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4, true);
+    else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5);
-    else PSC_LAUNCH_PUSH1(false, 0, 128, 5);
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5, true);
+    else PSC_LAUNCH_PUSH1(false, 0, 128, 5, false);
   }
 #undef PSC_LAUNCH_PUSH1
 #undef PSC_LAUNCH_PUSH1_

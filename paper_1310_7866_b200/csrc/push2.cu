@@ -536,9 +536,9 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
   const int threads = PUSH2_THREADS;
   auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
-  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.C, sd.ncol)
-                               : CellWalker<false, true, false>::smem_bytes(sd.C, sd.ncol));
-  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.C, sd.ncol));
+  const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)
+                               : CellWalker<false, true, false>::smem_bytes(sd.imgC, sd.ncol));
+  const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.imgC, sd.ncol));
   const size_t tile_bytes = (size_t)(9 * tvol + PSC_MAX_SPECIES + 27 + 2 * gd.cpb + 2) * sizeof(float);
   const size_t smem_img = (size_t)(threads / 32) * ws_img + tile_bytes;
   const size_t smem_big = (size_t)(threads / 32) * ws_big + tile_bytes;

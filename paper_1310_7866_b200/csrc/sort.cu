@@ -711,7 +711,7 @@ StoreDesc psc_store_desc(const psc_ctx *c) {
   if (!p.id) sd.xin.id = sd.xout.id = nullptr;
   sd.spill = c->spill;
   if (!p.id) sd.spill.id = nullptr;
-  sd.C = c->bufC;
+  sd.imgC = c->bufC;
   sd.bigflag = c->bigflag;
   sd.flags = c->d_flags + PSC_DW_FLAGS;
   return sd;
@@ -881,7 +881,7 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, s));
   PSC_CUDA_TRY(c, cudaStreamSynchronize(s));
   const int mx = (int)dw[PSC_DW_MAXCNT];
-  int C = (mx + mx / 8 + 24 + 31) / 32 * 32;
+  int C = (mx + mx / 8 + 24 + 63) / 64 * 64;  // one of 64, 128, 192, 256
   c->bufC = C < 64 ? 64 : (C > 256 ? 256 : C);
   if ((int64_t)dw[PSC_DW_SLOTS] > c->capacity) return PSC_ERR_WORKSPACE;
   return PSC_OK;

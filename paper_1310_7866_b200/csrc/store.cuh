@@ -122,7 +122,9 @@ constexpr int WALK_AC = 128;  // arrival-list window (entries)
 // Per-warp view of the store.  XC: optional columns (id, carried x of a 2-d run) may be bound.
 // BIG == false: the shared-memory image path (cells with n + arrivals <= C; others are skipped
 // and reported); BIG == true: the global-memory path for exactly those others.
-template <bool D3, bool XC, bool BIG>
+// CT != 0: the image has CT slots per column (a compile-time stride folds the column offsets of
+// every image access into immediates); CT == 0: the stride is the run-time sd.imgC.
+template <bool D3, bool XC, bool BIG, int CT = 0>
 struct CellWalker {
   static constexpr int ND = D3 ? 27 : 9, STAY = D3 ? 13 : 4, NDYN = D3 ? 6 : 5, NREC = D3 ? 8 : 7;
   static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
@@ -139,7 +141,8 @@ struct CellWalker {
   unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole
   uint64_t *bar;
   const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
-  int C, ncol, lane;
+  int Crt, ncol, lane;
+#define C (CT ? CT : Crt)
   int sx, sy, sz;  // the direction this lane looks at when a cell collects its arrivals (lane = code)
   unsigned lt;
   unsigned parity;
@@ -150,7 +153,7 @@ struct CellWalker {
   int nh, tcur, nleave, a0, my_start;
 
   __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_, const int *nbt_) {
-    C = sd.C;
+    Crt = sd.imgC;
     ncol = XC ? sd.ncol : NREC;
     lane = lane_;
     nbt = nbt_;
@@ -176,6 +179,9 @@ struct CellWalker {
   // lane 0: fetch the resident run of a cell into the image (n <= C)
   __device__ __forceinline__ void issue_loads(const StoreDesc &sd, int n_, int base_) {
     if (BIG) return;
+    // (broadcasts from lane 0: tells the compiler the operands of the bulk copies are warp-uniform)
+    n_ = __shfl_sync(0xffffffffu, n_, 0);
+    base_ = __shfl_sync(0xffffffffu, base_, 0);
     loads_armed = n_ > 0 && n_ <= C;
     if (loads_armed && lane == 0) {
       const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
@@ -372,11 +378,14 @@ struct CellWalker {
       for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + s, buf[c * C + s]);
     fence_proxy_async();
     __syncwarp();
-    if (lane == 0 && newcnt > 0) {
-      const unsigned bytes = (unsigned)((newcnt + 3) & ~3) * 4u;
+    {
+      const int cnt_u = __shfl_sync(0xffffffffu, newcnt, 0), base_u = __shfl_sync(0xffffffffu, base, 0);
+      if (lane == 0 && cnt_u > 0) {
+        const unsigned bytes = (unsigned)((cnt_u + 3) & ~3) * 4u;
 #pragma unroll
-      for (int c = 0; c < NDYN; c++) bulk_s2g(sd.col[c] + base, buf + c * C, bytes);
-      bulk_commit();
+        for (int c = 0; c < NDYN; c++) bulk_s2g(sd.col[c] + base_u, buf + c * C, bytes);
+        bulk_commit();
+      }
     }
     publish(sd, newcnt);
     if (lane == 0) bulk_wait_read0();  // the image may be overwritten once the copy engine has read it
@@ -523,3 +532,4 @@ struct CellWalker {
     __syncwarp();
   }
 };
+#undef C
