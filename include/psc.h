@@ -127,9 +127,10 @@ int psc_bind_fields(psc_ctx *ctx, float *E, float *B, float *J);
 /* Number of floats in one of E/B/J (3 * ex * ey * ez) and the extents; host only. */
 int64_t psc_field_elems(const psc_ctx *ctx, int32_t ext[3]);
 
-/* Entries every particle column must have for n particles: n + n/8 + 48 per cell, rounded up to a
- * multiple of 32 -- every cell of the store gets an eighth of spare room (at least 16 slots) and
- * starts on a 128-byte boundary.  Host only. */
+/* Entries every particle column must have for n particles: n + n/8 + 6 sqrt(cells * n) + 56 per
+ * cell, rounded up to a multiple of 32 -- every cell of the store gets spare room (an eighth of
+ * its population, at least six Poisson standard deviations) and starts on a 128-byte boundary.
+ * Host only. */
 int64_t psc_particle_capacity(const psc_ctx *ctx, int64_t n);
 
 /* `primary` holds the n particles (absolute positions, entries [0, n)); `secondary` is a second

@@ -87,6 +87,7 @@ struct StoreDesc {
   Spill spill;
   int imgC;        // slots of the per-warp cell image (multiple of 32, <= 256)
   int32_t *bigflag;  // [ntiles]: the image launch left a cell of this tile to the BIG launch
+  uint8_t *bigcell;  // [nkeys]: ... this cell (set by the image launch, cleared by the BIG launch)
   uint32_t *flags;
 };
 
@@ -149,6 +150,7 @@ struct psc_ctx {
   size_t ws_bytes;
   int64_t ws_cap;  // max particles the bound workspace was sized for
   int32_t *key, *perm, *cell_idx, *offs_dense, *base, *cnt, *cursor, *big_list, *tot, *doffs, *bigflag;
+  uint8_t *bigcell;
   long long *pack, *packloc, *scan_tmp;
   Exchange xch[2];
   Spill spill;

@@ -345,7 +345,9 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   using Walker = CellWalker<D3, XC, BIG, CT>;
   TileGeom<D3, CBS> tg;
   tg.init(gd, blockIdx.x);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  const int lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+  // (broadcast from lane 0: lets the compiler keep everything derived from the warp index uniform)
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   // per-warp areas first (128-byte aligned cell images), then the block's tiles and tables
   constexpr int QROWS = D3 ? QROWS3 : QROWS2;
   float *myQ = (float *)(smraw + (size_t)nwarps * wstride) + warp * (QROWS * QCAP);  // [QROWS][QCAP]
@@ -490,8 +492,15 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int src = src_next;
     mask_next = wk.fetch_mask(sd, tg, nx, src_next);
     wk.begin_cell(kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], mask, src);
-    if (wk.fits == BIG) {  // the other launch's cell
+    // Whose cell is it?  The image launch decides (its count is the one before the push) and
+    // leaves a note; the BIG launch takes exactly the noted cells.
+    if (BIG) {
+      if (!sd.bigcell[kbase + ci]) continue;
+      __syncwarp();
+      if (lane == 0) sd.bigcell[kbase + ci] = 0;
+    } else if (!wk.fits) {
       left_out = true;
+      if (lane == 0) sd.bigcell[kbase + ci] = 1;
       wk.skip_cell(sd, next_n, next_base);
       continue;
     }

@@ -26,6 +26,7 @@
 // bring them back.  Whether that is needed is known on the device only, so these launches carry a
 // condition word and return at once when it is zero.
 #include <limits.h>
+#include <math.h>
 
 #include "store.cuh"
 
@@ -140,11 +141,14 @@ k_cell_idx(GridDesc gd, int n, const int *__restrict__ key, int *__restrict__ ce
   cell_idx[a] = (c[2] * gd.n[1] + c[1]) * gd.n[0] + c[0];
 }
 
-// Capacity of a cell holding cnt particles: room for an eighth more (at least 16), rounded up to
-// a multiple of 32 slots so that every column of every cell starts on a 128-byte line.
-// Sum over cells <= n + n/8 + 47 nkeys (psc_store_capacity).
-__device__ __forceinline__ int cell_capacity(int cnt) {
-  const int spare = max(cnt >> 3, 16);
+// Capacity of a cell holding cnt particles: room for an eighth more, and at least for six
+// standard deviations of a Poisson count (the population of a cell of a uniform plasma fluctuates
+// by sqrt(cnt); with millions of cells some reach +5 sigma within a few steps), rounded up to a
+// multiple of 32 slots so that every column of every cell starts on a 128-byte line.
+// Sum over cells <= n + n/8 + 6 sqrt(nkeys n) + 56 nkeys (psc_store_capacity; Cauchy-Schwarz).
+__host__ __device__ __forceinline__ int cell_capacity(int cnt) {
+  const int sig = (int)(6.0f * sqrtf((float)cnt)) + 8;
+  const int spare = max(max(cnt >> 3, 16), sig);
   return (cnt + spare + PSC_SLOT_ALIGN - 1) & ~(PSC_SLOT_ALIGN - 1);
 }
 
@@ -595,13 +599,15 @@ k_gather_spill(GridDesc gd, Spill sp, const int *__restrict__ doffs, Cols out, i
 
 // after a (re-)layout: every exchange row empty, nothing spilled; records the slots in use
 __global__ void __launch_bounds__(SORT_THREADS)
-k_store_reset(int nk, int xw, uint32_t *__restrict__ m0, uint32_t *__restrict__ m1, const int *__restrict__ base,
-              uint32_t *__restrict__ dw, long long capacity, const uint32_t *__restrict__ cond) {
+k_store_reset(int nk, int xw, uint32_t *__restrict__ m0, uint32_t *__restrict__ m1, uint8_t *__restrict__ bigcell,
+              const int *__restrict__ base, uint32_t *__restrict__ dw, long long capacity,
+              const uint32_t *__restrict__ cond) {
   PSC_COND_RETURN(cond);
   const int m = nk * xw;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) {
     m0[i] = 0u;
     m1[i] = 0u;
+    if (i < nk) bigcell[i] = 0;
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     dw[PSC_DW_SLOTS] = (uint32_t)base[nk];
@@ -623,11 +629,13 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // slots per column a store of n particles can need (see cell_capacity)
 int64_t psc_store_capacity(const psc_ctx *c, int64_t n) {
-  const int64_t v = n + n / 8 + 48 * (int64_t)c->gd.nkeys;
+  const int64_t nk = c->gd.nkeys;
+  const int64_t v = n + n / 8 + (int64_t)(6.0 * sqrt((double)nk * (double)n)) + 56 * nk;
   return (v + 31) / 32 * 32;
 }
 
-static int64_t spill_capacity(int64_t n) { return n / 16 > 4096 ? n / 16 : 4096; }
+// a quarter of the particles may be homeless at once before PSC_F_OVERFLOW
+static int64_t spill_capacity(int64_t n) { return n / 4 > 8192 ? n / 4 : 8192; }
 
 size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   const size_t nk = (size_t)c->gd.nkeys;
@@ -639,6 +647,7 @@ size_t psc_sort_workspace_bytes(const psc_ctx *c, int64_t n) {
   b += align_up((nk / SCAN_TILE + 3) * 8, 256);               // scan_tmp
   b += align_up(((size_t)n / WARP_SEG_CAP + 16) * 4, 256);    // big_list
   b += align_up((size_t)c->gd.ntiles * 4, 256);               // bigflag
+  b += align_up(nk, 256);                                     // bigcell
   b += 2 * (align_up(nx * sizeof(XRec), 256) + align_up(nk * PSC_XW3 * 4, 256) + align_up(nx * 4, 256));  // exchange x2
   const size_t sc = (size_t)spill_capacity(n);
   b += align_up(sc * sizeof(XRec), 256) + 2 * align_up(sc * 4, 256);  // spill
@@ -668,6 +677,7 @@ int psc_sort_carve(psc_ctx *c, int64_t n) {
   c->scan_tmp = (long long *)take((nk / SCAN_TILE + 3) * 8);
   c->big_list = (int32_t *)take(((size_t)n / WARP_SEG_CAP + 16) * 4);
   c->bigflag = (int32_t *)take((size_t)c->gd.ntiles * 4);
+  c->bigcell = (uint8_t *)take(nk);
   for (int i = 0; i < 2; i++) {
     c->xch[i].rec = (XRec *)take(nx * sizeof(XRec));
     c->xch[i].mask = (uint32_t *)take(nk * PSC_XW3 * 4);
@@ -713,6 +723,7 @@ StoreDesc psc_store_desc(const psc_ctx *c) {
   if (!p.id) sd.spill.id = nullptr;
   sd.imgC = c->bufC;
   sd.bigflag = c->bigflag;
+  sd.bigcell = c->bigcell;
   sd.flags = c->d_flags + PSC_DW_FLAGS;
   return sd;
 }
@@ -825,7 +836,7 @@ int sort_core(psc_ctx *c, const Cols &src, const Cols &dst, bool from_abs, bool 
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_REORDER, s);
   k_store_reset<<<grid_for(c, (int64_t)nk * 16, SORT_THREADS), SORT_THREADS, 0, s>>>(
-      nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, c->xch[0].mask, c->xch[1].mask, c->base, c->d_flags,
+      nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, c->xch[0].mask, c->xch[1].mask, c->bigcell, c->base, c->d_flags,
       (long long)c->capacity, cond);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;

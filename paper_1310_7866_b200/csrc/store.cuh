@@ -250,7 +250,7 @@ struct CellWalker {
     my_start = inc - cntm;
     a0 = 0;
     fits = n + na <= C && na <= WALK_AC;
-    if (na && fits != BIG) fill_window(mask);
+    if (na && (BIG || fits)) fill_window(mask);
     nh = 0;
     tcur = 0;
     nleave = 0;
