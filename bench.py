@@ -20,6 +20,10 @@ The JSON line carries
   roofline     the fused gather-push-deposit kernel: algorithmic bytes / CUDA-event duration of
                the kernel launch (psc_profile brackets, on the launching stream, inside the timed
                region) against MEASURED_PEAKS.json's copy bandwidth
+  other_configs  BASELINE.json's other four configs at full size, a short run each (3 warm-up +
+               10 timed steps): value, ms_per_step, phase_ms, roofline, clocks
+  sort_general one explicit psc_particles_sort of the workload in random order (outside the
+               steady-state loop: psc_step never sorts after its first step)
   cpu_baseline the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded
                sample of the same workload (rank 0, N = 1 only)
 --impl reference times only the oracle (there is no reference code).
@@ -50,8 +54,6 @@ WORKLOADS = {
 }
 # algorithmic bytes per particle of the fused kernel
 PUSH_BYTES = {2: 48, 3: 56}
-# k_push2: smsp__inst_executed.sum / particles of the committed capture (profiles/r1e_push_kernels_ncu.md)
-PUSH2_WARP_INST_PER_PARTICLE = 5.5695e9 / 83886080
 
 
 def peaks():
@@ -234,13 +236,132 @@ def run_reference(args):
     return 0
 
 
+# algorithmic bytes per particle of the explicit general sort: keys (read the
+# active coordinates + species, write the key), scatter (read key, write perm), reorder (read perm +
+# key, read and write every bound column)
+def sort_bytes(ndim, ncols):
+    return (4 * ndim + 4 + 4) + (4 + 4) + (8 + 8 * ncols)
+
+
+def traffic_of(cfg, kernel):
+    """dram bytes per launch from the committed ncu captures (profiles/traffic.csv)"""
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tr):
+        return None, None
+    import csv
+    val = com = None
+    with open(tr) as f:
+        for row in csv.DictReader(f):     # the last row of this config + kernel wins
+            if int(row["config"]) == cfg and row["kernel"] == kernel:
+                val, com = float(row["dram_bytes_per_launch"]), row["commit"]
+    return val, com
+
+
+def measure(cfg, scale, warmup, steps, dev, world, local):
+    """W warm-up steps, K timed steps of psc_step on one config, device resident -> dict, sim"""
+    import torch
+
+    import psc_inputs
+    from paper_1310_7866_b200.harness import Simulation
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_gen = time.perf_counter()
+    pl = psc_inputs.make_config(cfg, device=dev, scale=scale)
+    sim = Simulation(pl, device=dev, with_id=False, with_x=pl.n[0] > 1)
+    for k in ("x", "y", "z", "ux", "uy", "uz", "qw", "species", "id"):
+        setattr(pl, k, getattr(pl, k)[:0])           # the simulation owns its copies
+    torch.cuda.empty_cache()
+    npart = sim.np
+    ndim = sum(1 for v in pl.n if v > 1)
+    torch.cuda.synchronize()
+    t_gen = time.perf_counter() - t_gen
+    psc = sim.psc
+    psc.set_option("profile", 1)
+    for _ in range(warmup):
+        psc.step()
+    barrier()
+    psc.profile()          # reset the phase accumulators
+    l0 = psc.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(steps):
+        psc.step()
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    launches = psc.launch_count() - l0
+    prof = psc.profile()
+    flags = psc.status()
+    info = psc.store_info()
+    ms_max = max_over_ranks(ms, world, dev)
+    # roofline of the fused gather-push-deposit kernel: algorithmic bytes / CUDA-event duration of
+    # the launch (psc_profile brackets on the launching stream, inside the timed region)
+    peak, peak_src = peaks()
+    push_ms, push_n = prof["push"]
+    push_avg = push_ms / max(push_n, 1)
+    bytes_pp = PUSH_BYTES[ndim]
+    achieved = bytes_pp * npart / (push_avg * 1e-3) / 1e9 if push_n else 0.0
+    kernel = "k_push%d" % pl.order
+    roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
+                "share_of_step": push_ms / ms if ms else None}
+    if scale is None:
+        roofline["traffic"], com = traffic_of(cfg, kernel)
+        if com:
+            roofline["traffic_commit"] = com
+    phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
+    res = {"value": job_throughput(npart, world, steps, ms_max), "ms_per_step": ms_max / steps,
+           "steps": steps, "warmup": warmup, "particles": npart, "grid": list(pl.n), "order": pl.order,
+           "phase_ms": phases, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
+           "status_flags": flags, "store": info, "setup_s": round(t_gen, 1)}
+    return res, sim, pl
+
+
+def time_general_sort(sim, pl, dev):
+    """one explicit psc_particles_sort (the stable general counting sort) of the current particles
+    in a seeded random order: milliseconds and the bytes-based fraction of the HBM peak"""
+    import torch
+
+    sim.psc.particles_export()
+    cur = sim.current()
+    g = torch.Generator(device=dev).manual_seed(20131029)
+    perm = torch.randperm(sim.np, generator=g, device=dev)
+    ncols = 0
+    for c, t in cur.items():
+        if t is not None:
+            t.copy_(t[perm])
+            ncols += 1
+    del perm
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    sim.psc.particles_sort()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    ndim = sum(1 for v in pl.n if v > 1)
+    bpp = sort_bytes(ndim, ncols)
+    peak, _ = peaks()
+    ach = bpp * sim.np / (ms * 1e-3) / 1e9
+    return {"ms": ms, "bytes_per_particle": bpp, "achieved": ach, "unit": "GB/s", "frac": ach / peak,
+            "input": "all particles of the workload in a seeded random order"}
+
+
 def run_psc(args):
     import torch
     import torch.distributed as dist
 
-    import psc_inputs
     from paper_1310_7866_b200 import COLUMNS
-    from paper_1310_7866_b200.harness import Simulation
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -257,72 +378,10 @@ def run_psc(args):
         torch.cuda.synchronize()
 
     scale = tuple(int(v) for v in args.scale.split("x")) if args.scale else None
-    t_gen = time.perf_counter()
-    pl = psc_inputs.make_config(args.config, device=dev, scale=scale)
-    if world > 1:  # replicas: same recipe, rank-dependent seed offset is not needed for timing
-        pass
-    sim = Simulation(pl, device=dev, with_id=False, with_x=pl.n[0] > 1)
-    npart = sim.np
-    ndim = sum(1 for v in pl.n if v > 1)
-    torch.cuda.synchronize()
-    t_gen = time.perf_counter() - t_gen
+    res, sim, pl = measure(args.config, scale, args.warmup, args.steps, dev, world, local)
     psc = sim.psc
-    psc.set_option("profile", 1)
-
-    # ---- device-resident: W warm-up steps, K timed steps ---------------------------------------
-    for _ in range(args.warmup):
-        psc.step()
-    barrier()
-    psc.profile()          # reset the phase accumulators
-    l0 = psc.launch_count()
-    sampler = ClockSampler(local)
-    sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    for _ in range(args.steps):
-        psc.step()
-    ev1.record()
-    barrier()
-    clocks = sampler.stop()
-    ms = ev0.elapsed_time(ev1)
-    launches = psc.launch_count() - l0
-    prof = psc.profile()
-    flags = psc.status()
-    ms_max = max_over_ranks(ms, world, dev)
-    value = job_throughput(npart, world, args.steps, ms_max)
-
-    # ---- roofline of the fused gather-push-deposit kernel ------------------------------------
-    peak, peak_src = peaks()
-    push_ms, push_n = prof["push"]
-    push_avg = push_ms / max(push_n, 1)
-    bytes_pp = PUSH_BYTES[ndim]
-    achieved = bytes_pp * npart / (push_avg * 1e-3) / 1e9 if push_n else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_push%d" % pl.order, "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
-                "share_of_step": push_ms / ms if ms else None}
-    if pl.order == 2 and push_n:
-        # the order-2 kernel is bound by plain ALU/FMA issue, not by HBM:
-        # achieved = warp instructions per particle (ncu smsp__inst_executed.sum of the committed
-        # capture / particles) * particles / kernel time; peak = SMs * 4 schedulers * SM clock
-        props = torch.cuda.get_device_properties(dev)
-        sm_clock_ghz = (clocks.get("sm_max_mhz") or 1965.0) / 1e3
-        peak_inst = props.multi_processor_count * 4 * sm_clock_ghz          # G warp-inst/s
-        ach_inst = PUSH2_WARP_INST_PER_PARTICLE * npart / (push_avg * 1e-3) / 1e9
-        roofline.update({"bound": "alu", "achieved": ach_inst, "peak": peak_inst, "unit": "Gwarp-inst/s",
-                         "frac": ach_inst / peak_inst, "hbm_achieved_gbs": achieved, "hbm_frac": achieved / peak,
-                         "peak_source": "148 SMs x 4 schedulers x max SM clock (1 warp instruction per scheduler and cycle)",
-                         "warp_inst_per_particle": PUSH2_WARP_INST_PER_PARTICLE})
-    tr = os.path.join(ROOT, "profiles", "traffic.csv")   # dram bytes per launch from the committed ncu captures
-    if os.path.exists(tr) and scale is None:
-        import csv
-        with open(tr) as f:
-            for row in csv.DictReader(f):     # the last row of this config + kernel wins
-                if int(row["config"]) == args.config and row["kernel"] == roofline["kernel"]:
-                    roofline["traffic"] = float(row["dram_bytes_per_launch"])
-                    roofline["traffic_commit"] = row["commit"]
-    phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
+    npart = sim.np
+    flags = res["status_flags"]
 
     # ---- end to end through psc_step_host with pinned host buffers -----------------------------
     e2e = None
@@ -356,20 +415,47 @@ def run_psc(args):
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ksteps,
                "api": "psc_step_host (pinned host columns + fields in, particles + E,B,J out)"}
         flags |= psc.status()
+        del host, hE, hB, hJ
+
+    # ---- the explicit general sort (outside the steady-state loop) -------------------------------
+    sort_general = None
+    if not args.no_sort:
+        sort_general = time_general_sort(sim, pl, dev)
+        flags |= psc.status()
+        res["phase_ms"]["sort_general"] = round(sort_general["ms"], 4)
 
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config] + (" [grid %s]" % args.scale if scale else ""),
                    "particles_per_gpu": npart, "grid": list(pl.n), "order": pl.order,
                    "parallelism": "replicas" if world > 1 else "single-gpu",
                    "l2": "inputs exceed L2 (particle columns %.2f GB vs 126 MB)" % (npart * 32 / 1e9)
                    if npart * 32 > 4 * 126e6 else "inputs smaller than L2 (small config)",
-                   "setup_s": round(t_gen, 1)},
-        "clocks": clocks, "gpu_launches": launches, "status_flags": flags,
-        "phase_ms": phases, "roofline": roofline, "e2e": e2e,
+                   "setup_s": res["setup_s"]},
+        "clocks": res["clocks"], "gpu_launches": res["gpu_launches"], "status_flags": flags,
+        "phase_ms": res["phase_ms"], "roofline": res["roofline"], "store": res["store"],
+        "sort_general": sort_general, "e2e": e2e,
     }
+
+    # ---- BASELINE.json's other configs: a short run each (rank 0, N = 1, full sizes) ------------
+    if world == 1 and not args.no_others and scale is None:
+        del sim
+        torch.cuda.empty_cache()
+        others = []
+        for cfg in (1, 2, 3, 4, 5):
+            if cfg == args.config:
+                continue
+            r, s2, p2 = measure(cfg, None, 3, args.other_steps, dev, 1, local)
+            r["workload"] = WORKLOADS[cfg]
+            r["unit"] = UNIT
+            others.append(r)
+            flags |= r["status_flags"]
+            del s2, p2
+            torch.cuda.empty_cache()
+        out["other_configs"] = others
+        out["status_flags"] = flags
 
     # ---- the oracle on the host cores (rank 0, N = 1 only) --------------------------------------
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -383,6 +469,14 @@ def run_psc(args):
             "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": "grid %dx%dx%d of the same recipe (%d particles), %d steps"
                       % (grid + (nsamp, args.cpu_steps))}
+        # the same oracle on ONE core, a smaller sample (about 5 s)
+        from oracle.psc_oracle import Oracle
+        g1 = sample_grids(args.config)[min(1, len(sample_grids(args.config)) - 1)]
+        Oracle.set_num_threads(1)
+        r1, t1, n1, _ = oracle_rate(args.config, g1, 4)
+        Oracle.set_num_threads(threads)
+        out["cpu_baseline"]["one_core"] = {"value": r1, "cores": t1,
+                                           "sample": "grid %dx%dx%d (%d particles), 4 steps" % (g1 + (n1,))}
     if rank == 0:
         print(json.dumps(out), flush=True)
     if world > 1:
@@ -403,6 +497,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick-cpu", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other four configs")
+    ap.add_argument("--other-steps", type=int, default=10)
+    ap.add_argument("--no-sort", action="store_true", help="skip the timing of the explicit general sort")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "psc":
         args.warmup = 3  # timing rule: at least 3 warm-up steps
