@@ -572,6 +572,33 @@ void orc_energy(const orc_params *p, const double *E, const double *B, int64_t n
 }
 
 /* ------------------------------------------------------------------------------------------ */
+/* Marder's Gauss-law correction, PAPER.md:206 ("the iterative method by Marder [24] to dissipate  */
+/* violations of Gauss's Law"; the paper cites only, A28 records the reading):           */
+/*   f = div- E - rho   on nodes  (Eq. 16, the Gauss residual of Eq. 24)                           */
+/*   E <- E + D grad+ f,  (grad+ f)_x,i+1/2,j,k = (f[i+1,j,k] - f[i,j,k]) / dx  (cyclic),          */
+/* repeated `iters` times with rho fixed.  D = d * dt is the diffusion number (units length^2):    */
+/* since div- grad+ is the 7-point Laplacian, every pass multiplies a Fourier mode of the residual */
+/* by 1 - D sum_d K_d^2, K_d = (2/dx_d) sin(k_d dx_d / 2); E with div- E = rho is left untouched.  */
+void orc_marder(const orc_params *p, double *E, const double *rho, double D, int iters) {
+  const int nx = p->n[0], ny = p->n[1], nz = p->n[2];
+  const int64_t nc = ncells(p);
+  double *f = (double *)malloc(sizeof(double) * nc);
+  for (int it = 0; it < iters; it++) {
+    orc_div_minus(p, E, f);
+    for (int64_t a = 0; a < nc; a++) f[a] -= rho[a];
+    for (int k = 0; k < nz; k++)
+      for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) {
+          const double f0 = f[fidx(p, 0, i, j, k)];
+          E[fidx(p, 0, i, j, k)] += D * (f[fidx(p, 0, i + 1, j, k)] - f0) / p->dx[0];
+          E[fidx(p, 1, i, j, k)] += D * (f[fidx(p, 0, i, j + 1, k)] - f0) / p->dx[1];
+          E[fidx(p, 2, i, j, k)] += D * (f[fidx(p, 0, i, j, k + 1)] - f0) / p->dx[2];
+        }
+  }
+  free(f);
+}
+
+/* ------------------------------------------------------------------------------------------ */
 /* cell-key counting sort.  One key orders by block (supercell) and by cell    */
 /* inside the block at once.  Positions are the fp32 values the GPU path sees; the cell index   */
 /* is floor of the fp32 product x * (1/dx) (both operands fp32), as the parity protocol fixes.  */

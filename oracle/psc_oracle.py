@@ -171,6 +171,10 @@ class Oracle:
                          _d(uz), _d(qw), _i(species), _d(out))
         return out
 
+    def marder(self, E, rho, D, iters=1):
+        """E += D grad+ (div- E - rho), `iters` passes"""
+        lib().orc_marder(C.byref(self.p), _d(E), _d(rho), C.c_double(float(D)), C.c_int(int(iters)))
+
     def sort(self, x32, y32, z32):
         """fp32 positions in -> (cell_idx, key, perm, cell_offsets), all int32."""
         n = x32.shape[0]
