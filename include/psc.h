@@ -10,7 +10,8 @@
  *   - Every pointer is a DEVICE pointer unless its name or comment says "host".
  *   - The library never allocates particle or field storage: the caller owns all buffers (and the
  *     stream) and the library borrows the pointers until the next bind or psc_destroy.  The only
- *     device memory the context owns is a 64-byte status/counter block.
+ *     device memory the context owns is a 64-byte status/counter block (and, once psc_marder or
+ *     psc_charge_density has been called, one scratch field of the size of E).
  *   - Every call that does device work enqueues it on `stream` (a cudaStream_t passed as void*)
  *     and returns without synchronising, except psc_status and psc_step_host.
  *   - Every call returns 0 (PSC_OK) or a negative PSC_ERR_* code; nothing aborts or throws across
@@ -177,6 +178,22 @@ int psc_exchange_j(psc_ctx *ctx, void *stream);
 /* fill_ghosts of Fig. 7/8 for which in {PSC_E, PSC_B, PSC_J}: ghosts := periodic images. */
 int psc_fill_ghosts(psc_ctx *ctx, int which, void *stream);
 
+/* Node charge density ("charge densities on corners"): rho(i,j,k) = sum over all
+ * particles of (q w / dV) S(x_p - x_ijk) with the weights of the bound order (b1 / b2, Eq. 31),
+ * into the caller's device array float[ez][ey][ex] (the extents of one field component), ghosts
+ * = periodic images.  Requires the internal form. */
+int psc_charge_density(psc_ctx *ctx, void *stream, float *rho);
+
+/* Marder's correction of Gauss's law (fp32 runs over very many steps drift away
+ * from div E = rho; "PSC implements the iterative method by Marder to dissipate violations"):
+ * `iters` passes of  E += diffusion * grad+ (div- E - rho)  with rho = psc_charge_density of the
+ * current particles (E at the time level of the positions, as stored between two psc_step).
+ * `diffusion` is Marder's d * dt (units length^2); a pass multiplies a Fourier mode of the
+ * residual by 1 - diffusion * sum_d (2/dx_d)^2 sin^2(k_d dx_d / 2), so it must satisfy
+ * diffusion * sum_d 4/dx_d^2 <= 1 (PSC_ERR_CFL).  Requires the internal form.  Uses one scratch
+ * field the context allocates on first use (freed by psc_destroy). */
+int psc_marder(psc_ctx *ctx, void *stream, float diffusion, int iters);
+
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
  * u^{n+1}.  Same fields and the same set of particles (up to the rounding of the atomically
@@ -245,6 +262,7 @@ int psc_last_cuda_error(const psc_ctx *ctx);
 #define PSC_PH_SORT_SCAN 7
 #define PSC_PH_SORT_RANK 8
 #define PSC_PH_SORT_REORDER 9
+#define PSC_PH_MARDER 10
 #define PSC_PH_COUNT 16
 int psc_profile(psc_ctx *ctx, void *stream, double *ms, int64_t *count);
 /* Host-side switches: "profile" (0/1: per-phase event timing), "clear_flags" (reset the sticky

@@ -17,13 +17,14 @@ PSC_E, PSC_B, PSC_J = 0, 1, 2
 PSC_F_OOB, PSC_F_NAN, PSC_F_SPECIES, PSC_F_OVERFLOW = 1, 4, 8, 32
 PSC_GHOST = 2
 PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
-          "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9}
+          "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9, "marder": 10}
 PSC_PH_COUNT = 16
 
 EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
     "psc_field_elems", "psc_particle_capacity", "psc_bind_particles", "psc_particles_sort",
     "psc_push_particles", "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step",
+    "psc_charge_density", "psc_marder",
     "psc_step_host", "psc_sort_result", "psc_particles_current", "psc_particles_form",
     "psc_particles_gather", "psc_particles_export", "psc_store_info", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
@@ -84,6 +85,8 @@ def lib():
             getattr(L, f).argtypes = [C.c_void_p, C.c_void_p]
         L.psc_push_fields.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_void_p]
         L.psc_fill_ghosts.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+        L.psc_charge_density.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.psc_marder.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int]
         L.psc_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(PscCols),
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.psc_sort_result.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
@@ -217,6 +220,14 @@ class Psc:
     def fill_ghosts(self, which, stream=None):
         """psc_fill_ghosts: ghosts := periodic images"""
         self._check(lib().psc_fill_ghosts(self._h, int(which), _stream(stream)), "psc_fill_ghosts")
+
+    def charge_density(self, rho, stream=None):
+        """psc_charge_density: node charge density with the bound order's weights"""
+        self._check(lib().psc_charge_density(self._h, _stream(stream), rho.data_ptr()), "psc_charge_density")
+
+    def marder(self, diffusion, iters=1, stream=None):
+        """psc_marder: E += diffusion * grad+ (div- E - rho), `iters` passes (PAPER.md:206)"""
+        self._check(lib().psc_marder(self._h, _stream(stream), float(diffusion), int(iters)), "psc_marder")
 
     def step(self, stream=None):
         """psc_step: one time step in the order of Fig. 8"""

@@ -305,6 +305,34 @@ int psc_push_fields(psc_ctx *c, int which, float frac, void *stream) {
   return PSC_ERR_INVALID_ARG;
 }
 
+int psc_charge_density(psc_ctx *c, void *stream, float *rho) {
+  if (!c || !rho) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->state != PSC_STATE_STORE) return PSC_ERR_NOT_SORTED;
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = psc_store_relayout_if_spilled(c, s);  // nobody may be waiting in the spill list
+  if (rc) return rc;
+  if ((rc = psc_charge_density_internal(c, s))) return rc;
+  PSC_CUDA_TRY(c, cudaMemcpyAsync(rho, c->rho, (size_t)c->gd.comp * sizeof(float), cudaMemcpyDeviceToDevice, s));
+  c->launches++;
+  return PSC_OK;
+}
+
+int psc_marder(psc_ctx *c, void *stream, float diffusion, int iters) {
+  if (!c || iters < 0 || !(diffusion >= 0.f)) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->state != PSC_STATE_STORE) return PSC_ERR_NOT_SORTED;
+  double lap = 0.0;  // largest eigenvalue of -div- grad+: sum 4/dx^2; a pass must not overshoot
+  for (int d = 0; d < 3; d++)
+    if (c->gd.n[d] > 1) lap += 4.0 / ((double)c->gd.dx[d] * (double)c->gd.dx[d]);
+  if ((double)diffusion * lap > 1.0 + 1e-6) return PSC_ERR_CFL;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int rc = psc_store_relayout_if_spilled(c, s);
+  if (rc) return rc;
+  ProfScope ps(c, PSC_PH_MARDER, s);
+  return psc_marder_pass(c, diffusion, iters, s);
+}
+
 int psc_fill_ghosts(psc_ctx *c, int which, void *stream) {
   if (!c) return PSC_ERR_INVALID_ARG;
   if (!c->have_fields) return PSC_ERR_NOT_BOUND;

@@ -212,3 +212,4 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s);
 int psc_push_order2(psc_ctx *c, cudaStream_t s);
 // marder.cu
 int psc_marder_pass(psc_ctx *c, float diffusion, int iters, cudaStream_t s);
+int psc_charge_density_internal(psc_ctx *c, cudaStream_t s);
