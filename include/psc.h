@@ -80,6 +80,8 @@ extern "C" {
  * |v| < c, so |move| < 1/2 cell; non-finite momenta raise PSC_F_NAN.) */
 
 #define PSC_MAX_SPECIES 8
+#define PSC_SCHEME_STANDARD 0
+#define PSC_SCHEME_ALTERNATING 1
 #define PSC_GHOST 2
 
 typedef struct psc_ctx psc_ctx; /* opaque, host side */
@@ -97,6 +99,12 @@ typedef struct {
   const float *m;    /* host array [n_species], mass */
   int32_t block[3];  /* sort block ("supercell") in cells; 0: library default;
                         must divide n[d]; 1 along invariant directions */
+  int32_t scheme;    /* PSC_SCHEME_STANDARD: every gather weight has the order above;
+                        PSC_SCHEME_ALTERNATING: the alternating-order interpolation of PAPER.md:204
+                        ("for improved energy conservation"): along a direction in which a field
+                        component is half-staggered on the Yee grid its gather weight is one order
+                        lower (order 1: b0 instead of b1; order 2: b1 instead of b2); the
+                        charge-conserving deposit is unchanged */
 } psc_params;
 
 /* One set of particle columns (structure of arrays), each of `capacity`

@@ -48,7 +48,7 @@ def _weights_1d(shape, n, xi, stag):
 
 
 class BruteForce:
-    def __init__(self, n, dx, dt, order, q, m):
+    def __init__(self, n, dx, dt, order, q, m, scheme=0):
         self.n = tuple(int(v) for v in n)
         self.dx = tuple(float(v) for v in dx)
         self.dt = float(dt)
@@ -56,14 +56,17 @@ class BruteForce:
         self.q = list(q)
         self.m = list(m)
         self.s = b1 if order == 1 else b2  # weights are one order above the particle shape
+        # alternating order: one order lower along half-staggered directions
+        self.s_stag = (b0 if order == 1 else b1) if scheme == 1 else self.s
         self.dV = self.dx[0] * self.dx[1] * self.dx[2]
 
     # ---- Eq. 11 with piecewise-constant fields: E_p = sum_grid F * s s s -------------------
     def gather_one(self, F, c, stag, pos):
         nx, ny, nz = self.n
-        wx = _weights_1d(self.s, nx, pos[0] / self.dx[0], stag[0])
-        wy = _weights_1d(self.s, ny, pos[1] / self.dx[1], stag[1])
-        wz = _weights_1d(self.s, nz, pos[2] / self.dx[2], stag[2])
+        sh = [self.s_stag if stag[d] != 0.0 else self.s for d in range(3)]
+        wx = _weights_1d(sh[0], nx, pos[0] / self.dx[0], stag[0])
+        wy = _weights_1d(sh[1], ny, pos[1] / self.dx[1], stag[1])
+        wz = _weights_1d(sh[2], nz, pos[2] / self.dx[2], stag[2])
         tot = 0.0
         for k in range(nz):
             for j in range(ny):

@@ -42,6 +42,10 @@ typedef struct {
   double dx[3];
   double dt;
   double q[8], m[8];
+  int32_t scheme;    /* 0: every weight of the gather has the order above; 1: alternating order
+                        ([22]; A29): along a direction in which a field
+                        component is half-staggered its gather weight is one order LOWER
+                        (order 1: b0 instead of b1; order 2: b1 instead of b2) */
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -184,7 +188,9 @@ static inline double b2(double xi) {
 
 /* ------------------------------------------------------------------------------------------ */
 /* gather, PAPER.md:88-92 (Eq. 11), 196: each component interpolated from its own staggered    */
-/* points with b1 (order 1) or b2 (order 2); factor 1 along an invariant direction.            */
+/* points with b1 (order 1) or b2 (order 2); factor 1 along an invariant direction.  With the   */
+/* alternating-order scheme the weight along a half-staggered direction of the   */
+/* component is one order lower; the deposit, and with it charge conservation, is unchanged.    */
 
 /* 1-d stencil for a sample point xi (in units of cells, measured from the first staggered
  * location of this component, i.e. stag already subtracted): fills idx0, npts, w[].           */
@@ -195,7 +201,11 @@ static inline void stencil(int order, int n, double xi, int *idx0, int *npts, do
     w[0] = 1.0;
     return;
   }
-  if (order == 1) {
+  if (order == 0) { /* b0: the nearest point (alternating-order gather of first-order particles) */
+    *idx0 = (int)floor(xi + 0.5);
+    *npts = 1;
+    w[0] = 1.0;
+  } else if (order == 1) {
     int i0 = (int)floor(xi);
     *idx0 = i0;
     *npts = 2;
@@ -216,7 +226,8 @@ static double gather_one(const orc_params *p, const double *F, int c, const doub
   int i0[3], np[3];
   double w[3][3];
   for (int d = 0; d < 3; d++)
-    stencil(p->order, p->n[d], x[d] / p->dx[d] - stag[d], &i0[d], &np[d], w[d]);
+    stencil(p->order - ((p->scheme == 1 && stag[d] != 0.0) ? 1 : 0), p->n[d], x[d] / p->dx[d] - stag[d],
+            &i0[d], &np[d], w[d]);
   double s = 0.0;
   for (int c2 = 0; c2 < np[2]; c2++)
     for (int c1 = 0; c1 < np[1]; c1++)

@@ -39,6 +39,7 @@ class OrcParams(C.Structure):
         ("dt", C.c_double),
         ("q", C.c_double * 8),
         ("m", C.c_double * 8),
+        ("scheme", C.c_int32),
     ]
 
 
@@ -73,7 +74,7 @@ def _i(a):
 class Oracle:
     """One grid + species table.  All methods call straight into the C oracle."""
 
-    def __init__(self, n, dx, dt, order, q, m, block=None):
+    def __init__(self, n, dx, dt, order, q, m, block=None, scheme=0):
         self.n = tuple(int(v) for v in n)
         self.dx = tuple(float(v) for v in dx)
         self.dt = float(dt)
@@ -90,6 +91,8 @@ class Oracle:
         p.dt = self.dt
         p.order = self.order
         p.n_species = len(self.q)
+        p.scheme = int(scheme)
+        self.scheme = int(scheme)
         for s in range(len(self.q)):
             p.q[s] = self.q[s]
             p.m[s] = self.m[s]

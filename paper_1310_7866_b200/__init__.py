@@ -16,6 +16,7 @@ PSC_OK = 0
 PSC_E, PSC_B, PSC_J = 0, 1, 2
 PSC_F_OOB, PSC_F_NAN, PSC_F_SPECIES, PSC_F_OVERFLOW = 1, 4, 8, 32
 PSC_GHOST = 2
+PSC_SCHEME_STANDARD, PSC_SCHEME_ALTERNATING = 0, 1
 PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
           "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9, "marder": 10}
 PSC_PH_COUNT = 16
@@ -44,6 +45,7 @@ class PscParams(C.Structure):
         ("q", C.POINTER(C.c_float)),
         ("m", C.POINTER(C.c_float)),
         ("block", C.c_int32 * 3),
+        ("scheme", C.c_int32),
     ]
 
 
@@ -131,7 +133,7 @@ def _cols(tensors) -> PscCols:
 class Psc:
     """One psc_ctx.  Method names are the C names without the psc_ prefix."""
 
-    def __init__(self, n, dx, dt, order, q, m, block=(0, 0, 0)):
+    def __init__(self, n, dx, dt, order, q, m, block=(0, 0, 0), scheme=0):
         self._h = None
         L = lib()
         p = PscParams()
@@ -142,6 +144,7 @@ class Psc:
         p.ghost = PSC_GHOST
         p.dt = float(dt)
         p.order = int(order)
+        p.scheme = int(scheme)
         p.n_species = len(q)
         self._q = (C.c_float * len(q))(*[float(v) for v in q])
         self._m = (C.c_float * len(m))(*[float(v) for v in m])

@@ -74,6 +74,7 @@ int psc_create(const psc_params *p, psc_ctx **out) {
   if (!p || !out) return PSC_ERR_INVALID_ARG;
   *out = nullptr;
   if (p->order != 1 && p->order != 2) return PSC_ERR_INVALID_ARG;
+  if (p->scheme != PSC_SCHEME_STANDARD && p->scheme != PSC_SCHEME_ALTERNATING) return PSC_ERR_INVALID_ARG;
   if (p->n_species < 1 || p->n_species > PSC_MAX_SPECIES || !p->q || !p->m) return PSC_ERR_INVALID_ARG;
   if (p->ghost != PSC_GHOST) return PSC_ERR_INVALID_ARG;
   if (!(p->dt > 0.f)) return PSC_ERR_INVALID_ARG;
@@ -137,6 +138,7 @@ int psc_create(const psc_params *p, psc_ctx **out) {
   gd.nkeys = (int)nk;
   gd.ntiles = gd.nb[0] * gd.nb[1] * gd.nb[2];
   gd.order = p->order;
+  gd.gmode = p->scheme;
   gd.nsp = p->n_species;
   gd.nd = is3d ? 27 : 9;
   for (int s = 0; s < p->n_species; s++) {

@@ -335,7 +335,7 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
 // XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id).
 // BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
 // launch for the tiles in which the first one had to leave a cell out.
-template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG, int CT>
+template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG, int CT, bool ALT>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
@@ -414,11 +414,13 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
 
   // One particle: gather (Eq. 11 with b1 weights; each component from its own Yee points:
   // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l (a < 1/2, weight
-  // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28).
+  // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28).  ALT: the alternating-order scheme
+  // (A29): along a half-staggered direction the weight is b0, i.e. the
+  // cell's own point l with weight 1.
   auto kick = [&](const float *cF, float ax, float ay, float az, float &ux, float &uy, float &uz, int sp) {
-    const bool hy = ay >= 0.5f, hz = az >= 0.5f, hx = D3 && ax >= 0.5f;
-    const float gy = hy ? ay - 0.5f : ay + 0.5f, gz = hz ? az - 0.5f : az + 0.5f;
-    const float gx = hx ? ax - 0.5f : ax + 0.5f;
+    const bool hy = ALT || ay >= 0.5f, hz = ALT || az >= 0.5f, hx = D3 && (ALT || ax >= 0.5f);
+    const float gy = ALT ? 0.f : (hy ? ay - 0.5f : ay + 0.5f), gz = ALT ? 0.f : (hz ? az - 0.5f : az + 0.5f);
+    const float gx = ALT ? 0.f : (hx ? ax - 0.5f : ax + 0.5f);
     const int oy = hy ? 0 : -fs1, oz = hz ? 0 : -fs2, ox = (!D3 || hx) ? 0 : -1;
     const float ex = gather1<D3>(cF + ox, fs1, fs2, gx, ay, az);
     const float ey = gather1<D3>(cF + fvol + oy, fs1, fs2, ax, gy, az);
@@ -652,9 +654,17 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, XC_, BIG_, CT_, SMEM_, WS_)                             \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_>,               \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false>,        \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    PSC_LAUNCH_CHECK(c);                                                                           \
+  } while (0)
+  // the alternating-order scheme runs the general instantiation (run-time tile, optional columns)
+#define PSC_LAUNCH_PUSH1_ALT(D3_, B_, BIG_, SMEM_, WS_)                                            \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, 0, 128, B_, true, BIG_, 0, true>,            \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
+    k_push1<D3_, 0, 128, B_, true, BIG_, 0, true><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the image launch, then the launch for the cells it had to leave out (its blocks return at
@@ -673,7 +683,15 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_big, ws_big);                       \
     }                                                                                              \
   } while (0)
-  if (d3) {
+  if (gd.gmode == PSC_SCHEME_ALTERNATING) {
+    if (d3) {
+      PSC_LAUNCH_PUSH1_ALT(true, 4, false, smem_img, ws_img);
+      PSC_LAUNCH_PUSH1_ALT(true, 2, true, smem_big, ws_big);
+    } else {
+      PSC_LAUNCH_PUSH1_ALT(false, 5, false, smem_img, ws_img);
+      PSC_LAUNCH_PUSH1_ALT(false, 2, true, smem_big, ws_big);
+    }
+  } else if (d3) {
     const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
     if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4, true);
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
@@ -684,5 +702,6 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   }
 #undef PSC_LAUNCH_PUSH1
 #undef PSC_LAUNCH_PUSH1_
+#undef PSC_LAUNCH_PUSH1_ALT
   return PSC_OK;
 }

@@ -131,11 +131,20 @@ struct Sten2 {
   int tn;           // first tile point of the node-centred stencil (l + (a >= 1/2))
   float wn[3];      // node-centred weights
   float ws[3];      // half-staggered weights; first tile point is l
+  // ALT: alternating-order scheme (A29): b1 instead of b2 along a
+  // half-staggered direction, on the same three points
+  template <bool ALT>
   __device__ __forceinline__ void set(int l, float a) {
     const bool up = a >= 0.5f;
     tn = l + (up ? 1 : 0);
     tsc3(up ? a - 1.0f : a, wn[0], wn[1], wn[2]);
-    tsc3(a - 0.5f, ws[0], ws[1], ws[2]);
+    if (ALT) {
+      ws[0] = up ? 0.f : 0.5f - a;
+      ws[1] = up ? 1.5f - a : 0.5f + a;
+      ws[2] = up ? a - 0.5f : 0.f;
+    } else {
+      tsc3(a - 0.5f, ws[0], ws[1], ws[2]);
+    }
   }
 };
 
@@ -206,7 +215,7 @@ __device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const flo
 
 // BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
 // launch for the tiles in which the first one had to leave a cell out.
-template <bool D3, int CBS, bool XC, bool BIG>
+template <bool D3, int CBS, bool XC, bool BIG, bool ALT>
 __global__ void __launch_bounds__(PUSH2_THREADS, 2)
 k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
@@ -354,9 +363,9 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       const int sp = cur.sp & (PSC_MAX_SPECIES - 1);
       // ---- gather (Eq. 11 with b2 weights; each component from its own Yee points) ---------
       Sten2 sx, sy, sz;
-      sx.set(lx, ax);
-      sy.set(ly, ay);
-      sz.set(lz, az);
+      sx.template set<ALT>(lx, ax);
+      sy.template set<ALT>(ly, ay);
+      sz.template set<ALT>(lz, az);
       const float ex = gather2<D3, true, false, false>(sEx, tg, lx, ly, lz, sx, sy, sz);
       const float ey = gather2<D3, false, true, false>(sEy, tg, lx, ly, lz, sx, sy, sz);
       const float ez = gather2<D3, false, false, true>(sEz, tg, lx, ly, lz, sx, sy, sz);
@@ -555,9 +564,17 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_, BIG_, SMEM_, WS_)                                         \
   do {                                                                                             \
-    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_, BIG_>,                            \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_, BIG_, false>,                     \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push2<D3_, CBS_, XC_, BIG_><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push2<D3_, CBS_, XC_, BIG_, false><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    PSC_LAUNCH_CHECK(c);                                                                           \
+  } while (0)
+  // the alternating-order scheme runs the general instantiation (run-time tile, optional columns)
+#define PSC_LAUNCH_PUSH2_ALT(D3_, BIG_, SMEM_, WS_)                                                 \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, 0, true, BIG_, true>,                        \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
+    k_push2<D3_, 0, true, BIG_, true><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
 #define PSC_LAUNCH_PUSH2(D3_, CBS_)                                       \
@@ -570,7 +587,15 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
       PSC_LAUNCH_PUSH2_(D3_, CBS_, false, true, smem_big, ws_big);        \
     }                                                                     \
   } while (0)
-  if (d3) {
+  if (gd.gmode == PSC_SCHEME_ALTERNATING) {
+    if (d3) {
+      PSC_LAUNCH_PUSH2_ALT(true, false, smem_img, ws_img);
+      PSC_LAUNCH_PUSH2_ALT(true, true, smem_big, ws_big);
+    } else {
+      PSC_LAUNCH_PUSH2_ALT(false, false, smem_img, ws_img);
+      PSC_LAUNCH_PUSH2_ALT(false, true, smem_big, ws_big);
+    }
+  } else if (d3) {
     if (gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4) PSC_LAUNCH_PUSH2(true, 4);
     else PSC_LAUNCH_PUSH2(true, 0);
   } else {
@@ -579,5 +604,6 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   }
 #undef PSC_LAUNCH_PUSH2
 #undef PSC_LAUNCH_PUSH2_
+#undef PSC_LAUNCH_PUSH2_ALT
   return PSC_OK;
 }

@@ -10,10 +10,10 @@ from . import COLUMNS, PSC_B, PSC_E, PSC_GHOST, Psc
 
 
 class Simulation:
-    def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True, with_x=True):
+    def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True, with_x=True, scheme=0):
         self.device = torch.device(device)
         self.plasma = plasma
-        self.psc = Psc(plasma.n, plasma.dx, plasma.dt, plasma.order, plasma.q, plasma.m, block)
+        self.psc = Psc(plasma.n, plasma.dx, plasma.dt, plasma.order, plasma.q, plasma.m, block, scheme)
         self.n = tuple(plasma.n)
         self.g = tuple(PSC_GHOST if v > 1 else 0 for v in self.n)
         self.np = plasma.n_particles

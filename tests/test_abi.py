@@ -56,6 +56,9 @@ def test_create_validates_before_touching_the_device():
     h = C.c_void_p()
     assert L.psc_create(None, C.byref(h)) == -1
     assert L.psc_create(C.byref(_params(order=3)), C.byref(h)) == -1
+    bad = _params()
+    bad.scheme = 2
+    assert L.psc_create(C.byref(bad), C.byref(h)) == -1
     assert L.psc_create(C.byref(_params(ghost=1)), C.byref(h)) == -1
     assert L.psc_create(C.byref(_params(n=(1, 3, 16))), C.byref(h)) == -1
     assert L.psc_create(C.byref(_params(dt=0.6)), C.byref(h)) == -4          # PSC_ERR_CFL

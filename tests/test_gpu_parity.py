@@ -522,3 +522,43 @@ def test_step_host_end_to_end():
     for k in ("y", "z", "ux", "uy", "uz"):
         assert np.abs(host[k].numpy() - ref[k]).max() < 1e-5, k
     assert (hE - refE).abs().max() <= 1e-5 * refE.abs().max()
+
+
+# ------------------------------------------------------------------------------------------------
+# alternating-order interpolation (A29)
+
+@pytest.mark.parametrize("kind", ["2d", "3d", "2d-o2", "beam", "3d-aniso", "2d-aniso-o2"])
+def test_alternating_order_ten_steps_match_oracle(kind):
+    """PSC_SCHEME_ALTERNATING against the oracle's scheme 1: ten psc_step, particles by id"""
+    from paper_1310_7866_b200.harness import Simulation
+    pl = _small(kind)
+    smooth_fields(pl, 0.05, seed=29)
+    sim = Simulation(pl, scheme=1)
+    orc = oracle_for(pl, scheme=1)
+    std = oracle_for(pl, scheme=0)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    s0 = {k: v.copy() for k, v in st.items()}
+    orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], 10)
+    sim.step(10)
+    assert sim.psc.status() == 0
+    got = gpu_cols(sim)
+    order = np.argsort(got["id"], kind="stable")
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for d, c in enumerate(("x", "y", "z")):
+        if pl.n[d] > 1:
+            assert (periodic_dist(got[c][order], st[c], L[d]) / L[d]).max() < TOL
+    for s_ in range(len(pl.q)):
+        m = st["species"] == s_
+        rms = np.sqrt(np.mean(st["ux"][m] ** 2 + st["uy"][m] ** 2 + st["uz"][m] ** 2))
+        for c in ("ux", "uy", "uz"):
+            assert np.abs(got[c][order][m] - st[c][m]).max() / rms < TOL
+    assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
+    assert rel_fieldnorm(sim.interior(sim.B).cpu().numpy(), B) < TOL
+    # and it is not the standard scheme in disguise
+    E0 = oracle_state(pl)[1]
+    B0 = oracle_state(pl)[2]
+    J0 = std.zeros_field()
+    std.step(E0, B0, J0, s0["x"], s0["y"], s0["z"], s0["ux"], s0["uy"], s0["uz"], s0["qw"], s0["species"], 10)
+    assert np.abs(s0["ux"] - st["ux"]).max() > 1e-4 * np.abs(st["ux"]).max()

@@ -209,3 +209,50 @@ def test_marder_fourier_mode_decays_by_the_closed_form_factor(n, dx):
     r0 = np.abs(orc.div_minus(E3) - rho_r).max()
     orc.marder(E3, rho_r, 1.0 / sum(4 / dx[d] ** 2 for d in range(3) if n[d] > 1), 30)
     assert np.abs(orc.div_minus(E3) - rho_r).max() < 0.8 * r0
+
+
+# ------------------------------------------------------------------------------------------------
+# alternating-order gather ([22]; A29)
+
+@pytest.mark.parametrize("order", [1, 2])
+@pytest.mark.parametrize("n", [(5, 6, 7), (1, 6, 5)])
+def test_alternating_gather_t1_equals_t0_and_closed_forms(order, n):
+    """scheme 1: along a direction in which a component is half-staggered the weight is one order
+    lower (b0 / b1 instead of b1 / b2).  T1 == the all-grid sum with those shapes; a uniform field
+    is reproduced; order 2 still reproduces a field linear in x (b1 does), order 1 returns the
+    value of the NEAREST staggered point along the staggered direction; and the unstaggered
+    directions are untouched (a component that varies only along them equals the standard gather)."""
+    dx = (1.0, 0.8, 1.25)
+    orc = Oracle(n, dx, 0.1, order, [-1.0], [1.0], scheme=1)
+    std = Oracle(n, dx, 0.1, order, [-1.0], [1.0], scheme=0)
+    bf = BruteForce(n, dx, 0.1, order, [-1.0], [1.0], scheme=1)
+    rng = np.random.default_rng(70 + order)
+    E, B = rng.standard_normal(orc.fshape), rng.standard_normal(orc.fshape)
+    npart = 12
+    pos = [np.ascontiguousarray(rng.random(npart) * n[d] * dx[d]) for d in range(3)]
+    EB = orc.gather(E, B, *pos)
+    for a in range(npart):
+        Ep, Bp = bf.gather(E, B, (pos[0][a], pos[1][a], pos[2][a]))
+        assert np.abs(EB[a, :3] - Ep).max() < 1e-13
+        assert np.abs(EB[a, 3:] - Bp).max() < 1e-13
+    assert np.abs(EB - std.gather(E, B, *pos)).max() > 1e-3         # it IS a different scheme
+    # uniform field
+    U = np.ones(orc.fshape) * np.array([0.3, -1.0, 2.0])[:, None, None, None]
+    EBu = orc.gather(U, 2 * U, *pos)
+    assert np.abs(EBu[:, :3] - [0.3, -1.0, 2.0]).max() < 1e-14 and np.abs(EBu[:, 3:] - [0.6, -2.0, 4.0]).max() < 1e-14
+    # E_z varying along z only (its staggered direction), particles away from the seam
+    kk = np.arange(n[2])[:, None, None] * np.ones((1, n[1], n[0]))
+    F = np.zeros(orc.fshape)
+    F[2] = 1.5 + 0.25 * (kk + 0.5) * dx[2]                          # linear in z, sampled at k + 1/2
+    z = np.ascontiguousarray((1.6 + rng.random(npart) * (n[2] - 3.5)) * dx[2])
+    got = orc.gather(F, F, pos[0], pos[1], z)[:, 2]
+    if order == 2:
+        assert np.abs(got - (1.5 + 0.25 * z)).max() < 1e-13
+    else:
+        nearest = np.floor(z / dx[2]) + 0.5                          # the half point of the particle's cell
+        assert np.abs(got - (1.5 + 0.25 * nearest * dx[2])).max() < 1e-13
+    # E_z varying along y only (unstaggered for E_z): same as the standard scheme
+    jj = np.arange(n[1])[None, :, None] * np.ones((n[2], 1, n[0]))
+    G = np.zeros(orc.fshape)
+    G[2] = np.sin(2 * np.pi * jj / n[1])
+    assert np.abs(orc.gather(G, G, *pos)[:, 2] - std.gather(G, G, *pos)[:, 2]).max() < 1e-14

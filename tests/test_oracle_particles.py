@@ -355,15 +355,16 @@ def _small_plasma(rng, n, dx, npart, vth):
 
 @pytest.mark.parametrize("order,n", [(1, (5, 4, 6)), (1, (1, 6, 5)), (2, (6, 6, 7)), (2, (1, 7, 6)), (1, (6, 1, 1))])
 @pytest.mark.parametrize("npart", [1, 8])
-def test_step_t1_equals_t0(order, n, npart):
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_step_t1_equals_t0(order, n, npart, scheme):
     """three full steps of the stencil oracle == the definition-level brute force (gather over the
     whole grid, flux-integral / whole-grid deposits, np.roll FDTD) on 1-8 particles."""
     dx = (1.0, 0.9, 1.2)
     dt = 0.45 / np.sqrt(sum(1 / dx[d] ** 2 for d in range(3) if n[d] > 1))
     q, m = [-1.0, 1.0], [1.0, 4.0]
     rng = np.random.default_rng(100 * order + npart + n[0])
-    orc = Oracle(n, dx, dt, order, q, m)
-    bf = BruteForce(n, dx, dt, order, q, m)
+    orc = Oracle(n, dx, dt, order, q, m, scheme=scheme)
+    bf = BruteForce(n, dx, dt, order, q, m, scheme=scheme)
     pos, u, qw, species = _small_plasma(rng, n, dx, npart, 0.6)
     E = 0.3 * rng.standard_normal(orc.fshape)
     B = 0.3 * rng.standard_normal(orc.fshape)
@@ -384,14 +385,15 @@ def test_step_t1_equals_t0(order, n, npart):
 
 
 @pytest.mark.parametrize("order,n", [(1, (1, 16, 16)), (1, (8, 8, 8)), (2, (8, 8, 8)), (2, (1, 12, 12))])
-def test_step_gauss_law_and_divb_invariants(order, n):
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_step_gauss_law_and_divb_invariants(order, n, scheme):
     """with a charge-conserving j, div- E - rho keeps its initial value and
     div+ B stays 0 to round-off; no particle moves more than one cell per step."""
     dx = (1.0, 1.0, 1.0)
     dt = 0.5 / np.sqrt(sum(1 / dx[d] ** 2 for d in range(3) if n[d] > 1))
     q, m = [-1.0, 1.0], [1.0, 25.0]
     rng = np.random.default_rng(5 + order)
-    orc = Oracle(n, dx, dt, order, q, m)
+    orc = Oracle(n, dx, dt, order, q, m, scheme=scheme)   # (the deposit, hence Gauss's law, is scheme independent)
     npart = 4000
     pos, u, qw, species = _small_plasma(rng, n, dx, npart, 0.3)
     E = 0.05 * rng.standard_normal(orc.fshape)
@@ -533,3 +535,23 @@ def test_wrap_lands_on_upper_edge():
     orc.push_particles(Z, Z, J, x, y, z, ux, uy, uz, _c(np.array([-1.0])), np.zeros(1, dtype=np.int32))
     g = np.sqrt(1 + 8.0)
     assert abs(y[0] - (0.1 - 0.3 * 2.0 / g + 8.0)) < 1e-14 and abs(z[0] - (7.9 + 0.3 * 2.0 / g - 8.0)) < 1e-14
+
+
+def test_alternating_order_improves_energy_conservation():
+    """"alternating-order interpolation schemes from [22] for improved energy
+    conservation" -- the reading of DESIGN.md A29 (gather weight one order lower along a
+    component's half-staggered directions) must deliver that: on config 1 the total-energy drift
+    over 400 steps is at least five times smaller than with the standard gather (measured: ~20x)."""
+    import psc_inputs
+
+    drift = []
+    for scheme in (0, 1):
+        pl = psc_inputs.make_config(1)
+        orc = Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m, scheme=scheme)
+        cols = [_c(t.numpy()) for t in (pl.x, pl.y, pl.z, pl.ux, pl.uy, pl.uz, pl.qw)]
+        sp = np.ascontiguousarray(pl.species.numpy())
+        E, B, J = _c(pl.E.numpy()), _c(pl.B.numpy()), orc.zeros_field()
+        e0 = orc.energy(E, B, cols[3], cols[4], cols[5], cols[6], sp).sum()
+        orc.step(E, B, J, *cols, sp, 400)
+        drift.append(abs(orc.energy(E, B, cols[3], cols[4], cols[5], cols[6], sp).sum() / e0 - 1))
+    assert drift[1] < 0.2 * drift[0], drift

@@ -7,8 +7,8 @@ from oracle.psc_oracle import Oracle
 PCOLS = ("x", "y", "z", "ux", "uy", "uz", "qw")
 
 
-def oracle_for(pl, block=(1, 1, 1)):
-    return Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m, block=block)
+def oracle_for(pl, block=(1, 1, 1), scheme=0):
+    return Oracle(pl.n, pl.dx, pl.dt, pl.order, pl.q, pl.m, block=block, scheme=scheme)
 
 
 def oracle_state(pl):
