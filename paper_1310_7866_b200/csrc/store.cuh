@@ -130,7 +130,7 @@ struct CellWalker {
   static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
   // bytes of per-warp shared memory for an image of C slots x ncol columns
   __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
-    return (BIG ? 0 : ncol * C * 4 + C /*holes*/) + WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ + 32 * 4 /*xrow*/ +
+    return (BIG ? WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ : ncol * C * 4 + C /*holes*/) + 32 * 4 /*xrow*/ +
            12 * 4 /*hbm*/ + 16 /*bar*/;
   }
   float *buf;      // [ncol][C]
@@ -138,7 +138,8 @@ struct CellWalker {
   uint16_t *arr;   // [WALK_AC]: arrival a -> direction lane << 8 | record index in that neighbour's row
   int *nbk;        // [32]: key of the neighbour cell a lane looks at
   unsigned *xrow;  // [32]: per direction code, which of the cell's records so far moved that way
-  unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole
+  unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole; hbm[11]: arrival counter
+  int *acnt;
   uint64_t *bar;
   const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
   int Crt, ncol, lane;
@@ -150,7 +151,8 @@ struct CellWalker {
   // current cell
   int key, n, na, base, cap;
   bool fits;         // n + na <= C: the cell takes the image path
-  int nh, tcur, nleave, a0, my_start;
+  int nh, tcur, nleave, a0, my_start, my_src;
+  unsigned my_mask;
 
   __device__ __forceinline__ void init(unsigned char *wsm, const StoreDesc &sd, int lane_, const int *nbt_) {
     Crt = sd.imgC;
@@ -161,11 +163,13 @@ struct CellWalker {
     lt = lanemask_lt_();
     buf = (float *)wsm;
     holes = (uint8_t *)(buf + (BIG ? 0 : ncol * C));
-    arr = (uint16_t *)(holes + (BIG ? 0 : C));
-    nbk = (int *)(arr + WALK_AC);
-    xrow = (unsigned *)(nbk + 32);
+    arr = (uint16_t *)(holes + (BIG ? 0 : C));  // (arr, nbk: the BIG form only)
+    nbk = (int *)(arr + (BIG ? WALK_AC : 0));
+    xrow = (unsigned *)(nbk + (BIG ? 32 : 0));
     hbm = xrow + 32;
     bar = (uint64_t *)(hbm + 12);
+    acnt = (int *)(hbm + 11);
+    if (lane == 0) *acnt = 0;
     parity = 0;
     loads_armed = false;
     xrow[lane] = 0u;
@@ -238,19 +242,25 @@ struct CellWalker {
     n = n_;
     base = base_;
     cap = cap_;
-    nbk[lane] = src;
     const int cntm = __popc(mask);
-    int inc = cntm;
+    my_mask = mask;
+    my_src = src;
+    if (BIG) {  // the global path walks the arrivals through a list in shared memory
+      nbk[lane] = src;
+      int inc = cntm;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+      }
+      na = __shfl_sync(0xffffffffu, inc, 31);
+      my_start = inc - cntm;
+      a0 = 0;
+      if (na) fill_window(mask);
+    } else {
+      na = __reduce_add_sync(0xffffffffu, cntm);
     }
-    na = __shfl_sync(0xffffffffu, inc, 31);
-    my_start = inc - cntm;
-    a0 = 0;
-    fits = n + na <= C && na <= WALK_AC;
-    if (na && (BIG || fits)) fill_window(mask);
+    fits = n + na <= C;
     nh = 0;
     tcur = 0;
     nleave = 0;
@@ -264,21 +274,31 @@ struct CellWalker {
   // ---- image path ---------------------------------------------------------------------------------
 
   // The arrivals' record words go to the image slots [n, n + na) behind the residents, by
-  // asynchronous 4-byte copies (a lane per arrival); wait with arrivals_landed().
+  // asynchronous 4-byte copies: the lane that looked at a neighbour's header copies the records it
+  // found there (which slot each takes is decided by a shared counter: the order of arrivals
+  // inside a cell is immaterial); wait with arrivals_landed().
   __device__ __forceinline__ void stage_arrivals(const StoreDesc &sd) {
-    for (int a = lane; a < na; a += 32) {
-      const int e = arr[a];
-      const size_t idx = (size_t)nbk[e >> 8] * PSC_XCAP + (e & 255);
-      const float *r = reinterpret_cast<const float *>(sd.xin.rec + idx);
-      float *q = buf + n + a;
+    unsigned m = my_mask;
+    if (m) {
+      int slot = n + atomicAdd(acnt, __popc(m));
+      const size_t row = (size_t)my_src * PSC_XCAP;
+      while (m) {
+        const size_t idx = row + (__ffs(m) - 1);
+        const float *r = reinterpret_cast<const float *>(sd.xin.rec + idx);
+        float *q = buf + slot;
 #pragma unroll
-      for (int w = 0; w < NREC; w++) cp_async4(q + w * C, r + w, true);
-      if (XC) {
-        if (sd.icol_x2d >= 0) cp_async4(q + sd.icol_x2d * C, r + 7, true);
-        if (sd.icol_id >= 0) cp_async4(q + sd.icol_id * C, sd.xin.id + idx, true);
+        for (int w = 0; w < NREC; w++) cp_async4(q + w * C, r + w, true);
+        if (XC) {
+          if (sd.icol_x2d >= 0) cp_async4(q + sd.icol_x2d * C, r + 7, true);
+          if (sd.icol_id >= 0) cp_async4(q + sd.icol_id * C, sd.xin.id + idx, true);
+        }
+        slot++;
+        m &= m - 1;
       }
     }
     cp_async_commit();
+    __syncwarp();
+    if (lane == 0) *acnt = 0;
   }
   // Before the first chunk that touches slots >= n: the arrivals are in the image, and the slots
   // between the last particle and the end of its chunk hold a harmless particle (at rest, no
