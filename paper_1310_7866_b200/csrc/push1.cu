@@ -40,9 +40,8 @@ namespace {
 
 constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
 // rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 endx (2-d: v_x),
-// 5 endy, 6 endz, 7 qw.  The drain reuses rows [0, NV) of a drained entry as its scratch column,
-// hence 12 rows in 3-d.
-constexpr int QROWS2 = 8, QROWS3 = 12;
+// 5 endy, 6 endz, 7 qw
+constexpr int QROWS2 = 8, QROWS3 = 8;
 
 
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
@@ -228,19 +227,17 @@ __device__ __forceinline__ void moments_to_values(float (&acc)[D3 ? 12 : 8]) {
 // Walks the straight line a -> end (cells; at most one face crossing per direction because
 // dt <= dx/2) and deposits every segment -- the slow path of the kernel below,
 // taken by the trajectories that leave their cell.
-// The segments' currents are added with shared-memory atomics, which are compare-and-swap loops
-// for fp32 (ATOMS.CAST.SPIN) and therefore pay for every same-address collision inside the
-// warp.  The trajectories drained together come from a few cells and cross the same faces, i.e.
-// hit the same J points in the same order; so each lane walks its NV values in a different
-// rotation (start = lane mod NV): the values go through a lane-private scratch column `scr`
-// ([NV][QCAP], the drained queue slots) and are picked with the rotated index, the point offsets
-// from the table `rel` ([NV], the order of vb_values).
+// The segments' currents go straight to the global J with fire-and-forget reductions (RED.ADD.F32,
+// resolved in the L2, where J lives): a shared-memory fp32 atomicAdd is a compare-and-swap loop on
+// sm_100a whose retries -- the trajectories drained together come from a few cells and hit the
+// same points -- made this path the largest single stall of the kernel.  (lx, ly, lz): the
+// trajectory's cell inside the tile; gnode0: global index of the tile's first cell's node; rel:
+// the NV point offsets of vb_values in the global array.
 template <bool D3, class TG>
-__device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, int lx,
+__device__ __forceinline__ void vb_walk(float *__restrict__ J, const GridDesc &gd, int gnode0, int lx,
                                         int ly, int lz, float ax, float ay, float az, float endx,
                                         float endy, float endz, float fx, float fy, float fz,
-                                        float qvx, const int *__restrict__ rel,
-                                        float *__restrict__ scr, int rot) {
+                                        float qvx, const int *__restrict__ rel) {
   constexpr int NV = D3 ? 12 : 8;
   const float ddx = endx - ax, ddy = endy - ay, ddz = endz - az;
   const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
@@ -269,17 +266,9 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
     {
       float v[NV];
       vb_values<D3>(v, px - rx, py - ry, pz - rz, qx - rx, qy - ry, qz - rz, t - tprev, fx, fy, fz, qvx);
-      const int cx = lx + rx, cy = ly + ry, cz = lz + rz;
-      float *node = sJ + (D3 ? ((cz + 1) * tg.je[1] + (cy + 1)) * tg.je[0] + (cx + 1)
-                             : (cz + 1) * tg.je[1] + (cy + 1));
+      float *node = J + gnode0 + (D3 ? (lx + rx) : 0) + (ly + ry) * gd.st[1] + (lz + rz) * gd.st[2];
 #pragma unroll
-      for (int i = 0; i < NV; i++) scr[i * QCAP] = v[i];
-      int idx = rot;
-#pragma unroll
-      for (int j = 0; j < NV; j++) {
-        atomicAdd(node + rel[idx], scr[idx * QCAP]);
-        idx = idx + 1 == NV ? 0 : idx + 1;
-      }
+      for (int i = 0; i < NV; i++) atomicAdd(node + rel[i], v[i]);
     }
     if (which == 3) break;
     if (which == 0) { rx += sxd; tx = 2.f; }
@@ -290,12 +279,11 @@ __device__ __forceinline__ void vb_walk(float *__restrict__ sJ, const TG &tg, in
   }
 }
 
-
 // Drains n (<= 32) queue entries starting at `start`: deposits every segment of each trajectory.
 template <bool D3, class TG>
-__device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg, const GridDesc &gd,
-                                            float *__restrict__ q, const int *__restrict__ rel,
-                                            int start, int n, int lane) {
+__device__ __forceinline__ void drain_queue(float *__restrict__ J, const TG &tg, const GridDesc &gd,
+                                            int gnode0, const float *__restrict__ q,
+                                            const int *__restrict__ rel, int start, int n, int lane) {
   if (lane < n) {
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
@@ -306,8 +294,8 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ sJ, const TG &tg
     // 2-d: the endx slot carries v_x: the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
     const float qvx = D3 ? 0.f : qw * gd.inv_dV * ex;
-    vb_walk<D3>(sJ, tg, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ex : 0.f, ey, ez, fx, fy, fz,
-                qvx, rel, q + e, lane % (D3 ? 12 : 8));
+    vb_walk<D3, TG>(J, gd, gnode0, lx, ly, lz, D3 ? ax : 0.f, ay, az, D3 ? ex : 0.f, ey, ez, fx, fy, fz,
+                    qvx, rel);
   }
   __syncwarp();
 }
@@ -354,8 +342,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP);  // [6][fvol]
   float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
   float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
-  int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [12]: J points of vb_values
-  int *sNbT = sRel + 12;                      // [27]: first key of the 3^3 neighbouring tiles
+  int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [24]: J points of vb_values (tile, global)
+  int *sNbT = sRel + 24;                      // [27]: first key of the 3^3 neighbouring tiles
   int *sBase = sNbT + 27;                     // [cpb + 1]: first slot of each cell
   int *sCnt = sBase + tg.cpb + 1;             // [cpb]: particles resident in each cell
   Walker wk;
@@ -369,12 +357,16 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     sNbT[t] = ((n2 * gd.nb[1] + n1) * gd.nb[0] + (D3 ? n0 : 0)) * tg.cpb;
   }
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
-  if (threadIdx.x < NV) {  // J points of the NV in-cell currents, relative to the cell's node
-    const int s1 = tg.je[0], s2 = tg.je[0] * tg.je[1], jv = tg.jvol;
+  if (threadIdx.x < 2 * NV) {  // J points of the NV in-cell currents, relative to the cell's node:
+    // [0, NV) in the block's J tile, [NV, 2 NV) in the global array
+    const bool glob = threadIdx.x >= NV;
+    const int i = glob ? threadIdx.x - NV : threadIdx.x;
+    const int s1 = glob ? gd.st[1] : tg.je[0], s2 = glob ? gd.st[2] : tg.je[0] * tg.je[1];
+    const int jv = glob ? gd.comp : tg.jvol;
     const int off3[12] = {0, s1, s2, s1 + s2, jv, jv + s2, jv + 1, jv + s2 + 1,
                           2 * jv, 2 * jv + 1, 2 * jv + s1, 2 * jv + s1 + 1};
-    const int off2[8] = {0, 1, s2, s2 + 1, jv, jv + s2, 2 * jv, 2 * jv + 1};
-    sRel[threadIdx.x] = D3 ? off3[threadIdx.x] : off2[threadIdx.x & 7];
+    const int off2[8] = {0, s1, s2, s2 + s1, jv, jv + s2, 2 * jv, 2 * jv + s1};
+    sRel[threadIdx.x] = D3 ? off3[i] : off2[i & 7];
   }
   const int kbase = blockIdx.x * tg.cpb;
   for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
@@ -410,6 +402,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     writer = (lane & 3) == 0;
   }
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
+  // global index of the node of the tile's first cell
+  const int gnode0 = ((tg.o[2] + gd.g[2]) * gd.ext[1] + (tg.o[1] + gd.g[1])) * gd.ext[0] + (D3 ? tg.o[0] + gd.g[0] : 0);
   bool left_out = false;  // this warp met a cell that does not fit the image
 
   // One particle: gather (Eq. 11 with b1 weights; each component from its own Yee points:
@@ -474,9 +468,11 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     }
     qcnt += __popc(cm);
     __syncwarp();
-    if (qcnt >= 32) {
+    // (the image path drains after the cell, while the next cell's run is being fetched; a cell
+    // with more than 32 leavers, and the global path, drain at once)
+    if (qcnt >= 32 && (BIG || qcnt + 32 > QCAP)) {
       qcnt -= 32;
-      drain_queue<D3>(sJ, tg, gd, myQ, sRel, qcnt, 32, lane);
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, 32, lane);
     }
   };
 
@@ -589,8 +585,15 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       }
     }
 
-    // ---- the cell is done: its in-cell currents take one warp reduction and one shared add per
-    // J point; its image goes back to global memory and the next cell's run is requested
+    // ---- the cell is done.  First its image goes back to global memory and the next cell's run
+    // is requested: everything below needs no image and runs while that request is in flight.
+    if (BIG) wk.end_global(sd);
+    else wk.end_image(sd, next_n, next_base);
+    if (qcnt >= 32) {
+      qcnt -= 32;
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, 32, lane);
+    }
+    // the in-cell currents take one warp reduction and one shared add per J point
     if (ntot) {
       float r;
       moments_to_values<D3>(acc);
@@ -603,10 +606,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         atomicAdd(&sJ[node + my_off], r);
       }
     }
-    if (BIG) wk.end_global(sd);
-    else wk.end_image(sd, next_n, next_base);
   }
-  if (qcnt) drain_queue<D3>(sJ, tg, gd, myQ, sRel, 0, qcnt, lane);
+  if (qcnt) drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
   const int any_left = __syncthreads_or(left_out ? 1 : 0);
@@ -642,7 +643,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const StoreDesc sd = psc_store_desc(c);
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
   constexpr int threads = 128;
-  const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 12 + 27 + 2 * gd.cpb + 2) * sizeof(float);
+  const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 24 + 27 + 2 * gd.cpb + 2) * sizeof(float);
   const size_t qbytes = (size_t)(d3 ? QROWS3 : QROWS2) * QCAP * 4;
   auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
   const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)

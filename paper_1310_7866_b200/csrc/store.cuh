@@ -66,6 +66,10 @@ __device__ __forceinline__ void bulk_s2g(void *gdst, const void *ssrc, unsigned 
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
                ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
 }
+// asks the L2 for a run of global memory (no destination: a later bulk copy finds it there)
+__device__ __forceinline__ void bulk_prefetch_l2(const void *gsrc, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -199,6 +203,23 @@ struct CellWalker {
     }
   }
 
+  // lane 0: ask the L2 for the resident run of the cell AFTER the current one, so that the bulk
+  // copies issued at the end of the current cell find it there (DRAM latency off the warp's path)
+  __device__ __forceinline__ void prefetch_l2(const StoreDesc &sd, int n_, int base_) {
+    if (BIG) return;
+    n_ = __shfl_sync(0xffffffffu, n_, 0);
+    base_ = __shfl_sync(0xffffffffu, base_, 0);
+    if (n_ > 0 && n_ <= C && lane == 0) {
+      const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
+      if (XC) {
+        for (int c = 0; c < ncol; c++) bulk_prefetch_l2(sd.col[c] + base_, bytes);
+      } else {
+#pragma unroll
+        for (int c = 0; c < NREC; c++) bulk_prefetch_l2(sd.col[c] + base_, bytes);
+      }
+    }
+  }
+
   // key of the cell that reaches cell (lx, ly, lz) of this tile by a move in this lane's direction
   template <class TG>
   __device__ __forceinline__ int source_key(const TG &tg, int lx, int ly, int lz) const {
@@ -274,31 +295,39 @@ struct CellWalker {
   // ---- image path ---------------------------------------------------------------------------------
 
   // The arrivals' record words go to the image slots [n, n + na) behind the residents, by
-  // asynchronous 4-byte copies: the lane that looked at a neighbour's header copies the records it
-  // found there (which slot each takes is decided by a shared counter: the order of arrivals
-  // inside a cell is immaterial); wait with arrivals_landed().
+  // asynchronous 4-byte copies, a lane per arrival.  Which record a slot takes is first noted in
+  // the slot itself (the lane that looked at a neighbour's header writes "my direction, record j"
+  // for every record it found; a shared counter hands out the slots: the order of arrivals inside
+  // a cell is immaterial).  Wait with arrivals_landed().
   __device__ __forceinline__ void stage_arrivals(const StoreDesc &sd) {
+    int *note = reinterpret_cast<int *>(buf) + (NREC - 1) * C + n;  // the species column's tail
     unsigned m = my_mask;
     if (m) {
-      int slot = n + atomicAdd(acnt, __popc(m));
-      const size_t row = (size_t)my_src * PSC_XCAP;
+      int a = atomicAdd(acnt, __popc(m));
       while (m) {
-        const size_t idx = row + (__ffs(m) - 1);
+        note[a++] = (lane << 8) | (__ffs(m) - 1);
+        m &= m - 1;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) *acnt = 0;
+    for (int a0_ = 0; a0_ < na; a0_ += 32) {
+      const int a = a0_ + lane;
+      const int e = a < na ? note[a] : 0;
+      const int src = __shfl_sync(0xffffffffu, my_src, (e >> 8) & 31);
+      if (a < na) {
+        const size_t idx = (size_t)src * PSC_XCAP + (e & 255);
         const float *r = reinterpret_cast<const float *>(sd.xin.rec + idx);
-        float *q = buf + slot;
+        float *q = buf + n + a;
 #pragma unroll
         for (int w = 0; w < NREC; w++) cp_async4(q + w * C, r + w, true);
         if (XC) {
           if (sd.icol_x2d >= 0) cp_async4(q + sd.icol_x2d * C, r + 7, true);
           if (sd.icol_id >= 0) cp_async4(q + sd.icol_id * C, sd.xin.id + idx, true);
         }
-        slot++;
-        m &= m - 1;
       }
     }
     cp_async_commit();
-    __syncwarp();
-    if (lane == 0) *acnt = 0;
   }
   // Before the first chunk that touches slots >= n: the arrivals are in the image, and the slots
   // between the last particle and the end of its chunk hold a harmless particle (at rest, no
