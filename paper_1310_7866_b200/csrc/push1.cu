@@ -694,7 +694,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     }
   } else if (d3) {
     const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
-    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 4, true);
+    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 5, true);
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
