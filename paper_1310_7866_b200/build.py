@@ -20,11 +20,12 @@ LIB = os.path.join(_HERE, "libpsc_b200.so")
 SOURCES = ["api.cu", "fields.cu", "sort.cu", "push1.cu", "push2.cu", "marder.cu"]
 HEADERS = ["psc_internal.cuh", "push_common.cuh", "store.cuh"]
 
-NVCC_FLAGS = [
+COMMON = [
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-lineinfo", "-O3", "-std=c++17", "--extended-lambda",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "4",
+    "-lineinfo", "-O3", "-std=c++17", "--extended-lambda", "-Xcompiler", "-fPIC",
 ]
+# sort.cu launches kernels from the device (the re-layout gate): relocatable device code + device link
+RDC_SOURCES = ["sort.cu"]
 
 
 def _nvcc() -> str:
@@ -46,11 +47,33 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile if the library is missing or older than its sources.  Returns its path."""
     if not force and not _stale():
         return LIB
-    tmp = LIB + ".%d.tmp" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
-        ["-I", INCLUDE, "-I", CSRC, "-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
-    subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
+    from concurrent.futures import ThreadPoolExecutor
+
+    nvcc = _nvcc()
+    bdir = os.path.join(_HERE, "build", "obj.%d" % os.getpid())
+    os.makedirs(bdir, exist_ok=True)
+    inc = ["-I", INCLUDE, "-I", CSRC]
+    vflags = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(f):
+        obj = os.path.join(bdir, f.replace(".cu", ".o"))
+        mode = ["-dc"] if f in RDC_SOURCES else ["-c"]
+        subprocess.check_call([nvcc] + COMMON + vflags + mode + inc + ["-o", obj, os.path.join(CSRC, f)])
+        return obj
+
+    try:
+        with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+            objs = list(ex.map(compile_one, SOURCES))
+        rdc_objs = [o for o, f in zip(objs, SOURCES) if f in RDC_SOURCES]
+        dlink = os.path.join(bdir, "dlink.o")
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fPIC",
+                               "-dlink", "-o", dlink] + rdc_objs + ["-lcudadevrt"])
+        tmp = LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
+                               "-o", tmp] + objs + [dlink, "-lcudadevrt"])
+        os.replace(tmp, LIB)
+    finally:
+        shutil.rmtree(bdir, ignore_errors=True)
     return LIB
 
 

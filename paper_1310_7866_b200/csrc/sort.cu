@@ -899,24 +899,88 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
 }
 
 // in the steady state nothing is sorted.  Only if the last push spilled
-// (device word PSC_DW_SPILL != 0) the store is flattened and laid out again; the launches below
-// return immediately otherwise.
+// (device word PSC_DW_SPILL != 0) the store is flattened and laid out again.  Whether that is
+// needed is known on the device only, so the step launches ONE single-thread kernel that looks at
+// the word and, if it is set, launches the chain itself (CUDA dynamic parallelism, tail launches:
+// they run in order after the launcher and before the next kernel of the stream).
+namespace {
+
+struct RelayoutArgs {
+  GridDesc gd;
+  Cols cur, tmp;         // the store's column set; the other one (dense scratch)
+  Exchange xin, x0, x1;  // the exchange holding the last push's records; both, for the reset
+  Spill spill;
+  int32_t *key, *perm, *offs_dense, *base, *cnt, *cursor, *tot, *doffs;
+  uint8_t *bigcell;
+  long long *pack, *packloc, *scan_tmp;
+  uint32_t *dw;
+  int *np_dev;
+  long long capacity;
+  int g_cells, g_cells8, g_warpcells, g_part, g_spill, g_reset, sblocks;
+};
+
+template <bool D3>
+__device__ void relayout_chain(const RelayoutArgs &a) {
+  const int nk = a.gd.nkeys, T = SORT_THREADS;
+  const cudaStream_t ts = cudaStreamTailLaunch;
+  const uint32_t *nc = nullptr;
+  constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;
+  // flatten: residents + exchange records + spill list -> tmp (dense), keys -> key
+  k_tot<<<a.g_cells, T, 0, ts>>>(nk, XW, a.gd.nd, a.cnt, a.xin.mask, a.tot, nc);
+  k_scan_local<int><<<a.sblocks, T, 0, ts>>>(nk, a.tot, a.doffs, (int *)a.scan_tmp, nc);
+  k_scan_tmp<int><<<1, 1024, 0, ts>>>(a.sblocks, (int *)a.scan_tmp, nc);
+  k_scan_add<<<a.sblocks, T, 0, ts>>>(nk, a.doffs, nullptr, (const int *)a.scan_tmp, a.sblocks, nc);
+  k_gather<D3, false><<<a.g_warpcells, T, 0, ts>>>(a.gd, a.cur, a.base, a.cnt, a.xin, a.doffs, a.tmp, a.key, nc);
+  k_gather_spill<D3, false><<<a.g_spill, T, 0, ts>>>(a.gd, a.spill, a.doffs, a.tmp, a.key, a.np_dev, nc);
+  // count, lay out, scatter back
+  k_zero<<<a.g_cells, T, 0, ts>>>(nk + 1, a.cursor, nc);
+  k_hist<<<a.g_part, T, 0, ts>>>(a.np_dev, nk, a.key, a.cursor, a.dw + PSC_DW_FLAGS, nc);
+  k_layout<<<a.g_cells, T, 0, ts>>>(nk, a.cursor, a.pack, a.cnt, a.dw, nc);
+  k_scan_local<long long><<<a.sblocks, T, 0, ts>>>(nk, a.pack, a.packloc, a.scan_tmp, nc);
+  k_scan_tmp<long long><<<1, 1024, 0, ts>>>(a.sblocks, a.scan_tmp, nc);
+  k_scan_add2<<<a.sblocks, T, 0, ts>>>(nk, a.packloc, a.base, a.offs_dense, a.cursor, a.scan_tmp, a.sblocks, nc);
+  k_scatter<<<a.g_part, T, 0, ts>>>(a.np_dev, a.key, a.cursor, a.perm, nc);
+  k_reorder<false><<<a.g_part, T, 0, ts>>>(a.gd, a.np_dev, a.perm, a.key, a.offs_dense, a.base, a.tmp, a.cur, nc);
+  k_store_reset<<<a.g_reset, T, 0, ts>>>(nk, XW, a.x0.mask, a.x1.mask, a.bigcell, a.base, a.dw, a.capacity, nc);
+  k_relayout_done<<<1, 32, 0, ts>>>(a.dw);
+}
+
+__global__ void k_relayout_gate(RelayoutArgs a) {
+  if (threadIdx.x != 0 || a.dw[PSC_DW_SPILL] == 0) return;
+  if (a.gd.n[0] > 1) relayout_chain<true>(a);
+  else relayout_chain<false>(a);
+}
+
+}  // namespace
+
 int psc_store_relayout_if_spilled(psc_ctx *c, cudaStream_t s) {
   const int nk = c->gd.nkeys;
-  const uint32_t *cond = c->d_flags + PSC_DW_SPILL;
-  int *np_dev = c->key + c->np;
-  const Cols &tmp = c->cols[c->cur ^ 1];
-  const Cols &dst = c->cols[c->cur];
-  int rc = gather_store(c, tmp, c->key, false, np_dev, s, cond);
-  if (rc) return rc;
-  k_zero<<<grid_for(c, nk, SORT_THREADS), SORT_THREADS, 0, s>>>(nk + 1, c->cursor, cond);
-  PSC_LAUNCH_CHECK(c);
-  k_hist<<<grid_for(c, c->np, SORT_THREADS), SORT_THREADS, 0, s>>>(np_dev, nk, c->key, c->cursor,
-                                                                  c->d_flags + PSC_DW_FLAGS, cond);
-  PSC_LAUNCH_CHECK(c);
-  rc = sort_core(c, tmp, dst, false, false, np_dev, s, cond);
-  if (rc) return rc;
-  k_relayout_done<<<1, 32, 0, s>>>(c->d_flags);
+  RelayoutArgs a;
+  a.gd = c->gd;
+  a.cur = c->cols[c->cur];
+  a.tmp = c->cols[c->cur ^ 1];
+  a.xin = c->xch[c->xcur];
+  a.x0 = c->xch[0];
+  a.x1 = c->xch[1];
+  a.spill = c->spill;
+  if (!a.cur.id) {
+    a.xin.id = nullptr;
+    a.spill.id = nullptr;
+  }
+  a.key = c->key; a.perm = c->perm; a.offs_dense = c->offs_dense; a.base = c->base; a.cnt = c->cnt;
+  a.cursor = c->cursor; a.tot = c->tot; a.doffs = c->doffs; a.bigcell = c->bigcell;
+  a.pack = c->pack; a.packloc = c->packloc; a.scan_tmp = c->scan_tmp;
+  a.dw = c->d_flags;
+  a.np_dev = c->key + c->np;
+  a.capacity = (long long)c->capacity;
+  a.g_cells = grid_for(c, nk, SORT_THREADS);
+  a.g_warpcells = grid_for(c, nk, SORT_THREADS / 32);
+  a.g_part = grid_for(c, c->np, SORT_THREADS);
+  a.g_spill = grid_for(c, c->spill.cap, SORT_THREADS);
+  a.g_reset = grid_for(c, (int64_t)nk * 16, SORT_THREADS);
+  a.g_cells8 = 0;
+  a.sblocks = (int)cdiv64(nk, SCAN_TILE);
+  k_relayout_gate<<<1, 32, 0, s>>>(a);
   PSC_LAUNCH_CHECK(c);
   c->have_sort_result = 0;
   return PSC_OK;
