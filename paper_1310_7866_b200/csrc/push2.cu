@@ -220,10 +220,16 @@ __global__ void __launch_bounds__(PUSH2_THREADS, 2)
 k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
         float *__restrict__ J, int wstride) {
   extern __shared__ __align__(128) unsigned char smraw[];
-  if (BIG && !sd.bigflag[blockIdx.x]) return;
+  // the image launch has one block per tile; the BIG launch a few blocks that walk the flagged tiles
+#pragma unroll 1
+  for (int tile = blockIdx.x;; tile += gridDim.x) {
+  if (BIG) {
+    if (tile >= gd.ntiles) break;
+    if (!sd.bigflag[tile]) continue;
+  }
   using Walker = CellWalker<D3, XC, BIG>;
   Geom2<D3, CBS> tg;
-  tg.init(gd, blockIdx.x);
+  tg.init(gd, tile);
   const int lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   // (broadcast from lane 0: lets the compiler keep everything derived from the warp index uniform)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -237,7 +243,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   wk.init(smraw + (size_t)warp * wstride, sd, lane, sNbT);
   if (threadIdx.x < 27) {  // periodic neighbour tiles (the single-GPU particle exchange)
     const int t = threadIdx.x;
-    const int b0 = blockIdx.x % gd.nb[0], br = blockIdx.x / gd.nb[0];
+    const int b0 = tile % gd.nb[0], br = tile / gd.nb[0];
     const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
     const int n0 = wrap_cell(b0 + t % 3 - 1, gd.nb[0]), n1 = wrap_cell(b1 + (t / 3) % 3 - 1, gd.nb[1]),
               n2 = wrap_cell(b2 + t / 9 - 1, gd.nb[2]);
@@ -245,7 +251,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
-  const int kbase = blockIdx.x * tg.cpb;
+  const int kbase = tile * tg.cpb;
   for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
     sBase[i] = sd.base[kbase + i];
     if (i < tg.cpb) sCnt[i] = sd.cnt[kbase + i];
@@ -525,7 +531,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
   const int any_left = __syncthreads_or(left_out ? 1 : 0);
-  if (!BIG && threadIdx.x == 0) sd.bigflag[blockIdx.x] = any_left;
+  if (!BIG && threadIdx.x == 0) sd.bigflag[tile] = any_left;
 
   // ---- flush the J tile to global J -----------------------------------------------------------
   for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) {
@@ -537,6 +543,9 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int gx = D3 ? tg.o[0] + tx - 1 + gd.g[0] : 0;
     const int gy = tg.o[1] + ty - 1 + gd.g[1], gz = tg.o[2] + tz - 1 + gd.g[2];
     atomicAdd(&J[c * gd.comp + (gz * gd.ext[1] + gy) * gd.ext[0] + gx], v);
+  }
+  if (!BIG) break;
+  __syncthreads();  // the next tile reuses the shared memory
   }
 }
 
@@ -561,12 +570,13 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   const size_t smem_img = (size_t)(threads / 32) * ws_img + tile_bytes;
   const size_t smem_big = (size_t)(threads / 32) * ws_big + tile_bytes;
   if (smem_img > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  const int big_grid = gd.ntiles < 2 * c->sm_count ? gd.ntiles : 2 * c->sm_count;
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH2_(D3_, CBS_, XC_, BIG_, SMEM_, WS_)                                         \
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, CBS_, XC_, BIG_, false>,                     \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push2<D3_, CBS_, XC_, BIG_, false><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push2<D3_, CBS_, XC_, BIG_, false><<<(BIG_) ? big_grid : gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the alternating-order scheme runs the general instantiation (run-time tile, optional columns)
@@ -574,7 +584,7 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s) {
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push2<D3_, 0, true, BIG_, true>,                        \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push2<D3_, 0, true, BIG_, true><<<gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push2<D3_, 0, true, BIG_, true><<<(BIG_) ? big_grid : gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
 #define PSC_LAUNCH_PUSH2(D3_, CBS_)                                       \
