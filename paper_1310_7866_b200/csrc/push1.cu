@@ -38,10 +38,10 @@
 
 namespace {
 
-constexpr int QCAP = 64;   // per-warp queue of trajectories that leave their cell
+constexpr int QCAP = 32;   // per-warp queue of trajectories that leave their cell (drained 24-32 at a time)
 // rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 endx (2-d: v_x),
 // 5 endy, 6 endz, 7 qw
-constexpr int QROWS2 = 8, QROWS3 = 8;
+constexpr int QROWS2 = 7, QROWS3 = 8;
 
 
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
@@ -287,9 +287,9 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ J, const TG &tg,
   if (lane < n) {
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
-    const float ax = q[1 * QCAP + e], ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
+    const float ax = D3 ? q[1 * QCAP + e] : 0.f, ay = q[2 * QCAP + e], az = q[3 * QCAP + e];
     const float ex = q[4 * QCAP + e], ey = q[5 * QCAP + e], ez = q[6 * QCAP + e];
-    const float qw = q[7 * QCAP + e];
+    const float qw = q[(D3 ? 7 : 1) * QCAP + e];
     const int lx = packed & 1023, ly = (packed >> 10) & 1023, lz = packed >> 20;
     // 2-d: the endx slot carries v_x: the out-of-plane current needs the velocity
     const float fx = qw * gd.cur[0], fy = qw * gd.cur[1], fz = qw * gd.cur[2];
@@ -446,6 +446,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
                     float endx, float endy, float endz, float vx, float ux, float uy, float uz, float qw,
                     int sp, float x2d, int id) {
     const unsigned cm = __ballot_sync(0xffffffffu, cross);
+    if (qcnt + __popc(cm) > QCAP) {  // no room for this batch: walk what is queued first
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
+      qcnt = 0;
+    }
     if (cross) {
       const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
       const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
@@ -464,22 +468,17 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
       const int e = qcnt + __popc(cm & lt);
       myQ[0 * QCAP + e] = __int_as_float(packed);
-      myQ[1 * QCAP + e] = ax;
+      if (D3) myQ[1 * QCAP + e] = ax;
       myQ[2 * QCAP + e] = ay;
       myQ[3 * QCAP + e] = az;
       myQ[4 * QCAP + e] = D3 ? endx : vx;
       myQ[5 * QCAP + e] = endy;
       myQ[6 * QCAP + e] = endz;
-      myQ[7 * QCAP + e] = qw;
+      myQ[(D3 ? 7 : 1) * QCAP + e] = qw;
     }
     qcnt += __popc(cm);
     __syncwarp();
-    // (the image path drains after the cell, while the next cell's run is being fetched; a cell
-    // with more than 32 leavers, and the global path, drain at once)
-    if (qcnt >= 32 && (BIG || qcnt + 32 > QCAP)) {
-      qcnt -= 32;
-      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, 32, lane);
-    }
+    // (a well-filled queue is walked after the cell, while the next cell's run is being fetched)
   };
 
   // The warp's cells: warp, warp + nwarps, ...  The header words that tell a cell's arrivals are
@@ -595,9 +594,9 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     // is requested: everything below needs no image and runs while that request is in flight.
     if (BIG) wk.end_global(sd);
     else wk.end_image(sd, next_n, next_base);
-    if (qcnt >= 32) {
-      qcnt -= 32;
-      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, 32, lane);
+    if (qcnt >= 24) {
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
+      qcnt = 0;
     }
     // the in-cell currents take one warp reduction and one shared add per J point
     if (ntot) {
@@ -651,23 +650,21 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   if (gd.bs[0] > 1000 || gd.bs[1] > 1000 || gd.bs[2] > 1000) return PSC_ERR_UNSUPPORTED;
   const StoreDesc sd = psc_store_desc(c);
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
-  constexpr int threads = 128;
   const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 24 + 27 + 2 * gd.cpb + 2) * sizeof(float);
   const size_t qbytes = (size_t)(d3 ? QROWS3 : QROWS2) * QCAP * 4;
   auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
   const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)
                                : CellWalker<false, true, false>::smem_bytes(sd.imgC, sd.ncol));
   const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.imgC, sd.ncol));
-  const size_t smem_img = (size_t)(threads / 32) * (ws_img + qbytes) + tile_bytes;
-  const size_t smem_big = (size_t)(threads / 32) * (ws_big + qbytes) + tile_bytes;
-  if (smem_img > 200 * 1024) return PSC_ERR_UNSUPPORTED;
+  auto smem_of = [&](int threads, int ws) { return (size_t)(threads / 32) * (ws + qbytes) + tile_bytes; };
+  if (smem_of(128, ws_img) > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const int big_grid = gd.ntiles < 2 * c->sm_count ? gd.ntiles : 2 * c->sm_count;
   ProfScope ps(c, PSC_PH_PUSH, s);
 #define PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, XC_, BIG_, CT_, SMEM_, WS_)                             \
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false>,        \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false><<<(BIG_) ? big_grid : gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false><<<(BIG_) ? big_grid : gd.ntiles, T_, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the alternating-order scheme runs the general instantiation (run-time tile, optional columns)
@@ -675,7 +672,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, 0, 128, B_, true, BIG_, 0, true>,            \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, 0, 128, B_, true, BIG_, 0, true><<<(BIG_) ? big_grid : gd.ntiles, threads, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, 0, 128, B_, true, BIG_, 0, true><<<(BIG_) ? big_grid : gd.ntiles, 128, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the image launch, then the launch for the cells it had to leave out (its blocks return at
@@ -684,23 +681,23 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
 #define PSC_LAUNCH_PUSH1(D3_, CBS_, T_, B_, FAST_)                                                 \
   do {                                                                                             \
     if (xc) {                                                                                      \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, true, false, 0, smem_img, ws_img);                      \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, true, true, 0, smem_big, ws_big);                        \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, true, false, 0, smem_of(T_, ws_img), ws_img);           \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, true, true, 0, smem_of(T_, ws_big), ws_big);             \
     } else {                                                                                       \
-      if (FAST_ && sd.imgC == 256) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 256, smem_img, ws_img); \
-      else if (FAST_ && sd.imgC == 192) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 192, smem_img, ws_img); \
-      else if (FAST_ && sd.imgC == 128) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 128, smem_img, ws_img); \
-      else PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 0, smem_img, ws_img);                \
-      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_big, ws_big);                       \
+      if (FAST_ && sd.imgC == 256) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 256, smem_of(T_, ws_img), ws_img); \
+      else if (FAST_ && sd.imgC == 192) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 192, smem_of(T_, ws_img), ws_img); \
+      else if (FAST_ && sd.imgC == 128) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 128, smem_of(T_, ws_img), ws_img); \
+      else PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 0, smem_of(T_, ws_img), ws_img);     \
+      PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_of(T_, ws_big), ws_big);            \
     }                                                                                              \
   } while (0)
   if (gd.gmode == PSC_SCHEME_ALTERNATING) {
     if (d3) {
-      PSC_LAUNCH_PUSH1_ALT(true, 4, false, smem_img, ws_img);
-      PSC_LAUNCH_PUSH1_ALT(true, 2, true, smem_big, ws_big);
+      PSC_LAUNCH_PUSH1_ALT(true, 4, false, smem_of(128, ws_img), ws_img);
+      PSC_LAUNCH_PUSH1_ALT(true, 2, true, smem_of(128, ws_big), ws_big);
     } else {
-      PSC_LAUNCH_PUSH1_ALT(false, 5, false, smem_img, ws_img);
-      PSC_LAUNCH_PUSH1_ALT(false, 2, true, smem_big, ws_big);
+      PSC_LAUNCH_PUSH1_ALT(false, 5, false, smem_of(128, ws_img), ws_img);
+      PSC_LAUNCH_PUSH1_ALT(false, 2, true, smem_of(128, ws_big), ws_big);
     }
   } else if (d3) {
     const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
@@ -708,7 +705,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 5, true);
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 6, true);
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5, false);
   }
 #undef PSC_LAUNCH_PUSH1

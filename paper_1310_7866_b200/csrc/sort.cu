@@ -812,7 +812,7 @@ int sort_core(psc_ctx *c, const Cols &src, const Cols &dst, bool from_abs, bool 
   k_scatter<<<pblocks, SORT_THREADS, 0, s>>>(np, c->key, c->cursor, c->perm, cond);
   PSC_LAUNCH_CHECK(c);
   if (stable) {
-    const int kblocks = (int)min((int64_t)c->sm_count * 8, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
+    const int kblocks = (int)min((int64_t)c->sm_count * 64, max((int64_t)1, cdiv64(nk, SORT_THREADS / 32)));
     k_segsort<<<kblocks, SORT_THREADS, 0, s>>>(nk, c->offs_dense, c->perm, c->big_list, c->d_flags + PSC_DW_BIG);
     PSC_LAUNCH_CHECK(c);
     if (c->np > WARP_SEG_CAP) {

@@ -122,6 +122,7 @@ struct Part {
 };
 
 constexpr int WALK_AC = 128;  // arrival-list window (entries)
+constexpr int WALK_HC = 128;  // hole-list entries kept as bytes (more holes are read off the bitmap)
 
 // Per-warp view of the store.  XC: optional columns (id, carried x of a 2-d run) may be bound.
 // BIG == false: the shared-memory image path (cells with n + arrivals <= C; others are skipped
@@ -134,14 +135,14 @@ struct CellWalker {
   static constexpr int XW = D3 ? PSC_XW3 : PSC_XW2;  // header words of an exchange row
   // bytes of per-warp shared memory for an image of C slots x ncol columns
   __host__ __device__ static constexpr int smem_bytes(int C, int ncol) {
-    return (BIG ? WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ : ncol * C * 4 + C /*holes*/) + 32 * 4 /*xrow*/ +
+    return (BIG ? WALK_AC * 2 /*arr*/ + 32 * 4 /*nbk*/ : ncol * C * 4 + WALK_HC /*holes*/) + XW * 4 /*xrow*/ +
            12 * 4 /*hbm*/ + 16 /*bar*/;
   }
   float *buf;      // [ncol][C]
-  uint8_t *holes;  // [C]: slots of the image whose particle left, ascending
+  uint8_t *holes;  // [WALK_HC]: slots of the image whose particle left, ascending (the first WALK_HC)
   uint16_t *arr;   // [WALK_AC]: arrival a -> direction lane << 8 | record index in that neighbour's row
   int *nbk;        // [32]: key of the neighbour cell a lane looks at
-  unsigned *xrow;  // [32]: per direction code, which of the cell's records so far moved that way
+  unsigned *xrow;  // [XW]: per direction code, which of the cell's records so far moved that way
   unsigned *hbm;   // [12] (9 used): bit v set <=> slot v of the image is a hole; hbm[11]: arrival counter
   int *acnt;
   uint64_t *bar;
@@ -167,16 +168,16 @@ struct CellWalker {
     lt = lanemask_lt_();
     buf = (float *)wsm;
     holes = (uint8_t *)(buf + (BIG ? 0 : ncol * C));
-    arr = (uint16_t *)(holes + (BIG ? 0 : C));  // (arr, nbk: the BIG form only)
+    arr = (uint16_t *)(holes + (BIG ? 0 : WALK_HC));  // (arr, nbk: the BIG form only)
     nbk = (int *)(arr + (BIG ? WALK_AC : 0));
     xrow = (unsigned *)(nbk + (BIG ? 32 : 0));
-    hbm = xrow + 32;
+    hbm = xrow + XW;
     bar = (uint64_t *)(hbm + 12);
     acnt = (int *)(hbm + 11);
     if (lane == 0) *acnt = 0;
     parity = 0;
     loads_armed = false;
-    xrow[lane] = 0u;
+    if (lane < XW) xrow[lane] = 0u;
     if (!BIG && lane == 0) {
       mbar_init(bar, 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -371,15 +372,31 @@ struct CellWalker {
         if (!leave) { q[0] = pn.ay; q[C] = pn.az; }
         q[2 * C] = pn.ux; q[3 * C] = pn.uy; q[4 * C] = pn.uz;
       }
-      if (leave) holes[nh + __popc(mrl & lt)] = (uint8_t)v;
+      if (leave) {
+        const int hi = nh + __popc(mrl & lt);
+        if (hi < WALK_HC) holes[hi] = (uint8_t)v;
+      }
     }
     if (lane == 0) hbm[v0 >> 5] = mrl;
     nh += __popc(mrl);
   }
 
+  // slot of the i-th hole (ascending): from the byte list, beyond it from the bitmap
+  __device__ __forceinline__ int hole_at(int i) const {
+    if (i < WALK_HC) return holes[i];
+    int acc = 0;
+    for (int w = 0; w < 8; w++) {
+      const unsigned m = hbm[w];
+      const int c = __popc(m);
+      if (i < acc + c) return w * 32 + (int)__fns(m, 0, i - acc + 1);
+      acc += c;
+    }
+    return 0;
+  }
+
   // leaver i of the hole list: its image values (OLD offsets, NEW momentum) and optional columns
   __device__ __forceinline__ void leaver(const StoreDesc &sd, int i, Part &p, float &x2d, int &id) const {
-    const int h = holes[i];
+    const int h = hole_at(i);
     load_image(h, p);
     x2d = 0.f;
     id = 0;
@@ -403,7 +420,7 @@ struct CellWalker {
         const bool valid = s < T && !((hbm[s >> 5] >> (s & 31)) & 1u);
         const unsigned mv = __ballot_sync(0xffffffffu, valid);
         if (valid) {
-          const int h = holes[done + __popc(mv & lt)];  // ascending list: its first entries are < newcnt
+          const int h = hole_at(done + __popc(mv & lt));  // ascending: the first holes are < newcnt
           for (int c = 0; c < ncol; c++) buf[c * C + h] = buf[c * C + s];
           if (h < n)
             for (int c = NDYN; c < ncol; c++) st_stream(sd.col[c] + (size_t)base + h, buf[c * C + s]);
@@ -451,7 +468,7 @@ struct CellWalker {
     if (lane == 0) sd.cnt[key] = newcnt;
     if (lane < XW) sd.xout.mask[(size_t)key * XW + lane] = xrow[lane];
     __syncwarp();
-    xrow[lane] = 0u;
+    if (lane < XW) xrow[lane] = 0u;
   }
 
   // ---- records ------------------------------------------------------------------------------------
