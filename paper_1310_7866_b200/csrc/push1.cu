@@ -38,7 +38,9 @@
 
 namespace {
 
-constexpr int QCAP = 32;   // per-warp queue of trajectories that leave their cell (drained 24-32 at a time)
+// per-warp queue of trajectories that leave their cell: 2-d (3 % leavers; shared memory decides
+// the blocks per SM) 32 entries, walked 24-32 at a time; 3-d (12 % leavers) 64, walked 32 at a time
+template <bool D3> struct QCap { static constexpr int v = D3 ? 64 : 32; };
 // rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 endx (2-d: v_x),
 // 5 endy, 6 endz, 7 qw
 constexpr int QROWS2 = 7, QROWS3 = 8;
@@ -284,6 +286,7 @@ template <bool D3, class TG>
 __device__ __forceinline__ void drain_queue(float *__restrict__ J, const TG &tg, const GridDesc &gd,
                                             int gnode0, const float *__restrict__ q,
                                             const int *__restrict__ rel, int start, int n, int lane) {
+  constexpr int QCAP = QCap<D3>::v;
   if (lane < n) {
     const int e = start + lane;
     const int packed = __float_as_int(q[0 * QCAP + e]);
@@ -343,7 +346,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   // (broadcast from lane 0: lets the compiler keep everything derived from the warp index uniform)
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   // per-warp areas first (128-byte aligned cell images), then the block's tiles and tables
-  constexpr int QROWS = D3 ? QROWS3 : QROWS2;
+  constexpr int QROWS = D3 ? QROWS3 : QROWS2, QCAP = QCap<D3>::v;
   float *myQ = (float *)(smraw + (size_t)nwarps * wstride) + warp * (QROWS * QCAP);  // [QROWS][QCAP]
   float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP);  // [6][fvol]
   float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
@@ -446,9 +449,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
                     float endx, float endy, float endz, float vx, float ux, float uy, float uz, float qw,
                     int sp, float x2d, int id) {
     const unsigned cm = __ballot_sync(0xffffffffu, cross);
-    if (qcnt + __popc(cm) > QCAP) {  // no room for this batch: walk what is queued first
-      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
-      qcnt = 0;
+    if (qcnt + __popc(cm) > QCAP) {  // no room for this batch: walk (up to 32 of) what is queued first
+      const int nd = qcnt < 32 ? qcnt : 32;
+      qcnt -= nd;
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, nd, lane);
     }
     if (cross) {
       const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
@@ -594,9 +598,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     // is requested: everything below needs no image and runs while that request is in flight.
     if (BIG) wk.end_global(sd);
     else wk.end_image(sd, next_n, next_base);
-    if (qcnt >= 24) {
-      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
-      qcnt = 0;
+    if (qcnt >= (QCAP == 32 ? 24 : 32)) {
+      const int nd = qcnt < 32 ? qcnt : 32;
+      qcnt -= nd;
+      drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, nd, lane);
     }
     // the in-cell currents take one warp reduction and one shared add per J point
     if (ntot) {
@@ -651,7 +656,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const StoreDesc sd = psc_store_desc(c);
   const bool xc = sd.icol_id >= 0 || sd.icol_x2d >= 0;
   const size_t tile_bytes = (size_t)(6 * fvol + 3 * jvol + PSC_MAX_SPECIES + 24 + 27 + 2 * gd.cpb + 2) * sizeof(float);
-  const size_t qbytes = (size_t)(d3 ? QROWS3 : QROWS2) * QCAP * 4;
+  const size_t qbytes = d3 ? (size_t)QROWS3 * QCap<true>::v * 4 : (size_t)QROWS2 * QCap<false>::v * 4;
   auto stride = [&](int wbytes) { return (wbytes + 127) / 128 * 128; };
   const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)
                                : CellWalker<false, true, false>::smem_bytes(sd.imgC, sd.ncol));
@@ -686,6 +691,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     } else {                                                                                       \
       if (FAST_ && sd.imgC == 256) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 256, smem_of(T_, ws_img), ws_img); \
       else if (FAST_ && sd.imgC == 192) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 192, smem_of(T_, ws_img), ws_img); \
+      else if (FAST_ && sd.imgC == 160) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 160, smem_of(T_, ws_img), ws_img); \
       else if (FAST_ && sd.imgC == 128) PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 128, smem_of(T_, ws_img), ws_img); \
       else PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, B_, false, false, 0, smem_of(T_, ws_img), ws_img);     \
       PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_of(T_, ws_big), ws_big);            \

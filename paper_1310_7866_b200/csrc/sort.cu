@@ -892,7 +892,7 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, s));
   PSC_CUDA_TRY(c, cudaStreamSynchronize(s));
   const int mx = (int)dw[PSC_DW_MAXCNT];
-  int C = (mx + mx / 8 + 24 + 63) / 64 * 64;  // one of 64, 128, 192, 256
+  int C = (mx + mx / 8 + 24 + 31) / 32 * 32;  // 64, 96, ..., 256
   c->bufC = C < 64 ? 64 : (C > 256 ? 256 : C);
   if ((int64_t)dw[PSC_DW_SLOTS] > c->capacity) return PSC_ERR_WORKSPACE;
   return PSC_OK;
