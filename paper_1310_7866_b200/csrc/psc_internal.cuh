@@ -88,6 +88,8 @@ struct StoreDesc {
   int imgC;        // slots of the per-warp cell image (multiple of 32, <= 256)
   int32_t *bigflag;  // [ntiles]: the image launch left a cell of this tile to the BIG launch
   uint8_t *bigcell;  // [nkeys]: ... this cell (set by the image launch, cleared by the BIG launch)
+  uint32_t *nbig;    // tiles flagged by this step's image launch (the BIG launch returns at once if 0)
+  uint32_t *nbig_next;  // the other step parity's counter: zeroed by this step's BIG launch
   uint32_t *flags;
 };
 
@@ -124,6 +126,7 @@ enum {
   PSC_DW_MAXCNT = 3,   // largest cell count seen by the last layout
   PSC_DW_SLOTS = 4,    // slots used by the last layout
   PSC_DW_RELAYOUTS = 5,  // number of re-layouts performed
+  PSC_DW_NBIG = 6,     // [2]: tiles with a cell left to the BIG launch, by step parity
   PSC_DW_COUNT = 16
 };
 

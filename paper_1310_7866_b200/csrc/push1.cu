@@ -333,6 +333,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   extern __shared__ __align__(128) unsigned char smraw[];
   // the image launch has one block per tile; the BIG launch a few blocks that walk the flagged tiles
 #pragma unroll 1
+  if (BIG) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) *sd.nbig_next = 0;
+    if (*sd.nbig == 0) return;  // the image launch left nothing out
+  }
   for (int tile = blockIdx.x;; tile += gridDim.x) {
   if (BIG) {
     if (tile >= gd.ntiles) break;
@@ -621,7 +625,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
   const int any_left = __syncthreads_or(left_out ? 1 : 0);
-  if (!BIG && threadIdx.x == 0) sd.bigflag[tile] = any_left;
+  if (!BIG && threadIdx.x == 0) {
+    sd.bigflag[tile] = any_left;
+    if (any_left) atomicAdd(sd.nbig, 1u);
+  }
 
   // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) {

@@ -724,6 +724,8 @@ StoreDesc psc_store_desc(const psc_ctx *c) {
   sd.imgC = c->bufC;
   sd.bigflag = c->bigflag;
   sd.bigcell = c->bigcell;
+  sd.nbig = c->d_flags + PSC_DW_NBIG + c->xcur;
+  sd.nbig_next = c->d_flags + PSC_DW_NBIG + (c->xcur ^ 1);
   sd.flags = c->d_flags + PSC_DW_FLAGS;
   return sd;
 }
