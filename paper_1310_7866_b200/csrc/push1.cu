@@ -36,11 +36,14 @@
 // the time average of v_x S_y S_z over the segment (A12).
 #include "store.cuh"
 
+#ifndef PSC_MINB2D
+#define PSC_MINB2D 6  // blocks per SM of the default 2-d kernel
+#endif
 namespace {
 
 // per-warp queue of trajectories that leave their cell: 2-d (3 % leavers; shared memory decides
-// the blocks per SM) 32 entries, walked 24-32 at a time; 3-d (12 % leavers) 64, walked 32 at a time
-template <bool D3> struct QCap { static constexpr int v = D3 ? 64 : 32; };
+// the blocks per SM) 24 entries, walked 16-24 at a time; 3-d (12 % leavers) 64, walked 32 at a time
+template <bool D3> struct QCap { static constexpr int v = D3 ? 64 : 24; };
 // rows of a queue entry: 0 packed cell (lx | ly << 10 | lz << 20), 1 ax, 2 ay, 3 az, 4 endx (2-d: v_x),
 // 5 endy, 6 endz, 7 qw
 constexpr int QROWS2 = 7, QROWS3 = 8;
@@ -303,6 +306,105 @@ __device__ __forceinline__ void drain_queue(float *__restrict__ J, const TG &tg,
   __syncwarp();
 }
 
+// ---- per-cell gather tables ------------------------------------------------------------------
+// Inside one cell the b1-weighted value of a field component (Eq. 11) is a
+// multilinear polynomial of the in-cell offsets a: along a direction in which the component sits
+// on the nodes the two stencil points are l, l+1 with weight a; along a direction in which it is
+// half-staggered they are l-1, l with weight a + 1/2 (a < 1/2) or l, l+1 with weight a - 1/2
+// (a >= 1/2) -- two PIECES.  So a component has 1, 2 or 4 pieces per cell (2-d: 13 in all, 3-d:
+// 18), each with 4 (2-d) / 8 (3-d) polynomial coefficients.  The warp that owns a cell computes
+// them once per cell (a lane per piece, from the block's field tile) into a small per-warp table;
+// a particle then needs one (two) 16-byte shared loads and 3 (7) FMAs per component instead of
+// 4 (8) loads and 5 (14) operations.
+template <bool D3> struct GTab {
+  static constexpr int NP = D3 ? 18 : 13;  // pieces
+  static constexpr int W = D3 ? 8 : 4;     // coefficients per piece
+  static constexpr int FLOATS = NP * W;
+};
+
+// What lane `l` (a piece) reads and how it shifts: off = offset of its base stencil point from
+// the cell's node in the field tile, sg* = weight shift (0 node-centred, +1/2 lower piece, -1/2
+// upper piece).  Piece order: Ex[hx] Ey[hy] Ez[hz] Bx[hy + 2 hz] By[hx + 2 hz] Bz[hx + 2 hy]
+// (2-d: no hx: Ex, Ey[hy], Ez[hz], Bx[hy + 2 hz], By[hz], Bz[hy]).
+template <bool D3>
+__device__ __forceinline__ void piece_desc(int l, int fs1, int fs2, int fvol, int &off, float &sgx,
+                                           float &sgy, float &sgz) {
+  int comp, hx = -1, hy = -1, hz = -1;  // -1: node-centred along that direction
+  if (D3) {
+    if (l < 2) { comp = 0; hx = l; }
+    else if (l < 4) { comp = 1; hy = l - 2; }
+    else if (l < 6) { comp = 2; hz = l - 4; }
+    else if (l < 10) { comp = 3; hy = (l - 6) & 1; hz = (l - 6) >> 1; }
+    else if (l < 14) { comp = 4; hx = (l - 10) & 1; hz = (l - 10) >> 1; }
+    else { comp = 5; hx = (l - 14) & 1; hy = ((l - 14) >> 1) & 1; }
+  } else {
+    if (l < 1) { comp = 0; }
+    else if (l < 3) { comp = 1; hy = l - 1; }
+    else if (l < 5) { comp = 2; hz = l - 3; }
+    else if (l < 9) { comp = 3; hy = (l - 5) & 1; hz = (l - 5) >> 1; }
+    else if (l < 11) { comp = 4; hz = l - 9; }
+    else { comp = 5; hy = (l - 11) & 1; }
+  }
+  off = comp * fvol;
+  sgx = sgy = sgz = 0.f;
+  if (hx >= 0) { off += hx - 1; sgx = 0.5f - (float)hx; }
+  if (hy >= 0) { off += (hy - 1) * fs1; sgy = 0.5f - (float)hy; }
+  if (hz >= 0) { off += (hz - 1) * fs2; sgz = 0.5f - (float)hz; }
+}
+
+// one lane = one piece: the polynomial coefficients of its component around base point q
+// 2-d: f = c0 + ay c1 + az c2 + ay az c3;  3-d: coefficient of ax^i ay^j az^k at [i + 2 j + 4 k]
+template <bool D3>
+__device__ __forceinline__ void piece_build(float *__restrict__ t, const float *__restrict__ q, int fs1,
+                                            int fs2, float sgx, float sgy, float sgz) {
+  if (D3) {
+    float c[8];
+#pragma unroll
+    for (int k = 0; k < 2; k++)
+#pragma unroll
+      for (int j = 0; j < 2; j++) {
+        const float v0 = q[k * fs2 + j * fs1], v1 = q[k * fs2 + j * fs1 + 1];
+        const float d = v1 - v0;
+        c[4 * k + 2 * j] = fmaf(sgx, d, v0);
+        c[4 * k + 2 * j + 1] = d;
+      }
+#pragma unroll
+    for (int k = 0; k < 2; k++)
+#pragma unroll
+      for (int i = 0; i < 2; i++) {
+        const float d = c[4 * k + 2 + i] - c[4 * k + i];
+        c[4 * k + i] = fmaf(sgy, d, c[4 * k + i]);
+        c[4 * k + 2 + i] = d;
+      }
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+      const float d = c[4 + i] - c[i];
+      c[i] = fmaf(sgz, d, c[i]);
+      c[4 + i] = d;
+    }
+    reinterpret_cast<float4 *>(t)[0] = make_float4(c[0], c[1], c[2], c[3]);
+    reinterpret_cast<float4 *>(t)[1] = make_float4(c[4], c[5], c[6], c[7]);
+  } else {
+    const float v00 = q[0], v10 = q[1], v01 = q[fs2], v11 = q[fs2 + 1];
+    const float d1 = v10 - v00, d2 = v01 - v00, d3 = (v11 - v10) - d2;
+    const float c2 = fmaf(sgy, d3, d2);
+    *reinterpret_cast<float4 *>(t) = make_float4(fmaf(sgz, c2, fmaf(sgy, d1, v00)), fmaf(sgz, d3, d1), c2, d3);
+  }
+}
+
+template <bool D3>
+__device__ __forceinline__ float piece_eval(const float *__restrict__ t, float ax, float ay, float az) {
+  if (D3) {
+    const float4 a = reinterpret_cast<const float4 *>(t)[0], b = reinterpret_cast<const float4 *>(t)[1];
+    const float lo = fmaf(ay, fmaf(ax, a.w, a.z), fmaf(ax, a.y, a.x));
+    const float hi = fmaf(ay, fmaf(ax, b.w, b.z), fmaf(ax, b.y, b.x));
+    return fmaf(az, hi, lo);
+  } else {
+    const float4 a = *reinterpret_cast<const float4 *>(t);
+    return fmaf(az, fmaf(ay, a.w, a.z), fmaf(ay, a.y, a.x));
+  }
+}
+
 // b1 gather of one component (Eq. 11; each component from its own staggered
 // points).  q points at the first stencil point, f* are the weights of the second point.
 template <bool D3>
@@ -352,7 +454,9 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   // per-warp areas first (128-byte aligned cell images), then the block's tiles and tables
   constexpr int QROWS = D3 ? QROWS3 : QROWS2, QCAP = QCap<D3>::v;
   float *myQ = (float *)(smraw + (size_t)nwarps * wstride) + warp * (QROWS * QCAP);  // [QROWS][QCAP]
-  float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP);  // [6][fvol]
+  // [NP][W] per warp: the gather table of the warp's current cell (16-byte aligned)
+  float *myT = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP) + warp * GTab<D3>::FLOATS;
+  float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP + GTab<D3>::FLOATS);  // [6][fvol]
   float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
   float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
   int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [24]: J points of vb_values (tile, global)
@@ -399,21 +503,11 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   __syncthreads();
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
-  uint32_t bad = 0;
   const unsigned lt = lanemask_lt_();
   const float cdx = D3 ? gd.dt_dx[0] : 0.f, cdy = gd.dt_dx[1], cdz = gd.dt_dx[2];
 
-  // which reduced value this lane ends up holding, and the J point (relative to the cell's
-  // (lx+1, ly+1, lz+1) tile node) it belongs to
-  int my_off;
-  bool writer;
-  if (D3) {
-    my_off = sRel[red12_index(lane)];
-    writer = (lane & 1) == 0 && !((lane & 2) && (lane & 4));
-  } else {
-    my_off = sRel[(lane >> 2) & 7];
-    writer = (lane & 3) == 0;
-  }
+  // (which reduced value a lane ends up holding after the per-cell reduction, and the J point it
+  // belongs to, is recomputed per cell: lane constants kept across the particle loop cost registers)
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
   // global index of the node of the tile's first cell
   const int gnode0 = ((tg.o[2] + gd.g[2]) * gd.ext[1] + (tg.o[1] + gd.g[1])) * gd.ext[0] + (D3 ? tg.o[0] + gd.g[0] : 0);
@@ -424,7 +518,38 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   // a + 1/2) or l, l+1 (weight a - 1/2)), Boris (Eq. 27-28).  ALT: the alternating-order scheme
   // (A29): along a half-staggered direction the weight is b0, i.e. the
   // cell's own point l with weight 1.
+  // this lane's piece of the gather table (lanes >= NP: none)
+  // packed in one register: offset << 6 | twice the three weight shifts as 2-bit signed fields
+  int pc_desc;
+  {
+    int off;
+    float sx_, sy_, sz_;
+    piece_desc<D3>(lane < GTab<D3>::NP ? lane : 0, fs1, fs2, fvol, off, sx_, sy_, sz_);
+    pc_desc = (off << 6) | (((int)(2.f * sx_) & 3) << 4) | (((int)(2.f * sy_) & 3) << 2) | ((int)(2.f * sz_) & 3);
+  }
   auto kick = [&](const float *cF, float ax, float ay, float az, float &ux, float &uy, float &uz, int sp) {
+    if (!ALT) {  // the cell's gather table (built at the start of the cell)
+      constexpr int W = GTab<D3>::W;
+      const int iy = ay >= 0.5f ? W : 0, iz = az >= 0.5f ? W : 0, ix = (D3 && ax >= 0.5f) ? W : 0;
+      float ex, ey, ez, bx, by, bz;
+      if (D3) {
+        ex = piece_eval<D3>(myT + ix, ax, ay, az);
+        ey = piece_eval<D3>(myT + 2 * W + iy, ax, ay, az);
+        ez = piece_eval<D3>(myT + 4 * W + iz, ax, ay, az);
+        bx = piece_eval<D3>(myT + 6 * W + iy + 2 * iz, ax, ay, az);
+        by = piece_eval<D3>(myT + 10 * W + ix + 2 * iz, ax, ay, az);
+        bz = piece_eval<D3>(myT + 14 * W + ix + 2 * iy, ax, ay, az);
+      } else {
+        ex = piece_eval<D3>(myT, ax, ay, az);
+        ey = piece_eval<D3>(myT + W + iy, ax, ay, az);
+        ez = piece_eval<D3>(myT + 3 * W + iz, ax, ay, az);
+        bx = piece_eval<D3>(myT + 5 * W + iy + 2 * iz, ax, ay, az);
+        by = piece_eval<D3>(myT + 9 * W + iz, ax, ay, az);
+        bz = piece_eval<D3>(myT + 11 * W + iy, ax, ay, az);
+      }
+      boris_push(ux, uy, uz, ex, ey, ez, bx, by, bz, sH[sp & (PSC_MAX_SPECIES - 1)]);
+      return;
+    }
     const bool hy = ALT || ay >= 0.5f, hz = ALT || az >= 0.5f, hx = D3 && (ALT || ax >= 0.5f);
     const float gy = ALT ? 0.f : (hy ? ay - 0.5f : ay + 0.5f), gz = ALT ? 0.f : (hz ? az - 0.5f : az + 0.5f);
     const float gx = ALT ? 0.f : (hx ? ax - 0.5f : ax + 0.5f);
@@ -475,16 +600,22 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
                         wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
       wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
       const int e = qcnt + __popc(cm & lt);
-      myQ[0 * QCAP + e] = __int_as_float(packed);
-      if (D3) myQ[1 * QCAP + e] = ax;
-      myQ[2 * QCAP + e] = ay;
-      myQ[3 * QCAP + e] = az;
-      myQ[4 * QCAP + e] = D3 ? endx : vx;
-      myQ[5 * QCAP + e] = endy;
-      myQ[6 * QCAP + e] = endz;
-      myQ[(D3 ? 7 : 1) * QCAP + e] = qw;
+      if (QCAP >= 32 || e < QCAP) {
+        myQ[0 * QCAP + e] = __int_as_float(packed);
+        if (D3) myQ[1 * QCAP + e] = ax;
+        myQ[2 * QCAP + e] = ay;
+        myQ[3 * QCAP + e] = az;
+        myQ[4 * QCAP + e] = D3 ? endx : vx;
+        myQ[5 * QCAP + e] = endy;
+        myQ[6 * QCAP + e] = endz;
+        myQ[(D3 ? 7 : 1) * QCAP + e] = qw;
+      } else {  // a batch of more than QCAP leavers (the BIG form only): the rest is walked at once
+        vb_walk<D3, decltype(tg)>(J, gd, gnode0, lx, ly, lz, ax, ay, az, endx, endy, endz, qw * gd.cur[0],
+                                  qw * gd.cur[1], qw * gd.cur[2], qw * gd.inv_dV * vx, sRel + NV);
+      }
     }
     qcnt += __popc(cm);
+    if (QCAP < 32 && qcnt > QCAP) qcnt = QCAP;
     __syncwarp();
     // (a well-filled queue is walked after the cell, while the next cell's run is being fetched)
   };
@@ -502,6 +633,21 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const unsigned mask = mask_next;
     const int src = src_next;
     mask_next = wk.fetch_mask(sd, tg, nx, src_next);
+    const int lx = ci % tg.bs[0];
+    const int lt_ = ci / tg.bs[0];
+    const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
+    // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
+    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
+                               : (lz + 1) * tg.fe[1] + (ly + 1));
+    if (!ALT) {  // the cell's gather table, while its resident run is still on its way
+      if (lane < GTab<D3>::NP) {
+        auto half = [](int two_bits_at_top) { return 0.5f * (float)(two_bits_at_top >> 30); };
+        const int pd = keep_in_loop(pc_desc);
+        piece_build<D3>(myT + lane * GTab<D3>::W, cF + (pd >> 6), fs1, fs2, half(pd << 26), half(pd << 28),
+                        half(pd << 30));
+      }
+      __syncwarp();
+    }
     wk.begin_cell(kbase + ci, sCnt[ci], sBase[ci], sBase[ci + 1] - sBase[ci], mask, src);
     // Whose cell is it?  The image launch decides (its count is the one before the push) and
     // leaves a note; the BIG launch takes exactly the noted cells.
@@ -515,14 +661,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       wk.skip_cell(sd, next_n, next_base);
       continue;
     }
-    const int lx = ci % tg.bs[0];
-    const int lt_ = ci / tg.bs[0];
-    const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
     const int ntot = wk.n + wk.na;
     const int packed = lx | (ly << 10) | (lz << 20);
-    // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
-    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
-                               : (lz + 1) * tg.fe[1] + (ly + 1));
     float acc[NV];
 #pragma unroll
     for (int i = 0; i < NV; i++) acc[i] = 0.f;
@@ -531,8 +671,9 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       // ---- image path: every particle of the cell, arrivals included, is a slot of the image ----
       if (wk.na) wk.stage_arrivals(sd);
       bool landed = false;
+      int v0 = 0;
 #pragma unroll 1
-      for (int v0 = 0; v0 < ntot; v0 += 32) {
+      for (; v0 < ntot; v0 += 32) {
         if (!landed && v0 + 32 > wk.n) {
           wk.arrivals_landed();
           landed = true;
@@ -555,8 +696,9 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       // ---- the cell's leavers, 32 at a time: records + the currents of their trajectories ------
       const int nl = wk.nh;
 #pragma unroll 1
-      for (int i0 = 0; i0 < nl; i0 += 32) {
-        const bool al = i0 + lane < nl;
+      constexpr int LB = QCAP < 32 ? QCAP : 32;  // a batch of leavers fits the empty queue
+      for (int i0 = 0; i0 < nl; i0 += LB) {
+        const bool al = lane < LB && i0 + lane < nl;
         Part q;
         float qx2d = 0.f;
         int qid = 0;
@@ -602,7 +744,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     // is requested: everything below needs no image and runs while that request is in flight.
     if (BIG) wk.end_global(sd);
     else wk.end_image(sd, next_n, next_base);
-    if (qcnt >= (QCAP == 32 ? 24 : 32)) {
+    if (qcnt >= (QCAP < 32 ? 16 : 32)) {
       const int nd = qcnt < 32 ? qcnt : 32;
       qcnt -= nd;
       drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, qcnt, nd, lane);
@@ -613,8 +755,11 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       moments_to_values<D3>(acc);
       if (D3) r = warp_reduce12(reinterpret_cast<const float(&)[12]>(acc), lane);
       else r = warp_reduce8(reinterpret_cast<const float(&)[8]>(acc), lane);
-      if (!(fabsf(r) < 3.0e38f)) bad |= PSC_F_NAN;  // a non-finite momentum poisons the cell's sums
+      if (!(fabsf(r) < 3.0e38f)) atomicOr(sd.flags, PSC_F_NAN);  // a non-finite momentum poisons the cell's sums
+      const int ln = keep_in_loop(lane);
+      const bool writer = D3 ? ((ln & 1) == 0 && !((ln & 2) && (ln & 4))) : ((ln & 3) == 0);
       if (writer) {
+        const int my_off = sRel[D3 ? red12_index(ln) : ((ln >> 2) & 7)];
         const int node = D3 ? ((lz + 1) * tg.je[1] + (ly + 1)) * tg.je[0] + (lx + 1)
                             : (lz + 1) * tg.je[1] + (ly + 1);
         atomicAdd(&sJ[node + my_off], r);
@@ -623,7 +768,6 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   if (qcnt) drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
   wk.finish();
-  if (bad) atomicOr(sd.flags, bad);
   const int any_left = __syncthreads_or(left_out ? 1 : 0);
   if (!BIG && threadIdx.x == 0) {
     sd.bigflag[tile] = any_left;
@@ -668,7 +812,8 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   const int ws_img = stride(d3 ? CellWalker<true, true, false>::smem_bytes(sd.imgC, sd.ncol)
                                : CellWalker<false, true, false>::smem_bytes(sd.imgC, sd.ncol));
   const int ws_big = stride(CellWalker<true, true, true>::smem_bytes(sd.imgC, sd.ncol));
-  auto smem_of = [&](int threads, int ws) { return (size_t)(threads / 32) * (ws + qbytes) + tile_bytes; };
+  const size_t tbytes = (size_t)(d3 ? GTab<true>::FLOATS : GTab<false>::FLOATS) * 4;  // gather table per warp
+  auto smem_of = [&](int threads, int ws) { return (size_t)(threads / 32) * (ws + qbytes + tbytes) + tile_bytes; };
   if (smem_of(128, ws_img) > 200 * 1024) return PSC_ERR_UNSUPPORTED;
   const int big_grid = gd.ntiles < 2 * c->sm_count ? gd.ntiles : 2 * c->sm_count;
   ProfScope ps(c, PSC_PH_PUSH, s);
@@ -718,7 +863,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, 6, true);
+    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, PSC_MINB2D, true);
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5, false);
   }
 #undef PSC_LAUNCH_PUSH1

@@ -60,3 +60,11 @@ __device__ __forceinline__ unsigned lanemask_lt_() {
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
 }
+
+// Returns v, but opaque to the optimiser: what is computed from the result inside a loop stays
+// inside the loop.  (Cheap per-cell recomputation of lane constants is deliberate: hoisted out of
+// the particle loop they cost registers the loop needs, and end up spilled to local memory.)
+__device__ __forceinline__ int keep_in_loop(int v) {
+  asm volatile("" : "+r"(v));
+  return v;
+}

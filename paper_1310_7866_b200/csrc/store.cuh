@@ -149,7 +149,6 @@ struct CellWalker {
   const int *nbt;  // [27] (block-wide): first key of the tile at tile offset (tx, ty, tz) in {-1,0,1}^3
   int Crt, ncol, lane;
 #define C (CT ? CT : Crt)
-  int sx, sy, sz;  // the direction this lane looks at when a cell collects its arrivals (lane = code)
   unsigned lt;
   unsigned parity;
   bool loads_armed;  // bulk loads for the cell about to be processed are in flight
@@ -164,7 +163,6 @@ struct CellWalker {
     ncol = XC ? sd.ncol : NREC;
     lane = lane_;
     nbt = nbt_;
-    dir_decode<D3>(lane < ND ? lane : STAY, sx, sy, sz);
     lt = lanemask_lt_();
     buf = (float *)wsm;
     holes = (uint8_t *)(buf + (BIG ? 0 : ncol * C));
@@ -224,6 +222,11 @@ struct CellWalker {
   // key of the cell that reaches cell (lx, ly, lz) of this tile by a move in this lane's direction
   template <class TG>
   __device__ __forceinline__ int source_key(const TG &tg, int lx, int ly, int lz) const {
+    // the direction this lane looks at when a cell collects its arrivals: lane = direction code
+    // (recomputed here: a lane constant kept across the particle loop costs registers)
+    int sx, sy, sz;
+    const int dc = keep_in_loop(lane);
+    dir_decode<D3>(dc < ND ? dc : STAY, sx, sy, sz);
     int qx = lx - sx, qy = ly - sy, qz = lz - sz;
     const int tx = D3 ? (qx < 0 ? -1 : (qx >= tg.bs[0] ? 1 : 0)) : 0;
     const int ty = qy < 0 ? -1 : (qy >= tg.bs[1] ? 1 : 0);
