@@ -465,6 +465,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   int *sCnt = sBase + tg.cpb + 1;             // [cpb]: particles resident in each cell
   Walker wk;
   wk.init(smraw + (size_t)warp * wstride, sd, lane, sNbT);
+  const int kbase = tile * tg.cpb;
+  // the resident run of the warp's first cell is requested before anything else: its DRAM latency
+  // passes while the block stages its field tile
+  if (!BIG && warp < tg.cpb) wk.issue_loads(sd, sd.cnt[kbase + warp], sd.base[kbase + warp]);
   if (threadIdx.x < 27) {  // periodic neighbour tiles (the single-GPU particle exchange)
     const int t = threadIdx.x;
     const int b0 = tile % gd.nb[0], br = tile / gd.nb[0];
@@ -485,10 +489,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int off2[8] = {0, s1, s2, s2 + s1, jv, jv + s2, 2 * jv, 2 * jv + s1};
     sRel[threadIdx.x] = D3 ? off3[i] : off2[i & 7];
   }
-  const int kbase = tile * tg.cpb;
+  // (asynchronous copies: all of a thread's requests are in flight together)
   for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
-    sBase[i] = sd.base[kbase + i];
-    if (i < tg.cpb) sCnt[i] = sd.cnt[kbase + i];
+    cp_async4(sBase + i, sd.base + kbase + i, true);
+    if (i < tg.cpb) cp_async4(sCnt + i, sd.cnt + kbase + i, true);
   }
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
@@ -497,9 +501,11 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int gx = D3 ? tg.o[0] + lx - 1 + gd.g[0] : 0;
     const int gy = tg.o[1] + ly - 1 + gd.g[1], gz = tg.o[2] + lz - 1 + gd.g[2];
     const int gi = (gz * gd.ext[1] + gy) * gd.ext[0] + gx;
-    sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
+    cp_async4(sF + i, c < 3 ? E + c * gd.comp + gi : B + (c - 3) * gd.comp + gi, true);
   }
+  cp_async_commit();
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
+  cp_async_wait<0>();
   __syncthreads();
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
@@ -625,7 +631,6 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   // as soon as the image of the current one has been written back.
   int src_next;
   unsigned mask_next = wk.fetch_mask(sd, tg, warp, src_next);
-  if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
     const int nx = ci + nwarps;
