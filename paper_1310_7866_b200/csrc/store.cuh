@@ -221,12 +221,11 @@ struct CellWalker {
 
   // key of the cell that reaches cell (lx, ly, lz) of this tile by a move in this lane's direction
   template <class TG>
-  __device__ __forceinline__ int source_key(const TG &tg, int lx, int ly, int lz) const {
+  __device__ __forceinline__ int source_key(const TG &tg, int dc, int lx, int ly, int lz) const {
     // the direction this lane looks at when a cell collects its arrivals: lane = direction code
     // (recomputed here: a lane constant kept across the particle loop costs registers)
     int sx, sy, sz;
-    const int dc = keep_in_loop(lane);
-    dir_decode<D3>(dc < ND ? dc : STAY, sx, sy, sz);
+    dir_decode<D3>(dc, sx, sy, sz);
     int qx = lx - sx, qy = ly - sy, qz = lz - sz;
     const int tx = D3 ? (qx < 0 ? -1 : (qx >= tg.bs[0] ? 1 : 0)) : 0;
     const int ty = qy < 0 ? -1 : (qy >= tg.bs[1] ? 1 : 0);
@@ -242,10 +241,11 @@ struct CellWalker {
   template <class TG>
   __device__ __forceinline__ unsigned fetch_mask(const StoreDesc &sd, const TG &tg, int ci, int &src) const {
     src = 0;
-    if (!(lane < ND && lane != STAY) || ci >= tg.cpb) return 0u;
+    const int dc = keep_in_loop(lane);  // lane = direction code
+    if (!(dc < ND && dc != STAY) || ci >= tg.cpb) return 0u;
     const int lx = ci % tg.bs[0], t = ci / tg.bs[0];
-    src = source_key(tg, lx, t % tg.bs[1], t / tg.bs[1]);
-    return sd.xin.mask[(size_t)src * XW + lane];
+    src = source_key(tg, dc, lx, t % tg.bs[1], t / tg.bs[1]);
+    return sd.xin.mask[(size_t)src * XW + dc];
   }
 
   // writes the arrival-list window [a0, a0 + WALK_AC): entry = direction lane << 8 | record index
