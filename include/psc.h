@@ -202,6 +202,35 @@ int psc_charge_density(psc_ctx *ctx, void *stream, float *rho);
  * field the context allocates on first use (freed by psc_destroy). */
 int psc_marder(psc_ctx *ctx, void *stream, float diffusion, int iters);
 
+/* ---- patch-based load balancing (Appendix A) -------------
+ * The domain is cut into many more patches than processing elements; the patches are enumerated
+ * along a Hilbert-Peano space-filling curve, and the 1-d curve is cut into as many segments as
+ * there are ranks so that every rank gets a load matching its capability.  A patch here is
+ * patch_blocks[d] sort blocks ("supercells") along direction d (must divide the number of blocks;
+ * 1 along an invariant direction), i.e. np[d] = n[d] / (block[d] * patch_blocks[d]) patches. */
+
+/* Load of every patch = its particles + its cells, counted on the device from the
+ * cell store (residents by their cell, records waiting in an exchange row by the cell they move
+ * to): loads[(pz * np[1] + py) * np[0] + px], a DEVICE array of np[0]*np[1]*np[2] int64.
+ * Requires the internal form.  np_out (host, may be NULL) receives np[]. */
+int psc_patch_loads(psc_ctx *ctx, void *stream, const int32_t patch_blocks[3], int64_t *loads,
+                    int32_t np_out[3]);
+
+/* Hilbert-Peano order of an np[0] x np[1] x np[2] grid of patches (Fig. 5(b)):
+ * order[i] (HOST array, np[0]*np[1]*np[2] entries) = row-major index (pz*np[1]+py)*np[0]+px of
+ * the i-th patch on the curve.  np[d] == 1 drops that direction (a 2-d curve for a 2-d grid).
+ * Extents that are not equal powers of two: the grid is embedded in the enclosing power-of-two
+ * cube and the curve's points outside the grid are skipped.  Host only, no device needed. */
+int psc_hilbert_order(const int32_t np[3], int32_t *order);
+
+/* Appendix A: loads[p] (HOST, double, p in CURVE order, n_patches entries, all >= 0),
+ * capability[r] (HOST, n_ranks entries, all > 0; e.g. 1 per CPU core and 60 for the
+ * rank that drives a GPU) -> count[r] (HOST): rank r takes the next count[r] consecutive patches of
+ * the curve.  Every rank gets at least one patch; requires n_patches >= n_ranks >= 1
+ * (PSC_ERR_INVALID_ARG).  Host only, no device needed. */
+int psc_balance(int64_t n_patches, const double *loads, int32_t n_ranks, const double *capability,
+                int32_t *count);
+
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
  * u^{n+1}.  Same fields and the same set of particles (up to the rounding of the atomically

@@ -25,7 +25,7 @@ EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
     "psc_field_elems", "psc_particle_capacity", "psc_bind_particles", "psc_particles_sort",
     "psc_push_particles", "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step",
-    "psc_charge_density", "psc_marder",
+    "psc_charge_density", "psc_marder", "psc_patch_loads", "psc_hilbert_order", "psc_balance",
     "psc_step_host", "psc_sort_result", "psc_particles_current", "psc_particles_form",
     "psc_particles_gather", "psc_particles_export", "psc_store_info", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
@@ -89,6 +89,11 @@ def lib():
         L.psc_fill_ghosts.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.psc_charge_density.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.psc_marder.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int]
+        L.psc_patch_loads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int32), C.c_void_p,
+                                      C.POINTER(C.c_int32)]
+        L.psc_hilbert_order.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.psc_balance.argtypes = [C.c_int64, C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_double),
+                                  C.POINTER(C.c_int32)]
         L.psc_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(PscCols),
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.psc_sort_result.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
@@ -232,6 +237,14 @@ class Psc:
         """psc_marder: E += diffusion * grad+ (div- E - rho), `iters` passes (PAPER.md:206)"""
         self._check(lib().psc_marder(self._h, _stream(stream), float(diffusion), int(iters)), "psc_marder")
 
+    def patch_loads(self, patch_blocks, loads, stream=None):
+        """psc_patch_loads: particles + cells of every patch into the device int64
+        tensor `loads`; returns the patch grid (npx, npy, npz)"""
+        pb = (C.c_int32 * 3)(*[int(v) for v in patch_blocks])
+        npo = (C.c_int32 * 3)()
+        self._check(lib().psc_patch_loads(self._h, _stream(stream), pb, loads.data_ptr(), npo), "psc_patch_loads")
+        return tuple(npo)
+
     def step(self, stream=None):
         """psc_step: one time step in the order of Fig. 8"""
         self._check(lib().psc_step(self._h, _stream(stream)), "psc_step")
@@ -300,3 +313,26 @@ class Psc:
 
 def version():
     return lib().psc_version().decode()
+
+
+def hilbert_order(np3):
+    """psc_hilbert_order: row-major patch indices in Hilbert-Peano curve order"""
+    n = int(np3[0]) * int(np3[1]) * int(np3[2])
+    a = (C.c_int32 * 3)(*[int(v) for v in np3])
+    out = (C.c_int32 * n)()
+    rc = lib().psc_hilbert_order(a, out)
+    if rc:
+        raise PscError(rc, "psc_hilbert_order")
+    return list(out)
+
+
+def balance(loads, capability):
+    """psc_balance: Appendix A: patches per rank along the curve"""
+    n, r = len(loads), len(capability)
+    L = (C.c_double * n)(*[float(v) for v in loads])
+    Cp = (C.c_double * r)(*[float(v) for v in capability])
+    out = (C.c_int32 * r)()
+    rc = lib().psc_balance(n, L, r, Cp, out)
+    if rc:
+        raise PscError(rc, "psc_balance")
+    return list(out)

@@ -17,7 +17,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libpsc_b200.so")
-SOURCES = ["api.cu", "fields.cu", "sort.cu", "push1.cu", "push2.cu", "marder.cu"]
+SOURCES = ["api.cu", "fields.cu", "sort.cu", "push1.cu", "push2.cu", "marder.cu", "balance.cu"]
 HEADERS = ["psc_internal.cuh", "push_common.cuh", "store.cuh"]
 
 COMMON = [

@@ -320,6 +320,13 @@ int psc_charge_density(psc_ctx *c, void *stream, float *rho) {
   return PSC_OK;
 }
 
+int psc_patch_loads(psc_ctx *c, void *stream, const int32_t patch_blocks[3], int64_t *loads, int32_t np_out[3]) {
+  if (!c || !patch_blocks || !loads) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->state != PSC_STATE_STORE) return PSC_ERR_NOT_SORTED;
+  return psc_patch_loads_internal(c, (cudaStream_t)stream, patch_blocks, loads, np_out);
+}
+
 int psc_marder(psc_ctx *c, void *stream, float diffusion, int iters) {
   if (!c || iters < 0 || !(diffusion >= 0.f)) return PSC_ERR_INVALID_ARG;
   if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;

@@ -216,3 +216,6 @@ int psc_push_order2(psc_ctx *c, cudaStream_t s);
 // marder.cu
 int psc_marder_pass(psc_ctx *c, float diffusion, int iters, cudaStream_t s);
 int psc_charge_density_internal(psc_ctx *c, cudaStream_t s);
+// balance.cu
+int psc_patch_loads_internal(psc_ctx *c, cudaStream_t s, const int32_t patch_blocks[3], int64_t *loads,
+                             int32_t np_out[3]);

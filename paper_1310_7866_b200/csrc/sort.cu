@@ -120,18 +120,6 @@ k_zero(int m, int *__restrict__ a, const uint32_t *__restrict__ cond) {
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < m; i += gridDim.x * blockDim.x) a[i] = 0;
 }
 
-// key -> cell coordinates
-__device__ __forceinline__ void key_to_cell(const GridDesc &gd, int k, int c[3]) {
-  const int b = k / gd.cpb, l = k - b * gd.cpb;
-  const int b0 = b % gd.nb[0], br = b / gd.nb[0];
-  const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
-  const int l0 = l % gd.bs[0], lr = l / gd.bs[0];
-  const int l1 = lr % gd.bs[1], l2 = lr / gd.bs[1];
-  c[0] = b0 * gd.bs[0] + l0;
-  c[1] = b1 * gd.bs[1] + l1;
-  c[2] = b2 * gd.bs[2] + l2;
-}
-
 __global__ void __launch_bounds__(SORT_THREADS)
 k_cell_idx(GridDesc gd, int n, const int *__restrict__ key, int *__restrict__ cell_idx) {
   const int a = blockIdx.x * blockDim.x + threadIdx.x;

@@ -82,6 +82,18 @@ __device__ __forceinline__ int cell_key(const GridDesc &gd, int cx, int cy, int 
   const int l0 = cx - b0 * gd.bs[0], l1 = cy - b1 * gd.bs[1], l2 = cz - b2 * gd.bs[2];
   return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
 }
+// key -> cell coordinates
+__device__ __forceinline__ void key_to_cell(const GridDesc &gd, int k, int c[3]) {
+  const int b = k / gd.cpb, l = k - b * gd.cpb;
+  const int b0 = b % gd.nb[0], br = b / gd.nb[0];
+  const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
+  const int l0 = l % gd.bs[0], lr = l / gd.bs[0];
+  const int l1 = lr % gd.bs[1], l2 = lr / gd.bs[1];
+  c[0] = b0 * gd.bs[0] + l0;
+  c[1] = b1 * gd.bs[1] + l1;
+  c[2] = b2 * gd.bs[2] + l2;
+}
+
 template <bool D3>
 __device__ __forceinline__ void dir_decode(int dc, int &sx, int &sy, int &sz) {
   if (D3) {
