@@ -278,19 +278,24 @@ k_scatter(const int *__restrict__ np, const int *__restrict__ key, int *__restri
           int *__restrict__ perm, const uint32_t *__restrict__ cond) {
   PSC_COND_RETURN(cond);
   const int n = *np;
-  const int a0 = blockIdx.x * blockDim.x + threadIdx.x;
-  const int stride = gridDim.x * blockDim.x;
-  const int nround = ((n + 31) / 32) * 32;
   const int lane = threadIdx.x & 31;
-  for (int a = a0; a < nround; a += stride) {
-    const bool valid = a < n;
+  // Every warp walks ONE contiguous span of the input, 32 particles at a time: a key whose
+  // particles all lie inside one span (a list that is already ordered by cell, e.g. as generated
+  // or after a few pushes) gets its positions in ascending input order, and k_segsort finds its
+  // segment already sorted.  (Spans are multiples of 32, so every load is a full 128-byte line.)
+  const long long nwarps = (long long)gridDim.x * (blockDim.x >> 5);
+  const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const long long span = ((n + nwarps - 1) / nwarps + 31) / 32 * 32;
+  const long long lo = wid * span, hi = lo + span < n ? lo + span : n;
+  for (long long a = lo + lane; a - lane < hi; a += 32) {
+    const bool valid = a < hi;
     const int k = valid ? key[a] : -1 - lane;
     const unsigned grp = __match_any_sync(0xffffffffu, k);
     const int leader = __ffs(grp) - 1;
     int base = 0;
     if (valid && lane == leader) base = atomicAdd(&cursor[k], __popc(grp));
     base = __shfl_sync(0xffffffffu, base, leader);
-    if (valid) perm[base + __popc(grp & lanemask_lt())] = a;
+    if (valid) perm[base + __popc(grp & lanemask_lt())] = (int)a;
   }
 }
 
