@@ -82,6 +82,34 @@ __device__ __forceinline__ void warp_reduce_n(const float (&v)[N], float (&r)[Re
   red_stage<S::H4, S::H5>(d, r, lane & 1, 1);
 }
 
+// The same reduction for the 48 values v[(jf * 4 + je) * 3 + i] of a 3-d current component when
+// the caller has filled them from transverse factors ALREADY PERMUTED per lane (perm4 below): a
+// lane whose bit 4 (3) is set has its jf index flipped by 2 (1), bit 2 (1) its je index by 2 (1),
+// so that in every one of the first four stages each lane keeps the lower half of its values and
+// hands the upper half to its partner -- no selects (2 per value and stage otherwise).  The
+// totals a lane ends up with are those of warp_reduce_n<48> on the unpermuted values.
+__device__ __forceinline__ void warp_reduce_48_permuted(const float (&v)[48], float (&r)[2], int lane) {
+  float a[24], b[12], c[6], d[3];
+#pragma unroll
+  for (int i = 0; i < 24; i++) a[i] = v[i] + __shfl_xor_sync(0xffffffffu, v[i + 24], 16);
+#pragma unroll
+  for (int i = 0; i < 12; i++) b[i] = a[i] + __shfl_xor_sync(0xffffffffu, a[i + 12], 8);
+#pragma unroll
+  for (int i = 0; i < 6; i++) c[i] = b[i] + __shfl_xor_sync(0xffffffffu, b[i + 6], 4);
+#pragma unroll
+  for (int i = 0; i < 3; i++) d[i] = c[i] + __shfl_xor_sync(0xffffffffu, c[i + 3], 2);
+  red_stage<3, 2>(d, r, lane & 1, 1);
+}
+
+// o[j] = a[j ^ (2 hi + lo)]
+__device__ __forceinline__ void perm4(float (&o)[4], const float (&a)[4], bool hi, bool lo) {
+  const float t0 = hi ? a[2] : a[0], t1 = hi ? a[3] : a[1], t2 = hi ? a[0] : a[2], t3 = hi ? a[1] : a[3];
+  o[0] = lo ? t1 : t0;
+  o[1] = lo ? t0 : t1;
+  o[2] = lo ? t3 : t2;
+  o[3] = lo ? t2 : t3;
+}
+
 // index (0..N-1) of the value whose total lane `lane` holds in r[j], or -1 for padding
 template <int N>
 __device__ __forceinline__ int red_index(int lane, int j) {
@@ -245,6 +273,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   int *sCnt = sBase + tg.cpb + 1;                            // [cpb]
   Walker wk;
   wk.init(smraw + (size_t)warp * wstride, sd, lane, sNbT);
+  const int kbase = tile * tg.cpb;
+  // the resident run of the warp's first cell is requested before anything else: its DRAM latency
+  // passes while the block stages its field tile
+  if (!BIG && warp < tg.cpb) wk.issue_loads(sd, sd.cnt[kbase + warp], sd.base[kbase + warp]);
   if (threadIdx.x < 27) {  // periodic neighbour tiles (the single-GPU particle exchange)
     const int t = threadIdx.x;
     const int b0 = tile % gd.nb[0], br = tile / gd.nb[0];
@@ -255,10 +287,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
 
   if (threadIdx.x < PSC_MAX_SPECIES) sH[threadIdx.x] = gd.qmh[threadIdx.x];
-  const int kbase = tile * tg.cpb;
+  // (asynchronous copies: all of a thread's requests are in flight together)
   for (int i = threadIdx.x; i <= tg.cpb; i += blockDim.x) {
-    sBase[i] = sd.base[kbase + i];
-    if (i < tg.cpb) sCnt[i] = sd.cnt[kbase + i];
+    cp_async4(sBase + i, sd.base + kbase + i, true);
+    if (i < tg.cpb) cp_async4(sCnt + i, sd.cnt + kbase + i, true);
   }
   for (int i = threadIdx.x; i < 6 * tg.tvol; i += blockDim.x) {
     const int c = i / tg.tvol, r = i - c * tg.tvol;
@@ -267,8 +299,9 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int gx = D3 ? tg.o[0] + tx - 1 + gd.g[0] : 0;
     const int gy = tg.o[1] + ty - 1 + gd.g[1], gz = tg.o[2] + tz - 1 + gd.g[2];
     const int gi = (gz * gd.ext[1] + gy) * gd.ext[0] + gx;
-    sF[i] = c < 3 ? E[c * gd.comp + gi] : B[(c - 3) * gd.comp + gi];
+    cp_async4(sF + i, c < 3 ? E + c * gd.comp + gi : B + (c - 3) * gd.comp + gi, true);
   }
+  cp_async_commit();
   for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) sJ[i] = 0.f;
 
   // which totals this lane holds after each reduction, as J-tile offsets from the cell's point
@@ -280,6 +313,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     offy[j] = j < RedShape<NY>::R ? value_offset<D3>(tg, 1, red_index<NY>(lane, j)) : INT_MIN;
     offz[j] = j < RedShape<NZ>::R ? value_offset<D3>(tg, 2, red_index<NZ>(lane, j)) : INT_MIN;
   }
+  cp_async_wait<0>();
   __syncthreads();
 
   const float *sEx = sF, *sEy = sF + tg.tvol, *sEz = sF + 2 * tg.tvol;
@@ -323,7 +357,6 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   bool left_out = false;  // this warp met a cell that does not fit the image
   int src_next;
   unsigned mask_next = wk.fetch_mask(sd, tg, warp, src_next);
-  if (warp < tg.cpb) wk.issue_loads(sd, sCnt[warp], sBase[warp]);
 #pragma unroll 1
   for (int ci = warp; ci < tg.cpb; ci += nwarps) {
     const int nx = ci + nwarps;
@@ -431,37 +464,37 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
               if (k < 3) { run -= f * Xd[k]; Ax[k] = run; }
             }
           }
-          float v[48];
-          // jx: transverse e = y, f = z
+          // one component at a time: 48 values A_c[i] * (Em[je] Fm[jf] + Ed[je] Fd[jf] / 12) from the
+          // transverse factors permuted for the select-free reduction (e-role: lane bits 2, 1;
+          // f-role: lane bits 4, 3)
+          const bool l4 = lane & 16, l3 = lane & 8, l2 = lane & 4, l1 = lane & 2;
+          auto component = [&](const float (&A)[3], const float (&Em)[4], const float (&Ed)[4],
+                               const float (&Fm)[4], const float (&Fd)[4], const int (&off)[2]) {
+            float em[4], ed[4], fm[4], fd[4];
+            perm4(em, Em, l2, l1);
+            perm4(ed, Ed, l2, l1);
+            perm4(fm, Fm, l4, l3);
+            perm4(fd, Fd, l4, l3);
 #pragma unroll
-          for (int jf = 0; jf < 4; jf++)
+            for (int k = 0; k < 4; k++) fd[k] *= (1.0f / 12.0f);
+            float v[48];
 #pragma unroll
-            for (int je = 0; je < 4; je++) {
-              const float br = fmaf(Ym[je], Zm[jf], Yd[je] * Zd[jf] * (1.0f / 12.0f));
+            for (int jf = 0; jf < 4; jf++)
 #pragma unroll
-              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Ax[i] * br;
-            }
-          add_reduced<48>(cellJ, v, offx, lane);
-          // jy: e = z, f = x
+              for (int je = 0; je < 4; je++) {
+                const float br = fmaf(em[je], fm[jf], ed[je] * fd[jf]);
 #pragma unroll
-          for (int jf = 0; jf < 4; jf++)
+                for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = A[i] * br;
+              }
+            float r[2];
+            warp_reduce_48_permuted(v, r, lane);
 #pragma unroll
-            for (int je = 0; je < 4; je++) {
-              const float br = fmaf(Zm[je], Xm[jf], Zd[je] * Xd[jf] * (1.0f / 12.0f));
-#pragma unroll
-              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Ay[i] * br;
-            }
-          add_reduced<48>(cellJ, v, offy, lane);
-          // jz: e = x, f = y
-#pragma unroll
-          for (int jf = 0; jf < 4; jf++)
-#pragma unroll
-            for (int je = 0; je < 4; je++) {
-              const float br = fmaf(Xm[je], Ym[jf], Xd[je] * Yd[jf] * (1.0f / 12.0f));
-#pragma unroll
-              for (int i = 0; i < 3; i++) v[(jf * 4 + je) * 3 + i] = Az[i] * br;
-            }
-          add_reduced<48>(cellJ, v, offz, lane);
+            for (int j = 0; j < 2; j++)
+              if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
+          };
+          component(Ax, Ym, Yd, Zm, Zd, offx);  // jx: transverse e = y, f = z
+          component(Ay, Zm, Zd, Xm, Xd, offy);  // jy: e = z, f = x
+          component(Az, Xm, Xd, Ym, Yd, offz);  // jz: e = x, f = y
         } else {
           const float qvx = qw * gd.inv_dV * vx;
           {
