@@ -230,17 +230,6 @@ __device__ __forceinline__ int value_offset(const TG &tg, int comp, int idx) {
   return 2 * tg.tvol + ((idx % 3) - 1) * s[2] + ((idx / 3) - 1) * s[1];
 }
 
-template <int N>
-__device__ __forceinline__ void add_reduced(float *__restrict__ cellJ, const float (&v)[N],
-                                            const int (&off)[2], int lane) {
-  float r[RedShape<N>::R];
-  warp_reduce_n<N>(v, r, lane);
-  static_assert(RedShape<N>::R <= 2, "two totals per lane at most");
-#pragma unroll
-  for (int j = 0; j < RedShape<N>::R; j++)
-    if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
-}
-
 // BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
 // launch for the tiles in which the first one had to leave a cell out.
 template <bool D3, int CBS, bool XC, bool BIG, bool ALT>
@@ -384,6 +373,9 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
                             : (lz + 1) * tg.te[1] + (ly + 1));
     if (!BIG && wk.na) wk.stage_arrivals(sd);
     bool landed = false;
+    // the lane's reduced totals, summed over the chunks of the cell: one shared-memory add per
+    // cell instead of one per chunk (a shared fp32 atomicAdd is a compare-and-swap loop)
+    float racc[3][2] = {{0.f, 0.f}, {0.f, 0.f}, {0.f, 0.f}};
 #pragma unroll 1
     for (int base = 0; base < np_cell; base += 32) {
       Part cur;
@@ -469,7 +461,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
           // f-role: lane bits 4, 3)
           const bool l4 = lane & 16, l3 = lane & 8, l2 = lane & 4, l1 = lane & 2;
           auto component = [&](const float (&A)[3], const float (&Em)[4], const float (&Ed)[4],
-                               const float (&Fm)[4], const float (&Fd)[4], const int (&off)[2]) {
+                               const float (&Fm)[4], const float (&Fd)[4], float (&rsum)[2]) {
             float em[4], ed[4], fm[4], fd[4];
             perm4(em, Em, l2, l1);
             perm4(ed, Ed, l2, l1);
@@ -488,13 +480,12 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
               }
             float r[2];
             warp_reduce_48_permuted(v, r, lane);
-#pragma unroll
-            for (int j = 0; j < 2; j++)
-              if (off[j] != INT_MIN) atomicAdd(cellJ + off[j], r[j]);
+            rsum[0] += r[0];
+            rsum[1] += r[1];
           };
-          component(Ax, Ym, Yd, Zm, Zd, offx);  // jx: transverse e = y, f = z
-          component(Ay, Zm, Zd, Xm, Xd, offy);  // jy: e = z, f = x
-          component(Az, Xm, Xd, Ym, Yd, offz);  // jz: e = x, f = y
+          component(Ax, Ym, Yd, Zm, Zd, racc[0]);  // jx: transverse e = y, f = z
+          component(Ay, Zm, Zd, Xm, Xd, racc[1]);  // jy: e = z, f = x
+          component(Az, Xm, Xd, Ym, Yd, racc[2]);  // jz: e = x, f = y
         } else {
           const float qvx = qw * gd.inv_dV * vx;
           {
@@ -504,7 +495,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
 #pragma unroll
               for (int jy = 0; jy < 4; jy++)
                 v[jz * 4 + jy] = qvx * fmaf(Ym[jy], Zm[jz], Yd[jy] * Zd[jz] * (1.0f / 12.0f));
-            add_reduced<16>(cellJ, v, offx, lane);
+            float r[RedShape<16>::R];
+            warp_reduce_n<16>(v, r, lane);
+#pragma unroll
+            for (int j = 0; j < RedShape<16>::R; j++) racc[0][j] += r[j];
           }
           {
             float v[12];
@@ -512,7 +506,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
             for (int jz = 0; jz < 4; jz++)
 #pragma unroll
               for (int i = 0; i < 3; i++) v[jz * 3 + i] = Ay[i] * Zm[jz];
-            add_reduced<12>(cellJ, v, offy, lane);
+            float r[RedShape<12>::R];
+            warp_reduce_n<12>(v, r, lane);
+#pragma unroll
+            for (int j = 0; j < RedShape<12>::R; j++) racc[1][j] += r[j];
           }
           {
             float v[12];
@@ -520,7 +517,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
             for (int jy = 0; jy < 4; jy++)
 #pragma unroll
               for (int i = 0; i < 3; i++) v[jy * 3 + i] = Az[i] * Ym[jy];
-            add_reduced<12>(cellJ, v, offz, lane);
+            float r[RedShape<12>::R];
+            warp_reduce_n<12>(v, r, lane);
+#pragma unroll
+            for (int j = 0; j < RedShape<12>::R; j++) racc[2][j] += r[j];
           }
         }
       }
@@ -542,6 +542,12 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         wk.store_image(base, act, leave, pn);
       }
       if (act && !(fabsf(ux) + fabsf(uy) + fabsf(uz) < 3.0e38f)) bad |= PSC_F_NAN;
+    }
+#pragma unroll
+    for (int j = 0; j < 2; j++) {
+      if (offx[j] != INT_MIN) atomicAdd(cellJ + offx[j], racc[0][j]);
+      if (offy[j] != INT_MIN) atomicAdd(cellJ + offy[j], racc[1][j]);
+      if (offz[j] != INT_MIN) atomicAdd(cellJ + offz[j], racc[2][j]);
     }
     if (BIG) {
       wk.end_global(sd);
