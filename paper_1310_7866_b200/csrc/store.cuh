@@ -388,7 +388,7 @@ struct CellWalker {
         q[2 * C] = pn.ux; q[3 * C] = pn.uy; q[4 * C] = pn.uz;
       }
       if (leave) {
-        const int hi = nh + __popc(mrl & lt);
+        const int hi = nh + __popc(mrl & ((1u << lane) - 1u));  // (not the lanemask register: an S2R per chunk)
         if (hi < WALK_HC) holes[hi] = (uint8_t)v;
       }
     }
