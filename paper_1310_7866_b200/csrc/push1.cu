@@ -517,7 +517,6 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   int qcnt = 0;  // warp-uniform: entries in this warp's queue
   // global index of the node of the tile's first cell
   const int gnode0 = ((tg.o[2] + gd.g[2]) * gd.ext[1] + (tg.o[1] + gd.g[1])) * gd.ext[0] + (D3 ? tg.o[0] + gd.g[0] : 0);
-  bool left_out = false;  // this warp met a cell that does not fit the image
 
   // One particle: gather (Eq. 11 with b1 weights; each component from its own Yee points:
   // node-centred along d: points l, l+1, weight a; half-staggered: points l-1, l (a < 1/2, weight
@@ -661,8 +660,10 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       __syncwarp();
       if (lane == 0) sd.bigcell[kbase + ci] = 0;
     } else if (!wk.fits) {
-      left_out = true;
-      if (lane == 0) sd.bigcell[kbase + ci] = 1;
+      if (lane == 0) {  // note the cell and (once) its tile for the BIG launch
+        sd.bigcell[kbase + ci] = 1;
+        if (atomicExch(&sd.bigflag[tile], 1) == 0) atomicAdd(sd.nbig, 1u);
+      }
       wk.skip_cell(sd, next_n, next_base);
       continue;
     }
@@ -773,11 +774,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   if (qcnt) drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
   wk.finish();
-  const int any_left = __syncthreads_or(left_out ? 1 : 0);
-  if (!BIG && threadIdx.x == 0) {
-    sd.bigflag[tile] = any_left;
-    if (any_left) atomicAdd(sd.nbig, 1u);
-  }
+  __syncthreads();
+  if (BIG && threadIdx.x == 0) sd.bigflag[tile] = 0;  // taken care of: the flag is the image launch's to set
 
   // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) {

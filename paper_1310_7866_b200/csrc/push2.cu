@@ -343,7 +343,6 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     }
   };
 
-  bool left_out = false;  // this warp met a cell that does not fit the image
   int src_next;
   unsigned mask_next = wk.fetch_mask(sd, tg, warp, src_next);
 #pragma unroll 1
@@ -361,8 +360,10 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       __syncwarp();
       if (lane == 0) sd.bigcell[kbase + ci] = 0;
     } else if (!wk.fits) {
-      left_out = true;
-      if (lane == 0) sd.bigcell[kbase + ci] = 1;
+      if (lane == 0) {  // note the cell and (once) its tile for the BIG launch
+        sd.bigcell[kbase + ci] = 1;
+        if (atomicExch(&sd.bigflag[tile], 1) == 0) atomicAdd(sd.nbig, 1u);
+      }
       wk.skip_cell(sd, next_n, next_base);
       continue;
     }
@@ -573,11 +574,8 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   wk.finish();
   if (bad) atomicOr(sd.flags, bad);
-  const int any_left = __syncthreads_or(left_out ? 1 : 0);
-  if (!BIG && threadIdx.x == 0) {
-    sd.bigflag[tile] = any_left;
-    if (any_left) atomicAdd(sd.nbig, 1u);
-  }
+  __syncthreads();
+  if (BIG && threadIdx.x == 0) sd.bigflag[tile] = 0;  // taken care of: the flag is the image launch's to set
 
   // ---- flush the J tile to global J -----------------------------------------------------------
   for (int i = threadIdx.x; i < 3 * tg.tvol; i += blockDim.x) {

@@ -593,7 +593,7 @@ k_gather_spill(GridDesc gd, Spill sp, const int *__restrict__ doffs, Cols out, i
 // after a (re-)layout: every exchange row empty, nothing spilled; records the slots in use
 __global__ void __launch_bounds__(SORT_THREADS)
 k_store_reset(int nk, int xw, uint32_t *__restrict__ m0, uint32_t *__restrict__ m1, uint8_t *__restrict__ bigcell,
-              const int *__restrict__ base, uint32_t *__restrict__ dw, long long capacity,
+              int ntiles, int32_t *__restrict__ bigflag, const int *__restrict__ base, uint32_t *__restrict__ dw, long long capacity,
               const uint32_t *__restrict__ cond) {
   PSC_COND_RETURN(cond);
   const int m = nk * xw;
@@ -601,6 +601,7 @@ k_store_reset(int nk, int xw, uint32_t *__restrict__ m0, uint32_t *__restrict__ 
     m0[i] = 0u;
     m1[i] = 0u;
     if (i < nk) bigcell[i] = 0;
+    if (i < ntiles) bigflag[i] = 0;
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     dw[PSC_DW_SLOTS] = (uint32_t)base[nk];
@@ -831,7 +832,8 @@ int sort_core(psc_ctx *c, const Cols &src, const Cols &dst, bool from_abs, bool 
   PSC_LAUNCH_CHECK(c);
   psc_prof_end(c, PSC_PH_SORT_REORDER, s);
   k_store_reset<<<grid_for(c, (int64_t)nk * 16, SORT_THREADS), SORT_THREADS, 0, s>>>(
-      nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, c->xch[0].mask, c->xch[1].mask, c->bigcell, c->base, c->d_flags,
+      nk, psc_is3d(gd) ? PSC_XW3 : PSC_XW2, c->xch[0].mask, c->xch[1].mask, c->bigcell, gd.ntiles, c->bigflag,
+      c->base, c->d_flags,
       (long long)c->capacity, cond);
   PSC_LAUNCH_CHECK(c);
   return PSC_OK;
@@ -907,6 +909,7 @@ struct RelayoutArgs {
   Spill spill;
   int32_t *key, *perm, *offs_dense, *base, *cnt, *cursor, *tot, *doffs;
   uint8_t *bigcell;
+  int32_t *bigflag;
   long long *pack, *packloc, *scan_tmp;
   uint32_t *dw;
   int *np_dev;
@@ -936,7 +939,8 @@ __device__ void relayout_chain(const RelayoutArgs &a) {
   k_scan_add2<<<a.sblocks, T, 0, ts>>>(nk, a.packloc, a.base, a.offs_dense, a.cursor, a.scan_tmp, a.sblocks, nc);
   k_scatter<<<a.g_part, T, 0, ts>>>(a.np_dev, a.key, a.cursor, a.perm, nc);
   k_reorder<false><<<a.g_part, T, 0, ts>>>(a.gd, a.np_dev, a.perm, a.key, a.offs_dense, a.base, a.tmp, a.cur, nc);
-  k_store_reset<<<a.g_reset, T, 0, ts>>>(nk, XW, a.x0.mask, a.x1.mask, a.bigcell, a.base, a.dw, a.capacity, nc);
+  k_store_reset<<<a.g_reset, T, 0, ts>>>(nk, XW, a.x0.mask, a.x1.mask, a.bigcell, a.gd.ntiles, a.bigflag, a.base,
+                                         a.dw, a.capacity, nc);
   k_relayout_done<<<1, 32, 0, ts>>>(a.dw);
 }
 
@@ -964,6 +968,7 @@ int psc_store_relayout_if_spilled(psc_ctx *c, cudaStream_t s) {
   }
   a.key = c->key; a.perm = c->perm; a.offs_dense = c->offs_dense; a.base = c->base; a.cnt = c->cnt;
   a.cursor = c->cursor; a.tot = c->tot; a.doffs = c->doffs; a.bigcell = c->bigcell;
+  a.bigflag = c->bigflag;
   a.pack = c->pack; a.packloc = c->packloc; a.scan_tmp = c->scan_tmp;
   a.dw = c->d_flags;
   a.np_dev = c->key + c->np;
