@@ -676,15 +676,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     if (!BIG) {
       // ---- image path: every particle of the cell, arrivals included, is a slot of the image ----
       if (wk.na) wk.stage_arrivals(sd);
-      bool landed = false;
-      int v0 = 0;
-#pragma unroll 1
-      for (; v0 < ntot; v0 += 32) {
-        if (!landed && v0 + 32 > wk.n) {
-          wk.arrivals_landed();
-          landed = true;
-        }
-        const bool act = v0 + lane < ntot;
+      auto chunk = [&](int v0, bool act) {
         Part p;
         wk.load_image(v0 + lane, p);
         kick(cF, p.ax, p.ay, p.az, p.ux, p.uy, p.uz, p.sp);
@@ -698,6 +690,28 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         vb_moments<D3>(acc, p.ax, p.ay, p.az, pn.ax, pn.ay, pn.az, qs * gd.cur[0], qs * gd.cur[1],
                        qs * gd.cur[2], qs * gd.inv_dV * vx);
         wk.store_image(v0, act, !stay, pn);
+      };
+      // the chunks that hold residents only (every lane a particle, nothing to wait for), then the
+      // rest: the residents' tail and the arrivals behind it
+      if (!D3) {
+        int v0 = 0;
+#pragma unroll 1
+        for (; v0 + 32 <= wk.n; v0 += 32) chunk(v0, true);
+        if (v0 < ntot) {
+          wk.arrivals_landed();
+#pragma unroll 1
+          for (; v0 < ntot; v0 += 32) chunk(v0, v0 + lane < ntot);
+        }
+      } else {  // (3-d: one copy of the larger chunk body; two cost more in instruction fetch than they save)
+        bool landed = false;
+#pragma unroll 1
+        for (int v0 = 0; v0 < ntot; v0 += 32) {
+          if (!landed && v0 + 32 > wk.n) {
+            wk.arrivals_landed();
+            landed = true;
+          }
+          chunk(v0, v0 + lane < ntot);
+        }
       }
       // ---- the cell's leavers, 32 at a time: records + the currents of their trajectories ------
       const int nl = wk.nh;
