@@ -39,6 +39,9 @@
 #ifndef PSC_MINB2D
 #define PSC_MINB2D 6  // blocks per SM of the default 2-d kernel
 #endif
+#ifndef PSC_MINB3D
+#define PSC_MINB3D 5  // ... of the default 3-d kernel
+#endif
 namespace {
 
 // per-warp queue of trajectories that leave their cell: 2-d (3 % leavers; shared memory decides
@@ -876,7 +879,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     }
   } else if (d3) {
     const bool def = gd.bs[0] == 4 && gd.bs[1] == 4 && gd.bs[2] == 4;
-    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, 5, true);
+    if (def) PSC_LAUNCH_PUSH1(true, 4, 128, PSC_MINB3D, true);
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
