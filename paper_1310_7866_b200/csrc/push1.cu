@@ -6,10 +6,11 @@
 // its cells can touch (tile + 1 halo point each side) in shared memory and accumulates current
 // in a shared J tile (tile + 1 low / 2 high halo nodes) that is flushed to global J once.  A
 // warp takes one CELL at a time and walks that cell's slots in chunks of 32, so the cell -- and
-// with it every tile address that does not depend on the in-cell offset -- is warp-uniform, the
-// gather reads are shared-memory broadcasts, and the currents of the trajectories that stay
-// inside the cell (the great majority) are summed in registers over the whole cell and
-// reduced across the warp once per cell.
+// with it every tile address that does not depend on the in-cell offset -- is warp-uniform: the
+// gather becomes the evaluation of per-cell polynomials (the warp turns the cell's field stencil
+// into a small coefficient table once per cell, "per-cell gather tables" below), and the currents
+// of the trajectories that stay inside the cell (the great majority) are summed in registers
+// over the whole cell and reduced across the warp once per cell.
 //
 // This is the single particle loop of PAPER.md:603 ("only one loop each time step that reads
 // and writes all particle data"), over the cell store of store.cuh: a cell's resident particles
