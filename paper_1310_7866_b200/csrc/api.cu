@@ -212,6 +212,7 @@ int psc_bind_fields(psc_ctx *c, float *E, float *B, float *J) {
   c->B = B;
   c->J = J;
   c->have_fields = 1;
+  psc_make_tile_maps(c);  // optional: the 3-d order-1 kernel stages its tiles by TMA where they apply
   return PSC_OK;
 }
 

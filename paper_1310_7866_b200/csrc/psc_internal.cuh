@@ -1,5 +1,6 @@
 // psc_internal.cuh -- internal declarations of the B200 PIC hot path (not part of the C ABI).
 #pragma once
+#include <cuda.h>  // CUtensorMap (type only: the encoder is fetched from the driver at run time)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -130,8 +131,16 @@ enum {
   PSC_DW_COUNT = 16
 };
 
+// TMA tensor maps of the three field arrays (float[3][ez][ey][ex] as a 4-d tensor x, y, z,
+// component) for the tile loads / the J-tile reduction of the 3-d order-1 kernel (push1.cu)
+struct TileMaps {
+  CUtensorMap E, B, J;
+};
+
 struct psc_ctx {
   GridDesc gd;
+  TileMaps tmaps;
+  int have_tmaps;  // tmaps describe the bound E, B, J (3-d, default 4x4x4 block, x extent a multiple of 4)
   Prof prof;
   float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
   float *E, *B, *J;
@@ -212,6 +221,7 @@ int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cud
 StoreDesc psc_store_desc(const psc_ctx *c);
 // push1.cu / push2.cu
 int psc_push_order1(psc_ctx *c, cudaStream_t s);
+int psc_make_tile_maps(psc_ctx *c);  // after psc_bind_fields; sets have_tmaps (0 if TMA maps are not applicable)
 int psc_push_order2(psc_ctx *c, cudaStream_t s);
 // marder.cu
 int psc_marder_pass(psc_ctx *c, float diffusion, int iters, cudaStream_t s);

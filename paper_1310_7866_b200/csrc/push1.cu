@@ -56,7 +56,10 @@ constexpr int QROWS2 = 7, QROWS3 = 8;
 // Tile geometry.  CBS != 0: the sort block is CBS cells along every active direction (the
 // library defaults, 8x8 in 2-d and 4x4x4 in 3-d), known at compile time so that every tile
 // extent, stride and shared-memory offset folds into an immediate; CBS == 0: run-time block.
-template <bool D3, int CBS>
+// TM: the tiles are staged by TMA tensor copies (3-d default block only), whose boxes must be a
+// multiple of 16 bytes along x: the field tile is 8 x 6 x 6 instead of 6 x 6 x 6, the J tile
+// 8 x 7 x 7 instead of 7 x 7 x 7 (the extra points are loaded / stay zero and are never used).
+template <bool D3, int CBS, bool TM = false>
 struct TileGeom {
   int o[3];        // first cell of the tile (global cell coordinates)
   int bs[3], cpb;  // block size in cells, cells per block
@@ -73,10 +76,10 @@ struct TileGeom {
     o[0] = b0 * bs[0];
     o[1] = b1 * bs[1];
     o[2] = b2 * bs[2];
-    fe[0] = D3 ? bs[0] + 2 : 1;
+    fe[0] = TM ? 8 : (D3 ? bs[0] + 2 : 1);
     fe[1] = bs[1] + 2;
     fe[2] = bs[2] + 2;
-    je[0] = D3 ? bs[0] + 3 : 1;
+    je[0] = TM ? 8 : (D3 ? bs[0] + 3 : 1);
     je[1] = bs[1] + 3;
     je[2] = bs[2] + 3;
     fvol = fe[0] * fe[1] * fe[2];
@@ -432,10 +435,13 @@ __device__ __forceinline__ float gather1(const float *__restrict__ q, int s1, in
 // XC: optional columns may be bound (the carried invariant coordinate of a 2-d run, the id).
 // BIG == false: the cells that fit the shared-memory image (store.cuh); BIG == true: a second
 // launch for the tiles in which the first one had to leave a cell out.
-template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG, int CT, bool ALT>
+// TM: the E/B tile arrives by two TMA tensor copies (one box of 8 x 6 x 6 x 3 values per field
+// array) and the J tile leaves by one TMA tensor reduction (add) -- three instructions of one
+// thread instead of 1300 4-byte copies and 1000 atomics with their index arithmetic.
+template <bool D3, int CBS, int THREADS, int MINB, bool XC, bool BIG, int CT, bool ALT, bool TM = false>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__restrict__ B,
-        float *__restrict__ J, int wstride) {
+        float *__restrict__ J, int wstride, const __grid_constant__ TileMaps tm) {
   extern __shared__ __align__(128) unsigned char smraw[];
   // the image launch has one block per tile; the BIG launch a few blocks that walk the flagged tiles
 #pragma unroll 1
@@ -450,7 +456,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   constexpr int NV = D3 ? 12 : 8;
   using Walker = CellWalker<D3, XC, BIG, CT>;
-  TileGeom<D3, CBS> tg;
+  static_assert(!TM || (D3 && CBS == 4 && !BIG), "TMA tiles: the 3-d default block, image launch");
+  TileGeom<D3, CBS, TM> tg;
   tg.init(gd, tile);
   const int lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
   // (broadcast from lane 0: lets the compiler keep everything derived from the warp index uniform)
@@ -462,7 +469,8 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   float *myT = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP) + warp * GTab<D3>::FLOATS;
   float *sF = (float *)(smraw + (size_t)nwarps * wstride) + nwarps * (QROWS * QCAP + GTab<D3>::FLOATS);  // [6][fvol]
   float *sJ = sF + 6 * tg.fvol;               // [3][jvol]
-  float *sH = sJ + 3 * tg.jvol;               // [8]: Boris h per species
+  uint64_t *tbar = (uint64_t *)(sJ + 3 * tg.jvol);  // TM: mbarrier of the tile loads (8-byte aligned)
+  float *sH = sJ + 3 * tg.jvol + (TM ? 2 : 0);  // [8]: Boris h per species
   int *sRel = (int *)(sH + PSC_MAX_SPECIES);  // [24]: J points of vb_values (tile, global)
   int *sNbT = sRel + 24;                      // [27]: first key of the 3^3 neighbouring tiles
   int *sBase = sNbT + 27;                     // [cpb + 1]: first slot of each cell
@@ -498,6 +506,21 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     cp_async4(sBase + i, sd.base + kbase + i, true);
     if (i < tg.cpb) cp_async4(sCnt + i, sd.cnt + kbase + i, true);
   }
+  // Without swizzle the box of a TMA tensor copy must start on a 16-byte boundary along x (measured:
+  // an x coordinate that is not a multiple of 4 floats raises "illegal instruction"), so the TMA
+  // tiles start one point further left (stored x = o, a multiple of 4) and every tile x index is
+  // one larger: XS.
+  constexpr int XS = TM ? 1 : 0;
+  const int tc0 = D3 ? tg.o[0] - 1 - XS + gd.g[0] : 0, tc1 = tg.o[1] - 1 + gd.g[1], tc2 = tg.o[2] - 1 + gd.g[2];
+  if (TM) {
+    if (threadIdx.x == 0) {
+      mbar_init(tbar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      mbar_expect_tx(tbar, 2u * 3u * (unsigned)tg.fvol * 4u);
+      tma_load_4d(sF, &tm.E, tc0, tc1, tc2, 0, tbar);
+      tma_load_4d(sF + 3 * tg.fvol, &tm.B, tc0, tc1, tc2, 0, tbar);
+    }
+  } else
   for (int i = threadIdx.x; i < 6 * tg.fvol; i += blockDim.x) {
     const int c = i / tg.fvol, r = i - c * tg.fvol;
     const int lx = r % tg.fe[0], t = r / tg.fe[0];
@@ -511,6 +534,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) sJ[i] = 0.f;
   cp_async_wait<0>();
   __syncthreads();
+  if (TM) mbar_wait(tbar, 0);  // (after the barrier: thread 0's mbarrier.init is visible)
 
   const int fs1 = tg.fe[0], fs2 = tg.fe[0] * tg.fe[1], fvol = tg.fvol;
   const unsigned lt = lanemask_lt_();
@@ -645,7 +669,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
     const int lt_ = ci / tg.bs[0];
     const int ly = lt_ % tg.bs[1], lz = lt_ / tg.bs[1];
     // node (lx, ly, lz) of the field tile (tile point t <-> node o + t - 1)
-    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1)
+    const float *cF = sF + (D3 ? ((lz + 1) * tg.fe[1] + (ly + 1)) * tg.fe[0] + (lx + 1 + XS)
                                : (lz + 1) * tg.fe[1] + (ly + 1));
     if (!ALT) {  // the cell's gather table, while its resident run is still on its way
       if (lane < GTab<D3>::NP) {
@@ -784,7 +808,7 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       const bool writer = D3 ? ((ln & 1) == 0 && !((ln & 2) && (ln & 4))) : ((ln & 3) == 0);
       if (writer) {
         const int my_off = sRel[D3 ? red12_index(ln) : ((ln >> 2) & 7)];
-        const int node = D3 ? ((lz + 1) * tg.je[1] + (ly + 1)) * tg.je[0] + (lx + 1)
+        const int node = D3 ? ((lz + 1) * tg.je[1] + (ly + 1)) * tg.je[0] + (lx + 1 + XS)
                             : (lz + 1) * tg.je[1] + (ly + 1);
         atomicAdd(&sJ[node + my_off], r);
       }
@@ -792,10 +816,18 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   }
   if (qcnt) drain_queue<D3>(J, tg, gd, gnode0, myQ, sRel + NV, 0, qcnt, lane);
   wk.finish();
+  if (TM) fence_proxy_async();  // this thread's adds to the J tile, for the TMA reduction below
   __syncthreads();
   if (BIG && threadIdx.x == 0) sd.bigflag[tile] = 0;  // taken care of: the flag is the image launch's to set
 
   // ---- flush the J tile (interior + halo nodes) to global J --------------------------------
+  if (TM) {  // one TMA tensor reduction: J[box] += tile (element-wise atomic adds in the L2)
+    if (threadIdx.x == 0) {
+      tma_reduce_add_4d(&tm.J, sJ, tc0, tc1, tc2, 0);
+      bulk_commit();
+      bulk_wait_all();
+    }
+  } else
   for (int i = threadIdx.x; i < 3 * tg.jvol; i += blockDim.x) {
     const float v = sJ[i];
     if (v == 0.f) continue;
@@ -842,7 +874,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false>,        \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false><<<(BIG_) ? big_grid : gd.ntiles, T_, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, CBS_, T_, B_, XC_, BIG_, CT_, false><<<(BIG_) ? big_grid : gd.ntiles, T_, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_, c->tmaps); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the alternating-order scheme runs the general instantiation (run-time tile, optional columns)
@@ -850,7 +882,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   do {                                                                                             \
     PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<D3_, 0, 128, B_, true, BIG_, 0, true>,            \
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_))); \
-    k_push1<D3_, 0, 128, B_, true, BIG_, 0, true><<<(BIG_) ? big_grid : gd.ntiles, 128, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_); \
+    k_push1<D3_, 0, 128, B_, true, BIG_, 0, true><<<(BIG_) ? big_grid : gd.ntiles, 128, SMEM_, s>>>(gd, sd, c->E, c->B, c->J, WS_, c->tmaps); \
     PSC_LAUNCH_CHECK(c);                                                                           \
   } while (0)
   // the image launch, then the launch for the cells it had to leave out (its blocks return at
@@ -870,7 +902,25 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
       PSC_LAUNCH_PUSH1_(D3_, CBS_, T_, 2, false, true, 0, smem_of(T_, ws_big), ws_big);            \
     }                                                                                              \
   } while (0)
-  if (gd.gmode == PSC_SCHEME_ALTERNATING) {
+  // 3-d default block, no optional columns, TMA maps available: tiles staged by TMA
+  const bool tma3 = d3 && c->have_tmaps && !xc && gd.gmode != PSC_SCHEME_ALTERNATING && gd.bs[0] == 4 &&
+                    gd.bs[1] == 4 && gd.bs[2] == 4 && (sd.imgC == 160 || sd.imgC == 128);
+  if (tma3) {
+    const size_t tile_tm = (size_t)(6 * 288 + 3 * 392 + 2 + PSC_MAX_SPECIES + 24 + 27 + 2 * gd.cpb + 2) * sizeof(float);
+    const size_t smem_tm = (size_t)4 * (ws_img + qbytes + tbytes) + tile_tm;
+#define PSC_LAUNCH_PUSH1_TM(CT_)                                                                   \
+  do {                                                                                             \
+    PSC_CUDA_TRY(c, cudaFuncSetAttribute(k_push1<true, 4, 128, PSC_MINB3D, false, false, CT_, false, true>, \
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_tm)); \
+    k_push1<true, 4, 128, PSC_MINB3D, false, false, CT_, false, true><<<gd.ntiles, 128, smem_tm, s>>>( \
+        gd, sd, c->E, c->B, c->J, ws_img, c->tmaps);                                               \
+    PSC_LAUNCH_CHECK(c);                                                                           \
+  } while (0)
+    if (sd.imgC == 160) PSC_LAUNCH_PUSH1_TM(160);
+    else PSC_LAUNCH_PUSH1_TM(128);
+#undef PSC_LAUNCH_PUSH1_TM
+    PSC_LAUNCH_PUSH1_(true, 4, 128, 2, false, true, 0, smem_of(128, ws_big), ws_big);  // the BIG launch as usual
+  } else if (gd.gmode == PSC_SCHEME_ALTERNATING) {
     if (d3) {
       PSC_LAUNCH_PUSH1_ALT(true, 4, false, smem_of(128, ws_img), ws_img);
       PSC_LAUNCH_PUSH1_ALT(true, 2, true, smem_of(128, ws_big), ws_big);
@@ -890,5 +940,42 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
 #undef PSC_LAUNCH_PUSH1
 #undef PSC_LAUNCH_PUSH1_
 #undef PSC_LAUNCH_PUSH1_ALT
+  return PSC_OK;
+}
+
+
+// TMA tensor maps of E, B, J for the 3-d default tiles (psc_bind_fields).  The encoder is a
+// driver entry point fetched through the runtime (the library links no libcuda); if it is not
+// there, or the layout does not qualify, the kernel stages its tiles with plain copies.
+int psc_make_tile_maps(psc_ctx *c) {
+  c->have_tmaps = 0;
+  const GridDesc &gd = c->gd;
+  if (!psc_is3d(gd) || gd.order != 1) return PSC_OK;
+  if (gd.bs[0] != 4 || gd.bs[1] != 4 || gd.bs[2] != 4) return PSC_OK;
+  if (gd.ext[0] % 4 != 0) return PSC_OK;  // global strides must be multiples of 16 bytes
+  typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qr;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn ||
+      qr != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return PSC_OK;
+  }
+  const cuuint64_t dims[4] = {(cuuint64_t)gd.ext[0], (cuuint64_t)gd.ext[1], (cuuint64_t)gd.ext[2], 3};
+  const cuuint64_t strides[3] = {(cuuint64_t)gd.ext[0] * 4, (cuuint64_t)gd.ext[0] * gd.ext[1] * 4,
+                                 (cuuint64_t)gd.comp * 4};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const cuuint32_t fbox[4] = {8, 6, 6, 3}, jbox[4] = {8, 7, 7, 3};
+  struct { CUtensorMap *m; float *p; const cuuint32_t *box; } todo[3] = {
+      {&c->tmaps.E, c->E, fbox}, {&c->tmaps.B, c->B, fbox}, {&c->tmaps.J, c->J, jbox}};
+  for (auto &t : todo) {
+    const CUresult r = ((encode_fn)fn)(t.m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, t.p, dims, strides, t.box, estr,
+                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return PSC_OK;
+  }
+  c->have_tmaps = 1;
   return PSC_OK;
 }
