@@ -231,6 +231,14 @@ int psc_hilbert_order(const int32_t np[3], int32_t *order);
 int psc_balance(int64_t n_patches, const double *loads, int32_t n_ranks, const double *capability,
                 int32_t *count);
 
+/* The assignment psc_balance's counts stand for: owner[i] (HOST, n_patches entries) = rank of the
+ * i-th patch ON THE CURVE (rank 0 takes the first count[0] patches, rank 1 the next count[1], ...).
+ * Comparing the owners before and after a re-balance gives the patches that have to move between
+ * ranks ("dynamically shifting the assignment of patches"); because the cut points
+ * only slide along the curve, a patch moves to a rank whose segment is adjacent on the curve.
+ * count[] must be >= 0 and sum to n_patches (PSC_ERR_INVALID_ARG).  Host only. */
+int psc_balance_owners(int64_t n_patches, int32_t n_ranks, const int32_t *count, int32_t *owner);
+
 /* One time step, Fig. 8: sort, B half, particle loop, B half,
  * J exchange, E full.  State E^{n+1/2}, B^n, x^{n+1/2}, u^n -> E^{n+3/2}, B^{n+1}, x^{n+3/2},
  * u^{n+1}.  Same fields and the same set of particles (up to the rounding of the atomically

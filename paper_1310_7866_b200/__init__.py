@@ -25,7 +25,7 @@ EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
     "psc_field_elems", "psc_particle_capacity", "psc_bind_particles", "psc_particles_sort",
     "psc_push_particles", "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step",
-    "psc_charge_density", "psc_marder", "psc_patch_loads", "psc_hilbert_order", "psc_balance",
+    "psc_charge_density", "psc_marder", "psc_patch_loads", "psc_hilbert_order", "psc_balance", "psc_balance_owners",
     "psc_step_host", "psc_sort_result", "psc_particles_current", "psc_particles_form",
     "psc_particles_gather", "psc_particles_export", "psc_store_info", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
@@ -94,6 +94,7 @@ def lib():
         L.psc_hilbert_order.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.psc_balance.argtypes = [C.c_int64, C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_double),
                                   C.POINTER(C.c_int32)]
+        L.psc_balance_owners.argtypes = [C.c_int64, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         L.psc_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(PscCols),
                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.psc_sort_result.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
@@ -336,3 +337,14 @@ def balance(loads, capability):
     if rc:
         raise PscError(rc, "psc_balance")
     return list(out)
+
+
+def balance_owners(count):
+    """psc_balance_owners: rank of every patch along the curve for the counts psc_balance returned"""
+    r, n = len(count), int(sum(count))
+    cnt = (C.c_int32 * r)(*[int(v) for v in count])
+    out = (C.c_int32 * max(n, 1))()
+    rc = lib().psc_balance_owners(n, r, cnt, out)
+    if rc:
+        raise PscError(rc, "psc_balance_owners")
+    return list(out)[:n]

@@ -196,3 +196,17 @@ extern "C" int psc_balance(int64_t n_patches, const double *loads, int32_t n_ran
   count[n_ranks - 1] = (int32_t)(n_patches - first);  // the last rank takes what is left
   return PSC_OK;
 }
+
+extern "C" int psc_balance_owners(int64_t n_patches, int32_t n_ranks, const int32_t *count, int32_t *owner) {
+  if (!count || !owner || n_ranks < 1 || n_patches < 0) return PSC_ERR_INVALID_ARG;
+  int64_t total = 0;
+  for (int r = 0; r < n_ranks; r++) {
+    if (count[r] < 0) return PSC_ERR_INVALID_ARG;
+    total += count[r];
+  }
+  if (total != n_patches) return PSC_ERR_INVALID_ARG;
+  int64_t i = 0;
+  for (int r = 0; r < n_ranks; r++)
+    for (int k = 0; k < count[r]; k++) owner[i++] = r;
+  return PSC_OK;
+}
