@@ -40,6 +40,9 @@
 #ifndef PSC_MINB2D
 #define PSC_MINB2D 6  // blocks per SM of the default 2-d kernel
 #endif
+#ifndef PSC_THREADS2D
+#define PSC_THREADS2D 128  // threads per block of the default 2-d kernel
+#endif
 #ifndef PSC_MINB3D
 #define PSC_MINB3D 5  // ... of the default 3-d kernel
 #endif
@@ -934,7 +937,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
     else PSC_LAUNCH_PUSH1(true, 0, 128, 4, false);
   } else {
     const bool def = gd.bs[1] == 8 && gd.bs[2] == 8;
-    if (def) PSC_LAUNCH_PUSH1(false, 8, 128, PSC_MINB2D, true);
+    if (def) PSC_LAUNCH_PUSH1(false, 8, PSC_THREADS2D, PSC_MINB2D, true);
     else PSC_LAUNCH_PUSH1(false, 0, 128, 5, false);
   }
 #undef PSC_LAUNCH_PUSH1
