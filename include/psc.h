@@ -281,7 +281,9 @@ int psc_particles_gather(psc_ctx *ctx, void *stream, const psc_particle_cols *ds
 int psc_particles_export(psc_ctx *ctx, void *stream);
 /* Synchronises `stream`; info[0] = largest cell count at the last layout, [1] = slots of the
  * store in use, [2] = re-layouts since psc_create, [3] = particles spilled by the last push,
- * [4] = slots of the per-warp cell image of the particle kernels.  Host array. */
+ * [4] = slots of the per-warp cell image of the particle kernels, [5] = 1 if the last particle
+ * push staged its field / J tiles by TMA tensor copies (3-d, order 1, default block, no optional
+ * columns).  Host array. */
 int psc_store_info(psc_ctx *ctx, void *stream, int64_t info[8]);
 /* Synchronises `stream`, returns and keeps the sticky flags. */
 int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);

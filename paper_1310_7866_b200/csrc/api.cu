@@ -483,6 +483,7 @@ int psc_store_info(psc_ctx *c, void *stream, int64_t info[8]) {
   info[2] = dw[PSC_DW_RELAYOUTS];
   info[3] = dw[PSC_DW_SPILL];
   info[4] = c->bufC;
+  info[5] = c->used_tma;
   return PSC_OK;
 }
 

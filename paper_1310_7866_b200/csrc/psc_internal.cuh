@@ -141,6 +141,7 @@ struct psc_ctx {
   GridDesc gd;
   TileMaps tmaps;
   int have_tmaps;  // tmaps describe the bound E, B, J (3-d, default 4x4x4 block, x extent a multiple of 4)
+  int used_tma;    // the last psc_push_particles staged its tiles by TMA tensor copies (psc_store_info)
   Prof prof;
   float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
   float *E, *B, *J;

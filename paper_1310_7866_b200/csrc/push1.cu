@@ -908,6 +908,7 @@ int psc_push_order1(psc_ctx *c, cudaStream_t s) {
   // 3-d default block, no optional columns, TMA maps available: tiles staged by TMA
   const bool tma3 = d3 && c->have_tmaps && !xc && gd.gmode != PSC_SCHEME_ALTERNATING && gd.bs[0] == 4 &&
                     gd.bs[1] == 4 && gd.bs[2] == 4 && (sd.imgC == 160 || sd.imgC == 128);
+  c->used_tma = tma3 ? 1 : 0;
   if (tma3) {
     const size_t tile_tm = (size_t)(6 * 288 + 3 * 392 + 2 + PSC_MAX_SPECIES + 24 + 27 + 2 * gd.cpb + 2) * sizeof(float);
     const size_t smem_tm = (size_t)4 * (ws_img + qbytes + tbytes) + tile_tm;

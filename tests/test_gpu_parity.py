@@ -15,10 +15,10 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-5
 
 
-def _sim(pl, block=(0, 0, 0)):
+def _sim(pl, block=(0, 0, 0), **kw):
     from paper_1310_7866_b200.harness import Simulation
 
-    return Simulation(pl, block=block)
+    return Simulation(pl, block=block, **kw)
 
 
 def _small(kind):
@@ -382,6 +382,33 @@ def test_big_cell_whole_chunks_leave():
         for c in ("ux", "uy", "uz"):
             assert np.abs(g1[c][o] - st[c]).max() < TOL
         assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+
+
+def test_3d_tma_tile_path_matches_oracle():
+    """the 3-d order-1 kernel with its tiles staged by TMA tensor copies (no optional columns, the
+    default 4x4x4 block, a cell image of 128 / 160 slots): J, E, B after five steps against the
+    oracle, and the same run with the id column bound (plain 4-byte staging) for comparison"""
+    pl = psc_inputs.thermal((16, 16, 16), 35, seed=31, name="3d-tma")
+    smooth_fields(pl, 0.05, seed=8)
+    sim = _sim(pl, with_id=False)
+    sim.step(5)
+    assert sim.psc.status() == 0
+    info = sim.psc.store_info()
+    assert info["tma_tiles"] == 1 and info["image_slots"] in (128, 160)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], 5)
+    for got, want in ((sim.J, J), (sim.E, E), (sim.B, B)):
+        g = sim.interior(got).cpu().numpy()
+        for c in range(3):
+            assert np.abs(g[c] - want[c]).max() <= TOL * np.abs(want[c]).max()
+    sim2 = _sim(pl, with_id=True)
+    sim2.step(5)
+    assert sim2.psc.store_info()["tma_tiles"] == 0
+    for a, b in ((sim.J, sim2.J), (sim.E, sim2.E)):
+        ga, gb = sim.interior(a).cpu().numpy(), sim2.interior(b).cpu().numpy()
+        assert np.abs(ga - gb).max() <= TOL * np.abs(gb).max()
 
 
 # ------------------------------------------------------------------------------------------------
