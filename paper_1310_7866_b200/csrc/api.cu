@@ -134,6 +134,11 @@ int psc_create(const psc_params *p, psc_ctx **out) {
   gd.dt = p->dt;
   gd.inv_dV = (float)(1.0 / dV);
   for (int d = 0; d < 3; d++) gd.cur[d] = (float)((double)p->dx[d] / ((double)p->dt * dV));
+  for (int d = 0; d < 3; d++) {
+    gd.bsh[d] = -1;
+    for (int k = 0; k < 12; k++)
+      if (gd.bs[d] == (1 << k)) gd.bsh[d] = k;
+  }
   gd.cpb = gd.bs[0] * gd.bs[1] * gd.bs[2];
   gd.nkeys = (int)nk;
   gd.ntiles = gd.nb[0] * gd.nb[1] * gd.nb[2];

@@ -21,6 +21,7 @@ struct GridDesc {
   float cur[3];      // dx[d] / (dt * dV): factor of the in-plane VB / Esirkepov current
   float inv_dV;
   int bs[3], nb[3];  // sort block (supercell) size in cells and number of blocks
+  int bsh[3];        // log2 of bs[d] if it is a power of two, else -1 (cell_key without divisions)
   int cpb;           // cells per block
   int nkeys;         // total cells
   int ntiles;        // number of blocks

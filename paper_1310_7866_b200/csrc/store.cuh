@@ -91,12 +91,27 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // cell key (block-major, cell-minor) of periodic cell coordinates
 __device__ __forceinline__ int wrap_cell(int c, int n) { return c < 0 ? c + n : (c >= n ? c - n : c); }
 __device__ __forceinline__ int cell_key(const GridDesc &gd, int cx, int cy, int cz) {
+  if ((gd.bsh[0] | gd.bsh[1] | gd.bsh[2]) >= 0) {  // power-of-two blocks (the defaults): shifts
+    const int b0 = cx >> gd.bsh[0], b1 = cy >> gd.bsh[1], b2 = cz >> gd.bsh[2];
+    const int l0 = cx & (gd.bs[0] - 1), l1 = cy & (gd.bs[1] - 1), l2 = cz & (gd.bs[2] - 1);
+    return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (((l2 << gd.bsh[1]) + l1) << gd.bsh[0]) + l0;
+  }
   const int b0 = cx / gd.bs[0], b1 = cy / gd.bs[1], b2 = cz / gd.bs[2];
   const int l0 = cx - b0 * gd.bs[0], l1 = cy - b1 * gd.bs[1], l2 = cz - b2 * gd.bs[2];
   return ((b2 * gd.nb[1] + b1) * gd.nb[0] + b0) * gd.cpb + (l2 * gd.bs[1] + l1) * gd.bs[0] + l0;
 }
 // key -> cell coordinates
 __device__ __forceinline__ void key_to_cell(const GridDesc &gd, int k, int c[3]) {
+  if ((gd.bsh[0] | gd.bsh[1] | gd.bsh[2]) >= 0) {  // power-of-two blocks: shifts for the in-block part
+    const int sh01 = gd.bsh[0] + gd.bsh[1];
+    const int b = k >> (sh01 + gd.bsh[2]), l = k & (gd.cpb - 1);
+    const int b0 = b % gd.nb[0], br = b / gd.nb[0];
+    const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
+    c[0] = (b0 << gd.bsh[0]) + (l & (gd.bs[0] - 1));
+    c[1] = (b1 << gd.bsh[1]) + ((l >> gd.bsh[0]) & (gd.bs[1] - 1));
+    c[2] = (b2 << gd.bsh[2]) + (l >> sh01);
+    return;
+  }
   const int b = k / gd.cpb, l = k - b * gd.cpb;
   const int b0 = b % gd.nb[0], br = b / gd.nb[0];
   const int b1 = br % gd.nb[1], b2 = br / gd.nb[1];
