@@ -283,7 +283,8 @@ int psc_particles_export(psc_ctx *ctx, void *stream);
  * store in use, [2] = re-layouts since psc_create, [3] = particles spilled by the last push,
  * [4] = slots of the per-warp cell image of the particle kernels, [5] = 1 if the last particle
  * push staged its field / J tiles by TMA tensor copies (3-d, order 1, default block, no optional
- * columns).  Host array. */
+ * columns), [6] = spilled particles that were filed straight into their cell without a re-layout
+ * since psc_create.  Host array. */
 int psc_store_info(psc_ctx *ctx, void *stream, int64_t info[8]);
 /* Synchronises `stream`, returns and keeps the sticky flags. */
 int psc_status(psc_ctx *ctx, void *stream, uint32_t *flags);

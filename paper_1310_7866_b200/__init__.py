@@ -282,7 +282,7 @@ class Psc:
         a = (C.c_int64 * 8)()
         self._check(lib().psc_store_info(self._h, _stream(stream), a), "psc_store_info")
         return {"max_count": int(a[0]), "slots": int(a[1]), "relayouts": int(a[2]),
-                "spilled": int(a[3]), "image_slots": int(a[4]), "tma_tiles": int(a[5])}
+                "spilled": int(a[3]), "image_slots": int(a[4]), "tma_tiles": int(a[5]), "inserted": int(a[6])}
 
     def particles_export(self, stream=None):
         self._check(lib().psc_particles_export(self._h, _stream(stream)), "psc_particles_export")

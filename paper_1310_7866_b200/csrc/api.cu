@@ -489,6 +489,7 @@ int psc_store_info(psc_ctx *c, void *stream, int64_t info[8]) {
   info[3] = dw[PSC_DW_SPILL];
   info[4] = c->bufC;
   info[5] = c->used_tma;
+  info[6] = dw[PSC_DW_INSERTED];
   return PSC_OK;
 }
 

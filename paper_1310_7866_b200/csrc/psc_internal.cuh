@@ -129,6 +129,7 @@ enum {
   PSC_DW_SLOTS = 4,    // slots used by the last layout
   PSC_DW_RELAYOUTS = 5,  // number of re-layouts performed
   PSC_DW_NBIG = 6,     // [2]: tiles with a cell left to the BIG launch, by step parity
+  PSC_DW_INSERTED = 8, // spilled particles filed straight into their cell (no re-layout needed), cumulative
   PSC_DW_COUNT = 16
 };
 

@@ -891,6 +891,9 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const int mx = (int)dw[PSC_DW_MAXCNT];
   int C = (mx + mx / 8 + 24 + 31) / 32 * 32;  // 64, 96, ..., 256
   c->bufC = C < 64 ? 64 : (C > 256 ? 256 : C);
+  // the order-2 kernel is bound by registers (2 blocks/SM), not by shared memory: it takes the largest
+  // image, so that cells which fill up while a run clumps stay on the image path
+  if (c->gd.order == 2) c->bufC = 256;
   if ((int64_t)dw[PSC_DW_SLOTS] > c->capacity) return PSC_ERR_WORKSPACE;
   return PSC_OK;
 }
@@ -944,10 +947,85 @@ __device__ void relayout_chain(const RelayoutArgs &a) {
   k_relayout_done<<<1, 32, 0, ts>>>(a.dw);
 }
 
-__global__ void k_relayout_gate(RelayoutArgs a) {
+// A spilled particle (the 33rd leaver of a cell in one step, mostly) does not need a re-layout if
+// its destination cell has a free slot: one block files the spill list straight into the cells
+// and keeps, compacted at the front of the list, only those that found no room.
+constexpr int SPILL_INSERT_MAX = 1 << 16;  // longer lists (mass migration) go to the re-layout at once
+template <bool D3>
+__global__ void __launch_bounds__(256) k_spill_insert(RelayoutArgs a) {
+  __shared__ int nfail;
+  const int ns = min(*a.spill.count, a.spill.cap);
+  if (threadIdx.x == 0) nfail = 0;
+  __syncthreads();
+  for (int i0 = 0; i0 < ns; i0 += blockDim.x) {
+    const int i = i0 + threadIdx.x;
+    const bool have = i < ns;
+    XRec r;
+    int key = 0, id = 0;
+    r.a = r.b = make_uint4(0, 0, 0, 0);
+    if (have) {
+      r = a.spill.rec[i];
+      key = a.spill.key[i];
+      if (a.spill.id) id = a.spill.id[i];
+    }
+    __syncthreads();  // the whole chunk is read before anything is written over the list's front
+    bool fail = false;
+    if (have) {
+      const int slot = atomicAdd(&a.cnt[key], 1);
+      if (slot < a.base[key + 1] - a.base[key]) {
+        const size_t o = (size_t)a.base[key] + slot;
+        const float w[8] = {__uint_as_float(r.a.x), __uint_as_float(r.a.y), __uint_as_float(r.a.z),
+                            __uint_as_float(r.a.w), __uint_as_float(r.b.x), __uint_as_float(r.b.y),
+                            __uint_as_float(r.b.z), __uint_as_float(r.b.w)};
+        if (D3) a.cur.x[o] = w[0];
+        else if (a.cur.x) a.cur.x[o] = w[7];
+        a.cur.y[o] = D3 ? w[1] : w[0];
+        a.cur.z[o] = D3 ? w[2] : w[1];
+        a.cur.ux[o] = D3 ? w[3] : w[2];
+        a.cur.uy[o] = D3 ? w[4] : w[3];
+        a.cur.uz[o] = D3 ? w[5] : w[4];
+        a.cur.qw[o] = D3 ? w[6] : w[5];
+        a.cur.sp[o] = __float_as_int(D3 ? w[7] : w[6]);
+        if (a.cur.id) a.cur.id[o] = id;
+      } else {
+        atomicSub(&a.cnt[key], 1);
+        fail = true;
+      }
+    }
+    if (fail) {
+      const int f = atomicAdd(&nfail, 1);
+      a.spill.rec[f] = r;
+      a.spill.key[f] = key;
+      if (a.spill.id) a.spill.id[f] = id;
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    a.dw[PSC_DW_INSERTED] += (uint32_t)(ns - nfail);
+    *a.spill.count = nfail;
+  }
+}
+
+// second look at the spill counter, after the insertion: what is left needs the re-layout
+__global__ void k_relayout_gate2(RelayoutArgs a) {
   if (threadIdx.x != 0 || a.dw[PSC_DW_SPILL] == 0) return;
   if (a.gd.n[0] > 1) relayout_chain<true>(a);
   else relayout_chain<false>(a);
+}
+
+__global__ void k_relayout_gate(RelayoutArgs a) {
+  if (threadIdx.x != 0) return;
+  const uint32_t ns = a.dw[PSC_DW_SPILL];
+  if (ns == 0) return;
+  if (ns <= (uint32_t)SPILL_INSERT_MAX && ns <= (uint32_t)a.spill.cap) {
+    if (a.gd.n[0] > 1) k_spill_insert<true><<<1, 256, 0, cudaStreamTailLaunch>>>(a);
+    else k_spill_insert<false><<<1, 256, 0, cudaStreamTailLaunch>>>(a);
+    k_relayout_gate2<<<1, 32, 0, cudaStreamTailLaunch>>>(a);
+  } else if (a.gd.n[0] > 1) {
+    relayout_chain<true>(a);
+  } else {
+    relayout_chain<false>(a);
+  }
 }
 
 }  // namespace

@@ -342,6 +342,47 @@ def test_store_spill_relayout_and_big_cells(order):
     assert info["relayouts"] >= 1 and info["max_count"] > 256
 
 
+def test_spilled_leavers_are_filed_without_a_relayout():
+    """more than 32 particles leave one cell in a step (the exchange row holds 32 records): the rest
+    goes to the spill list, and because their destination cell has room the next step files them
+    straight into it -- no re-layout.  Five steps against the oracle, particle by particle."""
+    pl = psc_inputs.thermal((1, 16, 16), 12, seed=37, name="row-overflow")
+    n = pl.y.numel()
+    vy = 0.33 * pl.dx[1] / pl.dt
+    gam = 1.0 / np.sqrt(1.0 - vy * vy)
+    pl.qw = pl.qw * 1e-2
+    g = torch.Generator().manual_seed(6)
+    extra = 38
+    for k in ("x", "ux", "uz"):
+        setattr(pl, k, torch.cat([getattr(pl, k), torch.zeros(extra)]))
+    pl.y = torch.cat([pl.y, 5.9 + 0.0999 * torch.rand(extra, generator=g)])
+    pl.z = torch.cat([pl.z, 9.2 + 0.6 * torch.rand(extra, generator=g)])
+    pl.uy = torch.cat([pl.uy, torch.full((extra,), float(gam * vy))])
+    pl.qw = torch.cat([pl.qw, torch.full((extra,), float(pl.qw[0]))])
+    pl.species = torch.cat([pl.species, torch.zeros(extra, dtype=torch.int32)])
+    pl.id = torch.arange(n + extra, dtype=torch.int32)
+    sim = _sim(pl)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for it in range(5):
+        orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], 1)
+        sim.step(1)
+        assert sim.psc.status() == 0
+        g1 = gpu_state(sim)
+        assert np.array_equal(np.sort(g1["id"]), np.arange(n + extra))
+        o = order_by_id(g1["id"], st["id"])
+        _, py, pz = positions_f64(g1, pl)
+        assert periodic_dist(py[o], st["y"], L[1]).max() < 1e-4
+        assert periodic_dist(pz[o], st["z"], L[2]).max() < 1e-4
+        for c in ("ux", "uy", "uz"):
+            assert np.abs(g1[c][o] - st[c]).max() < TOL
+        assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+    info = sim.psc.store_info()
+    assert info["inserted"] >= 2 and info["relayouts"] == 0
+
+
 def test_big_cell_whole_chunks_leave():
     """a cell of the BIG launch (more particles than the image holds) whose particles ALL cross
     the same face in one step: batches of 32 leavers against a 24-entry crosser queue (2-d) -- the
