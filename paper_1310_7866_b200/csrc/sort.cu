@@ -20,11 +20,13 @@
 // PAPER.md:597-603 ("a particle moves at most one cell per step", "reorder on load"): between
 // pushes NO sort runs.  The push kernels keep every cell's particles dense in the cell's own
 // slots and hand the few cell-changers over through the exchange rows (store.cuh).  Only when a
-// push had to spill (an exchange row or a cell ran out of room) the next step re-lays the store
-// out: k_tot / scan / k_gather flatten residents + exchange records + spill list into the other
+// push had to spill (an exchange row or a cell ran out of room) something happens between two
+// pushes: k_spill_insert files the spilled particles straight into their destination cells where
+// these have a free slot; if some are left (cells that are really full) the store is re-laid out:
+// k_tot / scan / k_gather flatten residents + exchange records + spill list into the other
 // column set, and steps 1-5 (without 4: the order inside a cell is immaterial, A17)
-// bring them back.  Whether that is needed is known on the device only, so these launches carry a
-// condition word and return at once when it is zero.
+// bring them back.  Whether any of that is needed is known on the device only: one gate kernel
+// looks at the spill counter and launches the rest from the device.
 #include <limits.h>
 #include <math.h>
 

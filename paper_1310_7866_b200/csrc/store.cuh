@@ -28,7 +28,7 @@
 // launch of the same kernel in its BIG form, which streams such cells straight from and to global
 // memory with an in-place compaction (rare; correct for any size; tiles without such a cell leave
 // at once).  A particle that finds no room (row or cell full) goes to the spill list; the next
-// step then re-lays the store out before pushing (sort.cu).
+// step files it into its cell if that has room by then, else re-lays the store out (sort.cu).
 #pragma once
 #include "push_common.cuh"
 
