@@ -483,6 +483,7 @@ int psc_store_info(psc_ctx *c, void *stream, int64_t info[8]) {
   PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   PSC_CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
   for (int i = 0; i < 8; i++) info[i] = 0;
+  if (c->state == PSC_STATE_STORE) psc_refresh_image_size(c, dw);
   info[0] = dw[PSC_DW_MAXCNT];
   info[1] = dw[PSC_DW_SLOTS];
   info[2] = dw[PSC_DW_RELAYOUTS];
@@ -495,8 +496,11 @@ int psc_store_info(psc_ctx *c, void *stream, int64_t info[8]) {
 
 int psc_status(psc_ctx *c, void *stream, uint32_t *flags) {
   if (!c || !flags) return PSC_ERR_INVALID_ARG;
-  PSC_CUDA_TRY(c, cudaMemcpyAsync(flags, c->d_flags, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+  uint32_t dw[PSC_DW_COUNT];
+  PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
   PSC_CUDA_TRY(c, cudaStreamSynchronize((cudaStream_t)stream));
+  *flags = dw[PSC_DW_FLAGS];
+  if (c->state == PSC_STATE_STORE) psc_refresh_image_size(c, dw);  // (the host has the block anyway)
   return PSC_OK;
 }
 

@@ -222,6 +222,7 @@ int psc_sort_cell_idx(psc_ctx *c, cudaStream_t s);
 // row, then the spill list) into `dst`, keys into `key` (may be null); to_abs: positions absolute
 int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cudaStream_t s);
 StoreDesc psc_store_desc(const psc_ctx *c);
+void psc_refresh_image_size(psc_ctx *c, const uint32_t *dw);  // dw: host copy of the status block
 // push1.cu / push2.cu
 int psc_push_order1(psc_ctx *c, cudaStream_t s);
 int psc_make_tile_maps(psc_ctx *c);  // after psc_bind_fields; sets have_tmaps (0 if TMA maps are not applicable)

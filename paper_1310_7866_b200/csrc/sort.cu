@@ -847,6 +847,20 @@ int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cud
   return gather_store(c, dst, key, to_abs, c->key + c->np /* scratch word behind key[] */, s, nullptr);
 }
 
+// Size of the per-warp cell image of the particle kernels: the largest cell of the last layout
+// plus room for its arrivals.  Called whenever the host has the status block anyway (after the
+// general sort, in psc_status / psc_store_info): a device-side re-layout of a run that clumps
+// raises the largest count, and the image follows at the next such call (it never shrinks).
+void psc_refresh_image_size(psc_ctx *c, const uint32_t *dw) {
+  const int mx = (int)dw[PSC_DW_MAXCNT];
+  int C = (mx + mx / 8 + 24 + 31) / 32 * 32;  // 64, 96, ..., 256
+  C = C < 64 ? 64 : (C > 256 ? 256 : C);
+  // the order-2 kernel is bound by registers (2 blocks/SM), not by shared memory: it takes the largest
+  // image, so that cells which fill up while a run clumps stay on the image path
+  if (c->gd.order == 2) C = 256;
+  if (C > c->bufC) c->bufC = C;
+}
+
 // general counting sort: any state in, the cell store (stable inside every cell) out
 int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   const GridDesc &gd = c->gd;
@@ -890,12 +904,8 @@ int psc_sort_general(psc_ctx *c, cudaStream_t s) {
   uint32_t dw[PSC_DW_COUNT];
   PSC_CUDA_TRY(c, cudaMemcpyAsync(dw, c->d_flags, sizeof(dw), cudaMemcpyDeviceToHost, s));
   PSC_CUDA_TRY(c, cudaStreamSynchronize(s));
-  const int mx = (int)dw[PSC_DW_MAXCNT];
-  int C = (mx + mx / 8 + 24 + 31) / 32 * 32;  // 64, 96, ..., 256
-  c->bufC = C < 64 ? 64 : (C > 256 ? 256 : C);
-  // the order-2 kernel is bound by registers (2 blocks/SM), not by shared memory: it takes the largest
-  // image, so that cells which fill up while a run clumps stay on the image path
-  if (c->gd.order == 2) c->bufC = 256;
+  c->bufC = 0;
+  psc_refresh_image_size(c, dw);
   if ((int64_t)dw[PSC_DW_SLOTS] > c->capacity) return PSC_ERR_WORKSPACE;
   return PSC_OK;
 }
