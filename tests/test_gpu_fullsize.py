@@ -173,3 +173,46 @@ def test_full_size_step_counts(cfg):
     assert np.abs(r1 - r0).max() < 1e-4 * scale_rho, np.abs(r1 - r0).max() / scale_rho
     info = sim.psc.store_info()
     assert info["spilled"] == 0 or info["relayouts"] > 0
+
+
+def test_config3_full_size_ten_steps_match_oracle_by_id():
+    """config 3 at BASELINE size (1x512x1024, 14.6 M particles, the 11x density contrast of the
+    double Harris sheet) in a closed loop: ten psc_step against ten oracle steps of the WHOLE
+    system, every particle matched by id (positions within 1e-5 of the domain and 1e-4 cell,
+    momenta within 1e-5 of the species rms), J and E within 1e-5 of the component max-norm, B
+    within 1e-5 of the field's max-norm."""
+    from paper_1310_7866_b200.harness import Simulation
+    from tests.util import (gpu_state, oracle_state, periodic_dist, positions_f64, rel_fieldnorm,
+                            rel_maxnorm)
+
+    pl = psc_inputs.make_config(3)                       # host tensors: the oracle needs them all
+    sim = Simulation(pl, with_id=True, with_x=False)
+    orc = oracle_for(pl)
+    st, E, B = oracle_state(pl)
+    J = orc.zeros_field()
+    nsteps = 10
+    orc.step(E, B, J, st["x"], st["y"], st["z"], st["ux"], st["uy"], st["uz"], st["qw"], st["species"], nsteps)
+    sim.step(nsteps)
+    assert sim.psc.status() == 0
+    g1 = gpu_state(sim)
+    o1 = np.argsort(g1["id"], kind="stable")
+    assert np.array_equal(g1["id"][o1], st["id"])
+    p64 = positions_f64(g1, pl)
+    L = [pl.n[d] * pl.dx[d] for d in range(3)]
+    for d, c in ((1, "y"), (2, "z")):
+        dist = periodic_dist(p64[d][o1], st[c], L[d])
+        assert dist.max() < 1e-4 * pl.dx[d]
+        assert (dist / L[d]).max() < TOL
+    for s in range(len(pl.q)):
+        m = st["species"] == s
+        rms = np.sqrt(np.mean(st["ux"][m] ** 2 + st["uy"][m] ** 2 + st["uz"][m] ** 2))
+        for c in ("ux", "uy", "uz"):
+            assert np.abs(g1[c][o1][m] - st[c][m]).max() / rms < TOL
+    assert rel_maxnorm(sim.interior(sim.J).cpu().numpy(), J) < TOL
+    # E and B: 1e-5 of the FIELD's max-norm (north_star), 1e-4 per component: E_x (max 1e-3) is
+    # advanced by differences of B_y (0.063), whose fp32 ulp (3.7e-9) times dt times ten steps is
+    # 3e-8 = 3e-5 of E_x but 8e-6 of the field; likewise B_x, B_z (1e-3) next to B_y
+    assert rel_fieldnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
+    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < 10 * TOL
+    assert rel_fieldnorm(sim.interior(sim.B).cpu().numpy(), B) < TOL
+    assert rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B) < 10 * TOL
