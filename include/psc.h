@@ -63,6 +63,7 @@ extern "C" {
 #define PSC_ERR_CUDA (-6)
 #define PSC_ERR_UNSUPPORTED (-7)
 #define PSC_ERR_WORKSPACE (-8)
+#define PSC_ERR_SCRATCH_LIMIT (-9) /* psc_marder_static: the grid does not fit the fixed scratch array */
 
 #define PSC_E 0
 #define PSC_B 1
@@ -201,6 +202,30 @@ int psc_charge_density(psc_ctx *ctx, void *stream, float *rho);
  * diffusion * sum_d 4/dx_d^2 <= 1 (PSC_ERR_CFL).  Requires the internal form.  Uses one scratch
  * field the context allocates on first use (freed by psc_destroy). */
 int psc_marder(psc_ctx *ctx, void *stream, float diffusion, int iters);
+
+/* psc_marder for callers that cannot allocate device memory at the point where they apply the
+ * correction.  psc_marder cudaMalloc's its scratch field on first use; that is not an option for
+ * a time loop that runs while another host thread captures a CUDA graph in the global capture
+ * mode (cudaMalloc is forbidden there), for one that cannot take cudaMalloc's implicit
+ * device-wide synchronisation, or inside a process whose own pool already holds all of the HBM
+ * so that a raw cudaMalloc from a library fails.  This call does the same arithmetic with the same
+ * kernels and the same arguments, results and error codes, but keeps rho and the residual in a
+ * fixed array that is part of the library's device image, and calls no cudaMalloc, cudaFree or
+ * any other allocating routine.
+ *   - Limit: the grid including ghosts, ex * ey * ez (psc_field_elems / 3), must not exceed
+ *     PSC_MARDER_STATIC_MAX_POINTS (e.g. 64^3 or 1 x 512 x 512 interior cells); a larger grid is
+ *     refused with PSC_ERR_SCRATCH_LIMIT before anything is enqueued.  Use psc_marder there.
+ *   - Cost: every GPU on which the library is loaded holds the array (3 * 4 *
+ *     PSC_MARDER_STATIC_MAX_POINTS bytes = 3.75 MiB) until the process exits.
+ *   - The device that owns the bound buffers must be current.  The first call on each device looks
+ *     up the array's address on that device (cudaGetSymbolAddress, which may load the module
+ *     there); make that first call during set-up, before any stream capture begins.
+ *   - The array is shared by every context and every call on a device and keeps the last call's
+ *     contents; the call zeroes what must start at zero on `stream`.  Two calls whose device work
+ *     can overlap (different streams, different contexts, different host threads) race on it:
+ *     order them yourself.  Calls on one stream are ordered by the stream. */
+#define PSC_MARDER_STATIC_MAX_POINTS 327680
+int psc_marder_static(psc_ctx *ctx, void *stream, float diffusion, int iters);
 
 /* ---- patch-based load balancing (Appendix A) -------------
  * The domain is cut into many more patches than processing elements; the patches are enumerated

@@ -16,6 +16,8 @@ PSC_OK = 0
 PSC_E, PSC_B, PSC_J = 0, 1, 2
 PSC_F_OOB, PSC_F_NAN, PSC_F_SPECIES, PSC_F_OVERFLOW = 1, 4, 8, 32
 PSC_GHOST = 2
+PSC_ERR_SCRATCH_LIMIT = -9
+MARDER_STATIC_MAX_POINTS = 327680
 PSC_SCHEME_STANDARD, PSC_SCHEME_ALTERNATING = 0, 1
 PHASES = {"sort": 0, "push": 1, "j_zero": 2, "field_b": 3, "j_exchange": 4, "field_e": 5,
           "sort_count": 6, "sort_scan": 7, "sort_rank": 8, "sort_reorder": 9, "marder": 10}
@@ -25,7 +27,7 @@ EXPORTS = [
     "psc_create", "psc_destroy", "psc_workspace_bytes", "psc_bind_workspace", "psc_bind_fields",
     "psc_field_elems", "psc_particle_capacity", "psc_bind_particles", "psc_particles_sort",
     "psc_push_particles", "psc_push_fields", "psc_exchange_j", "psc_fill_ghosts", "psc_step",
-    "psc_charge_density", "psc_marder", "psc_patch_loads", "psc_hilbert_order", "psc_balance", "psc_balance_owners",
+    "psc_charge_density", "psc_marder", "psc_marder_static", "psc_patch_loads", "psc_hilbert_order", "psc_balance", "psc_balance_owners",
     "psc_step_host", "psc_sort_result", "psc_particles_current", "psc_particles_form",
     "psc_particles_gather", "psc_particles_export", "psc_store_info", "psc_status", "psc_launch_count",
     "psc_last_cuda_error", "psc_set_option", "psc_profile", "psc_strerror", "psc_version",
@@ -89,6 +91,7 @@ def lib():
         L.psc_fill_ghosts.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.psc_charge_density.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.psc_marder.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int]
+        L.psc_marder_static.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_int]
         L.psc_patch_loads.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_int32), C.c_void_p,
                                       C.POINTER(C.c_int32)]
         L.psc_hilbert_order.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
@@ -237,6 +240,13 @@ class Psc:
     def marder(self, diffusion, iters=1, stream=None):
         """psc_marder: E += diffusion * grad+ (div- E - rho), `iters` passes (PAPER.md:206)"""
         self._check(lib().psc_marder(self._h, _stream(stream), float(diffusion), int(iters)), "psc_marder")
+
+    def marder_static(self, diffusion, iters=1, stream=None):
+        """psc_marder_static: psc_marder with its scratch in a fixed device array of the library, for
+        callers that cannot allocate device memory when they apply the correction (include/psc.h:
+        grids up to MARDER_STATIC_MAX_POINTS points incl. ghosts; overlapping calls race)"""
+        self._check(lib().psc_marder_static(self._h, _stream(stream), float(diffusion), int(iters)),
+                    "psc_marder_static")
 
     def patch_loads(self, patch_blocks, loads, stream=None):
         """psc_patch_loads: particles + cells of every patch into the device int64

@@ -66,6 +66,7 @@ const char *psc_strerror(int code) {
     case PSC_ERR_CUDA: return "CUDA runtime error (see psc_last_cuda_error)";
     case PSC_ERR_UNSUPPORTED: return "configuration not supported by this build";
     case PSC_ERR_WORKSPACE: return "workspace too small";
+    case PSC_ERR_SCRATCH_LIMIT: return "grid larger than the fixed scratch array of psc_marder_static (PSC_MARDER_STATIC_MAX_POINTS)";
     default: return "unknown error";
   }
 }

@@ -17,6 +17,8 @@
 // added record by record.
 #include "store.cuh"
 
+#include <mutex>
+
 namespace {
 
 constexpr int MT = 256;
@@ -209,6 +211,92 @@ int psc_marder_pass(psc_ctx *c, float D, int iters, cudaStream_t s) {
     k_gauss_residual<<<blocks, MT, 0, s>>>(gd, c->E, c->rho, f);
     PSC_LAUNCH_CHECK(c);
     k_marder_apply<<<blocks, MT, 0, s>>>(gd, c->E, f, D);
+    PSC_LAUNCH_CHECK(c);
+  }
+  return PSC_OK;
+}
+
+// ---- psc_marder_static: the same correction for callers that must not allocate --------------------
+//
+// psc_marder keeps rho and f in a field the context cudaMalloc's on its first use.  Some users of
+// this library cannot afford that call where they apply the correction: a time loop that runs while
+// another host thread captures a CUDA graph in the global capture mode (cudaMalloc is prohibited
+// there and breaks the capture), a loop in which the implicit device-wide synchronisation of
+// cudaMalloc would stall every other stream, or a process whose own memory pool (PyTorch's caching
+// allocator, say) has already taken all of the HBM, so that a raw cudaMalloc from inside a library
+// fails.  For them the scratch lives in the array below, which is part of the library's device
+// image: every GPU that loads libpsc_b200.so holds these 3.75 MiB from then until the process
+// exits, whether psc_marder_static is ever called or not.
+//
+// In host code the identifier g_marder_scratch is only a handle of the symbol, not a device
+// address (passing it to a kernel would make the kernel fault, or scribble over host memory on a
+// system where the GPU can reach it), so the host asks the runtime for the address once per
+// device, with that device current, and hands the kernels that pointer.
+static __device__ __align__(256) float g_marder_scratch[3 * PSC_MARDER_STATIC_MAX_POINTS];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+float *g_marder_scratch_addr[STATIC_MAX_DEVICES];  // device address of the array on device i (0: not asked yet)
+std::mutex g_marder_scratch_mu;
+
+// Address of g_marder_scratch on the CURRENT device.  The first call on a device resolves the
+// symbol (which may make the runtime load the module on that device); later calls read the table.
+int marder_static_scratch(psc_ctx *c, float **out) {
+  int dev = -1;
+  PSC_CUDA_TRY(c, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return PSC_ERR_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_marder_scratch_mu);
+  if (!g_marder_scratch_addr[dev]) {
+    float *p = nullptr;
+    PSC_CUDA_TRY(c, cudaGetSymbolAddress((void **)&p, g_marder_scratch));
+    if (!p) return PSC_ERR_CUDA;
+    g_marder_scratch_addr[dev] = p;
+  }
+  *out = g_marder_scratch_addr[dev];
+  return PSC_OK;
+}
+
+}  // namespace
+
+extern "C" int psc_marder_static(psc_ctx *c, void *stream, float diffusion, int iters) {
+  if (!c || iters < 0 || !(diffusion >= 0.f)) return PSC_ERR_INVALID_ARG;
+  if (!c->have_particles || !c->have_fields || !c->ws || c->ws_cap != c->np) return PSC_ERR_NOT_BOUND;
+  if (c->state != PSC_STATE_STORE) return PSC_ERR_NOT_SORTED;
+  const GridDesc &gd = c->gd;
+  if ((int64_t)gd.comp > (int64_t)PSC_MARDER_STATIC_MAX_POINTS) return PSC_ERR_SCRATCH_LIMIT;
+  double lap = 0.0;  // the same bound on the diffusion number as psc_marder
+  for (int d = 0; d < 3; d++)
+    if (gd.n[d] > 1) lap += 4.0 / ((double)gd.dx[d] * (double)gd.dx[d]);
+  if ((double)diffusion * lap > 1.0 + 1e-6) return PSC_ERR_CFL;
+  float *scratch = nullptr;
+  int rc = marder_static_scratch(c, &scratch);
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  if ((rc = psc_store_relayout_if_spilled(c, s))) return rc;  // nobody may be waiting in the spill list
+
+  // The array still holds whatever the previous call (of any context on this device) left in it.
+  // rho is accumulated with atomics and must start from zero; f is overwritten point by point
+  // before it is read; the third component is only there because the ghost kernels work on three.
+  float *rho = scratch, *f = scratch + gd.comp;
+  PSC_CUDA_TRY(c, cudaMemsetAsync(scratch, 0, (size_t)3 * gd.comp * sizeof(float), s));
+  c->launches++;
+  const Cols &in = c->cols[c->cur];
+  const Exchange &xin = c->xch[c->xcur];
+  const int rblocks = (int)min((int64_t)c->sm_count * 16, max((int64_t)1, cdiv64(gd.nkeys, MT / 32)));
+  const bool d3 = psc_is3d(gd);
+  if (d3 && gd.order == 1) k_rho<true, 1><<<rblocks, MT, 0, s>>>(gd, in, c->base, c->cnt, xin, rho);
+  else if (d3) k_rho<true, 2><<<rblocks, MT, 0, s>>>(gd, in, c->base, c->cnt, xin, rho);
+  else if (gd.order == 1) k_rho<false, 1><<<rblocks, MT, 0, s>>>(gd, in, c->base, c->cnt, xin, rho);
+  else k_rho<false, 2><<<rblocks, MT, 0, s>>>(gd, in, c->base, c->cnt, xin, rho);
+  PSC_LAUNCH_CHECK(c);
+  if ((rc = psc_fields_fold(c, scratch, s))) return rc;
+  if ((rc = psc_fields_fill_ghosts(c, scratch, s))) return rc;
+  const int blocks = (int)cdiv64(gd.comp, MT);
+  for (int it = 0; it < iters; it++) {
+    k_gauss_residual<<<blocks, MT, 0, s>>>(gd, c->E, rho, f);
+    PSC_LAUNCH_CHECK(c);
+    k_marder_apply<<<blocks, MT, 0, s>>>(gd, c->E, f, diffusion);
     PSC_LAUNCH_CHECK(c);
   }
   return PSC_OK;
