@@ -324,6 +324,10 @@ def measure(cfg, scale, warmup, steps, dev, world, local):
            "steps": steps, "warmup": warmup, "particles": npart, "grid": list(pl.n), "order": pl.order,
            "phase_ms": phases, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
            "status_flags": flags, "store": info, "setup_s": round(t_gen, 1)}
+    mem = sim.memory()  # dense set (n entries) + store set (capacity entries) + workspace
+    res["memory"] = {"column_multiplier": round(mem["multiplier"], 3),
+                     "bytes_per_particle": round(mem["bytes_per_particle"], 1),
+                     "total_gb": round((mem["columns"] + mem["workspace"] + mem["fields"]) / 1e9, 2)}
     return res, sim, pl
 
 
@@ -445,7 +449,7 @@ def run_psc(args):
                    if npart * 32 > 4 * 126e6 else "inputs smaller than L2 (small config)",
                    "setup_s": res["setup_s"]},
         "clocks": res["clocks"], "gpu_launches": res["gpu_launches"], "status_flags": flags,
-        "phase_ms": res["phase_ms"], "roofline": res["roofline"], "store": res["store"],
+        "phase_ms": res["phase_ms"], "roofline": res["roofline"], "store": res["store"], "memory": res["memory"],
         "sort_general": sort_general, "e2e": e2e,
     }
 

@@ -30,8 +30,8 @@
  * particles into the INTERNAL form, the "cell store": positions become in-cell offsets in [0,1)
  * (units of cells), and the particles of cell k (key order of the sort) occupy the slots
  * [base[k], base[k] + count[k]) of the other column set, where base[k] is a multiple of 32 and
- * leaves every cell spare room -- which is why every column must be psc_particle_capacity(n)
- * entries long, not n.  A push updates particles that stay in their cell in place and hands the
+ * leaves every cell spare room -- which is why the columns of that set (the `secondary` set of
+ * psc_bind_particles) must be psc_particle_capacity(n) entries long, not n.  A push updates particles that stay in their cell in place and hands the
  * others over through per-cell exchange rows in the workspace (see psc_push_particles), so
  * between two pushes some particles live outside the columns.  psc_particles_gather returns a
  * dense copy of everything (offsets + cell keys, or absolute positions) without changing the
@@ -137,16 +137,20 @@ int psc_bind_fields(psc_ctx *ctx, float *E, float *B, float *J);
 /* Number of floats in one of E/B/J (3 * ex * ey * ez) and the extents; host only. */
 int64_t psc_field_elems(const psc_ctx *ctx, int32_t ext[3]);
 
-/* Entries every particle column must have for n particles: n + n/8 + 6 sqrt(cells * n) + 56 per
+/* Entries every column of the store set must have for n particles: n + n/8 + 6 sqrt(cells * n) + 56 per
  * cell, rounded up to a multiple of 32 -- every cell of the store gets spare room (an eighth of
  * its population, at least six Poisson standard deviations) and starts on a 128-byte boundary.
  * Host only. */
 int64_t psc_particle_capacity(const psc_ctx *ctx, int64_t n);
 
-/* `primary` holds the n particles (absolute positions, entries [0, n)); `secondary` is a second
- * buffer set of the same shapes the sort, the export and a re-layout write into.  Every column
- * of both sets has `capacity` >= psc_particle_capacity(n) entries (PSC_ERR_WORKSPACE) and is
- * 16-byte aligned (PSC_ERR_ALIGN).  Binding marks the particle list as unsorted. */
+/* The two column sets have fixed roles.  `primary` is the DENSE set: it holds the n particles the
+ * caller hands over (absolute positions, entries [0, n)), receives the n dense entries of
+ * psc_particles_export / psc_step_host, and serves as the n-entry scratch of a re-layout; the
+ * library never touches an entry beyond n, so its columns need only n entries.  `secondary` is
+ * the STORE set: the sort files the particles into it and the pushes update them there; each of
+ * its columns has `capacity` >= psc_particle_capacity(n) entries (PSC_ERR_WORKSPACE).  Device
+ * memory per particle is therefore (1 + capacity/n) column entries, not 2 * capacity/n.  All
+ * columns are 16-byte aligned (PSC_ERR_ALIGN).  Binding marks the particle list as unsorted. */
 int psc_bind_particles(psc_ctx *ctx, int64_t n, int64_t capacity, const psc_particle_cols *primary,
                        const psc_particle_cols *secondary);
 
@@ -154,7 +158,7 @@ int psc_bind_particles(psc_ctx *ctx, int64_t n, int64_t capacity, const psc_part
  * input index inside a key).  Afterwards the particles are in the internal form (the cell store
  * above) in sorted order: cell after cell, inside a cell in input order.  Arbitrary input order
  * is accepted.  From absolute columns the keys come from floor(fl32(x * (1/dx))) and the result
- * is written to the other column set (the two sets swap roles); from the internal form (sorted,
+ * is written to the store set; from the internal form (sorted,
  * or advanced by psc_push_particles) the input order is the dense order of psc_particles_gather
  * and the keys are the cells the particles are filed under.  psc_sort_result describes this
  * call's permutation.  Synchronises `stream` (it reads the layout statistics back).  psc_step

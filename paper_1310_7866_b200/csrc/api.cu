@@ -392,6 +392,7 @@ int psc_step_host(psc_ctx *c, void *stream, int64_t n, const psc_particle_cols *
   cudaStream_t s = (cudaStream_t)stream;
   const size_t fb = (size_t)3 * c->gd.comp * 4, pb = (size_t)n * 4;
   {
+    c->cur = 0;  // the dense set takes the host's particles; the sort below files them into the store set
     Cols &d = c->cols[c->cur];
     if ((d.id != nullptr) != (h->id != nullptr)) return PSC_ERR_INVALID_ARG;
     if ((d.x != nullptr) != (h->x != nullptr)) return PSC_ERR_INVALID_ARG;

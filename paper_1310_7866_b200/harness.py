@@ -4,12 +4,18 @@
 arithmetic of the method lives here."""
 from __future__ import annotations
 
+import weakref
+
 import torch
 
 from . import COLUMNS, PSC_B, PSC_E, PSC_GHOST, Psc
 
 
 class Simulation:
+    GUARD = 64               # sentinel entries behind the n entries of every dense column
+    SENTINEL = 0x7FC0DEAD    # (a NaN pattern as fp32)
+    live = weakref.WeakSet()  # the simulations alive in this process (tests check their guards)
+
     def __init__(self, plasma, block=(0, 0, 0), device="cuda:0", with_id=True, with_x=True, scheme=0):
         self.device = torch.device(device)
         self.plasma = plasma
@@ -33,7 +39,13 @@ class Simulation:
                     s[c] = None       # optional columns (include/psc.h): not carried
                     continue
                 dt = torch.int32 if c in ("species", "id") else torch.float32
-                s[c] = torch.empty(self.capacity, dtype=dt, device=dev)
+                # set 0 is the dense set (n entries, include/psc.h) followed by GUARD sentinel
+                # entries the library must never write; set 1 is the store set (capacity entries)
+                if k == 0:
+                    s[c] = torch.empty(self.np + self.GUARD, dtype=dt, device=dev)
+                    s[c][self.np:].view(torch.int32).fill_(self.SENTINEL)
+                else:
+                    s[c] = torch.empty(self.capacity, dtype=dt, device=dev)
             self.sets.append(s)
         for c in COLUMNS:
             if self.sets[0][c] is not None and self.np:
@@ -44,10 +56,27 @@ class Simulation:
         self.psc.bind_particles(self.np, self.capacity, self.sets[0], self.sets[1])
         self.psc.fill_ghosts(PSC_E)
         self.psc.fill_ghosts(PSC_B)
+        Simulation.live.add(self)
 
     def interior(self, F):
         g, n = self.g, self.n
         return F[:, g[2]:g[2] + n[2], g[1]:g[1] + n[1], g[0]:g[0] + n[0]]
+
+    def guards_intact(self):
+        """True while no entry behind the n entries of a dense-set column has been written"""
+        for t in self.sets[0].values():
+            if t is not None and not bool((t[self.np:].view(torch.int32) == self.SENTINEL).all()):
+                return False
+        return True
+
+    def memory(self):
+        """device bytes the library works in: particle columns of both sets (guards excluded),
+        workspace, fields; `multiplier` = column bytes / (n * bytes of one dense particle)"""
+        ncol = sum(1 for t in self.sets[0].values() if t is not None)
+        cols = 4 * ncol * (self.np + self.capacity)
+        return {"columns": cols, "workspace": self.ws.numel(), "fields": 3 * 4 * self.E.numel(),
+                "bytes_per_particle": (cols + self.ws.numel()) / max(self.np, 1),
+                "multiplier": cols / max(4 * ncol * self.np, 1)}
 
     def current(self):
         """the column set (dict of tensors, trimmed to n particles) that holds the particles now;

@@ -17,3 +17,15 @@ def _build_oracle():
     from oracle import psc_oracle
 
     psc_oracle.build()
+
+
+@pytest.fixture(autouse=True)
+def _dense_set_guards():
+    """include/psc.h: the dense (primary) column set needs only n entries.  The harness puts
+    sentinel entries behind them; after every test that built a Simulation they must be intact."""
+    yield
+    mod = sys.modules.get("paper_1310_7866_b200.harness")
+    if mod is None:
+        return
+    for sim in list(mod.Simulation.live):
+        assert sim.guards_intact(), "the library wrote behind the n entries of a dense column"

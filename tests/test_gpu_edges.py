@@ -128,3 +128,51 @@ def test_full_step_counts_keep_gauss_law(cfg, scale, steps):
     assert np.array_equal(ids0, ids1)
     # one fp32 rounding of J per step and node, accumulated: well below 1e-4 of the species density
     assert np.abs(r1 - r0).max() < 1e-4 * scale_rho, np.abs(r1 - r0).max() / scale_rho
+
+
+def test_column_sets_have_fixed_roles():
+    """include/psc.h (psc_bind_particles): the primary set is the dense one -- n entries, never
+    written beyond -- and the secondary set holds the store, whatever the sequence of calls: sort,
+    steps with re-layouts, export, a second sort, psc_step_host entered in the store form."""
+    pl = psc_inputs.thermal((1, 16, 16), 150, seed=23, name="dense")
+    vy = 0.33 * pl.dx[1] / pl.dt
+    pl.uy = pl.uy + float(vy / np.sqrt(1.0 - vy * vy))       # a third of the particles leave per step
+    pl.qw = pl.qw * 1e-2
+    extra, g = 900, torch.Generator().manual_seed(4)         # a clump that outgrows its cell's room
+    for k in ("x", "ux", "uz"):
+        setattr(pl, k, torch.cat([getattr(pl, k), torch.zeros(extra)]))
+    pl.y = torch.cat([pl.y, 5.0 + torch.rand(extra, generator=g)])
+    pl.z = torch.cat([pl.z, 9.0 + torch.rand(extra, generator=g)])
+    pl.uy = torch.cat([pl.uy, torch.full((extra,), float(pl.uy[0]))])
+    pl.qw = torch.cat([pl.qw, torch.full((extra,), float(pl.qw[0]))])
+    pl.species = torch.cat([pl.species, torch.zeros(extra, dtype=torch.int32)])
+    pl.id = torch.arange(pl.y.numel(), dtype=torch.int32)
+    sim = _sim(pl)
+    dense, store = sim.sets[0]["y"].data_ptr(), sim.sets[1]["y"].data_ptr()
+    assert sim.sets[0]["y"].numel() == sim.np + sim.GUARD < sim.capacity
+    cur = lambda: sim.psc.particles_current()["y"]
+    assert cur() == dense and sim.psc.particles_form() == 0
+    sim.psc.particles_sort()
+    assert cur() == store and sim.psc.particles_form() == 1
+    sim.step(4)
+    info = sim.psc.store_info()
+    assert info["relayouts"] >= 1 and cur() == store, info
+    sim.psc.particles_sort()                                 # a store sorted again stays where it is
+    assert cur() == store
+    sim.psc.particles_export()
+    assert cur() == dense and sim.psc.particles_form() == 0
+    sim.step(2)
+    assert cur() == store
+    # psc_step_host while the particles are in the store: the host's list goes to the dense set
+    host = {c: (None if t is None else t.cpu().pin_memory()) for c, t in sim.gather(absolute=True).items()
+            if c != "key"}
+    hE, hB = sim.E.cpu().pin_memory(), sim.B.cpu().pin_memory()
+    sim.psc.step_host(sim.np, host, hE, hB, None, 2)
+    assert cur() == dense and sim.psc.particles_form() == 0
+    assert np.array_equal(np.sort(host["id"].numpy()), np.arange(sim.np))
+    sim.step(1)
+    assert cur() == store
+    assert sim.psc.status() == 0
+    assert sim.guards_intact()
+    m = sim.memory()
+    assert m["multiplier"] == pytest.approx(1 + sim.capacity / sim.np)
