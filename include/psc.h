@@ -72,7 +72,8 @@ extern "C" {
 /* sticky device flags (psc_status) */
 #define PSC_F_OOB 1u      /* a particle position outside [0, n*dx) was seen by the sort (the particle
                              is filed under the nearest edge cell) */
-#define PSC_F_NAN 4u      /* a non-finite momentum was produced */
+#define PSC_F_NAN 4u      /* a non-finite momentum was produced; the particle is kept (in its cell, at its
+                             last finite offsets), but its current has poisoned J around it */
 #define PSC_F_SPECIES 8u  /* a species index outside [0, n_species) was seen by the sort (the
                              particle is treated as species 0) */
 #define PSC_F_OVERFLOW 32u /* a particle found no room although the columns / workspace have the

@@ -623,18 +623,24 @@ k_push1(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
       const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
       const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      // A non-finite end position (a non-finite momentum: PSC_F_NAN) fails every comparison
+      // above and would travel under the code of "no move", which no cell collects.  Such a
+      // particle keeps its old offsets and goes through the spill list back into its own cell,
+      // so that the population stays complete.
+      const bool nowhere = (sxd | syd | szd) == 0;
       Part pr;
       pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
       pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
       pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+      if (nowhere) { pr.ax = ax; pr.ay = ay; pr.az = az; }
       pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
       float w[8];
       Walker::to_words(w, pr, x2d);
       int dest = 0;
-      if (xi >= PSC_XCAP)
+      if (xi >= PSC_XCAP || nowhere)
         dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
                         wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-      wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+      wk.emit(sd, nowhere ? PSC_XCAP : xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
       const int e = qcnt + __popc(cm & lt);
       if (QCAP >= 32 || e < QCAP) {
         myQ[0 * QCAP + e] = __int_as_float(packed);

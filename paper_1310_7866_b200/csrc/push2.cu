@@ -322,24 +322,28 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
   };
   // a particle that leaves its cell: its record (offsets relative to the destination cell) goes
   // to the cell's exchange row
-  auto depart = [&](bool leave, int xi, int lx, int ly, int lz, float endx, float endy, float endz,
-                    float ux, float uy, float uz, float qw, int sp, float x2d, int id) {
+  auto depart = [&](bool leave, int xi, int lx, int ly, int lz, float ax, float ay, float az, float endx,
+                    float endy, float endz, float ux, float uy, float uz, float qw, int sp, float x2d, int id) {
     if (leave) {
       const int sxd = D3 ? (endx >= 1.f ? 1 : (endx < 0.f ? -1 : 0)) : 0;
       const int syd = endy >= 1.f ? 1 : (endy < 0.f ? -1 : 0);
       const int szd = endz >= 1.f ? 1 : (endz < 0.f ? -1 : 0);
+      // a non-finite end position (PSC_F_NAN) compares false everywhere: the particle keeps its old
+      // offsets and returns to its own cell through the spill list instead of being dropped
+      const bool nowhere = (sxd | syd | szd) == 0;
       Part pr;
       pr.ax = D3 ? fminf(fmaxf(endx - (float)sxd, 0.f), 0.99999994f) : 0.f;
       pr.ay = fminf(fmaxf(endy - (float)syd, 0.f), 0.99999994f);
       pr.az = fminf(fmaxf(endz - (float)szd, 0.f), 0.99999994f);
+      if (nowhere) { pr.ax = D3 ? ax : 0.f; pr.ay = ay; pr.az = az; }
       pr.ux = ux; pr.uy = uy; pr.uz = uz; pr.qw = qw; pr.sp = sp;
       float w[8];
       Walker::to_words(w, pr, x2d);
       int dest = 0;
-      if (xi >= PSC_XCAP)
+      if (xi >= PSC_XCAP || nowhere)
         dest = cell_key(gd, D3 ? wrap_cell(tg.o[0] + lx + sxd, gd.n[0]) : 0,
                         wrap_cell(tg.o[1] + ly + syd, gd.n[1]), wrap_cell(tg.o[2] + lz + szd, gd.n[2]));
-      wk.emit(sd, xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
+      wk.emit(sd, nowhere ? PSC_XCAP : xi, dir_code<D3>(sxd, syd, szd), w, id, dest);
     }
   };
 
@@ -536,7 +540,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
       if (BIG) {
         if (__any_sync(0xffffffffu, leave)) {
           const int xi = wk.leaver_slot(leave);
-          depart(leave, xi, lx, ly, lz, endx, endy, endz, ux, uy, uz, qw, sp, x2d, id);
+          depart(leave, xi, lx, ly, lz, ax, ay, az, endx, endy, endz, ux, uy, uz, qw, sp, x2d, id);
         }
         wk.store_global(sd, act && stay, pn, x2d, id);
       } else {
@@ -566,7 +570,7 @@ k_push2(GridDesc gd, StoreDesc sd, const float *__restrict__ E, const float *__r
         if (al) wk.leaver(sd, i0 + lane, q, qx2d, qid);
         float qvx, qex, qey, qez;
         move(D3 ? q.ax : 0.25f, q.ay, q.az, q.ux, q.uy, q.uz, qvx, qex, qey, qez);
-        depart(al, i0 + lane, lx, ly, lz, qex, qey, qez, q.ux, q.uy, q.uz, q.qw,
+        depart(al, i0 + lane, lx, ly, lz, q.ax, q.ay, q.az, qex, qey, qez, q.ux, q.uy, q.uz, q.qw,
                q.sp & (PSC_MAX_SPECIES - 1), qx2d, qid);
       }
       wk.end_image(sd, next_n, next_base);

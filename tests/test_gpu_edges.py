@@ -176,3 +176,42 @@ def test_column_sets_have_fixed_roles():
     assert sim.guards_intact()
     m = sim.memory()
     assert m["multiplier"] == pytest.approx(1 + sim.capacity / sim.np)
+
+
+@pytest.mark.parametrize("kind", ["2d", "3d", "2d-o2", "beam"])
+def test_a_non_finite_momentum_is_flagged_and_the_particle_is_kept(kind):
+    """one particle with u = NaN, one with u = +inf: PSC_F_NAN is raised, and both stay in the
+    population (in their cells, old offsets) instead of leaving under the code of "no move" that no
+    cell collects; every other particle still moves"""
+    if kind == "2d":
+        pl = psc_inputs.make_config(1)
+    elif kind == "3d":
+        pl = psc_inputs.thermal((12, 20, 8), 5, seed=12, dx=(0.8, 1.25, 0.5), name="3d")
+    elif kind == "2d-o2":
+        pl = psc_inputs.thermal((1, 24, 40), 9, seed=14, order=2, dx=(1.0, 0.5, 2.0), name="o2")
+    else:
+        pl = psc_inputs.make_config(5, scale=(8, 8, 32))
+    n = pl.n_particles
+    bad = [n // 3, 2 * n // 3]
+    pl.ux[bad[0]] = float("nan")
+    pl.uz[bad[1]] = float("inf")
+    sim = _sim(pl)
+    sim.psc.particles_sort()
+    before = sim.gather()
+    # the NaN current spreads by a stencil width per step; the steps taken here keep the number of
+    # affected particles below the spill list's n/4 entries (8^2 x 32 cells at order 2: one step)
+    for it in range(1 if kind == "beam" else 2):
+        sim.step(1)
+        flags = sim.psc.status()
+        assert flags & psc.PSC_F_NAN and not flags & psc.PSC_F_OVERFLOW
+        g = sim.gather()
+        ids = g["id"].cpu().numpy()
+        assert np.array_equal(np.sort(ids), np.arange(n)), (kind, it)      # nobody lost or duplicated
+    pos = {int(i): k for k, i in enumerate(before["id"].cpu().numpy())}
+    now = {int(i): k for k, i in enumerate(ids)}
+    for b in bad:                                                          # same cell, same offsets
+        assert int(g["key"][now[b]]) == int(before["key"][pos[b]])
+        for c in ("y", "z"):
+            assert float(g[c][now[b]]) == float(before[c][pos[b]])
+    info = sim.psc.store_info()
+    assert info["spilled"] >= 2 or info["inserted"] + info["relayouts"] > 0    # they travel through the spill list
