@@ -250,7 +250,10 @@ int psc_patch_loads(psc_ctx *ctx, void *stream, const int32_t patch_blocks[3], i
  * order[i] (HOST array, np[0]*np[1]*np[2] entries) = row-major index (pz*np[1]+py)*np[0]+px of
  * the i-th patch on the curve.  np[d] == 1 drops that direction (a 2-d curve for a 2-d grid).
  * Extents that are not equal powers of two: the grid is embedded in the enclosing power-of-two
- * cube and the curve's points outside the grid are skipped.  Host only, no device needed. */
+ * cube and the curve's points outside the grid are skipped -- consecutive patches are then no
+ * longer always face neighbours (the curve re-enters the grid elsewhere), and the walk costs one
+ * visit per point of the cube: a grid whose cube has more than 2^32 points (e.g. 2 x 2 x 65536) is
+ * refused with PSC_ERR_UNSUPPORTED.  Host only, no device needed. */
 int psc_hilbert_order(const int32_t np[3], int32_t *order);
 
 /* Appendix A: loads[p] (HOST, double, p in CURVE order, n_patches entries, all >= 0),

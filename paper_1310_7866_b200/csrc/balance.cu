@@ -136,6 +136,9 @@ extern "C" int psc_hilbert_order(const int32_t np[3], int32_t *order) {
   }
   int b = 0;
   while ((1 << b) < mx) b++;
+  // the walk below visits every point of the enclosing cube: a very anisotropic grid such as
+  // 2 x 2 x 65536 would need 2^48 of them (and 1 << 64 is undefined): refused
+  if (b * n > 32) return PSC_ERR_UNSUPPORTED;
   const uint64_t total = (uint64_t)1 << (b * n);
   int64_t out = 0;
   for (uint64_t h = 0; h < total; h++) {

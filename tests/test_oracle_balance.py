@@ -250,3 +250,26 @@ def test_library_argument_errors():
         psc.balance([1.0, 1.0], [1.0, 0.0])
     with pytest.raises(psc.PscError):
         psc.hilbert_order((0, 1, 1))
+
+
+def test_library_curve_refuses_a_cube_it_cannot_walk():
+    """psc_hilbert_order visits every point of the enclosing power-of-two cube: 2 x 2 x 65536 would
+    be 2^48 visits (PSC_ERR_UNSUPPORTED, at once); the widest cube it accepts still works and is a
+    bijection; on a grid of unequal extents the curve re-enters the grid, as include/psc.h says"""
+    import ctypes as C
+    import time
+    L = psc.lib()
+    out = (C.c_int32 * 4)()
+    t = time.perf_counter()
+    assert L.psc_hilbert_order((C.c_int32 * 3)(2, 2, 65536), out) == -7
+    assert L.psc_hilbert_order((C.c_int32 * 3)(1, 2, 1 << 20), out) == -7      # 2-d: 2 x 20 bits
+    assert time.perf_counter() - t < 1.0
+    order = psc.hilbert_order((1, 4, 2048))                                    # 2 x 11 bits: 4 M visits
+    assert sorted(order) == list(range(4 * 2048))
+    jumps = 0
+    for a, b in zip(order, order[1:]):
+        dy, dz = abs(a % 4 - b % 4), abs(a // 4 - b // 4)
+        jumps += (dy + dz) != 1
+    assert jumps > 0                       # not a face-neighbour walk on such a grid
+    sq = psc.hilbert_order((1, 16, 16))    # equal powers of two: every step is to a face neighbour
+    assert all(abs(a % 16 - b % 16) + abs(a // 16 - b // 16) == 1 for a, b in zip(sq, sq[1:]))
