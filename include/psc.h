@@ -12,8 +12,17 @@
  *     stream) and the library borrows the pointers until the next bind or psc_destroy.  The only
  *     device memory the context owns is a 64-byte status/counter block (and, once psc_marder or
  *     psc_charge_density has been called, one scratch field of the size of E).
- *   - Every call that does device work enqueues it on `stream` (a cudaStream_t passed as void*)
- *     and returns without synchronising, except psc_status and psc_step_host.
+ *   - Every call that does device work enqueues it on `stream` (a cudaStream_t passed as void*).
+ *     The steady-state calls -- psc_step, psc_push_particles, psc_push_fields, psc_exchange_j,
+ *     psc_fill_ghosts, psc_marder_static, psc_patch_loads, psc_particles_gather / _export -- return
+ *     without synchronising.  These SYNCHRONISE the stream because they read the device's status
+ *     block back: psc_particles_sort (and therefore the first psc_step after a bind, an export or
+ *     a psc_step_host, which sorts), psc_status, psc_store_info, psc_profile, psc_step_host.
+ *     psc_marder and psc_charge_density cudaMalloc their scratch field on their first call, which
+ *     synchronises the whole device once (psc_marder_static never does).
+ *   - psc_step / psc_push_particles start with a one-thread gate kernel that may launch the store's
+ *     re-layout from the device (tail launches); a stream capture of these calls into a CUDA graph
+ *     is therefore not supported by this library version.
  *   - Every call returns 0 (PSC_OK) or a negative PSC_ERR_* code; nothing aborts or throws across
  *     the ABI.  Data-dependent faults are sticky device flags read with psc_status.
  *   - There is no CPU fallback anywhere: without a CUDA device every compute call fails with

@@ -54,7 +54,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(bdir, exist_ok=True)
     inc = ["-I", INCLUDE, "-I", CSRC]
     vflags = ["-Xptxas", "-v"] if verbose else []
-    vflags += os.environ.get("PSC_NVCC_FLAGS", "").split()  # e.g. -DNAME for a kernel experiment
 
     def compile_one(f):
         obj = os.path.join(bdir, f.replace(".cu", ".o"))

@@ -93,6 +93,8 @@ struct StoreDesc {
   uint32_t *nbig;    // tiles flagged by this step's image launch (the BIG launch returns at once if 0)
   uint32_t *nbig_next;  // the other step parity's counter: zeroed by this step's BIG launch
   uint32_t *flags;
+  uint32_t *maxcnt;  // device word PSC_DW_MAXCNT: largest cell count (layouts, and cells that grew since)
+  int maxcnt_known;  // its value when the host last read the status block: only a larger cell reports
 };
 
 // Where the particle list is in the sort / push cycle:
@@ -125,7 +127,7 @@ enum {
   PSC_DW_FLAGS = 0,    // sticky flags (psc_status)
   PSC_DW_BIG = 1,      // big-segment counter of the general sort
   PSC_DW_SPILL = 2,    // spill counter: != 0 => the next step re-lays the store out
-  PSC_DW_MAXCNT = 3,   // largest cell count seen by the last layout
+  PSC_DW_MAXCNT = 3,   // largest cell count: of the last layout, raised by cells that grew since
   PSC_DW_SLOTS = 4,    // slots used by the last layout
   PSC_DW_RELAYOUTS = 5,  // number of re-layouts performed
   PSC_DW_NBIG = 6,     // [2]: tiles with a cell left to the BIG launch, by step parity
@@ -147,6 +149,7 @@ struct psc_ctx {
   Prof prof;
   float q[PSC_MAX_SPECIES], m[PSC_MAX_SPECIES];
   float *E, *B, *J;
+  int maxcnt_known;  // PSC_DW_MAXCNT as last read back (psc_refresh_image_size)
   float *rho;      // owned: node charge density of psc_marder ([ext2][ext1][ext0]), lazily allocated
   Cols cols[2];
   int cur;

@@ -723,6 +723,8 @@ StoreDesc psc_store_desc(const psc_ctx *c) {
   sd.nbig = c->d_flags + PSC_DW_NBIG + c->xcur;
   sd.nbig_next = c->d_flags + PSC_DW_NBIG + (c->xcur ^ 1);
   sd.flags = c->d_flags + PSC_DW_FLAGS;
+  sd.maxcnt = c->d_flags + PSC_DW_MAXCNT;
+  sd.maxcnt_known = c->maxcnt_known;
   return sd;
 }
 
@@ -853,6 +855,7 @@ int psc_store_gather(psc_ctx *c, const Cols &dst, int32_t *key, bool to_abs, cud
 // raises the largest count, and the image follows at the next such call (it never shrinks).
 void psc_refresh_image_size(psc_ctx *c, const uint32_t *dw) {
   const int mx = (int)dw[PSC_DW_MAXCNT];
+  c->maxcnt_known = mx;
   int C = (mx + mx / 8 + 24 + 31) / 32 * 32;  // 64, 96, ..., 256
   C = C < 64 ? 64 : (C > 256 ? 256 : C);
   // the order-2 kernel is bound by registers (2 blocks/SM), not by shared memory: it takes the largest
@@ -929,7 +932,7 @@ struct RelayoutArgs {
   uint32_t *dw;
   int *np_dev;
   long long capacity;
-  int g_cells, g_cells8, g_warpcells, g_part, g_spill, g_reset, sblocks;
+  int g_cells, g_warpcells, g_part, g_spill, g_reset, sblocks;
 };
 
 template <bool D3>
@@ -999,6 +1002,7 @@ __global__ void __launch_bounds__(256) k_spill_insert(RelayoutArgs a) {
         a.cur.qw[o] = D3 ? w[6] : w[5];
         a.cur.sp[o] = __float_as_int(D3 ? w[7] : w[6]);
         if (a.cur.id) a.cur.id[o] = id;
+        atomicMax(&a.dw[PSC_DW_MAXCNT], (uint32_t)(slot + 1));
       } else {
         atomicSub(&a.cnt[key], 1);
         fail = true;
@@ -1068,7 +1072,6 @@ int psc_store_relayout_if_spilled(psc_ctx *c, cudaStream_t s) {
   a.g_part = grid_for(c, c->np, SORT_THREADS);
   a.g_spill = grid_for(c, c->spill.cap, SORT_THREADS);
   a.g_reset = grid_for(c, (int64_t)nk * 16, SORT_THREADS);
-  a.g_cells8 = 0;
   a.sblocks = (int)cdiv64(nk, SCAN_TILE);
   k_relayout_gate<<<1, 32, 0, s>>>(a);
   PSC_LAUNCH_CHECK(c);

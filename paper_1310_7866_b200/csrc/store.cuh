@@ -66,10 +66,6 @@ __device__ __forceinline__ void bulk_s2g(void *gdst, const void *ssrc, unsigned 
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
                ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
 }
-// asks the L2 for a run of global memory (no destination: a later bulk copy finds it there)
-__device__ __forceinline__ void bulk_prefetch_l2(const void *gsrc, unsigned bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
-}
 // TMA tensor copies (4-d tiled tensor map): global box at coordinates (c0, c1, c2, c3) -> shared
 // (128-byte aligned), completion on `bar`; shared -> global with element-wise add
 __device__ __forceinline__ void tma_load_4d(void *sdst, const void *map, int c0, int c1, int c2, int c3,
@@ -238,23 +234,6 @@ struct CellWalker {
       } else {
 #pragma unroll
         for (int c = 0; c < NREC; c++) bulk_g2s(buf + c * C, sd.col[c] + base_, bytes, bar);
-      }
-    }
-  }
-
-  // lane 0: ask the L2 for the resident run of the cell AFTER the current one, so that the bulk
-  // copies issued at the end of the current cell find it there (DRAM latency off the warp's path)
-  __device__ __forceinline__ void prefetch_l2(const StoreDesc &sd, int n_, int base_) {
-    if (BIG) return;
-    n_ = __shfl_sync(0xffffffffu, n_, 0);
-    base_ = __shfl_sync(0xffffffffu, base_, 0);
-    if (n_ > 0 && n_ <= C && lane == 0) {
-      const unsigned bytes = (unsigned)((n_ + 3) & ~3) * 4u;
-      if (XC) {
-        for (int c = 0; c < ncol; c++) bulk_prefetch_l2(sd.col[c] + base_, bytes);
-      } else {
-#pragma unroll
-        for (int c = 0; c < NREC; c++) bulk_prefetch_l2(sd.col[c] + base_, bytes);
       }
     }
   }
@@ -508,7 +487,12 @@ struct CellWalker {
   }
 
   __device__ __forceinline__ void publish(const StoreDesc &sd, int newcnt) {
-    if (lane == 0) sd.cnt[key] = newcnt;
+    if (lane == 0) {
+      sd.cnt[key] = newcnt;
+      // a cell that has outgrown every cell the host knows of reports its size: the per-warp image
+      // of the kernels follows the largest cell at the host's next look at the status block
+      if (newcnt > sd.maxcnt_known) atomicMax(sd.maxcnt, (uint32_t)newcnt);
+    }
     if (lane < XW) sd.xout.mask[(size_t)key * XW + lane] = xrow[lane];
     __syncwarp();
     if (lane < XW) xrow[lane] = 0u;

@@ -215,3 +215,27 @@ def test_a_non_finite_momentum_is_flagged_and_the_particle_is_kept(kind):
             assert float(g[c][now[b]]) == float(before[c][pos[b]])
     info = sim.psc.store_info()
     assert info["spilled"] >= 2 or info["inserted"] + info["relayouts"] > 0    # they travel through the spill list
+
+
+def test_image_size_follows_cells_that_grow_between_layouts():
+    """a column of cells whose particles all walk through the next column: the cell counts there
+    nearly double without any re-layout (the spare room suffices); the status block's largest count and, from the
+    host's next look at it, the per-warp image of the kernels follow"""
+    pl = psc_inputs.thermal((1, 16, 16), 20, vth_e=1e-4, vth_i=1e-4, seed=3, name="walk")
+    pl.qw = pl.qw * 1e-6                                    # (no fields to speak of)
+    v = 0.9
+    walkers = (pl.y >= 4.0) & (pl.y < 5.0)
+    pl.uy = torch.where(walkers, torch.full_like(pl.uy, v / np.sqrt(1.0 - v * v)), pl.uy)
+    sim = _sim(pl)
+    sim.psc.particles_sort()
+    i0 = sim.psc.store_info()
+    assert i0["max_count"] == 40 and i0["image_slots"] == 96
+    sim.step(3)                     # 0.45 cell per step: most walkers are in the next column, none beyond
+    assert sim.psc.status() == 0
+    i1 = sim.psc.store_info()
+    assert i1["relayouts"] == 0 and 65 <= i1["max_count"] <= 80, i1
+    assert i1["image_slots"] == 128                         # e.g. 74 + 74/8 + 24 -> 128
+    sim.step(3)
+    g = sim.gather()
+    assert np.array_equal(np.sort(g["id"].cpu().numpy()), np.arange(sim.np))
+    assert sim.psc.status() == 0

@@ -171,8 +171,9 @@ def test_full_size_step_counts(cfg):
     r1, _, c1 = residual()
     assert c1 == counts0                                   # nobody lost, nobody duplicated
     assert np.abs(r1 - r0).max() < 1e-4 * scale_rho, np.abs(r1 - r0).max() / scale_rho
+    sim.step(1)                    # what the last push spilled is filed or re-laid out by the next step's gate
     info = sim.psc.store_info()
-    assert info["spilled"] == 0 or info["relayouts"] > 0
+    assert info["spilled"] == 0 or info["relayouts"] + info["inserted"] > 0, info
 
 
 def test_config3_full_size_ten_steps_match_oracle_by_id():
