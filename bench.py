@@ -21,7 +21,8 @@ The JSON line carries
                the kernel launch (psc_profile brackets, on the launching stream, inside the timed
                region) against MEASURED_PEAKS.json's copy bandwidth
   other_configs  BASELINE.json's other four configs at full size, a short run each (3 warm-up +
-               10 timed steps): value, ms_per_step, phase_ms, roofline, clocks
+               10 timed steps), one compact object per config: value, ms_per_step, kernel_ms, frac
+               (of the measured HBM peak), frac_nominal (of 8000 GB/s), traffic_ratio, clocks
   sort_general one explicit psc_particles_sort of the workload in random order (outside the
                steady-state loop: psc_step never sorts after its first step)
   cpu_baseline the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded
@@ -54,6 +55,8 @@ WORKLOADS = {
 }
 # algorithmic bytes per particle of the fused kernel
 PUSH_BYTES = {2: 48, 3: 56}
+NOMINAL_HBM_GBS = 8000.0     # B200 data sheet (BASELINE.md section 2 quotes fractions against both)
+MIN_CLOCK_SAMPLES = 8
 
 
 def peaks():
@@ -296,10 +299,24 @@ def measure(cfg, scale, warmup, steps, dev, world, local):
         psc.step()
     ev1.record()
     barrier()
-    clocks = sampler.stop()
     ms = ev0.elapsed_time(ev1)
     launches = psc.launch_count() - l0
     prof = psc.profile()
+    # a short timed region (the driver's 20 steps are 50 ms) yields one or two NVML samples: the same
+    # steps keep running, untimed, until there are MIN_CLOCK_SAMPLES of them (at most 2 s)
+    in_region = len(sampler.sm)
+    t_extra = time.perf_counter()
+    while sampler.nvml is not None and len(sampler.sm) < MIN_CLOCK_SAMPLES and time.perf_counter() - t_extra < 2.0:
+        for _ in range(10):
+            psc.step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    clocks["samples_in_timed_region"] = in_region
+    if clocks.get("samples", 0) < MIN_CLOCK_SAMPLES:
+        clocks["note"] = "fewer than %d clock samples" % MIN_CLOCK_SAMPLES
+    elif in_region < MIN_CLOCK_SAMPLES:
+        clocks["note"] = "timed region too short for %d samples: the rest taken while the same steps kept running" % MIN_CLOCK_SAMPLES
+    psc.profile()          # (the extra steps' brackets are dropped)
     flags = psc.status()
     info = psc.store_info()
     ms_max = max_over_ranks(ms, world, dev)
@@ -312,13 +329,16 @@ def measure(cfg, scale, warmup, steps, dev, world, local):
     achieved = bytes_pp * npart / (push_avg * 1e-3) / 1e9 if push_n else 0.0
     kernel = "k_push%d" % pl.order
     roofline = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak,
-                "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "unit": "GB/s", "frac": achieved / peak, "frac_nominal": achieved / NOMINAL_HBM_GBS,
+                "traffic": None,
                 "bytes_per_particle": bytes_pp, "kernel_ms": push_avg, "peak_source": peak_src,
                 "share_of_step": push_ms / ms if ms else None}
     if scale is None:
         roofline["traffic"], com = traffic_of(cfg, kernel)
         if com:
             roofline["traffic_commit"] = com
+        if roofline["traffic"]:
+            roofline["traffic_ratio"] = roofline["traffic"] / (bytes_pp * npart)
     phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
     res = {"value": job_throughput(npart, world, steps, ms_max), "ms_per_step": ms_max / steps,
            "steps": steps, "warmup": warmup, "particles": npart, "grid": list(pl.n), "order": pl.order,
@@ -462,9 +482,13 @@ def run_psc(args):
             if cfg == args.config:
                 continue
             r, s2, p2 = measure(cfg, None, 3, args.other_steps, dev, 1, local)
-            r["workload"] = WORKLOADS[cfg]
-            r["unit"] = UNIT
-            others.append(r)
+            rf = r["roofline"]
+            others.append({"config": cfg, "value": float("%.4g" % r["value"]), "ms_per_step": round(r["ms_per_step"], 4),
+                           "steps": r["steps"], "kernel": rf["kernel"], "kernel_ms": round(rf["kernel_ms"], 4),
+                           "frac": round(rf["frac"], 4), "frac_nominal": round(rf["frac_nominal"], 4),
+                           "traffic_ratio": None if not rf.get("traffic_ratio") else round(rf["traffic_ratio"], 3),
+                           "sm_mhz": r["clocks"].get("sm_mhz"), "reasons": r["clocks"].get("reasons"),
+                           "flags": r["status_flags"], "mem_x": r["memory"]["column_multiplier"]})
             flags |= r["status_flags"]
             del s2, p2
             torch.cuda.empty_cache()
@@ -478,11 +502,14 @@ def run_psc(args):
             est = {1: 4.5e7, 2: 4.5e7, 3: 2.9e7, 4: 2.9e7, 5: 5e6}[args.config]
             nsample = grid[0] * grid[1] * grid[2] * ppc_of(args.config)
             args.cpu_steps = max(2, min(200, int(10.0 * est / nsample)))
-        rate, threads, nsamp, _ = oracle_rate(args.config, grid, args.cpu_steps)
+        # two runs of about 10 s each, the faster one reported (the first run of a process pays for page
+        # faults and thread start-up: round 2 saw 3.8e7 and 5.2e7 from the same oracle on the same box)
+        runs = [oracle_rate(args.config, grid, args.cpu_steps)[:3] for _ in range(2)]
+        rate, threads, nsamp = max(runs, key=lambda r: r[0])
         out["cpu_baseline"] = {
             "value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "grid %dx%dx%d of the same recipe (%d particles), %d steps"
-                      % (grid + (nsamp, args.cpu_steps))}
+            "sample": "grid %dx%dx%d of the same recipe (%d particles), %d steps, best of 2 runs (%.3g, %.3g)"
+                      % (grid + (nsamp, args.cpu_steps, runs[0][0], runs[1][0]))}
         # the same oracle on ONE core, a smaller sample (about 5 s)
         from oracle.psc_oracle import Oracle
         g1 = sample_grids(args.config)[min(1, len(sample_grids(args.config)) - 1)]

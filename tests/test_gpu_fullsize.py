@@ -180,8 +180,10 @@ def test_config3_full_size_ten_steps_match_oracle_by_id():
     """config 3 at BASELINE size (1x512x1024, 14.6 M particles, the 11x density contrast of the
     double Harris sheet) in a closed loop: ten psc_step against ten oracle steps of the WHOLE
     system, every particle matched by id (positions within 1e-5 of the domain and 1e-4 cell,
-    momenta within 1e-5 of the species rms), J and E within 1e-5 of the component max-norm, B
-    within 1e-5 of the field's max-norm."""
+    momenta within 1e-5 of the species rms), J within 1e-5 of each component's max-norm, E and B
+    within 1e-5 of the FIELD's max-norm and within 1e-4 of each component's (the split DESIGN.md
+    section 4 derives: E_x and B_x, B_z are a thousand times smaller than B_y here).  The measured
+    ratios are printed by the assertions."""
     from paper_1310_7866_b200.harness import Simulation
     from tests.util import (gpu_state, oracle_state, periodic_dist, positions_f64, rel_fieldnorm,
                             rel_maxnorm)
@@ -213,7 +215,9 @@ def test_config3_full_size_ten_steps_match_oracle_by_id():
     # E and B: 1e-5 of the FIELD's max-norm (north_star), 1e-4 per component: E_x (max 1e-3) is
     # advanced by differences of B_y (0.063), whose fp32 ulp (3.7e-9) times dt times ten steps is
     # 3e-8 = 3e-5 of E_x but 8e-6 of the field; likewise B_x, B_z (1e-3) next to B_y
-    assert rel_fieldnorm(sim.interior(sim.E).cpu().numpy(), E) < TOL
-    assert rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E) < 10 * TOL
-    assert rel_fieldnorm(sim.interior(sim.B).cpu().numpy(), B) < TOL
-    assert rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B) < 10 * TOL
+    rE = (rel_fieldnorm(sim.interior(sim.E).cpu().numpy(), E), rel_maxnorm(sim.interior(sim.E).cpu().numpy(), E))
+    rB = (rel_fieldnorm(sim.interior(sim.B).cpu().numpy(), B), rel_maxnorm(sim.interior(sim.B).cpu().numpy(), B))
+    msg = "E: %.2e of the field norm, %.2e of the worst component; B: %.2e, %.2e (limits 1e-5, 1e-4)" % (rE + rB)
+    print(msg)
+    assert rE[0] < TOL and rE[1] < 10 * TOL, msg
+    assert rB[0] < TOL and rB[1] < 10 * TOL, msg

@@ -555,3 +555,39 @@ def test_alternating_order_improves_energy_conservation():
         orc.step(E, B, J, *cols, sp, 400)
         drift.append(abs(orc.energy(E, B, cols[3], cols[4], cols[5], cols[6], sp).sum() / e0 - 1))
     assert drift[1] < 0.2 * drift[0], drift
+
+
+@pytest.mark.parametrize("order,n", [(1, (1, 12, 10)), (2, (6, 5, 7))])
+def test_fig7_ordering_is_fig8_shifted_by_half_a_step(order, n):
+    """the original time step (Fig. 7: E half, B half, particle loop, B half,
+    J exchange, E half) and the optimised one (Fig. 8) are the same scheme; Fig. 7 merely splits the
+    E update around the integer time level.  Entering Fig. 7 after its first E half step (that is,
+    with E^{1/2}) and leaving N cycles later with one more E half step lands on Fig. 8's state after
+    N steps: the two half steps E += dt/2 (curl B - j) with the same B^{n+1}, j^{n+1} add up to the
+    one full step."""
+    dx = (1.0, 0.9, 1.2)
+    dt = 0.45 / np.sqrt(sum(1 / dx[d] ** 2 for d in range(3) if n[d] > 1))
+    q, m = [-1.0, 1.0], [1.0, 4.0]
+    rng = np.random.default_rng(7 + order)
+    orc = Oracle(n, dx, dt, order, q, m)
+    pos, u, qw, species = _small_plasma(rng, n, dx, 40, 0.6)
+    E = 0.3 * rng.standard_normal(orc.fshape)
+    B = 0.3 * rng.standard_normal(orc.fshape)
+    J = orc.zeros_field()
+    E7, B7, J7 = E.copy(), B.copy(), J.copy()
+    pos7, u7 = [a.copy() for a in pos], [a.copy() for a in u]
+    N = 5
+    orc.step(E, B, J, *pos, *u, qw, species, N)                       # Fig. 8
+    for k in range(N):                                                # Fig. 7
+        if k > 0:
+            orc.push_e(E7, B7, J7, 0.5)                               # E^n -> E^{n+1/2}
+        orc.push_b(E7, B7, 0.5)
+        orc.push_particles(E7, B7, J7, *pos7, *u7, qw, species)
+        orc.push_b(E7, B7, 0.5)
+        orc.push_e(E7, B7, J7, 0.5)                                   # E^{n+1/2} -> E^{n+1}
+    Eint = E7.copy()                                                  # E at the integer level t^N
+    orc.push_e(E7, B7, J7, 0.5)
+    assert np.abs(E7 - E).max() < 1e-13 and np.abs(B7 - B).max() < 1e-13 and np.abs(J7 - J).max() < 1e-13
+    for a, b in zip(pos + u, pos7 + u7):
+        assert np.abs(a - b).max() < 1e-12
+    assert np.abs(Eint - E).max() > 1e-4                              # (the half step is not a no-op)
