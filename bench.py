@@ -55,6 +55,10 @@ WORKLOADS = {
 }
 # algorithmic bytes per particle of the fused kernel
 PUSH_BYTES = {2: 48, 3: 56}
+# the method's own fp32 operations per particle, counted from the scheme (DESIGN.md section 6,
+# "roofline_alu"): keyed by (order, dimensions)
+METHOD_FLOPS = {(1, 2): 180, (1, 3): 280, (2, 2): 470, (2, 3): 1570}
+FP32_LANES = 148 * 128       # B200: 148 SMs x 128 fp32 lanes, one FMA (2 flops) per lane and clock
 NOMINAL_HBM_GBS = 8000.0     # B200 data sheet (BASELINE.md section 2 quotes fractions against both)
 MIN_CLOCK_SAMPLES = 8
 
@@ -339,10 +343,17 @@ def measure(cfg, scale, warmup, steps, dev, world, local):
             roofline["traffic_commit"] = com
         if roofline["traffic"]:
             roofline["traffic_ratio"] = roofline["traffic"] / (bytes_pp * npart)
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    fpp = METHOD_FLOPS[(pl.order, ndim)]
+    alu_peak = FP32_LANES * 2 * sm_max * 1e6 / 1e12
+    alu_ach = fpp * npart / (push_avg * 1e-3) / 1e12 if push_n else 0.0
+    roofline_alu = {"bound": "alu", "kernel": kernel, "flops_per_particle": fpp, "achieved": alu_ach,
+                    "peak": alu_peak, "unit": "TFLOP/s", "frac": alu_ach / alu_peak,
+                    "peak_source": "148 SMs x 128 lanes x 2 x sm_max_mhz; flops counted from the scheme (DESIGN.md section 6)"}
     phases = {k: round(v[0] / max(v[1], 1), 4) for k, v in prof.items() if v[1]}
     res = {"value": job_throughput(npart, world, steps, ms_max), "ms_per_step": ms_max / steps,
            "steps": steps, "warmup": warmup, "particles": npart, "grid": list(pl.n), "order": pl.order,
-           "phase_ms": phases, "roofline": roofline, "clocks": clocks, "gpu_launches": launches,
+           "phase_ms": phases, "roofline": roofline, "roofline_alu": roofline_alu, "clocks": clocks, "gpu_launches": launches,
            "status_flags": flags, "store": info, "setup_s": round(t_gen, 1)}
     mem = sim.memory()  # dense set (n entries) + store set (capacity entries) + workspace
     res["memory"] = {"column_multiplier": round(mem["multiplier"], 3),
@@ -469,7 +480,8 @@ def run_psc(args):
                    if npart * 32 > 4 * 126e6 else "inputs smaller than L2 (small config)",
                    "setup_s": res["setup_s"]},
         "clocks": res["clocks"], "gpu_launches": res["gpu_launches"], "status_flags": flags,
-        "phase_ms": res["phase_ms"], "roofline": res["roofline"], "store": res["store"], "memory": res["memory"],
+        "phase_ms": res["phase_ms"], "roofline": res["roofline"], "roofline_alu": res["roofline_alu"], "store": res["store"],
+        "memory": res["memory"],
         "sort_general": sort_general, "e2e": e2e,
     }
 
@@ -486,6 +498,7 @@ def run_psc(args):
             others.append({"config": cfg, "value": float("%.4g" % r["value"]), "ms_per_step": round(r["ms_per_step"], 4),
                            "steps": r["steps"], "kernel": rf["kernel"], "kernel_ms": round(rf["kernel_ms"], 4),
                            "frac": round(rf["frac"], 4), "frac_nominal": round(rf["frac_nominal"], 4),
+                           "frac_alu": round(r["roofline_alu"]["frac"], 4),
                            "traffic_ratio": None if not rf.get("traffic_ratio") else round(rf["traffic_ratio"], 3),
                            "sm_mhz": r["clocks"].get("sm_mhz"), "reasons": r["clocks"].get("reasons"),
                            "flags": r["status_flags"], "mem_x": r["memory"]["column_multiplier"]})
