@@ -496,7 +496,7 @@ def run_psc(args):
             r, s2, p2 = measure(cfg, None, 3, args.other_steps, dev, 1, local)
             rf = r["roofline"]
             others.append({"config": cfg, "value": float("%.4g" % r["value"]), "ms_per_step": round(r["ms_per_step"], 4),
-                           "steps": r["steps"], "kernel": rf["kernel"], "kernel_ms": round(rf["kernel_ms"], 4),
+                           "kernel_ms": round(rf["kernel_ms"], 4),
                            "frac": round(rf["frac"], 4), "frac_nominal": round(rf["frac_nominal"], 4),
                            "frac_alu": round(r["roofline_alu"]["frac"], 4),
                            "traffic_ratio": None if not rf.get("traffic_ratio") else round(rf["traffic_ratio"], 3),
